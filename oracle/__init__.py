@@ -1,0 +1,173 @@
+"""ORACLE — TEST INFRASTRUCTURE ONLY (see oracle/sem_oracle.cpp header).
+
+ctypes/numpy wrapper around the plain CPU C++ oracle of the spectral-element Poisson/Helmholtz hot path of
+arXiv 2110.01716.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this package.  It imports nothing from paper_2110_01716_b200 and shares no code with the CUDA path.
+
+Array conventions: p = N+1, local node l = ((e*p + k)*p + j)*p + i (i fastest), vertex v = a+2b+4c,
+G[E][7][p^3] = (rr, rs, rt, ss, st, tt, B).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "sem_oracle.cpp")
+_SO = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with g++ -O3 -fopenmp (no other tuning).  Returns the .so path."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        cmd = ["g++", "-O3", "-std=c++17", "-fopenmp", "-fPIC", "-shared", "-ffp-contract=off", _SRC, "-o", _SO]
+        subprocess.run(cmd, check=True)
+    return _SO
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.orc_count_unique.restype = C.c_int64
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p) if a is not None else None
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
+
+
+def gll(N: int):
+    """O1: (xi[p], rho[p], D[p,p]) — D[i,l] = dh_l/dr at xi_i."""
+    p = N + 1
+    xi, rho, D = np.empty(p), np.empty(p), np.empty((p, p))
+    rc = lib().orc_gll(C.c_int(N), _p(xi), _p(rho), _p(D))
+    if rc:
+        raise ValueError(f"orc_gll rc={rc}")
+    return xi, rho, D
+
+
+def node_xyz(vert: np.ndarray, N: int) -> np.ndarray:
+    """O2: trilinear images of the GLL points.  vert[E,8,3] -> xyz[E,p^3,3]."""
+    vert = _f64(vert)
+    E = vert.shape[0]
+    out = np.empty((E, (N + 1) ** 3, 3))
+    rc = lib().orc_node_xyz(C.c_int64(E), C.c_int(N), _p(vert), _p(out))
+    assert rc == 0
+    return out
+
+
+def geom_iso(xyz: np.ndarray, N: int):
+    """O3 (isoparametric): xyz[E,p^3,3] -> (G[E,7,p^3], detJ[E,p^3], rc) ; rc=-2 if some detJ <= 0."""
+    xyz = _f64(xyz)
+    E = xyz.shape[0]
+    p3 = (N + 1) ** 3
+    G, dJ = np.empty((E, 7, p3)), np.empty((E, p3))
+    rc = lib().orc_geom_iso(C.c_int64(E), C.c_int(N), _p(xyz), _p(G), _p(dJ))
+    return G, dJ, rc
+
+
+def geom_trilinear(vert: np.ndarray, N: int):
+    """O3 (trilinear-analytic): vert[E,8,3] -> (G[E,7,p^3], detJ[E,p^3], rc)."""
+    vert = _f64(vert)
+    E = vert.shape[0]
+    p3 = (N + 1) ** 3
+    G, dJ = np.empty((E, 7, p3)), np.empty((E, p3))
+    rc = lib().orc_geom_trilinear(C.c_int64(E), C.c_int(N), _p(vert), _p(G), _p(dJ))
+    return G, dJ, rc
+
+
+def ax(G: np.ndarray, u: np.ndarray, N: int, lam: float = 0.0) -> np.ndarray:
+    """O4: local w = D^T G D u (+ lam B u); no gather-scatter."""
+    G, u = _f64(G), _f64(u)
+    E = G.shape[0]
+    w = np.empty_like(u)
+    rc = lib().orc_ax(C.c_int64(E), C.c_int(N), _p(G), _p(u), _p(w), C.c_double(lam))
+    assert rc == 0
+    return w
+
+
+class Maps:
+    """O6 canonical maps."""
+
+    def __init__(self, gid: np.ndarray):
+        gid = np.ascontiguousarray(gid, dtype=np.int64).ravel()
+        nL = gid.size
+        U = int(lib().orc_count_unique(C.c_int64(nL), _p(gid)))
+        self.nL, self.U = nL, U
+        self.uniq_gid = np.empty(U, np.int64)
+        self.l2u = np.empty(nL, np.int32)
+        self.mult = np.empty(U, np.int32)
+        self.seg_off = np.empty(U + 1, np.int64)
+        self.seg_idx = np.empty(nL, np.int32)
+        rc = lib().orc_maps(C.c_int64(nL), _p(gid), C.c_int64(U), _p(self.uniq_gid), _p(self.l2u), _p(self.mult),
+                            _p(self.seg_off), _p(self.seg_idx))
+        if rc:
+            raise ValueError("orc_maps: negative gid or inconsistent U")
+        self.S = int(self.mult[self.mult > 1].sum())
+        self.Us = int((self.mult > 1).sum())
+
+
+def gs(w: np.ndarray, maps: Maps) -> np.ndarray:
+    """O5: QQ^T, op=add.  Returns a new array."""
+    out = _f64(w).copy()
+    rc = lib().orc_gs(C.c_int64(maps.nL), C.c_int64(maps.U), _p(maps.l2u), _p(out))
+    assert rc == 0
+    return out
+
+
+def diag_local(G: np.ndarray, N: int, lam: float = 0.0) -> np.ndarray:
+    """O7: exact diagonal of the local operator, [E,p^3] (assemble with gs())."""
+    G = _f64(G)
+    E = G.shape[0]
+    d = np.empty((E, (N + 1) ** 3))
+    rc = lib().orc_diag_local(C.c_int64(E), C.c_int(N), _p(G), _p(d), C.c_double(lam))
+    assert rc == 0
+    return d
+
+
+def mask_unique(dirichlet_local, maps: Maps) -> np.ndarray:
+    """S14: a unique node is masked if any of its local copies is flagged."""
+    m = np.zeros(maps.U, np.uint8)
+    if dirichlet_local is not None:
+        np.maximum.at(m, maps.l2u, np.ascontiguousarray(dirichlet_local, np.uint8).ravel())
+    return m
+
+
+def apply_Ag(G, N, maps: Maps, mask_u, x_u, lam: float = 0.0) -> np.ndarray:
+    """O8: y = M Q^T A_L Q M x in unique storage."""
+    G, x_u = _f64(G), _f64(x_u)
+    y = np.empty(maps.U)
+    mask_u = np.ascontiguousarray(mask_u, np.uint8)
+    lib().orc_apply_Ag(C.c_int64(G.shape[0]), C.c_int(N), _p(G), C.c_double(lam), C.c_int64(maps.nL),
+                       C.c_int64(maps.U), _p(maps.l2u), _p(mask_u), _p(x_u), _p(y))
+    return y
+
+
+def pcg(G, N, maps: Maps, mask_u, b_u, x0_u=None, tol=1e-8, maxit=100, lam=0.0, snap_its=()):
+    """O8 Jacobi-PCG in unique storage.  Returns dict(x, iters, relres, hist, snaps{it: x})."""
+    G, b_u = _f64(G), _f64(b_u)
+    x = np.zeros(maps.U) if x0_u is None else _f64(x0_u).copy()
+    mask_u = np.ascontiguousarray(mask_u, np.uint8)
+    hist = np.full(maxit + 1, np.nan)
+    relres = C.c_double(0.0)
+    snap_its = np.ascontiguousarray(sorted(int(s) for s in snap_its), dtype=np.int32)
+    ns = snap_its.size
+    xs = np.empty((max(ns, 1), maps.U))
+    it = lib().orc_pcg(C.c_int64(G.shape[0]), C.c_int(N), _p(G), C.c_double(lam), C.c_int64(maps.nL), C.c_int64(maps.U),
+                       _p(maps.l2u), _p(mask_u), _p(b_u), _p(x), C.c_double(tol), C.c_int(maxit), C.byref(relres),
+                       _p(hist), C.c_int(ns), _p(snap_its), _p(xs))
+    return dict(x=x, iters=int(it), relres=float(relres.value), hist=hist[: it + 1],
+                snaps={int(s): xs[n] for n, s in enumerate(snap_its) if s <= it})

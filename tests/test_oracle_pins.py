@@ -1,0 +1,443 @@
+"""Pins for the CPU oracle: everything here is fixed by the paper's definitions and by
+mathematics, and is computed WITHOUT the oracle's own formulas (closed forms, numpy.polynomial, dense Kronecker /
+weak-form brute force, dense Cholesky), so that a dropped term, wrong sign/index or transposed operand fails."""
+import os
+
+import numpy as np
+import numpy.polynomial.legendre as npleg
+import numpy.polynomial.polynomial as nppoly
+import pytest
+
+from paper_2110_01716_b200 import inputs
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def read_golden(name):
+    out = {}
+    for line in open(os.path.join(GOLD, name)):
+        if line.startswith("#") or not line.strip():
+            continue
+        k, v = line.split(None, 1)
+        out[k] = v.strip()
+    return out
+
+
+# ---------- independent 1-D data (numpy.polynomial, Lagrange polynomials differentiated explicitly) -------------
+def ref_gll(N):
+    PN = npleg.Legendre.basis(N)
+    xi = np.concatenate([[-1.0], np.sort(PN.deriv().roots().real), [1.0]])
+    rho = 2.0 / (N * (N + 1) * PN(xi) ** 2)
+    return xi, rho
+
+
+def ref_D(xi):
+    p = xi.size
+    D = np.zeros((p, p))
+    for l in range(p):
+        others = np.delete(xi, l)
+        c = nppoly.polyfromroots(others) / np.prod(xi[l] - others)   # h_l as monomial coefficients
+        D[:, l] = nppoly.polyval(xi, nppoly.polyder(c))              # dh_l/dr at xi_i
+    return D
+
+
+def ref_trilinear(vert_e, r, s, t):
+    """x(r,s,t) for one element; r,s,t arrays of equal shape -> [...,3]."""
+    X = 0.0
+    for v in range(8):
+        a, b, c = v & 1, (v >> 1) & 1, (v >> 2) & 1
+        phi = (1 + (2 * a - 1) * r) * (1 + (2 * b - 1) * s) * (1 + (2 * c - 1) * t) / 8.0
+        X = X + phi[..., None] * vert_e[v]
+    return X
+
+
+def dense_element_matrix(vert_e, N):
+    """Weak-form brute force: A_mn = sum_q rho_q detJ_q grad(phi_m)(x_q) . grad(phi_n)(x_q) with PHYSICAL gradients,
+    phi the 3-D Lagrange basis; the O(N^6) formation of P:75 / P:107.  Also returns the diagonal mass."""
+    xi, rho = ref_gll(N)
+    D1 = ref_D(xi)
+    p = N + 1
+    I = np.eye(p)
+    Dref = [np.kron(I, np.kron(I, D1)), np.kron(I, np.kron(D1, I)), np.kron(D1, np.kron(I, I))]  # d/dr, d/ds, d/dt
+    T, S, R = np.meshgrid(xi, xi, xi, indexing="ij")            # node (k,j,i): t=xi_k, s=xi_j, r=xi_i
+    X = ref_trilinear(vert_e, R.ravel(), S.ravel(), T.ravel())  # [p^3,3]
+    W = (rho[:, None, None] * rho[None, :, None] * rho[None, None, :]).ravel()
+    J = np.stack([np.stack([Dref[b] @ X[:, a] for b in range(3)], axis=-1) for a in range(3)], axis=1)  # [q,a,b]
+    det = np.linalg.det(J)
+    Rinv = np.linalg.inv(J)                                      # [q,b,a] = dr_b/dx_a
+    A = np.zeros((p ** 3, p ** 3))
+    for a in range(3):
+        Ga = sum(Rinv[:, b, a][:, None] * Dref[b] for b in range(3))   # d phi_n / d x_a at q
+        A += Ga.T @ ((W * det)[:, None] * Ga)
+    return A, W * det
+
+
+def assemble_dense(mesh):
+    gids, inv = np.unique(mesh.gid.ravel(), return_inverse=True)
+    inv = inv.reshape(mesh.gid.shape)
+    U = gids.size
+    A = np.zeros((U, U))
+    B = np.zeros(U)
+    for e in range(mesh.E):
+        Ae, Be = dense_element_matrix(mesh.vert[e], mesh.N)
+        A[np.ix_(inv[e], inv[e])] += Ae
+        np.add.at(B, inv[e], Be)
+    return A, B, inv
+
+
+def tiny_mesh(N=3):
+    m = inputs.box_mesh(2, 2, 2, N, "affine")
+    # perturb the single interior vertex (it is vertex 7 of element 0, 6 of element 1, ... ) consistently
+    target = np.array([0.5, 0.5, 0.5])
+    sel = np.all(np.isclose(m.vert, target), axis=-1)
+    m.vert[sel] = target + np.array([0.07, -0.05, 0.04])
+    return m
+
+
+# ---------------------------------------------- P1, P2 -----------------------------------------------------------
+def test_P1_closed_forms(oracle_mod):
+    xi, rho, D = oracle_mod.gll(1)
+    assert np.allclose(xi, [-1, 1], atol=0) and np.allclose(rho, [1, 1], atol=1e-15)
+    assert np.allclose(D, [[-0.5, 0.5], [-0.5, 0.5]], atol=1e-15)
+    xi, rho, D = oracle_mod.gll(2)
+    assert np.allclose(xi, [-1, 0, 1], atol=1e-16) and np.allclose(rho, [1 / 3, 4 / 3, 1 / 3], atol=1e-15)
+    assert np.allclose(D, [[-1.5, 2, -0.5], [-0.5, 0, 0.5], [0.5, -2, 1.5]], atol=1e-14)
+    xi, rho, _ = oracle_mod.gll(3)
+    assert np.allclose(xi, [-1, -1 / np.sqrt(5), 1 / np.sqrt(5), 1], atol=1e-15)
+    assert np.allclose(rho, [1 / 6, 5 / 6, 5 / 6, 1 / 6], atol=1e-15)
+    xi, rho, _ = oracle_mod.gll(4)
+    assert np.allclose(xi, [-1, -np.sqrt(3 / 7), 0, np.sqrt(3 / 7), 1], atol=1e-15)
+    assert np.allclose(rho, [1 / 10, 49 / 90, 32 / 45, 49 / 90, 1 / 10], atol=1e-15)
+    xi, rho, D = oracle_mod.gll(7)   # standard Lobatto tables
+    assert np.allclose(xi[4:], [0.2092992179024789, 0.5917001814331423, 0.8717401485096066, 1.0], atol=1e-15)
+    assert np.allclose(rho[4:], [0.4124587946587038, 0.3411226924835044, 0.2107042271435061, 1 / 28], atol=1e-15)
+    assert D[0, 0] == pytest.approx(-14.0, abs=1e-13) and D[0, 7] == pytest.approx(0.5, abs=1e-13)
+    assert D[7, 7] == pytest.approx(14.0, abs=1e-13)
+
+
+@pytest.mark.parametrize("N", [1, 2, 3, 4, 5, 6, 7, 8, 9, 11, 15])
+def test_P2_exactness_and_independent_tables(oracle_mod, N):
+    xi, rho, D = oracle_mod.gll(N)
+    rxi, rrho = ref_gll(N)
+    assert np.allclose(xi, rxi, atol=2e-14) and np.allclose(rho, rrho, rtol=1e-12)
+    assert np.allclose(D, ref_D(rxi), atol=1e-10 * N * N)
+    assert np.all(np.diff(xi) > 0) and np.allclose(xi, -xi[::-1], atol=0)
+    assert abs(rho.sum() - 2.0) < 1e-14
+    assert np.abs(D.sum(axis=1)).max() < 1e-12 * N * N             # D annihilates constants
+    for m in range(1, N + 1):                                      # D xi^m = m xi^(m-1) exactly for m <= N
+        assert np.allclose(D @ xi ** m, m * xi ** (m - 1), atol=1e-11 * N)
+    for m in range(0, 2 * N):                                      # quadrature exact to degree 2N-1
+        exact = 0.0 if m % 2 else 2.0 / (m + 1)
+        assert abs(rho @ xi ** m - exact) < 1e-14
+    # antisymmetry D[i,l] = -D[N-i,N-l] (centro-skew-symmetric): catches a transposed / flipped operand
+    assert np.allclose(D, -D[::-1, ::-1], atol=1e-12 * N * N)
+
+
+# ---------------------------------------------- P3..P8, P11 ------------------------------------------------------
+@pytest.fixture(scope="module")
+def cfg1(oracle_mod):
+    m = inputs.config1()
+    xyz = oracle_mod.node_xyz(m.vert, m.N)
+    G, dJ, rc = oracle_mod.geom_iso(xyz, m.N)
+    assert rc == 0
+    maps = oracle_mod.Maps(m.gid)
+    return m, xyz, G, dJ, maps
+
+
+def test_O2_nodes_match_independent_trilinear(oracle_mod, cfg1):
+    m, xyz, *_ = cfg1
+    xi, _ = ref_gll(m.N)
+    T, S, R = np.meshgrid(xi, xi, xi, indexing="ij")
+    for e in (0, 21, 63):
+        assert np.allclose(xyz[e], ref_trilinear(m.vert[e], R.ravel(), S.ravel(), T.ravel()), atol=1e-15)
+
+
+def test_P3_constants_annihilated(oracle_mod, cfg1):
+    m, xyz, G, *_ = cfg1
+    w = oracle_mod.ax(G, np.ones((m.E, m.p ** 3)), m.N)
+    scale = np.abs(oracle_mod.ax(G, xyz[..., 0].copy(), m.N)).max()
+    assert np.abs(w).max() < 1e-13 * scale
+
+
+def test_P4_symmetric_positive_semidefinite(oracle_mod, cfg1):
+    m, xyz, G, dJ, maps = cfg1
+    u = inputs.field_uniform(m.gid, 11)
+    v = inputs.field_uniform(m.gid, 12)
+    Au, Av = oracle_mod.ax(G, u, m.N), oracle_mod.ax(G, v, m.N)
+    assert abs((v * Au).sum() - (u * Av).sum()) < 1e-13 * abs((u * Au).sum())
+    assert (u * Au).sum() > 0 and (v * Av).sum() > 0
+    # the same through gs: (QQ^T A u) weighted by 1/mult is the assembled product
+    wts = 1.0 / maps.mult[maps.l2u].reshape(u.shape)
+    gAu, gAv = oracle_mod.gs(Au, maps), oracle_mod.gs(Av, maps)
+    assert abs((wts * v * gAu).sum() - (wts * u * gAv).sum()) < 1e-13 * abs((wts * u * gAu).sum())
+
+
+def test_P5_volume_and_P13_detJ(oracle_mod, cfg1):
+    m, xyz, G, dJ, maps = cfg1
+    assert abs(G[:, 6].sum() - 1.0) < 1e-13                       # sum of B = volume of [0,1]^3
+    gold = read_golden("p13_config1_pcg.txt")
+    assert dJ.min() == pytest.approx(float(gold["detJ_min"]), rel=1e-10)
+    assert dJ.max() == pytest.approx(float(gold["detJ_max"]), rel=1e-10)
+    for cfg in (inputs.config3(3, 2), inputs.config3(2, 5)):
+        Gc, dJc, rc = oracle_mod.geom_trilinear(cfg.vert, cfg.N)
+        assert rc == 0 and abs(Gc[:, 6].sum() - 1.0) < 1e-13
+
+
+def test_P6_linear_field_energy(oracle_mod, cfg1):
+    m, xyz, G, *_ = cfg1
+    for d in range(3):
+        u = xyz[..., d].copy()
+        assert abs((u * oracle_mod.ax(G, u, m.N)).sum() - 1.0) < 1e-12     # |grad x|^2 integrated over the unit box
+    u, v = xyz[..., 0].copy(), xyz[..., 1].copy()
+    assert abs((v * oracle_mod.ax(G, u, m.N)).sum()) < 1e-12               # grad x . grad y = 0
+
+
+@pytest.mark.parametrize("N", [2, 3, 7])
+def test_P7_affine_kronecker(oracle_mod, N):
+    h = np.array([0.5, 0.25, 0.125])                                       # anisotropic box element
+    m = inputs.box_mesh(2, 4, 8, N, "affine")
+    xi, rho = ref_gll(N)
+    D1 = ref_D(xi)
+    M, K = np.diag(rho), D1.T @ np.diag(rho) @ D1
+    # A_L = (hy hz / (2 hx)) M(x)M(x)K + ... with index order (k,j,i): kron(t, kron(s, r))
+    AL = (h[1] * h[2] / (2 * h[0])) * np.kron(M, np.kron(M, K)) + (h[0] * h[2] / (2 * h[1])) * np.kron(M, np.kron(K, M)) \
+        + (h[0] * h[1] / (2 * h[2])) * np.kron(K, np.kron(M, M))
+    G, dJ, rc = oracle_mod.geom_iso(oracle_mod.node_xyz(m.vert, N), N)
+    assert rc == 0
+    W = (rho[:, None, None] * rho[None, :, None] * rho[None, None, :]).ravel()
+    assert np.allclose(G[5, 0], W * h[1] * h[2] / (2 * h[0]), rtol=1e-12)
+    assert np.allclose(G[5, 3], W * h[0] * h[2] / (2 * h[1]), rtol=1e-12)
+    assert np.allclose(G[5, 5], W * h[0] * h[1] / (2 * h[2]), rtol=1e-12)
+    assert np.abs(G[:, [1, 2, 4]]).max() < 1e-15
+    u = inputs.field_uniform(m.gid, 5)
+    w = oracle_mod.ax(G, u, N)
+    assert np.allclose(w[5], AL @ u[5], atol=1e-13 * np.abs(w).max())
+    lam = 0.7                                                              # Helmholtz term (S18)
+    wl = oracle_mod.ax(G, u, N, lam)
+    assert np.allclose(wl[5], AL @ u[5] + lam * W * np.prod(h) / 8 * u[5], atol=1e-13 * np.abs(wl).max())
+
+
+def test_P8_trilinear_equals_isoparametric(oracle_mod):
+    for m in (inputs.config1(), inputs.config3(3, 4), inputs.config3(2, 9), inputs.config3(3, 1)):
+        Gi, dJi, rc1 = oracle_mod.geom_iso(oracle_mod.node_xyz(m.vert, m.N), m.N)
+        Gt, dJt, rc2 = oracle_mod.geom_trilinear(m.vert, m.N)
+        assert rc1 == 0 and rc2 == 0
+        assert np.abs(Gi - Gt).max() < 1e-12 * np.abs(Gi).max()
+        assert np.abs(dJi - dJt).max() < 1e-12 * np.abs(dJi).max()
+
+
+def test_negative_jacobian_flagged(oracle_mod):
+    m = inputs.box_mesh(1, 1, 1, 3, "affine")
+    m.vert[0, [0, 1]] = m.vert[0, [1, 0]]                                  # swap two vertices: inverted element
+    _, _, rc = oracle_mod.geom_trilinear(m.vert, 3)
+    assert rc == -2
+
+
+def test_P11_sin_product_energy(oracle_mod, cfg1):
+    m, xyz, G, *_ = cfg1
+    u = np.sin(np.pi * xyz[..., 0]) * np.sin(np.pi * xyz[..., 1]) * np.sin(np.pi * xyz[..., 2])
+    assert (u * oracle_mod.ax(G, u, m.N)).sum() == pytest.approx(3 * np.pi ** 2 / 8, rel=1e-10)
+
+
+# ---------------------------------------------- O5/O6 maps and gs ------------------------------------------------
+def test_O6_maps_bruteforce(oracle_mod):
+    rng = np.random.default_rng(3)
+    gid = rng.integers(0, 40, size=300).astype(np.int64) * 1000003        # non-contiguous ids, many duplicates
+    mp = oracle_mod.Maps(gid)
+    uniq = sorted(set(gid.tolist()))
+    assert mp.U == len(uniq) and mp.uniq_gid.tolist() == uniq
+    assert mp.l2u.tolist() == [uniq.index(g) for g in gid.tolist()]
+    assert mp.mult.tolist() == [gid.tolist().count(g) for g in uniq]
+    assert mp.seg_off.tolist() == [0] + np.cumsum(mp.mult).tolist()
+    expect_idx = [l for g in uniq for l in range(gid.size) if gid[l] == g]   # (l2u, l) ascending
+    assert mp.seg_idx.tolist() == expect_idx
+    w = rng.standard_normal(300)
+    out = oracle_mod.gs(w, mp)
+    for l in range(300):
+        assert out[l] == pytest.approx(sum(w[q] for q in range(300) if gid[q] == gid[l]), abs=1e-13)
+    with pytest.raises(ValueError):
+        oracle_mod.Maps(np.array([3, -1, 2], np.int64))
+
+
+def test_config1_counts(oracle_mod, cfg1):
+    m, *_, maps = cfg1
+    gold = read_golden("p13_config1_pcg.txt")
+    assert (maps.U, maps.S, maps.Us) == (int(gold["U"]), int(gold["S"]), int(gold["Us"]))
+    assert maps.U == m.unique_nodes == 29 ** 3
+    hist = {int(k): int(v) for k, v in (t.split(":") for t in gold["mult_hist"].split())}
+    bc = np.bincount(maps.mult)
+    assert {k: int(bc[k]) for k in np.nonzero(bc)[0]} == hist
+
+
+# ---------------------------------------------- P9, P10, P14: dense brute force ----------------------------------
+@pytest.fixture(scope="module")
+def tiny(oracle_mod):
+    m = tiny_mesh(3)
+    Adense, Bdense, inv = assemble_dense(m)
+    G, dJ, rc = oracle_mod.geom_iso(oracle_mod.node_xyz(m.vert, m.N), m.N)
+    assert rc == 0 and dJ.min() > 0
+    maps = oracle_mod.Maps(m.gid)
+    assert np.array_equal(maps.l2u.reshape(inv.shape), inv)
+    return m, Adense, Bdense, G, maps
+
+
+def test_P9_dense_assembly_matches_matrix_free(oracle_mod, tiny):
+    m, Adense, Bdense, G, maps = tiny
+    U = maps.U
+    assert U == 343
+    nomask = np.zeros(U, np.uint8)
+    Amf = np.stack([oracle_mod.apply_Ag(G, m.N, maps, nomask, np.eye(U)[g]) for g in range(U)], axis=1)
+    assert np.abs(Amf - Adense).max() < 1e-13 * np.abs(Adense).max()
+    assert np.abs(Adense - Adense.T).max() < 1e-14 * np.abs(Adense).max()
+    ev = np.linalg.eigvalsh(0.5 * (Adense + Adense.T))
+    assert abs(ev[0]) < 1e-12 * ev[-1] and ev[1] > 1e-6 * ev[-1]          # exactly one zero eigenvalue
+    Bo = np.zeros(U)
+    np.add.at(Bo, maps.l2u, G[:, 6].ravel())
+    assert np.allclose(Bo, Bdense, rtol=1e-12)
+    lam = 2.5                                                              # Helmholtz: A + lam B
+    y = oracle_mod.apply_Ag(G, m.N, maps, nomask, np.arange(U) / U, lam)
+    assert np.allclose(y, (Adense + lam * np.diag(Bdense)) @ (np.arange(U) / U), atol=1e-13 * np.abs(y).max())
+
+
+def test_P10_exact_diagonal(oracle_mod, tiny):
+    m, Adense, Bdense, G, maps = tiny
+    dl = oracle_mod.diag_local(G, m.N)
+    dg = np.zeros(maps.U)
+    np.add.at(dg, maps.l2u, dl.ravel())
+    assert np.abs(dg - np.diag(Adense)).max() < 1e-13 * np.diag(Adense).max()
+    dl2 = oracle_mod.diag_local(G, m.N, 1.5)
+    dg2 = np.zeros(maps.U)
+    np.add.at(dg2, maps.l2u, dl2.ravel())
+    assert np.allclose(dg2, np.diag(Adense) + 1.5 * Bdense, rtol=1e-12)
+
+
+def test_P14_pcg_vs_dense_solve_and_krylov_optimality(oracle_mod, tiny):
+    m, Adense, Bdense, G, maps = tiny
+    mask = oracle_mod.mask_unique(m.dirichlet, maps)
+    free = np.nonzero(mask == 0)[0]
+    assert free.size == 125
+    rng = np.random.default_rng(7)
+    b = np.zeros(maps.U)
+    b[free] = rng.standard_normal(free.size)
+    Aff = Adense[np.ix_(free, free)]
+    L = np.linalg.cholesky(Aff)
+    xs = np.zeros(maps.U)
+    xs[free] = np.linalg.solve(L.T, np.linalg.solve(L, b[free]))
+    res = oracle_mod.pcg(G, m.N, maps, mask, b, tol=1e-13, maxit=500)
+    assert res["relres"] <= 1e-13 and res["iters"] <= 125 + 20
+    assert np.abs(res["x"] - xs).max() < 1e-10 * np.abs(xs).max()
+    assert np.all(res["x"][mask == 1] == 0)
+    # x_k minimises the A-norm error over span{M^-1 b, (M^-1 A) M^-1 b, ...}: dense least squares in the A-norm
+    Minv = 1.0 / np.diag(Aff)
+    for k in (1, 2, 3):
+        xk = oracle_mod.pcg(G, m.N, maps, mask, b, tol=1e-30, maxit=k)
+        assert xk["iters"] == k
+        V = [Minv * b[free]]
+        for _ in range(k - 1):
+            V.append(Minv * (Aff @ V[-1]))
+        V = np.stack(V, axis=1)
+        c = np.linalg.solve(V.T @ Aff @ V, V.T @ b[free])
+        assert np.abs(xk["x"][free] - V @ c).max() < 1e-9 * np.abs(V @ c).max()
+    # relres is the recurrence residual relative to ||r0|| and the history is consistent with the returned value
+    r1 = b[free] - Aff @ oracle_mod.pcg(G, m.N, maps, mask, b, tol=1e-30, maxit=5)["x"][free]
+    h5 = oracle_mod.pcg(G, m.N, maps, mask, b, tol=1e-30, maxit=5)
+    assert h5["hist"][5] == pytest.approx(np.linalg.norm(r1) / np.linalg.norm(b[free]), rel=1e-9)
+    # non-zero initial guess converges to the same solution; b = 0 returns x0 (masked) with 0 iterations
+    x0 = np.zeros(maps.U)
+    x0[free] = rng.standard_normal(free.size)
+    res2 = oracle_mod.pcg(G, m.N, maps, mask, b, x0_u=x0, tol=1e-13, maxit=500)
+    assert np.abs(res2["x"] - xs).max() < 1e-9 * np.abs(xs).max()
+    res3 = oracle_mod.pcg(G, m.N, maps, mask, np.zeros(maps.U), tol=1e-8, maxit=10)
+    assert res3["iters"] == 0 and np.all(res3["x"] == 0)
+
+
+def test_P14_element_permutation_invariance(oracle_mod):
+    a = inputs.box_mesh(3, 3, 3, 4, "random", seed=5)
+    b = inputs.box_mesh(3, 3, 3, 4, "random", seed=5, permute_seed=9)
+    assert not np.array_equal(a.perm, b.perm) and sorted(b.perm.tolist()) == list(range(27))
+    out = []
+    for m in (a, b):
+        G, _, rc = oracle_mod.geom_trilinear(m.vert, m.N)
+        maps = oracle_mod.Maps(m.gid)
+        u = inputs.field_uniform(m.gid, 0)
+        w = oracle_mod.gs(oracle_mod.ax(G, u, m.N), maps)
+        wu = np.zeros(maps.U)
+        wu[maps.l2u] = w.ravel()
+        out.append((maps.uniq_gid, wu))
+    assert np.array_equal(out[0][0], out[1][0])
+    assert np.abs(out[0][1] - out[1][1]).max() < 1e-13 * np.abs(out[0][1]).max()
+
+
+# ---------------------------------------------- P12: spectral convergence ----------------------------------------
+def test_P12_spectral_convergence(oracle_mod):
+    gold = {int(k): float(v) for k, v in read_golden("p12_spectral_convergence.txt").items()}
+    errs = {}
+    for N in range(2, 9):
+        m = inputs.box_mesh(2, 2, 2, N, "affine")
+        xyz = oracle_mod.node_xyz(m.vert, N)
+        G, _, _ = oracle_mod.geom_iso(xyz, N)
+        maps = oracle_mod.Maps(m.gid)
+        mask = oracle_mod.mask_unique(m.dirichlet, maps)
+        sp = np.sin(np.pi * xyz[..., 0]) * np.sin(np.pi * xyz[..., 1]) * np.sin(np.pi * xyz[..., 2])
+        b = np.zeros(maps.U)
+        np.add.at(b, maps.l2u, (G[:, 6] * 3 * np.pi ** 2 * sp).ravel())    # Q^T (B f)
+        b[mask == 1] = 0
+        res = oracle_mod.pcg(G, N, maps, mask, b, tol=1e-14, maxit=2000)
+        ue = np.zeros(maps.U)
+        ue[maps.l2u] = sp.ravel()
+        errs[N] = np.abs(res["x"] - ue).max()
+        # Rayleigh quotient of the interpolated eigenfunction approaches 3 pi^2 from below
+        um = np.where(mask == 1, 0.0, ue)
+        rq = um @ oracle_mod.apply_Ag(G, N, maps, mask, um) / (um ** 2 @ np.bincount(maps.l2u, G[:, 6].ravel()))
+        assert rq < 3 * np.pi ** 2 + 1e-9 and abs(rq - 3 * np.pi ** 2) < 0.2 * 30.0 ** (2 - N) + 1e-9
+    for N in range(3, 9):
+        assert errs[N] < errs[N - 1] / 10.0                                # exponential decay in N
+    for N, e in errs.items():
+        assert e == pytest.approx(gold[N], rel=0.06)                       # survey cross-check (2 printed digits)
+
+
+# ---------------------------------------------- P13: config-1 PCG history ----------------------------------------
+def test_P13_config1_pcg_history(oracle_mod, cfg1):
+    m, xyz, G, dJ, maps = cfg1
+    gold = read_golden("p13_config1_pcg.txt")
+    mask = oracle_mod.mask_unique(m.dirichlet, maps)
+    sp = np.sin(np.pi * xyz[..., 0]) * np.sin(np.pi * xyz[..., 1]) * np.sin(np.pi * xyz[..., 2])
+    xu = np.zeros(maps.U)
+    xu[maps.l2u] = sp.ravel()
+    xu[mask == 1] = 0
+    b = oracle_mod.apply_Ag(G, m.N, maps, mask, xu)
+    assert np.linalg.norm(b) == pytest.approx(float(gold["norm_b"]), rel=1e-11)
+    dg = np.bincount(maps.l2u, oracle_mod.diag_local(G, m.N).ravel())
+    assert dg.min() == pytest.approx(float(gold["diag_min"]), rel=1e-11)    # over all unique nodes (corner of the box)
+    assert dg.max() == pytest.approx(float(gold["diag_max"]), rel=1e-11)
+    z = np.where(mask == 1, 0.0, b / dg)
+    alpha1 = (b @ z) / (z @ oracle_mod.apply_Ag(G, m.N, maps, mask, z))
+    assert alpha1 == pytest.approx(float(gold["alpha1"]), rel=1e-9)
+    res = oracle_mod.pcg(G, m.N, maps, mask, b, tol=1e-30, maxit=20, snap_its=(1, 20))
+    assert res["iters"] == 20
+    for it in (1, 5, 10, 15, 20):
+        assert res["hist"][it] == pytest.approx(float(gold[f"relres_it{it}"]), rel=2e-10)
+    assert np.abs(res["snaps"][20] - xu).max() == pytest.approx(float(gold["err_inf_it20"]), rel=1e-9)
+    assert np.allclose(res["snaps"][1], alpha1 * z, rtol=1e-12, atol=1e-16)
+    full = oracle_mod.pcg(G, m.N, maps, mask, b, tol=1e-14, maxit=400)
+    assert abs(full["iters"] - int(gold["iters_to_1e-14"])) <= 2
+    assert np.abs(full["x"] - xu).max() < 1e-11                           # converges to the masked sin-product itself
+
+
+def test_inputs_fields_are_continuous_and_seeded():
+    m = inputs.config1()
+    u = inputs.field_uniform(m.gid, 0)
+    assert u.min() >= -1 and u.max() <= 1 and abs(u.mean()) < 0.02
+    _, first = np.unique(m.gid.ravel(), return_index=True)
+    _, inv = np.unique(m.gid.ravel(), return_inverse=True)
+    assert np.array_equal(u.ravel()[first][inv], u.ravel())              # equal on all copies of a shared node
+    assert np.array_equal(u, inputs.field_uniform(m.gid, 0)) and not np.array_equal(u, inputs.field_uniform(m.gid, 1))
+    g = inputs.field_normal(m.gid, 2)
+    assert abs(g.mean()) < 0.02 and abs(g.std() - 1) < 0.02
+    r = inputs.config3(4, 3)
+    h = 0.25
+    V0 = inputs.vertex_grid(4, 4, 4)
+    V1 = inputs.deform_random(V0, 0.1, 1)
+    assert np.abs(V1 - V0).max() <= 0.1 * h and np.abs(V1 - V0)[1:-1, 1:-1, 1:-1].min() > 0
+    assert np.array_equal(V1[0], V0[0]) and np.array_equal(V1[:, :, -1], V0[:, :, -1])
+    assert r.dirichlet.sum() > 0 and r.gid.max() == r.unique_nodes - 1
