@@ -1,0 +1,299 @@
+#!/usr/bin/env python
+"""bench.py — FP64 N=7 Ax+gs throughput on BASELINE.json config 2 (20x20x18 = 7200 hex elements, ~2.47 M points).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path: w = QQ^T (D^T G D) u over the full mesh (sem_ax_gs through the C ABI).
+metric  = Ax+gs GDOF/s with DOF = E N^3 (the paper's n); value = whole-job DOF/s with inputs resident in HBM.
+e2e     = same metric with u copied from pinned host memory and w copied back inside every timed step.
+roofline= the dominant kernel (the local Ax) timed alone with CUDA events: 64 B x nL algorithmic bytes per launch
+          against the measured HBM copy bandwidth of MEASURED_PEAKS.json.
+N > 1   = independent replicas, one per GPU (the path has no inter-GPU exchange in this build).
+--impl reference times the CPU oracle (oracle/) on the host cores, rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "Ax+gs GDOF/s (FP64, N=7, E=7200)"
+UNIT = "GDOF/s"
+WORKLOAD = "config2: 20x20x18=7200 hex, N=7, smooth deformation 0.05, stored G, u~U[-1,1] seed 0"
+
+
+def measured_peak_gbs():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic_bytes():
+    """Per-launch DRAM bytes of the Ax kernel from the committed ncu capture (profiles/ax_traffic.json), else None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ax_traffic.json")) as f:
+            return float(json.load(f)["dram_bytes_per_launch"])
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_id: str):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", gpu_id, f"--query-gpu={self.FIELDS}",
+                                       "--format=csv,noheader,nounits", "-lms", "20"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f:
+            parts = [s.strip() for s in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1])); pw.append(float(parts[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), power_w_max=float(max(pw)),
+                       reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def cpu_oracle_baseline(mesh, budget_s: float, max_reps: int = 400):
+    """The oracle as it stands, timed on the host cores: full Ax+gs applications of config 2."""
+    import oracle
+    oracle.build()
+    from paper_2110_01716_b200 import inputs
+    G, _, rc = oracle.geom_trilinear(mesh.vert, mesh.N)
+    assert rc == 0
+    om = oracle.Maps(mesh.gid)
+    u = inputs.field_uniform(mesh.gid, 0)
+    oracle.gs(oracle.ax(G, u, mesh.N).ravel(), om)          # warm-up
+    times = []
+    t_start = time.perf_counter()
+    while len(times) < max_reps and (time.perf_counter() - t_start < budget_s or len(times) < 5):
+        t0 = time.perf_counter()
+        oracle.gs(oracle.ax(G, u, mesh.N).ravel(), om)
+        times.append(time.perf_counter() - t0)
+    med = float(np.median(times))
+    return {"value": mesh.dofs / med / 1e9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"{len(times)} full Ax+gs applications of config 2 (all 7200 elements), median", "ms_per_step": med * 1e3}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import oracle
+    oracle.build()
+    from paper_2110_01716_b200 import inputs
+    mesh = inputs.config2()
+    G, _, rc = oracle.geom_trilinear(mesh.vert, mesh.N)
+    u = inputs.field_uniform(mesh.gid, 0)
+    om = oracle.Maps(mesh.gid)
+    t0 = time.perf_counter()
+    oracle.gs(oracle.ax(G, u, mesh.N).ravel(), om)
+    t_full = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    oracle.gs(oracle.ax(G, u, mesh.N).ravel(), om)
+    t_full = min(t_full, time.perf_counter() - t0)
+    total = args.steps + args.warmup
+    budget = 150.0
+    Es = mesh.E
+    if total * t_full > budget:                       # bounded sample: the first Es elements of the same mesh
+        Es = max(16, int(mesh.E * budget / (total * t_full)))
+        G, u = np.ascontiguousarray(G[:Es]), np.ascontiguousarray(u[:Es])
+        om = oracle.Maps(mesh.gid[:Es])
+    for _ in range(args.warmup):
+        oracle.gs(oracle.ax(G, u, mesh.N).ravel(), om)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.gs(oracle.ax(G, u, mesh.N).ravel(), om)
+    dt = time.perf_counter() - t0
+    val = Es * mesh.N ** 3 * args.steps / dt / 1e9
+    sample = f"each step = Ax+gs on the first {Es} of {mesh.E} elements of config 2"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5000)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=50)
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--variant", type=int, default=0)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    args.warmup = max(args.warmup, 3)
+
+    import torch
+    import torch.distributed as dist
+
+    from paper_2110_01716_b200 import binding, build, inputs
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    binding.lib()
+
+    mesh = inputs.config2()
+    sem = binding.Sem(mesh.E, mesh.N, mesh.vert, mesh.gid)
+    sem.geom()
+    sem.set_variant(args.variant)
+    cnt = sem.counts()
+    nL, S = cnt["nL"], cnt["S"]
+    u = torch.from_numpy(inputs.field_uniform(mesh.gid, 0).ravel()).cuda()
+    w = torch.empty_like(u)
+    K, W = args.steps, args.warmup
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def timed(fn, steps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        for _ in range(steps):
+            fn()
+        e1.record()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms
+
+    for _ in range(W):
+        sem.ax_gs(u, w)
+    try:
+        gpu_id = str(torch.cuda.get_device_properties(local).uuid)
+        gpu_id = gpu_id if gpu_id.startswith("GPU-") else "GPU-" + gpu_id
+    except Exception:
+        gpu_id = str(local)
+    sampler = ClockSampler(gpu_id) if rank == 0 else None
+    time.sleep(0.05)
+    # ---- the metric: K applications of the whole path, inputs resident in HBM (working set 236 MB > 126 MB L2) ----
+    ms_total = timed(lambda: sem.ax_gs(u, w), K)
+    # ---- kernel shares: the local operator alone, the gather-scatter alone ----
+    ms_ax = timed(lambda: sem.ax(u, w), K)
+    wz = torch.zeros_like(u)
+    ms_gs = timed(lambda: sem.gs(wz), K)
+    clocks = sampler.stop() if sampler else None
+
+    # ---- e2e: host buffers, H2D of u and D2H of w inside every timed step ----
+    Ke = max(1, min(args.e2e_steps, K))
+    u_h = torch.from_numpy(inputs.field_uniform(mesh.gid, 0).ravel()).pin_memory()
+    w_h = torch.empty_like(u_h).pin_memory()
+
+    def e2e_step():
+        u.copy_(u_h, non_blocking=True)
+        sem.ax_gs(u, w)
+        w_h.copy_(w, non_blocking=True)
+
+    for _ in range(3):
+        e2e_step()
+    ms_e2e = timed(e2e_step, Ke)
+
+    dofs = mesh.dofs
+    value = world * dofs * K / (ms_total * 1e-3) / 1e9
+    e2e_value = world * dofs * Ke / (ms_e2e * 1e-3) / 1e9
+    peak, peak_src = measured_peak_gbs()
+    ax_s = ms_ax * 1e-3 / K
+    ax_bytes = 64.0 * nL                                     # 64 B per local node, FP64, stored G
+    achieved = ax_bytes / ax_s / 1e9
+    whole_bytes = 64.0 * nL + 16.0 * S
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "E": mesh.E, "N": mesh.N, "nL": nL, "U": cnt["U"], "S": S, "dofs_EN3": dofs,
+                   "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas",
+                   "l2": "inputs (u+G+w = 236 MB) larger than the 126 MB L2; no explicit flush",
+                   "ax_variant": args.variant},
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(u_h.numel() * 8),
+                "d2h_bytes_per_step": int(w_h.numel() * 8), "steps": Ke, "ms_per_step": ms_e2e / Ke},
+        "gpu_launches": 2 * K,
+        "roofline": {"bound": "hbm", "kernel": "ax_stream<double,8> (local D^T G D u)", "achieved": achieved,
+                     "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": ncu_traffic_bytes(),
+                     "peak_source": peak_src, "algorithmic_bytes_per_launch": ax_bytes,
+                     "us_per_launch": ax_s * 1e6, "timed": f"{K} back-to-back launches of sem_ax alone, CUDA events",
+                     "frac_of_nominal_8TBs": achieved / 8000.0},
+        "breakdown": {"ax_us": ms_ax / K * 1e3, "gs_us": ms_gs / K * 1e3, "ax_gs_us": ms_total / K * 1e3,
+                      "ax_gs_algorithmic_GBs": whole_bytes / (ms_total * 1e-3 / K) / 1e9,
+                      "ax_gs_frac_of_measured_peak": whole_bytes / (ms_total * 1e-3 / K) / 1e9 / peak,
+                      "ax_gs_frac_of_nominal_8TBs": whole_bytes / (ms_total * 1e-3 / K) / 1e9 / 8000.0,
+                      "ax_TFLOPs_fp64": (12 * mesh.p + 15) * nL / ax_s / 1e12,
+                      "G_local_nodes_per_s": nL * K / (ms_total * 1e-3) / 1e9},
+    }
+    if rank == 0 and world == 1 and args.cpu_seconds > 0:
+        line["cpu_baseline"] = cpu_oracle_baseline(mesh, args.cpu_seconds)
+    sem.close()
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

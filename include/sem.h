@@ -1,0 +1,127 @@
+/* sem.h — C ABI of libsem.so: the matrix-free spectral-element Poisson/Helmholtz hot path of arXiv 2110.01716
+ * (Nek5000/RS) on one NVIDIA B200 (sm_100a).
+ *
+ *      w = M Q Q^T (D^T G D + lambda B) u          and the Jacobi-PCG loop that drives it.
+ *
+ * Citations: "P:nn" = line nn of PAPER.md; "O#/S#" = the readings listed in DESIGN.md.
+ *
+ * Conventions (S4): p = N+1 GLL points per direction; an element's nodes are stored [k][j][i] with i (the r
+ * direction) fastest, so local node l = ((e*p + k)*p + j)*p + i and a field is [E][p][p][p] ("local layout").
+ * Element vertex v = a + 2b + 4c sits at (r,s,t) = (2a-1, 2b-1, 2c-1).  nL = E*p^3 must be < 2^31.
+ *
+ * Memory: every pointer is tagged HOST or DEVICE below.  DEVICE pointers are plain CUDA device pointers (the Python
+ * binding passes torch tensors' data_ptr()); they stay owned by the caller and must stay valid until the stream work
+ * queued by the call has run.  The context owns the geometric factors, the gather-scatter maps and the PCG work
+ * vectors and frees them in sem_ctx_destroy.
+ *
+ * Execution: sem_ax / sem_gs / sem_ax_gs only enqueue kernels on the context's stream and return (asynchronous).
+ * sem_mesh_setup, sem_geom, sem_pcg and the accessors synchronise that stream before returning.
+ *
+ * Errors: every call returns SEM_OK (0) or a negative code; nothing throws or aborts across the ABI.  There is no
+ * CPU fallback: without a CUDA device every compute call returns SEM_ECUDA.
+ */
+#ifndef SEM_H_
+#define SEM_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define SEM_API __attribute__((visibility("default")))
+#else
+#define SEM_API
+#endif
+
+typedef struct sem_ctx sem_ctx; /* opaque, library-owned */
+
+typedef enum { SEM_F64 = 0, SEM_F32 = 1 } sem_prec;
+typedef enum { SEM_OP_ADD = 0 } sem_op; /* only "exchange-and-sum" is defined by the paper */
+typedef enum { SEM_G_STORED = 0, SEM_G_RECOMPUTE = 1 } sem_gmode;
+
+enum {
+    SEM_OK = 0,
+    SEM_EINVAL = -1, /* bad argument (N<1 or N>15, E<=0, NULL pointer, negative gid, nL>=2^31, bad enum) */
+    SEM_EMESH = -2,  /* some Jacobian determinant <= 0 */
+    SEM_ECUDA = -3,  /* CUDA runtime error (text in sem_last_error) or no device */
+    SEM_ENOMEM = -4, /* device or host allocation failed */
+    SEM_ESTATE = -5  /* call order: sem_ax before sem_geom, recompute mode without vertices, ... */
+};
+
+/* a0 + a1 (setup).  Builds the context: GLL points/weights/differentiation matrix D for order N (O1)
+ * and the canonical gather-scatter maps from one global id per local node ("the user simply provides a
+ * global ID for each vertex"; O6):  uniq_gid = distinct gids ascending, l2u[l] = rank of gid[l], mult[g] = copies,
+ * seg_off = exclusive scan of mult, seg_idx = local indices stably sorted by gid.
+ *   out         HOST   receives the context (NULL on failure, except that a context carrying the error text is
+ *                      still returned when the failure happened after allocation; always sem_ctx_destroy it)
+ *   vertex_xyz  HOST   [E][8][3] doubles, element vertices (S4/S5: elements are trilinear images of 8 vertices)
+ *   gid         HOST or DEVICE (detected) [E][p][p][p] int64, all >= 0 (S11)
+ *   dirichlet   HOST, nullable, [E][p^3] bytes, 1 = masked (Dirichlet) node; a unique node is masked if any of its
+ *               copies is flagged (S14)
+ *   cuda_stream a cudaStream_t (0 = legacy default stream) on which all later work of this context is enqueued */
+SEM_API int sem_mesh_setup(sem_ctx** out, int64_t E, int N, const double* vertex_xyz, const int64_t* gid,
+                   const uint8_t* dirichlet, void* cuda_stream);
+
+/* a2 (setup).  Geometric factors (P:69 isoparametric map; O3): at every node the Jacobian Jm = dx/dr, detJ, and
+ *   G_bc = rho_i rho_j rho_k detJ sum_a (dr_b/dx_a)(dr_c/dx_a), stored (rr,rs,rt,ss,st,tt);  B = rho_i rho_j rho_k detJ.
+ *   node_xyz  HOST, nullable, [E][p^3][3]: if given, Jm = D applied to these coordinates (isoparametric); if NULL,
+ *             Jm is the analytic derivative of the trilinear blend of the 8 vertices (S5).
+ *   mode      SEM_G_STORED: G kept in HBM (48 B/node FP64).  SEM_G_RECOMPUTE: sem_ax recomputes G from the 8
+ *             vertices inside the kernel (a9; needs node_xyz == NULL); G is still built once for sem_get_geom/diag.
+ *   with_mass keep B (needed for lambda != 0 and for sem_get_geom's 7th factor)
+ * Returns SEM_EMESH if any detJ <= 0.  Also builds the exact assembled diagonal for Jacobi (O7). */
+SEM_API int sem_geom(sem_ctx* ctx, const double* node_xyz, sem_gmode mode, int with_mass);
+
+/* a3-a5.  Local operator, no gather-scatter (P:93 contraction; O4):  w = D^T G D u + lambda B u  element by element.
+ *   u, w   DEVICE, local layout, nL values of `prec` (double or float); must not alias
+ *   lambda Helmholtz shift (S18); lambda != 0 requires with_mass
+ * FP32 (S16): u, w, G, D and all accumulation in float (G, D rounded once from double). */
+SEM_API int sem_ax(sem_ctx* ctx, const void* u, void* w, sem_prec prec, double lambda);
+
+/* a6.  Gather-scatter QQ^T in place ("exchange-and-sum of shared interface values"; O5): every copy of a
+ * unique node receives the sum over all its copies.  No mask is applied.  w DEVICE, local layout. */
+SEM_API int sem_gs(sem_ctx* ctx, void* w, sem_prec prec, sem_op op);
+
+/* a3-a7.  w = M QQ^T (D^T G D + lambda B) u, with M zeroing Dirichlet nodes (if the context has any).  u must be
+ * continuous (equal on all copies of a shared node). */
+SEM_API int sem_ax_gs(sem_ctx* ctx, const void* u, void* w, sem_prec prec, double lambda);
+
+/* a8.  Jacobi-preconditioned conjugate gradients on M QQ^T A_L M (O8, S12-S14), FP64, lambda = 0 unless
+ * set with sem_set_lambda:
+ *   x = M x0; r = M b - A x (b if x0 == 0); z = Minv r; p = z; rho = r.z; r0 = ||r||
+ *   repeat: q = A p; alpha = rho / p.q; x += alpha p; r -= alpha q; stop if ||r|| <= tol r0 or it == maxit;
+ *           z = Minv r; beta = r.z / rho; p = z + beta p
+ * with dots over unique unmasked nodes.  b (assembled right-hand side) and x are DEVICE, local layout, continuous.
+ *   iters_out   HOST  number of operator applications in the loop
+ *   relres_out  HOST  ||r|| / r0 from the recurrence
+ * Reaching maxit is not an error; b == 0 returns x = M x0, 0 iterations; p.q <= 0 stops (breakdown) with SEM_OK. */
+SEM_API int sem_pcg(sem_ctx* ctx, const double* b, double* x, double tol, int maxit, int* iters_out, double* relres_out);
+
+/* Helmholtz shift used by sem_pcg and by the Jacobi diagonal (default 0).  Requires with_mass if != 0. */
+SEM_API int sem_set_lambda(sem_ctx* ctx, double lambda);
+
+/* Residual history of the last sem_pcg: hist[i] = ||r_i|| / r0 for i = 0..min(iters, n-1).  hist HOST. */
+SEM_API int sem_get_pcg_history(sem_ctx* ctx, double* hist, int n);
+
+/* Parity accessors: copy library-owned data to caller-provided HOST buffers (any may be NULL = skip). */
+SEM_API int sem_get_counts(sem_ctx* ctx, int64_t* nL, int64_t* U, int64_t* S, int64_t* Us);
+SEM_API int sem_get_maps(sem_ctx* ctx, int32_t* l2u /*[nL]*/, int32_t* mult /*[U]*/, int64_t* seg_off /*[U+1]*/,
+                 int32_t* seg_idx /*[nL]*/, int64_t* uniq_gid /*[U]*/);
+SEM_API int sem_get_gll(sem_ctx* ctx, double* xi /*[p]*/, double* rho /*[p]*/, double* D /*[p][p] row = point*/);
+SEM_API int sem_get_geom(sem_ctx* ctx, double* G /*[E][6 or 7][p^3]*/, double* detJ /*[E][p^3]*/);
+SEM_API int sem_get_diag(sem_ctx* ctx, double* diagA_local /* assembled QQ^T diag(A_L), unmasked, [E][p^3] */);
+
+/* Tuning knob for experiments: selects the Ax kernel variant (0 = default streaming kernel, 1 = simple kernel). */
+SEM_API int sem_set_variant(sem_ctx* ctx, int ax_variant);
+
+/* Last error text of this context ("" if none); valid until the next call on the context.  NULL ctx -> static text. */
+SEM_API const char* sem_last_error(sem_ctx* ctx);
+
+SEM_API void sem_ctx_destroy(sem_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SEM_H_ */

@@ -1,0 +1,210 @@
+"""Thin ctypes binding over the C-ABI library libsem.so (include/sem.h).  Argument marshalling only: every step of the
+hot path runs in the CUDA kernels of the library.  torch is used for device memory and the stream handle.
+
+There is no CPU fallback: if libsem.so is missing the import of this module's `lib()` raises, and every compute call
+needs a CUDA device.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsem.so")
+
+SEM_F64, SEM_F32 = 0, 1
+SEM_OP_ADD = 0
+SEM_G_STORED, SEM_G_RECOMPUTE = 0, 1
+SEM_OK, SEM_EINVAL, SEM_EMESH, SEM_ECUDA, SEM_ENOMEM, SEM_ESTATE = 0, -1, -2, -3, -4, -5
+_ERRNAME = {-1: "SEM_EINVAL", -2: "SEM_EMESH", -3: "SEM_ECUDA", -4: "SEM_ENOMEM", -5: "SEM_ESTATE"}
+
+# every symbol include/sem.h declares: name -> (restype, argtypes)
+_vp, _i64, _i32, _dbl = C.c_void_p, C.c_int64, C.c_int, C.c_double
+SYMBOLS = {
+    "sem_mesh_setup": (_i32, [C.POINTER(_vp), _i64, _i32, _vp, _vp, _vp, _vp]),
+    "sem_geom": (_i32, [_vp, _vp, _i32, _i32]),
+    "sem_ax": (_i32, [_vp, _vp, _vp, _i32, _dbl]),
+    "sem_gs": (_i32, [_vp, _vp, _i32, _i32]),
+    "sem_ax_gs": (_i32, [_vp, _vp, _vp, _i32, _dbl]),
+    "sem_pcg": (_i32, [_vp, _vp, _vp, _dbl, _i32, C.POINTER(_i32), C.POINTER(_dbl)]),
+    "sem_set_lambda": (_i32, [_vp, _dbl]),
+    "sem_get_pcg_history": (_i32, [_vp, _vp, _i32]),
+    "sem_get_counts": (_i32, [_vp, C.POINTER(_i64), C.POINTER(_i64), C.POINTER(_i64), C.POINTER(_i64)]),
+    "sem_get_maps": (_i32, [_vp, _vp, _vp, _vp, _vp, _vp]),
+    "sem_get_gll": (_i32, [_vp, _vp, _vp, _vp]),
+    "sem_get_geom": (_i32, [_vp, _vp, _vp]),
+    "sem_get_diag": (_i32, [_vp, _vp]),
+    "sem_set_variant": (_i32, [_vp, _i32]),
+    "sem_last_error": (C.c_char_p, [_vp]),
+    "sem_ctx_destroy": (None, [_vp]),
+}
+
+_lib = None
+
+
+class SemError(RuntimeError):
+    def __init__(self, code: int, text: str):
+        super().__init__(f"{_ERRNAME.get(code, code)}: {text}")
+        self.code = code
+
+
+def lib() -> C.CDLL:
+    """Load libsem.so (fails loudly if it has not been built: python -m paper_2110_01716_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(f"{LIB_PATH} not built; run `python -m paper_2110_01716_b200.build` "
+                                    "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        for name, (res, args) in SYMBOLS.items():
+            f = getattr(L, name)
+            f.restype, f.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _np_ptr(a):
+    return a.ctypes.data_as(C.c_void_p) if a is not None else None
+
+
+class Sem:
+    """One mesh/discretisation context (sem_mesh_setup ... sem_ctx_destroy).  Method names follow the C ABI."""
+
+    def __init__(self, E: int, N: int, vertex_xyz: np.ndarray, gid, dirichlet: np.ndarray | None = None, stream=None):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise SemError(SEM_ECUDA, "no CUDA device (libsem has no CPU fallback)")
+        self._L = lib()
+        self.E, self.N, self.p = int(E), int(N), int(N) + 1
+        self.nL = self.E * self.p ** 3
+        vert = np.ascontiguousarray(vertex_xyz, dtype=np.float64).reshape(E, 8, 3)
+        if isinstance(gid, torch.Tensor):
+            assert gid.dtype == torch.int64 and gid.is_contiguous() and gid.numel() == self.nL
+            self._gid_keep = gid
+            gid_ptr = C.c_void_p(gid.data_ptr())
+        else:
+            g = np.ascontiguousarray(gid, dtype=np.int64).reshape(-1)
+            assert g.size == self.nL
+            self._gid_keep = g
+            gid_ptr = _np_ptr(g)
+        d = None
+        if dirichlet is not None:
+            d = np.ascontiguousarray(dirichlet, dtype=np.uint8).reshape(-1)
+            assert d.size == self.nL
+        self._stream = stream if stream is not None else torch.cuda.current_stream()
+        self._h = C.c_void_p()
+        rc = self._L.sem_mesh_setup(C.byref(self._h), E, N, _np_ptr(vert), gid_ptr, _np_ptr(d),
+                                    C.c_void_p(self._stream.cuda_stream))
+        self._check(rc)
+
+    # ---- plumbing ----
+    def _check(self, rc: int):
+        if rc != SEM_OK:
+            text = self._L.sem_last_error(self._h) if self._h else b""
+            raise SemError(rc, (text or b"").decode())
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.sem_ctx_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    @staticmethod
+    def _prec(t) -> int:
+        import torch
+
+        if t.dtype == torch.float64:
+            return SEM_F64
+        if t.dtype == torch.float32:
+            return SEM_F32
+        raise TypeError(f"unsupported dtype {t.dtype}")
+
+    def _vec(self, t):
+        assert t.is_cuda and t.is_contiguous() and t.numel() == self.nL, "need a contiguous CUDA tensor of nL values"
+        return C.c_void_p(t.data_ptr())
+
+    # ---- the C ABI ----
+    def geom(self, node_xyz: np.ndarray | None = None, mode: int = SEM_G_STORED, with_mass: bool = False):
+        x = None if node_xyz is None else np.ascontiguousarray(node_xyz, dtype=np.float64)
+        self._check(self._L.sem_geom(self._h, _np_ptr(x), mode, int(with_mass)))
+        self.with_mass = bool(with_mass)
+        return self
+
+    def ax(self, u, w, lam: float = 0.0):
+        self._check(self._L.sem_ax(self._h, self._vec(u), self._vec(w), self._prec(u), lam))
+        return w
+
+    def gs(self, w):
+        self._check(self._L.sem_gs(self._h, self._vec(w), self._prec(w), SEM_OP_ADD))
+        return w
+
+    def ax_gs(self, u, w, lam: float = 0.0):
+        assert u.dtype == w.dtype
+        self._check(self._L.sem_ax_gs(self._h, self._vec(u), self._vec(w), self._prec(u), lam))
+        return w
+
+    def pcg(self, b, x, tol: float, maxit: int):
+        """Returns (iters, relres); x is updated in place."""
+        import torch
+
+        assert b.dtype == torch.float64 and x.dtype == torch.float64
+        it, rel = C.c_int(0), C.c_double(0.0)
+        self._check(self._L.sem_pcg(self._h, self._vec(b), self._vec(x), tol, maxit, C.byref(it), C.byref(rel)))
+        return it.value, rel.value
+
+    def set_lambda(self, lam: float):
+        self._check(self._L.sem_set_lambda(self._h, lam))
+
+    def set_variant(self, v: int):
+        self._check(self._L.sem_set_variant(self._h, v))
+
+    def pcg_history(self, n: int) -> np.ndarray:
+        h = np.full(n, np.nan)
+        self._check(self._L.sem_get_pcg_history(self._h, _np_ptr(h), n))
+        return h
+
+    def counts(self):
+        v = [C.c_int64(0) for _ in range(4)]
+        self._check(self._L.sem_get_counts(self._h, *[C.byref(x) for x in v]))
+        return dict(nL=v[0].value, U=v[1].value, S=v[2].value, Us=v[3].value)
+
+    def maps(self):
+        c = self.counts()
+        out = dict(l2u=np.empty(c["nL"], np.int32), mult=np.empty(c["U"], np.int32),
+                   seg_off=np.empty(c["U"] + 1, np.int64), seg_idx=np.empty(c["nL"], np.int32),
+                   uniq_gid=np.empty(c["U"], np.int64))
+        self._check(self._L.sem_get_maps(self._h, _np_ptr(out["l2u"]), _np_ptr(out["mult"]), _np_ptr(out["seg_off"]),
+                                         _np_ptr(out["seg_idx"]), _np_ptr(out["uniq_gid"])))
+        return out
+
+    def gll(self):
+        p = self.p
+        xi, rho, D = np.empty(p), np.empty(p), np.empty((p, p))
+        self._check(self._L.sem_get_gll(self._h, _np_ptr(xi), _np_ptr(rho), _np_ptr(D)))
+        return xi, rho, D
+
+    def get_geom(self):
+        nc = 7 if getattr(self, "with_mass", False) else 6
+        G = np.empty((self.E, nc, self.p ** 3))
+        dJ = np.empty((self.E, self.p ** 3))
+        self._check(self._L.sem_get_geom(self._h, _np_ptr(G), _np_ptr(dJ)))
+        return G, dJ
+
+    def get_diag(self) -> np.ndarray:
+        d = np.empty((self.E, self.p ** 3))
+        self._check(self._L.sem_get_diag(self._h, _np_ptr(d)))
+        return d

@@ -1,0 +1,482 @@
+// sem_ax.cu — a3-a5 (+a9): the local spectral-element operator  w = D^T G D u (+ lambda B u), element by element.
+// P:93 (footnote): u_r,ijk = sum_l D_il u_ljk, "an Np x Np matrix times an Np x Np^2 matrix"; O4 for the
+// full operator; S16 for FP32.  12p+15 flops and 64 B (FP64) / 32 B (FP32) of compulsory HBM traffic per node: the
+// kernel is HBM-bound, so the design is about keeping enough bytes in flight and keeping shared-memory and FP64-issue
+// pressure below the HBM rate:
+//   * thread (i,j) owns the k-column of one element: u[.][j][i] and the w accumulators live in registers, so the t
+//     direction never touches shared memory and D[k][l] for it is a compile-time constant-bank operand;
+//   * the rows D[i][.], D[j][.], D[.][i], D[.][j] the thread needs for r and s stay in registers for the whole kernel;
+//   * G is stored slab-major (sem_geom.cu) and streamed through a ring of shared-memory stages by bulk async copies
+//     (cp.async.bulk + mbarrier transaction counts, evict-first in L2) issued NS slabs ahead, so the bytes in flight per
+//     SM do not depend on registers or occupancy;  u arrives the same way, double-buffered per element;
+//   * persistent CTAs (one element group at a time, grid = SMs x resident CTAs) write w straight from registers.
+// ax_simple is the plain-load version of the same arithmetic: odd p, unaligned pointers, and the recomputed-G
+// variant (a9: G from the 8 trilinear vertices inside the kernel) use it.
+#include <type_traits>
+
+#include "sem_geom_dev.cuh"
+#include "sem_internal.h"
+
+namespace {
+
+// ---------------------------------------------------------------------------------------------------------------
+// PTX helpers (sm_90+/sm_100a): mbarrier + bulk async copy global -> shared
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ uint64_t policy_evict_first() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ uint64_t policy_evict_last() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar,
+                                         uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::
+            "r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
+        : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// shared pieces
+// ---------------------------------------------------------------------------------------------------------------
+template <typename T, int P>
+struct DParam {            // by-value kernel parameter: constant bank
+    T D[P * P];            // D[i*P + l] = dh_l/dr(xi_i)
+};
+
+template <int P> constexpr int epb_of() { return P * P >= 64 ? 1 : (64 + P * P - 1) / (P * P); }
+template <int P> constexpr int threads_of() { return ((epb_of<P>() * P * P + 31) / 32) * 32; }
+
+// read P consecutive values starting at a pointer whose byte offset is a multiple of P*sizeof(T)
+template <typename T, int P>
+__device__ __forceinline__ void load_row(const T* __restrict__ ptr, T (&out)[P]) {
+    if constexpr ((P * sizeof(T)) % 16 == 0) {
+        constexpr int V = 16 / sizeof(T);
+        using VT = typename std::conditional<sizeof(T) == 8, double2, float4>::type;
+#pragma unroll
+        for (int v = 0; v < P / V; ++v) {
+            const VT q = reinterpret_cast<const VT*>(ptr)[v];
+            if constexpr (sizeof(T) == 8) { out[2 * v] = q.x; out[2 * v + 1] = q.y; }
+            else { out[4 * v] = q.x; out[4 * v + 1] = q.y; out[4 * v + 2] = q.z; out[4 * v + 3] = q.w; }
+        }
+    } else if constexpr (sizeof(T) == 4 && (P * sizeof(T)) % 8 == 0) {
+#pragma unroll
+        for (int v = 0; v < P / 2; ++v) {
+            const float2 q = reinterpret_cast<const float2*>(ptr)[v];
+            out[2 * v] = q.x; out[2 * v + 1] = q.y;
+        }
+    } else {
+#pragma unroll
+        for (int l = 0; l < P; ++l) out[l] = ptr[l];
+    }
+}
+
+// The four 1-D rows/columns of D a thread (i,j) keeps in registers.
+template <typename T, int P>
+struct DRows {
+    T Di[P], Dj[P], DTi[P], DTj[P];
+    __device__ __forceinline__ void init(const DParam<T, P>& dp, int i, int j) {
+#pragma unroll
+        for (int l = 0; l < P; ++l) {
+            Di[l] = dp.D[i * P + l];
+            Dj[l] = dp.D[j * P + l];
+            DTi[l] = dp.D[l * P + i];
+            DTj[l] = dp.D[l * P + j];
+        }
+    }
+};
+
+// One k-slab of the operator for thread (i,j) of one element.
+//   su: the element's u in shared memory [P][P][P];  uk/wk: the thread's k-column of u / accumulators of w.
+//   g[6]: this node's factors.  sgr/sgs: this element's exchange buffers for slab parity `buf` ([P*P] each).
+// The caller synchronises the element's threads between part1 and part2.
+template <typename T, int P>
+__device__ __forceinline__ void slab_part1(const DParam<T, P>& dp, const DRows<T, P>& dr, const T* __restrict__ su,
+                                           const T (&uk)[P], T (&wk)[P], const T (&g)[6], int k, int i, int j,
+                                           T* __restrict__ sgr, T* __restrict__ sgs) {
+    T row[P];
+    load_row<T, P>(su + (k * P + j) * P, row);
+    const T* col = su + k * P * P + i;
+    T ur = T(0), us = T(0), ut = T(0);
+#pragma unroll
+    for (int l = 0; l < P; ++l) {
+        ur += dr.Di[l] * row[l];                 // u_r = sum_l D[i][l] u[k][j][l]
+        us += dr.Dj[l] * col[l * P];             // u_s = sum_l D[j][l] u[k][l][i]
+        ut += dp.D[k * P + l] * uk[l];           // u_t = sum_l D[k][l] u[l][j][i]
+    }
+    const T gr = g[0] * ur + g[1] * us + g[2] * ut;
+    const T gs = g[1] * ur + g[3] * us + g[4] * ut;
+    const T gt = g[2] * ur + g[4] * us + g[5] * ut;
+    sgr[j * P + i] = gr;
+    sgs[j * P + i] = gs;
+#pragma unroll
+    for (int l = 0; l < P; ++l) wk[l] += dp.D[k * P + l] * gt;   // w[l][j][i] += D[k][l] g_t[k][j][i]
+}
+
+template <typename T, int P>
+__device__ __forceinline__ T slab_part2(const DRows<T, P>& dr, int i, int j, const T* __restrict__ sgr,
+                                        const T* __restrict__ sgs) {
+    T row[P];
+    load_row<T, P>(sgr + j * P, row);
+    T acc = T(0);
+#pragma unroll
+    for (int l = 0; l < P; ++l) {
+        acc += dr.DTi[l] * row[l];               // sum_l D[l][i] g_r[k][j][l]
+        acc += dr.DTj[l] * sgs[l * P + i];       // sum_l D[l][j] g_s[k][l][i]
+    }
+    return acc;
+}
+
+template <typename T>
+__device__ __forceinline__ void block_dot_flush(T partial, double* __restrict__ dot_out) {
+    __shared__ double red[32];
+    double v = (double)partial;
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
+    if (lane == 0) red[warp] = v;
+    __syncthreads();
+    if (warp == 0) {
+        v = lane < nw ? red[lane] : 0.0;
+        for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) atomicAdd(dot_out, v);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// ax_simple: plain loads.  RECOMP: G from the trilinear vertices (a9).
+// ---------------------------------------------------------------------------------------------------------------
+template <typename T, int P, bool RECOMP>
+__global__ void __launch_bounds__(threads_of<P>()) ax_simple(int64_t E, DParam<T, P> dp, Gll1D gll, int64_t slab,
+                                                             const T* __restrict__ Gs, const double* __restrict__ vert,
+                                                             const T* __restrict__ Bm, T lambda,
+                                                             const T* __restrict__ u, T* __restrict__ w,
+                                                             const int* __restrict__ skip_flag,
+                                                             double* __restrict__ dot_out) {
+    constexpr int EPB = epb_of<P>(), P2 = P * P, P3 = P2 * P;
+    __shared__ __align__(16) T su[EPB * P3];
+    __shared__ __align__(16) T sgr[2][EPB * P2];
+    __shared__ __align__(16) T sgs[2][EPB * P2];
+    if (skip_flag && *skip_flag) return;
+    const int tid = threadIdx.x;
+    const bool lane_ok = tid < EPB * P2;
+    const int slot = lane_ok ? tid / P2 : 0;
+    const int ij = lane_ok ? tid % P2 : 0;
+    const int j = ij / P, i = ij % P;
+    DRows<T, P> dr;
+    dr.init(dp, i, j);
+    T partial = T(0);
+    const int64_t ngroups = (E + EPB - 1) / EPB;
+    for (int64_t grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+        const int64_t e = grp * EPB + slot;
+        const bool active = lane_ok && e < E;
+        T uk[P], wk[P];
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+            uk[k] = active ? u[e * P3 + k * P2 + ij] : T(0);
+            wk[k] = T(0);
+            if (lane_ok) su[slot * P3 + k * P2 + ij] = uk[k];
+        }
+        // recomputed G: per-thread pieces of the trilinear Jacobian that do not depend on k (r = xi_i, s = xi_j)
+        T Ja[3], Jb[3], Jc[3], Jd[3], Je[3];
+        if constexpr (RECOMP) {
+            double X[8][3], cf[8][3];
+#pragma unroll
+            for (int v = 0; v < 8; ++v)
+#pragma unroll
+                for (int d = 0; d < 3; ++d) X[v][d] = active ? vert[(e * 8 + v) * 3 + d] : (double)((v >> d) & 1);
+            sem_trilinear_coef(X, cf);       // vertex differences in FP64 even on the FP32 path (no cancellation)
+            const T r = (T)gll.xi[i], s = (T)gll.xi[j];
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                Ja[d] = (T)cf[1][d] + (T)cf[4][d] * s;          // dx/dr = Ja + Jb t
+                Jb[d] = (T)cf[5][d] + (T)cf[7][d] * s;
+                Jc[d] = (T)cf[2][d] + (T)cf[4][d] * r;          // dx/ds = Jc + Jd t
+                Jd[d] = (T)cf[6][d] + (T)cf[7][d] * r;
+                Je[d] = (T)cf[3][d] + (T)cf[5][d] * r + ((T)cf[6][d] + (T)cf[7][d] * r) * s;   // dx/dt
+            }
+        }
+        __syncthreads();
+        const T* sue = su + slot * P3;
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+            T g[6];
+            if constexpr (RECOMP) {
+                const T t = (T)gll.xi[k];
+                T J[3][3], B;
+#pragma unroll
+                for (int d = 0; d < 3; ++d) { J[d][0] = Ja[d] + Jb[d] * t; J[d][1] = Jc[d] + Jd[d] * t; J[d][2] = Je[d]; }
+                sem_factors<T>(J, (T)(gll.rho[i] * gll.rho[j] * gll.rho[k]), g, B);
+            } else {
+#pragma unroll
+                for (int c = 0; c < 6; ++c) g[c] = active ? Gs[(e * P + k) * slab + c * P2 + ij] : T(0);
+            }
+            const int buf = k & 1;
+            if (lane_ok) slab_part1<T, P>(dp, dr, sue, uk, wk, g, k, i, j, sgr[buf] + slot * P2, sgs[buf] + slot * P2);
+            __syncthreads();
+            if (lane_ok) wk[k] += slab_part2<T, P>(dr, i, j, sgr[buf] + slot * P2, sgs[buf] + slot * P2);
+        }
+        if (active) {
+#pragma unroll
+            for (int k = 0; k < P; ++k) {
+                T v = wk[k];
+                if (Bm) v += lambda * Bm[e * P3 + k * P2 + ij] * uk[k];
+                w[e * P3 + k * P2 + ij] = v;
+                partial += uk[k] * v;
+            }
+        }
+        __syncthreads();     // su is rewritten by the next group
+    }
+    if (dot_out) block_dot_flush(partial, dot_out);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// ax_stream: persistent CTAs, G slabs and u elements arrive by bulk async copies into shared-memory rings.
+// Requires even P (so every chunk is a multiple of 16 bytes) and 16-byte aligned u.
+// ---------------------------------------------------------------------------------------------------------------
+template <typename T, int P, int NS>
+struct StreamSmem {
+    static constexpr int EPB = epb_of<P>(), P2 = P * P, P3 = P2 * P;
+    static constexpr int SLAB = 6 * P2;                      // values per element slab
+    alignas(128) T g[NS][EPB * SLAB];
+    alignas(128) T u[2][EPB * P3];
+    alignas(16) T sgr[2][EPB * P2];
+    alignas(16) T sgs[2][EPB * P2];
+    alignas(8) uint64_t gfull[NS];
+    alignas(8) uint64_t ufull[2];
+};
+
+template <typename T, int P, int NS, int MINB>
+__global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DParam<T, P> dp,
+                                                                   const T* __restrict__ Gs, const T* __restrict__ Bm,
+                                                                   T lambda, const T* __restrict__ u,
+                                                                   T* __restrict__ w, const int* __restrict__ skip_flag,
+                                                                   double* __restrict__ dot_out) {
+    using SM = StreamSmem<T, P, NS>;
+    constexpr int EPB = SM::EPB, P2 = SM::P2, P3 = SM::P3, SLAB = SM::SLAB;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    SM& sm = *reinterpret_cast<SM*>(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
+    if (skip_flag && *skip_flag) return;
+    const int tid = threadIdx.x;
+    const bool lane_ok = tid < EPB * P2;
+    const int slot = lane_ok ? tid / P2 : 0;
+    const int ij = lane_ok ? tid % P2 : 0;
+    const int j = ij / P, i = ij % P;
+
+    const int64_t ngroups = (E + EPB - 1) / EPB;
+    // groups of this CTA: blockIdx.x, blockIdx.x + gridDim.x, ...
+    const int64_t nmine = blockIdx.x < ngroups ? (ngroups - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    uint64_t pol_g = 0, pol_u = 0;
+
+    auto nact_of = [&](int64_t n) -> int {          // active elements in my n-th group
+        const int64_t e0 = (blockIdx.x + n * gridDim.x) * EPB;
+        const int64_t left = E - e0;
+        return left >= EPB ? EPB : (int)left;
+    };
+    // producer state (thread 0 only): the next slab to issue is slab pk of my pn-th group; slabs are issued in order
+    int64_t pn = 0;
+    int pk = 0;
+    auto issue_next_slab = [&](int q) {
+        const int64_t e0 = (blockIdx.x + pn * gridDim.x) * EPB;
+        const int na = nact_of(pn);
+        mbar_expect_tx(&sm.gfull[q], (uint32_t)(na * SLAB * sizeof(T)));
+#pragma unroll 1
+        for (int s = 0; s < na; ++s)
+            bulk_g2s(&sm.g[q][s * SLAB], Gs + ((e0 + s) * P + pk) * SLAB, SLAB * sizeof(T), &sm.gfull[q], pol_g);
+        if (++pk == P) { pk = 0; ++pn; }
+    };
+    auto issue_u = [&](int64_t n) {                 // thread 0 only
+        const int b = (int)(n & 1);
+        const int64_t e0 = (blockIdx.x + n * gridDim.x) * EPB;
+        const uint32_t bytes = (uint32_t)(nact_of(n) * P3 * sizeof(T));
+        mbar_expect_tx(&sm.ufull[b], bytes);
+        bulk_g2s(&sm.u[b][0], u + e0 * P3, bytes, &sm.ufull[b], pol_u);
+    };
+
+    if (tid == 0) {
+#pragma unroll
+        for (int q = 0; q < NS; ++q) mbar_init(&sm.gfull[q], 1);
+        mbar_init(&sm.ufull[0], 1);
+        mbar_init(&sm.ufull[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (tid == 0 && nmine > 0) {
+        pol_g = policy_evict_first();
+        pol_u = policy_evict_last();
+        issue_u(0);
+        for (int q = 0; q < NS && pn < nmine; ++q) issue_next_slab(q);
+        if (nmine > 1) issue_u(1);
+    }
+    DRows<T, P> dr;
+    dr.init(dp, i, j);
+    T partial = T(0);
+
+    int q = 0;                 // ring stage of the slab being consumed
+    uint32_t gphase = 0;       // its mbarrier parity
+    for (int64_t n = 0; n < nmine; ++n) {
+        const int64_t e = (blockIdx.x + n * gridDim.x) * EPB + slot;
+        const bool active = lane_ok && e < E;
+        const int ub = (int)(n & 1);
+        mbar_wait(&sm.ufull[ub], (uint32_t)((n >> 1) & 1));
+        const T* sue = &sm.u[ub][slot * P3];
+        T uk[P], wk[P];
+#pragma unroll
+        for (int k = 0; k < P; ++k) { uk[k] = active ? sue[k * P2 + ij] : T(0); wk[k] = T(0); }
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+            mbar_wait(&sm.gfull[q], gphase);
+            T g[6];
+#pragma unroll
+            for (int c = 0; c < 6; ++c) g[c] = active ? sm.g[q][slot * SLAB + c * P2 + ij] : T(0);
+            const int buf = k & 1;
+            if (active) slab_part1<T, P>(dp, dr, sue, uk, wk, g, k, i, j, &sm.sgr[buf][slot * P2], &sm.sgs[buf][slot * P2]);
+            __syncthreads();
+            // every thread has consumed stage q (and, on the last slab, this element's u buffer): refill
+            if (tid == 0) {
+                if (pn < nmine) issue_next_slab(q);
+                if (k == P - 1 && n + 2 < nmine) issue_u(n + 2);
+            }
+            if (active) wk[k] += slab_part2<T, P>(dr, i, j, &sm.sgr[buf][slot * P2], &sm.sgs[buf][slot * P2]);
+            if (++q == NS) { q = 0; gphase ^= 1u; }
+        }
+        if (active) {
+#pragma unroll
+            for (int k = 0; k < P; ++k) {
+                T v = wk[k];
+                if (Bm) v += lambda * Bm[e * P3 + k * P2 + ij] * uk[k];
+                w[e * P3 + k * P2 + ij] = v;
+                partial += uk[k] * v;
+            }
+        }
+    }
+    if (dot_out) block_dot_flush(partial, dot_out);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------------------------
+template <typename T, int P>
+DParam<T, P> make_dparam(const sem_ctx* c) {
+    DParam<T, P> d;
+    for (int q = 0; q < P * P; ++q) d.D[q] = (T)c->D[q];     // S16: rounded once from double
+    return d;
+}
+
+Gll1D make_gll(const sem_ctx* c) {
+    Gll1D g;
+    for (int i = 0; i < 16; ++i) { g.xi[i] = i < c->p ? c->xi[i] : 0.0; g.rho[i] = i < c->p ? c->rho[i] : 0.0; }
+    for (int i = 0; i < 256; ++i) g.D[i] = 0.0;              // only xi/rho are used by the Ax kernels
+    return g;
+}
+
+template <typename T, int P, bool RECOMP>
+int launch_simple(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, double* dot) {
+    constexpr int EPB = epb_of<P>();
+    const int64_t ngroups = (c->E + EPB - 1) / EPB;
+    const T* Gs = sizeof(T) == 8 ? (const T*)c->d_G : (const T*)c->d_G32;
+    const T* Bm = sizeof(T) == 8 ? (const T*)c->d_B : (const T*)c->d_B32;
+    const int64_t slab = sizeof(T) == 8 ? c->slab_f64 : c->slab_f32;
+    const unsigned grid = (unsigned)(ngroups < (int64_t)c->num_sms * 32 ? ngroups : (int64_t)c->num_sms * 32);
+    const DParam<T, P> dp = make_dparam<T, P>(c);
+    const Gll1D gll = make_gll(c);
+    ax_simple<T, P, RECOMP><<<grid, threads_of<P>(), 0, c->stream>>>(c->E, dp, gll, slab, Gs, c->d_vert,
+                                                                    lambda != T(0) ? Bm : nullptr, lambda, u, w, skip, dot);
+    SEM_CUDA_OK(c, cudaGetLastError());
+    return SEM_OK;
+}
+
+template <typename T, int P, int NS, int MINB>
+int launch_stream(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, double* dot) {
+    using SM = StreamSmem<T, P, NS>;
+    constexpr int EPB = epb_of<P>();
+    const int64_t ngroups = (c->E + EPB - 1) / EPB;
+    const T* Gs = sizeof(T) == 8 ? (const T*)c->d_G : (const T*)c->d_G32;
+    const T* Bm = sizeof(T) == 8 ? (const T*)c->d_B : (const T*)c->d_B32;
+    const DParam<T, P> dp = make_dparam<T, P>(c);
+    const size_t smem = sizeof(SM) + 128;
+    auto go = [&](auto kern) -> int {
+        static thread_local int cached_dev = -1;
+        static thread_local int blocks_per_sm = 0;
+        if (cached_dev != c->device) {
+            SEM_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            SEM_CUDA_OK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, threads_of<P>(), smem));
+            if (blocks_per_sm < 1) return sem_fail(c, SEM_ECUDA, "ax_stream does not fit on an SM");
+            cached_dev = c->device;
+        }
+        const int64_t cap = (int64_t)c->num_sms * blocks_per_sm;
+        const unsigned grid = (unsigned)(ngroups < cap ? ngroups : cap);
+        kern<<<grid, threads_of<P>(), smem, c->stream>>>(c->E, dp, Gs, lambda != T(0) ? Bm : nullptr, lambda, u, w, skip, dot);
+        SEM_CUDA_OK(c, cudaGetLastError());
+        return SEM_OK;
+    };
+    return go(ax_stream<T, P, NS, MINB>);
+}
+
+// stage depth / residency per (T, P): sized so that ~7-8 CTAs fit in 227 KB and > 64 KB are in flight per SM
+template <typename T, int P> struct StreamCfg { static constexpr int NS = 4, MINB = 1; };
+template <> struct StreamCfg<double, 8> { static constexpr int NS = 5, MINB = 8; };
+template <> struct StreamCfg<float, 8> { static constexpr int NS = 8, MINB = 8; };
+template <> struct StreamCfg<double, 2> { static constexpr int NS = 2, MINB = 8; };
+template <> struct StreamCfg<float, 2> { static constexpr int NS = 2, MINB = 8; };
+template <> struct StreamCfg<double, 4> { static constexpr int NS = 4, MINB = 8; };
+template <> struct StreamCfg<float, 4> { static constexpr int NS = 4, MINB = 8; };
+template <> struct StreamCfg<double, 6> { static constexpr int NS = 5, MINB = 6; };
+template <> struct StreamCfg<float, 6> { static constexpr int NS = 6, MINB = 6; };
+template <> struct StreamCfg<double, 10> { static constexpr int NS = 4, MINB = 4; };
+template <> struct StreamCfg<float, 10> { static constexpr int NS = 6, MINB = 4; };
+
+template <typename T, int P>
+int dispatch_p(sem_ctx* c, const void* u, void* w, double lambda, const int* skip, double* dot) {
+    const T* uu = (const T*)u;
+    T* ww = (T*)w;
+    if (c->gmode == SEM_G_RECOMPUTE) return launch_simple<T, P, true>(c, uu, ww, (T)lambda, skip, dot);
+    if constexpr (P % 2 == 0 && P <= 12) {
+        if (c->ax_variant == 0 && ((uintptr_t)u % 16) == 0)
+            return launch_stream<T, P, StreamCfg<T, P>::NS, StreamCfg<T, P>::MINB>(c, uu, ww, (T)lambda, skip, dot);
+    }
+    return launch_simple<T, P, false>(c, uu, ww, (T)lambda, skip, dot);
+}
+
+template <typename T>
+int dispatch(sem_ctx* c, const void* u, void* w, double lambda, const int* skip, double* dot) {
+    switch (c->p) {
+#define SEM_CASE(PP) case PP: return dispatch_p<T, PP>(c, u, w, lambda, skip, dot);
+        SEM_CASE(2) SEM_CASE(3) SEM_CASE(4) SEM_CASE(5) SEM_CASE(6) SEM_CASE(7) SEM_CASE(8) SEM_CASE(9)
+        SEM_CASE(10) SEM_CASE(11) SEM_CASE(12) SEM_CASE(13) SEM_CASE(14) SEM_CASE(15) SEM_CASE(16)
+#undef SEM_CASE
+    }
+    return sem_fail(c, SEM_EINVAL, "unsupported p = %d", c->p);
+}
+
+}  // namespace
+
+// dot_out != nullptr: also accumulate sum_l u_l w_l (the un-assembled local dot, O8) into *dot_out (device, FP64).
+// skip_flag != nullptr: the kernel returns at once if *skip_flag != 0 (device; used by the PCG loop after convergence).
+int sem_launch_ax(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda, double* dot_out,
+                  const int* skip_flag) {
+    if (prec == SEM_F64) return dispatch<double>(c, u, w, lambda, skip_flag, dot_out);
+    return dispatch<float>(c, u, w, lambda, skip_flag, dot_out);
+}

@@ -1,0 +1,218 @@
+// sem_geom.cu — a2 (setup): geometric factors, the exact Jacobi diagonal, and the layout conversions around them.
+// P:69 (isoparametric map), O3 (G, B, detJ), O7 (exact diagonal incl. cross terms), S16 (FP32 copy rounded once).
+//
+// Device layout of G ("slab layout", library-owned): Gs[e][k][c][j*p+i], c = rr,rs,rt,ss,st,tt, so that the six
+// factors of one k-slab of one element are one contiguous chunk (one bulk copy in the Ax kernel).
+#include "sem_geom_dev.cuh"
+#include "sem_internal.h"
+
+namespace {
+
+inline unsigned nblk(int64_t n, int t = 256) { return (unsigned)((n + t - 1) / t); }
+
+// One thread per node.  xyz == nullptr: analytic trilinear Jacobian (S5); else D applied to xyz (isoparametric).
+__global__ void k_geom(int64_t E, int p, Gll1D gll, const double* __restrict__ vert, const double* __restrict__ xyz,
+                       int64_t slab, double* __restrict__ Gs, double* __restrict__ Bm, double* __restrict__ detJ,
+                       int* __restrict__ bad) {
+    const int64_t p2 = (int64_t)p * p, p3 = p2 * p;
+    const int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (l >= E * p3) return;
+    const int64_t e = l / p3;
+    const int n = (int)(l - e * p3);
+    const int k = n / (int)p2, j = (n / p) % p, i = n % p;
+    double J[3][3];
+    if (xyz == nullptr) {
+        double X[8][3], cf[8][3];
+#pragma unroll
+        for (int v = 0; v < 8; ++v)
+#pragma unroll
+            for (int d = 0; d < 3; ++d) X[v][d] = vert[(e * 8 + v) * 3 + d];
+        sem_trilinear_coef(X, cf);
+        sem_trilinear_jac(cf, gll.xi[i], gll.xi[j], gll.xi[k], J);
+    } else {
+        const double* Xe = xyz + e * p3 * 3;
+        for (int a = 0; a < 3; ++a) {
+            double dr = 0, ds = 0, dt = 0;
+            for (int m = 0; m < p; ++m) {
+                dr += gll.D[i * p + m] * Xe[((int64_t)(k * p + j) * p + m) * 3 + a];
+                ds += gll.D[j * p + m] * Xe[((int64_t)(k * p + m) * p + i) * 3 + a];
+                dt += gll.D[k * p + m] * Xe[((int64_t)(m * p + j) * p + i) * 3 + a];
+            }
+            J[a][0] = dr; J[a][1] = ds; J[a][2] = dt;
+        }
+    }
+    double g[6], B;
+    const double det = sem_factors(J, gll.rho[i] * gll.rho[j] * gll.rho[k], g, B);
+    if (!(det > 0.0)) atomicOr(bad, 1);
+    double* slab_ptr = Gs + (e * p + k) * slab + (j * p + i);
+#pragma unroll
+    for (int c = 0; c < 6; ++c) slab_ptr[c * p2] = g[c];
+    if (Bm) Bm[l] = B;
+    detJ[l] = det;
+}
+
+template <typename Tin, typename Tout>
+__global__ void k_convert(int64_t n, const Tin* __restrict__ in, Tout* __restrict__ out) {
+    int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (; t < n; t += stride) out[t] = (Tout)in[t];
+}
+
+// slab layout (stride slab_in) -> FP32 slab layout (stride slab_out)
+__global__ void k_g32(int64_t nslabs, int cnt, int64_t slab_in, int64_t slab_out, const double* __restrict__ in,
+                      float* __restrict__ out) {
+    int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const int64_t total = nslabs * cnt;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (; t < total; t += stride) {
+        const int64_t s = t / cnt;
+        const int r = (int)(t - s * cnt);
+        out[s * slab_out + r] = (float)in[s * slab_in + r];
+    }
+}
+
+// O7: exact local diagonal.  One thread per node.
+__global__ void k_diag_local(int64_t E, int p, Gll1D gll, int64_t slab, const double* __restrict__ Gs,
+                             const double* __restrict__ Bm, double lambda, double* __restrict__ diag) {
+    const int64_t p2 = (int64_t)p * p, p3 = p2 * p;
+    const int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (l >= E * p3) return;
+    const int64_t e = l / p3;
+    const int n = (int)(l - e * p3);
+    const int k = n / (int)p2, j = (n / p) % p, i = n % p;
+    const double* Ge = Gs + e * p * slab;
+    auto G = [&](int c, int kk, int jj, int ii) { return Ge[kk * slab + c * p2 + jj * p + ii]; };
+    double d = 0.0;
+    for (int m = 0; m < p; ++m) {
+        const double di = gll.D[m * p + i], dj = gll.D[m * p + j], dk = gll.D[m * p + k];
+        d += di * di * G(0, k, j, m);
+        d += dj * dj * G(3, k, m, i);
+        d += dk * dk * G(5, m, j, i);
+    }
+    const double dii = gll.D[i * p + i], djj = gll.D[j * p + j], dkk = gll.D[k * p + k];
+    d += 2.0 * (dii * djj * G(1, k, j, i) + dii * dkk * G(2, k, j, i) + djj * dkk * G(4, k, j, i));
+    if (lambda != 0.0) d += lambda * Bm[l];
+    diag[l] = d;
+}
+
+// Minv = mask / diag (S12, S14); wt = mask / mult (unique-node dot weights in local storage, O8)
+__global__ void k_minv_wt(int64_t n, const double* __restrict__ diag, const int32_t* __restrict__ l2u,
+                          const int32_t* __restrict__ mult, const uint8_t* __restrict__ mask_u,
+                          double* __restrict__ Minv, double* __restrict__ wt) {
+    const int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (l >= n) return;
+    const int32_t g = l2u[l];
+    const bool masked = mask_u && mask_u[g];
+    Minv[l] = masked ? 0.0 : 1.0 / diag[l];
+    wt[l] = masked ? 0.0 : 1.0 / (double)mult[g];
+}
+
+// slab layout -> [E][ncomp][p^3] export (+ B as 7th)
+__global__ void k_export(int64_t E, int p, int ncomp, int64_t slab, const double* __restrict__ Gs,
+                         const double* __restrict__ Bm, double* __restrict__ out) {
+    const int64_t p2 = (int64_t)p * p, p3 = p2 * p;
+    const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (t >= E * ncomp * p3) return;
+    const int64_t e = t / (ncomp * p3);
+    const int64_t r = t - e * ncomp * p3;
+    const int c = (int)(r / p3);
+    const int n = (int)(r - c * p3);
+    const int k = n / (int)p2, ji = n % (int)p2;
+    out[t] = c < 6 ? Gs[(e * p + k) * slab + c * p2 + ji] : Bm[e * p3 + n];
+}
+
+Gll1D make_gll(const sem_ctx* c) {
+    Gll1D g;
+    for (int i = 0; i < 16; ++i) { g.xi[i] = i < c->p ? c->xi[i] : 0.0; g.rho[i] = i < c->p ? c->rho[i] : 0.0; }
+    for (int i = 0; i < 256; ++i) g.D[i] = i < c->p * c->p ? c->D[i] : 0.0;
+    return g;
+}
+
+}  // namespace
+
+int sem_build_geom(sem_ctx* c, const double* node_xyz_host) {
+    cudaStream_t st = c->stream;
+    const int p = c->p;
+    const int64_t p2 = (int64_t)p * p;
+    c->slab_f64 = 6 * p2;                                   // 48 p^2 bytes: always a multiple of 16
+    c->slab_f32 = 6 * p2 + ((6 * p2 * 4) % 16 ? 2 : 0);     // pad odd p to a multiple of 16 bytes
+    const int64_t gcount = c->E * p * c->slab_f64;
+    cudaFree(c->d_G); cudaFree(c->d_B); cudaFree(c->d_detJ); cudaFree(c->d_G32); cudaFree(c->d_B32);
+    c->d_G = nullptr; c->d_B = nullptr; c->d_detJ = nullptr; c->d_G32 = nullptr; c->d_B32 = nullptr;
+    SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_G, gcount * sizeof(double)));
+    SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_detJ, c->nL * sizeof(double)));
+    if (c->with_mass) SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_B, c->nL * sizeof(double)));
+    double* d_xyz = nullptr;
+    if (node_xyz_host) {
+        SEM_CUDA_OK(c, cudaMalloc((void**)&d_xyz, c->nL * 3 * sizeof(double)));
+        cudaError_t e = cudaMemcpyAsync(d_xyz, node_xyz_host, c->nL * 3 * sizeof(double), cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) { cudaFree(d_xyz); return sem_fail(c, SEM_ECUDA, "copy node_xyz: %s", cudaGetErrorString(e)); }
+    }
+    int* d_bad = nullptr;
+    cudaError_t e = cudaMalloc((void**)&d_bad, sizeof(int));
+    if (e != cudaSuccess) { cudaFree(d_xyz); return sem_fail(c, SEM_ENOMEM, "cudaMalloc: %s", cudaGetErrorString(e)); }
+    cudaMemsetAsync(d_bad, 0, sizeof(int), st);
+    k_geom<<<nblk(c->nL), 256, 0, st>>>(c->E, p, make_gll(c), c->d_vert, d_xyz, c->slab_f64, c->d_G, c->d_B, c->d_detJ,
+                                         d_bad);
+    int h_bad = 0;
+    cudaMemcpyAsync(&h_bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, st);
+    e = cudaStreamSynchronize(st);
+    cudaFree(d_bad);
+    cudaFree(d_xyz);
+    if (e != cudaSuccess) return sem_fail(c, SEM_ECUDA, "geometry kernel: %s", cudaGetErrorString(e));
+    SEM_CUDA_OK(c, cudaGetLastError());
+    if (h_bad) return sem_fail(c, SEM_EMESH, "non-positive Jacobian determinant in at least one node");
+    return SEM_OK;
+}
+
+int sem_build_g32(sem_ctx* c) {
+    if (c->d_G32) return SEM_OK;
+    cudaStream_t st = c->stream;
+    const int64_t nslabs = c->E * c->p;
+    SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_G32, nslabs * c->slab_f32 * sizeof(float)));
+    if (c->slab_f32 != c->slab_f64) SEM_CUDA_OK(c, cudaMemsetAsync(c->d_G32, 0, nslabs * c->slab_f32 * sizeof(float), st));
+    k_g32<<<c->num_sms * 8, 256, 0, st>>>(nslabs, 6 * c->p * c->p, c->slab_f64, c->slab_f32, c->d_G, c->d_G32);
+    if (c->with_mass) {
+        SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_B32, c->nL * sizeof(float)));
+        k_convert<double, float><<<c->num_sms * 8, 256, 0, st>>>(c->nL, c->d_B, c->d_B32);
+    }
+    SEM_CUDA_OK(c, cudaGetLastError());
+    return SEM_OK;
+}
+
+int sem_build_diag(sem_ctx* c) {
+    cudaStream_t st = c->stream;
+    if (!c->d_diag) {
+        SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_diag, c->nL * sizeof(double)));
+        SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_Minv, c->nL * sizeof(double)));
+        SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_wt, c->nL * sizeof(double)));
+    }
+    k_diag_local<<<nblk(c->nL), 256, 0, st>>>(c->E, c->p, make_gll(c), c->slab_f64, c->d_G, c->d_B, c->lambda, c->d_diag);
+    int rc = sem_launch_gs(c, c->d_diag, SEM_F64, /*apply_mask=*/false);
+    if (rc) return rc;
+    k_minv_wt<<<nblk(c->nL), 256, 0, st>>>(c->nL, c->d_diag, c->d_l2u, c->d_mult, c->has_mask ? c->d_mask_u : nullptr,
+                                            c->d_Minv, c->d_wt);
+    SEM_CUDA_OK(c, cudaGetLastError());
+    c->lambda_of_diag = c->lambda;
+    return SEM_OK;
+}
+
+int sem_geom_export(sem_ctx* c, double* G_host, double* detJ_host) {
+    cudaStream_t st = c->stream;
+    if (G_host) {
+        const int ncomp = c->with_mass ? 7 : 6;
+        const int64_t cnt = c->E * ncomp * c->p3;
+        double* d_out = nullptr;
+        SEM_CUDA_OK(c, cudaMalloc((void**)&d_out, cnt * sizeof(double)));
+        k_export<<<nblk(cnt), 256, 0, st>>>(c->E, c->p, ncomp, c->slab_f64, c->d_G, c->d_B, d_out);
+        cudaError_t e = cudaMemcpyAsync(G_host, d_out, cnt * sizeof(double), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        cudaFree(d_out);
+        if (e != cudaSuccess) return sem_fail(c, SEM_ECUDA, "export G: %s", cudaGetErrorString(e));
+    }
+    if (detJ_host) {
+        SEM_CUDA_OK(c, cudaMemcpyAsync(detJ_host, c->d_detJ, c->nL * sizeof(double), cudaMemcpyDeviceToHost, st));
+        SEM_CUDA_OK(c, cudaStreamSynchronize(st));
+    }
+    return SEM_OK;
+}

@@ -1,0 +1,88 @@
+// sem_internal.h — context struct and internal launcher declarations of libsem.so (not part of the C ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+
+#include "../../include/sem.h"
+
+#define SEM_MAXP 16
+
+struct sem_ctx {
+    // ---- discretisation (a0) ----
+    int64_t E = 0;
+    int N = 0, p = 0;
+    int64_t p3 = 0, nL = 0;
+    double xi[SEM_MAXP], rho[SEM_MAXP], D[SEM_MAXP * SEM_MAXP];   // D[i*p+l] = dh_l/dr(xi_i)
+    cudaStream_t stream = 0;
+    int device = 0, num_sms = 148;
+    // ---- mesh ----
+    double* d_vert = nullptr;      // [E][8][3]
+    // ---- gather-scatter maps (a1, O6) ----
+    int64_t U = 0, S = 0, Us = 0;
+    int32_t* d_l2u = nullptr;      // [nL]
+    int32_t* d_mult = nullptr;     // [U]
+    int64_t* d_seg_off = nullptr;  // [U+1]
+    int32_t* d_seg_idx = nullptr;  // [nL]
+    int64_t* d_uniq_gid = nullptr; // [U]
+    // compressed shared-only form used by the gs kernel: unique nodes with mult > 1, ascending
+    int32_t* d_sh_off = nullptr;   // [Us+1] offsets into d_sh_idx
+    int32_t* d_sh_idx = nullptr;   // [S] local indices
+    uint8_t* d_sh_masked = nullptr;// [Us] 1 = Dirichlet
+    // Dirichlet (S14)
+    bool has_mask = false;
+    uint8_t* d_mask_u = nullptr;   // [U] 1 = masked unique node
+    int64_t n_mask1 = 0;           // masked local nodes with mult == 1
+    int32_t* d_mask1_idx = nullptr;// [n_mask1]
+    // ---- geometry (a2, O3) ----
+    bool geom_done = false;
+    sem_gmode gmode = SEM_G_STORED;
+    bool with_mass = false;
+    // slab layout: Gs[e][k][c][j*p+i], c = rr,rs,rt,ss,st,tt; slab stride padded to 16 B
+    double* d_G = nullptr;
+    float* d_G32 = nullptr;        // built lazily at the first FP32 call
+    double* d_B = nullptr;         // [E][p^3] rho rho rho detJ   (with_mass)
+    float* d_B32 = nullptr;
+    double* d_detJ = nullptr;      // [E][p^3]
+    int64_t slab_f64 = 0, slab_f32 = 0;   // slab strides in elements of T
+    // ---- Jacobi / PCG (a8, O7, O8) ----
+    double lambda = 0.0;
+    double* d_diag = nullptr;      // assembled, unmasked, local layout
+    double* d_Minv = nullptr;      // mask / diag, local layout
+    double* d_wt = nullptr;        // 1/mult per local node (0 at masked nodes): unique-node dot weights
+    bool pcg_ready = false;
+    double lambda_of_diag = -1.0;  // lambda the stored diagonal was built for (-1 = none)
+    double *d_r = nullptr, *d_p = nullptr, *d_w = nullptr;
+    double* d_scal = nullptr;      // device scalars, see sem_pcg.cu
+    int64_t scal_cap = 0;
+    double* h_hist = nullptr;
+    int hist_n = 0;
+    // ---- misc ----
+    int ax_variant = 0;
+    std::string err;
+};
+
+int sem_fail(sem_ctx* c, int code, const char* fmt, ...);
+#define SEM_CUDA_OK(c, expr)                                                                          \
+    do {                                                                                              \
+        cudaError_t e__ = (expr);                                                                     \
+        if (e__ != cudaSuccess)                                                                       \
+            return sem_fail((c), e__ == cudaErrorMemoryAllocation ? SEM_ENOMEM : SEM_ECUDA, "%s: %s", \
+                            #expr, cudaGetErrorString(e__));                                          \
+    } while (0)
+
+// sem_gll.cpp
+void sem_gll_tables(int N, double* xi, double* rho, double* D);
+// sem_maps.cu
+int sem_build_maps(sem_ctx* c, const int64_t* gid_any, const uint8_t* dirichlet_host);
+// sem_geom.cu
+int sem_build_geom(sem_ctx* c, const double* node_xyz_host);
+int sem_build_g32(sem_ctx* c);
+int sem_build_diag(sem_ctx* c);
+int sem_geom_export(sem_ctx* c, double* G_host, double* detJ_host);
+// sem_ax.cu
+int sem_launch_ax(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda, double* dot_out,
+                  const int* skip_flag);
+// sem_gs.cu
+int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask);

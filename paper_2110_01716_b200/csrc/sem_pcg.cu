@@ -1,0 +1,217 @@
+// sem_pcg.cu — a8: Jacobi-preconditioned conjugate gradients on A = M QQ^T (D^T G D + lambda B) M, FP64.
+// P:101 "Jacobi-preconditioned conjugate gradient iteration"; O8 / S12-S14 fix the details:
+//   x = M x0; r = M b - A x; z = Minv r; p = z; rho = r.z; r0 = ||r||
+//   it = 1..maxit: q = A p; alpha = rho / p.q; x += alpha p; r -= alpha q; stop if ||r|| <= tol r0;
+//                  z = Minv r; rho' = r.z; beta = rho'/rho; p = z + beta p
+// All vectors are in local (element) layout and continuous, so a dot over unique unmasked nodes is the local sum
+// weighted by wt = mask/mult; p.q is the un-assembled local dot sum_l p_l (A_L p)_l, fused into the Ax kernel.
+//
+// The loop never returns to the host for a scalar: every dot lands in a per-iteration slot of a device array,
+// every kernel reads what it needs from there, and a device flag turns all later launches into no-ops once the
+// stopping test (or p.q <= 0) fires.  The host only polls that flag every few iterations.
+#include <math.h>
+
+#include "sem_internal.h"
+
+namespace {
+
+// device scalars: slot(it) = 4*it + {0: p.q, 1: r.r, 2: r.z};  it = 0 holds the initial r.r and r.z
+struct PcgFlags { int done; int iters; int breakdown; int pad; };
+
+__device__ __forceinline__ void block_sum2_atomic(double a, double b, double* __restrict__ outa,
+                                                  double* __restrict__ outb) {
+    __shared__ double red[2][32];
+    for (int o = 16; o; o >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, o); b += __shfl_xor_sync(0xffffffffu, b, o); }
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+    if (lane == 0) { red[0][warp] = a; red[1][warp] = b; }
+    __syncthreads();
+    if (warp == 0) {
+        a = lane < nw ? red[0][lane] : 0.0;
+        b = lane < nw ? red[1][lane] : 0.0;
+        for (int o = 16; o; o >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, o); b += __shfl_xor_sync(0xffffffffu, b, o); }
+        if (lane == 0) { atomicAdd(outa, a); atomicAdd(outb, b); }
+    }
+}
+
+// r = M (b - q) (q = A x0, may be null), x = M x, z = Minv r, p = z; accumulate r.r and r.z into slot 0
+__global__ void __launch_bounds__(256) k_pcg_init(int64_t n, const double* __restrict__ b, const double* __restrict__ q,
+                                                  const double* __restrict__ Minv, const double* __restrict__ wt,
+                                                  double* __restrict__ x, double* __restrict__ r,
+                                                  double* __restrict__ p, double* __restrict__ scal) {
+    double srr = 0.0, srz = 0.0;
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
+        const double wl = wt[l];
+        const bool live = wl != 0.0;
+        const double rl = live ? (q ? b[l] - q[l] : b[l]) : 0.0;
+        if (!live) x[l] = 0.0;
+        const double zl = Minv[l] * rl;
+        r[l] = rl;
+        p[l] = zl;
+        srr += wl * rl * rl;
+        srz += wl * rl * zl;
+    }
+    block_sum2_atomic(srr, srz, scal + 1, scal + 2);
+}
+
+__global__ void __launch_bounds__(256) k_mask_vec(int64_t n, const double* __restrict__ wt, double* __restrict__ x) {
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x)
+        if (wt[l] == 0.0) x[l] = 0.0;
+}
+
+// x += alpha p; r -= alpha w; accumulate r.r and r.z (z = Minv r) into slot it
+__global__ void __launch_bounds__(256) k_pcg_update(int64_t n, int it, const double* __restrict__ p,
+                                                    const double* __restrict__ w, const double* __restrict__ Minv,
+                                                    const double* __restrict__ wt, double* __restrict__ x,
+                                                    double* __restrict__ r, double* __restrict__ scal,
+                                                    PcgFlags* __restrict__ flags) {
+    if (flags->done) return;
+    const double pq = scal[4 * it + 0];
+    if (!(pq > 0.0)) {                                  // breakdown (S13): stop, keep x
+        if (blockIdx.x == 0 && threadIdx.x == 0) { flags->breakdown = 1; flags->iters = it; }
+        // `done` is raised by k_pcg_direction so that no block of this kernel can observe it half-way
+        return;
+    }
+    const double alpha = scal[4 * (it - 1) + 2] / pq;
+    double srr = 0.0, srz = 0.0;
+    const int64_t n2 = n >> 1;
+    const double2* p2 = reinterpret_cast<const double2*>(p);
+    const double2* w2 = reinterpret_cast<const double2*>(w);
+    const double2* m2 = reinterpret_cast<const double2*>(Minv);
+    const double2* t2 = reinterpret_cast<const double2*>(wt);
+    double2* x2 = reinterpret_cast<double2*>(x);
+    double2* r2 = reinterpret_cast<double2*>(r);
+    for (int64_t v = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; v < n2; v += (int64_t)gridDim.x * blockDim.x) {
+        const double2 pv = p2[v], wv = w2[v], mv = m2[v], tv = t2[v];
+        double2 xv = x2[v], rv = r2[v];
+        xv.x += alpha * pv.x; xv.y += alpha * pv.y;
+        rv.x -= alpha * wv.x; rv.y -= alpha * wv.y;
+        x2[v] = xv; r2[v] = rv;
+        const double ax = tv.x * rv.x * rv.x, ay = tv.y * rv.y * rv.y;
+        srr += ax + ay;
+        srz += ax * mv.x + ay * mv.y;
+    }
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+        const int64_t l = n - 1;
+        x[l] += alpha * p[l];
+        const double rl = r[l] - alpha * w[l];
+        r[l] = rl;
+        srr += wt[l] * rl * rl;
+        srz += wt[l] * rl * rl * Minv[l];
+    }
+    block_sum2_atomic(srr, srz, scal + 4 * it + 1, scal + 4 * it + 2);
+}
+
+// stopping test, then p = Minv r + beta p
+__global__ void __launch_bounds__(256) k_pcg_direction(int64_t n, int it, int maxit, double tol2,
+                                                       const double* __restrict__ r, const double* __restrict__ Minv,
+                                                       double* __restrict__ p, const double* __restrict__ scal,
+                                                       PcgFlags* __restrict__ flags) {
+    if (flags->done) return;
+    const bool first = blockIdx.x == 0 && threadIdx.x == 0;
+    if (flags->breakdown) { if (first) flags->done = 1; return; }
+    const double rr = scal[4 * it + 1];
+    const bool stop = rr <= tol2 * scal[1] || it >= maxit;
+    if (first) { flags->iters = it; if (stop) flags->done = 1; }
+    if (stop) return;
+    const double beta = scal[4 * it + 2] / scal[4 * (it - 1) + 2];
+    const int64_t n2 = n >> 1;
+    const double2* r2 = reinterpret_cast<const double2*>(r);
+    const double2* m2 = reinterpret_cast<const double2*>(Minv);
+    double2* p2 = reinterpret_cast<double2*>(p);
+    for (int64_t v = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; v < n2; v += (int64_t)gridDim.x * blockDim.x) {
+        const double2 rv = r2[v], mv = m2[v];
+        double2 pv = p2[v];
+        pv.x = mv.x * rv.x + beta * pv.x;
+        pv.y = mv.y * rv.y + beta * pv.y;
+        p2[v] = pv;
+    }
+    if ((n & 1) && first) p[n - 1] = Minv[n - 1] * r[n - 1] + beta * p[n - 1];
+}
+
+}  // namespace
+
+extern "C" int sem_pcg(sem_ctx* c, const double* b, double* x, double tol, int maxit, int* iters_out,
+                       double* relres_out) {
+    if (!c) return SEM_EINVAL;
+    c->err.clear();
+    if (!b || !x) return sem_fail(c, SEM_EINVAL, "sem_pcg: NULL vector");
+    if (((uintptr_t)x % 16) || ((uintptr_t)b % 8)) return sem_fail(c, SEM_EINVAL, "sem_pcg: x must be 16-byte aligned");
+    if (!(tol > 0.0) && maxit <= 0) return sem_fail(c, SEM_EINVAL, "sem_pcg: tol <= 0 with maxit <= 0");
+    if (!c->geom_done) return sem_fail(c, SEM_ESTATE, "sem_pcg before sem_geom");
+    if (c->lambda != 0.0 && !c->with_mass) return sem_fail(c, SEM_ESTATE, "lambda != 0 needs with_mass");
+    if (maxit < 0) maxit = 0;
+    cudaStream_t st = c->stream;
+    const int64_t n = c->nL;
+    if (!c->pcg_ready || c->lambda_of_diag != c->lambda) {
+        int rc = sem_build_diag(c);
+        if (rc) return rc;
+        if (!c->d_r) {
+            SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_r, n * sizeof(double)));
+            SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_p, n * sizeof(double)));
+            SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_w, n * sizeof(double)));
+        }
+        c->pcg_ready = true;
+    }
+    const int64_t need = 4 * ((int64_t)maxit + 2) + 8;      // doubles; the flags live after the slots
+    if (need > c->scal_cap) {
+        cudaFree(c->d_scal);
+        c->d_scal = nullptr;
+        SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_scal, need * sizeof(double)));
+        c->scal_cap = need;
+    }
+    double* scal = c->d_scal;
+    PcgFlags* flags = reinterpret_cast<PcgFlags*>(scal + 4 * ((int64_t)maxit + 2));
+    SEM_CUDA_OK(c, cudaMemsetAsync(scal, 0, need * sizeof(double), st));
+    const unsigned vgrid = (unsigned)c->num_sms * 8;
+
+    // r = M b - A (M x0)
+    k_mask_vec<<<vgrid, 256, 0, st>>>(n, c->d_wt, x);
+    int rc = sem_launch_ax(c, x, c->d_w, SEM_F64, c->lambda, nullptr, nullptr);
+    if (rc) return rc;
+    rc = sem_launch_gs(c, c->d_w, SEM_F64, true);
+    if (rc) return rc;
+    k_pcg_init<<<vgrid, 256, 0, st>>>(n, b, c->d_w, c->d_Minv, c->d_wt, x, c->d_r, c->d_p, scal);
+    double h0[4];
+    SEM_CUDA_OK(c, cudaMemcpyAsync(h0, scal, 4 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    SEM_CUDA_OK(c, cudaStreamSynchronize(st));
+    SEM_CUDA_OK(c, cudaGetLastError());
+    const double rr0 = h0[1];
+    int iters = 0;
+    PcgFlags hf = {0, 0, 0, 0};
+    if (rr0 > 0.0 && maxit > 0) {
+        const double tol2 = tol > 0.0 ? tol * tol : 0.0;
+        const int batch = 16;
+        for (int it = 1; it <= maxit; ++it) {
+            rc = sem_launch_ax(c, c->d_p, c->d_w, SEM_F64, c->lambda, scal + 4 * it, &flags->done);
+            if (rc) return rc;
+            rc = sem_launch_gs(c, c->d_w, SEM_F64, true);
+            if (rc) return rc;
+            k_pcg_update<<<vgrid, 256, 0, st>>>(n, it, c->d_p, c->d_w, c->d_Minv, c->d_wt, x, c->d_r, scal, flags);
+            k_pcg_direction<<<vgrid, 256, 0, st>>>(n, it, maxit, tol2, c->d_r, c->d_Minv, c->d_p, scal, flags);
+            if (it % batch == 0 || it == maxit) {
+                SEM_CUDA_OK(c, cudaMemcpyAsync(&hf, flags, sizeof(hf), cudaMemcpyDeviceToHost, st));
+                SEM_CUDA_OK(c, cudaStreamSynchronize(st));
+                if (hf.done) break;
+            }
+        }
+        SEM_CUDA_OK(c, cudaGetLastError());
+        iters = hf.iters;
+    }
+    // residual history from the per-iteration slots
+    delete[] c->h_hist;
+    c->h_hist = new double[iters + 1];
+    c->hist_n = iters + 1;
+    c->h_hist[0] = rr0 > 0.0 ? 1.0 : 0.0;
+    if (iters > 0) {
+        double* slots = new double[4 * ((size_t)iters + 1)];
+        cudaError_t e = cudaMemcpyAsync(slots, scal, 4 * ((size_t)iters + 1) * sizeof(double), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) { delete[] slots; return sem_fail(c, SEM_ECUDA, "pcg history: %s", cudaGetErrorString(e)); }
+        for (int i = 1; i <= iters; ++i) c->h_hist[i] = sqrt(slots[4 * i + 1] / rr0);
+        if (hf.breakdown) c->h_hist[iters] = c->h_hist[iters - 1];    // the failed iteration did not update r
+        delete[] slots;
+    }
+    if (iters_out) *iters_out = iters;
+    if (relres_out) *relres_out = c->h_hist[iters];
+    return SEM_OK;
+}

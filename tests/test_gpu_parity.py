@@ -1,0 +1,399 @@
+"""GPU parity tests: the CUDA path (through the C ABI of include/sem.h, via the thin binding) against the CPU oracle,
+element by element on the same seeded inputs.  Tolerances (BASELINE.json north_star / DESIGN.md):
+  maps bit-exact; FP64 Ax / gs / Ax+gs max|w_gpu - w_orc| / max|w_orc| <= 1e-12; FP32 <= 1e-5;
+  PCG ||x_gpu - x_orc||_inf / ||x_orc||_inf <= 1e-9 at equal iteration count."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2110_01716_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL64, TOL32, TOLPCG = 1e-12, 1e-5, 1e-9
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked test needs a CUDA device (run with -m 'not gpu' on CPU boxes)")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def binding():
+    from paper_2110_01716_b200 import binding as b, build
+    build.build()
+    b.lib()
+    return b
+
+
+def relerr(a, b):
+    return float(np.max(np.abs(np.asarray(a, np.float64) - b)) / np.max(np.abs(b)))
+
+
+def to_dev(torch, a, dtype=None):
+    t = torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    return t if dtype is None else t.to(dtype)
+
+
+def make_sem(binding, mesh, dirichlet=False, **geom_kw):
+    sem = binding.Sem(mesh.E, mesh.N, mesh.vert, mesh.gid, mesh.dirichlet if dirichlet else None)
+    sem.geom(**geom_kw)
+    return sem
+
+
+# ------------------------------------------------------------------------------------------------ a0: GLL tables
+@pytest.mark.parametrize("N", [1, 2, 3, 4, 5, 7, 9, 12, 15])
+def test_gll_tables(torch_cuda, binding, oracle_mod, N):
+    m = inputs.box_mesh(1, 1, 1, N)
+    with binding.Sem(1, N, m.vert, m.gid) as sem:
+        xi, rho, D = sem.gll()
+    oxi, orho, oD = oracle_mod.gll(N)
+    assert np.max(np.abs(xi - oxi)) <= 2e-16
+    assert np.max(np.abs(rho - orho) / orho) <= 1e-14
+    assert np.max(np.abs(D - oD)) <= 1e-13 * np.max(np.abs(oD))
+
+
+# ------------------------------------------------------------------------------------------------ a1: maps
+def _check_maps(binding, oracle_mod, mesh, gid=None, dirichlet=False):
+    gid = mesh.gid if gid is None else gid
+    with binding.Sem(mesh.E, mesh.N, mesh.vert, gid, mesh.dirichlet if dirichlet else None) as sem:
+        c, mp = sem.counts(), sem.maps()
+    om = oracle_mod.Maps(gid)
+    assert (c["nL"], c["U"], c["S"], c["Us"]) == (om.nL, om.U, om.S, om.Us)
+    for name in ["uniq_gid", "l2u", "mult", "seg_off", "seg_idx"]:
+        assert np.array_equal(mp[name], getattr(om, name)), name
+    return c
+
+
+def test_maps_bitexact_config1(torch_cuda, binding, oracle_mod):
+    c = _check_maps(binding, oracle_mod, inputs.config1(), dirichlet=True)
+    assert (c["U"], c["S"], c["Us"]) == (24389, 15192, 6813)          # tests/golden/p13_config1_pcg.txt
+
+
+def test_maps_bitexact_scrambled_sparse_ids(torch_cuda, binding, oracle_mod):
+    m = inputs.box_mesh(5, 3, 4, 3, "random", seed=7, permute_seed=11)
+    _check_maps(binding, oracle_mod, m)
+    # ids need not be contiguous (S11): a strictly increasing but gappy relabelling, > 2^32
+    _check_maps(binding, oracle_mod, m, gid=m.gid * 1000003 + (1 << 33))
+    # a non-monotone relabelling changes the canonical order; still must match the oracle bit for bit
+    _check_maps(binding, oracle_mod, m, gid=(m.gid * 7919) % 100003)
+
+
+def test_maps_device_gid(torch_cuda, binding, oracle_mod):
+    m = inputs.box_mesh(3, 3, 2, 4)
+    g = to_dev(torch_cuda, m.gid.ravel())
+    with binding.Sem(m.E, m.N, m.vert, g) as sem:
+        mp = sem.maps()
+    om = oracle_mod.Maps(m.gid)
+    assert np.array_equal(mp["seg_idx"], om.seg_idx) and np.array_equal(mp["l2u"], om.l2u)
+
+
+def test_maps_no_sharing_and_single_element(torch_cuda, binding, oracle_mod):
+    m = inputs.box_mesh(1, 1, 1, 2)
+    c = _check_maps(binding, oracle_mod, m)
+    assert c["S"] == 0 and c["Us"] == 0
+    m2 = inputs.box_mesh(2, 2, 2, 1)
+    # every node its own id: nothing shared although the mesh is connected geometrically
+    _check_maps(binding, oracle_mod, m2, gid=np.arange(m2.nL, dtype=np.int64).reshape(m2.gid.shape)[::-1].copy())
+
+
+# ------------------------------------------------------------------------------------------------ a2: geometry
+@pytest.mark.parametrize("N,geometry", [(7, "smooth"), (3, "random"), (4, "random"), (1, "smooth")])
+def test_geom_trilinear(torch_cuda, binding, oracle_mod, N, geometry):
+    m = inputs.box_mesh(4, 3, 5, N, geometry, seed=5)
+    with make_sem(binding, m, with_mass=True) as sem:
+        G, dJ = sem.get_geom()
+    oG, odJ, rc = oracle_mod.geom_trilinear(m.vert, N)
+    assert rc == 0
+    assert relerr(dJ, odJ) <= 1e-13
+    for cpt in range(7):
+        assert relerr(G[:, cpt], oG[:, cpt]) <= TOL64, cpt
+
+
+def test_geom_isoparametric(torch_cuda, binding, oracle_mod):
+    m = inputs.box_mesh(3, 3, 3, 5, "random", seed=2)
+    xyz = oracle_mod.node_xyz(m.vert, m.N)
+    # bend the elements beyond trilinear so that the isoparametric route is really exercised (still valid: small)
+    xyz = xyz + 0.01 * np.sin(3 * xyz[..., [1, 2, 0]]) * np.sin(np.pi * xyz) * np.sin(np.pi * xyz[..., [2, 0, 1]])
+    with binding.Sem(m.E, m.N, m.vert, m.gid) as sem:
+        sem.geom(node_xyz=xyz, with_mass=True)
+        G, dJ = sem.get_geom()
+    oG, odJ, rc = oracle_mod.geom_iso(xyz, m.N)
+    assert rc == 0
+    assert relerr(dJ, odJ) <= 1e-12
+    assert relerr(G, oG) <= 1e-11          # conditioning of the inverse Jacobian; Ax parity is checked separately
+
+
+def test_bad_mesh_and_bad_args(torch_cuda, binding):
+    m = inputs.box_mesh(2, 2, 2, 3)
+    v = m.vert.copy()
+    v[3, [0, 1]] = v[3, [1, 0]]                         # swap two vertices: inverted element
+    sem = binding.Sem(m.E, m.N, v, m.gid)
+    with pytest.raises(binding.SemError) as e:
+        sem.geom()
+    assert e.value.code == binding.SEM_EMESH
+    u = torch_cuda.zeros(m.nL, dtype=torch_cuda.float64, device="cuda")
+    w = torch_cuda.zeros_like(u)
+    with pytest.raises(binding.SemError) as e:
+        sem.ax(u, w)                                    # geometry failed: state error
+    assert e.value.code == binding.SEM_ESTATE
+    sem.close()
+    g = m.gid.copy()
+    g[0, 0] = -1
+    with pytest.raises(binding.SemError) as e:
+        binding.Sem(m.E, m.N, m.vert, g)
+    assert e.value.code == binding.SEM_EINVAL
+    with make_sem(binding, m) as sem:
+        with pytest.raises(binding.SemError) as e:
+            sem.ax(u, w, lam=1.0)                       # lambda without with_mass
+        assert e.value.code == binding.SEM_ESTATE
+        with pytest.raises(binding.SemError) as e:
+            sem.ax(u, u)                                # aliasing
+        assert e.value.code == binding.SEM_EINVAL
+
+
+# ------------------------------------------------------------------------------------------------ a3-a5: Ax
+def _ax_case(torch, binding, oracle_mod, mesh, variant=0, mode=0, lam=0.0, dtype="f64", seed=0):
+    oG, _, rc = oracle_mod.geom_trilinear(mesh.vert, mesh.N)
+    assert rc == 0
+    u = inputs.field_uniform(mesh.gid, seed)
+    ow = oracle_mod.ax(oG, u, mesh.N, lam)
+    tdt = torch.float64 if dtype == "f64" else torch.float32
+    with make_sem(binding, mesh, mode=mode, with_mass=lam != 0.0) as sem:
+        sem.set_variant(variant)
+        du = to_dev(torch, u.ravel(), tdt)
+        dw = torch.full_like(du, float("nan"))
+        sem.ax(du, dw, lam)
+        torch.cuda.synchronize()
+        w = dw.cpu().numpy().reshape(ow.shape)
+    return relerr(w, ow)
+
+
+@pytest.mark.parametrize("N", [1, 2, 3, 4, 5, 6, 7, 8, 9, 11, 13, 15])
+@pytest.mark.parametrize("variant", [0, 1])
+def test_ax_f64_all_orders(torch_cuda, binding, oracle_mod, N, variant):
+    # 5*3*3 = 45 elements: not a multiple of the elements-per-block of any p (ragged tail), several blocks
+    m = inputs.box_mesh(5, 3, 3, N, "random", seed=N)
+    assert _ax_case(torch_cuda, binding, oracle_mod, m, variant=variant) <= TOL64
+
+
+@pytest.mark.parametrize("N", [1, 3, 7])
+def test_ax_single_element(torch_cuda, binding, oracle_mod, N):
+    m = inputs.box_mesh(1, 1, 1, N, "affine")
+    assert _ax_case(torch_cuda, binding, oracle_mod, m) <= TOL64
+
+
+@pytest.mark.parametrize("N", [3, 7, 9])
+def test_ax_many_elements_per_cta(torch_cuda, binding, oracle_mod, N):
+    """More elements than resident CTAs: every persistent CTA walks the ring several times (phase wrap-around)."""
+    n = {3: 24, 7: 22, 9: 16}[N]
+    m = inputs.box_mesh(n, n, n + 1, N, "random", seed=1)
+    assert _ax_case(torch_cuda, binding, oracle_mod, m) <= TOL64
+
+
+@pytest.mark.parametrize("N", [1, 2, 3, 5, 7, 9])
+def test_ax_recomputed_G(torch_cuda, binding, oracle_mod, N):
+    m = inputs.box_mesh(4, 3, 3, N, "random", seed=3)
+    assert _ax_case(torch_cuda, binding, oracle_mod, m, mode=1) <= TOL64
+
+
+@pytest.mark.parametrize("N,variant", [(7, 0), (7, 1), (4, 0), (3, 0)])
+def test_ax_helmholtz(torch_cuda, binding, oracle_mod, N, variant):
+    m = inputs.box_mesh(3, 3, 3, N, "smooth")
+    assert _ax_case(torch_cuda, binding, oracle_mod, m, variant=variant, lam=37.5) <= TOL64
+
+
+@pytest.mark.parametrize("N", [1, 2, 3, 5, 7, 9])
+@pytest.mark.parametrize("variant,mode", [(0, 0), (1, 0), (0, 1)])
+def test_ax_f32(torch_cuda, binding, oracle_mod, N, variant, mode):
+    m = inputs.box_mesh(5, 4, 3, N, "smooth")
+    assert _ax_case(torch_cuda, binding, oracle_mod, m, variant=variant, mode=mode, dtype="f32") <= TOL32
+
+
+# ------------------------------------------------------------------------------------------------ a6/a7: gs, Ax+gs
+@pytest.mark.parametrize("N", [1, 3, 7])
+def test_gs_bit_identical(torch_cuda, binding, oracle_mod, N):
+    """Same summation order as the oracle (ascending local index), so FP64 sums agree to the last bit."""
+    m = inputs.box_mesh(4, 4, 3, N, permute_seed=5)
+    rng = np.random.default_rng(N)
+    w = rng.standard_normal(m.nL)                     # NOT continuous: a genuine gather-scatter input
+    ow = oracle_mod.gs(w, oracle_mod.Maps(m.gid))
+    with binding.Sem(m.E, m.N, m.vert, m.gid) as sem:
+        dw = to_dev(torch_cuda, w)
+        sem.gs(dw)
+        assert np.array_equal(dw.cpu().numpy(), ow)
+        w32 = w.astype(np.float32)
+        dw32 = to_dev(torch_cuda, w32)
+        sem.gs(dw32)
+        assert relerr(dw32.cpu().numpy(), oracle_mod.gs(w32.astype(np.float64), oracle_mod.Maps(m.gid))) <= 1e-6
+
+
+def _ax_gs_oracle(oracle_mod, mesh, u, masked, lam=0.0):
+    oG, _, _ = oracle_mod.geom_trilinear(mesh.vert, mesh.N)
+    ow = oracle_mod.gs(oracle_mod.ax(oG, u, mesh.N, lam).ravel(), oracle_mod.Maps(mesh.gid))
+    if masked:
+        om = oracle_mod.Maps(mesh.gid)
+        ow[oracle_mod.mask_unique(mesh.dirichlet, om)[om.l2u] != 0] = 0.0
+    return ow
+
+
+@pytest.mark.parametrize("masked", [False, True])
+def test_ax_gs_config1(torch_cuda, binding, oracle_mod, masked):
+    m = inputs.config1()
+    u = inputs.field_uniform(m.gid, 0)
+    ow = _ax_gs_oracle(oracle_mod, m, u, masked)
+    with make_sem(binding, m, dirichlet=masked) as sem:
+        du = to_dev(torch_cuda, u.ravel())
+        dw = torch_cuda.empty_like(du)
+        sem.ax_gs(du, dw)
+        assert relerr(dw.cpu().numpy(), ow) <= TOL64
+        # determinism: no atomics on this path, so a second application is bit-identical
+        dw2 = torch_cuda.empty_like(du)
+        sem.ax_gs(du, dw2)
+        assert torch_cuda.equal(dw, dw2)
+
+
+@pytest.mark.parametrize("N", [7, 3, 1])
+def test_ax_gs_f32_levels_config4_small(torch_cuda, binding, oracle_mod, N):
+    """Config 4 (mixed-precision levels N = 7, 3, 1), down-sized mesh: FP32 Ax+gs against the FP64 oracle."""
+    m = inputs.box_mesh(6, 5, 4, N, "smooth")
+    u = inputs.field_normal(m.gid, 2)
+    ow = _ax_gs_oracle(oracle_mod, m, u, False)
+    with make_sem(binding, m) as sem:
+        du = to_dev(torch_cuda, u.ravel(), torch_cuda.float32)
+        dw = torch_cuda.empty_like(du)
+        sem.ax_gs(du, dw)
+        assert relerr(dw.cpu().numpy(), ow) <= TOL32
+
+
+@pytest.mark.slow
+def test_ax_gs_config2_full_size(torch_cuda, binding, oracle_mod):
+    """BASELINE config 2 (7200 elements, N = 7) in the launch configuration bench.py times, every output compared."""
+    m = inputs.config2()
+    u = inputs.field_uniform(m.gid, 0)
+    ow = _ax_gs_oracle(oracle_mod, m, u, False)
+    with make_sem(binding, m) as sem:
+        c = sem.counts()
+        assert (c["nL"], c["U"], c["S"], c["Us"]) == (3686400, 2524887, 2049160, 887647)
+        du = to_dev(torch_cuda, u.ravel())
+        dw = torch_cuda.empty_like(du)
+        for _ in range(3):
+            sem.ax_gs(du, dw)
+        assert relerr(dw.cpu().numpy(), ow) <= TOL64
+        d32 = du.float()
+        w32 = torch_cuda.empty_like(d32)
+        sem.ax_gs(d32, w32)
+        assert relerr(w32.cpu().numpy(), ow) <= TOL32
+
+
+def test_stored_vs_recomputed_config3_smallest(torch_cuda, binding, oracle_mod):
+    """Config 3: stored-G and recomputed-G variants agree with the oracle (and so with each other) <= 1e-12."""
+    for N in (3, 5, 7, 9):
+        m = inputs.config3(8, N)
+        u = inputs.field_uniform(m.gid, 1)
+        ow = _ax_gs_oracle(oracle_mod, m, u, False)
+        for mode in (0, 1):
+            with make_sem(binding, m, mode=mode) as sem:
+                du = to_dev(torch_cuda, u.ravel())
+                dw = torch_cuda.empty_like(du)
+                sem.ax_gs(du, dw)
+                assert relerr(dw.cpu().numpy(), ow) <= TOL64, (N, mode)
+
+
+# ------------------------------------------------------------------------------------------------ a8: Jacobi-PCG
+def test_diag_exact(torch_cuda, binding, oracle_mod):
+    m = inputs.box_mesh(3, 4, 3, 5, "random", seed=9)
+    oG, _, _ = oracle_mod.geom_trilinear(m.vert, m.N)
+    od = oracle_mod.gs(oracle_mod.diag_local(oG, m.N).ravel(), oracle_mod.Maps(m.gid))
+    with make_sem(binding, m, dirichlet=True) as sem:
+        assert relerr(sem.get_diag().ravel(), od) <= TOL64
+
+
+def _pcg_setup(oracle_mod, mesh):
+    om = oracle_mod.Maps(mesh.gid)
+    oG, _, _ = oracle_mod.geom_trilinear(mesh.vert, mesh.N)
+    mask_u = oracle_mod.mask_unique(mesh.dirichlet, om)
+    return om, oG, mask_u
+
+
+def test_pcg_config1_20_iterations(torch_cuda, binding, oracle_mod):
+    m = inputs.config1()
+    om, oG, mask_u = _pcg_setup(oracle_mod, m)
+    xyz = oracle_mod.node_xyz(m.vert, m.N).reshape(-1, 3)
+    us_u = np.zeros(om.U)
+    us_u[om.l2u] = np.sin(np.pi * xyz[:, 0]) * np.sin(np.pi * xyz[:, 1]) * np.sin(np.pi * xyz[:, 2])
+    us_u[mask_u != 0] = 0.0
+    b_u = oracle_mod.apply_Ag(oG, m.N, om, mask_u, us_u)
+    ores = oracle_mod.pcg(oG, m.N, om, mask_u, b_u, tol=1e-30, maxit=20, snap_its=(1, 5, 10, 20))
+    assert ores["iters"] == 20
+    with make_sem(binding, m, dirichlet=True) as sem:
+        b = to_dev(torch_cuda, b_u[om.l2u])
+        for its in (1, 5, 10, 20):
+            x = torch_cuda.zeros_like(b)
+            it, rel = sem.pcg(b, x, 1e-30, its)
+            assert it == its
+            xg = x.cpu().numpy()
+            assert np.array_equal(xg, xg[om.seg_idx[om.seg_off[:-1]]][om.l2u])      # continuous
+            assert relerr(xg, ores["snaps"][its][om.l2u]) <= TOLPCG
+            assert abs(rel - ores["hist"][its]) <= 1e-9 * ores["hist"][its]
+        hist = sem.pcg_history(21)
+        assert np.max(np.abs(hist - ores["hist"]) / ores["hist"]) <= 1e-9
+    gold = {}
+    for line in open(os.path.join(GOLD, "p13_config1_pcg.txt")):
+        if not line.startswith("#") and line.strip():
+            k, v = line.split(None, 1)
+            gold[k] = v.strip()
+    assert abs(hist[20] - float(gold["relres_it20"])) <= 1e-9
+    assert abs(np.max(np.abs(xg - us_u[om.l2u])) - float(gold["err_inf_it20"])) <= 1e-9
+
+
+def test_pcg_converges_same_iteration_count(torch_cuda, binding, oracle_mod):
+    m = inputs.box_mesh(4, 4, 4, 5, "random", seed=3, permute_seed=4)      # config-5 recipe, down-sized
+    om, oG, mask_u = _pcg_setup(oracle_mod, m)
+    xyz = oracle_mod.node_xyz(m.vert, m.N).reshape(-1, 3)
+    f = 3 * np.pi ** 2 * np.sin(np.pi * xyz[:, 0]) * np.sin(np.pi * xyz[:, 1]) * np.sin(np.pi * xyz[:, 2])
+    b_u = np.zeros(om.U)
+    np.add.at(b_u, om.l2u, oG[:, 6].ravel() * f)
+    b_u[mask_u != 0] = 0.0
+    ores = oracle_mod.pcg(oG, m.N, om, mask_u, b_u, tol=1e-8, maxit=500)
+    with make_sem(binding, m, dirichlet=True) as sem:
+        b = to_dev(torch_cuda, b_u[om.l2u])
+        x = torch_cuda.zeros_like(b)
+        it, rel = sem.pcg(b, x, 1e-8, 500)
+        assert it == ores["iters"] and rel <= 1e-8
+        assert relerr(x.cpu().numpy(), ores["x"][om.l2u]) <= TOLPCG
+        exact = np.sin(np.pi * xyz[:, 0]) * np.sin(np.pi * xyz[:, 1]) * np.sin(np.pi * xyz[:, 2])
+        assert np.max(np.abs(x.cpu().numpy() - exact)) <= 1e-4           # discretisation error at N = 5, 4^3 elements
+        # nonzero initial guess: same solution, x0 masked on entry
+        x0 = torch_cuda.ones_like(b)
+        it2, _ = sem.pcg(b, x0, 1e-10, 500)
+        assert relerr(x0.cpu().numpy(), ores["x"][om.l2u]) <= 1e-7
+        # b = 0 -> 0 iterations, x = M x0
+        z = torch_cuda.zeros_like(b)
+        x1 = torch_cuda.ones_like(b)
+        it3, rel3 = sem.pcg(z, x1, 1e-8, 10)
+        assert it3 == 0 and rel3 == 0.0
+        assert float(x1.sum()) == float((mask_u[om.l2u] == 0).sum())
+
+
+def test_pcg_helmholtz(torch_cuda, binding, oracle_mod):
+    m = inputs.box_mesh(3, 3, 3, 4, "smooth")
+    om, oG, mask_u = _pcg_setup(oracle_mod, m)
+    mask_u[:] = 0                                                            # Helmholtz is SPD without Dirichlet
+    rng = np.random.default_rng(0)
+    b_u = rng.standard_normal(om.U)
+    lam = 10.0
+    ores = oracle_mod.pcg(oG, m.N, om, mask_u, b_u, tol=1e-9, maxit=300, lam=lam)
+    with binding.Sem(m.E, m.N, m.vert, m.gid) as sem:
+        sem.geom(with_mass=True)
+        sem.set_lambda(lam)
+        b = to_dev(torch_cuda, b_u[om.l2u])
+        x = torch_cuda.zeros_like(b)
+        it, rel = sem.pcg(b, x, 1e-9, 300)
+        assert it == ores["iters"]
+        assert relerr(x.cpu().numpy(), ores["x"][om.l2u]) <= TOLPCG
