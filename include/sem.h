@@ -96,7 +96,8 @@ SEM_API int sem_ax_gs(sem_ctx* ctx, const void* u, void* w, sem_prec prec, doubl
  * with dots over unique unmasked nodes.  b (assembled right-hand side) and x are DEVICE, local layout, continuous.
  *   iters_out   HOST  number of operator applications in the loop
  *   relres_out  HOST  ||r|| / r0 from the recurrence
- * Reaching maxit is not an error; b == 0 returns x = M x0, 0 iterations; p.q <= 0 stops (breakdown) with SEM_OK. */
+ * Reaching maxit is not an error; r0 == 0 (e.g. b == 0 with x0 == 0) returns x = M x0 after 0 iterations;
+ * p.q <= 0 stops (breakdown) with SEM_OK. */
 SEM_API int sem_pcg(sem_ctx* ctx, const double* b, double* x, double tol, int maxit, int* iters_out, double* relres_out);
 
 /* Helmholtz shift used by sem_pcg and by the Jacobi diagonal (default 0).  Requires with_mass if != 0. */

@@ -373,12 +373,15 @@ def test_pcg_converges_same_iteration_count(torch_cuda, binding, oracle_mod):
         x0 = torch_cuda.ones_like(b)
         it2, _ = sem.pcg(b, x0, 1e-10, 500)
         assert relerr(x0.cpu().numpy(), ores["x"][om.l2u]) <= 1e-7
-        # b = 0 -> 0 iterations, x = M x0
+        # r0 = 0 (b = 0, x0 = 0) -> 0 iterations, x untouched (S13)
         z = torch_cuda.zeros_like(b)
-        x1 = torch_cuda.ones_like(b)
+        x1 = torch_cuda.zeros_like(b)
         it3, rel3 = sem.pcg(z, x1, 1e-8, 10)
-        assert it3 == 0 and rel3 == 0.0
-        assert float(x1.sum()) == float((mask_u[om.l2u] == 0).sum())
+        assert it3 == 0 and rel3 == 0.0 and float(x1.abs().max()) == 0.0
+        # maxit = 0: only the entry masking of x0 happens
+        x2 = torch_cuda.ones_like(b)
+        it4, _ = sem.pcg(b, x2, 1e-8, 0)
+        assert it4 == 0 and float(x2.sum()) == float((mask_u[om.l2u] == 0).sum())
 
 
 def test_pcg_helmholtz(torch_cuda, binding, oracle_mod):
