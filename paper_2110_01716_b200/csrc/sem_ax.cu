@@ -106,6 +106,15 @@ struct DRows {
             DTi[l] = dp.D[l * P + i];
             DTj[l] = dp.D[l * P + j];
         }
+        // pin the rows in registers: without this the compiler re-reads them with indexed constant loads (LDC
+        // c[0x0][R+..]) inside the slab loop, and the indexed-constant cache becomes the busiest unit of the SM
+#pragma unroll
+        for (int l = 0; l < P; ++l) {
+            if constexpr (sizeof(T) == 8)
+                asm volatile("" : "+d"(Di[l]), "+d"(Dj[l]), "+d"(DTi[l]), "+d"(DTj[l]));
+            else
+                asm volatile("" : "+f"(Di[l]), "+f"(Dj[l]), "+f"(DTi[l]), "+f"(DTj[l]));
+        }
     }
 };
 
@@ -277,7 +286,7 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
     using SM = StreamSmem<T, P, NS>;
     constexpr int EPB = SM::EPB, P2 = SM::P2, P3 = SM::P3, SLAB = SM::SLAB;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    SM& sm = *reinterpret_cast<SM*>(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
+    SM& sm = *reinterpret_cast<SM*>(smem_raw);      // dynamic smem starts 128-byte aligned (static part is 256 B)
     if (skip_flag && *skip_flag) return;
     const int tid = threadIdx.x;
     const bool lane_ok = tid < EPB * P2;
@@ -453,8 +462,12 @@ int dispatch_p(sem_ctx* c, const void* u, void* w, double lambda, const int* ski
     const T* uu = (const T*)u;
     T* ww = (T*)w;
     if (c->gmode == SEM_G_RECOMPUTE) return launch_simple<T, P, true>(c, uu, ww, (T)lambda, skip, dot);
+    if constexpr (P == 8 && sizeof(T) == 8) {     // experiment knobs: other ring depths / residencies
+        if (c->ax_variant == 2 && ((uintptr_t)u % 16) == 0) return launch_stream<T, P, 7, 7>(c, uu, ww, (T)lambda, skip, dot);
+        if (c->ax_variant == 3 && ((uintptr_t)u % 16) == 0) return launch_stream<T, P, 10, 6>(c, uu, ww, (T)lambda, skip, dot);
+    }
     if constexpr (P % 2 == 0 && P <= 12) {
-        if (c->ax_variant == 0 && ((uintptr_t)u % 16) == 0)
+        if (c->ax_variant != 1 && ((uintptr_t)u % 16) == 0)
             return launch_stream<T, P, StreamCfg<T, P>::NS, StreamCfg<T, P>::MINB>(c, uu, ww, (T)lambda, skip, dot);
     }
     return launch_simple<T, P, false>(c, uu, ww, (T)lambda, skip, dot);
