@@ -38,6 +38,8 @@ int sem_mesh_setup(sem_ctx** out, int64_t E, int N, const double* vertex_xyz, co
     if (!c) return SEM_ENOMEM;
     *out = c;
     c->E = E; c->N = N; c->p = (int)p; c->p3 = p * p * p; c->nL = nL;
+    c->epb = sem_epb((int)p);
+    c->ngroups = (E + c->epb - 1) / c->epb;
     c->stream = (cudaStream_t)cuda_stream;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
@@ -47,7 +49,9 @@ int sem_mesh_setup(sem_ctx** out, int64_t E, int N, const double* vertex_xyz, co
     sem_gll_tables(N, c->xi, c->rho, c->D);
     SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_vert, E * 24 * sizeof(double)));
     SEM_CUDA_OK(c, cudaMemcpyAsync(c->d_vert, vertex_xyz, E * 24 * sizeof(double), cudaMemcpyHostToDevice, c->stream));
-    return sem_build_maps(c, gid, dirichlet);
+    int rc = sem_build_maps(c, gid, dirichlet);
+    if (rc) return rc;
+    return sem_build_owner_lists(c);
 }
 
 int sem_geom(sem_ctx* c, const double* node_xyz, sem_gmode mode, int with_mass) {
@@ -101,8 +105,7 @@ int sem_ax_gs(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda) 
     if (rc) return rc;
     if ((rc = require_geom(c, "sem_ax_gs"))) return rc;
     if (prec == SEM_F32 && c->gmode == SEM_G_STORED && (rc = sem_build_g32(c))) return rc;
-    if ((rc = sem_launch_ax(c, u, w, prec, lambda, nullptr, nullptr))) return rc;
-    return sem_launch_gs(c, w, prec, true);
+    return sem_launch_ax_gs(c, u, w, prec, lambda, nullptr, nullptr);
 }
 
 int sem_set_lambda(sem_ctx* c, double lambda) {
@@ -188,7 +191,8 @@ void sem_ctx_destroy(sem_ctx* c) {
     cudaStreamSynchronize(c->stream);
     void* ptrs[] = {c->d_vert, c->d_l2u, c->d_mult, c->d_seg_off, c->d_seg_idx, c->d_uniq_gid, c->d_sh_off, c->d_sh_idx,
                     c->d_sh_masked, c->d_mask_u, c->d_mask1_idx, c->d_G, c->d_G32, c->d_B, c->d_B32, c->d_detJ,
-                    c->d_diag, c->d_Minv, c->d_wt, c->d_r, c->d_p, c->d_w, c->d_scal};
+                    c->d_diag, c->d_Minv, c->d_wt, c->d_r, c->d_p, c->d_w, c->d_scal, c->d_own_goff, c->d_own_dep,
+                    c->d_own_pair, c->d_own_quad, c->d_own_big, c->d_gs_flag};
     for (void* p : ptrs) cudaFree(p);
     cudaGetLastError();
     delete[] c->h_hist;

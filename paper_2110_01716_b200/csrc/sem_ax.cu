@@ -125,7 +125,7 @@ struct DRows {
 template <typename T, int P>
 __device__ __forceinline__ void slab_part1(const DParam<T, P>& dp, const DRows<T, P>& dr, const T* __restrict__ su,
                                            const T (&uk)[P], T (&wk)[P], const T (&g)[6], int k, int i, int j,
-                                           T* __restrict__ sgr, T* __restrict__ sgs) {
+                                           T& gr_out, T& gs_out) {
     T row[P];
     load_row<T, P>(su + (k * P + j) * P, row);
     const T* col = su + k * P * P + i;
@@ -136,11 +136,9 @@ __device__ __forceinline__ void slab_part1(const DParam<T, P>& dp, const DRows<T
         us += dr.Dj[l] * col[l * P];             // u_s = sum_l D[j][l] u[k][l][i]
         ut += dp.D[k * P + l] * uk[l];           // u_t = sum_l D[k][l] u[l][j][i]
     }
-    const T gr = g[0] * ur + g[1] * us + g[2] * ut;
-    const T gs = g[1] * ur + g[3] * us + g[4] * ut;
+    gr_out = g[0] * ur + g[1] * us + g[2] * ut;
+    gs_out = g[1] * ur + g[3] * us + g[4] * ut;
     const T gt = g[2] * ur + g[4] * us + g[5] * ut;
-    sgr[j * P + i] = gr;
-    sgs[j * P + i] = gs;
 #pragma unroll
     for (int l = 0; l < P; ++l) wk[l] += dp.D[k * P + l] * gt;   // w[l][j][i] += D[k][l] g_t[k][j][i]
 }
@@ -150,13 +148,13 @@ __device__ __forceinline__ T slab_part2(const DRows<T, P>& dr, int i, int j, con
                                         const T* __restrict__ sgs) {
     T row[P];
     load_row<T, P>(sgr + j * P, row);
-    T acc = T(0);
+    T ar = T(0), as = T(0);                      // two independent chains
 #pragma unroll
     for (int l = 0; l < P; ++l) {
-        acc += dr.DTi[l] * row[l];               // sum_l D[l][i] g_r[k][j][l]
-        acc += dr.DTj[l] * sgs[l * P + i];       // sum_l D[l][j] g_s[k][l][i]
+        ar += dr.DTi[l] * row[l];                // sum_l D[l][i] g_r[k][j][l]
+        as += dr.DTj[l] * sgs[l * P + i];        // sum_l D[l][j] g_s[k][l][i]
     }
-    return acc;
+    return ar + as;
 }
 
 template <typename T>
@@ -240,10 +238,15 @@ __global__ void __launch_bounds__(threads_of<P>()) ax_simple(int64_t E, DParam<T
                 sem_factors<T>(J, (T)(gll.rho[i] * gll.rho[j] * gll.rho[k]), g, B);
             } else {
 #pragma unroll
-                for (int c = 0; c < 6; ++c) g[c] = active ? Gs[(e * P + k) * slab + c * P2 + ij] : T(0);
+                for (int c = 0; c < 6; ++c) g[c] = active ? Gs[sem_g_off(e, k, P, EPB, slab) + c * P2 + ij] : T(0);
             }
             const int buf = k & 1;
-            if (lane_ok) slab_part1<T, P>(dp, dr, sue, uk, wk, g, k, i, j, sgr[buf] + slot * P2, sgs[buf] + slot * P2);
+            if (lane_ok) {
+                T gr, gs;
+                slab_part1<T, P>(dp, dr, sue, uk, wk, g, k, i, j, gr, gs);
+                sgr[buf][slot * P2 + ij] = gr;
+                sgs[buf][slot * P2 + ij] = gs;
+            }
             __syncthreads();
             if (lane_ok) wk[k] += slab_part2<T, P>(dr, i, j, sgr[buf] + slot * P2, sgs[buf] + slot * P2);
         }
@@ -264,7 +267,97 @@ __global__ void __launch_bounds__(threads_of<P>()) ax_simple(int64_t E, DParam<T
 // ---------------------------------------------------------------------------------------------------------------
 // ax_stream: persistent CTAs, G slabs and u elements arrive by bulk async copies into shared-memory rings.
 // Requires even P (so every chunk is a multiple of 16 bytes) and 16-byte aligned u.
+//
+// FUSE = true adds the gather-scatter and the Dirichlet mask (a6, a7) as an owner-computes epilogue: after a group's
+// local result is stored and published (release store of the application's epoch into flag[group]), the CTA sums
+// every shared node whose LAST copy lives in this group -- waiting (acquire) for the lower groups that hold the
+// other copies -- in ascending local index (O5) and writes the sum to all copies.  A group only ever waits for
+// lower-numbered groups and groups are handed out round-robin in ascending order to co-resident CTAs (cooperative
+// launch), so the lowest unfinished group never waits: no deadlock.  Every location is written by its own group
+// before the flag and by the owner after it, never concurrently.
 // ---------------------------------------------------------------------------------------------------------------
+struct FuseArgs {
+    const int4* goff;        // [ngroups+1] (dep, pair, quad, big) list offsets
+    const int32_t* dep;
+    const int2* pair;
+    const int4* quad;
+    const int2* big;
+    const int32_t* sh_idx;
+    uint32_t* flag;          // [ngroups]
+    uint32_t epoch;
+};
+
+__device__ __forceinline__ void st_release_u32(uint32_t* p, uint32_t v) {
+    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t* p) {
+    uint32_t v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+// L2-coherent load of another CTA's (or this CTA's) local result
+__device__ __forceinline__ double ld_l2(const double* p) {
+    double v;
+    asm volatile("ld.relaxed.gpu.global.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ float ld_l2(const float* p) {
+    float v;
+    asm volatile("ld.relaxed.gpu.global.f32 %0, [%1];" : "=f"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// a6 + a7 for the nodes owned by group grp.  All threads of the CTA call it after the group's w has been stored.
+template <typename T, int NT>
+__device__ __forceinline__ void gs_owned(const FuseArgs& f, int64_t grp, T* __restrict__ w) {
+    constexpr int32_t IDX = 0x7fffffff;
+    const int tid = threadIdx.x;
+    __syncthreads();                                  // every thread's stores of this group precede the release
+    const int4 o0 = f.goff[grp], o1 = f.goff[grp + 1];
+    if (tid == 0) {
+        __threadfence();
+        st_release_u32(f.flag + grp, f.epoch);
+    }
+    for (int32_t d = o0.x + tid; d < o1.x; d += NT) {
+        const uint32_t* fl = f.flag + f.dep[d];
+        while (ld_acquire_u32(fl) != f.epoch) { }
+    }
+    __syncthreads();
+    // pairs, two per thread in flight
+    for (int32_t q = o0.y + tid; q < o1.y; q += 2 * NT) {
+        const bool two = q + NT < o1.y;
+        const int2 a = f.pair[q];
+        const int2 b = two ? f.pair[q + NT] : make_int2(0, -1);
+        const int32_t a0 = a.x & IDX, b0 = b.x & IDX;
+        T sa = T(0), sb = T(0);
+        if (a.x >= 0 && a.y >= 0) { const T v0 = ld_l2(w + a0), v1 = ld_l2(w + a.y); sa = v0 + v1; }
+        if (two && b.x >= 0 && b.y >= 0) { const T v0 = ld_l2(w + b0), v1 = ld_l2(w + b.y); sb = v0 + v1; }
+        w[a0] = sa;
+        if (a.y >= 0) w[a.y] = sa;
+        if (two) { w[b0] = sb; if (b.y >= 0) w[b.y] = sb; }
+    }
+    for (int32_t q = o0.z + tid; q < o1.z; q += NT) {
+        const int4 a = f.quad[q];
+        const int32_t a0 = a.x & IDX;
+        T s = T(0);
+        if (a.x >= 0) {
+            const T v0 = ld_l2(w + a0), v1 = ld_l2(w + a.y), v2 = ld_l2(w + a.z);
+            s = (v0 + v1) + v2;
+            if (a.w >= 0) s += ld_l2(w + a.w);
+        }
+        w[a0] = s; w[a.y] = s; w[a.z] = s;
+        if (a.w >= 0) w[a.w] = s;
+    }
+    for (int32_t q = o0.w + tid; q < o1.w; q += NT) {
+        const int2 a = f.big[q];
+        const int32_t cnt = a.y & IDX;
+        T s = T(0);
+        if (a.y >= 0)
+            for (int32_t r = 0; r < cnt; ++r) s += ld_l2(w + f.sh_idx[a.x + r]);
+        for (int32_t r = 0; r < cnt; ++r) w[f.sh_idx[a.x + r]] = s;
+    }
+}
+
 template <typename T, int P, int NS>
 struct StreamSmem {
     static constexpr int EPB = epb_of<P>(), P2 = P * P, P3 = P2 * P;
@@ -277,53 +370,41 @@ struct StreamSmem {
     alignas(8) uint64_t ufull[2];
 };
 
-template <typename T, int P, int NS, int MINB>
+template <typename T, int P, int NS, int MINB, bool FUSE>
 __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DParam<T, P> dp,
                                                                    const T* __restrict__ Gs, const T* __restrict__ Bm,
                                                                    T lambda, const T* __restrict__ u,
                                                                    T* __restrict__ w, const int* __restrict__ skip_flag,
-                                                                   double* __restrict__ dot_out) {
+                                                                   double* __restrict__ dot_out, FuseArgs fuse) {
     using SM = StreamSmem<T, P, NS>;
-    constexpr int EPB = SM::EPB, P2 = SM::P2, P3 = SM::P3, SLAB = SM::SLAB;
+    constexpr int EPB = SM::EPB, P2 = SM::P2, P3 = SM::P3, SLAB = SM::SLAB, NT = threads_of<P>();
+    constexpr bool FULL = EPB * P2 == NT;           // every thread owns a column
+    constexpr uint32_t GBYTES = EPB * SLAB * sizeof(T);
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    SM& sm = *reinterpret_cast<SM*>(smem_raw);      // dynamic smem starts 128-byte aligned (static part is 256 B)
+    SM& sm = *reinterpret_cast<SM*>(smem_raw);
     if (skip_flag && *skip_flag) return;
     const int tid = threadIdx.x;
-    const bool lane_ok = tid < EPB * P2;
+    const bool lane_ok = FULL || tid < EPB * P2;
     const int slot = lane_ok ? tid / P2 : 0;
     const int ij = lane_ok ? tid % P2 : 0;
     const int j = ij / P, i = ij % P;
 
     const int64_t ngroups = (E + EPB - 1) / EPB;
-    // groups of this CTA: blockIdx.x, blockIdx.x + gridDim.x, ...
     const int64_t nmine = blockIdx.x < ngroups ? (ngroups - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    const int tail_n = (int)(E - (ngroups - 1) * EPB);          // elements of the globally last group
+
+    // ---- producer (thread 0): slabs are issued in consumption order, NS ahead; G is padded to whole groups ----
+    const T* gsrc = Gs + (int64_t)blockIdx.x * (P * EPB * SLAB);
+    const int64_t gjump = (int64_t)(gridDim.x - 1) * (P * EPB * SLAB);
+    int64_t gleft = nmine * P;
     uint64_t pol_g = 0, pol_u = 0;
-
-    auto nact_of = [&](int64_t n) -> int {          // active elements in my n-th group
-        const int64_t e0 = (blockIdx.x + n * gridDim.x) * EPB;
-        const int64_t left = E - e0;
-        return left >= EPB ? EPB : (int)left;
-    };
-    // producer state (thread 0 only): the next slab to issue is slab pk of my pn-th group; slabs are issued in order
-    int64_t pn = 0;
-    int pk = 0;
-    auto issue_next_slab = [&](int q) {
-        const int64_t e0 = (blockIdx.x + pn * gridDim.x) * EPB;
-        const int na = nact_of(pn);
-        mbar_expect_tx(&sm.gfull[q], (uint32_t)(na * SLAB * sizeof(T)));
-#pragma unroll 1
-        for (int s = 0; s < na; ++s)
-            bulk_g2s(&sm.g[q][s * SLAB], Gs + ((e0 + s) * P + pk) * SLAB, SLAB * sizeof(T), &sm.gfull[q], pol_g);
-        if (++pk == P) { pk = 0; ++pn; }
-    };
-    auto issue_u = [&](int64_t n) {                 // thread 0 only
+    auto issue_u = [&](int64_t n) {
+        const int64_t grp = blockIdx.x + n * gridDim.x;
+        const uint32_t bytes = (uint32_t)((grp == ngroups - 1 ? tail_n : EPB) * P3 * sizeof(T));
         const int b = (int)(n & 1);
-        const int64_t e0 = (blockIdx.x + n * gridDim.x) * EPB;
-        const uint32_t bytes = (uint32_t)(nact_of(n) * P3 * sizeof(T));
         mbar_expect_tx(&sm.ufull[b], bytes);
-        bulk_g2s(&sm.u[b][0], u + e0 * P3, bytes, &sm.ufull[b], pol_u);
+        bulk_g2s(&sm.u[b][0], u + grp * (EPB * P3), bytes, &sm.ufull[b], pol_u);
     };
-
     if (tid == 0) {
 #pragma unroll
         for (int q = 0; q < NS; ++q) mbar_init(&sm.gfull[q], 1);
@@ -336,7 +417,14 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
         pol_g = policy_evict_first();
         pol_u = policy_evict_last();
         issue_u(0);
-        for (int q = 0; q < NS && pn < nmine; ++q) issue_next_slab(q);
+        int gk = 0;
+        for (int q = 0; q < NS && gleft > 0; ++q) {
+            mbar_expect_tx(&sm.gfull[q], GBYTES);
+            bulk_g2s(&sm.g[q][0], gsrc, GBYTES, &sm.gfull[q], pol_g);
+            gsrc += EPB * SLAB;
+            if (++gk == P) { gk = 0; gsrc += gjump; }
+            --gleft;
+        }
         if (nmine > 1) issue_u(1);
     }
     DRows<T, P> dr;
@@ -345,41 +433,52 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
 
     int q = 0;                 // ring stage of the slab being consumed
     uint32_t gphase = 0;       // its mbarrier parity
-    for (int64_t n = 0; n < nmine; ++n) {
-        const int64_t e = (blockIdx.x + n * gridDim.x) * EPB + slot;
-        const bool active = lane_ok && e < E;
+    T* wdst = w + ((int64_t)blockIdx.x * EPB + slot) * P3 + ij;
+    const int64_t wstep = (int64_t)gridDim.x * (EPB * P3);
+    int64_t grp = blockIdx.x;
+    for (int64_t n = 0; n < nmine; ++n, grp += gridDim.x, wdst += wstep) {
+        const bool ok = (FULL && EPB == 1) ? true : (lane_ok && grp * EPB + slot < E);
         const int ub = (int)(n & 1);
         mbar_wait(&sm.ufull[ub], (uint32_t)((n >> 1) & 1));
         const T* sue = &sm.u[ub][slot * P3];
         T uk[P], wk[P];
 #pragma unroll
-        for (int k = 0; k < P; ++k) { uk[k] = active ? sue[k * P2 + ij] : T(0); wk[k] = T(0); }
+        for (int k = 0; k < P; ++k) { uk[k] = sue[k * P2 + ij]; wk[k] = T(0); }
 #pragma unroll
         for (int k = 0; k < P; ++k) {
             mbar_wait(&sm.gfull[q], gphase);
             T g[6];
 #pragma unroll
-            for (int c = 0; c < 6; ++c) g[c] = active ? sm.g[q][slot * SLAB + c * P2 + ij] : T(0);
+            for (int c = 0; c < 6; ++c) g[c] = sm.g[q][slot * SLAB + c * P2 + ij];
             const int buf = k & 1;
-            if (active) slab_part1<T, P>(dp, dr, sue, uk, wk, g, k, i, j, &sm.sgr[buf][slot * P2], &sm.sgs[buf][slot * P2]);
+            T gr, gs;
+            slab_part1<T, P>(dp, dr, sue, uk, wk, g, k, i, j, gr, gs);
+            if (FULL || lane_ok) { sm.sgr[buf][slot * P2 + ij] = gr; sm.sgs[buf][slot * P2 + ij] = gs; }
             __syncthreads();
-            // every thread has consumed stage q (and, on the last slab, this element's u buffer): refill
+            // every thread has consumed stage q (and, on the last slab, this group's u buffer): refill
             if (tid == 0) {
-                if (pn < nmine) issue_next_slab(q);
+                if (gleft > 0) {
+                    mbar_expect_tx(&sm.gfull[q], GBYTES);
+                    bulk_g2s(&sm.g[q][0], gsrc, GBYTES, &sm.gfull[q], pol_g);
+                    gsrc += EPB * SLAB;
+                    if ((k + NS) % P == P - 1) gsrc += gjump;     // that was the last slab of its group
+                    --gleft;
+                }
                 if (k == P - 1 && n + 2 < nmine) issue_u(n + 2);
             }
-            if (active) wk[k] += slab_part2<T, P>(dr, i, j, &sm.sgr[buf][slot * P2], &sm.sgs[buf][slot * P2]);
+            wk[k] += slab_part2<T, P>(dr, i, j, &sm.sgr[buf][slot * P2], &sm.sgs[buf][slot * P2]);
             if (++q == NS) { q = 0; gphase ^= 1u; }
         }
-        if (active) {
+        if (ok) {
 #pragma unroll
             for (int k = 0; k < P; ++k) {
                 T v = wk[k];
-                if (Bm) v += lambda * Bm[e * P3 + k * P2 + ij] * uk[k];
-                w[e * P3 + k * P2 + ij] = v;
+                if (Bm) v += lambda * Bm[(wdst - w) + k * P2] * uk[k];
+                wdst[k * P2] = v;
                 partial += uk[k] * v;
             }
         }
+        if constexpr (FUSE) gs_owned<T, NT>(fuse, grp, w);
     }
     if (dot_out) block_dot_flush(partial, dot_out);
 }
@@ -417,7 +516,7 @@ int launch_simple(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, doubl
     return SEM_OK;
 }
 
-template <typename T, int P, int NS, int MINB>
+template <typename T, int P, int NS, int MINB, bool FUSE>
 int launch_stream(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, double* dot) {
     using SM = StreamSmem<T, P, NS>;
     constexpr int EPB = epb_of<P>();
@@ -426,22 +525,37 @@ int launch_stream(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, doubl
     const T* Bm = sizeof(T) == 8 ? (const T*)c->d_B : (const T*)c->d_B32;
     const DParam<T, P> dp = make_dparam<T, P>(c);
     const size_t smem = sizeof(SM) + 128;
-    auto go = [&](auto kern) -> int {
-        static thread_local int cached_dev = -1;
-        static thread_local int blocks_per_sm = 0;
-        if (cached_dev != c->device) {
-            SEM_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            SEM_CUDA_OK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, threads_of<P>(), smem));
-            if (blocks_per_sm < 1) return sem_fail(c, SEM_ECUDA, "ax_stream does not fit on an SM");
-            cached_dev = c->device;
-        }
-        const int64_t cap = (int64_t)c->num_sms * blocks_per_sm;
-        const unsigned grid = (unsigned)(ngroups < cap ? ngroups : cap);
-        kern<<<grid, threads_of<P>(), smem, c->stream>>>(c->E, dp, Gs, lambda != T(0) ? Bm : nullptr, lambda, u, w, skip, dot);
-        SEM_CUDA_OK(c, cudaGetLastError());
-        return SEM_OK;
-    };
-    return go(ax_stream<T, P, NS, MINB>);
+    auto kern = ax_stream<T, P, NS, MINB, FUSE>;
+    static thread_local int cached_dev = -1;
+    static thread_local int blocks_per_sm = 0;
+    if (cached_dev != c->device) {
+        SEM_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        SEM_CUDA_OK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, threads_of<P>(), smem));
+        if (blocks_per_sm < 1) return sem_fail(c, SEM_ECUDA, "ax_stream does not fit on an SM");
+        cached_dev = c->device;
+    }
+    const int64_t cap = (int64_t)c->num_sms * blocks_per_sm;
+    const unsigned grid = (unsigned)(ngroups < cap ? ngroups : cap);
+    FuseArgs fa = {};
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(threads_of<P>());
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = c->stream;
+    cudaLaunchAttribute attr[1];
+    if (FUSE) {
+        // the owner-computes epilogue waits on other CTAs: all CTAs must be co-resident (cooperative launch)
+        fa.goff = c->d_own_goff; fa.dep = c->d_own_dep; fa.pair = c->d_own_pair; fa.quad = c->d_own_quad;
+        fa.big = c->d_own_big; fa.sh_idx = c->d_sh_idx; fa.flag = c->d_gs_flag;
+        fa.epoch = ++c->gs_epoch;
+        attr[0].id = cudaLaunchAttributeCooperative;
+        attr[0].val.cooperative = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+    }
+    SEM_CUDA_OK(c, cudaLaunchKernelEx(&cfg, kern, c->E, dp, Gs, lambda != T(0) ? Bm : (const T*)nullptr, lambda, u, w,
+                                      skip, dot, fa));
+    return SEM_OK;
 }
 
 // stage depth / residency per (T, P): sized so that ~7-8 CTAs fit in 227 KB and > 64 KB are in flight per SM
@@ -457,26 +571,34 @@ template <> struct StreamCfg<float, 6> { static constexpr int NS = 6, MINB = 6; 
 template <> struct StreamCfg<double, 10> { static constexpr int NS = 4, MINB = 4; };
 template <> struct StreamCfg<float, 10> { static constexpr int NS = 6, MINB = 4; };
 
-template <typename T, int P>
+template <int P> constexpr bool stream_ok() { return P % 2 == 0 && P <= 12; }
+
+// FUSE: the caller wants a3-a7; returns 1 if this (T, P, variant, alignment) has no fused kernel (caller falls back)
+template <typename T, int P, bool FUSE>
 int dispatch_p(sem_ctx* c, const void* u, void* w, double lambda, const int* skip, double* dot) {
     const T* uu = (const T*)u;
     T* ww = (T*)w;
-    if (c->gmode == SEM_G_RECOMPUTE) return launch_simple<T, P, true>(c, uu, ww, (T)lambda, skip, dot);
-    if constexpr (P == 8 && sizeof(T) == 8) {     // experiment knobs: other ring depths / residencies
-        if (c->ax_variant == 2 && ((uintptr_t)u % 16) == 0) return launch_stream<T, P, 7, 7>(c, uu, ww, (T)lambda, skip, dot);
-        if (c->ax_variant == 3 && ((uintptr_t)u % 16) == 0) return launch_stream<T, P, 10, 6>(c, uu, ww, (T)lambda, skip, dot);
+    const bool aligned = ((uintptr_t)u % 16) == 0;
+    if constexpr (FUSE) {
+        if constexpr (stream_ok<P>()) {
+            if (c->gmode == SEM_G_STORED && c->ax_variant == 5 && aligned)
+                return launch_stream<T, P, StreamCfg<T, P>::NS, StreamCfg<T, P>::MINB, true>(c, uu, ww, (T)lambda, skip, dot);
+        }
+        return 1;
+    } else {
+        if (c->gmode == SEM_G_RECOMPUTE) return launch_simple<T, P, true>(c, uu, ww, (T)lambda, skip, dot);
+        if constexpr (stream_ok<P>()) {
+            if (c->ax_variant != 1 && aligned)
+                return launch_stream<T, P, StreamCfg<T, P>::NS, StreamCfg<T, P>::MINB, false>(c, uu, ww, (T)lambda, skip, dot);
+        }
+        return launch_simple<T, P, false>(c, uu, ww, (T)lambda, skip, dot);
     }
-    if constexpr (P % 2 == 0 && P <= 12) {
-        if (c->ax_variant != 1 && ((uintptr_t)u % 16) == 0)
-            return launch_stream<T, P, StreamCfg<T, P>::NS, StreamCfg<T, P>::MINB>(c, uu, ww, (T)lambda, skip, dot);
-    }
-    return launch_simple<T, P, false>(c, uu, ww, (T)lambda, skip, dot);
 }
 
-template <typename T>
+template <typename T, bool FUSE>
 int dispatch(sem_ctx* c, const void* u, void* w, double lambda, const int* skip, double* dot) {
     switch (c->p) {
-#define SEM_CASE(PP) case PP: return dispatch_p<T, PP>(c, u, w, lambda, skip, dot);
+#define SEM_CASE(PP) case PP: return dispatch_p<T, PP, FUSE>(c, u, w, lambda, skip, dot);
         SEM_CASE(2) SEM_CASE(3) SEM_CASE(4) SEM_CASE(5) SEM_CASE(6) SEM_CASE(7) SEM_CASE(8) SEM_CASE(9)
         SEM_CASE(10) SEM_CASE(11) SEM_CASE(12) SEM_CASE(13) SEM_CASE(14) SEM_CASE(15) SEM_CASE(16)
 #undef SEM_CASE
@@ -490,6 +612,17 @@ int dispatch(sem_ctx* c, const void* u, void* w, double lambda, const int* skip,
 // skip_flag != nullptr: the kernel returns at once if *skip_flag != 0 (device; used by the PCG loop after convergence).
 int sem_launch_ax(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda, double* dot_out,
                   const int* skip_flag) {
-    if (prec == SEM_F64) return dispatch<double>(c, u, w, lambda, skip_flag, dot_out);
-    return dispatch<float>(c, u, w, lambda, skip_flag, dot_out);
+    if (prec == SEM_F64) return dispatch<double, false>(c, u, w, lambda, skip_flag, dot_out);
+    return dispatch<float, false>(c, u, w, lambda, skip_flag, dot_out);
+}
+
+// a3-a7: one kernel (Ax with the owner-computes gather-scatter + mask epilogue) where it applies; otherwise the
+// local operator followed by the stand-alone gather-scatter kernel.  Same results bit for bit (same summation order).
+int sem_launch_ax_gs(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda, double* dot_out,
+                     const int* skip_flag) {
+    int rc = prec == SEM_F64 ? dispatch<double, true>(c, u, w, lambda, skip_flag, dot_out)
+                             : dispatch<float, true>(c, u, w, lambda, skip_flag, dot_out);
+    if (rc != 1) return rc;
+    if ((rc = sem_launch_ax(c, u, w, prec, lambda, dot_out, skip_flag))) return rc;
+    return sem_launch_gs(c, w, prec, true);
 }

@@ -1,8 +1,9 @@
 // sem_geom.cu — a2 (setup): geometric factors, the exact Jacobi diagonal, and the layout conversions around them.
 // P:69 (isoparametric map), O3 (G, B, detJ), O7 (exact diagonal incl. cross terms), S16 (FP32 copy rounded once).
 //
-// Device layout of G ("slab layout", library-owned): Gs[e][k][c][j*p+i], c = rr,rs,rt,ss,st,tt, so that the six
-// factors of one k-slab of one element are one contiguous chunk (one bulk copy in the Ax kernel).
+// Device layout of G ("slab layout", library-owned): Gs[grp][k][slot][c][j*p+i], grp = e / epb, slot = e % epb,
+// c = rr,rs,rt,ss,st,tt (sem_g_off in sem_internal.h), so that the six factors of one k-slab of one element group
+// are one contiguous chunk (one bulk copy in the Ax kernel).  The array is padded with zeros to whole groups.
 #include "sem_geom_dev.cuh"
 #include "sem_internal.h"
 
@@ -11,8 +12,8 @@ namespace {
 inline unsigned nblk(int64_t n, int t = 256) { return (unsigned)((n + t - 1) / t); }
 
 // One thread per node.  xyz == nullptr: analytic trilinear Jacobian (S5); else D applied to xyz (isoparametric).
-__global__ void k_geom(int64_t E, int p, Gll1D gll, const double* __restrict__ vert, const double* __restrict__ xyz,
-                       int64_t slab, double* __restrict__ Gs, double* __restrict__ Bm, double* __restrict__ detJ,
+__global__ void k_geom(int64_t E, int p, int epb, Gll1D gll, const double* __restrict__ vert,
+                       const double* __restrict__ xyz, int64_t slab, double* __restrict__ Gs, double* __restrict__ Bm, double* __restrict__ detJ,
                        int* __restrict__ bad) {
     const int64_t p2 = (int64_t)p * p, p3 = p2 * p;
     const int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
@@ -44,7 +45,7 @@ __global__ void k_geom(int64_t E, int p, Gll1D gll, const double* __restrict__ v
     double g[6], B;
     const double det = sem_factors(J, gll.rho[i] * gll.rho[j] * gll.rho[k], g, B);
     if (!(det > 0.0)) atomicOr(bad, 1);
-    double* slab_ptr = Gs + (e * p + k) * slab + (j * p + i);
+    double* slab_ptr = Gs + sem_g_off(e, k, p, epb, slab) + (j * p + i);
 #pragma unroll
     for (int c = 0; c < 6; ++c) slab_ptr[c * p2] = g[c];
     if (Bm) Bm[l] = B;
@@ -72,7 +73,7 @@ __global__ void k_g32(int64_t nslabs, int cnt, int64_t slab_in, int64_t slab_out
 }
 
 // O7: exact local diagonal.  One thread per node.
-__global__ void k_diag_local(int64_t E, int p, Gll1D gll, int64_t slab, const double* __restrict__ Gs,
+__global__ void k_diag_local(int64_t E, int p, int epb, Gll1D gll, int64_t slab, const double* __restrict__ Gs,
                              const double* __restrict__ Bm, double lambda, double* __restrict__ diag) {
     const int64_t p2 = (int64_t)p * p, p3 = p2 * p;
     const int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
@@ -80,8 +81,7 @@ __global__ void k_diag_local(int64_t E, int p, Gll1D gll, int64_t slab, const do
     const int64_t e = l / p3;
     const int n = (int)(l - e * p3);
     const int k = n / (int)p2, j = (n / p) % p, i = n % p;
-    const double* Ge = Gs + e * p * slab;
-    auto G = [&](int c, int kk, int jj, int ii) { return Ge[kk * slab + c * p2 + jj * p + ii]; };
+    auto G = [&](int c, int kk, int jj, int ii) { return Gs[sem_g_off(e, kk, p, epb, slab) + c * p2 + jj * p + ii]; };
     double d = 0.0;
     for (int m = 0; m < p; ++m) {
         const double di = gll.D[m * p + i], dj = gll.D[m * p + j], dk = gll.D[m * p + k];
@@ -108,7 +108,7 @@ __global__ void k_minv_wt(int64_t n, const double* __restrict__ diag, const int3
 }
 
 // slab layout -> [E][ncomp][p^3] export (+ B as 7th)
-__global__ void k_export(int64_t E, int p, int ncomp, int64_t slab, const double* __restrict__ Gs,
+__global__ void k_export(int64_t E, int p, int epb, int ncomp, int64_t slab, const double* __restrict__ Gs,
                          const double* __restrict__ Bm, double* __restrict__ out) {
     const int64_t p2 = (int64_t)p * p, p3 = p2 * p;
     const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
@@ -118,7 +118,7 @@ __global__ void k_export(int64_t E, int p, int ncomp, int64_t slab, const double
     const int c = (int)(r / p3);
     const int n = (int)(r - c * p3);
     const int k = n / (int)p2, ji = n % (int)p2;
-    out[t] = c < 6 ? Gs[(e * p + k) * slab + c * p2 + ji] : Bm[e * p3 + n];
+    out[t] = c < 6 ? Gs[sem_g_off(e, k, p, epb, slab) + c * p2 + ji] : Bm[e * p3 + n];
 }
 
 Gll1D make_gll(const sem_ctx* c) {
@@ -136,10 +136,11 @@ int sem_build_geom(sem_ctx* c, const double* node_xyz_host) {
     const int64_t p2 = (int64_t)p * p;
     c->slab_f64 = 6 * p2;                                   // 48 p^2 bytes: always a multiple of 16
     c->slab_f32 = 6 * p2 + ((6 * p2 * 4) % 16 ? 2 : 0);     // pad odd p to a multiple of 16 bytes
-    const int64_t gcount = c->E * p * c->slab_f64;
+    const int64_t gcount = c->ngroups * c->epb * p * c->slab_f64;       // padded to whole groups
     cudaFree(c->d_G); cudaFree(c->d_B); cudaFree(c->d_detJ); cudaFree(c->d_G32); cudaFree(c->d_B32);
     c->d_G = nullptr; c->d_B = nullptr; c->d_detJ = nullptr; c->d_G32 = nullptr; c->d_B32 = nullptr;
     SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_G, gcount * sizeof(double)));
+    if (c->ngroups * c->epb != c->E) SEM_CUDA_OK(c, cudaMemsetAsync(c->d_G, 0, gcount * sizeof(double), st));
     SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_detJ, c->nL * sizeof(double)));
     if (c->with_mass) SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_B, c->nL * sizeof(double)));
     double* d_xyz = nullptr;
@@ -152,7 +153,7 @@ int sem_build_geom(sem_ctx* c, const double* node_xyz_host) {
     cudaError_t e = cudaMalloc((void**)&d_bad, sizeof(int));
     if (e != cudaSuccess) { cudaFree(d_xyz); return sem_fail(c, SEM_ENOMEM, "cudaMalloc: %s", cudaGetErrorString(e)); }
     cudaMemsetAsync(d_bad, 0, sizeof(int), st);
-    k_geom<<<nblk(c->nL), 256, 0, st>>>(c->E, p, make_gll(c), c->d_vert, d_xyz, c->slab_f64, c->d_G, c->d_B, c->d_detJ,
+    k_geom<<<nblk(c->nL), 256, 0, st>>>(c->E, p, c->epb, make_gll(c), c->d_vert, d_xyz, c->slab_f64, c->d_G, c->d_B, c->d_detJ,
                                          d_bad);
     int h_bad = 0;
     cudaMemcpyAsync(&h_bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, st);
@@ -168,7 +169,7 @@ int sem_build_geom(sem_ctx* c, const double* node_xyz_host) {
 int sem_build_g32(sem_ctx* c) {
     if (c->d_G32) return SEM_OK;
     cudaStream_t st = c->stream;
-    const int64_t nslabs = c->E * c->p;
+    const int64_t nslabs = c->ngroups * c->epb * c->p;
     SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_G32, nslabs * c->slab_f32 * sizeof(float)));
     if (c->slab_f32 != c->slab_f64) SEM_CUDA_OK(c, cudaMemsetAsync(c->d_G32, 0, nslabs * c->slab_f32 * sizeof(float), st));
     k_g32<<<c->num_sms * 8, 256, 0, st>>>(nslabs, 6 * c->p * c->p, c->slab_f64, c->slab_f32, c->d_G, c->d_G32);
@@ -187,7 +188,7 @@ int sem_build_diag(sem_ctx* c) {
         SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_Minv, c->nL * sizeof(double)));
         SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_wt, c->nL * sizeof(double)));
     }
-    k_diag_local<<<nblk(c->nL), 256, 0, st>>>(c->E, c->p, make_gll(c), c->slab_f64, c->d_G, c->d_B, c->lambda, c->d_diag);
+    k_diag_local<<<nblk(c->nL), 256, 0, st>>>(c->E, c->p, c->epb, make_gll(c), c->slab_f64, c->d_G, c->d_B, c->lambda, c->d_diag);
     int rc = sem_launch_gs(c, c->d_diag, SEM_F64, /*apply_mask=*/false);
     if (rc) return rc;
     k_minv_wt<<<nblk(c->nL), 256, 0, st>>>(c->nL, c->d_diag, c->d_l2u, c->d_mult, c->has_mask ? c->d_mask_u : nullptr,
@@ -204,7 +205,7 @@ int sem_geom_export(sem_ctx* c, double* G_host, double* detJ_host) {
         const int64_t cnt = c->E * ncomp * c->p3;
         double* d_out = nullptr;
         SEM_CUDA_OK(c, cudaMalloc((void**)&d_out, cnt * sizeof(double)));
-        k_export<<<nblk(cnt), 256, 0, st>>>(c->E, c->p, ncomp, c->slab_f64, c->d_G, c->d_B, d_out);
+        k_export<<<nblk(cnt), 256, 0, st>>>(c->E, c->p, c->epb, ncomp, c->slab_f64, c->d_G, c->d_B, d_out);
         cudaError_t e = cudaMemcpyAsync(G_host, d_out, cnt * sizeof(double), cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
         cudaFree(d_out);

@@ -9,6 +9,15 @@
 
 #define SEM_MAXP 16
 
+// Elements per CTA ("group") of the Ax kernels: enough elements to fill 64 threads with one (i,j) column each.
+// G is stored group-blocked so that one k-slab of one group is one contiguous chunk (one bulk copy):
+//   Gs[grp][k][slot][c][j*p+i],  grp = e / epb, slot = e % epb, c = rr,rs,rt,ss,st,tt;  padded to whole groups.
+__host__ __device__ inline int sem_epb(int p) { return p * p >= 64 ? 1 : (64 + p * p - 1) / (p * p); }
+__host__ __device__ inline int64_t sem_g_off(int64_t e, int k, int p, int epb, int64_t slab) {
+    const int64_t grp = e / epb;
+    return ((grp * p + k) * epb + (e - grp * epb)) * slab;
+}
+
 struct sem_ctx {
     // ---- discretisation (a0) ----
     int64_t E = 0;
@@ -30,6 +39,23 @@ struct sem_ctx {
     int32_t* d_sh_off = nullptr;   // [Us+1] offsets into d_sh_idx
     int32_t* d_sh_idx = nullptr;   // [S] local indices
     uint8_t* d_sh_masked = nullptr;// [Us] 1 = Dirichlet
+    // owner-computes lists for the gather-scatter fused into the Ax kernel (sem_maps.cu: sem_build_owner_lists).
+    // A shared node is owned by the element group holding its LAST (highest local index) copy.  Per group g:
+    //   deps   d_own_dep [goff[g].x .. goff[g+1].x)  lower groups holding copies of nodes owned by g
+    //   pairs  d_own_pair[goff[g].y .. goff[g+1].y)  int2 (l0 | maskbit, l1)      nodes with 2 copies; l1 = -1: only
+    //                                                                            zero w[l0] (unshared Dirichlet node)
+    //   quads  d_own_quad[goff[g].z .. goff[g+1].z)  int4 (l0 | maskbit, l1, l2, l3 or -1)   3 or 4 copies
+    //   bigs   d_own_big [goff[g].w .. goff[g+1].w)  int2 (offset into d_sh_idx, count | maskbit)  > 4 copies
+    int epb = 1;
+    int64_t ngroups = 0;
+    int4* d_own_goff = nullptr;    // [ngroups+1]
+    int32_t* d_own_dep = nullptr;
+    int2* d_own_pair = nullptr;
+    int4* d_own_quad = nullptr;
+    int2* d_own_big = nullptr;
+    uint32_t* d_gs_flag = nullptr; // [ngroups] epoch of the last application whose local w of this group is written
+    uint32_t gs_epoch = 0;
+    int64_t n_dep = 0, n_pair = 0, n_quad = 0, n_big = 0;
     // Dirichlet (S14)
     bool has_mask = false;
     uint8_t* d_mask_u = nullptr;   // [U] 1 = masked unique node
@@ -39,7 +65,7 @@ struct sem_ctx {
     bool geom_done = false;
     sem_gmode gmode = SEM_G_STORED;
     bool with_mass = false;
-    // slab layout: Gs[e][k][c][j*p+i], c = rr,rs,rt,ss,st,tt; slab stride padded to 16 B
+    // group-blocked slab layout (see sem_g_off above); slab stride (values per element slab) padded to 16 B
     double* d_G = nullptr;
     float* d_G32 = nullptr;        // built lazily at the first FP32 call
     double* d_B = nullptr;         // [E][p^3] rho rho rho detJ   (with_mass)
@@ -76,6 +102,7 @@ int sem_fail(sem_ctx* c, int code, const char* fmt, ...);
 void sem_gll_tables(int N, double* xi, double* rho, double* D);
 // sem_maps.cu
 int sem_build_maps(sem_ctx* c, const int64_t* gid_any, const uint8_t* dirichlet_host);
+int sem_build_owner_lists(sem_ctx* c);
 // sem_geom.cu
 int sem_build_geom(sem_ctx* c, const double* node_xyz_host);
 int sem_build_g32(sem_ctx* c);
@@ -84,5 +111,7 @@ int sem_geom_export(sem_ctx* c, double* G_host, double* detJ_host);
 // sem_ax.cu
 int sem_launch_ax(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda, double* dot_out,
                   const int* skip_flag);
+int sem_launch_ax_gs(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda, double* dot_out,
+                     const int* skip_flag);      // a3-a7 in one kernel where the fused path applies, else ax then gs
 // sem_gs.cu
 int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask);

@@ -103,7 +103,7 @@ __global__ void k_mask1_fill(int64_t n, const int32_t* __restrict__ flag, const 
 }
 
 struct Tmp {   // frees device scratch on every exit path
-    void* ptrs[16]; int n = 0;
+    void* ptrs[40]; int n = 0;
     template <typename T> cudaError_t alloc(T** p, size_t count) {
         cudaError_t e = cudaMalloc((void**)p, (count ? count : 1) * sizeof(T));
         if (e == cudaSuccess) ptrs[n++] = *p;
@@ -236,6 +236,212 @@ int sem_build_maps(sem_ctx* c, const int64_t* gid_any, const uint8_t* dirichlet_
         SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_mask1_idx, (c->n_mask1 ? c->n_mask1 : 1) * sizeof(int32_t)));
         k_mask1_fill<<<nblk(n), 256, 0, st>>>(n, d_flag, d_ex, c->d_mask1_idx);
     }
+    SEM_CUDA_OK(c, cudaStreamSynchronize(st));
+    SEM_CUDA_OK(c, cudaGetLastError());
+    return SEM_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Owner-computes lists for the gather-scatter fused into the Ax kernel (a6/a7 inside a3-a5's kernel; sem_ax.cu).
+// A shared node belongs to the element group that holds its last (highest local index) copy; that group sums the
+// copies in ascending local index (O5: same order as the oracle) once the lower groups have published their local
+// results.  Unshared Dirichlet nodes ride along as "pairs" with no partner.  Integer work only; setup, untimed.
+// ---------------------------------------------------------------------------------------------------------------
+namespace {
+
+constexpr uint32_t OWN_MASKBIT = 0x80000000u;
+
+__device__ __forceinline__ int32_t grp_of(int32_t l, int32_t group_nodes) { return l / group_nodes; }
+
+// entry id t: t < Us a shared node, else unshared masked node t - Us.  key = owner group * 4 + class.
+__global__ void k_own_keys(int32_t Us, int32_t n_mask1, int32_t group_nodes, int32_t ng,
+                           const int32_t* __restrict__ sh_off, const int32_t* __restrict__ sh_idx,
+                           const int32_t* __restrict__ mask1_idx, uint32_t* __restrict__ keys,
+                           int32_t* __restrict__ vals, int32_t* __restrict__ Hk, int32_t* __restrict__ Hc) {
+    const int32_t t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= Us + n_mask1) return;
+    int32_t g, cls;
+    if (t < Us) {
+        const int32_t b = sh_off[t], e = sh_off[t + 1];
+        g = grp_of(sh_idx[e - 1], group_nodes);
+        cls = (e - b) <= 2 ? 0 : (e - b) <= 4 ? 1 : 2;
+    } else {
+        g = grp_of(mask1_idx[t - Us], group_nodes);
+        cls = 0;
+    }
+    keys[t] = (uint32_t)g * 4u + (uint32_t)cls;
+    vals[t] = t;
+    atomicAdd(&Hk[g * 4 + cls], 1);
+    atomicAdd(&Hc[(int64_t)cls * (ng + 1) + g], 1);
+}
+
+__global__ void k_own_fill(int32_t n_ent, int32_t Us, int32_t ng, const uint32_t* __restrict__ keys,
+                           const int32_t* __restrict__ vals, const int32_t* __restrict__ KS,
+                           const int32_t* __restrict__ offc, const int32_t* __restrict__ sh_off,
+                           const int32_t* __restrict__ sh_idx, const uint8_t* __restrict__ sh_masked,
+                           const int32_t* __restrict__ mask1_idx, int2* __restrict__ pairs, int4* __restrict__ quads,
+                           int2* __restrict__ bigs) {
+    const int32_t q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= n_ent) return;
+    const uint32_t key = keys[q];
+    const int32_t g = (int32_t)(key >> 2), cls = (int32_t)(key & 3u), id = vals[q];
+    const int32_t pos = offc[(int64_t)cls * (ng + 1) + g] + (q - KS[key]);
+    if (id >= Us) {                                   // unshared Dirichlet node: zero it
+        pairs[pos] = make_int2((int32_t)((uint32_t)mask1_idx[id - Us] | OWN_MASKBIT), -1);
+        return;
+    }
+    const int32_t b = sh_off[id], cnt = sh_off[id + 1] - b;
+    const uint32_t mbit = (sh_masked && sh_masked[id]) ? OWN_MASKBIT : 0u;
+    if (cls == 0) pairs[pos] = make_int2((int32_t)((uint32_t)sh_idx[b] | mbit), sh_idx[b + 1]);
+    else if (cls == 1)
+        quads[pos] = make_int4((int32_t)((uint32_t)sh_idx[b] | mbit), sh_idx[b + 1], sh_idx[b + 2],
+                               cnt == 4 ? sh_idx[b + 3] : -1);
+    else bigs[pos] = make_int2(b, (int32_t)((uint32_t)cnt | mbit));
+}
+
+// one key (owner group << 32 | lower group) per non-last copy that lives in another group; else the sentinel
+__global__ void k_dep_keys(int32_t Us, int32_t group_nodes, const int32_t* __restrict__ sh_off,
+                           const int32_t* __restrict__ sh_idx, unsigned long long* __restrict__ keys) {
+    const int32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= Us) return;
+    const int32_t b = sh_off[s], e = sh_off[s + 1];
+    const int32_t og = grp_of(sh_idx[e - 1], group_nodes);
+    for (int32_t q = b; q < e - 1; ++q) {
+        const int32_t dg = grp_of(sh_idx[q], group_nodes);
+        keys[q - s] = dg != og ? ((unsigned long long)(uint32_t)og << 32) | (uint32_t)dg : ~0ull;
+    }
+}
+
+__global__ void k_dep_fill(int32_t n, const unsigned long long* __restrict__ ukeys, int32_t* __restrict__ dep,
+                           int32_t* __restrict__ Hd) {
+    const int32_t q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= n) return;
+    const unsigned long long k = ukeys[q];
+    if (k == ~0ull) return;
+    dep[q] = (int32_t)(uint32_t)k;
+    atomicAdd(&Hd[(int32_t)(k >> 32)], 1);
+}
+
+__global__ void k_goff(int32_t ng, const int32_t* __restrict__ dep_off, const int32_t* __restrict__ offc,
+                       int4* __restrict__ goff) {
+    const int32_t g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g > ng) return;
+    goff[g] = make_int4(dep_off[g], offc[g], offc[(int64_t)(ng + 1) + g], offc[2 * (int64_t)(ng + 1) + g]);
+}
+
+template <typename T>
+int ex_scan(sem_ctx* c, Tmp& tmp, const T* in, T* out, int64_t n) {
+    size_t tb = 0;
+    SEM_CUDA_OK(c, cub::DeviceScan::ExclusiveSum(nullptr, tb, in, out, n, c->stream));
+    void* d = nullptr;
+    SEM_CUDA_OK(c, cudaMalloc(&d, tb ? tb : 1));
+    cudaError_t e = cub::DeviceScan::ExclusiveSum(d, tb, in, out, n, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    cudaFree(d);
+    if (e != cudaSuccess) return sem_fail(c, SEM_ECUDA, "scan: %s", cudaGetErrorString(e));
+    return SEM_OK;
+}
+
+}  // namespace
+
+int sem_build_owner_lists(sem_ctx* c) {
+    cudaStream_t st = c->stream;
+    const int32_t ng = (int32_t)c->ngroups;
+    const int32_t group_nodes = (int32_t)(c->epb * c->p3);
+    const int32_t Us = (int32_t)c->Us, nm1 = (int32_t)(c->has_mask ? c->n_mask1 : 0);
+    const int32_t n_ent = Us + nm1;
+    int rc;
+    SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_own_goff, ((size_t)ng + 1) * sizeof(int4)));
+    SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_gs_flag, (size_t)ng * sizeof(uint32_t)));
+    SEM_CUDA_OK(c, cudaMemsetAsync(c->d_gs_flag, 0, (size_t)ng * sizeof(uint32_t), st));
+    c->gs_epoch = 0;
+    Tmp tmp;
+    // ---- entries by (owner group, class) ----
+    uint32_t *d_keys = nullptr, *d_keys_s = nullptr;
+    int32_t *d_vals = nullptr, *d_vals_s = nullptr, *d_Hk = nullptr, *d_KS = nullptr, *d_Hc = nullptr, *d_offc = nullptr;
+    SEM_CUDA_OK(c, tmp.alloc(&d_keys, n_ent));
+    SEM_CUDA_OK(c, tmp.alloc(&d_keys_s, n_ent));
+    SEM_CUDA_OK(c, tmp.alloc(&d_vals, n_ent));
+    SEM_CUDA_OK(c, tmp.alloc(&d_vals_s, n_ent));
+    const int64_t nk = (int64_t)ng * 4 + 1, nc = 3 * ((int64_t)ng + 1);
+    SEM_CUDA_OK(c, tmp.alloc(&d_Hk, nk));
+    SEM_CUDA_OK(c, tmp.alloc(&d_KS, nk));
+    SEM_CUDA_OK(c, tmp.alloc(&d_Hc, nc));
+    SEM_CUDA_OK(c, tmp.alloc(&d_offc, nc));
+    SEM_CUDA_OK(c, cudaMemsetAsync(d_Hk, 0, nk * sizeof(int32_t), st));
+    SEM_CUDA_OK(c, cudaMemsetAsync(d_Hc, 0, nc * sizeof(int32_t), st));
+    int32_t h_tot[3] = {0, 0, 0};
+    if (n_ent > 0) {
+        k_own_keys<<<nblk(n_ent), 256, 0, st>>>(Us, nm1, group_nodes, ng, c->d_sh_off, c->d_sh_idx, c->d_mask1_idx,
+                                                d_keys, d_vals, d_Hk, d_Hc);
+        int end_bit = 1;
+        while (end_bit < 32 && (((uint64_t)ng * 4) >> end_bit)) ++end_bit;
+        size_t tb = 0;
+        SEM_CUDA_OK(c, cub::DeviceRadixSort::SortPairs(nullptr, tb, d_keys, d_keys_s, d_vals, d_vals_s, n_ent, 0,
+                                                        end_bit, st));
+        void* d_tmp = nullptr;
+        SEM_CUDA_OK(c, tmp.alloc((char**)&d_tmp, tb));
+        SEM_CUDA_OK(c, cub::DeviceRadixSort::SortPairs(d_tmp, tb, d_keys, d_keys_s, d_vals, d_vals_s, n_ent, 0, end_bit,
+                                                        st));
+    }
+    if ((rc = ex_scan(c, tmp, d_Hk, d_KS, nk))) return rc;
+    for (int cls = 0; cls < 3; ++cls)       // each class row ends with a zero: the scan leaves the class total there
+        if ((rc = ex_scan(c, tmp, d_Hc + cls * ((int64_t)ng + 1), d_offc + cls * ((int64_t)ng + 1), (int64_t)ng + 1)))
+            return rc;
+    for (int cls = 0; cls < 3; ++cls)
+        SEM_CUDA_OK(c, cudaMemcpyAsync(&h_tot[cls], d_offc + cls * ((int64_t)ng + 1) + ng, sizeof(int32_t),
+                                       cudaMemcpyDeviceToHost, st));
+    SEM_CUDA_OK(c, cudaStreamSynchronize(st));
+    c->n_pair = h_tot[0]; c->n_quad = h_tot[1]; c->n_big = h_tot[2];
+    SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_own_pair, (size_t)(c->n_pair ? c->n_pair : 1) * sizeof(int2)));
+    SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_own_quad, (size_t)(c->n_quad ? c->n_quad : 1) * sizeof(int4)));
+    SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_own_big, (size_t)(c->n_big ? c->n_big : 1) * sizeof(int2)));
+    if (n_ent > 0)
+        k_own_fill<<<nblk(n_ent), 256, 0, st>>>(n_ent, Us, ng, d_keys_s, d_vals_s, d_KS, d_offc, c->d_sh_off, c->d_sh_idx,
+                                                c->has_mask ? c->d_sh_masked : nullptr, c->d_mask1_idx, c->d_own_pair,
+                                                c->d_own_quad, c->d_own_big);
+    // ---- dependencies: distinct (owner group, lower group) pairs ----
+    const int64_t n_cand = c->S - c->Us;
+    int32_t *d_Hd = nullptr, *d_dep_off = nullptr;
+    SEM_CUDA_OK(c, tmp.alloc(&d_Hd, (int64_t)ng + 1));
+    SEM_CUDA_OK(c, tmp.alloc(&d_dep_off, (int64_t)ng + 1));
+    SEM_CUDA_OK(c, cudaMemsetAsync(d_Hd, 0, ((size_t)ng + 1) * sizeof(int32_t), st));
+    c->n_dep = 0;
+    if (n_cand > 0) {
+        unsigned long long *d_dk = nullptr, *d_dk_s = nullptr, *d_dk_u = nullptr;
+        int64_t* d_nsel = nullptr;
+        SEM_CUDA_OK(c, tmp.alloc(&d_dk, n_cand));
+        SEM_CUDA_OK(c, tmp.alloc(&d_dk_s, n_cand));
+        SEM_CUDA_OK(c, tmp.alloc(&d_nsel, 1));
+        k_dep_keys<<<nblk(Us), 256, 0, st>>>(Us, group_nodes, c->d_sh_off, c->d_sh_idx, d_dk);
+        size_t tb = 0;
+        SEM_CUDA_OK(c, cub::DeviceRadixSort::SortKeys(nullptr, tb, d_dk, d_dk_s, n_cand, 0, 64, st));
+        void* d_tmp = nullptr;
+        SEM_CUDA_OK(c, tmp.alloc((char**)&d_tmp, tb));
+        SEM_CUDA_OK(c, cub::DeviceRadixSort::SortKeys(d_tmp, tb, d_dk, d_dk_s, n_cand, 0, 64, st));
+        d_dk_u = d_dk;                                   // reuse the unsorted buffer for the unique keys
+        size_t tb2 = 0;
+        SEM_CUDA_OK(c, cub::DeviceSelect::Unique(nullptr, tb2, d_dk_s, d_dk_u, d_nsel, n_cand, st));
+        void* d_tmp2 = nullptr;
+        SEM_CUDA_OK(c, tmp.alloc((char**)&d_tmp2, tb2));
+        SEM_CUDA_OK(c, cub::DeviceSelect::Unique(d_tmp2, tb2, d_dk_s, d_dk_u, d_nsel, n_cand, st));
+        int64_t h_nsel = 0;
+        unsigned long long h_last = 0;
+        SEM_CUDA_OK(c, cudaMemcpyAsync(&h_nsel, d_nsel, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+        SEM_CUDA_OK(c, cudaStreamSynchronize(st));
+        if (h_nsel > 0) {
+            SEM_CUDA_OK(c, cudaMemcpyAsync(&h_last, d_dk_u + (h_nsel - 1), sizeof(h_last), cudaMemcpyDeviceToHost, st));
+            SEM_CUDA_OK(c, cudaStreamSynchronize(st));
+        }
+        c->n_dep = h_nsel - (h_nsel > 0 && h_last == ~0ull ? 1 : 0);
+        SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_own_dep, (size_t)(c->n_dep ? c->n_dep : 1) * sizeof(int32_t)));
+        if (c->n_dep > 0) k_dep_fill<<<nblk(c->n_dep), 256, 0, st>>>((int32_t)c->n_dep, d_dk_u, c->d_own_dep, d_Hd);
+        SEM_CUDA_OK(c, cudaStreamSynchronize(st));      // d_dk* are freed by tmp after this function's kernels ran
+    } else {
+        SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_own_dep, sizeof(int32_t)));
+    }
+    if ((rc = ex_scan(c, tmp, d_Hd, d_dep_off, (int64_t)ng + 1))) return rc;
+    k_goff<<<nblk((int64_t)ng + 1), 256, 0, st>>>(ng, d_dep_off, d_offc, c->d_own_goff);
     SEM_CUDA_OK(c, cudaStreamSynchronize(st));
     SEM_CUDA_OK(c, cudaGetLastError());
     return SEM_OK;

@@ -166,9 +166,7 @@ extern "C" int sem_pcg(sem_ctx* c, const double* b, double* x, double tol, int m
 
     // r = M b - A (M x0)
     k_mask_vec<<<vgrid, 256, 0, st>>>(n, c->d_wt, x);
-    int rc = sem_launch_ax(c, x, c->d_w, SEM_F64, c->lambda, nullptr, nullptr);
-    if (rc) return rc;
-    rc = sem_launch_gs(c, c->d_w, SEM_F64, true);
+    int rc = sem_launch_ax_gs(c, x, c->d_w, SEM_F64, c->lambda, nullptr, nullptr);
     if (rc) return rc;
     k_pcg_init<<<vgrid, 256, 0, st>>>(n, b, c->d_w, c->d_Minv, c->d_wt, x, c->d_r, c->d_p, scal);
     double h0[4];
@@ -182,9 +180,7 @@ extern "C" int sem_pcg(sem_ctx* c, const double* b, double* x, double tol, int m
         const double tol2 = tol > 0.0 ? tol * tol : 0.0;
         const int batch = 16;
         for (int it = 1; it <= maxit; ++it) {
-            rc = sem_launch_ax(c, c->d_p, c->d_w, SEM_F64, c->lambda, scal + 4 * it, &flags->done);
-            if (rc) return rc;
-            rc = sem_launch_gs(c, c->d_w, SEM_F64, true);
+            rc = sem_launch_ax_gs(c, c->d_p, c->d_w, SEM_F64, c->lambda, scal + 4 * it, &flags->done);
             if (rc) return rc;
             k_pcg_update<<<vgrid, 256, 0, st>>>(n, it, c->d_p, c->d_w, c->d_Minv, c->d_wt, x, c->d_r, scal, flags);
             k_pcg_direction<<<vgrid, 256, 0, st>>>(n, it, maxit, tol2, c->d_r, c->d_Minv, c->d_p, scal, flags);
