@@ -268,94 +268,17 @@ __global__ void __launch_bounds__(threads_of<P>()) ax_simple(int64_t E, DParam<T
 // ax_stream: persistent CTAs, G slabs and u elements arrive by bulk async copies into shared-memory rings.
 // Requires even P (so every chunk is a multiple of 16 bytes) and 16-byte aligned u.
 //
-// FUSE = true adds the gather-scatter and the Dirichlet mask (a6, a7) as an owner-computes epilogue: after a group's
-// local result is stored and published (release store of the application's epoch into flag[group]), the CTA sums
-// every shared node whose LAST copy lives in this group -- waiting (acquire) for the lower groups that hold the
-// other copies -- in ascending local index (O5) and writes the sum to all copies.  A group only ever waits for
-// lower-numbered groups and groups are handed out round-robin in ascending order to co-resident CTAs (cooperative
-// launch), so the lowest unfinished group never waits: no deadlock.  Every location is written by its own group
-// before the flag and by the owner after it, never concurrently.
+// FUSE = true: the launch is the first half of the single-pass Ax+gs (sem_gs.cu, k_gs_worker runs concurrently as a
+// programmatic dependent launch on the SM resources this kernel leaves free).  The only additions are
+//   * griddepcontrol.launch_dependents at the start (the worker grid may start once every CTA of this grid runs),
+//   * groups are handed out round-robin in ascending order, so CTAs finish them in "waves" of gridDim.x groups; half-way
+//     through its group of wave n+1 (after a bar.sync that every thread reaches after its stores of wave n) one
+//     thread does red.release.gpu.add(done[n]); the CTA's last group is published right after its stores.
+// This kernel never waits on the workers.
 // ---------------------------------------------------------------------------------------------------------------
-struct FuseArgs {
-    const int4* goff;        // [ngroups+1] (dep, pair, quad, big) list offsets
-    const int32_t* dep;
-    const int2* pair;
-    const int4* quad;
-    const int2* big;
-    const int32_t* sh_idx;
-    uint32_t* flag;          // [ngroups]
-    uint32_t epoch;
-};
-
-__device__ __forceinline__ void st_release_u32(uint32_t* p, uint32_t v) {
-    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-__device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t* p) {
-    uint32_t v;
-    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-// L2-coherent load of another CTA's (or this CTA's) local result
-__device__ __forceinline__ double ld_l2(const double* p) {
-    double v;
-    asm volatile("ld.relaxed.gpu.global.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ float ld_l2(const float* p) {
-    float v;
-    asm volatile("ld.relaxed.gpu.global.f32 %0, [%1];" : "=f"(v) : "l"(p) : "memory");
-    return v;
-}
-
-// a6 + a7 for the nodes owned by group grp.  All threads of the CTA call it after the group's w has been stored.
-template <typename T, int NT>
-__device__ __forceinline__ void gs_owned(const FuseArgs& f, int64_t grp, T* __restrict__ w) {
-    constexpr int32_t IDX = 0x7fffffff;
-    const int tid = threadIdx.x;
-    __syncthreads();                                  // every thread's stores of this group precede the release
-    const int4 o0 = f.goff[grp], o1 = f.goff[grp + 1];
-    if (tid == 0) {
-        __threadfence();
-        st_release_u32(f.flag + grp, f.epoch);
-    }
-    for (int32_t d = o0.x + tid; d < o1.x; d += NT) {
-        const uint32_t* fl = f.flag + f.dep[d];
-        while (ld_acquire_u32(fl) != f.epoch) { }
-    }
-    __syncthreads();
-    // pairs, two per thread in flight
-    for (int32_t q = o0.y + tid; q < o1.y; q += 2 * NT) {
-        const bool two = q + NT < o1.y;
-        const int2 a = f.pair[q];
-        const int2 b = two ? f.pair[q + NT] : make_int2(0, -1);
-        const int32_t a0 = a.x & IDX, b0 = b.x & IDX;
-        T sa = T(0), sb = T(0);
-        if (a.x >= 0 && a.y >= 0) { const T v0 = ld_l2(w + a0), v1 = ld_l2(w + a.y); sa = v0 + v1; }
-        if (two && b.x >= 0 && b.y >= 0) { const T v0 = ld_l2(w + b0), v1 = ld_l2(w + b.y); sb = v0 + v1; }
-        w[a0] = sa;
-        if (a.y >= 0) w[a.y] = sa;
-        if (two) { w[b0] = sb; if (b.y >= 0) w[b.y] = sb; }
-    }
-    for (int32_t q = o0.z + tid; q < o1.z; q += NT) {
-        const int4 a = f.quad[q];
-        const int32_t a0 = a.x & IDX;
-        T s = T(0);
-        if (a.x >= 0) {
-            const T v0 = ld_l2(w + a0), v1 = ld_l2(w + a.y), v2 = ld_l2(w + a.z);
-            s = (v0 + v1) + v2;
-            if (a.w >= 0) s += ld_l2(w + a.w);
-        }
-        w[a0] = s; w[a.y] = s; w[a.z] = s;
-        if (a.w >= 0) w[a.w] = s;
-    }
-    for (int32_t q = o0.w + tid; q < o1.w; q += NT) {
-        const int2 a = f.big[q];
-        const int32_t cnt = a.y & IDX;
-        T s = T(0);
-        if (a.y >= 0)
-            for (int32_t r = 0; r < cnt; ++r) s += ld_l2(w + f.sh_idx[a.x + r]);
-        for (int32_t r = 0; r < cnt; ++r) w[f.sh_idx[a.x + r]] = s;
-    }
+// release at gpu scope (orders, through the preceding bar.sync, every store of the CTA) + relaxed add; no L1 invalidate
+__device__ __forceinline__ void red_release_add(uint32_t* p) {
+    asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(p) : "memory");
 }
 
 template <typename T, int P, int NS>
@@ -375,7 +298,7 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
                                                                    const T* __restrict__ Gs, const T* __restrict__ Bm,
                                                                    T lambda, const T* __restrict__ u,
                                                                    T* __restrict__ w, const int* __restrict__ skip_flag,
-                                                                   double* __restrict__ dot_out, FuseArgs fuse) {
+                                                                   double* __restrict__ dot_out, uint32_t* __restrict__ done) {
     using SM = StreamSmem<T, P, NS>;
     constexpr int EPB = SM::EPB, P2 = SM::P2, P3 = SM::P3, SLAB = SM::SLAB, NT = threads_of<P>();
     constexpr bool FULL = EPB * P2 == NT;           // every thread owns a column
@@ -384,6 +307,7 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
     SM& sm = *reinterpret_cast<SM*>(smem_raw);
     if (skip_flag && *skip_flag) return;
     const int tid = threadIdx.x;
+    if constexpr (FUSE) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     const bool lane_ok = FULL || tid < EPB * P2;
     const int slot = lane_ok ? tid / P2 : 0;
     const int ij = lane_ok ? tid % P2 : 0;
@@ -427,6 +351,9 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
         }
         if (nmine > 1) issue_u(1);
     }
+    // the slab after which the previous group is published: staggered over the CTAs of an SM (CTAs are placed
+    // breadth-first, so b, b + #SM, ... share an SM) so that their fences do not stall the SM at the same time
+    const int kpub = 1 + (int)((blockIdx.x / 148u) % (unsigned)(P - 1));
     DRows<T, P> dr;
     dr.init(dp, i, j);
     T partial = T(0);
@@ -455,6 +382,11 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
             slab_part1<T, P>(dp, dr, sue, uk, wk, g, k, i, j, gr, gs);
             if (FULL || lane_ok) { sm.sgr[buf][slot * P2 + ij] = gr; sm.sgs[buf][slot * P2 + ij] = gs; }
             __syncthreads();
+            if constexpr (FUSE) {
+                // deferred publish of the PREVIOUS group (wave n-1): its stores were issued half a group ago, so the
+                // fence finds nothing outstanding; done by the last thread, not by the producer thread 0
+                if (k == kpub && n > 0 && tid == NT - 1) red_release_add(done + SEM_CTR_STRIDE * (n - 1));
+            }
             // every thread has consumed stage q (and, on the last slab, this group's u buffer): refill
             if (tid == 0) {
                 if (gleft > 0) {
@@ -478,7 +410,10 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
                 partial += uk[k] * v;
             }
         }
-        if constexpr (FUSE) gs_owned<T, NT>(fuse, grp, w);
+    }
+    if constexpr (FUSE) {                         // publish this CTA's last group (wave nmine-1)
+        __syncthreads();
+        if (tid == NT - 1 && nmine > 0) red_release_add(done + SEM_CTR_STRIDE * (nmine - 1));
     }
     if (dot_out) block_dot_flush(partial, dot_out);
 }
@@ -534,27 +469,27 @@ int launch_stream(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, doubl
         if (blocks_per_sm < 1) return sem_fail(c, SEM_ECUDA, "ax_stream does not fit on an SM");
         cached_dev = c->device;
     }
-    const int64_t cap = (int64_t)c->num_sms * blocks_per_sm;
-    const unsigned grid = (unsigned)(ngroups < cap ? ngroups : cap);
-    FuseArgs fa = {};
+    int64_t cap = (int64_t)c->num_sms * blocks_per_sm;
     cudaLaunchConfig_t cfg = {};
+    uint32_t* done = nullptr;
+    int reserve = 0;
+    if (FUSE) {
+        // leave `reserve` CTA slots per SM (registers, mostly) to the concurrently running gather-scatter workers
+        reserve = c->ax_variant >= 6 && c->ax_variant <= 8 ? c->ax_variant - 4 : 1;
+        if (reserve > blocks_per_sm - 1) reserve = blocks_per_sm - 1;
+        cap = (int64_t)c->num_sms * (blocks_per_sm - reserve);
+        done = c->d_gs_flag + SEM_CTR_DONE;
+    }
+    const unsigned grid = (unsigned)(ngroups < cap ? ngroups : cap);
     cfg.gridDim = dim3(grid);
     cfg.blockDim = dim3(threads_of<P>());
     cfg.dynamicSmemBytes = smem;
     cfg.stream = c->stream;
-    cudaLaunchAttribute attr[1];
-    if (FUSE) {
-        // the owner-computes epilogue waits on other CTAs: all CTAs must be co-resident (cooperative launch)
-        fa.goff = c->d_own_goff; fa.dep = c->d_own_dep; fa.pair = c->d_own_pair; fa.quad = c->d_own_quad;
-        fa.big = c->d_own_big; fa.sh_idx = c->d_sh_idx; fa.flag = c->d_gs_flag;
-        fa.epoch = ++c->gs_epoch;
-        attr[0].id = cudaLaunchAttributeCooperative;
-        attr[0].val.cooperative = 1;
-        cfg.attrs = attr;
-        cfg.numAttrs = 1;
-    }
     SEM_CUDA_OK(c, cudaLaunchKernelEx(&cfg, kern, c->E, dp, Gs, lambda != T(0) ? Bm : (const T*)nullptr, lambda, u, w,
-                                      skip, dot, fa));
+                                      skip, dot, done));
+    if (FUSE)
+        return sem_launch_gs_worker(c, w, sizeof(T) == 8 ? SEM_F64 : SEM_F32, (int32_t)grid, (int32_t)ngroups,
+                                    EPB * P * P * P, skip);
     return SEM_OK;
 }
 
@@ -581,7 +516,7 @@ int dispatch_p(sem_ctx* c, const void* u, void* w, double lambda, const int* ski
     const bool aligned = ((uintptr_t)u % 16) == 0;
     if constexpr (FUSE) {
         if constexpr (stream_ok<P>()) {
-            if (c->gmode == SEM_G_STORED && c->ax_variant == 5 && aligned)
+            if (c->gmode == SEM_G_STORED && c->ax_variant >= 5 && c->ax_variant <= 8 && aligned)
                 return launch_stream<T, P, StreamCfg<T, P>::NS, StreamCfg<T, P>::MINB, true>(c, uu, ww, (T)lambda, skip, dot);
         }
         return 1;
@@ -616,8 +551,9 @@ int sem_launch_ax(sem_ctx* c, const void* u, void* w, sem_prec prec, double lamb
     return dispatch<float, false>(c, u, w, lambda, skip_flag, dot_out);
 }
 
-// a3-a7: one kernel (Ax with the owner-computes gather-scatter + mask epilogue) where it applies; otherwise the
-// local operator followed by the stand-alone gather-scatter kernel.  Same results bit for bit (same summation order).
+// a3-a7: single pass (the operator kernel publishing per-wave progress + concurrently running gather-scatter workers,
+// see sem_gs.cu) where it applies; otherwise the local operator followed by the stand-alone gather-scatter kernel.
+// Same results bit for bit (same summation order).
 int sem_launch_ax_gs(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda, double* dot_out,
                      const int* skip_flag) {
     int rc = prec == SEM_F64 ? dispatch<double, true>(c, u, w, lambda, skip_flag, dot_out)

@@ -18,6 +18,13 @@ __host__ __device__ inline int64_t sem_g_off(int64_t e, int k, int p, int epb, i
     return ((grp * p + k) * epb + (e - grp * epb)) * slab;
 }
 
+#define SEM_CTR_STRIDE 32            /* uint32 words per counter */
+#define SEM_CTR_CHUNK 0
+#define SEM_CTR_TICKET SEM_CTR_STRIDE
+#define SEM_CTR_DONE (2 * SEM_CTR_STRIDE)
+// waves <= ngroups / (operator CTAs) + 1 and there are >= num_sms operator CTAs whenever there is more than one wave
+inline size_t sem_ctr_words(int64_t ngroups) { return (size_t)(ngroups / 64 + 8) * SEM_CTR_STRIDE; }
+
 struct sem_ctx {
     // ---- discretisation (a0) ----
     int64_t E = 0;
@@ -53,7 +60,10 @@ struct sem_ctx {
     int2* d_own_pair = nullptr;
     int4* d_own_quad = nullptr;
     int2* d_own_big = nullptr;
-    uint32_t* d_gs_flag = nullptr; // [ngroups] epoch of the last application whose local w of this group is written
+    // counters of the single-pass Ax+gs, all zero between launches, each on its own 128-byte line (they are polled
+    // and incremented concurrently): next gs chunk, exit ticket, and per wave v the number of element groups whose
+    // local w is stored                                                  (sem_ctr_words(ngroups) words)
+    uint32_t* d_gs_flag = nullptr;
     uint32_t gs_epoch = 0;
     int64_t n_dep = 0, n_pair = 0, n_quad = 0, n_big = 0;
     // Dirichlet (S14)
@@ -115,3 +125,5 @@ int sem_launch_ax_gs(sem_ctx* c, const void* u, void* w, sem_prec prec, double l
                      const int* skip_flag);      // a3-a7 in one kernel where the fused path applies, else ax then gs
 // sem_gs.cu
 int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask);
+int sem_launch_gs_worker(sem_ctx* c, void* w, sem_prec prec, int32_t n_ax, int32_t ngroups, int32_t group_nodes,
+                         const int* skip_flag);

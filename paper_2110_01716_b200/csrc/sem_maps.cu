@@ -352,8 +352,8 @@ int sem_build_owner_lists(sem_ctx* c) {
     const int32_t n_ent = Us + nm1;
     int rc;
     SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_own_goff, ((size_t)ng + 1) * sizeof(int4)));
-    SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_gs_flag, (size_t)ng * sizeof(uint32_t)));
-    SEM_CUDA_OK(c, cudaMemsetAsync(c->d_gs_flag, 0, (size_t)ng * sizeof(uint32_t), st));
+    SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_gs_flag, sem_ctr_words(ng) * sizeof(uint32_t)));
+    SEM_CUDA_OK(c, cudaMemsetAsync(c->d_gs_flag, 0, sem_ctr_words(ng) * sizeof(uint32_t), st));
     c->gs_epoch = 0;
     Tmp tmp;
     // ---- entries by (owner group, class) ----

@@ -258,6 +258,36 @@ def test_ax_gs_config1(torch_cuda, binding, oracle_mod, masked):
         assert torch_cuda.equal(dw, dw2)
 
 
+@pytest.mark.parametrize("variant", [5, 6])
+@pytest.mark.parametrize("case", ["cfg1", "cfg1_masked", "perm_N7", "N3_masked", "N1", "N5", "one_element", "N7_many"])
+def test_ax_gs_fused_equals_two_kernels(torch_cuda, binding, oracle_mod, case, variant):
+    """The single-launch path (operator CTAs + gather-scatter worker CTAs, variants 5/6) sums in the same order as
+    the two-kernel path: results are bit-identical to it and within tolerance of the oracle, FP64 and FP32, over
+    repeated launches (the in-kernel counters must come back to zero)."""
+    masked = case.endswith("masked")
+    m = {"cfg1": inputs.config1, "cfg1_masked": inputs.config1,
+         "perm_N7": lambda: inputs.box_mesh(5, 4, 3, 7, "random", seed=3, permute_seed=4),
+         "N3_masked": lambda: inputs.box_mesh(7, 6, 5, 3, "smooth"),
+         "N1": lambda: inputs.box_mesh(9, 8, 7, 1, "smooth"),
+         "N5": lambda: inputs.box_mesh(4, 3, 5, 5, "random", seed=2, permute_seed=1),
+         "one_element": lambda: inputs.box_mesh(1, 1, 1, 7),
+         "N7_many": lambda: inputs.box_mesh(13, 12, 11, 7, "smooth")}[case]()
+    u = inputs.field_uniform(m.gid, 7)
+    ow = _ax_gs_oracle(oracle_mod, m, u, masked)
+    with make_sem(binding, m, dirichlet=masked) as sem:
+        for dt, tol in ((torch_cuda.float64, TOL64), (torch_cuda.float32, TOL32)):
+            du = to_dev(torch_cuda, u.ravel(), dt)
+            ref = torch_cuda.empty_like(du)
+            sem.set_variant(0)
+            sem.ax_gs(du, ref)
+            sem.set_variant(variant)
+            for _ in range(3):
+                dw = torch_cuda.full_like(du, float("nan"))
+                sem.ax_gs(du, dw)
+                assert torch_cuda.equal(dw, ref), (case, variant, dt)
+            assert relerr(dw.cpu().numpy(), ow) <= tol
+
+
 @pytest.mark.parametrize("N", [7, 3, 1])
 def test_ax_gs_f32_levels_config4_small(torch_cuda, binding, oracle_mod, N):
     """Config 4 (mixed-precision levels N = 7, 3, 1), down-sized mesh: FP32 Ax+gs against the FP64 oracle."""
