@@ -239,6 +239,7 @@ int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask) {
     int64_t blocks = (int64_t)(ops / (4.0 * NT * PPT)) + 1;
     const int64_t cap = (int64_t)c->num_sms * 8;
     if (blocks > cap) blocks = cap;
+    blocks = (blocks + c->num_sms - 1) / c->num_sms * c->num_sms;      // same number of CTAs on every SM
 #define SEM_GS_LAUNCH(T, M)                                                                                      \
     k_gs_records<T, M><<<(unsigned)blocks, NT, 0, c->stream>>>(np, c->d_own_pair, nq, c->d_own_quad, nb,          \
                                                                 c->d_own_big, c->d_sh_idx, (T*)w)
