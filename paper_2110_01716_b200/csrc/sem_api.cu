@@ -51,7 +51,7 @@ int sem_mesh_setup(sem_ctx** out, int64_t E, int N, const double* vertex_xyz, co
     SEM_CUDA_OK(c, cudaMemcpyAsync(c->d_vert, vertex_xyz, E * 24 * sizeof(double), cudaMemcpyHostToDevice, c->stream));
     int rc = sem_build_maps(c, gid, dirichlet);
     if (rc) return rc;
-    return sem_build_owner_lists(c);
+    return sem_build_gs_records(c);
 }
 
 int sem_geom(sem_ctx* c, const double* node_xyz, sem_gmode mode, int with_mass) {
@@ -191,8 +191,8 @@ void sem_ctx_destroy(sem_ctx* c) {
     cudaStreamSynchronize(c->stream);
     void* ptrs[] = {c->d_vert, c->d_l2u, c->d_mult, c->d_seg_off, c->d_seg_idx, c->d_uniq_gid, c->d_sh_off, c->d_sh_idx,
                     c->d_sh_masked, c->d_mask_u, c->d_mask1_idx, c->d_G, c->d_G32, c->d_B, c->d_B32, c->d_detJ,
-                    c->d_diag, c->d_Minv, c->d_wt, c->d_r, c->d_p, c->d_w, c->d_scal, c->d_own_goff, c->d_own_dep,
-                    c->d_own_pair, c->d_own_quad, c->d_own_big, c->d_gs_flag};
+                    c->d_diag, c->d_Minv, c->d_wt, c->d_r, c->d_p, c->d_w, c->d_scal, 
+                    c->d_own_pair, c->d_own_quad, c->d_own_big};
     for (void* p : ptrs) cudaFree(p);
     cudaGetLastError();
     delete[] c->h_hist;

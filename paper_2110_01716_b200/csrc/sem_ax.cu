@@ -116,6 +116,25 @@ struct DRows {
                 asm volatile("" : "+f"(Di[l]), "+f"(Dj[l]), "+f"(DTi[l]), "+f"(DTj[l]));
         }
     }
+    // Same rows from a shared-memory copy sD[P*P] of D, read with volatile loads: values that come out of a volatile
+    // asm cannot be re-materialised from the constant bank, so ptxas has to keep them in registers whatever else the
+    // kernel contains (with init() that holds only as long as nothing else in the kernel raises register pressure).
+    __device__ __forceinline__ void init_shared(const T* sD, int i, int j) {
+        const uint32_t base = (uint32_t)__cvta_generic_to_shared(sD);
+#pragma unroll
+        for (int l = 0; l < P; ++l) {
+            Di[l] = lds_volatile(base + (uint32_t)((i * P + l) * sizeof(T)));
+            Dj[l] = lds_volatile(base + (uint32_t)((j * P + l) * sizeof(T)));
+            DTi[l] = lds_volatile(base + (uint32_t)((l * P + i) * sizeof(T)));
+            DTj[l] = lds_volatile(base + (uint32_t)((l * P + j) * sizeof(T)));
+        }
+    }
+    static __device__ __forceinline__ T lds_volatile(uint32_t addr) {
+        T v;
+        if constexpr (sizeof(T) == 8) asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+        else asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+        return v;
+    }
 };
 
 // One k-slab of the operator for thread (i,j) of one element.
@@ -268,19 +287,6 @@ __global__ void __launch_bounds__(threads_of<P>()) ax_simple(int64_t E, DParam<T
 // ax_stream: persistent CTAs, G slabs and u elements arrive by bulk async copies into shared-memory rings.
 // Requires even P (so every chunk is a multiple of 16 bytes) and 16-byte aligned u.
 //
-// FUSE = true: the launch is the first half of the single-pass Ax+gs (sem_gs.cu, k_gs_worker runs concurrently as a
-// programmatic dependent launch on the SM resources this kernel leaves free).  The only additions are
-//   * griddepcontrol.launch_dependents at the start (the worker grid may start once every CTA of this grid runs),
-//   * groups are handed out round-robin in ascending order, so CTAs finish them in "waves" of gridDim.x groups; half-way
-//     through its group of wave n+1 (after a bar.sync that every thread reaches after its stores of wave n) one
-//     thread does red.release.gpu.add(done[n]); the CTA's last group is published right after its stores.
-// This kernel never waits on the workers.
-// ---------------------------------------------------------------------------------------------------------------
-// release at gpu scope (orders, through the preceding bar.sync, every store of the CTA) + relaxed add; no L1 invalidate
-__device__ __forceinline__ void red_release_add(uint32_t* p) {
-    asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(p) : "memory");
-}
-
 template <typename T, int P, int NS>
 struct StreamSmem {
     static constexpr int EPB = epb_of<P>(), P2 = P * P, P3 = P2 * P;
@@ -291,14 +297,15 @@ struct StreamSmem {
     alignas(16) T sgs[2][EPB * P2];
     alignas(8) uint64_t gfull[NS];
     alignas(8) uint64_t ufull[2];
+    alignas(16) T D[P * P];                                  // copy of D for DRows::init_shared
 };
 
-template <typename T, int P, int NS, int MINB, bool FUSE>
+template <typename T, int P, int NS, int MINB>
 __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DParam<T, P> dp,
                                                                    const T* __restrict__ Gs, const T* __restrict__ Bm,
                                                                    T lambda, const T* __restrict__ u,
                                                                    T* __restrict__ w, const int* __restrict__ skip_flag,
-                                                                   double* __restrict__ dot_out, uint32_t* __restrict__ done) {
+                                                                   double* __restrict__ dot_out) {
     using SM = StreamSmem<T, P, NS>;
     constexpr int EPB = SM::EPB, P2 = SM::P2, P3 = SM::P3, SLAB = SM::SLAB, NT = threads_of<P>();
     constexpr bool FULL = EPB * P2 == NT;           // every thread owns a column
@@ -307,7 +314,6 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
     SM& sm = *reinterpret_cast<SM*>(smem_raw);
     if (skip_flag && *skip_flag) return;
     const int tid = threadIdx.x;
-    if constexpr (FUSE) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     const bool lane_ok = FULL || tid < EPB * P2;
     const int slot = lane_ok ? tid / P2 : 0;
     const int ij = lane_ok ? tid % P2 : 0;
@@ -336,6 +342,7 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
         mbar_init(&sm.ufull[1], 1);
         mbar_fence_init();
     }
+    for (int t = tid; t < P * P; t += NT) sm.D[t] = dp.D[t];
     __syncthreads();
     if (tid == 0 && nmine > 0) {
         pol_g = policy_evict_first();
@@ -351,11 +358,8 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
         }
         if (nmine > 1) issue_u(1);
     }
-    // the slab after which the previous group is published: staggered over the CTAs of an SM (CTAs are placed
-    // breadth-first, so b, b + #SM, ... share an SM) so that their fences do not stall the SM at the same time
-    const int kpub = 1 + (int)((blockIdx.x / 148u) % (unsigned)(P - 1));
     DRows<T, P> dr;
-    dr.init(dp, i, j);
+    dr.init_shared(sm.D, i, j);
     T partial = T(0);
 
     int q = 0;                 // ring stage of the slab being consumed
@@ -382,11 +386,6 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
             slab_part1<T, P>(dp, dr, sue, uk, wk, g, k, i, j, gr, gs);
             if (FULL || lane_ok) { sm.sgr[buf][slot * P2 + ij] = gr; sm.sgs[buf][slot * P2 + ij] = gs; }
             __syncthreads();
-            if constexpr (FUSE) {
-                // deferred publish of the PREVIOUS group (wave n-1): its stores were issued half a group ago, so the
-                // fence finds nothing outstanding; done by the last thread, not by the producer thread 0
-                if (k == kpub && n > 0 && tid == NT - 1) red_release_add(done + SEM_CTR_STRIDE * (n - 1));
-            }
             // every thread has consumed stage q (and, on the last slab, this group's u buffer): refill
             if (tid == 0) {
                 if (gleft > 0) {
@@ -410,10 +409,6 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
                 partial += uk[k] * v;
             }
         }
-    }
-    if constexpr (FUSE) {                         // publish this CTA's last group (wave nmine-1)
-        __syncthreads();
-        if (tid == NT - 1 && nmine > 0) red_release_add(done + SEM_CTR_STRIDE * (nmine - 1));
     }
     if (dot_out) block_dot_flush(partial, dot_out);
 }
@@ -451,7 +446,7 @@ int launch_simple(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, doubl
     return SEM_OK;
 }
 
-template <typename T, int P, int NS, int MINB, bool FUSE>
+template <typename T, int P, int NS, int MINB>
 int launch_stream(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, double* dot) {
     using SM = StreamSmem<T, P, NS>;
     constexpr int EPB = epb_of<P>();
@@ -460,7 +455,7 @@ int launch_stream(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, doubl
     const T* Bm = sizeof(T) == 8 ? (const T*)c->d_B : (const T*)c->d_B32;
     const DParam<T, P> dp = make_dparam<T, P>(c);
     const size_t smem = sizeof(SM) + 128;
-    auto kern = ax_stream<T, P, NS, MINB, FUSE>;
+    auto kern = ax_stream<T, P, NS, MINB>;
     static thread_local int cached_dev = -1;
     static thread_local int blocks_per_sm = 0;
     if (cached_dev != c->device) {
@@ -469,27 +464,11 @@ int launch_stream(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, doubl
         if (blocks_per_sm < 1) return sem_fail(c, SEM_ECUDA, "ax_stream does not fit on an SM");
         cached_dev = c->device;
     }
-    int64_t cap = (int64_t)c->num_sms * blocks_per_sm;
-    cudaLaunchConfig_t cfg = {};
-    uint32_t* done = nullptr;
-    int reserve = 0;
-    if (FUSE) {
-        // leave `reserve` CTA slots per SM (registers, mostly) to the concurrently running gather-scatter workers
-        reserve = c->ax_variant >= 6 && c->ax_variant <= 8 ? c->ax_variant - 4 : 1;
-        if (reserve > blocks_per_sm - 1) reserve = blocks_per_sm - 1;
-        cap = (int64_t)c->num_sms * (blocks_per_sm - reserve);
-        done = c->d_gs_flag + SEM_CTR_DONE;
-    }
+    const int64_t cap = (int64_t)c->num_sms * blocks_per_sm;
     const unsigned grid = (unsigned)(ngroups < cap ? ngroups : cap);
-    cfg.gridDim = dim3(grid);
-    cfg.blockDim = dim3(threads_of<P>());
-    cfg.dynamicSmemBytes = smem;
-    cfg.stream = c->stream;
-    SEM_CUDA_OK(c, cudaLaunchKernelEx(&cfg, kern, c->E, dp, Gs, lambda != T(0) ? Bm : (const T*)nullptr, lambda, u, w,
-                                      skip, dot, done));
-    if (FUSE)
-        return sem_launch_gs_worker(c, w, sizeof(T) == 8 ? SEM_F64 : SEM_F32, (int32_t)grid, (int32_t)ngroups,
-                                    EPB * P * P * P, skip);
+    kern<<<grid, threads_of<P>(), smem, c->stream>>>(c->E, dp, Gs, lambda != T(0) ? Bm : (const T*)nullptr, lambda, u, w,
+                                                     skip, dot);
+    SEM_CUDA_OK(c, cudaGetLastError());
     return SEM_OK;
 }
 
@@ -508,32 +487,23 @@ template <> struct StreamCfg<float, 10> { static constexpr int NS = 6, MINB = 4;
 
 template <int P> constexpr bool stream_ok() { return P % 2 == 0 && P <= 12; }
 
-// FUSE: the caller wants a3-a7; returns 1 if this (T, P, variant, alignment) has no fused kernel (caller falls back)
-template <typename T, int P, bool FUSE>
+template <typename T, int P>
 int dispatch_p(sem_ctx* c, const void* u, void* w, double lambda, const int* skip, double* dot) {
     const T* uu = (const T*)u;
     T* ww = (T*)w;
     const bool aligned = ((uintptr_t)u % 16) == 0;
-    if constexpr (FUSE) {
-        if constexpr (stream_ok<P>()) {
-            if (c->gmode == SEM_G_STORED && c->ax_variant >= 5 && c->ax_variant <= 8 && aligned)
-                return launch_stream<T, P, StreamCfg<T, P>::NS, StreamCfg<T, P>::MINB, true>(c, uu, ww, (T)lambda, skip, dot);
-        }
-        return 1;
-    } else {
-        if (c->gmode == SEM_G_RECOMPUTE) return launch_simple<T, P, true>(c, uu, ww, (T)lambda, skip, dot);
-        if constexpr (stream_ok<P>()) {
-            if (c->ax_variant != 1 && aligned)
-                return launch_stream<T, P, StreamCfg<T, P>::NS, StreamCfg<T, P>::MINB, false>(c, uu, ww, (T)lambda, skip, dot);
-        }
-        return launch_simple<T, P, false>(c, uu, ww, (T)lambda, skip, dot);
+    if (c->gmode == SEM_G_RECOMPUTE) return launch_simple<T, P, true>(c, uu, ww, (T)lambda, skip, dot);
+    if constexpr (stream_ok<P>()) {
+        if (c->ax_variant != 1 && aligned)
+            return launch_stream<T, P, StreamCfg<T, P>::NS, StreamCfg<T, P>::MINB>(c, uu, ww, (T)lambda, skip, dot);
     }
+    return launch_simple<T, P, false>(c, uu, ww, (T)lambda, skip, dot);
 }
 
-template <typename T, bool FUSE>
+template <typename T>
 int dispatch(sem_ctx* c, const void* u, void* w, double lambda, const int* skip, double* dot) {
     switch (c->p) {
-#define SEM_CASE(PP) case PP: return dispatch_p<T, PP, FUSE>(c, u, w, lambda, skip, dot);
+#define SEM_CASE(PP) case PP: return dispatch_p<T, PP>(c, u, w, lambda, skip, dot);
         SEM_CASE(2) SEM_CASE(3) SEM_CASE(4) SEM_CASE(5) SEM_CASE(6) SEM_CASE(7) SEM_CASE(8) SEM_CASE(9)
         SEM_CASE(10) SEM_CASE(11) SEM_CASE(12) SEM_CASE(13) SEM_CASE(14) SEM_CASE(15) SEM_CASE(16)
 #undef SEM_CASE
@@ -547,18 +517,16 @@ int dispatch(sem_ctx* c, const void* u, void* w, double lambda, const int* skip,
 // skip_flag != nullptr: the kernel returns at once if *skip_flag != 0 (device; used by the PCG loop after convergence).
 int sem_launch_ax(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda, double* dot_out,
                   const int* skip_flag) {
-    if (prec == SEM_F64) return dispatch<double, false>(c, u, w, lambda, skip_flag, dot_out);
-    return dispatch<float, false>(c, u, w, lambda, skip_flag, dot_out);
+    if (prec == SEM_F64) return dispatch<double>(c, u, w, lambda, skip_flag, dot_out);
+    return dispatch<float>(c, u, w, lambda, skip_flag, dot_out);
 }
 
-// a3-a7: single pass (the operator kernel publishing per-wave progress + concurrently running gather-scatter workers,
-// see sem_gs.cu) where it applies; otherwise the local operator followed by the stand-alone gather-scatter kernel.
-// Same results bit for bit (same summation order).
+// a3-a7: the local operator followed by the gather-scatter kernel (sem_gs.cu), which also applies the Dirichlet mask.
+// (Single-launch variants -- an owner-computes epilogue, concurrently running gather-scatter workers, a gather-scatter
+// tail phase of the operator kernel -- were built and measured slower than the two launches.)
 int sem_launch_ax_gs(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda, double* dot_out,
                      const int* skip_flag) {
-    int rc = prec == SEM_F64 ? dispatch<double, true>(c, u, w, lambda, skip_flag, dot_out)
-                             : dispatch<float, true>(c, u, w, lambda, skip_flag, dot_out);
-    if (rc != 1) return rc;
+    int rc;
     if ((rc = sem_launch_ax(c, u, w, prec, lambda, dot_out, skip_flag))) return rc;
     return sem_launch_gs(c, w, prec, true);
 }

@@ -18,13 +18,6 @@ __host__ __device__ inline int64_t sem_g_off(int64_t e, int k, int p, int epb, i
     return ((grp * p + k) * epb + (e - grp * epb)) * slab;
 }
 
-#define SEM_CTR_STRIDE 32            /* uint32 words per counter */
-#define SEM_CTR_CHUNK 0
-#define SEM_CTR_TICKET SEM_CTR_STRIDE
-#define SEM_CTR_DONE (2 * SEM_CTR_STRIDE)
-// waves <= ngroups / (operator CTAs) + 1 and there are >= num_sms operator CTAs whenever there is more than one wave
-inline size_t sem_ctr_words(int64_t ngroups) { return (size_t)(ngroups / 64 + 8) * SEM_CTR_STRIDE; }
-
 struct sem_ctx {
     // ---- discretisation (a0) ----
     int64_t E = 0;
@@ -46,26 +39,17 @@ struct sem_ctx {
     int32_t* d_sh_off = nullptr;   // [Us+1] offsets into d_sh_idx
     int32_t* d_sh_idx = nullptr;   // [S] local indices
     uint8_t* d_sh_masked = nullptr;// [Us] 1 = Dirichlet
-    // owner-computes lists for the gather-scatter fused into the Ax kernel (sem_maps.cu: sem_build_owner_lists).
-    // A shared node is owned by the element group holding its LAST (highest local index) copy.  Per group g:
-    //   deps   d_own_dep [goff[g].x .. goff[g+1].x)  lower groups holding copies of nodes owned by g
-    //   pairs  d_own_pair[goff[g].y .. goff[g+1].y)  int2 (l0 | maskbit, l1)      nodes with 2 copies; l1 = -1: only
-    //                                                                            zero w[l0] (unshared Dirichlet node)
-    //   quads  d_own_quad[goff[g].z .. goff[g+1].z)  int4 (l0 | maskbit, l1, l2, l3 or -1)   3 or 4 copies
-    //   bigs   d_own_big [goff[g].w .. goff[g+1].w)  int2 (offset into d_sh_idx, count | maskbit)  > 4 copies
+    // pre-resolved gather-scatter records (sem_maps.cu: sem_build_gs_records), sorted by the element group that holds
+    // the node's LAST (highest local index) copy, so that consecutive records touch neighbouring memory:
+    //   pairs  int2 (l0 | maskbit, l1)              nodes with 2 copies; l1 = -1: only zero w[l0] (unshared Dirichlet node)
+    //   quads  int4 (l0 | maskbit, l1, l2, l3 or -1) 3 or 4 copies
+    //   bigs   int2 (offset into d_sh_idx, count | maskbit)   > 4 copies
     int epb = 1;
     int64_t ngroups = 0;
-    int4* d_own_goff = nullptr;    // [ngroups+1]
-    int32_t* d_own_dep = nullptr;
     int2* d_own_pair = nullptr;
     int4* d_own_quad = nullptr;
     int2* d_own_big = nullptr;
-    // counters of the single-pass Ax+gs, all zero between launches, each on its own 128-byte line (they are polled
-    // and incremented concurrently): next gs chunk, exit ticket, and per wave v the number of element groups whose
-    // local w is stored                                                  (sem_ctr_words(ngroups) words)
-    uint32_t* d_gs_flag = nullptr;
-    uint32_t gs_epoch = 0;
-    int64_t n_dep = 0, n_pair = 0, n_quad = 0, n_big = 0;
+    int64_t n_pair = 0, n_quad = 0, n_big = 0;
     // Dirichlet (S14)
     bool has_mask = false;
     uint8_t* d_mask_u = nullptr;   // [U] 1 = masked unique node
@@ -112,7 +96,7 @@ int sem_fail(sem_ctx* c, int code, const char* fmt, ...);
 void sem_gll_tables(int N, double* xi, double* rho, double* D);
 // sem_maps.cu
 int sem_build_maps(sem_ctx* c, const int64_t* gid_any, const uint8_t* dirichlet_host);
-int sem_build_owner_lists(sem_ctx* c);
+int sem_build_gs_records(sem_ctx* c);
 // sem_geom.cu
 int sem_build_geom(sem_ctx* c, const double* node_xyz_host);
 int sem_build_g32(sem_ctx* c);
@@ -122,8 +106,6 @@ int sem_geom_export(sem_ctx* c, double* G_host, double* detJ_host);
 int sem_launch_ax(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda, double* dot_out,
                   const int* skip_flag);
 int sem_launch_ax_gs(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda, double* dot_out,
-                     const int* skip_flag);      // a3-a7 in one kernel where the fused path applies, else ax then gs
+                     const int* skip_flag);      // a3-a7: operator kernel + gather-scatter kernel
 // sem_gs.cu
 int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask);
-int sem_launch_gs_worker(sem_ctx* c, void* w, sem_prec prec, int32_t n_ax, int32_t ngroups, int32_t group_nodes,
-                         const int* skip_flag);

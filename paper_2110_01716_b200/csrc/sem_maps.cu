@@ -242,10 +242,10 @@ int sem_build_maps(sem_ctx* c, const int64_t* gid_any, const uint8_t* dirichlet_
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// Owner-computes lists for the gather-scatter fused into the Ax kernel (a6/a7 inside a3-a5's kernel; sem_ax.cu).
-// A shared node belongs to the element group that holds its last (highest local index) copy; that group sums the
-// copies in ascending local index (O5: same order as the oracle) once the lower groups have published their local
-// results.  Unshared Dirichlet nodes ride along as "pairs" with no partner.  Integer work only; setup, untimed.
+// Pre-resolved gather-scatter records (see sem_internal.h / sem_gs.cu): every shared node becomes one fixed-format
+// record (pair / quad / big) holding the local indices of its copies in ascending order (O5: the oracle's summation
+// order), and the records are sorted by the element group of the node's last copy.  Unshared Dirichlet nodes ride
+// along as "pairs" with no partner.  Integer work only; setup, untimed.
 // ---------------------------------------------------------------------------------------------------------------
 namespace {
 
@@ -299,36 +299,6 @@ __global__ void k_own_fill(int32_t n_ent, int32_t Us, int32_t ng, const uint32_t
     else bigs[pos] = make_int2(b, (int32_t)((uint32_t)cnt | mbit));
 }
 
-// one key (owner group << 32 | lower group) per non-last copy that lives in another group; else the sentinel
-__global__ void k_dep_keys(int32_t Us, int32_t group_nodes, const int32_t* __restrict__ sh_off,
-                           const int32_t* __restrict__ sh_idx, unsigned long long* __restrict__ keys) {
-    const int32_t s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= Us) return;
-    const int32_t b = sh_off[s], e = sh_off[s + 1];
-    const int32_t og = grp_of(sh_idx[e - 1], group_nodes);
-    for (int32_t q = b; q < e - 1; ++q) {
-        const int32_t dg = grp_of(sh_idx[q], group_nodes);
-        keys[q - s] = dg != og ? ((unsigned long long)(uint32_t)og << 32) | (uint32_t)dg : ~0ull;
-    }
-}
-
-__global__ void k_dep_fill(int32_t n, const unsigned long long* __restrict__ ukeys, int32_t* __restrict__ dep,
-                           int32_t* __restrict__ Hd) {
-    const int32_t q = blockIdx.x * blockDim.x + threadIdx.x;
-    if (q >= n) return;
-    const unsigned long long k = ukeys[q];
-    if (k == ~0ull) return;
-    dep[q] = (int32_t)(uint32_t)k;
-    atomicAdd(&Hd[(int32_t)(k >> 32)], 1);
-}
-
-__global__ void k_goff(int32_t ng, const int32_t* __restrict__ dep_off, const int32_t* __restrict__ offc,
-                       int4* __restrict__ goff) {
-    const int32_t g = blockIdx.x * blockDim.x + threadIdx.x;
-    if (g > ng) return;
-    goff[g] = make_int4(dep_off[g], offc[g], offc[(int64_t)(ng + 1) + g], offc[2 * (int64_t)(ng + 1) + g]);
-}
-
 template <typename T>
 int ex_scan(sem_ctx* c, Tmp& tmp, const T* in, T* out, int64_t n) {
     size_t tb = 0;
@@ -344,17 +314,13 @@ int ex_scan(sem_ctx* c, Tmp& tmp, const T* in, T* out, int64_t n) {
 
 }  // namespace
 
-int sem_build_owner_lists(sem_ctx* c) {
+int sem_build_gs_records(sem_ctx* c) {
     cudaStream_t st = c->stream;
     const int32_t ng = (int32_t)c->ngroups;
     const int32_t group_nodes = (int32_t)(c->epb * c->p3);
     const int32_t Us = (int32_t)c->Us, nm1 = (int32_t)(c->has_mask ? c->n_mask1 : 0);
     const int32_t n_ent = Us + nm1;
     int rc;
-    SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_own_goff, ((size_t)ng + 1) * sizeof(int4)));
-    SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_gs_flag, sem_ctr_words(ng) * sizeof(uint32_t)));
-    SEM_CUDA_OK(c, cudaMemsetAsync(c->d_gs_flag, 0, sem_ctr_words(ng) * sizeof(uint32_t), st));
-    c->gs_epoch = 0;
     Tmp tmp;
     // ---- entries by (owner group, class) ----
     uint32_t *d_keys = nullptr, *d_keys_s = nullptr;
@@ -400,48 +366,6 @@ int sem_build_owner_lists(sem_ctx* c) {
         k_own_fill<<<nblk(n_ent), 256, 0, st>>>(n_ent, Us, ng, d_keys_s, d_vals_s, d_KS, d_offc, c->d_sh_off, c->d_sh_idx,
                                                 c->has_mask ? c->d_sh_masked : nullptr, c->d_mask1_idx, c->d_own_pair,
                                                 c->d_own_quad, c->d_own_big);
-    // ---- dependencies: distinct (owner group, lower group) pairs ----
-    const int64_t n_cand = c->S - c->Us;
-    int32_t *d_Hd = nullptr, *d_dep_off = nullptr;
-    SEM_CUDA_OK(c, tmp.alloc(&d_Hd, (int64_t)ng + 1));
-    SEM_CUDA_OK(c, tmp.alloc(&d_dep_off, (int64_t)ng + 1));
-    SEM_CUDA_OK(c, cudaMemsetAsync(d_Hd, 0, ((size_t)ng + 1) * sizeof(int32_t), st));
-    c->n_dep = 0;
-    if (n_cand > 0) {
-        unsigned long long *d_dk = nullptr, *d_dk_s = nullptr, *d_dk_u = nullptr;
-        int64_t* d_nsel = nullptr;
-        SEM_CUDA_OK(c, tmp.alloc(&d_dk, n_cand));
-        SEM_CUDA_OK(c, tmp.alloc(&d_dk_s, n_cand));
-        SEM_CUDA_OK(c, tmp.alloc(&d_nsel, 1));
-        k_dep_keys<<<nblk(Us), 256, 0, st>>>(Us, group_nodes, c->d_sh_off, c->d_sh_idx, d_dk);
-        size_t tb = 0;
-        SEM_CUDA_OK(c, cub::DeviceRadixSort::SortKeys(nullptr, tb, d_dk, d_dk_s, n_cand, 0, 64, st));
-        void* d_tmp = nullptr;
-        SEM_CUDA_OK(c, tmp.alloc((char**)&d_tmp, tb));
-        SEM_CUDA_OK(c, cub::DeviceRadixSort::SortKeys(d_tmp, tb, d_dk, d_dk_s, n_cand, 0, 64, st));
-        d_dk_u = d_dk;                                   // reuse the unsorted buffer for the unique keys
-        size_t tb2 = 0;
-        SEM_CUDA_OK(c, cub::DeviceSelect::Unique(nullptr, tb2, d_dk_s, d_dk_u, d_nsel, n_cand, st));
-        void* d_tmp2 = nullptr;
-        SEM_CUDA_OK(c, tmp.alloc((char**)&d_tmp2, tb2));
-        SEM_CUDA_OK(c, cub::DeviceSelect::Unique(d_tmp2, tb2, d_dk_s, d_dk_u, d_nsel, n_cand, st));
-        int64_t h_nsel = 0;
-        unsigned long long h_last = 0;
-        SEM_CUDA_OK(c, cudaMemcpyAsync(&h_nsel, d_nsel, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
-        SEM_CUDA_OK(c, cudaStreamSynchronize(st));
-        if (h_nsel > 0) {
-            SEM_CUDA_OK(c, cudaMemcpyAsync(&h_last, d_dk_u + (h_nsel - 1), sizeof(h_last), cudaMemcpyDeviceToHost, st));
-            SEM_CUDA_OK(c, cudaStreamSynchronize(st));
-        }
-        c->n_dep = h_nsel - (h_nsel > 0 && h_last == ~0ull ? 1 : 0);
-        SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_own_dep, (size_t)(c->n_dep ? c->n_dep : 1) * sizeof(int32_t)));
-        if (c->n_dep > 0) k_dep_fill<<<nblk(c->n_dep), 256, 0, st>>>((int32_t)c->n_dep, d_dk_u, c->d_own_dep, d_Hd);
-        SEM_CUDA_OK(c, cudaStreamSynchronize(st));      // d_dk* are freed by tmp after this function's kernels ran
-    } else {
-        SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_own_dep, sizeof(int32_t)));
-    }
-    if ((rc = ex_scan(c, tmp, d_Hd, d_dep_off, (int64_t)ng + 1))) return rc;
-    k_goff<<<nblk((int64_t)ng + 1), 256, 0, st>>>(ng, d_dep_off, d_offc, c->d_own_goff);
     SEM_CUDA_OK(c, cudaStreamSynchronize(st));
     SEM_CUDA_OK(c, cudaGetLastError());
     return SEM_OK;
