@@ -41,12 +41,15 @@ def measured_peak_gbs():
 
 
 def ncu_traffic_bytes():
-    """Per-launch DRAM bytes of the Ax kernel from the committed ncu capture (profiles/ax_traffic.json), else None."""
+    """Per-launch DRAM bytes (read + write) of the Ax kernel from the committed ncu capture, else None."""
     try:
-        with open(os.path.join(ROOT, "profiles", "ax_traffic.json")) as f:
-            return float(json.load(f)["dram_bytes_per_launch"])
+        with open(os.path.join(ROOT, "profiles", "ax_traffic.txt")) as f:
+            for line in f:
+                if line.startswith("dram_bytes_per_launch="):
+                    return float(line.split("=", 1)[1])
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler:
@@ -168,6 +171,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=50)
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--pcg-iters", type=int, default=300)
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -254,6 +258,28 @@ def main():
         e2e_step()
     ms_e2e = timed(e2e_step, Ke)
 
+    # ---- PCG iterations/s (second half of BASELINE.json's metric): config 2 with the Dirichlet mask, fixed count ----
+    pcg = None
+    if rank == 0 and world == 1 and args.pcg_iters > 0:
+        semd = binding.Sem(mesh.E, mesh.N, mesh.vert, mesh.gid, mesh.dirichlet)
+        semd.geom()
+        rhs = torch.empty_like(u)
+        semd.ax_gs(u, rhs)                               # an assembled, masked right-hand side
+        x = torch.zeros_like(u)
+        semd.pcg(rhs, x, 1e-30, 20)                      # warm-up (allocates the work vectors)
+        x.zero_()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        nit, rel = semd.pcg(rhs, x, 1e-30, args.pcg_iters)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        # Ax 64 + gs 16 S/nL + update 56 + direction 32 bytes per local node per iteration
+        pcg_bytes = (64.0 + 56.0 + 32.0) * nL + 16.0 * S
+        pcg = {"iters_per_s": nit / dt, "us_per_iter": dt / nit * 1e6, "iters": nit, "relres": rel,
+               "algorithmic_GBs": pcg_bytes * nit / dt / 1e9,
+               "timed": "wall clock around one sem_pcg call (host polls a device flag every 16 iterations)"}
+        semd.close()
+
     dofs = mesh.dofs
     value = world * dofs * K / (ms_total * 1e-3) / 1e9
     e2e_value = world * dofs * Ke / (ms_e2e * 1e-3) / 1e9
@@ -274,7 +300,7 @@ def main():
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(u_h.numel() * 8),
                 "d2h_bytes_per_step": int(w_h.numel() * 8), "steps": Ke, "ms_per_step": ms_e2e / Ke},
         "gpu_launches": 2 * K,
-        "roofline": {"bound": "hbm", "kernel": "ax_stream<double,8> (local D^T G D u)", "achieved": achieved,
+        "roofline": {"bound": "hbm", "kernel": "ax_stream<double,8,5,8> (local D^T G D u)", "achieved": achieved,
                      "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": ncu_traffic_bytes(),
                      "peak_source": peak_src, "algorithmic_bytes_per_launch": ax_bytes,
                      "us_per_launch": ax_s * 1e6, "timed": f"{K} back-to-back launches of sem_ax alone, CUDA events",
@@ -286,6 +312,9 @@ def main():
                       "ax_TFLOPs_fp64": (12 * mesh.p + 15) * nL / ax_s / 1e12,
                       "G_local_nodes_per_s": nL * K / (ms_total * 1e-3) / 1e9},
     }
+    if pcg is not None:
+        pcg["frac_of_measured_peak"] = pcg["algorithmic_GBs"] / peak
+        line["pcg"] = pcg
     if rank == 0 and world == 1 and args.cpu_seconds > 0:
         line["cpu_baseline"] = cpu_oracle_baseline(mesh, args.cpu_seconds)
     sem.close()

@@ -23,10 +23,10 @@ using namespace semgs;
 // Stand-alone kernel (sem_gs, and sem_ax_gs where the single-pass path does not apply).  The grid is ONE wave
 // (<= resident CTAs of the device) and every CTA owns the same share of every record class: no tail, no imbalance.
 // ---------------------------------------------------------------------------------------------------------------
-constexpr int NT = 256;
+constexpr int NT = 256, GS_CTAS = 5;      // threads per CTA, resident CTAs per SM (48 registers, no spills)
 
 template <typename T, bool MASK>
-__global__ void __launch_bounds__(NT) k_gs_records(int32_t n_pair, const int2* __restrict__ pair, int32_t n_quad,
+__global__ void __launch_bounds__(NT, GS_CTAS) k_gs_records(int32_t n_pair, const int2* __restrict__ pair, int32_t n_quad,
                                                    const int4* __restrict__ quad, int32_t n_big,
                                                    const int2* __restrict__ big, const int32_t* __restrict__ sh_idx,
                                                    T* __restrict__ w) {
@@ -49,7 +49,7 @@ int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask) {
     // one wave of CTAs (8 x 256 threads per SM), fewer when there is less than one row of PPT pairs per thread
     const double ops = 4.0 * np + 8.0 * nq + 16.0 * nb;
     int64_t blocks = (int64_t)(ops / (4.0 * NT * PPT)) + 1;
-    const int64_t cap = (int64_t)c->num_sms * 8;
+    const int64_t cap = (int64_t)c->num_sms * GS_CTAS;
     if (blocks > cap) blocks = cap;
     blocks = (blocks + c->num_sms - 1) / c->num_sms * c->num_sms;      // same number of CTAs on every SM
 #define SEM_GS_LAUNCH(T, M)                                                                                      \
