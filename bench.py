@@ -162,6 +162,22 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def max_over_ranks(ms: float, world: int, device: str) -> float:
+    """Device time of a timed region for the whole job: the maximum over the ranks (replicas run independently)."""
+    if world <= 1:
+        return ms
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(units_per_rank_per_step: float, world: int, steps: int, ms: float) -> float:
+    """Whole-job throughput in 1e9 units/s: every rank processed `units_per_rank_per_step` per step (weak scaling)."""
+    return world * units_per_rank_per_step * steps / (ms * 1e-3) / 1e9
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -220,12 +236,7 @@ def main():
             fn()
         e1.record()
         barrier()
-        ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        return ms
+        return max_over_ranks(e0.elapsed_time(e1), world, "cuda")
 
     for _ in range(W):
         sem.ax_gs(u, w)
@@ -281,8 +292,8 @@ def main():
         semd.close()
 
     dofs = mesh.dofs
-    value = world * dofs * K / (ms_total * 1e-3) / 1e9
-    e2e_value = world * dofs * Ke / (ms_e2e * 1e-3) / 1e9
+    value = whole_job_value(dofs, world, K, ms_total)
+    e2e_value = whole_job_value(dofs, world, Ke, ms_e2e)
     peak, peak_src = measured_peak_gbs()
     ax_s = ms_ax * 1e-3 / K
     ax_bytes = 64.0 * nL                                     # 64 B per local node, FP64, stored G

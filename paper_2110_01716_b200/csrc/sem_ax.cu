@@ -480,9 +480,9 @@ template <> struct StreamCfg<double, 2> { static constexpr int NS = 2, MINB = 8;
 template <> struct StreamCfg<float, 2> { static constexpr int NS = 2, MINB = 8; };
 template <> struct StreamCfg<double, 4> { static constexpr int NS = 4, MINB = 8; };
 template <> struct StreamCfg<float, 4> { static constexpr int NS = 4, MINB = 8; };
-template <> struct StreamCfg<double, 6> { static constexpr int NS = 5, MINB = 6; };
+template <> struct StreamCfg<double, 6> { static constexpr int NS = 5, MINB = 5; };
 template <> struct StreamCfg<float, 6> { static constexpr int NS = 6, MINB = 6; };
-template <> struct StreamCfg<double, 10> { static constexpr int NS = 4, MINB = 4; };
+template <> struct StreamCfg<double, 10> { static constexpr int NS = 4, MINB = 3; };
 template <> struct StreamCfg<float, 10> { static constexpr int NS = 6, MINB = 4; };
 
 template <int P> constexpr bool stream_ok() { return P % 2 == 0 && P <= 12; }

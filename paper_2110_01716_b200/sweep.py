@@ -1,0 +1,100 @@
+"""Bandwidth sweep (BASELINE.json config 3) and mixed-precision levels (config 4) through the C ABI.
+
+    python -m paper_2110_01716_b200.sweep [--max-n 64] [--orders 3,5,7,9] [--levels]
+
+Box meshes of n^3 elements (n = 8, 16, 32, 64), random +-10 % interior-vertex perturbation (seed 1), FP64, stored G and
+G recomputed from the 8 trilinear vertices; with --levels also config 4 (20x20x18, N = 7, 3, 1, FP32).  Every case is
+timed with CUDA events over back-to-back launches after warm-up and printed as one markdown table row:
+algorithmic bytes are 64 B (FP64) / 32 B (FP32) per local node for Ax with stored G, 16 + 192/p^3 B recomputed, and
+16 B (8 B) per shared copy for gs.  Needs a CUDA device; there is no CPU fallback.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+
+import torch
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2110_01716_b200 import binding, inputs  # noqa: E402
+
+
+def _peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"])
+    except Exception:
+        return 6650.0
+
+
+def _time(fn, reps):
+    for _ in range(3):
+        fn()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(reps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) * 1e3 / reps          # us
+
+
+def run_case(mesh, dtype, peak, label):
+    esize = 8 if dtype == torch.float64 else 4
+    u = torch.from_numpy(inputs.field_uniform(mesh.gid, 1).ravel()).cuda().to(dtype)
+    w = torch.empty_like(u)
+    row = {}
+    for mode in (binding.SEM_G_STORED, binding.SEM_G_RECOMPUTE):
+        with binding.Sem(mesh.E, mesh.N, mesh.vert, mesh.gid) as sem:
+            sem.geom(mode=mode)
+            cnt = sem.counts()
+            nL, S = cnt["nL"], cnt["S"]
+            reps = max(20, min(2000, int(2e9 / (nL * 64))))
+            t_ax = _time(lambda: sem.ax(u, w), reps)
+            if mode == binding.SEM_G_STORED:
+                t_gs = _time(lambda: sem.gs(w), reps)
+                t_axgs = _time(lambda: sem.ax_gs(u, w), reps)
+                b_ax = 8.0 * esize * nL
+                row.update(nL=nL, S=S, ax=t_ax, gs=t_gs, axgs=t_axgs, ax_gbs=b_ax / t_ax / 1e3,
+                           axgs_gbs=(b_ax + 2.0 * esize * S) / t_axgs / 1e3,
+                           gdofs=mesh.dofs / t_axgs / 1e3)
+            else:
+                p3 = mesh.p ** 3
+                row.update(ax_re=t_ax, re_gbs=(2.0 * esize + 192.0 / p3) * nL / t_ax / 1e3,
+                           re_tflops=(12 * mesh.p + 15 + 125) * nL / t_ax / 1e6)
+    print(f"| {label} | {mesh.E} | {mesh.N} | {row['nL']} | {row['ax']:.1f} | {row['ax_gbs']:.0f} | "
+          f"{row['ax_gbs'] / peak:.2f} | {row['gs']:.1f} | {row['axgs']:.1f} | {row['axgs_gbs']:.0f} | "
+          f"{row['gdofs']:.1f} | {row['ax_re']:.1f} | {row['re_tflops']:.1f} |", flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--max-n", type=int, default=64)
+    ap.add_argument("--orders", default="3,5,7,9")
+    ap.add_argument("--levels", action="store_true")
+    args = ap.parse_args()
+    if not torch.cuda.is_available():
+        raise SystemExit("sweep needs a CUDA device: the product path has no CPU fallback")
+    peak = _peak()
+    print(f"peak = {peak:.0f} GB/s (MEASURED_PEAKS.json hbm_gbs, else the profiling guide's fallback)")
+    print("| case | E | N | nL | Ax us | Ax GB/s | frac of peak | gs us | Ax+gs us | Ax+gs GB/s | GDOF/s (E N^3) | "
+          "Ax recomputed-G us | recomputed TFLOP/s |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|---|---|")
+    for N in [int(x) for x in args.orders.split(",")]:
+        n = 8
+        while n <= args.max_n:
+            run_case(inputs.config3(n, N), torch.float64, peak, f"cfg3 {n}^3 f64")
+            n *= 2
+    if args.levels:
+        for N in (7, 3, 1):
+            run_case(inputs.config4(N), torch.float32, peak, "cfg4 20x20x18 f32")
+
+
+if __name__ == "__main__":
+    main()

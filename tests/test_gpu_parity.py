@@ -416,6 +416,29 @@ def test_pcg_converges_same_iteration_count(torch_cuda, binding, oracle_mod):
         assert it4 == 0 and float(x2.sum()) == float((mask_u[om.l2u] == 0).sum())
 
 
+def test_pcg_trajectory_config5_replica(torch_cuda, binding, oracle_mod):
+    """S20: config-5 recipe (N = 7, random +-10 % vertices seed 3, element permutation seed 4, b = M Q^T(B f)) on a
+    6^3 replica: the iterates x_k at k = 1, 5, 10, 25 and the residual history agree with the oracle's."""
+    m = inputs.config5(6)
+    om, oG, mask_u = _pcg_setup(oracle_mod, m)
+    xyz = oracle_mod.node_xyz(m.vert, m.N).reshape(-1, 3)
+    f = 3 * np.pi ** 2 * np.sin(np.pi * xyz[:, 0]) * np.sin(np.pi * xyz[:, 1]) * np.sin(np.pi * xyz[:, 2])
+    b_u = np.zeros(om.U)
+    np.add.at(b_u, om.l2u, oG[:, 6].ravel() * f)
+    b_u[mask_u != 0] = 0.0
+    ores = oracle_mod.pcg(oG, m.N, om, mask_u, b_u, tol=1e-30, maxit=25, snap_its=(1, 5, 10, 25))
+    with make_sem(binding, m, dirichlet=True) as sem:
+        b = to_dev(torch_cuda, b_u[om.l2u])
+        for k in (1, 5, 10, 25):
+            x = torch_cuda.zeros_like(b)
+            it, rel = sem.pcg(b, x, 1e-30, k)
+            assert it == k
+            assert relerr(x.cpu().numpy(), ores["snaps"][k][om.l2u]) <= TOLPCG, k
+            assert abs(rel - ores["hist"][k]) <= 1e-9 * ores["hist"][k], k
+        hist = sem.pcg_history(26)
+        assert np.max(np.abs(hist - ores["hist"]) / ores["hist"]) <= 1e-9
+
+
 def test_pcg_helmholtz(torch_cuda, binding, oracle_mod):
     m = inputs.box_mesh(3, 3, 3, 4, "smooth")
     om, oG, mask_u = _pcg_setup(oracle_mod, m)
