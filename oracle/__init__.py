@@ -171,3 +171,27 @@ def pcg(G, N, maps: Maps, mask_u, b_u, x0_u=None, tol=1e-8, maxit=100, lam=0.0, 
                        _p(hist), C.c_int(ns), _p(snap_its), _p(xs))
     return dict(x=x, iters=int(it), relres=float(relres.value), hist=hist[: it + 1],
                 snaps={int(s): xs[n] for n, s in enumerate(snap_its) if s <= it})
+
+
+# ---- NEXT-1: p-multigrid transfer operators --------------------------------------------------------------
+def interp(Nc: int, Nf: int) -> np.ndarray:
+    """J[i, j] = coarse (order Nc) Lagrange cardinal function j at fine (order Nf) GLL point i."""
+    J = np.empty((Nf + 1, Nc + 1))
+    assert lib().orc_interp(C.c_int(Nc), C.c_int(Nf), _p(J)) == 0
+    return J
+
+
+def prolong(uc: np.ndarray, Nc: int, Nf: int) -> np.ndarray:
+    """u_f = (J x J x J) u_c per element; uc [E, (Nc+1)^3] -> [E, (Nf+1)^3]."""
+    uc = _f64(uc).reshape(-1, (Nc + 1) ** 3)
+    uf = np.empty((uc.shape[0], (Nf + 1) ** 3))
+    assert lib().orc_prolong(C.c_int64(uc.shape[0]), C.c_int(Nc), C.c_int(Nf), _p(uc), _p(uf)) == 0
+    return uf
+
+
+def restrict(rf: np.ndarray, Nc: int, Nf: int) -> np.ndarray:
+    """r_c = (J^T x J^T x J^T) r_f per element; rf [E, (Nf+1)^3] -> [E, (Nc+1)^3]."""
+    rf = _f64(rf).reshape(-1, (Nf + 1) ** 3)
+    rc = np.empty((rf.shape[0], (Nc + 1) ** 3))
+    assert lib().orc_restrict(C.c_int64(rf.shape[0]), C.c_int(Nc), C.c_int(Nf), _p(rf), _p(rc)) == 0
+    return rc

@@ -418,4 +418,70 @@ int orc_pcg(int64_t E, int N, const double* G, double lambda, int64_t nL, int64_
     return it;
 }
 
+// ---- NEXT-1: p-multigrid transfer operators ----------------------------------------------------
+// P:103 "Coarse-to-fine interpolations are cast as efficient tensor contractions, u_f = (J x J x J) u_c, where J is the
+// 1D polynomial interpolation operator from the coarse GLL points to the fine GLL points."
+// J[i*(Nc+1) + j] = h^c_j(xi^f_i): Lagrange cardinal function j of the Nc+1 coarse GLL points at fine GLL point i,
+// written out as the plain product formula  prod_{m != j} (x - xi^c_m) / (xi^c_j - xi^c_m).
+int orc_interp(int Nc, int Nf, double* J) {
+    if (Nc < 1 || Nf < 1) return -1;
+    const int pc = Nc + 1, pf = Nf + 1;
+    std::vector<double> xc(pc), xf(pf), rho(std::max(pc, pf)), D((size_t)std::max(pc, pf) * std::max(pc, pf));
+    orc_gll(Nc, xc.data(), rho.data(), D.data());
+    orc_gll(Nf, xf.data(), rho.data(), D.data());
+    for (int i = 0; i < pf; ++i)
+        for (int j = 0; j < pc; ++j) {
+            long double h = 1.0L;
+            for (int m = 0; m < pc; ++m)
+                if (m != j) h *= ((long double)xf[i] - (long double)xc[m]) / ((long double)xc[j] - (long double)xc[m]);
+            J[i * pc + j] = (double)h;
+        }
+    return 0;
+}
+
+// Prolongation, element by element (local layout, i fastest):  uf[k][j][i] = sum_{c,b,a} J[k][c] J[j][b] J[i][a] uc[c][b][a].
+int orc_prolong(int64_t E, int Nc, int Nf, const double* uc, double* uf) {
+    const int pc = Nc + 1, pf = Nf + 1;
+    std::vector<double> J((size_t)pf * pc);
+    if (orc_interp(Nc, Nf, J.data())) return -1;
+    const int64_t pc3 = (int64_t)pc * pc * pc, pf3 = (int64_t)pf * pf * pf;
+#pragma omp parallel for
+    for (int64_t e = 0; e < E; ++e)
+        for (int k = 0; k < pf; ++k)
+            for (int j = 0; j < pf; ++j)
+                for (int i = 0; i < pf; ++i) {
+                    long double s = 0.0L;
+                    for (int c = 0; c < pc; ++c)
+                        for (int b = 0; b < pc; ++b)
+                            for (int a = 0; a < pc; ++a)
+                                s += (long double)J[k * pc + c] * J[j * pc + b] * J[i * pc + a] *
+                                     uc[e * pc3 + ((int64_t)c * pc + b) * pc + a];
+                    uf[e * pf3 + ((int64_t)k * pf + j) * pf + i] = (double)s;
+                }
+    return 0;
+}
+
+// Restriction = the transpose of the prolongation (residuals are functionals: r_c = (J^T x J^T x J^T) r_f), element by
+// element:  rc[c][b][a] = sum_{k,j,i} J[k][c] J[j][b] J[i][a] rf[k][j][i].
+int orc_restrict(int64_t E, int Nc, int Nf, const double* rf, double* rc) {
+    const int pc = Nc + 1, pf = Nf + 1;
+    std::vector<double> J((size_t)pf * pc);
+    if (orc_interp(Nc, Nf, J.data())) return -1;
+    const int64_t pc3 = (int64_t)pc * pc * pc, pf3 = (int64_t)pf * pf * pf;
+#pragma omp parallel for
+    for (int64_t e = 0; e < E; ++e)
+        for (int c = 0; c < pc; ++c)
+            for (int b = 0; b < pc; ++b)
+                for (int a = 0; a < pc; ++a) {
+                    long double s = 0.0L;
+                    for (int k = 0; k < pf; ++k)
+                        for (int j = 0; j < pf; ++j)
+                            for (int i = 0; i < pf; ++i)
+                                s += (long double)J[k * pc + c] * J[j * pc + b] * J[i * pc + a] *
+                                     rf[e * pf3 + ((int64_t)k * pf + j) * pf + i];
+                    rc[e * pc3 + ((int64_t)c * pc + b) * pc + a] = (double)s;
+                }
+    return 0;
+}
+
 }  // extern "C"

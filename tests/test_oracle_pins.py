@@ -441,3 +441,69 @@ def test_inputs_fields_are_continuous_and_seeded():
     assert np.abs(V1 - V0).max() <= 0.1 * h and np.abs(V1 - V0)[1:-1, 1:-1, 1:-1].min() > 0
     assert np.array_equal(V1[0], V0[0]) and np.array_equal(V1[:, :, -1], V0[:, :, -1])
     assert r.dirichlet.sum() > 0 and r.gid.max() == r.unique_nodes - 1
+
+
+# ---------------------------------------------------------------------------------- NEXT-1: pMG transfer operators
+# P:103 "u_f = (J x J x J) u_c, where J is the 1D polynomial interpolation operator from the coarse GLL points to the
+# fine GLL points".  Pins: polynomial reproduction (the defining property of interpolation), partition of unity,
+# identity at equal orders, nesting of levels, the paper's level schedules, exact 3-D reproduction, and adjointness of
+# the restriction.
+@pytest.mark.parametrize("Nc,Nf", [(1, 3), (3, 7), (1, 7), (5, 8), (4, 6), (1, 8), (7, 7), (2, 5)])
+def test_T1_interp_reproduces_polynomials(oracle_mod, Nc, Nf):
+    J = oracle_mod.interp(Nc, Nf)
+    xc, _, _ = oracle_mod.gll(Nc)
+    xf, _, _ = oracle_mod.gll(Nf)
+    assert J.shape == (Nf + 1, Nc + 1)
+    for m in range(Nc + 1):                                   # degree <= Nc is reproduced exactly
+        assert np.max(np.abs(J @ xc ** m - xf ** m)) <= 1e-13
+    assert np.max(np.abs(J.sum(axis=1) - 1.0)) <= 1e-14       # partition of unity
+    assert np.max(np.abs(J[0] - np.eye(Nc + 1)[0])) <= 1e-15 and np.max(np.abs(J[-1] - np.eye(Nc + 1)[-1])) <= 1e-15
+    if Nc == Nf:
+        assert np.max(np.abs(J - np.eye(Nc + 1))) <= 1e-14
+
+
+def test_T1_interp_closed_form_N1():
+    """N_c = 1: the two cardinal functions are (1 -+ x)/2, so J = [(1 - xi_f)/2, (1 + xi_f)/2] (closed form)."""
+    import oracle
+    xf, _, _ = oracle.gll(7)
+    J = oracle.interp(1, 7)
+    assert np.max(np.abs(J - np.stack([(1 - xf) / 2, (1 + xf) / 2], axis=1))) <= 1e-15
+
+
+def test_T2_levels_nest(oracle_mod):
+    """Interpolating 1 -> 3 -> 7 equals interpolating 1 -> 7 (config 4's schedule), likewise the paper's 1-5-8."""
+    for a, b, c in ((1, 3, 7), (1, 5, 8), (1, 4, 6)):
+        assert np.max(np.abs(oracle_mod.interp(b, c) @ oracle_mod.interp(a, b) - oracle_mod.interp(a, c))) <= 1e-13
+
+
+def test_T3_prolong_reproduces_3d_polynomial_and_is_kron(oracle_mod):
+    Nc, Nf, E = 3, 7, 3
+    xc, _, _ = oracle_mod.gll(Nc)
+    xf, _, _ = oracle_mod.gll(Nf)
+    f = lambda r, s, t: 1.0 + r - 2 * s * t + r ** 3 * s ** 2 - 0.5 * t ** 3 * r * s ** 3        # degree <= 3 per variable
+    uc = np.stack([f(xc[None, None, :], xc[None, :, None], xc[:, None, None]) * (e + 1) for e in range(E)])
+    uf = oracle_mod.prolong(uc.reshape(E, -1), Nc, Nf).reshape(E, Nf + 1, Nf + 1, Nf + 1)
+    for e in range(E):
+        assert np.max(np.abs(uf[e] - f(xf[None, None, :], xf[None, :, None], xf[:, None, None]) * (e + 1))) <= 1e-13
+    # dense Kronecker product, no shared code: index (k, j, i) with i fastest <-> J (x) J (x) J
+    J = oracle_mod.interp(Nc, Nf)
+    K = np.kron(J, np.kron(J, J))
+    rng = np.random.default_rng(0)
+    v = rng.standard_normal((2, (Nc + 1) ** 3))
+    assert np.max(np.abs(oracle_mod.prolong(v, Nc, Nf) - v @ K.T)) <= 1e-13
+    r = rng.standard_normal((2, (Nf + 1) ** 3))
+    assert np.max(np.abs(oracle_mod.restrict(r, Nc, Nf) - r @ K)) <= 1e-13
+
+
+@pytest.mark.parametrize("Nc,Nf", [(1, 3), (3, 7), (5, 8)])
+def test_T4_restriction_is_the_adjoint(oracle_mod, Nc, Nf):
+    rng = np.random.default_rng(Nc * 10 + Nf)
+    uc = rng.standard_normal((4, (Nc + 1) ** 3))
+    rf = rng.standard_normal((4, (Nf + 1) ** 3))
+    lhs = np.sum(oracle_mod.prolong(uc, Nc, Nf) * rf)
+    rhs = np.sum(uc * oracle_mod.restrict(rf, Nc, Nf))
+    assert abs(lhs - rhs) <= 1e-12 * abs(lhs)
+    # a transposed operand or swapped index order would break this: restrict(prolong(u)) = (J^T J)^{x3} u
+    J = oracle_mod.interp(Nc, Nf)
+    M = J.T @ J
+    assert np.max(np.abs(oracle_mod.restrict(oracle_mod.prolong(uc, Nc, Nf), Nc, Nf) - uc @ np.kron(M, np.kron(M, M)).T)) <= 1e-12
