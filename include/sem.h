@@ -114,6 +114,20 @@ SEM_API int sem_get_gll(sem_ctx* ctx, double* xi /*[p]*/, double* rho /*[p]*/, d
 SEM_API int sem_get_geom(sem_ctx* ctx, double* G /*[E][6 or 7][p^3]*/, double* detJ /*[E][p^3]*/);
 SEM_API int sem_get_diag(sem_ctx* ctx, double* diagA_local /* assembled QQ^T diag(A_L), unmasked, [E][p^3] */);
 
+/* NEXT-1.  p-multigrid transfer between two discretisations of the SAME E elements ("u_f =
+ * (J x J x J) u_c, where J is the 1D polynomial interpolation operator from the coarse GLL points to the fine GLL
+ * points"), element by element, no gather-scatter and no weighting (the multigrid cycle applies those):
+ *   SEM_PROLONG:   out[E][pf^3] = (J   x J   x J  ) in[E][pc^3]
+ *   SEM_RESTRICT:  out[E][pc^3] = (J^T x J^T x J^T) in[E][pf^3]
+ * J[i][j] = Lagrange cardinal function j of the coarse GLL points at fine GLL point i ([pf][pc], pc = N_c+1 <= pf).
+ *   coarse, fine  contexts from sem_mesh_setup with equal E and N_c <= N_f (else SEM_EINVAL, text in fine's error)
+ *   in, out       DEVICE, local layout, `prec` values; must not alias
+ * Asynchronous on the FINE context's stream.  FP32 (S16): J rounded once from double, accumulation in float. */
+typedef enum { SEM_PROLONG = 0, SEM_RESTRICT = 1 } sem_transfer_dir;
+SEM_API int sem_transfer(sem_ctx* coarse, sem_ctx* fine, const void* in, void* out, sem_prec prec, sem_transfer_dir dir);
+/* Parity accessor: the interpolation matrix J, [pf][pc] doubles, HOST. */
+SEM_API int sem_get_interp(sem_ctx* coarse, sem_ctx* fine, double* J);
+
 /* Tuning knob for experiments: selects the Ax kernel variant (0 = default streaming kernel, 1 = simple kernel). */
 SEM_API int sem_set_variant(sem_ctx* ctx, int ax_variant);
 

@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libsem.so")
 SEM_F64, SEM_F32 = 0, 1
 SEM_OP_ADD = 0
 SEM_G_STORED, SEM_G_RECOMPUTE = 0, 1
+SEM_PROLONG, SEM_RESTRICT = 0, 1
 SEM_OK, SEM_EINVAL, SEM_EMESH, SEM_ECUDA, SEM_ENOMEM, SEM_ESTATE = 0, -1, -2, -3, -4, -5
 _ERRNAME = {-1: "SEM_EINVAL", -2: "SEM_EMESH", -3: "SEM_ECUDA", -4: "SEM_ENOMEM", -5: "SEM_ESTATE"}
 
@@ -37,6 +38,8 @@ SYMBOLS = {
     "sem_get_geom": (_i32, [_vp, _vp, _vp]),
     "sem_get_diag": (_i32, [_vp, _vp]),
     "sem_set_variant": (_i32, [_vp, _i32]),
+    "sem_transfer": (_i32, [_vp, _vp, _vp, _vp, _i32, _i32]),
+    "sem_get_interp": (_i32, [_vp, _vp, _vp]),
     "sem_last_error": (C.c_char_p, [_vp]),
     "sem_ctx_destroy": (None, [_vp]),
 }
@@ -168,6 +171,25 @@ class Sem:
 
     def set_lambda(self, lam: float):
         self._check(self._L.sem_set_lambda(self._h, lam))
+
+    def transfer(self, fine: "Sem", vin, vout, direction: int):
+        """sem_transfer with self as the COARSE context: SEM_PROLONG coarse -> fine, SEM_RESTRICT fine -> coarse."""
+        n_in, n_out = (fine.nL, self.nL) if direction == SEM_RESTRICT else (self.nL, fine.nL)
+        for t, n in ((vin, n_in), (vout, n_out)):
+            assert t.is_cuda and t.is_contiguous() and t.numel() == n and t.dtype == vin.dtype, \
+                "need contiguous CUDA tensors of the coarse / fine local sizes"
+        rc = self._L.sem_transfer(self._h, fine._h, C.c_void_p(vin.data_ptr()), C.c_void_p(vout.data_ptr()),
+                                  self._prec(vin), direction)
+        if rc != SEM_OK:
+            raise SemError(rc, self._L.sem_last_error(fine._h).decode())
+        return vout
+
+    def interp(self, fine: "Sem") -> np.ndarray:
+        J = np.empty((fine.N + 1, self.N + 1))
+        rc = self._L.sem_get_interp(self._h, fine._h, _np_ptr(J))
+        if rc != SEM_OK:
+            raise SemError(rc, self._L.sem_last_error(fine._h).decode())
+        return J
 
     def set_variant(self, v: int):
         self._check(self._L.sem_set_variant(self._h, v))

@@ -78,6 +78,8 @@ struct sem_ctx {
     int64_t scal_cap = 0;
     double* h_hist = nullptr;
     int hist_n = 0;
+    // ---- p-multigrid transfer (NEXT-1, sem_transfer.cu) ----
+    void* d_J = nullptr;           // [SEM_MAXP^2] interpolation matrix of the last transfer, in its precision
     // ---- misc ----
     int ax_variant = 0;
     std::string err;

@@ -1,0 +1,127 @@
+// sem_transfer.cu — NEXT-1: p-multigrid transfer operators between two discretisations (orders
+// N_c <= N_f) of the same E elements.  P:103: "Coarse-to-fine interpolations are cast as efficient tensor contractions,
+// u_f = (J x J x J) u_c, where J is the 1D polynomial interpolation operator from the coarse GLL points to the fine GLL
+// points ... only a single J matrix (of size N+1 or less) is needed for the entire domain, for each pMG level."
+// Restriction is the transpose, r_c = (J^T x J^T x J^T) r_f.  Element by element, local layout, no gather-scatter.
+//
+// Sum-factorised: three 1-D contractions through shared memory (i, then j, then k), J in shared memory.  The work is
+// tiny and the kernel is bound by the read of p_in^3 and the write of p_out^3 values per element (and, at the paper's
+// E ~ 7000 per GPU, by launch latency), so the orders are run-time values: one kernel for every level pair.
+#include "sem_internal.h"
+
+namespace {
+
+constexpr int TNT = 128;
+
+// dst[o2][o1][o0] = sum over the contracted axis of M * src[n2][n1][n0]; AXIS 0/1/2 = i/j/k (i fastest).
+// TRANSPOSED = false: M = J used as J[out][in] (prolongation);  true: J[in][out] (restriction).  J is [pf][pc].
+template <typename T, int AXIS, bool TRANSPOSED>
+__device__ __forceinline__ void contract(T* __restrict__ dst, const T* __restrict__ src, const T* __restrict__ J, int pc,
+                                         int n0, int n1, int n2, int nin, int nout) {
+    const int o0 = AXIS == 0 ? nout : n0, o1 = AXIS == 1 ? nout : n1, o2 = AXIS == 2 ? nout : n2;
+    const int total = o0 * o1 * o2;
+    const int sstride = AXIS == 0 ? 1 : AXIS == 1 ? n0 : n0 * n1;
+    for (int t = threadIdx.x; t < total; t += TNT) {
+        const int a0 = t % o0, a1 = (t / o0) % o1, a2 = t / (o0 * o1);
+        const int out = AXIS == 0 ? a0 : AXIS == 1 ? a1 : a2;
+        const int base = (AXIS == 0 ? 0 : a0) + n0 * ((AXIS == 1 ? 0 : a1) + n1 * (AXIS == 2 ? 0 : a2));
+        T s = T(0);
+        for (int l = 0; l < nin; ++l) s += (TRANSPOSED ? J[l * pc + out] : J[out * pc + l]) * src[base + l * sstride];
+        dst[t] = s;
+    }
+}
+
+template <typename T, bool RESTRICT>
+__global__ void __launch_bounds__(TNT) k_transfer(int64_t E, int pc, int pf, const T* __restrict__ Jg,
+                                                  const T* __restrict__ in, T* __restrict__ out) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* sJ = reinterpret_cast<T*>(smem_raw);
+    const int pin = RESTRICT ? pf : pc, pout = RESTRICT ? pc : pf;
+    const int big = pf * pf * pf;
+    T* bufA = sJ + ((pf * pc + 3) & ~3);
+    T* bufB = bufA + big;
+    for (int t = threadIdx.x; t < pf * pc; t += TNT) sJ[t] = Jg[t];
+    const int64_t nin3 = (int64_t)pin * pin * pin, nout3 = (int64_t)pout * pout * pout;
+    for (int64_t e = blockIdx.x; e < E; e += gridDim.x) {
+        __syncthreads();                                   // bufA free (and sJ filled, first time round)
+        for (int t = threadIdx.x; t < nin3; t += TNT) bufA[t] = in[e * nin3 + t];
+        __syncthreads();
+        contract<T, 0, RESTRICT>(bufB, bufA, sJ, pc, pin, pin, pin, pin, pout);      // [pin][pin][pout]
+        __syncthreads();
+        contract<T, 1, RESTRICT>(bufA, bufB, sJ, pc, pout, pin, pin, pin, pout);     // [pin][pout][pout]
+        __syncthreads();
+        contract<T, 2, RESTRICT>(out + e * nout3, bufA, sJ, pc, pout, pout, pin, pin, pout);
+    }
+}
+
+// J[i][j] = coarse Lagrange cardinal function j at fine point i, by the barycentric formula (host, long double)
+void interp_matrix(const sem_ctx* cc, const sem_ctx* cf, double* J) {
+    const int pc = cc->p, pf = cf->p;
+    long double wb[SEM_MAXP];
+    for (int j = 0; j < pc; ++j) {
+        long double d = 1.0L;
+        for (int m = 0; m < pc; ++m) if (m != j) d *= (long double)cc->xi[j] - (long double)cc->xi[m];
+        wb[j] = 1.0L / d;
+    }
+    for (int i = 0; i < pf; ++i) {
+        const long double x = cf->xi[i];
+        int hit = -1;
+        for (int j = 0; j < pc; ++j) if (x == (long double)cc->xi[j]) hit = j;
+        if (hit >= 0) {
+            for (int j = 0; j < pc; ++j) J[i * pc + j] = j == hit ? 1.0 : 0.0;
+            continue;
+        }
+        long double den = 0.0L;
+        for (int j = 0; j < pc; ++j) den += wb[j] / (x - (long double)cc->xi[j]);
+        for (int j = 0; j < pc; ++j) J[i * pc + j] = (double)((wb[j] / (x - (long double)cc->xi[j])) / den);
+    }
+}
+
+template <typename T>
+int launch(sem_ctx* cf, int pc, const double* Jh, const void* in, void* out, bool restrict_) {
+    const int pf = cf->p;
+    T hJ[SEM_MAXP * SEM_MAXP];
+    for (int q = 0; q < pf * pc; ++q) hJ[q] = (T)Jh[q];              // S16: computed in double, rounded once
+    T* dJ = (T*)cf->d_J;
+    SEM_CUDA_OK(cf, cudaMemcpyAsync(dJ, hJ, sizeof(T) * pf * pc, cudaMemcpyHostToDevice, cf->stream));
+    const size_t smem = sizeof(T) * (((size_t)(pf * pc + 3) & ~(size_t)3) + 2 * (size_t)pf * pf * pf);
+    auto kern = restrict_ ? k_transfer<T, true> : k_transfer<T, false>;
+    if (smem > 48 * 1024) SEM_CUDA_OK(cf, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int64_t grid = (int64_t)cf->num_sms * 8;
+    if (grid > cf->E) grid = cf->E;
+    kern<<<(unsigned)grid, TNT, smem, cf->stream>>>(cf->E, pc, pf, dJ, (const T*)in, (T*)out);
+    SEM_CUDA_OK(cf, cudaGetLastError());
+    return SEM_OK;
+}
+
+int check_pair(sem_ctx* cc, sem_ctx* cf) {
+    if (!cc || !cf) return SEM_EINVAL;
+    cf->err.clear();
+    if (cc->E != cf->E) return sem_fail(cf, SEM_EINVAL, "sem_transfer: contexts have different element counts");
+    if (cc->N > cf->N) return sem_fail(cf, SEM_EINVAL, "sem_transfer: coarse order exceeds fine order");
+    return SEM_OK;
+}
+
+}  // namespace
+
+extern "C" int sem_get_interp(sem_ctx* coarse, sem_ctx* fine, double* J) {
+    int rc = check_pair(coarse, fine);
+    if (rc) return rc;
+    if (!J) return sem_fail(fine, SEM_EINVAL, "sem_get_interp: NULL buffer");
+    interp_matrix(coarse, fine, J);
+    return SEM_OK;
+}
+
+extern "C" int sem_transfer(sem_ctx* coarse, sem_ctx* fine, const void* in, void* out, sem_prec prec,
+                            sem_transfer_dir dir) {
+    int rc = check_pair(coarse, fine);
+    if (rc) return rc;
+    if (!in || !out || in == out) return sem_fail(fine, SEM_EINVAL, "sem_transfer: NULL or aliased vectors");
+    if (prec != SEM_F64 && prec != SEM_F32) return sem_fail(fine, SEM_EINVAL, "sem_transfer: bad sem_prec");
+    if (dir != SEM_PROLONG && dir != SEM_RESTRICT) return sem_fail(fine, SEM_EINVAL, "sem_transfer: bad direction");
+    if (!fine->d_J) SEM_CUDA_OK(fine, cudaMalloc((void**)&fine->d_J, sizeof(double) * SEM_MAXP * SEM_MAXP));
+    double Jh[SEM_MAXP * SEM_MAXP];
+    interp_matrix(coarse, fine, Jh);
+    if (prec == SEM_F64) return launch<double>(fine, coarse->p, Jh, in, out, dir == SEM_RESTRICT);
+    return launch<float>(fine, coarse->p, Jh, in, out, dir == SEM_RESTRICT);
+}

@@ -455,3 +455,41 @@ def test_pcg_helmholtz(torch_cuda, binding, oracle_mod):
         it, rel = sem.pcg(b, x, 1e-9, 300)
         assert it == ores["iters"]
         assert relerr(x.cpu().numpy(), ores["x"][om.l2u]) <= TOLPCG
+
+
+# ------------------------------------------------------------------------------------ NEXT-1: pMG transfer
+@pytest.mark.parametrize("Nc,Nf", [(1, 3), (3, 7), (1, 7), (5, 8), (7, 7), (2, 5), (9, 15)])
+def test_transfer_parity(torch_cuda, binding, oracle_mod, Nc, Nf):
+    """sem_transfer against the oracle: interpolation matrix, prolongation and restriction, FP64 (1e-12) and FP32
+    (1e-5), on a mesh with more elements than resident CTAs of the kernel."""
+    nx, ny, nz = (13, 12, 11) if Nf <= 8 else (5, 4, 3)
+    mc, mf = inputs.box_mesh(nx, ny, nz, Nc, "smooth"), inputs.box_mesh(nx, ny, nz, Nf, "smooth")
+    uc = inputs.field_normal(mc.gid, 2)
+    rf = inputs.field_uniform(mf.gid, 5) * (1.0 + np.arange(mf.E)[:, None] % 7)      # not continuous on purpose
+    o_p, o_r = oracle_mod.prolong(uc, Nc, Nf), oracle_mod.restrict(rf, Nc, Nf)
+    with binding.Sem(mc.E, Nc, mc.vert, mc.gid) as sc, binding.Sem(mf.E, Nf, mf.vert, mf.gid) as sf:
+        assert np.max(np.abs(sc.interp(sf) - oracle_mod.interp(Nc, Nf))) <= 1e-14
+        for dt, tol in ((torch_cuda.float64, TOL64), (torch_cuda.float32, TOL32)):
+            d_uc, d_rf = to_dev(torch_cuda, uc.ravel(), dt), to_dev(torch_cuda, rf.ravel(), dt)
+            d_uf = torch_cuda.full((mf.nL,), float("nan"), dtype=dt, device="cuda")
+            d_rc = torch_cuda.full((mc.nL,), float("nan"), dtype=dt, device="cuda")
+            sc.transfer(sf, d_uc, d_uf, binding.SEM_PROLONG)
+            sc.transfer(sf, d_rf, d_rc, binding.SEM_RESTRICT)
+            assert relerr(d_uf.cpu().numpy(), o_p.ravel()) <= tol, (Nc, Nf, dt)
+            assert relerr(d_rc.cpu().numpy(), o_r.ravel()) <= tol, (Nc, Nf, dt)
+
+
+def test_transfer_bad_args(torch_cuda, binding):
+    m3, m7, other = inputs.box_mesh(2, 2, 2, 3), inputs.box_mesh(2, 2, 2, 7), inputs.box_mesh(3, 2, 2, 3)
+    with binding.Sem(m3.E, 3, m3.vert, m3.gid) as s3, binding.Sem(m7.E, 7, m7.vert, m7.gid) as s7, \
+            binding.Sem(other.E, 3, other.vert, other.gid) as so:
+        a = torch_cuda.zeros(m3.nL, dtype=torch_cuda.float64, device="cuda")
+        b = torch_cuda.zeros(m7.nL, dtype=torch_cuda.float64, device="cuda")
+        with pytest.raises(binding.SemError) as e:
+            s7.transfer(s3, b, a, binding.SEM_PROLONG)            # coarse order exceeds fine order
+        assert e.value.code == binding.SEM_EINVAL
+        with pytest.raises(binding.SemError) as e:
+            so.transfer(s7, torch_cuda.zeros(other.nL, dtype=torch_cuda.float64, device="cuda"), b, binding.SEM_PROLONG)   # different meshes
+        assert e.value.code == binding.SEM_EINVAL
+        with pytest.raises(binding.SemError):
+            s3.transfer(s7, a, b, 7)                              # bad direction
