@@ -80,6 +80,7 @@ struct sem_ctx {
     int hist_n = 0;
     // ---- p-multigrid transfer (NEXT-1, sem_transfer.cu) ----
     void* d_J = nullptr;           // [SEM_MAXP^2] interpolation matrix of the last transfer, in its precision
+    int J_key = -1;                // (coarse p) * 2 + (FP32 ? 1 : 0) of what d_J holds
     // ---- misc ----
     int ax_variant = 0;
     std::string err;

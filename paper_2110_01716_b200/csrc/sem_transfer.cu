@@ -13,44 +13,57 @@ namespace {
 
 constexpr int TNT = 128;
 
-// dst[o2][o1][o0] = sum over the contracted axis of M * src[n2][n1][n0]; AXIS 0/1/2 = i/j/k (i fastest).
-// TRANSPOSED = false: M = J used as J[out][in] (prolongation);  true: J[in][out] (restriction).  J is [pf][pc].
+// For each of `ne` elements (element strides es_dst / es_src):  dst[o2][o1][o0] = sum over the contracted axis of
+// M * src[n2][n1][n0];  AXIS 0/1/2 = i/j/k (i fastest).  TRANSPOSED = false: M = J used as J[out][in] (prolongation);
+// true: J[in][out] (restriction).  J is [pf][pc].
 template <typename T, int AXIS, bool TRANSPOSED>
-__device__ __forceinline__ void contract(T* __restrict__ dst, const T* __restrict__ src, const T* __restrict__ J, int pc,
-                                         int n0, int n1, int n2, int nin, int nout) {
+__device__ __forceinline__ void contract(T* __restrict__ dst, int64_t es_dst, const T* __restrict__ src, int es_src,
+                                         const T* __restrict__ J, int pc, int ne, int n0, int n1, int n2, int nin,
+                                         int nout) {
     const int o0 = AXIS == 0 ? nout : n0, o1 = AXIS == 1 ? nout : n1, o2 = AXIS == 2 ? nout : n2;
-    const int total = o0 * o1 * o2;
+    const int per = o0 * o1 * o2, total = per * ne;
     const int sstride = AXIS == 0 ? 1 : AXIS == 1 ? n0 : n0 * n1;
     for (int t = threadIdx.x; t < total; t += TNT) {
-        const int a0 = t % o0, a1 = (t / o0) % o1, a2 = t / (o0 * o1);
+        const int el = t / per, q = t - el * per;
+        const int a0 = q % o0, a1 = (q / o0) % o1, a2 = q / (o0 * o1);
         const int out = AXIS == 0 ? a0 : AXIS == 1 ? a1 : a2;
-        const int base = (AXIS == 0 ? 0 : a0) + n0 * ((AXIS == 1 ? 0 : a1) + n1 * (AXIS == 2 ? 0 : a2));
+        const T* sp = src + el * es_src + (AXIS == 0 ? 0 : a0) + n0 * ((AXIS == 1 ? 0 : a1) + n1 * (AXIS == 2 ? 0 : a2));
+        const T* jp = TRANSPOSED ? J + out : J + out * pc;
+        const int jstride = TRANSPOSED ? pc : 1;
         T s = T(0);
-        for (int l = 0; l < nin; ++l) s += (TRANSPOSED ? J[l * pc + out] : J[out * pc + l]) * src[base + l * sstride];
-        dst[t] = s;
+        for (int l = 0; l < nin; ++l) s += jp[l * jstride] * sp[l * sstride];
+        dst[el * es_dst + q] = s;
     }
 }
 
-template <typename T, bool RESTRICT>
-__global__ void __launch_bounds__(TNT) k_transfer(int64_t E, int pc, int pf, const T* __restrict__ Jg,
+// One CTA works on `epc` consecutive elements at a time so that small orders still fill its threads.
+// PC, PF > 0: the level pair is known at compile time (index arithmetic folds, loops unroll); 0: run-time orders.
+template <typename T, bool RESTRICT, int PC, int PF>
+__global__ void __launch_bounds__(TNT) k_transfer(int64_t E, int pc_rt, int pf_rt, int epc_rt, const T* __restrict__ Jg,
                                                   const T* __restrict__ in, T* __restrict__ out) {
+    const int pc = PC > 0 ? PC : pc_rt, pf = PF > 0 ? PF : pf_rt;
+    const int epc = PF > 0 ? (TNT / (PF * PF) > 0 ? TNT / (PF * PF) : 1) : epc_rt;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T* sJ = reinterpret_cast<T*>(smem_raw);
     const int pin = RESTRICT ? pf : pc, pout = RESTRICT ? pc : pf;
     const int big = pf * pf * pf;
     T* bufA = sJ + ((pf * pc + 3) & ~3);
-    T* bufB = bufA + big;
+    T* bufB = bufA + epc * big;
     for (int t = threadIdx.x; t < pf * pc; t += TNT) sJ[t] = Jg[t];
-    const int64_t nin3 = (int64_t)pin * pin * pin, nout3 = (int64_t)pout * pout * pout;
-    for (int64_t e = blockIdx.x; e < E; e += gridDim.x) {
+    const int nin3 = pin * pin * pin;
+    const int64_t nout3 = (int64_t)pout * pout * pout;
+    const int64_t ngrp = (E + epc - 1) / epc;
+    for (int64_t g = blockIdx.x; g < ngrp; g += gridDim.x) {
+        const int64_t e0 = g * epc;
+        const int ne = (int)(E - e0 < epc ? E - e0 : epc);
         __syncthreads();                                   // bufA free (and sJ filled, first time round)
-        for (int t = threadIdx.x; t < nin3; t += TNT) bufA[t] = in[e * nin3 + t];
+        for (int t = threadIdx.x; t < ne * nin3; t += TNT) bufA[t] = in[e0 * nin3 + t];     // contiguous elements
         __syncthreads();
-        contract<T, 0, RESTRICT>(bufB, bufA, sJ, pc, pin, pin, pin, pin, pout);      // [pin][pin][pout]
+        contract<T, 0, RESTRICT>(bufB, big, bufA, nin3, sJ, pc, ne, pin, pin, pin, pin, pout);      // [pin][pin][pout]
         __syncthreads();
-        contract<T, 1, RESTRICT>(bufA, bufB, sJ, pc, pout, pin, pin, pin, pout);     // [pin][pout][pout]
+        contract<T, 1, RESTRICT>(bufA, big, bufB, big, sJ, pc, ne, pout, pin, pin, pin, pout);      // [pin][pout][pout]
         __syncthreads();
-        contract<T, 2, RESTRICT>(out + e * nout3, bufA, sJ, pc, pout, pout, pin, pin, pout);
+        contract<T, 2, RESTRICT>(out + e0 * nout3, nout3, bufA, big, sJ, pc, ne, pout, pout, pin, pin, pout);
     }
 }
 
@@ -80,16 +93,30 @@ void interp_matrix(const sem_ctx* cc, const sem_ctx* cf, double* J) {
 template <typename T>
 int launch(sem_ctx* cf, int pc, const double* Jh, const void* in, void* out, bool restrict_) {
     const int pf = cf->p;
-    T hJ[SEM_MAXP * SEM_MAXP];
-    for (int q = 0; q < pf * pc; ++q) hJ[q] = (T)Jh[q];              // S16: computed in double, rounded once
-    T* dJ = (T*)cf->d_J;
-    SEM_CUDA_OK(cf, cudaMemcpyAsync(dJ, hJ, sizeof(T) * pf * pc, cudaMemcpyHostToDevice, cf->stream));
-    const size_t smem = sizeof(T) * (((size_t)(pf * pc + 3) & ~(size_t)3) + 2 * (size_t)pf * pf * pf);
-    auto kern = restrict_ ? k_transfer<T, true> : k_transfer<T, false>;
+    const int key = pc * 2 + (sizeof(T) == 8 ? 0 : 1);
+    if (cf->J_key != key) {                       // the matrix on the device is for another level pair / precision
+        T hJ[SEM_MAXP * SEM_MAXP];
+        for (int q = 0; q < pf * pc; ++q) hJ[q] = (T)Jh[q];          // S16: computed in double, rounded once
+        SEM_CUDA_OK(cf, cudaStreamSynchronize(cf->stream));          // earlier transfers may still read the old one
+        SEM_CUDA_OK(cf, cudaMemcpy(cf->d_J, hJ, sizeof(T) * pf * pc, cudaMemcpyHostToDevice));
+        cf->J_key = key;
+    }
+    int epc = TNT / (pf * pf);
+    if (epc < 1) epc = 1;
+    const size_t smem = sizeof(T) * (((size_t)(pf * pc + 3) & ~(size_t)3) + 2 * (size_t)epc * pf * pf * pf);
+    // the level pairs of config 4 (N = 7-3-1) and of the paper's schedules 8-5-1 and 8-6-4-1 are specialised
+    using kern_t = void (*)(int64_t, int, int, int, const T*, const T*, T*);
+    kern_t kern = restrict_ ? k_transfer<T, true, 0, 0> : k_transfer<T, false, 0, 0>;
+#define SEM_TR_CASE(A, B) \
+    if (pc == A && pf == B) kern = restrict_ ? k_transfer<T, true, A, B> : k_transfer<T, false, A, B>;
+    SEM_TR_CASE(2, 4) SEM_TR_CASE(4, 8) SEM_TR_CASE(2, 8) SEM_TR_CASE(2, 6) SEM_TR_CASE(6, 9) SEM_TR_CASE(2, 5)
+    SEM_TR_CASE(5, 7) SEM_TR_CASE(7, 9)
+#undef SEM_TR_CASE
     if (smem > 48 * 1024) SEM_CUDA_OK(cf, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int64_t ngrp = (cf->E + epc - 1) / epc;
     int64_t grid = (int64_t)cf->num_sms * 8;
-    if (grid > cf->E) grid = cf->E;
-    kern<<<(unsigned)grid, TNT, smem, cf->stream>>>(cf->E, pc, pf, dJ, (const T*)in, (T*)out);
+    if (grid > ngrp) grid = ngrp;
+    kern<<<(unsigned)grid, TNT, smem, cf->stream>>>(cf->E, pc, pf, epc, (const T*)cf->d_J, (const T*)in, (T*)out);
     SEM_CUDA_OK(cf, cudaGetLastError());
     return SEM_OK;
 }

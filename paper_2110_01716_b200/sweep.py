@@ -94,6 +94,22 @@ def main():
     if args.levels:
         for N in (7, 3, 1):
             run_case(inputs.config4(N), torch.float32, peak, "cfg4 20x20x18 f32")
+        # NEXT-1: transfers between config 4's levels, FP32; bytes = one read of the input + one write of the output
+        print()
+        print("| transfer (FP32, E = 7200) | us | GB/s | frac of peak |")
+        print("|---|---|---|---|")
+        sems = {N: binding.Sem(m.E, N, m.vert, m.gid) for N, m in ((N, inputs.config4(N)) for N in (7, 3, 1))}
+        for Nc, Nf in ((3, 7), (1, 3)):
+            sc, sf = sems[Nc], sems[Nf]
+            vc = torch.randn(sc.nL, device="cuda", dtype=torch.float32)
+            vf = torch.randn(sf.nL, device="cuda", dtype=torch.float32)
+            for name, fn in ((f"prolong {Nc}->{Nf}", lambda: sc.transfer(sf, vc, vf, binding.SEM_PROLONG)),
+                             (f"restrict {Nf}->{Nc}", lambda: sc.transfer(sf, vf, vc, binding.SEM_RESTRICT))):
+                t = _time(fn, 2000)
+                gbs = 4.0 * (sc.nL + sf.nL) / t / 1e3
+                print(f"| {name} | {t:.2f} | {gbs:.0f} | {gbs / peak:.2f} |", flush=True)
+        for s_ in sems.values():
+            s_.close()
 
 
 if __name__ == "__main__":
