@@ -195,3 +195,14 @@ def restrict(rf: np.ndarray, Nc: int, Nf: int) -> np.ndarray:
     rc = np.empty((rf.shape[0], (Nc + 1) ** 3))
     assert lib().orc_restrict(C.c_int64(rf.shape[0]), C.c_int(Nc), C.c_int(Nf), _p(rf), _p(rc)) == 0
     return rc
+
+
+def cheby(G, N, maps: Maps, mask_u, b_u, x0_u, order: int, lmin: float, lmax: float, lam=0.0) -> np.ndarray:
+    """Chebyshev-accelerated point-Jacobi smoother (reading S23), `order` steps, unique storage; returns x."""
+    G, b_u = _f64(G), _f64(b_u)
+    x = np.zeros(maps.U) if x0_u is None else _f64(x0_u).copy()
+    mask_u = np.ascontiguousarray(mask_u, np.uint8)
+    rc = lib().orc_cheby(C.c_int64(G.shape[0]), C.c_int(N), _p(G), C.c_double(lam), C.c_int64(maps.nL), C.c_int64(maps.U),
+                         _p(maps.l2u), _p(mask_u), _p(b_u), _p(x), C.c_int(order), C.c_double(lmin), C.c_double(lmax))
+    assert rc == 0
+    return x

@@ -484,4 +484,45 @@ int orc_restrict(int64_t E, int Nc, int Nf, const double* rf, double* rc) {
     return 0;
 }
 
+// ---- NEXT-1: Chebyshev-accelerated point-Jacobi smoother ("Smoothers for pMG include Chebyshev-accelerated
+// point-Jacobi") ---------------------------------------------------------------------------------------------------
+// The paper names the smoother and nothing else (reading S23): this is the textbook Chebyshev semi-iteration
+// (Saad, Iterative Methods, Alg. 12.1) on the Jacobi-preconditioned operator M^-1 A with M = diag(A), for eigenvalue
+// bounds [lmin, lmax] of M^-1 A supplied by the caller:
+//   theta = (lmax+lmin)/2, delta = (lmax-lmin)/2, sigma = theta/delta, rho_0 = 1/sigma
+//   r = M^-1 (b - A x);  d = r / theta
+//   for k = 1 .. order-1:  x += d;  r -= M^-1 A d;  rho_k = 1/(2 sigma - rho_{k-1});
+//                          d = rho_k rho_{k-1} d + (2 rho_k / delta) r
+//   x += d
+// so `order` applications of M^-1 are made and the error is multiplied by T_order((theta - t)/delta)/T_order(sigma) on
+// the eigenvalue t of M^-1 A.  Unique storage; A = masked assembled operator (O8), b assembled and masked.
+int orc_cheby(int64_t E, int N, const double* G, double lambda, int64_t nL, int64_t U, const int32_t* l2u,
+              const uint8_t* mask_u, const double* b, double* x, int order, double lmin, double lmax) {
+    if (order < 1 || !(lmax > lmin) || !(lmin > 0.0)) return -1;
+    std::vector<double> uL(nL), wL(nL), diagL(nL), Minv(U, 0.0), r(U), d(U), q(U);
+    orc_diag_local(E, N, G, diagL.data(), lambda);
+    {
+        std::vector<double> dg(U, 0.0);
+        for (int64_t l = 0; l < nL; ++l) dg[l2u[l]] += diagL[l];
+        for (int64_t g = 0; g < U; ++g) Minv[g] = mask_u[g] ? 0.0 : 1.0 / dg[g];
+    }
+    const double theta = 0.5 * (lmax + lmin), delta = 0.5 * (lmax - lmin), sigma = theta / delta;
+    double rho = 1.0 / sigma;
+    for (int64_t g = 0; g < U; ++g) if (mask_u[g]) x[g] = 0.0;
+    apply_Ag(E, N, G, lambda, nL, U, l2u, mask_u, x, q.data(), uL.data(), wL.data());
+    for (int64_t g = 0; g < U; ++g) { r[g] = Minv[g] * (b[g] - q[g]); d[g] = r[g] / theta; }
+    for (int k = 1; k < order; ++k) {
+        for (int64_t g = 0; g < U; ++g) x[g] += d[g];
+        apply_Ag(E, N, G, lambda, nL, U, l2u, mask_u, d.data(), q.data(), uL.data(), wL.data());
+        const double rho1 = 1.0 / (2.0 * sigma - rho);
+        for (int64_t g = 0; g < U; ++g) {
+            r[g] -= Minv[g] * q[g];
+            d[g] = rho1 * rho * d[g] + (2.0 * rho1 / delta) * r[g];
+        }
+        rho = rho1;
+    }
+    for (int64_t g = 0; g < U; ++g) x[g] += d[g];
+    return 0;
+}
+
 }  // extern "C"

@@ -507,3 +507,72 @@ def test_T4_restriction_is_the_adjoint(oracle_mod, Nc, Nf):
     J = oracle_mod.interp(Nc, Nf)
     M = J.T @ J
     assert np.max(np.abs(oracle_mod.restrict(oracle_mod.prolong(uc, Nc, Nf), Nc, Nf) - uc @ np.kron(M, np.kron(M, M)).T)) <= 1e-12
+
+
+# ------------------------------------------------------------------------- NEXT-1: Chebyshev-Jacobi smoother
+def _dense_masked_operator(oracle_mod, m):
+    om = oracle_mod.Maps(m.gid)
+    G, _, _ = oracle_mod.geom_trilinear(m.vert, m.N)
+    mask_u = oracle_mod.mask_unique(m.dirichlet, om)
+    A = np.stack([oracle_mod.apply_Ag(G, m.N, om, mask_u, e) for e in np.eye(om.U)], axis=1)
+    return om, G, mask_u, A
+
+
+def test_C1_chebyshev_error_polynomial(oracle_mod):
+    """The smoother's error propagation is the scaled Chebyshev polynomial T_k((theta - t)/delta) / T_k(sigma) of
+    M^-1 A (the definition of the method, Saad Alg. 12.1): checked against the dense matrix of a tiny mesh, built from
+    numpy's Chebyshev class -- no code shared with the oracle's three-term recurrence."""
+    m = inputs.box_mesh(2, 2, 2, 3, "random", seed=5)
+    om, G, mask_u, A = _dense_masked_operator(oracle_mod, m)
+    free = mask_u == 0
+    Af = A[np.ix_(free, free)]
+    Dinv = 1.0 / np.diag(Af)
+    lam_all = np.linalg.eigvals(Dinv[:, None] * Af).real
+    lmax, lmin = 1.1 * lam_all.max(), 0.1 * lam_all.max()
+    theta, delta = (lmax + lmin) / 2, (lmax - lmin) / 2
+    rng = np.random.default_rng(1)
+    xs = np.zeros(om.U); xs[free] = rng.standard_normal(free.sum())
+    b = oracle_mod.apply_Ag(G, m.N, om, mask_u, xs)
+    x0 = np.zeros(om.U); x0[free] = rng.standard_normal(free.sum())
+    B = np.eye(free.sum()) - 0.0                                   # error e_k = p_k(M^-1 A) e_0
+    MA = Dinv[:, None] * Af
+    for order in (1, 2, 3, 5):
+        xk = oracle_mod.cheby(G, m.N, om, mask_u, b, x0, order, lmin, lmax)
+        Tk = np.polynomial.chebyshev.Chebyshev.basis(order)
+        # evaluate p_k(MA) through the eigen-decomposition of the (similar to symmetric) matrix
+        w, V = np.linalg.eig(MA)
+        pk = (V * (Tk((theta - w.real) / delta) / Tk(theta / delta))) @ np.linalg.inv(V)
+        e_expected = (pk @ (x0 - xs)[free]).real
+        assert np.max(np.abs((xk - xs)[free] - e_expected)) <= 1e-10 * np.max(np.abs(e_expected)), order
+        assert np.all(xk[~free] == 0.0)
+    # order 1 is damped Jacobi with weight 1/theta (closed form)
+    x1 = oracle_mod.cheby(G, m.N, om, mask_u, b, x0, 1, lmin, lmax)
+    r0 = np.zeros(om.U); r0[free] = Dinv * (b - oracle_mod.apply_Ag(G, m.N, om, mask_u, x0))[free]
+    assert np.max(np.abs(x1 - (x0 + r0 / theta))) <= 1e-14
+
+
+def test_C2_chebyshev_damps_the_upper_spectrum(oracle_mod):
+    """On a down-sized smooth mesh with bounds [lmax/10, 1.1 lmax]: in the basis of the generalised eigenvectors
+    A v = t M v (A- and M-orthogonal), every error component with t inside the bounds is damped by at least
+    1/T_k(sigma) -- the min-max property that makes it a smoother -- and no component below them is amplified."""
+    import scipy.linalg
+    m = inputs.box_mesh(3, 3, 3, 3, "smooth")
+    om, G, mask_u, A = _dense_masked_operator(oracle_mod, m)
+    free = mask_u == 0
+    Af = A[np.ix_(free, free)]
+    Af = 0.5 * (Af + Af.T)
+    t, V = scipy.linalg.eigh(Af, np.diag(np.diag(Af)))           # V^T M V = I
+    lmax, lmin = 1.1 * t.max(), 0.11 * t.max()
+    sigma = (lmax + lmin) / (lmax - lmin)
+    rng = np.random.default_rng(3)
+    xs = np.zeros(om.U); xs[free] = rng.standard_normal(free.sum())
+    b = oracle_mod.apply_Ag(G, m.N, om, mask_u, xs)
+    c0 = V.T @ (np.diag(Af) * (0.0 - xs[free]))                  # coefficients of e_0 = x_0 - x* in the basis V
+    inside = t >= lmin
+    assert inside.sum() > 10 and (~inside).sum() > 3
+    for order in (1, 2, 4, 8):
+        e = (oracle_mod.cheby(G, m.N, om, mask_u, b, None, order, lmin, lmax) - xs)[free]
+        ck = V.T @ (np.diag(Af) * e)
+        bound = 1.0 / np.polynomial.chebyshev.Chebyshev.basis(order)(sigma)
+        assert np.all(np.abs(ck[inside]) <= bound * np.abs(c0[inside]) * (1 + 1e-9) + 1e-13), order
+        assert np.all(np.abs(ck[~inside]) <= np.abs(c0[~inside]) * (1 + 1e-9) + 1e-13), order
