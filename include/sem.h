@@ -128,6 +128,18 @@ SEM_API int sem_transfer(sem_ctx* coarse, sem_ctx* fine, const void* in, void* o
 /* Parity accessor: the interpolation matrix J, [pf][pc] doubles, HOST. */
 SEM_API int sem_get_interp(sem_ctx* coarse, sem_ctx* fine, double* J);
 
+/* NEXT-1.  Chebyshev-accelerated point-Jacobi smoother, `order` steps on
+ * M QQ^T (D^T G D + lambda B) M with the exact Jacobi diagonal (O7), for eigenvalue bounds [lmin, lmax] of diag^-1 A
+ * given by the caller (reading S23 in DESIGN.md; the recurrence is written out in csrc/sem_cheby.cu):
+ *   x <- x + p(diag^-1 A) diag^-1 (b - A x),  error multiplied by T_order((theta - t)/delta) / T_order(theta/delta)
+ *   b, x        DEVICE, local layout, continuous, `prec` values; b assembled; x: in = initial guess (masked on entry),
+ *               out = smoothed iterate; must not alias; x 16-byte aligned
+ *   zero_guess  != 0: x is taken as 0 and not read (saves one operator application)
+ * `order` operator applications (order - 1 with zero_guess).  Asynchronous on the context's stream.
+ * SEM_EINVAL for order < 1 or bounds not 0 < lmin < lmax. */
+SEM_API int sem_cheby(sem_ctx* ctx, const void* b, void* x, int order, double lmin, double lmax, int zero_guess,
+                      sem_prec prec);
+
 /* Tuning knob for experiments: selects the Ax kernel variant (0 = default streaming kernel, 1 = simple kernel). */
 SEM_API int sem_set_variant(sem_ctx* ctx, int ax_variant);
 

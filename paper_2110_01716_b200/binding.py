@@ -40,6 +40,7 @@ SYMBOLS = {
     "sem_set_variant": (_i32, [_vp, _i32]),
     "sem_transfer": (_i32, [_vp, _vp, _vp, _vp, _i32, _i32]),
     "sem_get_interp": (_i32, [_vp, _vp, _vp]),
+    "sem_cheby": (_i32, [_vp, _vp, _vp, _i32, _dbl, _dbl, _i32, _i32]),
     "sem_last_error": (C.c_char_p, [_vp]),
     "sem_ctx_destroy": (None, [_vp]),
 }
@@ -190,6 +191,11 @@ class Sem:
         if rc != SEM_OK:
             raise SemError(rc, self._L.sem_last_error(fine._h).decode())
         return J
+
+    def cheby(self, b, x, order: int, lmin: float, lmax: float, zero_guess: bool = False):
+        self._check(self._L.sem_cheby(self._h, self._vec(b), self._vec(x), order, lmin, lmax, int(zero_guess),
+                                      self._prec(x)))
+        return x
 
     def set_variant(self, v: int):
         self._check(self._L.sem_set_variant(self._h, v))

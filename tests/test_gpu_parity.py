@@ -493,3 +493,60 @@ def test_transfer_bad_args(torch_cuda, binding):
         assert e.value.code == binding.SEM_EINVAL
         with pytest.raises(binding.SemError):
             s3.transfer(s7, a, b, 7)                              # bad direction
+
+
+# ------------------------------------------------------------------------ NEXT-1: Chebyshev-Jacobi smoother
+def _lmax_power(oracle_mod, G, N, om, mask_u, its=12):
+    """Largest eigenvalue of diag^-1 A by power iteration, on the oracle side (the bounds are inputs of the smoother)."""
+    dg = np.zeros(om.U)
+    np.add.at(dg, om.l2u, oracle_mod.diag_local(G, N).ravel())
+    Minv = np.where(mask_u != 0, 0.0, 1.0 / dg)
+    v = np.where(mask_u != 0, 0.0, np.cos(np.arange(om.U) * 0.37))
+    lam = 1.0
+    for _ in range(its):
+        w = Minv * oracle_mod.apply_Ag(G, N, om, mask_u, v)
+        lam = float(np.linalg.norm(w) / np.linalg.norm(v))
+        v = w / np.linalg.norm(w)
+    return lam
+
+
+@pytest.mark.parametrize("N,order,zero_guess", [(7, 1, False), (7, 2, True), (7, 4, False), (3, 3, True), (1, 2, False),
+                                                (5, 6, False)])
+def test_cheby_parity(torch_cuda, binding, oracle_mod, N, order, zero_guess):
+    m = inputs.box_mesh(5, 4, 3, N, "smooth")
+    om, oG, mask_u = _pcg_setup(oracle_mod, m)
+    lmax = 1.1 * _lmax_power(oracle_mod, oG, N, om, mask_u)
+    lmin = 0.1 * lmax
+    xs = np.where(mask_u != 0, 0.0, inputs.field_normal(om.uniq_gid, 4))
+    b_u = oracle_mod.apply_Ag(oG, N, om, mask_u, xs)
+    x0_u = None if zero_guess else np.where(mask_u != 0, 0.0, inputs.field_uniform(om.uniq_gid, 6))
+    ox = oracle_mod.cheby(oG, N, om, mask_u, b_u, x0_u, order, lmin, lmax)[om.l2u]
+    with make_sem(binding, m, dirichlet=True) as sem:
+        for dt, tol in ((torch_cuda.float64, TOL64), (torch_cuda.float32, TOL32)):
+            b = to_dev(torch_cuda, b_u[om.l2u], dt)
+            # with zero_guess the content of x must not matter; otherwise a nonzero guess that is NOT masked on entry
+            x = torch_cuda.full_like(b, 3.0) if zero_guess else to_dev(torch_cuda, x0_u[om.l2u] + (mask_u[om.l2u] != 0), dt)
+            sem.cheby(b, x, order, lmin, lmax, zero_guess)
+            assert relerr(x.cpu().numpy(), ox) <= tol, (N, order, dt)
+        with pytest.raises(binding.SemError):
+            sem.cheby(b, x, 0, lmin, lmax)
+        with pytest.raises(binding.SemError):
+            sem.cheby(b, x, 2, lmax, lmin)
+
+
+def test_cheby_smooths(torch_cuda, binding, oracle_mod):
+    """What the smoother is for: on config 1 the FP32 smoother of order 4 reduces the energy norm of a rough error by
+    more than the min-max bound 1/T_4(sigma) guarantees for the upper 90 % of the spectrum (loose, property check)."""
+    m = inputs.config1()
+    om, oG, mask_u = _pcg_setup(oracle_mod, m)
+    lmax = 1.1 * _lmax_power(oracle_mod, oG, m.N, om, mask_u)
+    rough = np.where(mask_u != 0, 0.0, inputs.field_uniform(om.uniq_gid, 8))          # white noise: mostly high modes
+    b_u = np.zeros(om.U)                                                               # solve A x = 0 from x0 = rough
+    with make_sem(binding, m, dirichlet=True) as sem:
+        b = to_dev(torch_cuda, b_u[om.l2u], torch_cuda.float32)
+        x = to_dev(torch_cuda, rough[om.l2u], torch_cuda.float32)
+        sem.cheby(b, x, 4, 0.1 * lmax, lmax)
+        e1 = np.zeros(om.U)
+        e1[om.l2u] = x.cpu().numpy().astype(np.float64)
+    en = lambda e: float(e @ oracle_mod.apply_Ag(oG, m.N, om, mask_u, e))
+    assert en(e1) < 0.25 * en(rough)
