@@ -108,6 +108,20 @@ def main():
                 t = _time(fn, 2000)
                 gbs = 4.0 * (sc.nL + sf.nL) / t / 1e3
                 print(f"| {name} | {t:.2f} | {gbs:.0f} | {gbs / peak:.2f} |", flush=True)
+        # NEXT-1: Chebyshev-Jacobi smoother, FP32, zero initial guess: order - 1 operator applications + order fused
+        # vector kernels; bytes = (order-1) x (Ax+gs) + vector traffic (init 16, step 32, final 12 B/node incl. Minv FP64)
+        print()
+        print("| smoother (FP32, E = 7200, zero guess) | us | us per operator application |")
+        print("|---|---|---|")
+        for N in (7, 3, 1):
+            m = inputs.config4(N)
+            with binding.Sem(m.E, N, m.vert, m.gid, m.dirichlet) as sd:
+                sd.geom()
+                b = torch.randn(sd.nL, device="cuda", dtype=torch.float32)
+                x = torch.zeros_like(b)
+                for order in (2, 4):
+                    t = _time(lambda: sd.cheby(b, x, order, 0.2, 2.2, True), 500)
+                    print(f"| N = {N}, order {order} | {t:.1f} | {t / (order - 1):.1f} |", flush=True)
         for s_ in sems.values():
             s_.close()
 
