@@ -206,3 +206,63 @@ def cheby(G, N, maps: Maps, mask_u, b_u, x0_u, order: int, lmin: float, lmax: fl
                          _p(maps.l2u), _p(mask_u), _p(b_u), _p(x), C.c_int(order), C.c_double(lmin), C.c_double(lmax))
     assert rc == 0
     return x
+
+
+# ---- NEXT-1c: p-multigrid V-cycle preconditioner -------------------------------------------
+class Level:
+    """One p-multigrid level: its own discretisation of order N on the same elements (S17)."""
+
+    def __init__(self, mesh, lmin_frac: float = 0.1, lmax_safety: float = 1.1, power_its: int = 60):
+        self.N = mesh.N
+        self.maps = Maps(mesh.gid)
+        self.G, _, rc = geom_trilinear(mesh.vert, mesh.N)
+        assert rc == 0
+        self.mask_u = mask_unique(mesh.dirichlet, self.maps)
+        dg = np.zeros(self.maps.U)
+        np.add.at(dg, self.maps.l2u, diag_local(self.G, self.N).ravel())
+        self.Minv = np.where(self.mask_u != 0, 0.0, 1.0 / dg)
+        # eigenvalue bounds of diag^-1 A for the smoother (S23): power iteration x safety, lmin = fraction of lmax
+        # (a rough start vector: an under-estimate of lmax would make the smoother amplify the modes above it)
+        v = np.where(self.mask_u != 0, 0.0, np.cos(np.arange(self.maps.U) ** 2 * 1.7))
+        lam = 1.0
+        for _ in range(power_its):
+            w = self.Minv * self.A(v)
+            lam = float(np.linalg.norm(w) / np.linalg.norm(v))
+            v = w / np.linalg.norm(w)
+        self.lmax = lmax_safety * lam
+        self.lmin = lmin_frac * self.lmax
+
+    def A(self, x_u):
+        return apply_Ag(self.G, self.N, self.maps, self.mask_u, x_u)
+
+    def smooth(self, b_u, x0_u, order):
+        return cheby(self.G, self.N, self.maps, self.mask_u, b_u, x0_u, order, self.lmin, self.lmax)
+
+
+def vcycle(levels, r_u, smooth_order: int, coarse_order: int, lvl: int = 0):
+    """z = M^-1 r, one V-cycle (reading S25 in DESIGN.md; the paper gives the ingredients, not the cycle):
+        coarsest level:  z = Chebyshev-Jacobi(A, r, coarse_order steps, zero guess)       (stands in for the AMG solve)
+        otherwise:       z   = smooth(A, r, zero guess)
+                         res = r - A z
+                         r_c = M_c Q_c^T J^T (W res)     W = 1/multiplicity on the local copies (un-assembly)
+                         z  += J e_c,  e_c = vcycle(r_c)
+                         z   = smooth(A, r, guess z)
+    Unique storage on every level; J = element-wise (J x J x J) between the two levels' local layouts."""
+    L = levels[lvl]
+    if lvl == len(levels) - 1:
+        return L.smooth(r_u, None, coarse_order)
+    C_ = levels[lvl + 1]
+    z = L.smooth(r_u, None, smooth_order)
+    res = r_u - L.A(z)
+    res[L.mask_u != 0] = 0.0
+    res_L = (res / L.maps.mult)[L.maps.l2u]                         # each copy carries 1/mult of the functional
+    rc_L = restrict(res_L.reshape(-1, (L.N + 1) ** 3), C_.N, L.N).ravel()
+    r_c = np.zeros(C_.maps.U)
+    np.add.at(r_c, C_.maps.l2u, rc_L)                               # Q_c^T
+    r_c[C_.mask_u != 0] = 0.0
+    e_c = vcycle(levels, r_c, smooth_order, coarse_order, lvl + 1)
+    e_L = prolong(e_c[C_.maps.l2u].reshape(-1, (C_.N + 1) ** 3), C_.N, L.N).ravel()
+    e_u = np.zeros(L.maps.U)
+    e_u[L.maps.l2u] = e_L                                           # continuous: every copy holds the same value
+    e_u[L.mask_u != 0] = 0.0
+    return L.smooth(r_u, z + e_u, smooth_order)

@@ -576,3 +576,50 @@ def test_C2_chebyshev_damps_the_upper_spectrum(oracle_mod):
         bound = 1.0 / np.polynomial.chebyshev.Chebyshev.basis(order)(sigma)
         assert np.all(np.abs(ck[inside]) <= bound * np.abs(c0[inside]) * (1 + 1e-9) + 1e-13), order
         assert np.all(np.abs(ck[~inside]) <= np.abs(c0[~inside]) * (1 + 1e-9) + 1e-13), order
+
+
+# --------------------------------------------------------------------- NEXT-1c: p-multigrid V-cycle
+@pytest.fixture(scope="module")
+def pmg_levels(oracle_mod):
+    return [oracle_mod.Level(inputs.box_mesh(3, 3, 2, N, "smooth")) for N in (5, 3, 1)]
+
+
+def _dense_of(fn, n):
+    return np.stack([fn(e) for e in np.eye(n)], axis=1)
+
+
+def test_V1_vcycle_is_a_symmetric_contraction(oracle_mod, pmg_levels):
+    """With equal pre- and post-smoothing from a zero guess the V-cycle is a fixed symmetric linear operator M^-1
+    (every ingredient is linear and restriction is the adjoint of prolongation), M^-1 A has a positive spectrum, and
+    the iteration x <- x + M^-1 (b - A x) contracts: rho(I - M^-1 A) < 1, far below the Jacobi smoother's own rate."""
+    L0 = pmg_levels[0]
+    free = L0.mask_u == 0
+    n = L0.maps.U
+    Minv = _dense_of(lambda r: oracle_mod.vcycle(pmg_levels, np.where(free, r, 0.0), 2, 8), n)[np.ix_(free, free)]
+    A = _dense_of(L0.A, n)[np.ix_(free, free)]
+    assert np.max(np.abs(Minv - Minv.T)) <= 1e-10 * np.max(np.abs(Minv))
+    ev = np.linalg.eigvals(Minv @ A).real
+    assert ev.min() > 0.0
+    rho = np.max(np.abs(1.0 - ev))
+    assert rho < 0.6
+    # the smoother alone (same work on the fine level, no coarse correction) is much worse on the smooth modes
+    S = _dense_of(lambda r: L0.smooth(np.where(free, r, 0.0), None, 4), n)[np.ix_(free, free)]
+    assert np.max(np.abs(1.0 - np.linalg.eigvals(S @ A).real)) > 0.9
+
+
+def test_V2_coarse_correction_helps_coarse_space_errors(oracle_mod, pmg_levels):
+    """Two levels: for an error that lies in the coarse space (a prolonged coarse function) the cycle -- whose coarse
+    problem is solved well (60 Chebyshev steps) -- leaves a much smaller energy-norm error than the same smoothing
+    work without the coarse correction.  (It cannot remove it: the re-discretised coarse operator is stiffer than the
+    Galerkin one, eig(A_c^-1 P^T A P) in [0.28, 1] on this mesh, so the correction under-shoots.)"""
+    L0, L1 = pmg_levels[0], pmg_levels[1]
+    rng = np.random.default_rng(2)
+    e_c = np.where(L1.mask_u != 0, 0.0, rng.standard_normal(L1.maps.U))
+    x_f = np.zeros(L0.maps.U)
+    x_f[L0.maps.l2u] = oracle_mod.prolong(e_c[L1.maps.l2u].reshape(-1, (L1.N + 1) ** 3), L1.N, L0.N).ravel()
+    x_f[L0.mask_u != 0] = 0.0
+    r = L0.A(x_f)
+    en = lambda e: float(e @ L0.A(e))
+    z_v = oracle_mod.vcycle(pmg_levels[:2], r, 2, 60)
+    z_s = L0.smooth(r, None, 4)
+    assert en(z_v - x_f) < 0.4 * en(z_s - x_f) and en(z_v - x_f) < en(x_f)
