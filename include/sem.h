@@ -140,6 +140,22 @@ SEM_API int sem_get_interp(sem_ctx* coarse, sem_ctx* fine, double* J);
 SEM_API int sem_cheby(sem_ctx* ctx, const void* b, void* x, int order, double lmin, double lmax, int zero_guess,
                       sem_prec prec);
 
+/* NEXT-1c.  p-multigrid V-cycle preconditioner z = M^-1 r over `nlevels` contexts, finest first
+ * (the cycle is reading S25 in DESIGN.md and is written out in csrc/sem_pmg.cu): Chebyshev-Jacobi
+ * pre- and post-smoothing of `smooth_order` steps on every level but the coarsest, multiplicity-weighted restriction
+ * J^T, prolongation J, `coarse_order` Chebyshev-Jacobi steps on the coarsest level.
+ *   levels      HOST array of contexts after sem_geom: equal E, strictly decreasing N, the same stream, all with or
+ *               all without a Dirichlet mask.  They must outlive the sem_pmg.
+ *   lmin, lmax  HOST [nlevels], eigenvalue bounds of diag^-1 A per level (S23)
+ *   prec        precision of r, z and of every step of the cycle (the paper runs it in FP32)
+ * sem_pmg_vcycle: r, z DEVICE, finest level's local layout, continuous, r assembled; z is overwritten; 16-byte aligned;
+ * asynchronous on the levels' stream.  The sem_pmg owns its work vectors; sem_pmg_destroy frees them. */
+typedef struct sem_pmg sem_pmg;
+SEM_API int sem_pmg_create(sem_pmg** out, int nlevels, sem_ctx* const* levels, const double* lmin, const double* lmax,
+                           int smooth_order, int coarse_order, sem_prec prec);
+SEM_API int sem_pmg_vcycle(sem_pmg* mg, const void* r, void* z);
+SEM_API void sem_pmg_destroy(sem_pmg* mg);
+
 /* Tuning knob for experiments: selects the Ax kernel variant (0 = default streaming kernel, 1 = simple kernel). */
 SEM_API int sem_set_variant(sem_ctx* ctx, int ax_variant);
 

@@ -41,6 +41,9 @@ SYMBOLS = {
     "sem_transfer": (_i32, [_vp, _vp, _vp, _vp, _i32, _i32]),
     "sem_get_interp": (_i32, [_vp, _vp, _vp]),
     "sem_cheby": (_i32, [_vp, _vp, _vp, _i32, _dbl, _dbl, _i32, _i32]),
+    "sem_pmg_create": (_i32, [C.POINTER(_vp), _i32, C.POINTER(_vp), C.POINTER(_dbl), C.POINTER(_dbl), _i32, _i32, _i32]),
+    "sem_pmg_vcycle": (_i32, [_vp, _vp, _vp]),
+    "sem_pmg_destroy": (None, [_vp]),
     "sem_last_error": (C.c_char_p, [_vp]),
     "sem_ctx_destroy": (None, [_vp]),
 }
@@ -236,3 +239,36 @@ class Sem:
         d = np.empty((self.E, self.p ** 3))
         self._check(self._L.sem_get_diag(self._h, _np_ptr(d)))
         return d
+
+
+class Pmg:
+    """p-multigrid V-cycle preconditioner over Sem contexts, finest first (sem_pmg_create ... sem_pmg_destroy)."""
+
+    def __init__(self, levels, lmin, lmax, smooth_order: int = 2, coarse_order: int = 8, prec: int = SEM_F32):
+        self._L = lib()
+        self.levels = list(levels)                     # keep the contexts alive
+        n = len(self.levels)
+        h = C.c_void_p()
+        arr = (C.c_void_p * n)(*[lv._h for lv in self.levels])
+        lo, hi = (C.c_double * n)(*lmin), (C.c_double * n)(*lmax)
+        rc = self._L.sem_pmg_create(C.byref(h), n, arr, lo, hi, smooth_order, coarse_order, prec)
+        if rc != SEM_OK:
+            raise SemError(rc, "; ".join(self._L.sem_last_error(lv._h).decode() for lv in self.levels))
+        self._h = h
+
+    def vcycle(self, r, z):
+        rc = self._L.sem_pmg_vcycle(self._h, C.c_void_p(r.data_ptr()), C.c_void_p(z.data_ptr()))
+        if rc != SEM_OK:
+            raise SemError(rc, "; ".join(self._L.sem_last_error(lv._h).decode() for lv in self.levels))
+        return z
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.sem_pmg_destroy(self._h)
+            self._h = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()

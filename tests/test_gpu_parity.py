@@ -550,3 +550,39 @@ def test_cheby_smooths(torch_cuda, binding, oracle_mod):
         e1[om.l2u] = x.cpu().numpy().astype(np.float64)
     en = lambda e: float(e @ oracle_mod.apply_Ag(oG, m.N, om, mask_u, e))
     assert en(e1) < 0.25 * en(rough)
+
+
+# ------------------------------------------------------------------------- NEXT-1c: p-multigrid V-cycle
+@pytest.mark.parametrize("orders", [(7, 3, 1), (5, 1), (8, 5, 1)])
+def test_vcycle_parity(torch_cuda, binding, oracle_mod, orders):
+    """sem_pmg_vcycle against the oracle's V-cycle with the same eigenvalue bounds: FP64 to 1e-11 (a chain of about a
+    dozen operator applications, each 1e-12-exact), FP32 to 5e-5 (P:109 runs the cycle in FP32; same chain at 1e-5
+    per step, normalised by max |z|)."""
+    meshes = [inputs.box_mesh(5, 4, 3, N, "smooth") for N in orders]
+    olv = [oracle_mod.Level(m) for m in meshes]
+    L0 = olv[0]
+    r_u = np.where(L0.mask_u != 0, 0.0, inputs.field_normal(L0.maps.uniq_gid, 9))
+    oz = oracle_mod.vcycle(olv, r_u, 2, 8)[L0.maps.l2u]
+    sems = [make_sem(binding, m, dirichlet=True) for m in meshes]
+    try:
+        for dt, prec, tol in ((torch_cuda.float64, binding.SEM_F64, 1e-11), (torch_cuda.float32, binding.SEM_F32, 5e-5)):
+            with binding.Pmg(sems, [l.lmin for l in olv], [l.lmax for l in olv], 2, 8, prec) as mg:
+                r = to_dev(torch_cuda, r_u[L0.maps.l2u], dt)
+                z = torch_cuda.full_like(r, float("nan"))
+                mg.vcycle(r, z)
+                assert relerr(z.cpu().numpy(), oz) <= tol, (orders, dt)
+                z2 = torch_cuda.full_like(r, float("nan"))
+                mg.vcycle(r, z2)                                   # work vectors carry no state between cycles
+                assert torch_cuda.equal(z, z2)
+    finally:
+        for s_ in sems:
+            s_.close()
+
+
+def test_pmg_bad_args(torch_cuda, binding):
+    m7, m3 = inputs.box_mesh(2, 2, 2, 7), inputs.box_mesh(2, 2, 2, 3)
+    with make_sem(binding, m7, dirichlet=True) as s7, make_sem(binding, m3, dirichlet=True) as s3:
+        with pytest.raises(binding.SemError):
+            binding.Pmg([s3, s7], [0.2, 0.2], [2.0, 2.0])           # orders must decrease
+        with pytest.raises(binding.SemError):
+            binding.Pmg([s7, s3], [0.2, 3.0], [2.0, 2.0])           # lmin >= lmax
