@@ -155,6 +155,12 @@ SEM_API int sem_pmg_create(sem_pmg** out, int nlevels, sem_ctx* const* levels, c
                            int smooth_order, int coarse_order, sem_prec prec);
 SEM_API int sem_pmg_vcycle(sem_pmg* mg, const void* r, void* z);
 SEM_API void sem_pmg_destroy(sem_pmg* mg);
+/* Flexible PCG on the finest level of `mg` with the V-cycle as preconditioner (reading S26): the recurrence of sem_pcg
+ * with the Polak-Ribiere beta = r_new.(z_new - z_old) / (r_old.z_old), FP64 outer iteration, x0 = 0, the cycle in mg's
+ * precision.  b, x DEVICE FP64, finest local layout, continuous, b assembled; x is overwritten.  Synchronises.
+ * iters_out / relres_out as in sem_pcg; sem_pmg_get_history copies ||r_k||/||r_0||, k = 0..min(iters, n-1), to HOST. */
+SEM_API int sem_fpcg(sem_pmg* mg, const double* b, double* x, double tol, int maxit, int* iters_out, double* relres_out);
+SEM_API int sem_pmg_get_history(sem_pmg* mg, double* hist, int n);
 
 /* Tuning knob for experiments: selects the Ax kernel variant (0 = default streaming kernel, 1 = simple kernel). */
 SEM_API int sem_set_variant(sem_ctx* ctx, int ax_variant);

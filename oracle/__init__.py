@@ -266,3 +266,39 @@ def vcycle(levels, r_u, smooth_order: int, coarse_order: int, lvl: int = 0):
     e_u[L.maps.l2u] = e_L                                           # continuous: every copy holds the same value
     e_u[L.mask_u != 0] = 0.0
     return L.smooth(r_u, z + e_u, smooth_order)
+
+
+def fpcg(level: "Level", precond, b_u, tol=1e-8, maxit=100):
+    """Flexible preconditioned CG (the preconditioner may change from iteration to iteration or be inexact, e.g. an FP32
+    V-cycle; reading S26): the PCG recurrence of O8 with the Polak-Ribiere beta
+        beta = r_new . (z_new - z_old) / (r_old . z_old).
+    x0 = 0; returns dict(x, iters, hist) with hist[k] = ||r_k|| / ||r_0||."""
+    A = level.A
+    x = np.zeros_like(b_u)
+    r = np.where(level.mask_u != 0, 0.0, b_u)
+    r0 = float(np.linalg.norm(r))
+    hist = [1.0 if r0 > 0 else 0.0]
+    if r0 == 0.0:
+        return dict(x=x, iters=0, hist=np.array(hist))
+    z = precond(r)
+    p = z.copy()
+    rz = float(r @ z)
+    it = 0
+    while it < maxit:
+        q = A(p)
+        pq = float(p @ q)
+        if not pq > 0.0:
+            break
+        alpha = rz / pq
+        x += alpha * p
+        r = r - alpha * q
+        it += 1
+        hist.append(float(np.linalg.norm(r)) / r0)
+        if hist[-1] <= tol:
+            break
+        z_new = precond(r)
+        beta = float(r @ (z_new - z)) / rz
+        rz = float(r @ z_new)
+        z = z_new
+        p = z + beta * p
+    return dict(x=x, iters=it, hist=np.array(hist))

@@ -44,6 +44,8 @@ SYMBOLS = {
     "sem_pmg_create": (_i32, [C.POINTER(_vp), _i32, C.POINTER(_vp), C.POINTER(_dbl), C.POINTER(_dbl), _i32, _i32, _i32]),
     "sem_pmg_vcycle": (_i32, [_vp, _vp, _vp]),
     "sem_pmg_destroy": (None, [_vp]),
+    "sem_fpcg": (_i32, [_vp, _vp, _vp, _dbl, _i32, C.POINTER(_i32), C.POINTER(_dbl)]),
+    "sem_pmg_get_history": (_i32, [_vp, _vp, _i32]),
     "sem_last_error": (C.c_char_p, [_vp]),
     "sem_ctx_destroy": (None, [_vp]),
 }
@@ -261,6 +263,19 @@ class Pmg:
         if rc != SEM_OK:
             raise SemError(rc, "; ".join(self._L.sem_last_error(lv._h).decode() for lv in self.levels))
         return z
+
+    def fpcg(self, b, x, tol: float, maxit: int):
+        it, rel = C.c_int(0), C.c_double(0.0)
+        rc = self._L.sem_fpcg(self._h, C.c_void_p(b.data_ptr()), C.c_void_p(x.data_ptr()), tol, maxit, C.byref(it),
+                              C.byref(rel))
+        if rc != SEM_OK:
+            raise SemError(rc, "; ".join(self._L.sem_last_error(lv._h).decode() for lv in self.levels))
+        return it.value, rel.value
+
+    def history(self, n: int) -> np.ndarray:
+        h = np.full(n, np.nan)
+        self._L.sem_pmg_get_history(self._h, _np_ptr(h), n)
+        return h
 
     def close(self):
         if getattr(self, "_h", None):

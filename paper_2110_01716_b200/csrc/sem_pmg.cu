@@ -11,6 +11,8 @@
 // Every level is its own context (its own discretisation of order N_l on the same elements, S17).  Host code only
 // sequences kernels that exist (sem_cheby, sem_ax_gs, sem_transfer, sem_gs) plus two element-wise vector kernels; no
 // synchronisation anywhere in the cycle.
+#include <math.h>
+
 #include <new>
 #include <vector>
 
@@ -22,6 +24,11 @@ struct sem_pmg {
     int smooth_order = 2, coarse_order = 8;
     sem_prec prec = SEM_F32;
     std::vector<void*> r, z, t, w;      // per level work vectors (r, z only below the finest)
+    // flexible PCG (sem_fpcg): FP64 outer vectors on the finest level, FP32 copies for an FP32 cycle, 4 device scalars
+    double* f[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};      // r, p, q, z, zold
+    float* f32[2] = {nullptr, nullptr};                                // r, z in the cycle's precision
+    double* fs = nullptr;
+    std::vector<double> hist;
 };
 
 namespace {
@@ -66,7 +73,169 @@ int cycle(sem_pmg* mg, int l, const T* r, T* z) {
     return sem_cheby(c, r, z, mg->smooth_order, mg->lmin[l], mg->lmax[l], 0, mg->prec);
 }
 
+__device__ __forceinline__ void block_add(double v, double* __restrict__ out) {
+    __shared__ double red[32];
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+    __syncthreads();
+    if (lane == 0) red[warp] = v;
+    __syncthreads();
+    if (warp == 0) {
+        v = lane < nw ? red[lane] : 0.0;
+        for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) atomicAdd(out, v);
+    }
+}
+
+// x = 0; r = M b; s[0] += r.r (unique-node dot: weights wt)
+__global__ void __launch_bounds__(256) k_f_init(int64_t n, const double* __restrict__ b, const double* __restrict__ wt,
+                                                double* __restrict__ x, double* __restrict__ r, double* __restrict__ s) {
+    double acc = 0.0;
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
+        const double w = wt[l], rl = w != 0.0 ? b[l] : 0.0;
+        x[l] = 0.0;
+        r[l] = rl;
+        acc += w * rl * rl;
+    }
+    block_add(acc, s + 0);
+}
+
+__global__ void __launch_bounds__(256) k_d2f(int64_t n, const double* __restrict__ a, float* __restrict__ o) {
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x)
+        o[l] = (float)a[l];
+}
+
+// z = (double) z_cycle; s[1] += r.z; s[2] += r.zold
+template <typename TZ>
+__global__ void __launch_bounds__(256) k_f_z(int64_t n, const TZ* __restrict__ zc, const double* __restrict__ wt,
+                                             const double* __restrict__ r, const double* __restrict__ zold,
+                                             double* __restrict__ z, double* __restrict__ s) {
+    double a1 = 0.0, a2 = 0.0;
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
+        const double zl = (double)zc[l], w = wt[l] * r[l];
+        z[l] = zl;
+        a1 += w * zl;
+        a2 += w * zold[l];
+    }
+    block_add(a1, s + 1);
+    block_add(a2, s + 2);
+}
+
+// p = z + beta p; zold = z
+__global__ void __launch_bounds__(256) k_f_p(int64_t n, double beta, const double* __restrict__ z,
+                                             double* __restrict__ p, double* __restrict__ zold) {
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
+        const double zl = z[l];
+        p[l] = zl + beta * p[l];
+        zold[l] = zl;
+    }
+}
+
+// x += alpha p; r -= alpha q; s[0] += r.r
+__global__ void __launch_bounds__(256) k_f_update(int64_t n, double alpha, const double* __restrict__ p,
+                                                  const double* __restrict__ q, const double* __restrict__ wt,
+                                                  double* __restrict__ x, double* __restrict__ r,
+                                                  double* __restrict__ s) {
+    double acc = 0.0;
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
+        x[l] += alpha * p[l];
+        const double rl = r[l] - alpha * q[l];
+        r[l] = rl;
+        acc += wt[l] * rl * rl;
+    }
+    block_add(acc, s + 0);
+}
+
 }  // namespace
+
+// Flexible PCG on the finest level with the V-cycle as preconditioner (reading S26): the recurrence of O8 with the
+// Polak-Ribiere beta = r_new.(z_new - z_old) / (r_old.z_old), FP64 outer iteration, cycle in mg's precision.
+// First version: the three scalars of an iteration (p.q, r.r, the two r.z) come back to the host (3 small syncs per
+// iteration, ~5 % of an iteration at config 2).
+extern "C" int sem_fpcg(sem_pmg* mg, const double* b, double* x, double tol, int maxit, int* iters_out,
+                        double* relres_out) {
+    if (!mg) return SEM_EINVAL;
+    sem_ctx* c = mg->lv[0];
+    c->err.clear();
+    if (!b || !x || b == x) return sem_fail(c, SEM_EINVAL, "sem_fpcg: NULL or aliased vectors");
+    if (((uintptr_t)x % 16) || ((uintptr_t)b % 8)) return sem_fail(c, SEM_EINVAL, "sem_fpcg: x must be 16-byte aligned");
+    if (!(tol > 0.0) && maxit <= 0) return sem_fail(c, SEM_EINVAL, "sem_fpcg: tol <= 0 with maxit <= 0");
+    if (maxit < 0) maxit = 0;
+    cudaStream_t st = c->stream;
+    const int64_t n = c->nL;
+    for (int q = 0; q < 5; ++q)
+        if (!mg->f[q]) SEM_CUDA_OK(c, cudaMalloc((void**)&mg->f[q], n * sizeof(double)));
+    if (mg->prec == SEM_F32)
+        for (int q = 0; q < 2; ++q)
+            if (!mg->f32[q]) SEM_CUDA_OK(c, cudaMalloc((void**)&mg->f32[q], n * sizeof(float)));
+    if (!mg->fs) SEM_CUDA_OK(c, cudaMalloc((void**)&mg->fs, 4 * sizeof(double)));
+    double *r = mg->f[0], *p = mg->f[1], *q = mg->f[2], *z = mg->f[3], *zold = mg->f[4], *s = mg->fs;
+    const unsigned grid = (unsigned)c->num_sms * 8;
+    double h[4];
+    auto fetch = [&]() -> int {
+        SEM_CUDA_OK(c, cudaMemcpyAsync(h, s, sizeof(h), cudaMemcpyDeviceToHost, st));
+        SEM_CUDA_OK(c, cudaStreamSynchronize(st));
+        return SEM_OK;
+    };
+    auto precondition = [&]() -> int {                 // z = M^-1 r, s[1] = r.z, s[2] = r.zold
+        int rc;
+        if (mg->prec == SEM_F32) {
+            k_d2f<<<grid, 256, 0, st>>>(n, r, mg->f32[0]);
+            if ((rc = sem_pmg_vcycle(mg, mg->f32[0], mg->f32[1]))) return rc;
+            k_f_z<float><<<grid, 256, 0, st>>>(n, mg->f32[1], c->d_wt, r, zold, z, s);
+        } else {
+            if ((rc = sem_pmg_vcycle(mg, r, q))) return rc;           // q is free here
+            k_f_z<double><<<grid, 256, 0, st>>>(n, q, c->d_wt, r, zold, z, s);
+        }
+        return SEM_OK;
+    };
+    mg->hist.clear();
+    int rc;
+    SEM_CUDA_OK(c, cudaMemsetAsync(s, 0, 4 * sizeof(double), st));
+    SEM_CUDA_OK(c, cudaMemsetAsync(zold, 0, n * sizeof(double), st));
+    SEM_CUDA_OK(c, cudaMemsetAsync(p, 0, n * sizeof(double), st));
+    k_f_init<<<grid, 256, 0, st>>>(n, b, c->d_wt, x, r, s);
+    if ((rc = fetch())) return rc;
+    const double rr0 = h[0];
+    int it = 0;
+    mg->hist.push_back(rr0 > 0.0 ? 1.0 : 0.0);
+    if (rr0 > 0.0 && maxit > 0) {
+        if ((rc = precondition())) return rc;
+        if ((rc = fetch())) return rc;
+        double rz = h[1];
+        k_f_p<<<grid, 256, 0, st>>>(n, 0.0, z, p, zold);
+        while (it < maxit) {
+            SEM_CUDA_OK(c, cudaMemsetAsync(s, 0, 4 * sizeof(double), st));
+            if ((rc = sem_launch_ax_gs(c, p, q, SEM_F64, c->lambda, s + 3, nullptr))) return rc;
+            if ((rc = fetch())) return rc;
+            const double pq = h[3];
+            if (!(pq > 0.0)) break;                     // breakdown (S13)
+            const double alpha = rz / pq;
+            k_f_update<<<grid, 256, 0, st>>>(n, alpha, p, q, c->d_wt, x, r, s);
+            if ((rc = fetch())) return rc;
+            ++it;
+            mg->hist.push_back(sqrt(h[0] / rr0));
+            if (h[0] <= tol * tol * rr0) break;
+            if (it >= maxit) break;
+            if ((rc = precondition())) return rc;
+            if ((rc = fetch())) return rc;
+            const double beta = (h[1] - h[2]) / rz;
+            rz = h[1];
+            k_f_p<<<grid, 256, 0, st>>>(n, beta, z, p, zold);
+        }
+    }
+    SEM_CUDA_OK(c, cudaStreamSynchronize(st));
+    SEM_CUDA_OK(c, cudaGetLastError());
+    if (iters_out) *iters_out = it;
+    if (relres_out) *relres_out = mg->hist.back();
+    return SEM_OK;
+}
+
+extern "C" int sem_pmg_get_history(sem_pmg* mg, double* hist, int n) {
+    if (!mg || !hist || n < 0) return SEM_EINVAL;
+    for (int i = 0; i < n && i < (int)mg->hist.size(); ++i) hist[i] = mg->hist[i];
+    return SEM_OK;
+}
 
 extern "C" int sem_pmg_create(sem_pmg** out, int nlevels, sem_ctx* const* levels, const double* lmin,
                               const double* lmax, int smooth_order, int coarse_order, sem_prec prec) {
@@ -124,6 +293,9 @@ extern "C" void sem_pmg_destroy(sem_pmg* mg) {
     if (!mg->lv.empty()) cudaStreamSynchronize(mg->lv[0]->stream);
     for (auto* v : {&mg->r, &mg->z, &mg->t, &mg->w})
         for (void* p : *v) cudaFree(p);
+    for (double* p : mg->f) cudaFree(p);
+    for (float* p : mg->f32) cudaFree(p);
+    cudaFree(mg->fs);
     cudaGetLastError();
     delete mg;
 }
