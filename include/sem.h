@@ -140,6 +140,10 @@ SEM_API int sem_get_interp(sem_ctx* coarse, sem_ctx* fine, double* J);
 SEM_API int sem_cheby(sem_ctx* ctx, const void* b, void* x, int order, double lmin, double lmax, int zero_guess,
                       sem_prec prec);
 
+/* Setup helper for the bounds above: `iters` power iterations on diag^-1 A (FP64, synchronises); *lam_out is the last
+ * estimate ||diag^-1 A v|| / ||v||, which approaches lambda_max from below: multiply by a safety factor (1.1). */
+SEM_API int sem_lambda_max(sem_ctx* ctx, int iters, double* lam_out);
+
 /* NEXT-1c.  p-multigrid V-cycle preconditioner z = M^-1 r over `nlevels` contexts, finest first
  * (the cycle is reading S25 in DESIGN.md and is written out in csrc/sem_pmg.cu): Chebyshev-Jacobi
  * pre- and post-smoothing of `smooth_order` steps on every level but the coarsest, multiplicity-weighted restriction

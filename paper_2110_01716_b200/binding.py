@@ -41,6 +41,7 @@ SYMBOLS = {
     "sem_transfer": (_i32, [_vp, _vp, _vp, _vp, _i32, _i32]),
     "sem_get_interp": (_i32, [_vp, _vp, _vp]),
     "sem_cheby": (_i32, [_vp, _vp, _vp, _i32, _dbl, _dbl, _i32, _i32]),
+    "sem_lambda_max": (_i32, [_vp, _i32, C.POINTER(_dbl)]),
     "sem_pmg_create": (_i32, [C.POINTER(_vp), _i32, C.POINTER(_vp), C.POINTER(_dbl), C.POINTER(_dbl), _i32, _i32, _i32]),
     "sem_pmg_vcycle": (_i32, [_vp, _vp, _vp]),
     "sem_pmg_destroy": (None, [_vp]),
@@ -201,6 +202,11 @@ class Sem:
         self._check(self._L.sem_cheby(self._h, self._vec(b), self._vec(x), order, lmin, lmax, int(zero_guess),
                                       self._prec(x)))
         return x
+
+    def lambda_max(self, iters: int = 30) -> float:
+        lam = C.c_double(0.0)
+        self._check(self._L.sem_lambda_max(self._h, iters, C.byref(lam)))
+        return lam.value
 
     def set_variant(self, v: int):
         self._check(self._L.sem_set_variant(self._h, v))

@@ -10,6 +10,8 @@
 // A = M QQ^T (D^T G D + lambda B) M through sem_launch_ax_gs; every vector in local layout and continuous.  All the
 // recurrence scalars depend on the bounds only, so they are computed on the host and nothing synchronises: per step
 // one operator application and ONE fused vector kernel (x += d; r -= Minv w; d = c1 d + c2 r).
+#include <math.h>
+
 #include "sem_internal.h"
 
 namespace {
@@ -82,7 +84,77 @@ int run(sem_ctx* c, const T* b, T* x, int order, double lmin, double lmax, bool 
     return SEM_OK;
 }
 
+// power iteration helpers: v = Minv * w, s[0] += wt v v   /   v *= scale
+__global__ void __launch_bounds__(256) k_pow_apply(int64_t n, const double* __restrict__ w, const double* __restrict__ Minv,
+                                                   const double* __restrict__ wt, double* __restrict__ v,
+                                                   double* __restrict__ s) {
+    double acc = 0.0;
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
+        const double vl = Minv[l] * w[l];
+        v[l] = vl;
+        acc += wt[l] * vl * vl;
+    }
+    __shared__ double red[32];
+    for (int o = 16; o; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        acc = threadIdx.x < (blockDim.x >> 5) ? red[threadIdx.x] : 0.0;
+        for (int o = 16; o; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if (threadIdx.x == 0) atomicAdd(s, acc);
+    }
+}
+__global__ void __launch_bounds__(256) k_pow_scale(int64_t n, double a, double* __restrict__ v) {
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) v[l] *= a;
+}
+// a rough, continuous, masked start vector: a hash of the unique node index (an under-estimate of lmax makes the
+// smoother amplify the modes above it, so the start must not be smooth)
+__global__ void __launch_bounds__(256) k_pow_start(int64_t n, const int32_t* __restrict__ l2u, const double* __restrict__ wt,
+                                                   double* __restrict__ v) {
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
+        uint32_t h = (uint32_t)l2u[l] * 2654435761u;
+        h ^= h >> 15; h *= 2246822519u; h ^= h >> 13;
+        v[l] = wt[l] != 0.0 ? (double)(h & 0xffffu) / 32768.0 - 1.0 : 0.0;
+    }
+}
+
 }  // namespace
+
+// Largest eigenvalue of diag^-1 A by `iters` power iterations (setup helper for sem_cheby / sem_pmg_create, S23):
+// returns the last Rayleigh-type estimate ||diag^-1 A v|| / ||v|| (a lower bound that converges from below; callers
+// multiply by a safety factor, usually 1.1).  FP64; synchronises once per iteration.
+extern "C" int sem_lambda_max(sem_ctx* c, int iters, double* lam_out) {
+    if (!c || !lam_out) return SEM_EINVAL;
+    c->err.clear();
+    if (iters < 1) return sem_fail(c, SEM_EINVAL, "sem_lambda_max: iters < 1");
+    if (!c->geom_done) return sem_fail(c, SEM_ESTATE, "sem_lambda_max before sem_geom");
+    int rc;
+    if (!c->d_Minv || c->lambda_of_diag != c->lambda) {
+        if ((rc = sem_build_diag(c))) return rc;
+    }
+    for (int q = 0; q < 3; ++q)
+        if (!c->d_cheb[q]) SEM_CUDA_OK(c, cudaMalloc(&c->d_cheb[q], c->nL * sizeof(double)));
+    double *v = (double*)c->d_cheb[0], *w = (double*)c->d_cheb[1], *s = (double*)c->d_cheb[2];
+    cudaStream_t st = c->stream;
+    const unsigned grid = (unsigned)c->num_sms * 8;
+    k_pow_start<<<grid, 256, 0, st>>>(c->nL, c->d_l2u, c->d_wt, v);
+    double lam = 0.0;                                     // iteration 0 only normalises the start vector
+    for (int it = 0; it <= iters; ++it) {
+        SEM_CUDA_OK(c, cudaMemsetAsync(s, 0, sizeof(double), st));
+        if ((rc = sem_launch_ax_gs(c, v, w, SEM_F64, c->lambda, nullptr, nullptr))) return rc;
+        k_pow_apply<<<grid, 256, 0, st>>>(c->nL, w, c->d_Minv, c->d_wt, v, s);
+        double h = 0.0;
+        SEM_CUDA_OK(c, cudaMemcpyAsync(&h, s, sizeof(double), cudaMemcpyDeviceToHost, st));
+        SEM_CUDA_OK(c, cudaStreamSynchronize(st));
+        const double wnorm = sqrt(h);
+        if (!(wnorm > 0.0)) return sem_fail(c, SEM_EINVAL, "sem_lambda_max: operator annihilates the start vector");
+        if (it > 0) lam = wnorm;                          // v had unit norm
+        k_pow_scale<<<grid, 256, 0, st>>>(c->nL, 1.0 / wnorm, v);
+    }
+    SEM_CUDA_OK(c, cudaGetLastError());
+    *lam_out = lam;
+    return SEM_OK;
+}
 
 extern "C" int sem_cheby(sem_ctx* c, const void* b, void* x, int order, double lmin, double lmax, int zero_guess,
                          sem_prec prec) {

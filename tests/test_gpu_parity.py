@@ -626,3 +626,16 @@ def test_fpcg_vcycle(torch_cuda, binding, oracle_mod):
     finally:
         for s_ in sems:
             s_.close()
+
+
+def test_lambda_max(torch_cuda, binding, oracle_mod):
+    """sem_lambda_max approaches the largest eigenvalue of diag^-1 A (dense, tiny mesh) from below."""
+    m = inputs.box_mesh(3, 3, 2, 4, "random", seed=2)
+    om, oG, mask_u = _pcg_setup(oracle_mod, m)
+    free = mask_u == 0
+    A = np.stack([oracle_mod.apply_Ag(oG, m.N, om, mask_u, e) for e in np.eye(om.U)], axis=1)[np.ix_(free, free)]
+    lam_true = float(np.max(np.linalg.eigvals((1.0 / np.diag(A))[:, None] * A).real))
+    with make_sem(binding, m, dirichlet=True) as sem:
+        lam = sem.lambda_max(60)
+        assert 0.95 * lam_true <= lam <= lam_true * (1 + 1e-12)
+        assert sem.lambda_max(5) <= lam * (1 + 1e-12)
