@@ -9,49 +9,64 @@
 //   x += d
 // A = M QQ^T (D^T G D + lambda B) M through sem_launch_ax_gs; every vector in local layout and continuous.  All the
 // recurrence scalars depend on the bounds only, so they are computed on the host and nothing synchronises: per step
-// one operator application and ONE fused vector kernel (x += d; r -= Minv w; d = c1 d + c2 r).
+// one operator application and ONE fused vector kernel (x += d; r -= Minv w; d = c1 d + c2 r); the final x += d is
+// folded into the last step, which then writes only x, and a zero initial guess is never read or pre-zeroed.
 #include <math.h>
 
 #include "sem_internal.h"
 
 namespace {
 
-template <typename T, typename TM>
-__global__ void __launch_bounds__(256) k_cheb_init(int64_t n, const T* __restrict__ b, const T* __restrict__ q,
-                                                   const TM* __restrict__ Minv, T inv_theta, T* __restrict__ x,
-                                                   T* __restrict__ r, T* __restrict__ d) {
+// r = Minv (b - q) (q == nullptr: zero initial guess); d = r / theta.  ONLY (order == 1): x <- x0 + d and nothing else
+// is written.  Otherwise x is only masked here (non-zero guess) or not touched at all (zero guess: the first step
+// writes it).
+template <typename T, bool ONLY>
+__global__ void __launch_bounds__(256) k_cheb_first(int64_t n, const T* __restrict__ b, const T* __restrict__ q,
+                                                    const T* __restrict__ Minv, T inv_theta, T* __restrict__ x,
+                                                    T* __restrict__ r, T* __restrict__ d) {
     for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
-        const T m = (T)Minv[l];
-        const T rl = m * (q ? b[l] - q[l] : b[l]);      // q == nullptr: zero initial guess
-        if (!q || m == T(0)) x[l] = T(0);               // zero guess, or a Dirichlet node (S14)
-        r[l] = rl;
-        d[l] = rl * inv_theta;
+        const T m = Minv[l];
+        const T rl = m * (q ? b[l] - q[l] : b[l]);
+        const T dl = rl * inv_theta;
+        if constexpr (ONLY) {
+            x[l] = (q && m != T(0)) ? x[l] + dl : dl;     // Dirichlet node (m == 0): dl == 0
+        } else {
+            r[l] = rl;
+            d[l] = dl;
+        }
     }
 }
 
 template <typename T>
-__global__ void __launch_bounds__(256) k_mask_x(int64_t n, const double* __restrict__ Minv, T* __restrict__ x) {
+__global__ void __launch_bounds__(256) k_mask_x(int64_t n, const T* __restrict__ Minv, T* __restrict__ x) {
     for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x)
-        if (Minv[l] == 0.0) x[l] = T(0);
+        if (Minv[l] == T(0)) x[l] = T(0);
 }
 
-template <typename T, typename TM>
-__global__ void __launch_bounds__(256) k_cheb_step(int64_t n, const T* __restrict__ w, const TM* __restrict__ Minv,
+// One step.  XZERO: x is (implicitly) zero before this step (zero guess, first step).  LAST: the final x += d is
+// folded in and r, d are not written back:  x <- x + d + (c1 d + c2 (r - Minv w)).
+template <typename T, bool XZERO, bool LAST>
+__global__ void __launch_bounds__(256) k_cheb_step(int64_t n, const T* __restrict__ w, const T* __restrict__ Minv,
                                                    T c1, T c2, T* __restrict__ x, T* __restrict__ r,
                                                    T* __restrict__ d) {
     for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
         const T dl = d[l];
-        x[l] += dl;
-        const T rl = r[l] - (T)Minv[l] * w[l];
-        r[l] = rl;
-        d[l] = c1 * dl + c2 * rl;
+        const T rl = r[l] - Minv[l] * w[l];
+        const T dn = c1 * dl + c2 * rl;
+        const T x0 = XZERO ? T(0) : x[l];
+        if constexpr (LAST) {
+            x[l] = x0 + dl + dn;
+        } else {
+            x[l] = x0 + dl;
+            r[l] = rl;
+            d[l] = dn;
+        }
     }
 }
 
-template <typename T>
-__global__ void __launch_bounds__(256) k_axpy1(int64_t n, const T* __restrict__ d, T* __restrict__ x) {
+__global__ void __launch_bounds__(256) k_minv32(int64_t n, const double* __restrict__ a, float* __restrict__ o) {
     for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x)
-        x[l] += d[l];
+        o[l] = (float)a[l];
 }
 
 template <typename T>
@@ -62,24 +77,30 @@ int run(sem_ctx* c, const T* b, T* x, int order, double lmin, double lmax, bool 
     T* r = (T*)c->d_cheb[0];
     T* d = (T*)c->d_cheb[1];
     T* w = (T*)c->d_cheb[2];
+    const T* Minv = sizeof(T) == 8 ? (const T*)c->d_Minv : (const T*)c->d_Minv32;
     const unsigned grid = (unsigned)c->num_sms * 8;
     const double theta = 0.5 * (lmax + lmin), delta = 0.5 * (lmax - lmin), sigma = theta / delta;
     double rho = 1.0 / sigma;
     int rc;
-    if (zero_guess) {
-        k_cheb_init<T, double><<<grid, 256, 0, st>>>(n, b, (const T*)nullptr, c->d_Minv, (T)(1.0 / theta), x, r, d);
-    } else {
-        k_mask_x<T><<<grid, 256, 0, st>>>(n, c->d_Minv, x);
+    const T* q = nullptr;
+    if (!zero_guess) {
+        k_mask_x<T><<<grid, 256, 0, st>>>(n, Minv, x);
         if ((rc = sem_launch_ax_gs(c, x, w, prec, c->lambda, nullptr, nullptr))) return rc;
-        k_cheb_init<T, double><<<grid, 256, 0, st>>>(n, b, (const T*)w, c->d_Minv, (T)(1.0 / theta), x, r, d);
+        q = w;
     }
+    if (order == 1) k_cheb_first<T, true><<<grid, 256, 0, st>>>(n, b, q, Minv, (T)(1.0 / theta), x, r, d);
+    else k_cheb_first<T, false><<<grid, 256, 0, st>>>(n, b, q, Minv, (T)(1.0 / theta), x, r, d);
     for (int k = 1; k < order; ++k) {
         if ((rc = sem_launch_ax_gs(c, d, w, prec, c->lambda, nullptr, nullptr))) return rc;
         const double rho1 = 1.0 / (2.0 * sigma - rho);
-        k_cheb_step<T, double><<<grid, 256, 0, st>>>(n, w, c->d_Minv, (T)(rho1 * rho), (T)(2.0 * rho1 / delta), x, r, d);
+        const T c1 = (T)(rho1 * rho), c2 = (T)(2.0 * rho1 / delta);
+        const bool xzero = zero_guess && k == 1, last = k == order - 1;
+        if (xzero && last) k_cheb_step<T, true, true><<<grid, 256, 0, st>>>(n, w, Minv, c1, c2, x, r, d);
+        else if (xzero) k_cheb_step<T, true, false><<<grid, 256, 0, st>>>(n, w, Minv, c1, c2, x, r, d);
+        else if (last) k_cheb_step<T, false, true><<<grid, 256, 0, st>>>(n, w, Minv, c1, c2, x, r, d);
+        else k_cheb_step<T, false, false><<<grid, 256, 0, st>>>(n, w, Minv, c1, c2, x, r, d);
         rho = rho1;
     }
-    k_axpy1<T><<<grid, 256, 0, st>>>(n, d, x);
     SEM_CUDA_OK(c, cudaGetLastError());
     return SEM_OK;
 }
@@ -175,6 +196,11 @@ extern "C" int sem_cheby(sem_ctx* c, const void* b, void* x, int order, double l
     if (prec == SEM_F32 && c->gmode == SEM_G_STORED && (rc = sem_build_g32(c))) return rc;
     for (int q = 0; q < 3; ++q)
         if (!c->d_cheb[q]) SEM_CUDA_OK(c, cudaMalloc(&c->d_cheb[q], c->nL * sizeof(double)));
+    if (prec == SEM_F32 && (!c->d_Minv32 || c->lambda_of_minv32 != c->lambda)) {       // S16: rounded once from double
+        if (!c->d_Minv32) SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_Minv32, c->nL * sizeof(float)));
+        k_minv32<<<(unsigned)c->num_sms * 8, 256, 0, c->stream>>>(c->nL, c->d_Minv, c->d_Minv32);
+        c->lambda_of_minv32 = c->lambda;
+    }
     if (prec == SEM_F64) return run<double>(c, (const double*)b, (double*)x, order, lmin, lmax, zero_guess != 0);
     return run<float>(c, (const float*)b, (float*)x, order, lmin, lmax, zero_guess != 0);
 }

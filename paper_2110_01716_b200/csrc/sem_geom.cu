@@ -195,6 +195,7 @@ int sem_build_diag(sem_ctx* c) {
                                             c->d_Minv, c->d_wt);
     SEM_CUDA_OK(c, cudaGetLastError());
     c->lambda_of_diag = c->lambda;
+    c->lambda_of_minv32 = -1.0;       // the FP32 copy (sem_cheby.cu) is stale now
     return SEM_OK;
 }
 

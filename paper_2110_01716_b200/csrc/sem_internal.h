@@ -81,6 +81,8 @@ struct sem_ctx {
     // ---- p-multigrid transfer (NEXT-1, sem_transfer.cu) ----
     void* d_J = nullptr;           // [SEM_MAXP^2] interpolation matrix of the last transfer, in its precision
     int J_key = -1;                // (coarse p) * 2 + (FP32 ? 1 : 0) of what d_J holds
+    float* d_Minv32 = nullptr;     // Minv rounded to FP32 for the FP32 smoother (sem_cheby.cu)
+    double lambda_of_minv32 = -1.0;
     void* d_cheb[3] = {nullptr, nullptr, nullptr};   // r, d, w of the Chebyshev smoother (sem_cheby.cu), nL doubles each
     // ---- misc ----
     int ax_variant = 0;
