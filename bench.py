@@ -291,6 +291,40 @@ def main():
                "timed": "wall clock around one sem_pcg call (host polls a device flag every 16 iterations)"}
         semd.close()
 
+    # ---- NEXT-1: the same Poisson problem solved to 1e-8 by Jacobi-PCG and by flexible PCG + FP32 p-multigrid V-cycle
+    solve = None
+    if rank == 0 and world == 1 and args.pcg_iters > 0:
+        side = torch.cuda.Stream()                       # the V-cycle replays a CUDA graph on a non-default stream
+        with torch.cuda.stream(side):
+            lv = []
+            for N in (7, 3, 1):
+                mN = inputs.config4(N)
+                sN = binding.Sem(mN.E, N, mN.vert, mN.gid, mN.dirichlet)
+                sN.geom()
+                lv.append(sN)
+            lam = [1.1 * s_.lambda_max(30) for s_ in lv]
+            rhs = torch.empty_like(u)
+            lv[0].ax_gs(u, rhs)
+            x = torch.zeros_like(u)
+
+            def wall(fn):
+                side.synchronize()
+                t0 = time.perf_counter()
+                out = fn()
+                side.synchronize()
+                return out, (time.perf_counter() - t0) * 1e3
+
+            with binding.Pmg(lv, [0.1 * l for l in lam], lam, 2, 8, binding.SEM_F32) as mg:
+                mg.fpcg(rhs, x, 1e-8, 3)                 # warm-up: allocations, graph capture
+                (it_m, rel_m), ms_m = wall(lambda: mg.fpcg(rhs, x, 1e-8, 200))
+            lv[0].pcg(rhs, x.zero_(), 1e-8, 20)
+            (it_j, rel_j), ms_j = wall(lambda: lv[0].pcg(rhs, x.zero_(), 1e-8, 5000))
+            solve = {"tol": 1e-8, "levels": "N = 7-3-1, Chebyshev-Jacobi order 2, FP32 V-cycle, FP64 flexible PCG",
+                     "pmg_fcg": {"iters": it_m, "relres": rel_m, "ms": ms_m},
+                     "jacobi_pcg": {"iters": it_j, "relres": rel_j, "ms": ms_j}}
+            for s_ in lv:
+                s_.close()
+
     dofs = mesh.dofs
     value = whole_job_value(dofs, world, K, ms_total)
     e2e_value = whole_job_value(dofs, world, Ke, ms_e2e)
@@ -323,6 +357,8 @@ def main():
                       "ax_TFLOPs_fp64": (12 * mesh.p + 15) * nL / ax_s / 1e12,
                       "G_local_nodes_per_s": nL * K / (ms_total * 1e-3) / 1e9},
     }
+    if solve is not None:
+        line["poisson_solve"] = solve
     if pcg is not None:
         pcg["frac_of_measured_peak"] = pcg["algorithmic_GBs"] / peak
         line["pcg"] = pcg

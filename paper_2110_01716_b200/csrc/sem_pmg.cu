@@ -29,6 +29,11 @@ struct sem_pmg {
     float* f32[2] = {nullptr, nullptr};                                // r, z in the cycle's precision
     double* fs = nullptr;
     std::vector<double> hist;
+    // CUDA graph of one cycle for the (r, z) pair it was captured with; calls = eager cycles run with that pair so far
+    const void* g_r = nullptr;
+    void* g_z = nullptr;
+    int g_calls = 0;
+    cudaGraphExec_t g_exec = nullptr;
 };
 
 namespace {
@@ -284,8 +289,43 @@ extern "C" int sem_pmg_vcycle(sem_pmg* mg, const void* r, void* z) {
     sem_ctx* c = mg->lv[0];
     c->err.clear();
     if (!r || !z || r == z) return sem_fail(c, SEM_EINVAL, "sem_pmg_vcycle: NULL or aliased vectors");
-    if (mg->prec == SEM_F64) return cycle<double>(mg, 0, (const double*)r, (double*)z);
-    return cycle<float>(mg, 0, (const float*)r, (float*)z);
+    auto eager = [&]() {
+        return mg->prec == SEM_F64 ? cycle<double>(mg, 0, (const double*)r, (double*)z)
+                                   : cycle<float>(mg, 0, (const float*)r, (float*)z);
+    };
+    // A cycle is ~70 small launches and the coarse levels are pure launch latency: when the same (r, z) pair
+    // comes back (a Krylov loop), the second call is captured into a CUDA graph and later calls replay it.  The first
+    // call runs eagerly because it may allocate and upload (interpolation matrices, work vectors), which cannot be
+    // captured.
+    if (mg->g_r != r || mg->g_z != z) {
+        if (mg->g_exec) { cudaGraphExecDestroy(mg->g_exec); mg->g_exec = nullptr; }
+        mg->g_r = r; mg->g_z = z; mg->g_calls = 0;
+    }
+    if (mg->g_exec) {
+        SEM_CUDA_OK(c, cudaGraphLaunch(mg->g_exec, c->stream));
+        return SEM_OK;
+    }
+    // (the legacy default stream cannot be captured: contexts created on it stay eager)
+    if (mg->g_calls++ == 0 || mg->g_calls < 0 || c->stream == nullptr || c->stream == cudaStreamLegacy) return eager();
+    cudaGraph_t graph = nullptr;
+    if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+        cudaGetLastError();
+        mg->g_calls = -1000000;
+        return eager();
+    }
+    const int rc = eager();
+    const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+    if (rc != SEM_OK || e != cudaSuccess || !graph) {      // not capturable after all: stay eager for this pair
+        if (graph) cudaGraphDestroy(graph);
+        cudaGetLastError();
+        mg->g_calls = -1000000;
+        return rc != SEM_OK ? rc : eager();
+    }
+    const cudaError_t ei = cudaGraphInstantiate(&mg->g_exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (ei != cudaSuccess) { mg->g_exec = nullptr; cudaGetLastError(); mg->g_calls = -1000000; return eager(); }
+    SEM_CUDA_OK(c, cudaGraphLaunch(mg->g_exec, c->stream));
+    return SEM_OK;
 }
 
 extern "C" void sem_pmg_destroy(sem_pmg* mg) {
@@ -293,6 +333,7 @@ extern "C" void sem_pmg_destroy(sem_pmg* mg) {
     if (!mg->lv.empty()) cudaStreamSynchronize(mg->lv[0]->stream);
     for (auto* v : {&mg->r, &mg->z, &mg->t, &mg->w})
         for (void* p : *v) cudaFree(p);
+    if (mg->g_exec) cudaGraphExecDestroy(mg->g_exec);
     for (double* p : mg->f) cudaFree(p);
     for (float* p : mg->f32) cudaFree(p);
     cudaFree(mg->fs);

@@ -639,3 +639,40 @@ def test_lambda_max(torch_cuda, binding, oracle_mod):
         lam = sem.lambda_max(60)
         assert 0.95 * lam_true <= lam <= lam_true * (1 + 1e-12)
         assert sem.lambda_max(5) <= lam * (1 + 1e-12)
+
+
+def test_vcycle_graph_replay_on_side_stream(torch_cuda, binding, oracle_mod):
+    """On a non-default stream sem_pmg_vcycle runs eagerly once, captures a CUDA graph on the second call with the same
+    (r, z) pair and replays it afterwards: the three paths give bit-identical results and match the oracle; a new
+    pair falls back to eager and is captured again."""
+    orders = (7, 3, 1)
+    meshes = [inputs.box_mesh(4, 3, 3, N, "smooth") for N in orders]
+    olv = [oracle_mod.Level(m) for m in meshes]
+    L0 = olv[0]
+    r_u = np.where(L0.mask_u != 0, 0.0, inputs.field_normal(L0.maps.uniq_gid, 11))
+    oz = oracle_mod.vcycle(olv, r_u, 2, 8)[L0.maps.l2u]
+    side = torch_cuda.cuda.Stream()
+    with torch_cuda.cuda.stream(side):
+        sems = [make_sem(binding, m, dirichlet=True) for m in meshes]
+        try:
+            with binding.Pmg(sems, [l.lmin for l in olv], [l.lmax for l in olv], 2, 8, binding.SEM_F64) as mg:
+                r = to_dev(torch_cuda, r_u[L0.maps.l2u])
+                zbuf = torch_cuda.empty_like(r)
+                outs = []
+                for _ in range(4):                       # eager, capture + launch, replay, replay
+                    zbuf.fill_(float("nan"))
+                    mg.vcycle(r, zbuf)
+                    side.synchronize()
+                    outs.append(zbuf.clone())
+                for o in outs[1:]:
+                    assert torch_cuda.equal(o, outs[0])
+                assert relerr(outs[0].cpu().numpy(), oz) <= 1e-11
+                r2 = r * 2.0                              # a different pair: eager again, then captured again
+                z2 = torch_cuda.empty_like(r)
+                for _ in range(3):
+                    mg.vcycle(r2, z2)
+                side.synchronize()
+                assert relerr(z2.cpu().numpy(), 2.0 * oz) <= 1e-11
+        finally:
+            for s_ in sems:
+                s_.close()
