@@ -73,8 +73,67 @@ def run_case(mesh, dtype, peak, label):
           f"{row['gdofs']:.1f} | {row['ax_re']:.1f} | {row['re_tflops']:.1f} |", flush=True)
 
 
+def run_config5(n: int, peak: float):
+    """BASELINE.json config 5: n^3 elements (100 at full size), N = 7, random +-10 % vertices (seed 3), scrambled element
+    order (seed 4), homogeneous Dirichlet, b = M Q^T(B f), f = 3 pi^2 sin(pi x) sin(pi y) sin(pi z), Jacobi-PCG to 1e-8.
+    The right-hand side and the node coordinates are built with torch on the device from sem_get-free data: B = the
+    7th geometric factor is not exported at this size, so b is assembled as A applied to nothing -- instead we use the
+    discrete identity b = A u_h-free form: b = Q Q^T (B f) with B f evaluated by the library's own mass factor."""
+    import time
+
+    import numpy as np
+    t0 = time.perf_counter()
+    mesh = inputs.config5(n)
+    t_mesh = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    sem = binding.Sem(mesh.E, mesh.N, mesh.vert, mesh.gid, mesh.dirichlet)
+    sem.geom(with_mass=True)
+    torch.cuda.synchronize()
+    t_setup = time.perf_counter() - t0
+    cnt = sem.counts()
+    nL, S = cnt["nL"], cnt["S"]
+    # node coordinates on the device: trilinear blend of the element vertices at the GLL points (S5)
+    xi = torch.from_numpy(sem.gll()[0]).cuda()
+    p = mesh.p
+    V = torch.from_numpy(mesh.vert).cuda()                                  # [E, 8, 3]
+    a = (1 - xi) / 2
+    bb = (1 + xi) / 2
+    w1 = torch.stack([a, bb])                                                # [2, p]
+    xyz = torch.zeros(mesh.E, p, p, p, 3, device="cuda", dtype=torch.float64)
+    for v in range(8):
+        ia, ib, ic = v & 1, (v >> 1) & 1, (v >> 2) & 1
+        wgt = w1[ic][:, None, None] * w1[ib][None, :, None] * w1[ia][None, None, :]
+        xyz += wgt[None, :, :, :, None] * V[:, v][:, None, None, None, :]
+    exact = (torch.sin(np.pi * xyz[..., 0]) * torch.sin(np.pi * xyz[..., 1]) * torch.sin(np.pi * xyz[..., 2])).reshape(-1)
+    del xyz
+    # b = M Q Q^T (B f): lambda B u with the Helmholtz term only is not exposed, so use  (A + 1 B) f - A f  = B f
+    f = 3 * np.pi ** 2 * exact
+    t1, t2 = torch.empty_like(f), torch.empty_like(f)
+    sem.ax(f, t1, 1.0)
+    sem.ax(f, t2, 0.0)
+    t1 -= t2                                                                 # B f, local
+    del t2
+    sem.gs(t1)
+    mask = torch.from_numpy(mesh.dirichlet.ravel()).cuda() != 0
+    t1[mask] = 0.0
+    x = torch.zeros_like(t1)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    it, rel = sem.pcg(t1, x, 1e-8, 20000)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    err = float((x - exact).abs().max())
+    bytes_it = (64.0 + 56.0 + 32.0) * nL + 16.0 * S
+    print(f"config 5 with {n}^3 elements: E = {mesh.E}, nL = {nL}, U = {cnt['U']}, S = {S}; mesh {t_mesh:.1f} s, "
+          f"setup {t_setup:.1f} s; PCG {it} iterations, relres {rel:.2e}, {dt:.2f} s = {it / dt:.1f} iterations/s, "
+          f"{bytes_it * it / dt / 1e9:.0f} GB/s algorithmic = {bytes_it * it / dt / 1e9 / peak:.2f} of peak; "
+          f"max |x - sin sin sin| = {err:.2e}", flush=True)
+    sem.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--config5", type=int, default=0, help="run config 5 with this many elements per direction")
     ap.add_argument("--max-n", type=int, default=64)
     ap.add_argument("--orders", default="3,5,7,9")
     ap.add_argument("--levels", action="store_true")
@@ -82,6 +141,8 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("sweep needs a CUDA device: the product path has no CPU fallback")
     peak = _peak()
+    if args.config5 > 0:
+        return run_config5(args.config5, peak)
     print(f"peak = {peak:.0f} GB/s (MEASURED_PEAKS.json hbm_gbs, else the profiling guide's fallback)")
     print("| case | E | N | nL | Ax us | Ax GB/s | frac of peak | gs us | Ax+gs us | Ax+gs GB/s | GDOF/s (E N^3) | "
           "Ax recomputed-G us | recomputed TFLOP/s |")

@@ -676,3 +676,38 @@ def test_vcycle_graph_replay_on_side_stream(torch_cuda, binding, oracle_mod):
         finally:
             for s_ in sems:
                 s_.close()
+
+
+@pytest.mark.slow
+def test_config5_solve_40cubed_against_analytic_solution(torch_cuda, binding):
+    """S20: config 5's recipe at 40^3 elements (32.8 M local nodes; the full 100^3 run is recorded in
+    profiles/r1d_config5.md): unique / shared counts from the closed forms, convergence to 1e-8, the iteration count
+    grows like the mesh (569 at 16^3, ~3.1 k at 100^3), and the converged solution is the analytic one to 1e-8."""
+    n = 40
+    m = inputs.config5(n)
+    with binding.Sem(m.E, m.N, m.vert, m.gid, m.dirichlet) as sem:
+        sem.geom(with_mass=True)
+        cnt = sem.counts()
+        assert cnt["U"] == (7 * n + 1) ** 3 and cnt["nL"] == n ** 3 * 512
+        xi = torch_cuda.from_numpy(sem.gll()[0]).cuda()
+        V = torch_cuda.from_numpy(m.vert).cuda()
+        w1 = torch_cuda.stack([(1 - xi) / 2, (1 + xi) / 2])
+        xyz = torch_cuda.zeros(m.E, 8, 8, 8, 3, device="cuda", dtype=torch_cuda.float64)
+        for v in range(8):
+            ia, ib, ic = v & 1, (v >> 1) & 1, (v >> 2) & 1
+            wgt = w1[ic][:, None, None] * w1[ib][None, :, None] * w1[ia][None, None, :]
+            xyz += wgt[None, :, :, :, None] * V[:, v][:, None, None, None, :]
+        exact = (torch_cuda.sin(np.pi * xyz[..., 0]) * torch_cuda.sin(np.pi * xyz[..., 1])
+                 * torch_cuda.sin(np.pi * xyz[..., 2])).reshape(-1)
+        del xyz
+        f = 3 * np.pi ** 2 * exact
+        bf, t2 = torch_cuda.empty_like(f), torch_cuda.empty_like(f)
+        sem.ax(f, bf, 1.0)
+        sem.ax(f, t2, 0.0)
+        bf -= t2                                              # (A + B) f - A f = B f, element by element
+        sem.gs(bf)
+        bf[torch_cuda.from_numpy(m.dirichlet.ravel()).cuda() != 0] = 0.0
+        x = torch_cuda.zeros_like(bf)
+        it, rel = sem.pcg(bf, x, 1e-8, 5000)
+        assert rel <= 1e-8 and 1000 <= it <= 1700
+        assert float((x - exact).abs().max()) <= 1e-8
