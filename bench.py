@@ -5,7 +5,8 @@
 
 A "step" is one pass of the whole hot path: w = QQ^T (D^T G D) u over the full mesh (sem_ax_gs through the C ABI).
 metric  = Ax+gs GDOF/s with DOF = E N^3 (the paper's n); value = whole-job DOF/s with inputs resident in HBM.
-e2e     = same metric with u copied from pinned host memory and w copied back inside every timed step.
+e2e     = same metric with u copied from pinned host memory and w copied back inside every timed step (two lanes,
+          each its own context and stream, take alternate steps so that H2D and D2H overlap on the full-duplex link).
 roofline= the dominant kernel (the local Ax) timed alone with CUDA events: 64 B x nL algorithmic bytes per launch
           against the measured HBM copy bandwidth of MEASURED_PEAKS.json.
 N > 1   = independent replicas, one per GPU (the path has no inter-GPU exchange in this build).
@@ -228,12 +229,16 @@ def main():
             dist.barrier()
             torch.cuda.synchronize()
 
-    def timed(fn, steps):
+    def timed(fn, steps, side_streams=()):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         e0.record()
-        for _ in range(steps):
-            fn()
+        for s_ in side_streams:
+            s_.wait_event(e0)
+        for j in range(steps):
+            fn(j) if side_streams else fn()
+        for s_ in side_streams:                      # the end event must come after the work of every lane
+            torch.cuda.current_stream().wait_stream(s_)
         e1.record()
         barrier()
         return max_over_ranks(e0.elapsed_time(e1), world, "cuda")
@@ -255,19 +260,35 @@ def main():
     ms_gs = timed(lambda: sem.gs(wz), K)
     clocks = sampler.stop() if sampler else None
 
-    # ---- e2e: host buffers, H2D of u and D2H of w inside every timed step ----
-    Ke = max(1, min(args.e2e_steps, K))
+    # ---- e2e: host buffers, H2D of u and D2H of w inside every timed step.  Two lanes (context + stream + device
+    # buffers each) take alternate steps, so one lane's H2D overlaps the other's D2H on the full-duplex link; every step
+    # still copies its own input in and its own result out.
+    Ke = max(2, min(args.e2e_steps, K))
     u_h = torch.from_numpy(inputs.field_uniform(mesh.gid, 0).ravel()).pin_memory()
-    w_h = torch.empty_like(u_h).pin_memory()
+    lanes = []
+    for _ in range(2):
+        st_ = torch.cuda.Stream()
+        with torch.cuda.stream(st_):
+            sl = binding.Sem(mesh.E, mesh.N, mesh.vert, mesh.gid)
+            sl.geom()
+        lanes.append((st_, sl, torch.empty_like(u), torch.empty_like(u), torch.empty_like(u_h).pin_memory()))
 
-    def e2e_step():
-        u.copy_(u_h, non_blocking=True)
-        sem.ax_gs(u, w)
-        w_h.copy_(w, non_blocking=True)
+    def e2e_step(j):
+        st_, sl, ud, wd, wh = lanes[j % 2]
+        with torch.cuda.stream(st_):
+            ud.copy_(u_h, non_blocking=True)
+            sl.ax_gs(ud, wd)
+            wh.copy_(wd, non_blocking=True)
 
-    for _ in range(3):
-        e2e_step()
-    ms_e2e = timed(e2e_step, Ke)
+    for j in range(4):
+        e2e_step(j)
+    ms_e2e = timed(e2e_step, Ke, side_streams=[l[0] for l in lanes])
+    sem.ax_gs(u, w)                                  # the device-resident path's result for the same input
+    torch.cuda.synchronize()
+    e2e_ok = bool(torch.equal(lanes[0][4], lanes[1][4]) and torch.equal(lanes[0][4], w.cpu()))
+    w_h = lanes[0][4]
+    for l in lanes:
+        l[1].close()
 
     # ---- PCG iterations/s (second half of BASELINE.json's metric): config 2 with the Dirichlet mask, fixed count ----
     pcg = None
@@ -343,7 +364,8 @@ def main():
                    "ax_variant": args.variant},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(u_h.numel() * 8),
-                "d2h_bytes_per_step": int(w_h.numel() * 8), "steps": Ke, "ms_per_step": ms_e2e / Ke},
+                "d2h_bytes_per_step": int(w_h.numel() * 8), "steps": Ke, "ms_per_step": ms_e2e / Ke,
+                "lanes": 2, "result_matches_device_path": e2e_ok},
         "gpu_launches": 2 * K,
         "roofline": {"bound": "hbm", "kernel": "ax_stream<double,8,5,8> (local D^T G D u)", "achieved": achieved,
                      "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": ncu_traffic_bytes(),
