@@ -302,3 +302,38 @@ def fpcg(level: "Level", precond, b_u, tol=1e-8, maxit=100):
         z = z_new
         p = z + beta * p
     return dict(x=x, iters=it, hist=np.array(hist))
+
+
+# ---- NEXT-3: projection onto previous solutions ----------------------------------------------------------
+class Projection:
+    """P:111 "For any n x L subspace of R^n with A-orthonormal basis P_L = [p_1 ... p_L], the best-fit approximation to
+    the solution of A p^m = b^m is pbar = P_L P_L^T b^m ... The residual for the reduced problem A dp = b^m - A pbar has
+    a significantly smaller norm ... We augment the space P_{L+1} = [P_L dp] after orthonormalizing dp against P_L with
+    one round of classical Gram-Schmidt ... L_max = 30 before restarting".  Unique storage, plain Euclidean dots.
+    Reading S27: A p_i is stored beside p_i, so the reduced right-hand side is b - sum alpha_i (A p_i); the
+    norm of the orthogonalised dp comes from the same reduction (dp^T A dp - sum beta_i^2); a restart empties the space
+    and the new direction becomes its first vector; a direction whose orthogonalised A-norm^2 is <= 1e-28 of its
+    A-norm^2 is dropped."""
+
+    def __init__(self, A, n: int, Lmax: int = 30):
+        self.A, self.n, self.Lmax = A, n, Lmax
+        self.P = np.zeros((0, n))
+        self.AP = np.zeros((0, n))
+
+    def guess(self, b):
+        alpha = self.P @ b
+        return alpha @ self.P, b - alpha @ self.AP
+
+    def update(self, dx):
+        w = self.A(dx)
+        if self.P.shape[0] >= self.Lmax:
+            self.P, self.AP = np.zeros((0, self.n)), np.zeros((0, self.n))
+        beta = self.P @ w                                  # p_i^T A dx
+        gamma = float(dx @ w)
+        nrm2 = gamma - float(beta @ beta)
+        if not (gamma > 0.0) or nrm2 <= 1e-28 * gamma:
+            return False
+        s = 1.0 / np.sqrt(nrm2)
+        self.P = np.vstack([self.P, (dx - beta @ self.P) * s])
+        self.AP = np.vstack([self.AP, (w - beta @ self.AP) * s])
+        return True

@@ -644,3 +644,40 @@ def test_V3_fpcg_with_vcycle_converges_fast_to_the_dense_solution(oracle_mod, pm
     fj = oracle_mod.fpcg(L0, lambda r: L0.Minv * r, b, tol=1e-10, maxit=500)
     assert fj["iters"] == jac["iters"]
     assert np.max(np.abs(fj["hist"] - jac["hist"])) <= 1e-6 * 1.0
+
+
+# ------------------------------------------------------------- NEXT-3: projection onto previous solutions
+def test_J1_projection_is_the_A_orthogonal_best_fit(oracle_mod, pmg_levels):
+    """The basis stays A-orthonormal, the guess is the A-norm best approximation of the solution in span(P) (checked
+    against a dense A-weighted least squares), the reduced right-hand side is b - A xbar, a repeated right-hand side is
+    solved by the guess alone, and the space restarts at L_max."""
+    L0 = pmg_levels[1]                                     # the N = 3 level: small enough for dense algebra
+    free = L0.mask_u == 0
+    n = L0.maps.U
+    A = _dense_of(L0.A, n)
+    rng = np.random.default_rng(5)
+    base = np.where(free, rng.standard_normal(n), 0.0)
+    drift = np.where(free, rng.standard_normal(n), 0.0)
+    wig = np.where(free, rng.standard_normal(n), 0.0)
+    proj = oracle_mod.Projection(L0.A, n, Lmax=4)
+    res_norms = []
+    for m in range(7):
+        xs = base + 0.1 * m * drift + 0.01 * np.sin(m) * wig          # a smoothly evolving solution: 3-dimensional span
+        b = L0.A(xs)
+        xbar, bred = proj.guess(b)
+        assert np.max(np.abs(bred - (b - L0.A(xbar)))) <= 1e-10 * np.max(np.abs(b))
+        P = proj.P
+        if P.shape[0]:
+            assert np.max(np.abs(P @ A @ P.T - np.eye(P.shape[0]))) <= 1e-9
+            c = np.linalg.solve(P @ A @ P.T, P @ A @ xs)               # A-orthogonal projection of xs on span(P)
+            assert np.max(np.abs(xbar - c @ P)) <= 1e-9 * np.max(np.abs(xs))
+        res_norms.append(np.linalg.norm(bred) / np.linalg.norm(b))
+        proj.update(xs - xbar)                                         # the reduced problem solved exactly
+        assert proj.P.shape[0] <= 4
+    assert res_norms[0] == 1.0 and res_norms[1] < 0.5 and max(res_norms[3:5]) < 1e-8     # span exhausted after 3
+    xbar, bred = proj.guess(b)                                          # the last right-hand side again
+    assert np.linalg.norm(bred) <= 1e-8 * np.linalg.norm(b)
+    # a direction already in the space is dropped (on a space that is not about to restart)
+    p2 = oracle_mod.Projection(L0.A, n, Lmax=30)
+    assert p2.update(base) and p2.update(drift)
+    assert p2.update(1e-3 * p2.P[0] + 2.0 * p2.P[1]) is False and p2.P.shape[0] == 2
