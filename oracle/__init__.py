@@ -312,8 +312,8 @@ class Projection:
     one round of classical Gram-Schmidt ... L_max = 30 before restarting".  Unique storage, plain Euclidean dots.
     Reading S27: A p_i is stored beside p_i, so the reduced right-hand side is b - sum alpha_i (A p_i); the
     norm of the orthogonalised dp comes from the same reduction (dp^T A dp - sum beta_i^2); a restart empties the space
-    and the new direction becomes its first vector; a direction whose orthogonalised A-norm^2 is <= 1e-28 of its
-    A-norm^2 is dropped."""
+    and the new direction becomes its first vector; a direction whose orthogonalised A-norm^2 is <= 1e-12 of its
+    A-norm^2 is dropped (after one round of classical Gram-Schmidt that remainder is rounding noise)."""
 
     def __init__(self, A, n: int, Lmax: int = 30):
         self.A, self.n, self.Lmax = A, n, Lmax
@@ -331,7 +331,7 @@ class Projection:
         beta = self.P @ w                                  # p_i^T A dx
         gamma = float(dx @ w)
         nrm2 = gamma - float(beta @ beta)
-        if not (gamma > 0.0) or nrm2 <= 1e-28 * gamma:
+        if not (gamma > 0.0) or nrm2 <= 1e-12 * gamma:
             return False
         s = 1.0 / np.sqrt(nrm2)
         self.P = np.vstack([self.P, (dx - beta @ self.P) * s])
