@@ -166,6 +166,23 @@ SEM_API void sem_pmg_destroy(sem_pmg* mg);
 SEM_API int sem_fpcg(sem_pmg* mg, const double* b, double* x, double tol, int maxit, int* iters_out, double* relres_out);
 SEM_API int sem_pmg_get_history(sem_pmg* mg, double* hist, int n);
 
+/* NEXT-3.  Projection onto previous solutions (reading S27 in DESIGN.md): an A-orthonormal
+ * basis P_L of up to Lmax earlier solution updates, A = the context's masked assembled operator (current lambda).
+ *   sem_proj_guess   xbar = P_L P_L^T b (the A-norm best fit in span P_L; 0 while the space is empty) and
+ *                    b_reduced = b - A xbar, the right-hand side of the reduced problem A dx = b_reduced.  Asynchronous.
+ *   sem_proj_update  after the caller has solved the reduced problem: dx is A-orthonormalised against P_L (one round of
+ *                    classical Gram-Schmidt, one reduction) and appended; the space restarts (is emptied first) when it
+ *                    already holds Lmax vectors; *accepted = 0 if dx was (numerically) inside the space.  One operator
+ *                    application; synchronises.
+ * b, xbar, b_reduced, dx: DEVICE, FP64, local layout, continuous; b assembled; dx 16-byte aligned.  The context must
+ * outlive the sem_proj, which owns 2 Lmax + 1 vectors of device memory. */
+typedef struct sem_proj sem_proj;
+SEM_API int sem_proj_create(sem_proj** out, sem_ctx* ctx, int Lmax);
+SEM_API int sem_proj_guess(sem_proj* pj, const double* b, double* xbar, double* b_reduced);
+SEM_API int sem_proj_update(sem_proj* pj, const double* dx, int* accepted);
+SEM_API int sem_proj_size(sem_proj* pj, int* L);
+SEM_API void sem_proj_destroy(sem_proj* pj);
+
 /* Tuning knob for experiments: selects the Ax kernel variant (0 = default streaming kernel, 1 = simple kernel). */
 SEM_API int sem_set_variant(sem_ctx* ctx, int ax_variant);
 

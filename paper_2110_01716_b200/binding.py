@@ -45,6 +45,11 @@ SYMBOLS = {
     "sem_pmg_create": (_i32, [C.POINTER(_vp), _i32, C.POINTER(_vp), C.POINTER(_dbl), C.POINTER(_dbl), _i32, _i32, _i32]),
     "sem_pmg_vcycle": (_i32, [_vp, _vp, _vp]),
     "sem_pmg_destroy": (None, [_vp]),
+    "sem_proj_create": (_i32, [C.POINTER(_vp), _vp, _i32]),
+    "sem_proj_guess": (_i32, [_vp, _vp, _vp, _vp]),
+    "sem_proj_update": (_i32, [_vp, _vp, C.POINTER(_i32)]),
+    "sem_proj_size": (_i32, [_vp, C.POINTER(_i32)]),
+    "sem_proj_destroy": (None, [_vp]),
     "sem_fpcg": (_i32, [_vp, _vp, _vp, _dbl, _i32, C.POINTER(_i32), C.POINTER(_dbl)]),
     "sem_pmg_get_history": (_i32, [_vp, _vp, _i32]),
     "sem_last_error": (C.c_char_p, [_vp]),
@@ -286,6 +291,47 @@ class Pmg:
     def close(self):
         if getattr(self, "_h", None):
             self._L.sem_pmg_destroy(self._h)
+            self._h = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+
+class Proj:
+    """Projection onto previous solutions (sem_proj_create ... sem_proj_destroy) on one Sem context."""
+
+    def __init__(self, sem: Sem, Lmax: int = 30):
+        self._L, self.sem = lib(), sem
+        h = C.c_void_p()
+        rc = self._L.sem_proj_create(C.byref(h), sem._h, Lmax)
+        if rc != SEM_OK:
+            raise SemError(rc, self._L.sem_last_error(sem._h).decode())
+        self._h = h
+
+    def _chk(self, rc):
+        if rc != SEM_OK:
+            raise SemError(rc, self._L.sem_last_error(self.sem._h).decode())
+
+    def guess(self, b, xbar, b_reduced):
+        self._chk(self._L.sem_proj_guess(self._h, self.sem._vec(b), self.sem._vec(xbar), self.sem._vec(b_reduced)))
+        return xbar, b_reduced
+
+    def update(self, dx) -> bool:
+        acc = C.c_int(0)
+        self._chk(self._L.sem_proj_update(self._h, self.sem._vec(dx), C.byref(acc)))
+        return bool(acc.value)
+
+    def size(self) -> int:
+        n = C.c_int(0)
+        self._L.sem_proj_size(self._h, C.byref(n))
+        return n.value
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.sem_proj_destroy(self._h)
             self._h = None
 
     def __enter__(self):

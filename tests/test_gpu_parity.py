@@ -711,3 +711,42 @@ def test_config5_solve_40cubed_against_analytic_solution(torch_cuda, binding):
         it, rel = sem.pcg(bf, x, 1e-8, 5000)
         assert rel <= 1e-8 and 1000 <= it <= 1700
         assert float((x - exact).abs().max()) <= 1e-8
+
+
+# ------------------------------------------------------------- NEXT-3: projection onto previous solutions
+def test_projection_parity(torch_cuda, binding, oracle_mod):
+    """sem_proj_* against the oracle's Projection over a sequence of smoothly evolving right-hand sides, including a
+    restart (Lmax = 4) and a dropped direction: guess and reduced right-hand side to 1e-9 at every step."""
+    m = inputs.box_mesh(4, 3, 3, 5, "random", seed=7)
+    L0 = oracle_mod.Level(m, power_its=2)
+    free = L0.mask_u == 0
+    n = L0.maps.U
+    l2u = L0.maps.l2u
+    base, drift, wig, extra = (np.where(free, inputs.field_normal(L0.maps.uniq_gid, s_), 0.0) for s_ in (21, 22, 23, 24))
+    oproj = oracle_mod.Projection(L0.A, n, Lmax=4)
+    with make_sem(binding, m, dirichlet=True) as sem, binding.Proj(sem, 4) as gproj:
+        for step in range(9):
+            # every step brings a genuinely new component (otherwise the update would orthonormalise rounding noise,
+            # which is valid on both sides but not comparable)
+            fresh = np.where(free, inputs.field_normal(L0.maps.uniq_gid, 100 + step), 0.0)
+            xs = base + 0.1 * step * drift + 0.01 * np.sin(step) * wig + 0.003 * fresh + (0.05 * extra if step >= 5 else 0.0)
+            b_u = L0.A(xs)
+            o_xbar, o_bred = oproj.guess(b_u)
+            b = to_dev(torch_cuda, b_u[l2u])
+            xbar, bred = torch_cuda.full_like(b, float("nan")), torch_cuda.full_like(b, float("nan"))
+            gproj.guess(b, xbar, bred)
+            scale = max(np.max(np.abs(xs)), 1e-300)
+            assert np.max(np.abs(xbar.cpu().numpy() - o_xbar[l2u])) <= 1e-9 * scale, step
+            assert np.max(np.abs(bred.cpu().numpy() - o_bred[l2u])) <= 1e-9 * np.max(np.abs(b_u)), step
+            o_acc = oproj.update(xs - o_xbar)                      # each side solves its own reduced problem exactly
+            dx = to_dev(torch_cuda, xs[l2u]) - xbar
+            g_acc = gproj.update(dx)
+            assert g_acc == o_acc and gproj.size() == oproj.P.shape[0], step
+        # a direction inside the space is dropped on both sides
+        inside = oproj.P[0] * 0.5 + oproj.P[-1] * 2.0 if oproj.P.shape[0] < 4 else None
+        if inside is not None:
+            assert oproj.update(inside) is False
+            assert gproj.update(to_dev(torch_cuda, inside[l2u])) is False
+    with make_sem(binding, m, dirichlet=True) as sem:
+        with pytest.raises(binding.SemError):
+            binding.Proj(sem, 0)
