@@ -131,8 +131,45 @@ def run_config5(n: int, peak: float):
     sem.close()
 
 
+def run_projection(peak: float):
+    """NEXT-3 at config 2: bandwidth of the tall-skinny kernels with L = 30 stored solutions, and what the projection
+    buys over a sequence of slowly evolving right-hand sides (Jacobi-PCG iterations to 1e-8 with and without it)."""
+    import numpy as np
+    mesh = inputs.config2()
+    with binding.Sem(mesh.E, mesh.N, mesh.vert, mesh.gid, mesh.dirichlet) as sem:
+        sem.geom()
+        nL = sem.nL
+        fields = [torch.from_numpy(inputs.field_uniform(mesh.gid, 40 + k).ravel()).cuda() for k in range(4)]
+        rhs = [torch.empty_like(fields[0]) for _ in range(4)]
+        for f_, r_ in zip(fields, rhs):
+            sem.ax_gs(f_, r_)                                   # assembled, masked right-hand sides A f_k
+        xbar, bred, x = (torch.empty_like(rhs[0]) for _ in range(3))
+        print("| step | PCG iterations without projection | with projection (L) | reduced / full right-hand side norm |")
+        print("|---|---|---|---|")
+        with binding.Proj(sem, 30) as pj:
+            for m_ in range(12):
+                t = 0.05 * m_
+                b = rhs[0] + t * rhs[1] + t * t * rhs[2] + np.sin(3 * t) * 0.1 * rhs[3]
+                it0, _ = sem.pcg(b, x.zero_(), 1e-8 , 5000)
+                pj.guess(b, xbar, bred)
+                ratio = float(bred.norm() / b.norm())
+                it1, _ = sem.pcg(bred, x.zero_(), 1e-8 * float(b.norm() / max(float(bred.norm()), 1e-300)), 5000)
+                L_before = pj.size()
+                pj.update(x)
+                print(f"| {m_} | {it0} | {it1} ({L_before}) | {ratio:.2e} |", flush=True)
+        with binding.Proj(sem, 30) as pj:                       # fill the space, then time the two kernels' passes
+            for k in range(30):
+                pj.update(torch.from_numpy(inputs.field_uniform(mesh.gid, 200 + k).ravel()).cuda())
+            assert pj.size() == 30
+            t_g = _time(lambda: pj.guess(rhs[0], xbar, bred), 50)
+            gb = 8.0 * nL * (31 + 61 + 2) / t_g / 1e3
+            print(f"\nsem_proj_guess with L = 30 at config 2: {t_g:.0f} us = {gb:.0f} GB/s ({gb / peak:.2f} of peak; "
+                  f"31 vectors read by the multi-dot, 61 read + 2 written by the update pass)")
+
+
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--proj", action="store_true", help="NEXT-3: projection onto previous solutions at config 2")
     ap.add_argument("--config5", type=int, default=0, help="run config 5 with this many elements per direction")
     ap.add_argument("--max-n", type=int, default=64)
     ap.add_argument("--orders", default="3,5,7,9")
@@ -143,6 +180,8 @@ def main():
     peak = _peak()
     if args.config5 > 0:
         return run_config5(args.config5, peak)
+    if args.proj:
+        return run_projection(peak)
     print(f"peak = {peak:.0f} GB/s (MEASURED_PEAKS.json hbm_gbs, else the profiling guide's fallback)")
     print("| case | E | N | nL | Ax us | Ax GB/s | frac of peak | gs us | Ax+gs us | Ax+gs GB/s | GDOF/s (E N^3) | "
           "Ax recomputed-G us | recomputed TFLOP/s |")
