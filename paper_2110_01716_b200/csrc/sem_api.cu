@@ -62,6 +62,7 @@ int sem_geom(sem_ctx* c, const double* node_xyz, sem_gmode mode, int with_mass) 
     if (mode == SEM_G_RECOMPUTE && node_xyz)
         return sem_fail(c, SEM_ESTATE, "SEM_G_RECOMPUTE needs trilinear geometry (node_xyz == NULL)");
     c->geom_done = false;
+    ++c->generation;
     c->pcg_ready = false;
     c->lambda_of_diag = -1.0;   // invalidates the Jacobi diagonal (lambda >= 0 always)
     c->gmode = mode;
@@ -113,6 +114,7 @@ int sem_set_lambda(sem_ctx* c, double lambda) {
     c->err.clear();
     if (!(lambda >= 0.0)) return sem_fail(c, SEM_EINVAL, "lambda must be >= 0 (S18)");
     if (lambda != 0.0 && c->geom_done && !c->with_mass) return sem_fail(c, SEM_ESTATE, "lambda != 0 needs with_mass");
+    if (c->lambda != lambda) ++c->generation;
     c->lambda = lambda;
     return SEM_OK;
 }

@@ -84,6 +84,8 @@ struct sem_ctx {
     float* d_Minv32 = nullptr;     // Minv rounded to FP32 for the FP32 smoother (sem_cheby.cu)
     double lambda_of_minv32 = -1.0;
     void* d_cheb[3] = {nullptr, nullptr, nullptr};   // r, d, w of the Chebyshev smoother (sem_cheby.cu), nL doubles each
+    uint64_t generation = 0;       // bumped whenever device pointers or parameters that launches capture may change
+                                   // (sem_geom, sem_set_lambda): invalidates CUDA graphs recorded over this context
     // ---- misc ----
     int ax_variant = 0;
     std::string err;

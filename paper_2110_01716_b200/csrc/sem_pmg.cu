@@ -33,6 +33,7 @@ struct sem_pmg {
     const void* g_r = nullptr;
     void* g_z = nullptr;
     int g_calls = 0;
+    uint64_t g_gen = 0;                 // sum of the levels' generations when the graph was recorded
     cudaGraphExec_t g_exec = nullptr;
 };
 
@@ -297,7 +298,10 @@ extern "C" int sem_pmg_vcycle(sem_pmg* mg, const void* r, void* z) {
     // comes back (a Krylov loop), the second call is captured into a CUDA graph and later calls replay it.  The first
     // call runs eagerly because it may allocate and upload (interpolation matrices, work vectors), which cannot be
     // captured.
-    if (mg->g_r != r || mg->g_z != z) {
+    uint64_t gen = 0;
+    for (sem_ctx* lv : mg->lv) gen += lv->generation;
+    if (mg->g_r != r || mg->g_z != z || mg->g_gen != gen) {       // another pair, or a level was re-built / re-parametrised
+        mg->g_gen = gen;
         if (mg->g_exec) { cudaGraphExecDestroy(mg->g_exec); mg->g_exec = nullptr; }
         mg->g_r = r; mg->g_z = z; mg->g_calls = 0;
     }

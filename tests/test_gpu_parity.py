@@ -667,6 +667,11 @@ def test_vcycle_graph_replay_on_side_stream(torch_cuda, binding, oracle_mod):
                 for o in outs[1:]:
                     assert torch_cuda.equal(o, outs[0])
                 assert relerr(outs[0].cpu().numpy(), oz) <= 1e-11
+                sems[1].geom()                            # a level is re-built: the recorded graph must not be replayed
+                zbuf.fill_(float("nan"))
+                mg.vcycle(r, zbuf)
+                side.synchronize()
+                assert torch_cuda.equal(zbuf, outs[0])
                 r2 = r * 2.0                              # a different pair: eager again, then captured again
                 z2 = torch_cuda.empty_like(r)
                 for _ in range(3):
