@@ -212,14 +212,15 @@ def cheby(G, N, maps: Maps, mask_u, b_u, x0_u, order: int, lmin: float, lmax: fl
 class Level:
     """One p-multigrid level: its own discretisation of order N on the same elements (S17)."""
 
-    def __init__(self, mesh, lmin_frac: float = 0.1, lmax_safety: float = 1.1, power_its: int = 60):
+    def __init__(self, mesh, lmin_frac: float = 0.1, lmax_safety: float = 1.1, power_its: int = 60, lam: float = 0.0):
         self.N = mesh.N
+        self.lam = lam                                  # Helmholtz shift (S18): H = A + lam B on every level
         self.maps = Maps(mesh.gid)
         self.G, _, rc = geom_trilinear(mesh.vert, mesh.N)
         assert rc == 0
         self.mask_u = mask_unique(mesh.dirichlet, self.maps)
         dg = np.zeros(self.maps.U)
-        np.add.at(dg, self.maps.l2u, diag_local(self.G, self.N).ravel())
+        np.add.at(dg, self.maps.l2u, diag_local(self.G, self.N, lam).ravel())
         self.Minv = np.where(self.mask_u != 0, 0.0, 1.0 / dg)
         # eigenvalue bounds of diag^-1 A for the smoother (S23): power iteration x safety, lmin = fraction of lmax
         # (a rough start vector: an under-estimate of lmax would make the smoother amplify the modes above it)
@@ -233,10 +234,10 @@ class Level:
         self.lmin = lmin_frac * self.lmax
 
     def A(self, x_u):
-        return apply_Ag(self.G, self.N, self.maps, self.mask_u, x_u)
+        return apply_Ag(self.G, self.N, self.maps, self.mask_u, x_u, self.lam)
 
     def smooth(self, b_u, x0_u, order):
-        return cheby(self.G, self.N, self.maps, self.mask_u, b_u, x0_u, order, self.lmin, self.lmax)
+        return cheby(self.G, self.N, self.maps, self.mask_u, b_u, x0_u, order, self.lmin, self.lmax, self.lam)
 
 
 def vcycle(levels, r_u, smooth_order: int, coarse_order: int, lvl: int = 0):

@@ -755,3 +755,34 @@ def test_projection_parity(torch_cuda, binding, oracle_mod):
     with make_sem(binding, m, dirichlet=True) as sem:
         with pytest.raises(binding.SemError):
             binding.Proj(sem, 0)
+
+
+def test_helmholtz_smoother_and_vcycle(torch_cuda, binding, oracle_mod):
+    """S18: H = A + lambda B through the NEXT-1 calls: the smoother and the V-cycle use the level's own Helmholtz
+    diagonal and operator (lambda = 4 on every level), against the oracle."""
+    lam = 4.0
+    orders = (5, 2)
+    meshes = [inputs.box_mesh(4, 3, 3, N, "random", seed=9) for N in orders]
+    olv = [oracle_mod.Level(m, lam=lam) for m in meshes]
+    L0 = olv[0]
+    r_u = np.where(L0.mask_u != 0, 0.0, inputs.field_normal(L0.maps.uniq_gid, 13))
+    o_s = L0.smooth(r_u, None, 3)[L0.maps.l2u]
+    o_v = oracle_mod.vcycle(olv, r_u, 2, 6)[L0.maps.l2u]
+    sems = []
+    try:
+        for m in meshes:
+            s_ = binding.Sem(m.E, m.N, m.vert, m.gid, m.dirichlet)
+            s_.geom(with_mass=True)
+            s_.set_lambda(lam)
+            sems.append(s_)
+        r = to_dev(torch_cuda, r_u[L0.maps.l2u])
+        x = torch_cuda.full_like(r, float("nan"))
+        sems[0].cheby(r, x, 3, L0.lmin, L0.lmax, True)
+        assert relerr(x.cpu().numpy(), o_s) <= TOL64
+        with binding.Pmg(sems, [l.lmin for l in olv], [l.lmax for l in olv], 2, 6, binding.SEM_F64) as mg:
+            z = torch_cuda.full_like(r, float("nan"))
+            mg.vcycle(r, z)
+            assert relerr(z.cpu().numpy(), o_v) <= 1e-11
+    finally:
+        for s_ in sems:
+            s_.close()
