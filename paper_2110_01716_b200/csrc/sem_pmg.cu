@@ -127,9 +127,11 @@ __global__ void __launch_bounds__(256) k_f_z(int64_t n, const TZ* __restrict__ z
     block_add(a2, s + 2);
 }
 
-// p = z + beta p; zold = z
-__global__ void __launch_bounds__(256) k_f_p(int64_t n, double beta, const double* __restrict__ z,
-                                             double* __restrict__ p, double* __restrict__ zold) {
+// Device scalars s[]: 0 r.r | 1 r.z_new | 2 r.z_old | 3 p.q | 4 r_old.z_old (kept across iterations) | 5 breakdown flag
+// p = z + beta p with beta = (s1 - s2) / s4 (Polak-Ribiere; 0 on the first call: s4 == 0);  zold = z
+__global__ void __launch_bounds__(256) k_f_p(int64_t n, const double* __restrict__ z, double* __restrict__ p,
+                                             double* __restrict__ zold, const double* __restrict__ s) {
+    const double beta = s[4] != 0.0 ? (s[1] - s[2]) / s[4] : 0.0;
     for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
         const double zl = z[l];
         p[l] = zl + beta * p[l];
@@ -137,11 +139,22 @@ __global__ void __launch_bounds__(256) k_f_p(int64_t n, double beta, const doubl
     }
 }
 
-// x += alpha p; r -= alpha q; s[0] += r.r
-__global__ void __launch_bounds__(256) k_f_update(int64_t n, double alpha, const double* __restrict__ p,
-                                                  const double* __restrict__ q, const double* __restrict__ wt,
-                                                  double* __restrict__ x, double* __restrict__ r,
-                                                  double* __restrict__ s) {
+// after k_f_p: r.z of this iteration becomes the "old" one, the accumulators are cleared for the next iteration
+__global__ void k_f_roll(double* __restrict__ s) {
+    s[4] = s[1];
+    s[0] = s[1] = s[2] = s[3] = 0.0;
+}
+
+// x += alpha p; r -= alpha q with alpha = s4 / s3 (p.q <= 0: breakdown, nothing is changed, s5 = 1); s[0] += r.r
+__global__ void __launch_bounds__(256) k_f_update(int64_t n, const double* __restrict__ p, const double* __restrict__ q,
+                                                  const double* __restrict__ wt, double* __restrict__ x,
+                                                  double* __restrict__ r, double* __restrict__ s) {
+    const double pq = s[3];
+    if (!(pq > 0.0)) {
+        if (blockIdx.x == 0 && threadIdx.x == 0) s[5] = 1.0;
+        return;
+    }
+    const double alpha = s[4] / pq;
     double acc = 0.0;
     for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
         x[l] += alpha * p[l];
@@ -156,8 +169,7 @@ __global__ void __launch_bounds__(256) k_f_update(int64_t n, double alpha, const
 
 // Flexible PCG on the finest level with the V-cycle as preconditioner (reading S26): the recurrence of O8 with the
 // Polak-Ribiere beta = r_new.(z_new - z_old) / (r_old.z_old), FP64 outer iteration, cycle in mg's precision.
-// First version: the three scalars of an iteration (p.q, r.r, the two r.z) come back to the host (3 small syncs per
-// iteration, ~5 % of an iteration at config 2).
+// alpha and beta are formed on the device; the host reads ||r||^2 once per iteration for the stopping test.
 extern "C" int sem_fpcg(sem_pmg* mg, const double* b, double* x, double tol, int maxit, int* iters_out,
                         double* relres_out) {
     if (!mg) return SEM_EINVAL;
@@ -174,10 +186,10 @@ extern "C" int sem_fpcg(sem_pmg* mg, const double* b, double* x, double tol, int
     if (mg->prec == SEM_F32)
         for (int q = 0; q < 2; ++q)
             if (!mg->f32[q]) SEM_CUDA_OK(c, cudaMalloc((void**)&mg->f32[q], n * sizeof(float)));
-    if (!mg->fs) SEM_CUDA_OK(c, cudaMalloc((void**)&mg->fs, 4 * sizeof(double)));
+    if (!mg->fs) SEM_CUDA_OK(c, cudaMalloc((void**)&mg->fs, 8 * sizeof(double)));
     double *r = mg->f[0], *p = mg->f[1], *q = mg->f[2], *z = mg->f[3], *zold = mg->f[4], *s = mg->fs;
     const unsigned grid = (unsigned)c->num_sms * 8;
-    double h[4];
+    double h[8];
     auto fetch = [&]() -> int {
         SEM_CUDA_OK(c, cudaMemcpyAsync(h, s, sizeof(h), cudaMemcpyDeviceToHost, st));
         SEM_CUDA_OK(c, cudaStreamSynchronize(st));
@@ -197,7 +209,7 @@ extern "C" int sem_fpcg(sem_pmg* mg, const double* b, double* x, double tol, int
     };
     mg->hist.clear();
     int rc;
-    SEM_CUDA_OK(c, cudaMemsetAsync(s, 0, 4 * sizeof(double), st));
+    SEM_CUDA_OK(c, cudaMemsetAsync(s, 0, 8 * sizeof(double), st));
     SEM_CUDA_OK(c, cudaMemsetAsync(zold, 0, n * sizeof(double), st));
     SEM_CUDA_OK(c, cudaMemsetAsync(p, 0, n * sizeof(double), st));
     k_f_init<<<grid, 256, 0, st>>>(n, b, c->d_wt, x, r, s);
@@ -206,28 +218,19 @@ extern "C" int sem_fpcg(sem_pmg* mg, const double* b, double* x, double tol, int
     int it = 0;
     mg->hist.push_back(rr0 > 0.0 ? 1.0 : 0.0);
     if (rr0 > 0.0 && maxit > 0) {
-        if ((rc = precondition())) return rc;
-        if ((rc = fetch())) return rc;
-        double rz = h[1];
-        k_f_p<<<grid, 256, 0, st>>>(n, 0.0, z, p, zold);
+        // alpha and beta are formed on the device from the scalar slots; the host only reads ||r||^2 (and the
+        // breakdown flag) once per iteration for the stopping test
         while (it < maxit) {
-            SEM_CUDA_OK(c, cudaMemsetAsync(s, 0, 4 * sizeof(double), st));
+            if ((rc = precondition())) return rc;                    // z, s1 = r.z, s2 = r.zold
+            k_f_p<<<grid, 256, 0, st>>>(n, z, p, zold, s);
+            k_f_roll<<<1, 1, 0, st>>>(s);
             if ((rc = sem_launch_ax_gs(c, p, q, SEM_F64, c->lambda, s + 3, nullptr))) return rc;
+            k_f_update<<<grid, 256, 0, st>>>(n, p, q, c->d_wt, x, r, s);
             if ((rc = fetch())) return rc;
-            const double pq = h[3];
-            if (!(pq > 0.0)) break;                     // breakdown (S13)
-            const double alpha = rz / pq;
-            k_f_update<<<grid, 256, 0, st>>>(n, alpha, p, q, c->d_wt, x, r, s);
-            if ((rc = fetch())) return rc;
+            if (h[5] != 0.0) break;                                  // breakdown (S13): x unchanged by this iteration
             ++it;
             mg->hist.push_back(sqrt(h[0] / rr0));
             if (h[0] <= tol * tol * rr0) break;
-            if (it >= maxit) break;
-            if ((rc = precondition())) return rc;
-            if ((rc = fetch())) return rc;
-            const double beta = (h[1] - h[2]) / rz;
-            rz = h[1];
-            k_f_p<<<grid, 256, 0, st>>>(n, beta, z, p, zold);
         }
     }
     SEM_CUDA_OK(c, cudaStreamSynchronize(st));
