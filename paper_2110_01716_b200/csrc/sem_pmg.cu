@@ -9,8 +9,8 @@
 //                    z  += J e_c,  e_c = vcycle(r_c)
 //                    z   = smooth(A, r, guess z)
 // Every level is its own context (its own discretisation of order N_l on the same elements, S17).  Host code only
-// sequences kernels that exist (sem_cheby, sem_ax_gs, sem_transfer, sem_gs) plus two element-wise vector kernels; no
-// synchronisation anywhere in the cycle.
+// sequences kernels that exist (sem_cheby, sem_ax_gs, sem_transfer with the weighted residual / the correction update
+// fused into its load / store, sem_gs); no synchronisation anywhere in the cycle.
 #include <math.h>
 
 #include <new>
@@ -23,7 +23,7 @@ struct sem_pmg {
     std::vector<double> lmin, lmax;
     int smooth_order = 2, coarse_order = 8;
     sem_prec prec = SEM_F32;
-    std::vector<void*> r, z, t, w;      // per level work vectors (r, z only below the finest)
+    std::vector<void*> r, z, w;         // per level work vectors (r, z below the finest; w above the coarsest)
     // flexible PCG (sem_fpcg): FP64 outer vectors on the finest level, FP32 copies for an FP32 cycle, 4 device scalars
     double* f[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};      // r, p, q, z, zold
     float* f32[2] = {nullptr, nullptr};                                // r, z in the cycle's precision
@@ -39,22 +39,6 @@ struct sem_pmg {
 
 namespace {
 
-// t = (r - w) * wt      wt = 1/multiplicity, 0 at Dirichlet nodes
-template <typename T>
-__global__ void __launch_bounds__(256) k_resw(int64_t n, const T* __restrict__ r, const T* __restrict__ w,
-                                              const double* __restrict__ wt, T* __restrict__ t) {
-    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x)
-        t[l] = (r[l] - w[l]) * (T)wt[l];
-}
-
-// z += t except at Dirichlet nodes
-template <typename T>
-__global__ void __launch_bounds__(256) k_add_unmasked(int64_t n, const T* __restrict__ t, const double* __restrict__ wt,
-                                                      T* __restrict__ z) {
-    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x)
-        if (wt[l] != 0.0) z[l] += t[l];
-}
-
 template <typename T>
 int cycle(sem_pmg* mg, int l, const T* r, T* z) {
     sem_ctx* c = mg->lv[l];
@@ -63,19 +47,16 @@ int cycle(sem_pmg* mg, int l, const T* r, T* z) {
     if (l == last) return sem_cheby(c, r, z, mg->coarse_order, mg->lmin[l], mg->lmax[l], 1, mg->prec);
     if ((rc = sem_cheby(c, r, z, mg->smooth_order, mg->lmin[l], mg->lmax[l], 1, mg->prec))) return rc;
     T* w = (T*)mg->w[l];
-    T* t = (T*)mg->t[l];
     if ((rc = sem_launch_ax_gs(c, z, w, mg->prec, c->lambda, nullptr, nullptr))) return rc;
-    const unsigned grid = (unsigned)c->num_sms * 8;
-    k_resw<T><<<grid, 256, 0, c->stream>>>(c->nL, r, w, c->d_wt, t);
     sem_ctx* cc = mg->lv[l + 1];
     T* rc_ = (T*)mg->r[l + 1];
     T* zc = (T*)mg->z[l + 1];
-    if ((rc = sem_transfer(cc, c, t, rc_, mg->prec, SEM_RESTRICT))) return rc;
+    // the weighted residual (r - w) W is formed while the restriction loads it, and the prolonged correction is added
+    // to z (except at Dirichlet nodes) while the prolongation stores it: no extra passes over the fine level
+    if ((rc = sem_launch_transfer(cc, c, r, rc_, mg->prec, SEM_RESTRICT, w, c->d_wt))) return rc;
     if ((rc = sem_launch_gs(cc, rc_, mg->prec, /*apply_mask=*/true))) return rc;
     if ((rc = cycle<T>(mg, l + 1, rc_, zc))) return rc;
-    if ((rc = sem_transfer(cc, c, zc, t, mg->prec, SEM_PROLONG))) return rc;
-    k_add_unmasked<T><<<grid, 256, 0, c->stream>>>(c->nL, t, c->d_wt, z);
-    SEM_CUDA_OK(c, cudaGetLastError());
+    if ((rc = sem_launch_transfer(cc, c, zc, z, mg->prec, SEM_PROLONG, nullptr, c->d_wt))) return rc;
     return sem_cheby(c, r, z, mg->smooth_order, mg->lmin[l], mg->lmax[l], 0, mg->prec);
 }
 
@@ -271,11 +252,11 @@ extern "C" int sem_pmg_create(sem_pmg** out, int nlevels, sem_ctx* const* levels
         mg->lv.push_back(c);
         mg->lmin.push_back(lmin[l]);
         mg->lmax.push_back(lmax[l]);
-        void *r = nullptr, *z = nullptr, *t = nullptr, *w = nullptr;
+        void *r = nullptr, *z = nullptr, *w = nullptr;
         cudaError_t e = cudaSuccess;
         if (l > 0) { e = cudaMalloc(&r, c->nL * es); if (e == cudaSuccess) e = cudaMalloc(&z, c->nL * es); }
-        if (e == cudaSuccess && l < nlevels - 1) { e = cudaMalloc(&t, c->nL * es); if (e == cudaSuccess) e = cudaMalloc(&w, c->nL * es); }
-        mg->r.push_back(r); mg->z.push_back(z); mg->t.push_back(t); mg->w.push_back(w);
+        if (e == cudaSuccess && l < nlevels - 1) e = cudaMalloc(&w, c->nL * es);
+        mg->r.push_back(r); mg->z.push_back(z); mg->w.push_back(w);
         if (e != cudaSuccess) {
             sem_fail(c, SEM_ENOMEM, "sem_pmg_create: %s", cudaGetErrorString(e));
             sem_pmg_destroy(mg);
@@ -338,7 +319,7 @@ extern "C" int sem_pmg_vcycle(sem_pmg* mg, const void* r, void* z) {
 extern "C" void sem_pmg_destroy(sem_pmg* mg) {
     if (!mg) return;
     if (!mg->lv.empty()) cudaStreamSynchronize(mg->lv[0]->stream);
-    for (auto* v : {&mg->r, &mg->z, &mg->t, &mg->w})
+    for (auto* v : {&mg->r, &mg->z, &mg->w})
         for (void* p : *v) cudaFree(p);
     if (mg->g_exec) cudaGraphExecDestroy(mg->g_exec);
     for (double* p : mg->f) cudaFree(p);

@@ -19,7 +19,7 @@ constexpr int TNT = 128;
 template <typename T, int AXIS, bool TRANSPOSED>
 __device__ __forceinline__ void contract(T* __restrict__ dst, int64_t es_dst, const T* __restrict__ src, int es_src,
                                          const T* __restrict__ J, int pc, int ne, int n0, int n1, int n2, int nin,
-                                         int nout) {
+                                         int nout, const double* __restrict__ acc_wt = nullptr) {
     const int o0 = AXIS == 0 ? nout : n0, o1 = AXIS == 1 ? nout : n1, o2 = AXIS == 2 ? nout : n2;
     const int per = o0 * o1 * o2, total = per * ne;
     const int sstride = AXIS == 0 ? 1 : AXIS == 1 ? n0 : n0 * n1;
@@ -32,7 +32,11 @@ __device__ __forceinline__ void contract(T* __restrict__ dst, int64_t es_dst, co
         const int jstride = TRANSPOSED ? pc : 1;
         T s = T(0);
         for (int l = 0; l < nin; ++l) s += jp[l * jstride] * sp[l * sstride];
-        dst[el * es_dst + q] = s;
+        if (acc_wt) {                                  // dst += result, except at Dirichlet nodes (weight 0)
+            if (acc_wt[el * es_dst + q] != 0.0) dst[el * es_dst + q] += s;
+        } else {
+            dst[el * es_dst + q] = s;
+        }
     }
 }
 
@@ -40,7 +44,11 @@ __device__ __forceinline__ void contract(T* __restrict__ dst, int64_t es_dst, co
 // PC, PF > 0: the level pair is known at compile time (index arithmetic folds, loops unroll); 0: run-time orders.
 template <typename T, bool RESTRICT, int PC, int PF>
 __global__ void __launch_bounds__(TNT) k_transfer(int64_t E, int pc_rt, int pf_rt, int epc_rt, const T* __restrict__ Jg,
-                                                  const T* __restrict__ in, T* __restrict__ out) {
+                                                  const T* __restrict__ in, T* __restrict__ out,
+                                                  const T* __restrict__ in_minus, const double* __restrict__ wt) {
+    // Fused forms used by the V-cycle (sem_pmg.cu), wt = 1/multiplicity, 0 at Dirichlet nodes (fine level):
+    //   RESTRICT with in_minus:  input = (in - in_minus) * wt         (weighted residual, never materialised)
+    //   PROLONG  with wt:        out  += result where wt != 0         (coarse correction added in place)
     const int pc = PC > 0 ? PC : pc_rt, pf = PF > 0 ? PF : pf_rt;
     const int epc = PF > 0 ? (TNT / (PF * PF) > 0 ? TNT / (PF * PF) : 1) : epc_rt;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -57,13 +65,19 @@ __global__ void __launch_bounds__(TNT) k_transfer(int64_t E, int pc_rt, int pf_r
         const int64_t e0 = g * epc;
         const int ne = (int)(E - e0 < epc ? E - e0 : epc);
         __syncthreads();                                   // bufA free (and sJ filled, first time round)
-        for (int t = threadIdx.x; t < ne * nin3; t += TNT) bufA[t] = in[e0 * nin3 + t];     // contiguous elements
+        if (RESTRICT && in_minus) {
+            for (int t = threadIdx.x; t < ne * nin3; t += TNT)
+                bufA[t] = (in[e0 * nin3 + t] - in_minus[e0 * nin3 + t]) * (T)wt[e0 * nin3 + t];
+        } else {
+            for (int t = threadIdx.x; t < ne * nin3; t += TNT) bufA[t] = in[e0 * nin3 + t];     // contiguous elements
+        }
         __syncthreads();
         contract<T, 0, RESTRICT>(bufB, big, bufA, nin3, sJ, pc, ne, pin, pin, pin, pin, pout);      // [pin][pin][pout]
         __syncthreads();
         contract<T, 1, RESTRICT>(bufA, big, bufB, big, sJ, pc, ne, pout, pin, pin, pin, pout);      // [pin][pout][pout]
         __syncthreads();
-        contract<T, 2, RESTRICT>(out + e0 * nout3, nout3, bufA, big, sJ, pc, ne, pout, pout, pin, pin, pout);
+        contract<T, 2, RESTRICT>(out + e0 * nout3, nout3, bufA, big, sJ, pc, ne, pout, pout, pin, pin, pout,
+                                 (!RESTRICT && wt) ? wt + e0 * nout3 : nullptr);
     }
 }
 
@@ -91,7 +105,8 @@ void interp_matrix(const sem_ctx* cc, const sem_ctx* cf, double* J) {
 }
 
 template <typename T>
-int launch(sem_ctx* cf, int pc, const double* Jh, const void* in, void* out, bool restrict_) {
+int launch(sem_ctx* cf, int pc, const double* Jh, const void* in, void* out, bool restrict_, const void* in_minus,
+           const double* wt) {
     const int pf = cf->p;
     const int key = pc * 2 + (sizeof(T) == 8 ? 0 : 1);
     if (cf->J_key != key) {                       // the matrix on the device is for another level pair / precision
@@ -105,7 +120,7 @@ int launch(sem_ctx* cf, int pc, const double* Jh, const void* in, void* out, boo
     if (epc < 1) epc = 1;
     const size_t smem = sizeof(T) * (((size_t)(pf * pc + 3) & ~(size_t)3) + 2 * (size_t)epc * pf * pf * pf);
     // the level pairs of config 4 (N = 7-3-1) and of the paper's schedules 8-5-1 and 8-6-4-1 are specialised
-    using kern_t = void (*)(int64_t, int, int, int, const T*, const T*, T*);
+    using kern_t = void (*)(int64_t, int, int, int, const T*, const T*, T*, const T*, const double*);
     kern_t kern = restrict_ ? k_transfer<T, true, 0, 0> : k_transfer<T, false, 0, 0>;
 #define SEM_TR_CASE(A, B) \
     if (pc == A && pf == B) kern = restrict_ ? k_transfer<T, true, A, B> : k_transfer<T, false, A, B>;
@@ -116,7 +131,8 @@ int launch(sem_ctx* cf, int pc, const double* Jh, const void* in, void* out, boo
     const int64_t ngrp = (cf->E + epc - 1) / epc;
     int64_t grid = (int64_t)cf->num_sms * 8;
     if (grid > ngrp) grid = ngrp;
-    kern<<<(unsigned)grid, TNT, smem, cf->stream>>>(cf->E, pc, pf, epc, (const T*)cf->d_J, (const T*)in, (T*)out);
+    kern<<<(unsigned)grid, TNT, smem, cf->stream>>>(cf->E, pc, pf, epc, (const T*)cf->d_J, (const T*)in, (T*)out,
+                                                    (const T*)in_minus, wt);
     SEM_CUDA_OK(cf, cudaGetLastError());
     return SEM_OK;
 }
@@ -139,8 +155,9 @@ extern "C" int sem_get_interp(sem_ctx* coarse, sem_ctx* fine, double* J) {
     return SEM_OK;
 }
 
-extern "C" int sem_transfer(sem_ctx* coarse, sem_ctx* fine, const void* in, void* out, sem_prec prec,
-                            sem_transfer_dir dir) {
+// in_minus / wt: the fused forms documented at k_transfer (internal callers only; the public call passes none)
+int sem_launch_transfer(sem_ctx* coarse, sem_ctx* fine, const void* in, void* out, sem_prec prec, sem_transfer_dir dir,
+                        const void* in_minus, const double* wt) {
     int rc = check_pair(coarse, fine);
     if (rc) return rc;
     if (!in || !out || in == out) return sem_fail(fine, SEM_EINVAL, "sem_transfer: NULL or aliased vectors");
@@ -149,6 +166,11 @@ extern "C" int sem_transfer(sem_ctx* coarse, sem_ctx* fine, const void* in, void
     if (!fine->d_J) SEM_CUDA_OK(fine, cudaMalloc((void**)&fine->d_J, sizeof(double) * SEM_MAXP * SEM_MAXP));
     double Jh[SEM_MAXP * SEM_MAXP];
     interp_matrix(coarse, fine, Jh);
-    if (prec == SEM_F64) return launch<double>(fine, coarse->p, Jh, in, out, dir == SEM_RESTRICT);
-    return launch<float>(fine, coarse->p, Jh, in, out, dir == SEM_RESTRICT);
+    if (prec == SEM_F64) return launch<double>(fine, coarse->p, Jh, in, out, dir == SEM_RESTRICT, in_minus, wt);
+    return launch<float>(fine, coarse->p, Jh, in, out, dir == SEM_RESTRICT, in_minus, wt);
+}
+
+extern "C" int sem_transfer(sem_ctx* coarse, sem_ctx* fine, const void* in, void* out, sem_prec prec,
+                            sem_transfer_dir dir) {
+    return sem_launch_transfer(coarse, fine, in, out, prec, dir, nullptr, nullptr);
 }
