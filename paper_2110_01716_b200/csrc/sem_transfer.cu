@@ -19,7 +19,7 @@ constexpr int TNT = 128;
 template <typename T, int AXIS, bool TRANSPOSED>
 __device__ __forceinline__ void contract(T* __restrict__ dst, int64_t es_dst, const T* __restrict__ src, int es_src,
                                          const T* __restrict__ J, int pc, int ne, int n0, int n1, int n2, int nin,
-                                         int nout, const double* __restrict__ acc_wt = nullptr) {
+                                         int nout, bool accumulate = false) {
     const int o0 = AXIS == 0 ? nout : n0, o1 = AXIS == 1 ? nout : n1, o2 = AXIS == 2 ? nout : n2;
     const int per = o0 * o1 * o2, total = per * ne;
     const int sstride = AXIS == 0 ? 1 : AXIS == 1 ? n0 : n0 * n1;
@@ -32,11 +32,8 @@ __device__ __forceinline__ void contract(T* __restrict__ dst, int64_t es_dst, co
         const int jstride = TRANSPOSED ? pc : 1;
         T s = T(0);
         for (int l = 0; l < nin; ++l) s += jp[l * jstride] * sp[l * sstride];
-        if (acc_wt) {                                  // dst += result, except at Dirichlet nodes (weight 0)
-            if (acc_wt[el * es_dst + q] != 0.0) dst[el * es_dst + q] += s;
-        } else {
-            dst[el * es_dst + q] = s;
-        }
+        if (accumulate) dst[el * es_dst + q] += s;
+        else dst[el * es_dst + q] = s;
     }
 }
 
@@ -48,7 +45,9 @@ __global__ void __launch_bounds__(TNT) k_transfer(int64_t E, int pc_rt, int pf_r
                                                   const T* __restrict__ in_minus, const double* __restrict__ wt) {
     // Fused forms used by the V-cycle (sem_pmg.cu), wt = 1/multiplicity, 0 at Dirichlet nodes (fine level):
     //   RESTRICT with in_minus:  input = (in - in_minus) * wt         (weighted residual, never materialised)
-    //   PROLONG  with wt:        out  += result where wt != 0         (coarse correction added in place)
+    //   PROLONG  with wt:        out  += result                        (coarse correction added in place; a
+    //                            correction that vanishes at the coarse Dirichlet nodes prolongs to exact zeros at the
+    //                            fine ones -- J has exact 0 / 1 entries at the end points -- so no mask is needed)
     const int pc = PC > 0 ? PC : pc_rt, pf = PF > 0 ? PF : pf_rt;
     const int epc = PF > 0 ? (TNT / (PF * PF) > 0 ? TNT / (PF * PF) : 1) : epc_rt;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -77,7 +76,7 @@ __global__ void __launch_bounds__(TNT) k_transfer(int64_t E, int pc_rt, int pf_r
         contract<T, 1, RESTRICT>(bufA, big, bufB, big, sJ, pc, ne, pout, pin, pin, pin, pout);      // [pin][pout][pout]
         __syncthreads();
         contract<T, 2, RESTRICT>(out + e0 * nout3, nout3, bufA, big, sJ, pc, ne, pout, pout, pin, pin, pout,
-                                 (!RESTRICT && wt) ? wt + e0 * nout3 : nullptr);
+                                 !RESTRICT && wt != nullptr);
     }
 }
 
