@@ -30,10 +30,9 @@ __device__ __forceinline__ void contract(T* __restrict__ dst, int64_t es_dst, co
         const T* sp = src + el * es_src + (AXIS == 0 ? 0 : a0) + n0 * ((AXIS == 1 ? 0 : a1) + n1 * (AXIS == 2 ? 0 : a2));
         const T* jp = TRANSPOSED ? J + out : J + out * pc;
         const int jstride = TRANSPOSED ? pc : 1;
-        T s = T(0);
+        T s = accumulate ? dst[el * es_dst + q] : T(0);      // loaded before the contraction, which hides its latency
         for (int l = 0; l < nin; ++l) s += jp[l * jstride] * sp[l * sstride];
-        if (accumulate) dst[el * es_dst + q] += s;
-        else dst[el * es_dst + q] = s;
+        dst[el * es_dst + q] = s;
     }
 }
 
