@@ -98,13 +98,16 @@ __global__ void k_diag_local(int64_t E, int p, int epb, Gll1D gll, int64_t slab,
 // Minv = mask / diag (S12, S14); wt = mask / mult (unique-node dot weights in local storage, O8)
 __global__ void k_minv_wt(int64_t n, const double* __restrict__ diag, const int32_t* __restrict__ l2u,
                           const int32_t* __restrict__ mult, const uint8_t* __restrict__ mask_u,
-                          double* __restrict__ Minv, double* __restrict__ wt) {
+                          double* __restrict__ Minv, double* __restrict__ wt, uint8_t* __restrict__ wt8,
+                          int* __restrict__ big_mult) {
     const int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (l >= n) return;
     const int32_t g = l2u[l];
     const bool masked = mask_u && mask_u[g];
     Minv[l] = masked ? 0.0 : 1.0 / diag[l];
     wt[l] = masked ? 0.0 : 1.0 / (double)mult[g];
+    wt8[l] = masked ? 0 : (uint8_t)(mult[g] & 255);
+    if (mult[g] > 255) *big_mult = 1;                 // benign race: every writer stores 1
 }
 
 // slab layout -> [E][ncomp][p^3] export (+ B as 7th)
@@ -191,8 +194,18 @@ int sem_build_diag(sem_ctx* c) {
     k_diag_local<<<nblk(c->nL), 256, 0, st>>>(c->E, c->p, c->epb, make_gll(c), c->slab_f64, c->d_G, c->d_B, c->lambda, c->d_diag);
     int rc = sem_launch_gs(c, c->d_diag, SEM_F64, /*apply_mask=*/false);
     if (rc) return rc;
+    if (!c->d_wt8) SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_wt8, c->nL));
+    int* d_big = nullptr;
+    SEM_CUDA_OK(c, cudaMalloc((void**)&d_big, sizeof(int)));
+    SEM_CUDA_OK(c, cudaMemsetAsync(d_big, 0, sizeof(int), st));
     k_minv_wt<<<nblk(c->nL), 256, 0, st>>>(c->nL, c->d_diag, c->d_l2u, c->d_mult, c->has_mask ? c->d_mask_u : nullptr,
-                                            c->d_Minv, c->d_wt);
+                                            c->d_Minv, c->d_wt, c->d_wt8, d_big);
+    int h_big = 0;
+    cudaError_t eb = cudaMemcpyAsync(&h_big, d_big, sizeof(int), cudaMemcpyDeviceToHost, st);
+    if (eb == cudaSuccess) eb = cudaStreamSynchronize(st);
+    cudaFree(d_big);
+    if (eb != cudaSuccess) return sem_fail(c, SEM_ECUDA, "diag: %s", cudaGetErrorString(eb));
+    if (h_big) { cudaFree(c->d_wt8); c->d_wt8 = nullptr; }        // a multiplicity above 255: keep the 8-byte weights only
     SEM_CUDA_OK(c, cudaGetLastError());
     c->lambda_of_diag = c->lambda;
     c->lambda_of_minv32 = -1.0;       // the FP32 copy (sem_cheby.cu) is stale now

@@ -71,6 +71,8 @@ struct sem_ctx {
     double* d_diag = nullptr;      // assembled, unmasked, local layout
     double* d_Minv = nullptr;      // mask / diag, local layout
     double* d_wt = nullptr;        // 1/mult per local node (0 at masked nodes): unique-node dot weights
+    uint8_t* d_wt8 = nullptr;      // multiplicity per local node as a byte (0 at masked nodes); nullptr if some
+                                   // multiplicity exceeds 255 (then the kernels read d_wt)
     bool pcg_ready = false;
     double lambda_of_diag = -1.0;  // lambda the stored diagonal was built for (-1 = none)
     double *d_r = nullptr, *d_p = nullptr, *d_w = nullptr;

@@ -59,11 +59,15 @@ __global__ void __launch_bounds__(256) k_mask_vec(int64_t n, const double* __res
 }
 
 // x += alpha p; r -= alpha w; accumulate r.r and r.z (z = Minv r) into slot it
+// W8: the dot weights come from wt8 (multiplicity as a byte, 0 = Dirichlet; 1 B instead of 8 B per node), wt = 1/wt8
+__device__ __forceinline__ double wt_of(uint8_t m) { return m ? 1.0 / (double)m : 0.0; }
+
+template <bool W8>
 __global__ void __launch_bounds__(256) k_pcg_update(int64_t n, int it, const double* __restrict__ p,
                                                     const double* __restrict__ w, const double* __restrict__ Minv,
-                                                    const double* __restrict__ wt, double* __restrict__ x,
-                                                    double* __restrict__ r, double* __restrict__ scal,
-                                                    PcgFlags* __restrict__ flags) {
+                                                    const double* __restrict__ wt, const uint8_t* __restrict__ wt8,
+                                                    double* __restrict__ x, double* __restrict__ r,
+                                                    double* __restrict__ scal, PcgFlags* __restrict__ flags) {
     if (flags->done) return;
     const double pq = scal[4 * it + 0];
     if (!(pq > 0.0)) {                                  // breakdown (S13): stop, keep x
@@ -81,7 +85,14 @@ __global__ void __launch_bounds__(256) k_pcg_update(int64_t n, int it, const dou
     double2* x2 = reinterpret_cast<double2*>(x);
     double2* r2 = reinterpret_cast<double2*>(r);
     for (int64_t v = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; v < n2; v += (int64_t)gridDim.x * blockDim.x) {
-        const double2 pv = p2[v], wv = w2[v], mv = m2[v], tv = t2[v];
+        const double2 pv = p2[v], wv = w2[v], mv = m2[v];
+        double2 tv;
+        if constexpr (W8) {
+            const uchar2 c8 = reinterpret_cast<const uchar2*>(wt8)[v];
+            tv = make_double2(wt_of(c8.x), wt_of(c8.y));
+        } else {
+            tv = t2[v];
+        }
         double2 xv = x2[v], rv = r2[v];
         xv.x += alpha * pv.x; xv.y += alpha * pv.y;
         rv.x -= alpha * wv.x; rv.y -= alpha * wv.y;
@@ -95,8 +106,9 @@ __global__ void __launch_bounds__(256) k_pcg_update(int64_t n, int it, const dou
         x[l] += alpha * p[l];
         const double rl = r[l] - alpha * w[l];
         r[l] = rl;
-        srr += wt[l] * rl * rl;
-        srz += wt[l] * rl * rl * Minv[l];
+        const double wl = W8 ? wt_of(wt8[l]) : wt[l];
+        srr += wl * rl * rl;
+        srz += wl * rl * rl * Minv[l];
     }
     block_sum2_atomic(srr, srz, scal + 4 * it + 1, scal + 4 * it + 2);
 }
@@ -182,7 +194,10 @@ extern "C" int sem_pcg(sem_ctx* c, const double* b, double* x, double tol, int m
         for (int it = 1; it <= maxit; ++it) {
             rc = sem_launch_ax_gs(c, c->d_p, c->d_w, SEM_F64, c->lambda, scal + 4 * it, &flags->done);
             if (rc) return rc;
-            k_pcg_update<<<vgrid, 256, 0, st>>>(n, it, c->d_p, c->d_w, c->d_Minv, c->d_wt, x, c->d_r, scal, flags);
+            if (c->d_wt8)
+                k_pcg_update<true><<<vgrid, 256, 0, st>>>(n, it, c->d_p, c->d_w, c->d_Minv, c->d_wt, c->d_wt8, x, c->d_r, scal, flags);
+            else
+                k_pcg_update<false><<<vgrid, 256, 0, st>>>(n, it, c->d_p, c->d_w, c->d_Minv, c->d_wt, nullptr, x, c->d_r, scal, flags);
             k_pcg_direction<<<vgrid, 256, 0, st>>>(n, it, maxit, tol2, c->d_r, c->d_Minv, c->d_p, scal, flags);
             if (it % batch == 0 || it == maxit) {
                 SEM_CUDA_OK(c, cudaMemcpyAsync(&hf, flags, sizeof(hf), cudaMemcpyDeviceToHost, st));
