@@ -786,3 +786,39 @@ def test_helmholtz_smoother_and_vcycle(torch_cuda, binding, oracle_mod):
     finally:
         for s_ in sems:
             s_.close()
+
+
+def test_high_multiplicity_node(torch_cuda, binding, oracle_mod):
+    """A node shared by 300 elements (a "star" of unit cubes glued at one vertex; gids are arbitrary, S11): the
+    gather-scatter's generic path for more than 8 copies, and the PCG's fallback to 8-byte dot weights when a
+    multiplicity does not fit a byte."""
+    E, N = 300, 2
+    p3 = (N + 1) ** 3
+    base = inputs.box_mesh(1, 1, 1, N)
+    vert = np.repeat(base.vert, E, axis=0)
+    gid = (1 + np.arange(E * p3, dtype=np.int64)).reshape(E, p3)
+    gid[:, 0] = 0                                            # local node 0 of every element is the same global node
+    dirichlet = np.zeros((E, p3), np.uint8)
+    dirichlet[:, p3 - 1] = 1                                 # one Dirichlet node per element: the operator is SPD
+    om = oracle_mod.Maps(gid)
+    assert om.mult.max() == E
+    oG, _, _ = oracle_mod.geom_trilinear(vert, N)
+    mask_u = oracle_mod.mask_unique(dirichlet, om)
+    u = inputs.field_uniform(gid, 3)
+    ow = oracle_mod.gs(oracle_mod.ax(oG, u, N).ravel(), om)
+    xs = np.where(mask_u != 0, 0.0, inputs.field_normal(om.uniq_gid, 5))
+    b_u = oracle_mod.apply_Ag(oG, N, om, mask_u, xs)
+    ores = oracle_mod.pcg(oG, N, om, mask_u, b_u, tol=1e-30, maxit=12)
+    with binding.Sem(E, N, vert, gid) as sem:
+        sem.geom()
+        du = to_dev(torch_cuda, u.ravel())
+        dw = torch_cuda.empty_like(du)
+        sem.ax_gs(du, dw)
+        assert relerr(dw.cpu().numpy(), ow) <= TOL64
+    with binding.Sem(E, N, vert, gid, dirichlet) as sem:
+        sem.geom()
+        b = to_dev(torch_cuda, b_u[om.l2u])
+        x = torch_cuda.zeros_like(b)
+        it, rel = sem.pcg(b, x, 1e-30, 12)
+        assert it == 12
+        assert relerr(x.cpu().numpy(), ores["x"][om.l2u]) <= TOLPCG
