@@ -205,6 +205,9 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
+    # a non-default stream: repeated sem_ax_gs calls and the V-cycle replay CUDA graphs, which the legacy default stream
+    # cannot record; every context created below runs on it and the timing events are recorded on it
+    torch.cuda.set_stream(torch.cuda.Stream())
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     if rank == 0:

@@ -106,7 +106,42 @@ int sem_ax_gs(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda) 
     if (rc) return rc;
     if ((rc = require_geom(c, "sem_ax_gs"))) return rc;
     if (prec == SEM_F32 && c->gmode == SEM_G_STORED && (rc = sem_build_g32(c))) return rc;
-    return sem_launch_ax_gs(c, u, w, prec, lambda, nullptr, nullptr);
+    // Repeated applications with the same arguments (a time loop, a benchmark) replay a two-node CUDA graph: the
+    // operator kernel and the gather-scatter kernel then start back to back instead of paying a stream launch each
+    // (an empty 2000-CTA kernel costs 4 us per launch on this machine).  The first call with a new argument set runs
+    // eagerly, the second is captured; the legacy default stream cannot be captured and stays eager.
+    const bool same = c->ag_exec_or_seen && c->ag_u == u && c->ag_w == w && c->ag_prec == (int)prec &&
+                      c->ag_lambda == lambda && c->ag_gen == c->generation && c->ag_variant == c->ax_variant;
+    if (same && c->ag_exec) {
+        SEM_CUDA_OK(c, cudaGraphLaunch(c->ag_exec, c->stream));
+        return SEM_OK;
+    }
+    if (!same) {
+        if (c->ag_exec) { cudaGraphExecDestroy(c->ag_exec); c->ag_exec = nullptr; }
+        c->ag_u = u; c->ag_w = w; c->ag_prec = (int)prec; c->ag_lambda = lambda; c->ag_gen = c->generation;
+        c->ag_variant = c->ax_variant;
+        c->ag_exec_or_seen = true;
+        c->ag_capturable = c->stream != nullptr && c->stream != cudaStreamLegacy;
+        return sem_launch_ax_gs(c, u, w, prec, lambda, nullptr, nullptr);
+    }
+    if (!c->ag_capturable || cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+        cudaGetLastError();
+        c->ag_capturable = false;
+        return sem_launch_ax_gs(c, u, w, prec, lambda, nullptr, nullptr);
+    }
+    rc = sem_launch_ax_gs(c, u, w, prec, lambda, nullptr, nullptr);
+    cudaGraph_t graph = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+    if (rc == SEM_OK && e == cudaSuccess && graph && cudaGraphInstantiate(&c->ag_exec, graph, 0) == cudaSuccess) {
+        cudaGraphDestroy(graph);
+        SEM_CUDA_OK(c, cudaGraphLaunch(c->ag_exec, c->stream));
+        return SEM_OK;
+    }
+    if (graph) cudaGraphDestroy(graph);
+    cudaGetLastError();
+    c->ag_exec = nullptr;
+    c->ag_capturable = false;
+    return rc != SEM_OK ? rc : sem_launch_ax_gs(c, u, w, prec, lambda, nullptr, nullptr);
 }
 
 int sem_set_lambda(sem_ctx* c, double lambda) {
@@ -191,6 +226,7 @@ const char* sem_last_error(sem_ctx* c) {
 void sem_ctx_destroy(sem_ctx* c) {
     if (!c) return;
     cudaStreamSynchronize(c->stream);
+    if (c->ag_exec) cudaGraphExecDestroy(c->ag_exec);
     void* ptrs[] = {c->d_vert, c->d_l2u, c->d_mult, c->d_seg_off, c->d_seg_idx, c->d_uniq_gid, c->d_sh_off, c->d_sh_idx,
                     c->d_sh_masked, c->d_mask_u, c->d_mask1_idx, c->d_G, c->d_G32, c->d_B, c->d_B32, c->d_detJ,
                     c->d_diag, c->d_Minv, c->d_wt, c->d_wt8, c->d_r, c->d_p, c->d_w, c->d_scal, 

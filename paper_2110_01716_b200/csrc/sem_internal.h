@@ -88,6 +88,14 @@ struct sem_ctx {
     void* d_cheb[3] = {nullptr, nullptr, nullptr};   // r, d, w of the Chebyshev smoother (sem_cheby.cu), nL doubles each
     uint64_t generation = 0;       // bumped whenever device pointers or parameters that launches capture may change
                                    // (sem_geom, sem_set_lambda): invalidates CUDA graphs recorded over this context
+    // ---- CUDA graph of one sem_ax_gs application (sem_api.cu), valid for the argument set it was recorded with ----
+    cudaGraphExec_t ag_exec = nullptr;
+    bool ag_exec_or_seen = false, ag_capturable = false;
+    const void* ag_u = nullptr;
+    void* ag_w = nullptr;
+    int ag_prec = -1, ag_variant = 0;
+    double ag_lambda = 0.0;
+    uint64_t ag_gen = 0;
     // ---- misc ----
     int ax_variant = 0;
     std::string err;

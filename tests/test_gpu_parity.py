@@ -822,3 +822,42 @@ def test_high_multiplicity_node(torch_cuda, binding, oracle_mod):
         it, rel = sem.pcg(b, x, 1e-30, 12)
         assert it == 12
         assert relerr(x.cpu().numpy(), ores["x"][om.l2u]) <= TOLPCG
+
+
+def test_ax_gs_graph_replay_on_side_stream(torch_cuda, binding, oracle_mod):
+    """Repeated sem_ax_gs with the same arguments on a non-default stream: eager, captured, replayed -- bit-identical,
+    equal to the oracle; new arguments, a new variant or a re-built geometry drop the recorded graph."""
+    m = inputs.box_mesh(6, 5, 4, 7, "smooth")
+    u = inputs.field_uniform(m.gid, 3)
+    ow = _ax_gs_oracle(oracle_mod, m, u, True)
+    side = torch_cuda.cuda.Stream()
+    with torch_cuda.cuda.stream(side):
+        with make_sem(binding, m, dirichlet=True) as sem:
+            du = to_dev(torch_cuda, u.ravel())
+            dw = torch_cuda.empty_like(du)
+            outs = []
+            for _ in range(4):
+                dw.fill_(float("nan"))
+                sem.ax_gs(du, dw)
+                side.synchronize()
+                outs.append(dw.clone())
+            for o in outs[1:]:
+                assert torch_cuda.equal(o, outs[0])
+            assert relerr(outs[0].cpu().numpy(), ow) <= TOL64
+            du2 = du * 3.0                                   # other arguments: eager, then recorded again
+            dw2 = torch_cuda.empty_like(du)
+            for _ in range(3):
+                sem.ax_gs(du2, dw2)
+            side.synchronize()
+            assert relerr(dw2.cpu().numpy(), 3.0 * ow) <= TOL64
+            sem.geom()                                       # re-built geometry: the graph over (du2, dw2) is stale
+            dw2.fill_(float("nan"))
+            sem.ax_gs(du2, dw2)
+            side.synchronize()
+            assert relerr(dw2.cpu().numpy(), 3.0 * ow) <= TOL64
+            d32 = du.float()
+            w32 = torch_cuda.empty_like(d32)
+            for _ in range(3):
+                sem.ax_gs(d32, w32)                          # another precision
+            side.synchronize()
+            assert relerr(w32.cpu().numpy(), ow) <= TOL32
