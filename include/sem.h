@@ -85,7 +85,9 @@ SEM_API int sem_ax(sem_ctx* ctx, const void* u, void* w, sem_prec prec, double l
 SEM_API int sem_gs(sem_ctx* ctx, void* w, sem_prec prec, sem_op op);
 
 /* a3-a7.  w = M QQ^T (D^T G D + lambda B) u, with M zeroing Dirichlet nodes (if the context has any).  u must be
- * continuous (equal on all copies of a shared node). */
+ * continuous (equal on all copies of a shared node).  Called repeatedly with the same (u, w, prec, lambda) on a
+ * non-default stream, the second call records the two kernels into a CUDA graph and later calls replay it (still
+ * asynchronous; the graph is dropped when the arguments, the geometry or the variant change). */
 SEM_API int sem_ax_gs(sem_ctx* ctx, const void* u, void* w, sem_prec prec, double lambda);
 
 /* a8.  Jacobi-preconditioned conjugate gradients on M QQ^T A_L M (O8, S12-S14), FP64, lambda = 0 unless
