@@ -35,6 +35,12 @@ struct sem_pmg {
     int g_calls = 0;
     uint64_t g_gen = 0;                 // sum of the levels' generations when the graph was recorded
     cudaGraphExec_t g_exec = nullptr;
+    // CUDA graph of one whole flexible-PCG iteration (cycle, direction, operator, update), for the x it was recorded with
+    bool outer_capture = false;         // the cycle is being recorded as part of that graph: run it eagerly
+    cudaGraphExec_t it_exec = nullptr;
+    const void* it_x = nullptr;
+    const void* it_b = nullptr;
+    uint64_t it_gen = 0;
 };
 
 namespace {
@@ -201,12 +207,49 @@ extern "C" int sem_fpcg(sem_pmg* mg, const double* b, double* x, double tol, int
     if (rr0 > 0.0 && maxit > 0) {
         // alpha and beta are formed on the device from the scalar slots; the host only reads ||r||^2 (and the
         // breakdown flag) once per iteration for the stopping test
-        while (it < maxit) {
-            if ((rc = precondition())) return rc;                    // z, s1 = r.z, s2 = r.zold
+        // Every launch of an iteration has the same arguments (the scalars live on the device), so from the second
+        // iteration on the whole iteration is one CUDA graph (recorded once per x; non-default streams only).
+        auto body = [&]() -> int {
+            int rb;
+            if ((rb = precondition())) return rb;                    // z, s1 = r.z, s2 = r.zold
             k_f_p<<<grid, 256, 0, st>>>(n, z, p, zold, s);
             k_f_roll<<<1, 1, 0, st>>>(s);
-            if ((rc = sem_launch_ax_gs(c, p, q, SEM_F64, c->lambda, s + 3, nullptr))) return rc;
+            if ((rb = sem_launch_ax_gs(c, p, q, SEM_F64, c->lambda, s + 3, nullptr))) return rb;
             k_f_update<<<grid, 256, 0, st>>>(n, p, q, c->d_wt, x, r, s);
+            return SEM_OK;
+        };
+        uint64_t gen = 0;
+        for (sem_ctx* lv : mg->lv) gen += lv->generation;
+        if (mg->it_exec && (mg->it_x != x || mg->it_b != b || mg->it_gen != gen)) {
+            cudaGraphExecDestroy(mg->it_exec);
+            mg->it_exec = nullptr;
+        }
+        bool capturable = st != nullptr && st != cudaStreamLegacy;
+        while (it < maxit) {
+            if (mg->it_exec) {
+                SEM_CUDA_OK(c, cudaGraphLaunch(mg->it_exec, st));
+            } else if (it >= 1 && capturable && cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+                mg->outer_capture = true;
+                rc = body();
+                mg->outer_capture = false;
+                cudaGraph_t graph = nullptr;
+                const cudaError_t e = cudaStreamEndCapture(st, &graph);
+                if (rc == SEM_OK && e == cudaSuccess && graph && cudaGraphInstantiate(&mg->it_exec, graph, 0) == cudaSuccess) {
+                    cudaGraphDestroy(graph);
+                    mg->it_x = x; mg->it_b = b; mg->it_gen = gen;
+                    SEM_CUDA_OK(c, cudaGraphLaunch(mg->it_exec, st));
+                } else {
+                    if (graph) cudaGraphDestroy(graph);
+                    cudaGetLastError();
+                    mg->it_exec = nullptr;
+                    capturable = false;
+                    if (rc != SEM_OK) return rc;
+                    if ((rc = body())) return rc;
+                }
+            } else {
+                if (it >= 1) { cudaGetLastError(); capturable = false; }
+                if ((rc = body())) return rc;
+            }
             if ((rc = fetch())) return rc;
             if (h[5] != 0.0) break;                                  // breakdown (S13): x unchanged by this iteration
             ++it;
@@ -282,6 +325,7 @@ extern "C" int sem_pmg_vcycle(sem_pmg* mg, const void* r, void* z) {
     // comes back (a Krylov loop), the second call is captured into a CUDA graph and later calls replay it.  The first
     // call runs eagerly because it may allocate and upload (interpolation matrices, work vectors), which cannot be
     // captured.
+    if (mg->outer_capture) return eager();                   // part of sem_fpcg's iteration graph
     uint64_t gen = 0;
     for (sem_ctx* lv : mg->lv) gen += lv->generation;
     if (mg->g_r != r || mg->g_z != z || mg->g_gen != gen) {       // another pair, or a level was re-built / re-parametrised
@@ -322,6 +366,7 @@ extern "C" void sem_pmg_destroy(sem_pmg* mg) {
     for (auto* v : {&mg->r, &mg->z, &mg->w})
         for (void* p : *v) cudaFree(p);
     if (mg->g_exec) cudaGraphExecDestroy(mg->g_exec);
+    if (mg->it_exec) cudaGraphExecDestroy(mg->it_exec);
     for (double* p : mg->f) cudaFree(p);
     for (float* p : mg->f32) cudaFree(p);
     cudaFree(mg->fs);

@@ -861,3 +861,35 @@ def test_ax_gs_graph_replay_on_side_stream(torch_cuda, binding, oracle_mod):
                 sem.ax_gs(d32, w32)                          # another precision
             side.synchronize()
             assert relerr(w32.cpu().numpy(), ow) <= TOL32
+
+
+def test_fpcg_iteration_graph_on_side_stream(torch_cuda, binding, oracle_mod):
+    """On a non-default stream sem_fpcg records one whole iteration as a CUDA graph (from the second iteration of the
+    first solve) and replays it, also in later solves: iteration counts, residual history and solution equal the
+    oracle's, solve after solve."""
+    orders = (5, 2)
+    meshes = [inputs.box_mesh(4, 4, 3, N, "random", seed=5) for N in orders]
+    olv = [oracle_mod.Level(m) for m in meshes]
+    L0 = olv[0]
+    xs = np.where(L0.mask_u != 0, 0.0, inputs.field_normal(L0.maps.uniq_gid, 17))
+    b_u = L0.A(xs)
+    ores = oracle_mod.fpcg(L0, lambda r: oracle_mod.vcycle(olv, r, 2, 6), b_u, tol=1e-9, maxit=60)
+    side = torch_cuda.cuda.Stream()
+    with torch_cuda.cuda.stream(side):
+        sems = [make_sem(binding, m, dirichlet=True) for m in meshes]
+        try:
+            with binding.Pmg(sems, [l.lmin for l in olv], [l.lmax for l in olv], 2, 6, binding.SEM_F64) as mg:
+                b = to_dev(torch_cuda, b_u[L0.maps.l2u])
+                x = torch_cuda.empty_like(b)
+                for solve in range(3):
+                    x.fill_(float("nan"))
+                    it, rel = mg.fpcg(b, x, 1e-9, 60)
+                    assert it == ores["iters"] and rel <= 1e-9, solve
+                    assert np.max(np.abs(mg.history(it + 1) - ores["hist"]) / ores["hist"]) <= 1e-6, solve
+                    assert relerr(x.cpu().numpy(), ores["x"][L0.maps.l2u]) <= 1e-8, solve
+                b2 = b * 2.0                                   # another right-hand side: the graph is recorded anew
+                it, _ = mg.fpcg(b2, x, 1e-9, 60)
+                assert it == ores["iters"] and relerr(x.cpu().numpy(), 2.0 * ores["x"][L0.maps.l2u]) <= 1e-8
+        finally:
+            for s_ in sems:
+                s_.close()
