@@ -258,9 +258,12 @@ def main():
     # ---- the metric: K applications of the whole path, inputs resident in HBM (working set 236 MB > 126 MB L2) ----
     ms_total = timed(lambda: sem.ax_gs(u, w), K)
     # ---- kernel shares: the local operator alone, the gather-scatter alone ----
-    ms_ax = timed(lambda: sem.ax(u, w), K)
+    # (bursts of at most 500 launches: MEASURED_PEAKS.json's hbm_gbs is a burst figure, "best of 10", and 5000 launches
+    # of one kernel alone run into the power cap, which the whole-step loop above already reflects)
+    Kk = min(K, 500)
+    ms_ax = timed(lambda: sem.ax(u, w), Kk)
     wz = torch.zeros_like(u)
-    ms_gs = timed(lambda: sem.gs(wz), K)
+    ms_gs = timed(lambda: sem.gs(wz), Kk)
     clocks = sampler.stop() if sampler else None
 
     # ---- e2e: host buffers, H2D of u and D2H of w inside every timed step.  Two lanes (context + stream + device
@@ -353,7 +356,7 @@ def main():
     value = whole_job_value(dofs, world, K, ms_total)
     e2e_value = whole_job_value(dofs, world, Ke, ms_e2e)
     peak, peak_src = measured_peak_gbs()
-    ax_s = ms_ax * 1e-3 / K
+    ax_s = ms_ax * 1e-3 / Kk
     ax_bytes = 64.0 * nL                                     # 64 B per local node, FP64, stored G
     achieved = ax_bytes / ax_s / 1e9
     whole_bytes = 64.0 * nL + 16.0 * S
@@ -373,9 +376,9 @@ def main():
         "roofline": {"bound": "hbm", "kernel": "ax_stream<double,8,5,8> (local D^T G D u)", "achieved": achieved,
                      "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": ncu_traffic_bytes(),
                      "peak_source": peak_src, "algorithmic_bytes_per_launch": ax_bytes,
-                     "us_per_launch": ax_s * 1e6, "timed": f"{K} back-to-back launches of sem_ax alone, CUDA events",
+                     "us_per_launch": ax_s * 1e6, "timed": f"{Kk} back-to-back launches of sem_ax alone, CUDA events",
                      "frac_of_nominal_8TBs": achieved / 8000.0},
-        "breakdown": {"ax_us": ms_ax / K * 1e3, "gs_us": ms_gs / K * 1e3, "ax_gs_us": ms_total / K * 1e3,
+        "breakdown": {"ax_us": ms_ax / Kk * 1e3, "gs_us": ms_gs / Kk * 1e3, "ax_gs_us": ms_total / K * 1e3,
                       "ax_gs_algorithmic_GBs": whole_bytes / (ms_total * 1e-3 / K) / 1e9,
                       "ax_gs_frac_of_measured_peak": whole_bytes / (ms_total * 1e-3 / K) / 1e9 / peak,
                       "ax_gs_frac_of_nominal_8TBs": whole_bytes / (ms_total * 1e-3 / K) / 1e9 / 8000.0,
