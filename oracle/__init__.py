@@ -338,3 +338,42 @@ class Projection:
         self.P = np.vstack([self.P, (dx - beta @ self.P) * s])
         self.AP = np.vstack([self.AP, (w - beta @ self.AP) * s])
         return True
+
+
+# ---- NEXT-2a: fast-diagonalisation local solve of the Schwarz smoother, Eq. (3) -------------------------
+def fdm_eig(A: np.ndarray, B: np.ndarray):
+    """One direction of one element: the generalised symmetric eigenproblem A s = lambda B s of the 1-D operator pair
+    (stiffness A, mass B; both m x m, symmetric, B positive definite), normalised S^T B S = I so that S^T A S = diag(lam)
+    (fast diagonalisation, Deville et al. 2002 as cited at P:103).  Library routine as a step: scipy.linalg.eigh.
+    Returns (S[m, m] with eigenvectors in columns, lam[m] ascending)."""
+    import scipy.linalg
+    lam, S = scipy.linalg.eigh(np.asarray(A, dtype=np.float64), np.asarray(B, dtype=np.float64))
+    return S, lam
+
+
+def fdm_inv_lambda(lam_x, lam_y, lam_z) -> np.ndarray:
+    """Lambda^-1 of Eq. (3) as an [m][m][m] array indexed [c][b][a] (z, y, x eigen-index; x fastest): the separable
+    operator Bz x By x Ax + Bz x Ay x Bx + Az x By x Bx is diagonalised by Sz x Sy x Sx to lam_x[a] + lam_y[b] + lam_z[c]
+    ("Lambda is a diagonal matrix with only 1,000 nonzeros" at m = 10)."""
+    lx, ly, lz = (np.asarray(v, dtype=np.float64) for v in (lam_x, lam_y, lam_z))
+    return 1.0 / (lz[:, None, None] + ly[None, :, None] + lx[None, None, :])
+
+
+def fdm_apply(S: np.ndarray, inv_lambda: np.ndarray, b: np.ndarray) -> np.ndarray:
+    """Eq. (3), for every element e:  u^e = (S_z x S_y x S_x) Lambda^-1 (S_z^T x S_y^T x S_x^T) b^e.
+    S[E][3][m][m] (direction x, y, z; S_d[row][col], eigenvectors in columns), inv_lambda[E][m][m][m], b[E][m][m][m]
+    stored [k][j][i] with i (x) fastest, like every local field.  FP64; the three 1-D contractions are written out one
+    by one in the order of the formula (transposes first, then the diagonal, then the forward matrices)."""
+    S = np.asarray(S, dtype=np.float64)
+    b = np.asarray(b, dtype=np.float64)
+    u = np.empty_like(b)
+    for e in range(b.shape[0]):
+        Sx, Sy, Sz = S[e, 0], S[e, 1], S[e, 2]
+        t = np.einsum("ia,kji->kja", Sx, b[e])           # S_x^T along i
+        t = np.einsum("jb,kja->kba", Sy, t)              # S_y^T along j
+        t = np.einsum("kc,kba->cba", Sz, t)              # S_z^T along k
+        t = t * inv_lambda[e]
+        t = np.einsum("kc,cba->kba", Sz, t)              # S_z
+        t = np.einsum("jb,kba->kja", Sy, t)              # S_y
+        u[e] = np.einsum("ia,kja->kji", Sx, t)           # S_x
+    return u

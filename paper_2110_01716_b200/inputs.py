@@ -176,3 +176,26 @@ def config4(N: int) -> BoxMesh:
 def config5(n: int = 100) -> BoxMesh:
     """Full solve: n^3 elements (100^3 at full size), N=7, random perturbation seed 3, element permutation seed 4."""
     return box_mesh(n, n, n, 7, "random", frac=0.1, seed=3, permute_seed=4, name=f"cfg5_{n}^3_N7_random_perm")
+
+
+def fdm_pairs(E: int, m: int, seed: int):
+    """Seeded stand-in for the 1-D operator pairs (A_d, B_d), d = x, y, z, of the Schwarz smoother's extended local
+    problems (the paper does not give their construction, reading S28 in DESIGN.md): on a 1-D grid of m
+    interior points clustered towards the ends like GLL points (x_q = -cos(pi q / (m+1)), homogeneous Dirichlet at
+    q = 0 and q = m+1), scaled by a seeded element length h_d in [0.5, 1.5], A = the linear finite-element stiffness
+    matrix (tridiagonal, SPD) and B = the lumped mass matrix (diagonal, positive).  Returns A[E][3][m][m], B[E][3][m][m]
+    (FP64).  Mesh-like data only: the eigen-decomposition and Eq. (3) are the method's, not this module's."""
+    cnt = np.arange(E * 3, dtype=np.uint64)
+    h = (0.5 + hash_uniform01(seed, 11, cnt)).reshape(E, 3)
+    x = -np.cos(np.pi * np.arange(m + 2) / (m + 1))                 # [m+2] reference grid on [-1, 1]
+    dx = np.diff(x)                                                 # [m+1]
+    A = np.zeros((E, 3, m, m))
+    B = np.zeros((E, 3, m, m))
+    q = np.arange(m)
+    for e in range(E):
+        for d in range(3):
+            s = 0.5 * h[e, d] * dx                                  # physical cell sizes
+            A[e, d, q, q] = 1.0 / s[:-1] + 1.0 / s[1:]
+            A[e, d, q[:-1], q[1:]] = A[e, d, q[1:], q[:-1]] = -1.0 / s[1:-1]
+            B[e, d, q, q] = 0.5 * (s[:-1] + s[1:])
+    return A, B

@@ -681,3 +681,87 @@ def test_J1_projection_is_the_A_orthogonal_best_fit(oracle_mod, pmg_levels):
     p2 = oracle_mod.Projection(L0.A, n, Lmax=30)
     assert p2.update(base) and p2.update(drift)
     assert p2.update(1e-3 * p2.P[0] + 2.0 * p2.P[1]) is False and p2.P.shape[0] == 2
+
+
+# --------------------------------------- NEXT-2a: fast-diagonalisation local solve of the Schwarz smoother, Eq. (3)
+def _spd(rng, m, shift):
+    M = rng.standard_normal((m, m))
+    return M @ M.T + shift * np.eye(m)
+
+
+def test_F1_fdm_is_the_inverse_of_the_separable_operator(oracle_mod):
+    """Eq. (3) with S_d, lam_d from A_d s = lam B_d s (S^T B S = I) is the exact inverse of the dense
+    Bz x By x Ax + Bz x Ay x Bx + Az x By x Bx (x fastest), built here with numpy.kron and solved with a dense LU:
+    different dense SPD pairs per direction, so a transposed S, a swapped direction or a wrong Lambda index fails."""
+    rng = np.random.default_rng(21)
+    m, E = 4, 3
+    S = np.empty((E, 3, m, m))
+    invL = np.empty((E, m, m, m))
+    K = []
+    for e in range(E):
+        A = [_spd(rng, m, 0.5) for _ in range(3)]
+        B = [_spd(rng, m, 2.0) for _ in range(3)]
+        lam = []
+        for d in range(3):
+            S[e, d], l = oracle_mod.fdm_eig(A[d], B[d])
+            lam.append(l)
+            assert np.max(np.abs(S[e, d].T @ B[d] @ S[e, d] - np.eye(m))) <= 1e-12
+            assert np.max(np.abs(S[e, d].T @ A[d] @ S[e, d] - np.diag(l))) <= 1e-11
+        invL[e] = oracle_mod.fdm_inv_lambda(*lam)
+        K.append(np.kron(B[2], np.kron(B[1], A[0])) + np.kron(B[2], np.kron(A[1], B[0]))
+                 + np.kron(A[2], np.kron(B[1], B[0])))
+    b = rng.standard_normal((E, m, m, m))
+    u = oracle_mod.fdm_apply(S, invL, b)
+    for e in range(E):
+        ref = np.linalg.solve(K[e], b[e].ravel())
+        assert np.max(np.abs(u[e].ravel() - ref)) <= 1e-10 * np.max(np.abs(ref))
+
+
+def test_F2_fdm_solves_the_7_point_laplacian_with_the_closed_form_spectrum(oracle_mod):
+    """Textbook special case: A_d = tridiag(-1, 2, -1), B_d = I on m_x x m_y x m_z interior points.  The eigenvalues are
+    2 - 2 cos(q pi / (m+1)) (closed form) and Eq. (3) solves the 7-point finite-difference Poisson problem, checked by
+    applying the stencil to the result with plain array shifts.  Unequal sizes are emulated by padding to a cube with
+    decoupled identity rows, which also pins that the three directions are not interchanged."""
+    m = 6
+    T = 2.0 * np.eye(m) - np.eye(m, k=1) - np.eye(m, k=-1)
+    Sx, lx = oracle_mod.fdm_eig(T, np.eye(m))
+    assert np.max(np.abs(lx - (2.0 - 2.0 * np.cos(np.arange(1, m + 1) * np.pi / (m + 1))))) <= 1e-13
+    # anisotropic: x uses T, y uses 4 T, z uses 9 T (grid spacings 1, 1/2, 1/3)
+    Sy, ly = oracle_mod.fdm_eig(4.0 * T, np.eye(m))
+    Sz, lz = oracle_mod.fdm_eig(9.0 * T, np.eye(m))
+    S = np.stack([Sx, Sy, Sz])[None]
+    invL = oracle_mod.fdm_inv_lambda(lx, ly, lz)[None]
+    rng = np.random.default_rng(22)
+    b = rng.standard_normal((1, m, m, m))
+    u = oracle_mod.fdm_apply(S, invL, b)[0]
+    up = np.pad(u, 1)                                                        # homogeneous Dirichlet halo
+    c = up[1:-1, 1:-1, 1:-1]
+    lap = (1.0 * (2 * c - up[1:-1, 1:-1, :-2] - up[1:-1, 1:-1, 2:])          # i = x, fastest
+           + 4.0 * (2 * c - up[1:-1, :-2, 1:-1] - up[1:-1, 2:, 1:-1])        # j = y
+           + 9.0 * (2 * c - up[:-2, 1:-1, 1:-1] - up[2:, 1:-1, 1:-1]))       # k = z
+    assert np.max(np.abs(lap - b[0])) <= 1e-11 * np.max(np.abs(b))
+
+
+def test_F3_fdm_is_symmetric_positive_definite_on_the_synthetic_pairs(oracle_mod):
+    """On the seeded operator pairs of inputs.fdm_pairs (the parity and bench inputs): c.F(b) = b.F(c), b.F(b) > 0,
+    and F inverts the dense separable operator (m = 5, E = 4)."""
+    m, E = 5, 4
+    A, B = inputs.fdm_pairs(E, m, seed=6)
+    assert np.all(A == np.transpose(A, (0, 1, 3, 2))) and np.all(np.linalg.eigvalsh(A) > 0) and np.all(np.linalg.eigvalsh(B) > 0)
+    S = np.empty_like(A)
+    invL = np.empty((E, m, m, m))
+    for e in range(E):
+        lam = []
+        for d in range(3):
+            S[e, d], l = oracle_mod.fdm_eig(A[e, d], B[e, d])
+            lam.append(l)
+        invL[e] = oracle_mod.fdm_inv_lambda(*lam)
+    rng = np.random.default_rng(23)
+    b, c = rng.standard_normal((2, E, m, m, m))
+    Fb, Fc = oracle_mod.fdm_apply(S, invL, b), oracle_mod.fdm_apply(S, invL, c)
+    for e in range(E):
+        assert abs(np.vdot(c[e], Fb[e]) - np.vdot(b[e], Fc[e])) <= 1e-12 * abs(np.vdot(c[e], Fb[e])) + 1e-14
+        assert np.vdot(b[e], Fb[e]) > 0
+        K = (np.kron(B[e, 2], np.kron(B[e, 1], A[e, 0])) + np.kron(B[e, 2], np.kron(A[e, 1], B[e, 0]))
+             + np.kron(A[e, 2], np.kron(B[e, 1], B[e, 0])))
+        assert np.max(np.abs(K @ Fb[e].ravel() - b[e].ravel())) <= 1e-10 * np.max(np.abs(b[e]))
