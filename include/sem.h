@@ -185,6 +185,22 @@ SEM_API int sem_proj_update(sem_proj* pj, const double* dx, int* accepted);
 SEM_API int sem_proj_size(sem_proj* pj, int* L);
 SEM_API void sem_proj_destroy(sem_proj* pj);
 
+/* NEXT-2a.  Fast-diagonalisation local solve of the Schwarz smoothers, Eq. (3): for every
+ * element e of the context
+ *      u^e = (S_z x S_y x S_x) Lambda^-1 (S_z^T x S_y^T x S_x^T) b^e
+ * on the element's extended m x m x m block (m = N + 3 in the paper: "for an 8 x 8 x 8 brick (N = 7), one solves a
+ * 10 x 10 x 10 local problem"; any 2 <= m <= 16 is accepted and m need not be related to the context's N).  With
+ * S_d^T B_d S_d = I, S_d^T A_d S_d = diag(lam_d) and Lambda[c][b][a] = lam_x[a] + lam_y[b] + lam_z[c] this is the exact
+ * inverse of Bz x By x Ax + Bz x Ay x Bx + Az x By x Bx.  Building the blocks (the face-only exchange of P:107), the
+ * weighting and the sum back into the residual are not part of this call (NEXT-2b).
+ *   S           DEVICE [E][3][m][m]: direction d = 0,1,2 = x,y,z; S_d[row][col] row-major, eigenvectors in columns
+ *   inv_lambda  DEVICE [E][m][m][m]: 1/Lambda, eigen-indices [c][b][a] (z, y, x; x fastest)
+ *   b, u        DEVICE [E][m][m][m], [k][j][i] with i (x) fastest; u may alias b (in place)
+ * All four arrays hold `prec` values (S and inv_lambda rounded by the caller; accumulation in `prec`).
+ * Asynchronous on the context's stream; needs only sem_mesh_setup (E and the stream).  SEM_EINVAL for m outside 2..16. */
+SEM_API int sem_fdm_apply(sem_ctx* ctx, int m, const void* S, const void* inv_lambda, const void* b, void* u,
+                          sem_prec prec);
+
 /* Tuning knob for experiments: selects the Ax kernel variant (0 = default streaming kernel, 1 = simple kernel). */
 SEM_API int sem_set_variant(sem_ctx* ctx, int ax_variant);
 

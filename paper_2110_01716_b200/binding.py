@@ -52,6 +52,7 @@ SYMBOLS = {
     "sem_proj_destroy": (None, [_vp]),
     "sem_fpcg": (_i32, [_vp, _vp, _vp, _dbl, _i32, C.POINTER(_i32), C.POINTER(_dbl)]),
     "sem_pmg_get_history": (_i32, [_vp, _vp, _i32]),
+    "sem_fdm_apply": (_i32, [_vp, _i32, _vp, _vp, _vp, _vp, _i32]),
     "sem_last_error": (C.c_char_p, [_vp]),
     "sem_ctx_destroy": (None, [_vp]),
 }
@@ -195,6 +196,16 @@ class Sem:
         if rc != SEM_OK:
             raise SemError(rc, self._L.sem_last_error(fine._h).decode())
         return vout
+
+    def fdm_apply(self, m: int, S, inv_lambda, b, u):
+        """sem_fdm_apply (Eq. (3)): S[E][3][m][m], inv_lambda[E][m^3], b, u [E][m^3]; u may be b."""
+        m3 = m * m * m
+        for t, n in ((S, self.E * 3 * m * m), (inv_lambda, self.E * m3), (b, self.E * m3), (u, self.E * m3)):
+            assert t.is_cuda and t.is_contiguous() and t.numel() == n and t.dtype == b.dtype, \
+                "need contiguous CUDA tensors of one dtype with E*3*m*m / E*m^3 values"
+        self._check(self._L.sem_fdm_apply(self._h, m, C.c_void_p(S.data_ptr()), C.c_void_p(inv_lambda.data_ptr()),
+                                          C.c_void_p(b.data_ptr()), C.c_void_p(u.data_ptr()), self._prec(b)))
+        return u
 
     def interp(self, fine: "Sem") -> np.ndarray:
         J = np.empty((fine.N + 1, self.N + 1))

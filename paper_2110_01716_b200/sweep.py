@@ -167,8 +167,37 @@ def run_projection(peak: float):
                   f"31 vectors read by the multi-dot, 61 read + 2 written by the update pass)")
 
 
+def run_fdm(peak: float):
+    """NEXT-2a: sem_fdm_apply (Eq. (3)) at the paper's per-GPU element count, m = N + 3 for N = 7, 5, 3, 1 and
+    the paper's 8-5-1 / 8-6-4-1 schedules.  Bytes = b, Lambda^-1, u (m^3 each) + S (3 m^2) per element; flops = 12 m^4."""
+    import numpy as np
+    import scipy.linalg
+    E = 7200
+    mesh = inputs.box_mesh(E, 1, 1, 1)
+    print("| m | precision | us | GB/s | frac of HBM peak | TFLOP/s |")
+    print("|---|---|---|---|---|---|")
+    with binding.Sem(mesh.E, 1, mesh.vert, mesh.gid) as sem:
+        for m in (10, 8, 7, 6, 5, 4, 12):
+            A, B = inputs.fdm_pairs(E, m, 7)
+            S = np.empty_like(A)
+            lam = np.empty((E, 3, m))
+            for e in range(E):
+                for d in range(3):
+                    lam[e, d], S[e, d] = scipy.linalg.eigh(A[e, d], B[e, d])
+            invL = 1.0 / (lam[:, 2, :, None, None] + lam[:, 1, None, :, None] + lam[:, 0, None, None, :])
+            for dt, name in ((torch.float32, "FP32"), (torch.float64, "FP64")):
+                dS, dL = (torch.from_numpy(a.ravel()).cuda().to(dt) for a in (S, invL))
+                b = torch.randn(E * m ** 3, device="cuda", dtype=dt)
+                u = torch.empty_like(b)
+                t = _time(lambda: sem.fdm_apply(m, dS, dL, b, u), 500)
+                nbytes = b.element_size() * E * (3 * m ** 3 + 3 * m * m)
+                print(f"| {m} | {name} | {t:.2f} | {nbytes / t / 1e3:.0f} | {nbytes / t / 1e3 / peak:.2f} | "
+                      f"{12.0 * m ** 4 * E / t / 1e6:.2f} |", flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--fdm", action="store_true", help="NEXT-2a: fast-diagonalisation local solve (Eq. (3)) at E = 7200")
     ap.add_argument("--proj", action="store_true", help="NEXT-3: projection onto previous solutions at config 2")
     ap.add_argument("--config5", type=int, default=0, help="run config 5 with this many elements per direction")
     ap.add_argument("--max-n", type=int, default=64)
@@ -182,6 +211,8 @@ def main():
         return run_config5(args.config5, peak)
     if args.proj:
         return run_projection(peak)
+    if args.fdm:
+        return run_fdm(peak)
     print(f"peak = {peak:.0f} GB/s (MEASURED_PEAKS.json hbm_gbs, else the profiling guide's fallback)")
     print("| case | E | N | nL | Ax us | Ax GB/s | frac of peak | gs us | Ax+gs us | Ax+gs GB/s | GDOF/s (E N^3) | "
           "Ax recomputed-G us | recomputed TFLOP/s |")

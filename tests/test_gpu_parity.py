@@ -893,3 +893,48 @@ def test_fpcg_iteration_graph_on_side_stream(torch_cuda, binding, oracle_mod):
         finally:
             for s_ in sems:
                 s_.close()
+
+
+# ------------------------------------------- NEXT-2a: fast-diagonalisation local solve of the Schwarz smoother, Eq. (3)
+def _fdm_inputs(oracle_mod, E, m, seed):
+    """Seeded operator pairs -> (S, Lambda^-1) by the oracle's eigen-decomposition (inputs of Eq. (3)) and a seeded b."""
+    A, B = inputs.fdm_pairs(E, m, seed)
+    S = np.empty_like(A)
+    invL = np.empty((E, m, m, m))
+    for e in range(E):
+        lam = []
+        for d in range(3):
+            S[e, d], l = oracle_mod.fdm_eig(A[e, d], B[e, d])
+            lam.append(l)
+        invL[e] = oracle_mod.fdm_inv_lambda(*lam)
+    b = 2.0 * inputs.hash_uniform01(seed, 12, np.arange(E * m ** 3)).reshape(E, m, m, m) - 1.0
+    return S, invL, b
+
+
+@pytest.mark.parametrize("m,E", [(10, 1500), (10, 3), (4, 5000), (6, 777), (8, 1201), (12, 301), (7, 450), (9, 333),
+                                 (2, 100), (3, 65), (5, 129), (16, 150), (13, 97)])
+def test_fdm_apply_parity(torch_cuda, binding, oracle_mod, m, E):
+    """sem_fdm_apply against the oracle's Eq. (3) on the same S, Lambda^-1, b: FP64 1e-12, FP32 1e-5 (normalised by
+    max |u| per case), more elements than one wave of CTAs holds at m = 10 and a ragged last group; in place too."""
+    S, invL, b = _fdm_inputs(oracle_mod, E, m, seed=30 + m)
+    ou = oracle_mod.fdm_apply(S, invL, b)
+    mesh = inputs.box_mesh(E, 1, 1, 1)                                   # the call only needs E and the stream
+    with binding.Sem(mesh.E, 1, mesh.vert, mesh.gid) as sem:
+        for dt, tol in ((torch_cuda.float64, TOL64), (torch_cuda.float32, TOL32)):
+            dS, dL, db = (to_dev(torch_cuda, a.ravel(), dt) for a in (S, invL, b))
+            du = torch_cuda.full_like(db, float("nan"))
+            sem.fdm_apply(m, dS, dL, db, du)
+            assert relerr(du.cpu().numpy(), ou.ravel()) <= tol, (m, E, dt)
+            sem.fdm_apply(m, dS, dL, db, db)                             # in place
+            assert torch_cuda.equal(db, du)
+
+
+def test_fdm_apply_bad_args(torch_cuda, binding):
+    mesh = inputs.box_mesh(2, 1, 1, 1)
+    with binding.Sem(mesh.E, 1, mesh.vert, mesh.gid) as sem:
+        z = torch_cuda.zeros(2 * 17 ** 3, dtype=torch_cuda.float64, device="cuda")
+        for m in (1, 17):
+            rc = sem._L.sem_fdm_apply(sem._h, m, z.data_ptr(), z.data_ptr(), z.data_ptr(), z.data_ptr(), binding.SEM_F64)
+            assert rc == binding.SEM_EINVAL
+        assert sem._L.sem_fdm_apply(sem._h, 4, None, z.data_ptr(), z.data_ptr(), z.data_ptr(), binding.SEM_F64) == binding.SEM_EINVAL
+        assert sem._L.sem_fdm_apply(sem._h, 4, z.data_ptr(), z.data_ptr(), z.data_ptr(), z.data_ptr(), 5) == binding.SEM_EINVAL
