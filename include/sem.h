@@ -196,7 +196,8 @@ SEM_API void sem_proj_destroy(sem_proj* pj);
  *   S           DEVICE [E][3][m][m]: direction d = 0,1,2 = x,y,z; S_d[row][col] row-major, eigenvectors in columns
  *   inv_lambda  DEVICE [E][m][m][m]: 1/Lambda, eigen-indices [c][b][a] (z, y, x; x fastest)
  *   b, u        DEVICE [E][m][m][m], [k][j][i] with i (x) fastest; u may alias b (in place)
- * All four arrays hold `prec` values (S and inv_lambda rounded by the caller; accumulation in `prec`).
+ * All four arrays hold `prec` values (S and inv_lambda rounded by the caller; accumulation in `prec`) and are 16-byte
+ * aligned (SEM_EINVAL otherwise).
  * Asynchronous on the context's stream; needs only sem_mesh_setup (E and the stream).  SEM_EINVAL for m outside 2..16. */
 SEM_API int sem_fdm_apply(sem_ctx* ctx, int m, const void* S, const void* inv_lambda, const void* b, void* u,
                           sem_prec prec);

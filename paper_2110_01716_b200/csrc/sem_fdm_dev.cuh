@@ -1,0 +1,208 @@
+// sem_fdm_dev.cuh -- the kernel of sem_fdm.cu (design notes there).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace sem_fdm_dev {
+
+
+template <typename T> struct vec16;
+template <> struct vec16<float> { using type = float4; static constexpr int n = 4; };
+template <> struct vec16<double> { using type = double2; static constexpr int n = 2; };
+
+// LPT_ = lines per thread (they share every S row load), EPC_ = elements per CTA
+template <typename T, int M, int LPT_, int EPC_>
+struct fdm_cfg {
+    static constexpr int VEC = vec16<T>::n;
+    static constexpr int MP = (M + VEC - 1) / VEC * VEC;          // padded row length: rows start 16-byte aligned
+    static constexpr int LINES = M * M;                           // lines per element and phase
+    static constexpr int LPT = LPT_;
+    static constexpr int TPE = (LINES + LPT - 1) / LPT;           // threads per element
+    static constexpr int EPC = EPC_;
+    static constexpr int NT = EPC * TPE;
+    static constexpr int S_EL = 3 * M * MP;                       // padded S values per element
+    static constexpr int B_EL = M * M * MP;                       // padded block values per element
+    static constexpr int STAGE = EPC * (S_EL + 2 * B_EL);         // S, Lambda^-1 and the block of EPC elements
+    static constexpr size_t SMEM1 = sizeof(T) * (size_t)STAGE;    // per stage
+};
+
+// row[0..M) <- the M values at `src` (16-byte aligned, padded to MP), 128-bit shared-memory loads
+template <typename T, int M>
+__device__ __forceinline__ void load_row(const T* __restrict__ src, T (&row)[fdm_cfg<T, M, 1, 1>::MP]) {
+    using V = typename vec16<T>::type;
+    constexpr int VEC = vec16<T>::n;
+#pragma unroll
+    for (int q = 0; q < fdm_cfg<T, M, 1, 1>::MP / VEC; ++q) {
+        const V v = reinterpret_cast<const V*>(src)[q];
+        if constexpr (VEC == 4) {
+            row[4 * q] = v.x; row[4 * q + 1] = v.y; row[4 * q + 2] = v.z; row[4 * q + 3] = v.w;
+        } else {
+            row[2 * q] = v.x; row[2 * q + 1] = v.y;
+        }
+    }
+}
+
+// One 1-D contraction of the thread's LPT lines, walking the rows of S (sS: [M][MP]) so that each row is loaded once
+// for all of them.  ld(r, l) yields element l of line r, st(r, o, v) takes element o of the result.
+//   TRANSPOSED (S^T applied):  out[o] = sum_l S[l][o] in[l]: the inputs are consumed one at a time (read just in time,
+//                              never all live), the M accumulators per line stay in registers and are stored at the end;
+//   otherwise  (S applied):    out[o] = sum_l S[o][l] in[l]: the inputs are read first, every result is stored as soon as
+//                              its dot product is done (never all live).
+// Either way a line costs M + small registers instead of 2 M.
+template <typename T, int M, int LPT, bool TRANSPOSED, class Ld, class St>
+__device__ __forceinline__ void contract_lines(const T* __restrict__ sS, Ld ld, St st) {
+    constexpr int MP = fdm_cfg<T, M, 1, 1>::MP;
+    if constexpr (TRANSPOSED) {
+        T acc[LPT][M];
+#pragma unroll
+        for (int r = 0; r < LPT; ++r)
+#pragma unroll
+            for (int o = 0; o < M; ++o) acc[r][o] = T(0);
+#pragma unroll
+        for (int l = 0; l < M; ++l) {
+            T row[MP];
+            load_row<T, M>(sS + l * MP, row);
+#pragma unroll
+            for (int r = 0; r < LPT; ++r) {
+                const T v = ld(r, l);
+#pragma unroll
+                for (int o = 0; o < M; ++o) acc[r][o] += row[o] * v;
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < LPT; ++r)
+#pragma unroll
+            for (int o = 0; o < M; ++o) st(r, o, acc[r][o]);
+    } else {
+        T in[LPT][M];
+#pragma unroll
+        for (int r = 0; r < LPT; ++r)
+#pragma unroll
+            for (int l = 0; l < M; ++l) in[r][l] = ld(r, l);
+#pragma unroll
+        for (int o = 0; o < M; ++o) {
+            T row[MP];
+            load_row<T, M>(sS + o * MP, row);
+#pragma unroll
+            for (int r = 0; r < LPT; ++r) {
+                T v = T(0);
+#pragma unroll
+                for (int l = 0; l < M; ++l) v += row[l] * in[r][l];
+                st(r, o, v);
+            }
+        }
+    }
+}
+
+// cp.async (LDGSTS) of BYTES (4, 8 or 16) from global to shared memory, no registers in between
+template <int BYTES>
+__device__ __forceinline__ void cp_async(void* smem_dst, const void* gsrc) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(d), "l"(gsrc), "n"(BYTES) : "memory");
+}
+
+// rows of M values, contiguous in global memory, to rows padded to MP in shared memory, by all NT threads of the CTA
+template <typename T, int M, int NT>
+__device__ __forceinline__ void copy_rows_async(T* __restrict__ sdst, const T* __restrict__ gsrc, int nrows) {
+    constexpr int MP = fdm_cfg<T, M, 1, 1>::MP;
+    constexpr int RB = M * (int)sizeof(T);
+    constexpr int CH = RB % 16 == 0 ? 16 : RB % 8 == 0 ? 8 : 4;      // chunk bytes: row starts stay CH-aligned
+    constexpr int CPR = RB / CH, VPC = CH / (int)sizeof(T);
+    for (int t = threadIdx.x; t < nrows * CPR; t += NT) {
+        const int row = t / CPR, c = t - row * CPR;
+        cp_async<CH>(sdst + row * MP + c * VPC, gsrc + (int64_t)row * M + c * VPC);
+    }
+}
+
+// MINB = resident CTAs per SM the register allocation is held to.  NSTAGE = 2: two shared-memory stages of
+// {S, Lambda^-1, block}: while a group of EPC elements is worked on in one stage, the next group's operands land in the
+// other (cp.async).  NSTAGE = 1: one stage (half the shared memory, twice the resident CTAs hide the copy instead).
+template <typename T, int M, int LPT_, int EPC_, int MINB, int NSTAGE>
+__global__ void __launch_bounds__((fdm_cfg<T, M, LPT_, EPC_>::NT), MINB)
+k_fdm(int64_t E, const T* __restrict__ S, const T* __restrict__ invL, const T* b, T* u) {
+    using C = fdm_cfg<T, M, LPT_, EPC_>;
+    constexpr int MP = C::MP, LPT = C::LPT, TPE = C::TPE, EPC = C::EPC, M2 = M * M, M3 = M * M * M, NT = C::NT;
+    constexpr int STG = C::STAGE;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* smem = reinterpret_cast<T*>(smem_raw);
+    const int el = threadIdx.x / TPE, tl = threadIdx.x - el * TPE;
+    const int64_t ngrp = (E + EPC - 1) / EPC;
+
+    auto issue = [&](int64_t grp, int stage) {
+        const int64_t e0 = grp * EPC;
+        const int ne = (int)((E - e0) < EPC ? (E - e0) : EPC);
+        T* st = smem + stage * STG;
+        copy_rows_async<T, M, NT>(st, S + e0 * 3 * M2, ne * 3 * M);
+        copy_rows_async<T, M, NT>(st + EPC * C::S_EL, invL + e0 * M3, ne * M2);
+        copy_rows_async<T, M, NT>(st + EPC * (C::S_EL + C::B_EL), b + e0 * M3, ne * M2);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+
+    if (NSTAGE == 2 && (int64_t)blockIdx.x < ngrp) issue(blockIdx.x, 0);
+    int stage = 0;
+    for (int64_t grp = blockIdx.x; grp < ngrp; grp += gridDim.x, stage ^= (NSTAGE - 1)) {
+        const int64_t e = grp * EPC + el;
+        const bool live = e < E;
+        T* stg = smem + stage * STG;
+        const T* sS = stg + el * C::S_EL;                              // [3][M][MP]: x, y, z
+        const T* sL = stg + EPC * C::S_EL + el * C::B_EL;              // [c][b][MP]
+        T* sB = stg + EPC * (C::S_EL + C::B_EL) + el * C::B_EL;        // [k][j][MP]
+        if (NSTAGE == 1) {
+            __syncthreads();              // the previous group is no longer read
+            issue(grp, 0);
+        }
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncthreads();                  // this stage has landed for everyone; the other stage is no longer read
+        if (NSTAGE == 2 && grp + gridDim.x < ngrp) issue(grp + gridDim.x, stage ^ 1);
+        int q[LPT], a[LPT], c[LPT];       // line q = a * M + c of the element
+        bool ok[LPT];
+#pragma unroll
+        for (int r = 0; r < LPT; ++r) {
+            q[r] = tl + r * TPE;
+            ok[r] = q[r] < M2;
+            if (!ok[r]) q[r] = M2 - 1;                // an idle slot (M^2 not a multiple of LPT) computes but never stores
+            a[r] = q[r] / M;
+            c[r] = q[r] - a[r] * M;
+        }
+        // line ownership: "outer" = (j,i) owns a k-line (element l at (l*M + a)*MP + c); "mid" = (k,i) owns a j-line
+        // (element l at (a*M + l)*MP + c); "inner" = (k,j) owns an i-line (row q).  A line is read and written by its
+        // owner only, so the barriers sit between the phases and nowhere else.
+        auto ld_outer = [&](int r, int l) { return sB[(l * M + a[r]) * MP + c[r]]; };
+        auto st_outer = [&](int r, int o, T v) { if (ok[r]) sB[(o * M + a[r]) * MP + c[r]] = v; };
+        auto ld_mid = [&](int r, int l) { return sB[(a[r] * M + l) * MP + c[r]]; };
+        auto st_mid = [&](int r, int o, T v) { if (ok[r]) sB[(a[r] * M + o) * MP + c[r]] = v; };
+        // ---- phase 1: S_z^T on k-lines ----
+        contract_lines<T, M, LPT, true>(sS + 2 * M * MP, ld_outer, st_outer);
+        __syncthreads();
+        // ---- phase 2: S_y^T on j-lines ----
+        contract_lines<T, M, LPT, true>(sS + M * MP, ld_mid, st_mid);
+        __syncthreads();
+        // ---- phase 3: S_x^T, Lambda^-1, S_x on i-lines (rows: 128-bit accesses) ----
+        {
+            T v[LPT][MP];
+#pragma unroll
+            for (int r = 0; r < LPT; ++r) load_row<T, M>(sB + q[r] * MP, v[r]);
+            T w[LPT][M];
+            contract_lines<T, M, LPT, true>(sS, [&](int r, int l) { return v[r][l]; },
+                                            [&](int r, int o, T x) { w[r][o] = x; });
+#pragma unroll
+            for (int r = 0; r < LPT; ++r) {
+                load_row<T, M>(sL + q[r] * MP, v[r]);
+#pragma unroll
+                for (int i = 0; i < M; ++i) w[r][i] *= v[r][i];
+            }
+            contract_lines<T, M, LPT, false>(sS, [&](int r, int l) { return w[r][l]; },
+                                             [&](int r, int o, T x) { if (ok[r]) sB[q[r] * MP + o] = x; });
+        }
+        __syncthreads();
+        // ---- phase 4: S_y on j-lines ----
+        contract_lines<T, M, LPT, false>(sS + M * MP, ld_mid, st_mid);
+        __syncthreads();
+        // ---- phase 5: S_z on k-lines, u to global (coalesced) ----
+        contract_lines<T, M, LPT, false>(sS + 2 * M * MP, ld_outer, [&](int r, int o, T x) {
+            if (live && ok[r]) u[e * M3 + o * M2 + q[r]] = x;
+        });
+    }
+}
+
+}  // namespace sem_fdm_dev
