@@ -23,18 +23,12 @@ namespace {
 
 using namespace sem_fdm_dev;
 
-// Configuration per (precision, m), from the variant sweep on B200 recorded in profiles/r1e_fdm.md: two lines per thread
-// wherever the registers hold them without spilling, small CTAs (one element at m >= 7; several at small m so that a CTA
-// is at least a warp), one shared-memory stage (resident CTAs hide the copies).
-template <typename T, int M>
-int launch_m(sem_ctx* c, const void* S, const void* invL, const void* b, void* u) {
-    constexpr int LPT = (M >= 6 && !(sizeof(T) == 8 && M >= 12)) ? 2 : 1;
-    constexpr int TPE = (M * M + LPT - 1) / LPT;
-    constexpr int EPC = (48 / TPE) > 0 ? 48 / TPE : 1;
+template <typename T, int M, int LPT, int EPC, int NST, bool SREG>
+int launch_cfg(sem_ctx* c, const void* S, const void* invL, const void* b, void* u) {
     using C = fdm_cfg<T, M, LPT, EPC>;
-    constexpr size_t SMEM = C::SMEM1;
+    constexpr size_t SMEM = C::SMEM1 * NST;
     static int resident = 0;                             // CTAs per SM of this instantiation
-    auto kern = k_fdm<T, M, LPT, EPC, 1, 1>;
+    auto kern = SREG ? k_fdm_sreg<T, M, LPT, EPC, 1, NST> : k_fdm<T, M, LPT, EPC, 1, NST>;
     if (!resident) {
         if (SMEM > 48 * 1024)
             SEM_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
@@ -43,11 +37,31 @@ int launch_m(sem_ctx* c, const void* S, const void* invL, const void* b, void* u
         resident = nb > 0 ? nb : 1;
     }
     const int64_t ngrp = (c->E + C::EPC - 1) / C::EPC;
-    int64_t grid = (int64_t)c->num_sms * resident;       // single wave of persistent CTAs
-    if (grid > ngrp) grid = ngrp;
+    int64_t grid = (int64_t)c->num_sms * resident;       // single wave of persistent CTAs (a grid cut down to equal
+    if (grid > ngrp) grid = ngrp;                        // shares per CTA measured 8-10 % slower)
     kern<<<(unsigned)grid, C::NT, SMEM, c->stream>>>(c->E, (const T*)S, (const T*)invL, (const T*)b, (T*)u);
     SEM_CUDA_OK(c, cudaGetLastError());
     return SEM_OK;
+}
+
+// Configuration per (precision, m), from the variant sweeps on B200 summarised in profiles/r1e_fdm.md.
+//   k_fdm:      two lines per thread wherever the registers hold them without spilling; one element per CTA at m >= 8,
+//               about 128 threads' worth of elements below; one shared-memory stage (the resident CTAs hide the
+//               copies) up to m = 11, two from m = 12 on (few CTAs fit).
+//   k_fdm_sreg: S_d resident in registers, where it measured faster: FP32 m = 8, 10, 12 and FP64 m = 8, 10.
+template <typename T, int M>
+int launch_m(sem_ctx* c, const void* S, const void* invL, const void* b, void* u) {
+    constexpr bool F32 = sizeof(T) == 4;
+    if constexpr (M == 8) return launch_cfg<T, M, 4, 2, 1, true>(c, S, invL, b, u);
+    else if constexpr (M == 10) return launch_cfg<T, M, 4, 1, 1, true>(c, S, invL, b, u);
+    else if constexpr (M == 12 && F32) return launch_cfg<T, M, 5, 1, 1, true>(c, S, invL, b, u);
+    else {
+        constexpr int LPT = (M >= 6 && !(!F32 && M >= 12)) ? 2 : 1;
+        constexpr int TPE = (M * M + LPT - 1) / LPT;
+        constexpr int EPC = (M >= 8 || 128 / TPE < 1) ? 1 : 128 / TPE;
+        constexpr int NST = M >= 12 ? 2 : 1;
+        return launch_cfg<T, M, LPT, EPC, NST, false>(c, S, invL, b, u);
+    }
 }
 
 template <typename T>

@@ -3,6 +3,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <type_traits>
+
 namespace sem_fdm_dev {
 
 
@@ -202,6 +204,126 @@ k_fdm(int64_t E, const T* __restrict__ S, const T* __restrict__ invL, const T* b
         contract_lines<T, M, LPT, false>(sS + 2 * M * MP, ld_outer, [&](int r, int o, T x) {
             if (live && ok[r]) u[e * M3 + o * M2 + q[r]] = x;
         });
+    }
+}
+
+// ---- variant with S_d resident in registers ------------------------------------------------------------------------
+// k_fdm above reads every row of S_d from shared memory once per LPT lines, and a warp-uniform 128-bit load still costs
+// two shared-memory wavefronts: those broadcasts are 55 % of its wavefronts, and the shared-memory pipe is its limiter.
+// Here a thread loads the whole m x m matrix of the phase into registers ONCE and then walks its LPS lines one after the
+// other (a line needs m inputs and one running dot product, so the lines do not multiply the register count):
+// m^2 / 4 broadcast loads per thread and phase instead of (m^2 / 4) x LPS / LPT.  Phase 3 uses the same S_x registers for
+// S_x^T and S_x.  FP32 up to m = 12 and FP64 up to m = 8 fit the register file.
+template <typename T, int M>
+__device__ __forceinline__ void load_matrix(const T* __restrict__ sS, T (&Sr)[M][fdm_cfg<T, M, 1, 1>::MP]) {
+#pragma unroll
+    for (int l = 0; l < M; ++l) load_row<T, M>(sS + l * fdm_cfg<T, M, 1, 1>::MP, Sr[l]);
+}
+
+// out[o] = sum_l (TRANSPOSED ? S[l][o] : S[o][l]) in[l], each result handed to st as soon as it is complete
+template <typename T, int M, bool TRANSPOSED, class St>
+__device__ __forceinline__ void apply_matrix(const T (&Sr)[M][fdm_cfg<T, M, 1, 1>::MP], const T (&in)[M], St st) {
+#pragma unroll
+    for (int o = 0; o < M; ++o) {
+        T v = T(0);
+#pragma unroll
+        for (int l = 0; l < M; ++l) v += (TRANSPOSED ? Sr[l][o] : Sr[o][l]) * in[l];
+        st(o, v);
+    }
+}
+
+template <typename T, int M, int LPS, int EPC_, int MINB, int NSTAGE>
+__global__ void __launch_bounds__((fdm_cfg<T, M, LPS, EPC_>::NT), MINB)
+k_fdm_sreg(int64_t E, const T* __restrict__ S, const T* __restrict__ invL, const T* b, T* u) {
+    using C = fdm_cfg<T, M, LPS, EPC_>;
+    constexpr int MP = C::MP, TPE = C::TPE, EPC = C::EPC, M2 = M * M, M3 = M * M * M, NT = C::NT;
+    constexpr int STG = C::STAGE;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* smem = reinterpret_cast<T*>(smem_raw);
+    const int el = threadIdx.x / TPE, tl = threadIdx.x - el * TPE;
+    const int64_t ngrp = (E + EPC - 1) / EPC;
+
+    auto issue = [&](int64_t grp, int stage) {
+        const int64_t e0 = grp * EPC;
+        const int ne = (int)((E - e0) < EPC ? (E - e0) : EPC);
+        T* st = smem + stage * STG;
+        copy_rows_async<T, M, NT>(st, S + e0 * 3 * M2, ne * 3 * M);
+        copy_rows_async<T, M, NT>(st + EPC * C::S_EL, invL + e0 * M3, ne * M2);
+        copy_rows_async<T, M, NT>(st + EPC * (C::S_EL + C::B_EL), b + e0 * M3, ne * M2);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+
+    if (NSTAGE == 2 && (int64_t)blockIdx.x < ngrp) issue(blockIdx.x, 0);
+    int stage = 0;
+    for (int64_t grp = blockIdx.x; grp < ngrp; grp += gridDim.x, stage ^= (NSTAGE - 1)) {
+        const int64_t e = grp * EPC + el;
+        const bool live = e < E;
+        T* stg = smem + stage * STG;
+        const T* sS = stg + el * C::S_EL;                              // [3][M][MP]: x, y, z
+        const T* sL = stg + EPC * C::S_EL + el * C::B_EL;              // [c][b][MP]
+        T* sB = stg + EPC * (C::S_EL + C::B_EL) + el * C::B_EL;        // [k][j][MP]
+        if (NSTAGE == 1) {
+            __syncthreads();
+            issue(grp, 0);
+        }
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncthreads();
+        if (NSTAGE == 2 && grp + gridDim.x < ngrp) issue(grp + gridDim.x, stage ^ 1);
+        T Sr[M][MP];
+        // One phase over the thread's lines q = tl, tl + TPE, ...: line element l sits at base(q) + l * STRIDE.
+        // OUTER: q = (j,i), k-line;  MID: q = (k,i), j-line.  In place: a line is read whole before it is written.
+        auto phase = [&](auto transposed, auto outer) {
+            constexpr bool TR = decltype(transposed)::value, OUTER = decltype(outer)::value;
+            constexpr int STRIDE = OUTER ? M * MP : MP;
+#pragma unroll 1
+            for (int q = tl; q < M2; q += TPE) {
+                const int a = q / M, c = q - a * M;
+                T* line = sB + (OUTER ? a * MP + c : a * M * MP + c);
+                T in[M];
+#pragma unroll
+                for (int l = 0; l < M; ++l) in[l] = line[l * STRIDE];
+                apply_matrix<T, M, TR>(Sr, in, [&](int o, T v) { line[o * STRIDE] = v; });
+            }
+        };
+        // ---- phase 1: S_z^T on k-lines ----
+        load_matrix<T, M>(sS + 2 * M * MP, Sr);
+        phase(std::true_type{}, std::true_type{});
+        __syncthreads();
+        // ---- phase 2: S_y^T on j-lines ----
+        load_matrix<T, M>(sS + M * MP, Sr);
+        phase(std::true_type{}, std::false_type{});
+        __syncthreads();
+        // ---- phase 3: S_x^T, Lambda^-1, S_x on i-lines (rows: 128-bit accesses) ----
+        load_matrix<T, M>(sS, Sr);
+#pragma unroll 1
+        for (int q = tl; q < M2; q += TPE) {
+            T row[MP], il[MP], t[M];
+            load_row<T, M>(sB + q * MP, row);
+            load_row<T, M>(sL + q * MP, il);
+            T in[M];
+#pragma unroll
+            for (int l = 0; l < M; ++l) in[l] = row[l];
+            apply_matrix<T, M, true>(Sr, in, [&](int o, T v) { t[o] = v * il[o]; });
+            apply_matrix<T, M, false>(Sr, t, [&](int o, T v) { sB[q * MP + o] = v; });
+        }
+        __syncthreads();
+        // ---- phase 4: S_y on j-lines ----
+        load_matrix<T, M>(sS + M * MP, Sr);
+        phase(std::false_type{}, std::false_type{});
+        __syncthreads();
+        // ---- phase 5: S_z on k-lines, u to global (coalesced) ----
+        load_matrix<T, M>(sS + 2 * M * MP, Sr);
+#pragma unroll 1
+        for (int q = tl; q < M2; q += TPE) {
+            const int a = q / M, c = q - a * M;
+            const T* line = sB + a * MP + c;
+            T in[M];
+#pragma unroll
+            for (int l = 0; l < M; ++l) in[l] = line[l * M * MP];
+            apply_matrix<T, M, false>(Sr, in, [&](int o, T v) {
+                if (live) u[e * M3 + o * M2 + q] = v;
+            });
+        }
     }
 }
 

@@ -172,12 +172,12 @@ def run_fdm(peak: float):
     the paper's 8-5-1 / 8-6-4-1 schedules.  Bytes = b, Lambda^-1, u (m^3 each) + S (3 m^2) per element; flops = 12 m^4."""
     import numpy as np
     import scipy.linalg
-    E = 7200
-    mesh = inputs.box_mesh(E, 1, 1, 1)
-    print("| m | precision | us | GB/s | frac of HBM peak | TFLOP/s |")
-    print("|---|---|---|---|---|---|")
-    with binding.Sem(mesh.E, 1, mesh.vert, mesh.gid) as sem:
-        for m in (10, 8, 7, 6, 5, 4, 12):
+    print("| E | m | precision | us | GB/s | frac of HBM peak | TFLOP/s |")
+    print("|---|---|---|---|---|---|---|")
+    # E = 7200: config 2's element count; (3573, 11): the paper's Table 2 case (E/P = 3573, N = 8, FP32: 171 us on V100)
+    for E, m in ((7200, 10), (7200, 8), (7200, 7), (7200, 6), (7200, 5), (7200, 4), (7200, 12), (3573, 11), (3573, 9), (3573, 7)):
+        mesh = inputs.box_mesh(E, 1, 1, 1)
+        with binding.Sem(mesh.E, 1, mesh.vert, mesh.gid) as sem:
             A, B = inputs.fdm_pairs(E, m, 7)
             S = np.empty_like(A)
             lam = np.empty((E, 3, m))
@@ -191,7 +191,7 @@ def run_fdm(peak: float):
                 u = torch.empty_like(b)
                 t = _time(lambda: sem.fdm_apply(m, dS, dL, b, u), 500)
                 nbytes = b.element_size() * E * (3 * m ** 3 + 3 * m * m)
-                print(f"| {m} | {name} | {t:.2f} | {nbytes / t / 1e3:.0f} | {nbytes / t / 1e3 / peak:.2f} | "
+                print(f"| {E} | {m} | {name} | {t:.2f} | {nbytes / t / 1e3:.0f} | {nbytes / t / 1e3 / peak:.2f} | "
                       f"{12.0 * m ** 4 * E / t / 1e6:.2f} |", flush=True)
 
 
