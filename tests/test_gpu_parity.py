@@ -912,7 +912,10 @@ def _fdm_inputs(oracle_mod, E, m, seed):
 
 
 @pytest.mark.parametrize("m,E", [(10, 1500), (10, 3), (4, 5000), (6, 777), (8, 1201), (12, 301), (7, 450), (9, 333),
-                                 (2, 100), (3, 65), (5, 129), (16, 150), (13, 97)])
+                                 (2, 100), (3, 65), (5, 129), (16, 150), (13, 97),
+                                 # several groups per persistent CTA (the stage is re-filled while in use), at the
+                                 # element counts the sweep times: config 2's E = 7200 and the paper's E/P = 3573
+                                 (10, 7200), (11, 3573), (8, 9001), (6, 30001), (12, 2500), (16, 701), (4, 60000)])
 def test_fdm_apply_parity(torch_cuda, binding, oracle_mod, m, E):
     """sem_fdm_apply against the oracle's Eq. (3) on the same S, Lambda^-1, b: FP64 1e-12, FP32 1e-5 (normalised by
     max |u| per case), more elements than one wave of CTAs holds at m = 10 and a ragged last group; in place too."""
