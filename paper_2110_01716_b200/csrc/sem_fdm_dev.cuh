@@ -23,7 +23,11 @@ struct fdm_cfg {
     static constexpr int EPC = EPC_;
     static constexpr int NT = EPC * TPE;
     static constexpr int S_EL = 3 * M * MP;                       // padded S values per element
-    static constexpr int B_EL = M * M * MP;                       // padded block values per element
+    // plane stride of the block: the lanes of a warp that own j-lines span several k-planes; their bank ranges
+    // [0, M) + k * PS must not overlap, so PS = MP modulo one bank cycle (32 floats / 16 doubles), rows stay 16-byte aligned
+    static constexpr int BANKW = 128 / (int)sizeof(T);
+    static constexpr int PS = M * MP + ((MP - M * MP) % BANKW + BANKW) % BANKW;
+    static constexpr int B_EL = M * PS;                           // padded block values per element
     static constexpr int STAGE = EPC * (S_EL + 2 * B_EL);         // S, Lambda^-1 and the block of EPC elements
     static constexpr size_t SMEM1 = sizeof(T) * (size_t)STAGE;    // per stage
 };
@@ -104,7 +108,8 @@ __device__ __forceinline__ void cp_async(void* smem_dst, const void* gsrc) {
 }
 
 // rows of M values, contiguous in global memory, to rows padded to MP in shared memory, by all NT threads of the CTA
-template <typename T, int M, int NT>
+// (PS = stride of a plane of M rows in shared memory)
+template <typename T, int M, int NT, int PS>
 __device__ __forceinline__ void copy_rows_async(T* __restrict__ sdst, const T* __restrict__ gsrc, int nrows) {
     constexpr int MP = fdm_cfg<T, M, 1, 1>::MP;
     constexpr int RB = M * (int)sizeof(T);
@@ -112,7 +117,8 @@ __device__ __forceinline__ void copy_rows_async(T* __restrict__ sdst, const T* _
     constexpr int CPR = RB / CH, VPC = CH / (int)sizeof(T);
     for (int t = threadIdx.x; t < nrows * CPR; t += NT) {
         const int row = t / CPR, c = t - row * CPR;
-        cp_async<CH>(sdst + row * MP + c * VPC, gsrc + (int64_t)row * M + c * VPC);
+        const int plane = row / M;
+        cp_async<CH>(sdst + plane * PS + (row - plane * M) * MP + c * VPC, gsrc + (int64_t)row * M + c * VPC);
     }
 }
 
@@ -124,7 +130,7 @@ __global__ void __launch_bounds__((fdm_cfg<T, M, LPT_, EPC_>::NT), MINB)
 k_fdm(int64_t E, const T* __restrict__ S, const T* __restrict__ invL, const T* b, T* u) {
     using C = fdm_cfg<T, M, LPT_, EPC_>;
     constexpr int MP = C::MP, LPT = C::LPT, TPE = C::TPE, EPC = C::EPC, M2 = M * M, M3 = M * M * M, NT = C::NT;
-    constexpr int STG = C::STAGE;
+    constexpr int STG = C::STAGE, PS = C::PS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T* smem = reinterpret_cast<T*>(smem_raw);
     const int el = threadIdx.x / TPE, tl = threadIdx.x - el * TPE;
@@ -134,9 +140,9 @@ k_fdm(int64_t E, const T* __restrict__ S, const T* __restrict__ invL, const T* b
         const int64_t e0 = grp * EPC;
         const int ne = (int)((E - e0) < EPC ? (E - e0) : EPC);
         T* st = smem + stage * STG;
-        copy_rows_async<T, M, NT>(st, S + e0 * 3 * M2, ne * 3 * M);
-        copy_rows_async<T, M, NT>(st + EPC * C::S_EL, invL + e0 * M3, ne * M2);
-        copy_rows_async<T, M, NT>(st + EPC * (C::S_EL + C::B_EL), b + e0 * M3, ne * M2);
+        copy_rows_async<T, M, NT, M * MP>(st, S + e0 * 3 * M2, ne * 3 * M);
+        copy_rows_async<T, M, NT, PS>(st + EPC * C::S_EL, invL + e0 * M3, ne * M2);
+        copy_rows_async<T, M, NT, PS>(st + EPC * (C::S_EL + C::B_EL), b + e0 * M3, ne * M2);
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
 
@@ -169,10 +175,10 @@ k_fdm(int64_t E, const T* __restrict__ S, const T* __restrict__ invL, const T* b
         // line ownership: "outer" = (j,i) owns a k-line (element l at (l*M + a)*MP + c); "mid" = (k,i) owns a j-line
         // (element l at (a*M + l)*MP + c); "inner" = (k,j) owns an i-line (row q).  A line is read and written by its
         // owner only, so the barriers sit between the phases and nowhere else.
-        auto ld_outer = [&](int r, int l) { return sB[(l * M + a[r]) * MP + c[r]]; };
-        auto st_outer = [&](int r, int o, T v) { if (ok[r]) sB[(o * M + a[r]) * MP + c[r]] = v; };
-        auto ld_mid = [&](int r, int l) { return sB[(a[r] * M + l) * MP + c[r]]; };
-        auto st_mid = [&](int r, int o, T v) { if (ok[r]) sB[(a[r] * M + o) * MP + c[r]] = v; };
+        auto ld_outer = [&](int r, int l) { return sB[l * PS + a[r] * MP + c[r]]; };
+        auto st_outer = [&](int r, int o, T v) { if (ok[r]) sB[o * PS + a[r] * MP + c[r]] = v; };
+        auto ld_mid = [&](int r, int l) { return sB[a[r] * PS + l * MP + c[r]]; };
+        auto st_mid = [&](int r, int o, T v) { if (ok[r]) sB[a[r] * PS + o * MP + c[r]] = v; };
         // ---- phase 1: S_z^T on k-lines ----
         contract_lines<T, M, LPT, true>(sS + 2 * M * MP, ld_outer, st_outer);
         __syncthreads();
@@ -183,18 +189,18 @@ k_fdm(int64_t E, const T* __restrict__ S, const T* __restrict__ invL, const T* b
         {
             T v[LPT][MP];
 #pragma unroll
-            for (int r = 0; r < LPT; ++r) load_row<T, M>(sB + q[r] * MP, v[r]);
+            for (int r = 0; r < LPT; ++r) load_row<T, M>(sB + a[r] * PS + c[r] * MP, v[r]);
             T w[LPT][M];
             contract_lines<T, M, LPT, true>(sS, [&](int r, int l) { return v[r][l]; },
                                             [&](int r, int o, T x) { w[r][o] = x; });
 #pragma unroll
             for (int r = 0; r < LPT; ++r) {
-                load_row<T, M>(sL + q[r] * MP, v[r]);
+                load_row<T, M>(sL + a[r] * PS + c[r] * MP, v[r]);
 #pragma unroll
                 for (int i = 0; i < M; ++i) w[r][i] *= v[r][i];
             }
             contract_lines<T, M, LPT, false>(sS, [&](int r, int l) { return w[r][l]; },
-                                             [&](int r, int o, T x) { if (ok[r]) sB[q[r] * MP + o] = x; });
+                                             [&](int r, int o, T x) { if (ok[r]) sB[a[r] * PS + c[r] * MP + o] = x; });
         }
         __syncthreads();
         // ---- phase 4: S_y on j-lines ----
@@ -237,7 +243,7 @@ __global__ void __launch_bounds__((fdm_cfg<T, M, LPS, EPC_>::NT), MINB)
 k_fdm_sreg(int64_t E, const T* __restrict__ S, const T* __restrict__ invL, const T* b, T* u) {
     using C = fdm_cfg<T, M, LPS, EPC_>;
     constexpr int MP = C::MP, TPE = C::TPE, EPC = C::EPC, M2 = M * M, M3 = M * M * M, NT = C::NT;
-    constexpr int STG = C::STAGE;
+    constexpr int STG = C::STAGE, PS = C::PS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T* smem = reinterpret_cast<T*>(smem_raw);
     const int el = threadIdx.x / TPE, tl = threadIdx.x - el * TPE;
@@ -247,9 +253,9 @@ k_fdm_sreg(int64_t E, const T* __restrict__ S, const T* __restrict__ invL, const
         const int64_t e0 = grp * EPC;
         const int ne = (int)((E - e0) < EPC ? (E - e0) : EPC);
         T* st = smem + stage * STG;
-        copy_rows_async<T, M, NT>(st, S + e0 * 3 * M2, ne * 3 * M);
-        copy_rows_async<T, M, NT>(st + EPC * C::S_EL, invL + e0 * M3, ne * M2);
-        copy_rows_async<T, M, NT>(st + EPC * (C::S_EL + C::B_EL), b + e0 * M3, ne * M2);
+        copy_rows_async<T, M, NT, M * MP>(st, S + e0 * 3 * M2, ne * 3 * M);
+        copy_rows_async<T, M, NT, PS>(st + EPC * C::S_EL, invL + e0 * M3, ne * M2);
+        copy_rows_async<T, M, NT, PS>(st + EPC * (C::S_EL + C::B_EL), b + e0 * M3, ne * M2);
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
 
@@ -274,11 +280,11 @@ k_fdm_sreg(int64_t E, const T* __restrict__ S, const T* __restrict__ invL, const
         // OUTER: q = (j,i), k-line;  MID: q = (k,i), j-line.  In place: a line is read whole before it is written.
         auto phase = [&](auto transposed, auto outer) {
             constexpr bool TR = decltype(transposed)::value, OUTER = decltype(outer)::value;
-            constexpr int STRIDE = OUTER ? M * MP : MP;
+            constexpr int STRIDE = OUTER ? PS : MP;
 #pragma unroll 1
             for (int q = tl; q < M2; q += TPE) {
                 const int a = q / M, c = q - a * M;
-                T* line = sB + (OUTER ? a * MP + c : a * M * MP + c);
+                T* line = sB + (OUTER ? a * MP + c : a * PS + c);
                 T in[M];
 #pragma unroll
                 for (int l = 0; l < M; ++l) in[l] = line[l * STRIDE];
@@ -298,13 +304,14 @@ k_fdm_sreg(int64_t E, const T* __restrict__ S, const T* __restrict__ invL, const
 #pragma unroll 1
         for (int q = tl; q < M2; q += TPE) {
             T row[MP], il[MP], t[M];
-            load_row<T, M>(sB + q * MP, row);
-            load_row<T, M>(sL + q * MP, il);
+            const int a = q / M, ro = a * PS + (q - a * M) * MP;
+            load_row<T, M>(sB + ro, row);
+            load_row<T, M>(sL + ro, il);
             T in[M];
 #pragma unroll
             for (int l = 0; l < M; ++l) in[l] = row[l];
             apply_matrix<T, M, true>(Sr, in, [&](int o, T v) { t[o] = v * il[o]; });
-            apply_matrix<T, M, false>(Sr, t, [&](int o, T v) { sB[q * MP + o] = v; });
+            apply_matrix<T, M, false>(Sr, t, [&](int o, T v) { sB[ro + o] = v; });
         }
         __syncthreads();
         // ---- phase 4: S_y on j-lines ----
@@ -319,7 +326,7 @@ k_fdm_sreg(int64_t E, const T* __restrict__ S, const T* __restrict__ invL, const
             const T* line = sB + a * MP + c;
             T in[M];
 #pragma unroll
-            for (int l = 0; l < M; ++l) in[l] = line[l * M * MP];
+            for (int l = 0; l < M; ++l) in[l] = line[l * PS];
             apply_matrix<T, M, false>(Sr, in, [&](int o, T v) {
                 if (live) u[e * M3 + o * M2 + q] = v;
             });
