@@ -202,6 +202,18 @@ SEM_API void sem_proj_destroy(sem_proj* pj);
 SEM_API int sem_fdm_apply(sem_ctx* ctx, int m, const void* S, const void* inv_lambda, const void* b, void* u,
                           sem_prec prec);
 
+/* NEXT-2a setup (host, synchronous, no context, no device): the eigen-decompositions behind sem_fdm_apply.  For every
+ * element and direction d the generalised symmetric eigenproblem A_d s = lambda B_d s is solved with S_d^T B_d S_d = I
+ * (Cholesky of B_d + cyclic Jacobi; "fast diagonalization (FDM) Deville et al. (2002)"), and
+ * inv_lambda[c][b][a] = 1 / (lambda_x[a] + lambda_y[b] + lambda_z[c]).
+ *   A, B        HOST [E][3][m][m] doubles (d = x, y, z), symmetric (the symmetric part is used), B positive definite
+ *   S           HOST out [E][3][m][m]: eigenvectors in columns, eigenvalues ascending; a column's sign is arbitrary
+ *               (Eq. (3) does not depend on it)
+ *   inv_lambda  HOST out [E][m][m][m]
+ * Round S and inv_lambda to the precision sem_fdm_apply is called with.  SEM_EINVAL for NULL pointers, E <= 0,
+ * m outside 2..16 or a B_d that is not positive definite. */
+SEM_API int sem_fdm_setup(int64_t E, int m, const double* A, const double* B, double* S, double* inv_lambda);
+
 /* Tuning knob for experiments: selects the Ax kernel variant (0 = default streaming kernel, 1 = simple kernel). */
 SEM_API int sem_set_variant(sem_ctx* ctx, int ax_variant);
 

@@ -53,11 +53,26 @@ SYMBOLS = {
     "sem_fpcg": (_i32, [_vp, _vp, _vp, _dbl, _i32, C.POINTER(_i32), C.POINTER(_dbl)]),
     "sem_pmg_get_history": (_i32, [_vp, _vp, _i32]),
     "sem_fdm_apply": (_i32, [_vp, _i32, _vp, _vp, _vp, _vp, _i32]),
+    "sem_fdm_setup": (_i32, [_i64, _i32, _vp, _vp, _vp, _vp]),
     "sem_last_error": (C.c_char_p, [_vp]),
     "sem_ctx_destroy": (None, [_vp]),
 }
 
 _lib = None
+
+
+def fdm_setup(A: np.ndarray, B: np.ndarray):
+    """sem_fdm_setup (host): A, B [E][3][m][m] float64 -> (S[E][3][m][m], inv_lambda[E][m][m][m]) for sem_fdm_apply."""
+    A = np.ascontiguousarray(A, dtype=np.float64)
+    B = np.ascontiguousarray(B, dtype=np.float64)
+    assert A.ndim == 4 and A.shape == B.shape and A.shape[1] == 3 and A.shape[2] == A.shape[3]
+    E, m = A.shape[0], A.shape[2]
+    S = np.empty_like(A)
+    inv_lambda = np.empty((E, m, m, m))
+    rc = lib().sem_fdm_setup(E, m, _np_ptr(A), _np_ptr(B), _np_ptr(S), _np_ptr(inv_lambda))
+    if rc != SEM_OK:
+        raise SemError(rc, "sem_fdm_setup: bad arguments or a mass matrix that is not positive definite")
+    return S, inv_lambda
 
 
 class SemError(RuntimeError):

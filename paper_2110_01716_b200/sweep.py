@@ -170,8 +170,6 @@ def run_projection(peak: float):
 def run_fdm(peak: float):
     """NEXT-2a: sem_fdm_apply (Eq. (3)) at the paper's per-GPU element count, m = N + 3 for N = 7, 5, 3, 1 and
     the paper's 8-5-1 / 8-6-4-1 schedules.  Bytes = b, Lambda^-1, u (m^3 each) + S (3 m^2) per element; flops = 12 m^4."""
-    import numpy as np
-    import scipy.linalg
     print("| E | m | precision | us | GB/s | frac of HBM peak | TFLOP/s |")
     print("|---|---|---|---|---|---|---|")
     # E = 7200: config 2's element count; (3573, 11): the paper's Table 2 case (E/P = 3573, N = 8, FP32: 171 us on V100)
@@ -179,12 +177,7 @@ def run_fdm(peak: float):
         mesh = inputs.box_mesh(E, 1, 1, 1)
         with binding.Sem(mesh.E, 1, mesh.vert, mesh.gid) as sem:
             A, B = inputs.fdm_pairs(E, m, 7)
-            S = np.empty_like(A)
-            lam = np.empty((E, 3, m))
-            for e in range(E):
-                for d in range(3):
-                    lam[e, d], S[e, d] = scipy.linalg.eigh(A[e, d], B[e, d])
-            invL = 1.0 / (lam[:, 2, :, None, None] + lam[:, 1, None, :, None] + lam[:, 0, None, None, :])
+            S, invL = binding.fdm_setup(A, B)
             for dt, name in ((torch.float32, "FP32"), (torch.float64, "FP64")):
                 dS, dL = (torch.from_numpy(a.ravel()).cuda().to(dt) for a in (S, invL))
                 b = torch.randn(E * m ** 3, device="cuda", dtype=dt)

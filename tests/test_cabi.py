@@ -61,3 +61,42 @@ def test_no_cpu_fallback(built_lib):
         L.sem_ctx_destroy(h)
         with pytest.raises(binding.SemError):
             binding.Sem(1, 2, vert, gid)
+
+
+# ------------------------------------------------------------------ NEXT-2a setup: sem_fdm_setup is host logic (no GPU)
+def test_fdm_setup_host_matches_the_oracle_eigen_decomposition(built_lib):
+    """sem_fdm_setup (Cholesky + cyclic Jacobi in the library) against the oracle's scipy.linalg.eigh on the seeded
+    operator pairs: eigenvalues, B-orthonormality, diagonalisation, Lambda^-1, and -- since eigenvectors are unique only
+    up to sign and up to rotations inside (nearly) degenerate eigenspaces -- the result of Eq. (3) computed by the oracle
+    from the library's (S, Lambda^-1) against the oracle's own."""
+    import numpy as np
+    import oracle
+    from paper_2110_01716_b200 import binding, inputs
+    for m, E in ((10, 12), (4, 7), (7, 5), (16, 3), (2, 4)):
+        A, B = inputs.fdm_pairs(E, m, seed=50 + m)
+        S, invL = binding.fdm_setup(A, B)
+        So, invLo = np.empty_like(A), np.empty((E, m, m, m))
+        for e in range(E):
+            lam = []
+            for d in range(3):
+                So[e, d], l = oracle.fdm_eig(A[e, d], B[e, d])
+                lam.append(l)
+                D = S[e, d].T @ A[e, d] @ S[e, d]
+                assert np.max(np.abs(np.diag(D) - l)) <= 1e-12 * l[-1]
+                assert np.max(np.abs(D - np.diag(np.diag(D)))) <= 1e-11 * l[-1]
+                assert np.max(np.abs(S[e, d].T @ B[e, d] @ S[e, d] - np.eye(m))) <= 1e-12
+            invLo[e] = oracle.fdm_inv_lambda(*lam)
+        assert np.max(np.abs(invL / invLo - 1.0)) <= 1e-12
+        b = 2.0 * inputs.hash_uniform01(9, 12, np.arange(E * m ** 3)).reshape(E, m, m, m) - 1.0
+        u_lib, u_orc = oracle.fdm_apply(S, invL, b), oracle.fdm_apply(So, invLo, b)
+        assert np.max(np.abs(u_lib - u_orc)) <= 1e-11 * np.max(np.abs(u_orc))
+
+
+def test_fdm_setup_bad_args(built_lib):
+    import numpy as np
+    from paper_2110_01716_b200 import binding
+    A = np.tile(np.eye(3), (1, 3, 1, 1))
+    with pytest.raises(binding.SemError):
+        binding.fdm_setup(A, -A)                                # mass matrix not positive definite
+    with pytest.raises(binding.SemError):
+        binding.fdm_setup(np.tile(np.eye(17), (1, 3, 1, 1)), np.tile(np.eye(17), (1, 3, 1, 1)))    # m > 16

@@ -941,3 +941,21 @@ def test_fdm_apply_bad_args(torch_cuda, binding):
             assert rc == binding.SEM_EINVAL
         assert sem._L.sem_fdm_apply(sem._h, 4, None, z.data_ptr(), z.data_ptr(), z.data_ptr(), binding.SEM_F64) == binding.SEM_EINVAL
         assert sem._L.sem_fdm_apply(sem._h, 4, z.data_ptr(), z.data_ptr(), z.data_ptr(), z.data_ptr(), 5) == binding.SEM_EINVAL
+
+
+@pytest.mark.parametrize("m,E", [(10, 2000), (6, 500)])
+def test_fdm_setup_and_apply_pipeline(torch_cuda, binding, oracle_mod, m, E):
+    """The library's own setup (sem_fdm_setup, host) feeding sem_fdm_apply, against the oracle's eigen-decomposition
+    feeding the oracle's Eq. (3): the result does not depend on eigenvector signs or on the basis chosen inside a
+    (nearly) degenerate eigenspace, so it is what is compared."""
+    A, B = inputs.fdm_pairs(E, m, seed=70 + m)
+    So, invLo, b = _fdm_inputs(oracle_mod, E, m, seed=70 + m)
+    ou = oracle_mod.fdm_apply(So, invLo, b)
+    S, invL = binding.fdm_setup(A, B)
+    mesh = inputs.box_mesh(E, 1, 1, 1)
+    with binding.Sem(mesh.E, 1, mesh.vert, mesh.gid) as sem:
+        for dt, tol in ((torch_cuda.float64, 1e-11), (torch_cuda.float32, TOL32)):
+            dS, dL, db = (to_dev(torch_cuda, a.ravel(), dt) for a in (S, invL, b))
+            du = torch_cuda.empty_like(db)
+            sem.fdm_apply(m, dS, dL, db, du)
+            assert relerr(du.cpu().numpy(), ou.ravel()) <= tol, (m, E, dt)
