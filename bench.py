@@ -352,6 +352,25 @@ def main():
             for s_ in lv:
                 s_.close()
 
+    # ---- NEXT-2a: the Schwarz smoothers' fast-diagonalisation local solve (Eq. (3)) on config 2's 7200 elements,
+    # extended blocks of m = N + 3 = 10 points per direction, FP32 (the paper's preconditioner precision) and FP64
+    fdm = None
+    if rank == 0 and world == 1 and args.pcg_iters > 0:
+        m_ = mesh.N + 3
+        S_h, iL_h = binding.fdm_setup(*inputs.fdm_pairs(mesh.E, m_, 7))
+        fdm = {"workload": f"E = {mesh.E} blocks of {m_}^3, seeded 1-D operator pairs", "m": m_,
+               "timed": "500 back-to-back launches of sem_fdm_apply, CUDA events"}
+        for dt_, name in ((torch.float32, "f32"), (torch.float64, "f64")):
+            dS, dL = (torch.from_numpy(a.ravel()).cuda().to(dt_) for a in (S_h, iL_h))
+            b_ = torch.randn(mesh.E * m_ ** 3, device="cuda", dtype=dt_)
+            u_ = torch.empty_like(b_)
+            for _ in range(3):
+                sem.fdm_apply(m_, dS, dL, b_, u_)
+            ms_f = timed(lambda: sem.fdm_apply(m_, dS, dL, b_, u_), 500)
+            nbytes = b_.element_size() * mesh.E * (3 * m_ ** 3 + 3 * m_ * m_)
+            fdm[name] = {"us": ms_f / 500 * 1e3, "TFLOPs": 12.0 * m_ ** 4 * mesh.E / (ms_f / 500 * 1e-3) / 1e12,
+                         "algorithmic_GBs": nbytes / (ms_f / 500 * 1e-3) / 1e9}
+
     dofs = mesh.dofs
     value = whole_job_value(dofs, world, K, ms_total)
     e2e_value = whole_job_value(dofs, world, Ke, ms_e2e)
@@ -387,6 +406,10 @@ def main():
     }
     if solve is not None:
         line["poisson_solve"] = solve
+    if fdm is not None:
+        for name in ("f32", "f64"):
+            fdm[name]["frac_of_measured_hbm_peak"] = fdm[name]["algorithmic_GBs"] / peak
+        line["fdm"] = fdm
     if pcg is not None:
         pcg["frac_of_measured_peak"] = pcg["algorithmic_GBs"] / peak
         line["pcg"] = pcg
