@@ -84,6 +84,14 @@ SEM_API int sem_ax(sem_ctx* ctx, const void* u, void* w, sem_prec prec, double l
  * unique node receives the sum over all its copies.  No mask is applied.  w DEVICE, local layout. */
 SEM_API int sem_gs(sem_ctx* ctx, void* w, sem_prec prec, sem_op op);
 
+/* NEXT-4, first piece: the gather-scatter of several fields in one pass (the paper's `gatherScatterMany`
+ * kernel, Table 3; the three velocity components of the Helmholtz solves).  Field f is the local-layout
+ * vector at w + f * field_stride (in values of `prec`, field_stride >= nL); every field receives exactly what sem_gs
+ * would give it (bit-identical), but the gather-scatter records are read once for up to 4 fields and the value loads of
+ * all of them are in flight together.  No mask is applied.  w DEVICE.  Asynchronous on the context's stream.
+ * SEM_EINVAL for nfields < 1 or field_stride < nL. */
+SEM_API int sem_gs_many(sem_ctx* ctx, void* w, int nfields, int64_t field_stride, sem_prec prec, sem_op op);
+
 /* a3-a7.  w = M QQ^T (D^T G D + lambda B) u, with M zeroing Dirichlet nodes (if the context has any).  u must be
  * continuous (equal on all copies of a shared node).  Called repeatedly with the same (u, w, prec, lambda) on a
  * non-default stream, the second call records the two kernels into a CUDA graph and later calls replay it (still

@@ -29,6 +29,7 @@ SYMBOLS = {
     "sem_ax": (_i32, [_vp, _vp, _vp, _i32, _dbl]),
     "sem_gs": (_i32, [_vp, _vp, _i32, _i32]),
     "sem_ax_gs": (_i32, [_vp, _vp, _vp, _i32, _dbl]),
+    "sem_gs_many": (_i32, [_vp, _vp, _i32, _i64, _i32, _i32]),
     "sem_pcg": (_i32, [_vp, _vp, _vp, _dbl, _i32, C.POINTER(_i32), C.POINTER(_dbl)]),
     "sem_set_lambda": (_i32, [_vp, _dbl]),
     "sem_get_pcg_history": (_i32, [_vp, _vp, _i32]),
@@ -181,6 +182,13 @@ class Sem:
 
     def gs(self, w):
         self._check(self._L.sem_gs(self._h, self._vec(w), self._prec(w), SEM_OP_ADD))
+        return w
+
+    def gs_many(self, w):
+        """sem_gs_many on a contiguous [nfields][stride >= nL] CUDA tensor, in place."""
+        assert w.is_cuda and w.is_contiguous() and w.dim() == 2 and w.shape[1] >= self.nL
+        self._check(self._L.sem_gs_many(self._h, C.c_void_p(w.data_ptr()), w.shape[0], w.shape[1], self._prec(w),
+                                        SEM_OP_ADD))
         return w
 
     def ax_gs(self, u, w, lam: float = 0.0):

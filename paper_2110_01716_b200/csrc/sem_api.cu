@@ -101,6 +101,24 @@ int sem_gs(sem_ctx* c, void* w, sem_prec prec, sem_op op) {
     return sem_launch_gs(c, w, prec, false);
 }
 
+int sem_gs_many(sem_ctx* c, void* w, int nfields, int64_t field_stride, sem_prec prec, sem_op op) {
+    int rc = check_vec(c, nullptr, w, prec, 0.0, "sem_gs_many");
+    if (rc) return rc;
+    if (op != SEM_OP_ADD) return sem_fail(c, SEM_EINVAL, "sem_gs_many: only SEM_OP_ADD is defined (P:119)");
+    if (nfields < 1 || field_stride < c->nL)
+        return sem_fail(c, SEM_EINVAL, "sem_gs_many: nfields < 1 or field_stride < nL");
+    if (!c->d_sh_off) return sem_fail(c, SEM_ESTATE, "sem_gs_many on a context whose setup failed");
+    const size_t vs = prec == SEM_F64 ? 8 : 4;
+    for (int f = 0; f < nfields;) {                          // launches of 4, 3 or 2 fields; a single one by sem_gs's kernel
+        const int left = nfields - f, take = left >= 4 && left != 5 ? 4 : left >= 3 ? 3 : left;
+        void* wf = (char*)w + (size_t)f * (size_t)field_stride * vs;
+        rc = take == 1 ? sem_launch_gs(c, wf, prec, false) : sem_launch_gs_many(c, wf, take, field_stride, prec, false);
+        if (rc) return rc;
+        f += take;
+    }
+    return SEM_OK;
+}
+
 int sem_ax_gs(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda) {
     int rc = check_vec(c, u, w, prec, lambda, "sem_ax_gs");
     if (rc) return rc;

@@ -40,6 +40,84 @@ __global__ void __launch_bounds__(NT, GS_CTAS) k_gs_records(int32_t n_pair, cons
     if (bg < n_big) gs_bigs<T, MASK, false, NT>(big, sh_idx, (int32_t)bg + threadIdx.x, min(n_big, (int32_t)bg + pg), w);
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Several fields in one launch (sem_gs_many; the paper's `gatherScatterMany`, Table 3: the three velocity
+// components of the Helmholtz solves): a record is read once and applied to NF fields w + f * stride, with the
+// value loads of all NF fields in flight together.  Same ascending-index sums per field, so each field is bit-identical
+// to sem_gs applied to it alone.
+// ---------------------------------------------------------------------------------------------------------------
+template <typename T, bool MASK, int NF>
+__global__ void __launch_bounds__(NT, 4) k_gs_records_many(int32_t n_pair, const int2* __restrict__ pair, int32_t n_quad,
+                                                           const int4* __restrict__ quad, int32_t n_big,
+                                                           const int2* __restrict__ big,
+                                                           const int32_t* __restrict__ sh_idx, T* __restrict__ w,
+                                                           int64_t stride) {
+    const int32_t b = blockIdx.x, nb = gridDim.x;
+    const int32_t pp = ((n_pair + nb - 1) / nb + 31) & ~31, pq = ((n_quad + nb - 1) / nb + 31) & ~31,
+                  pg = (n_big + nb - 1) / nb;
+    const int64_t bp = (int64_t)b * pp, bq = (int64_t)b * pq, bg = (int64_t)b * pg;
+    constexpr int PP = 2;                                     // pairs per thread and pass: PP x NF x 2 loads in flight
+    if (bp < n_pair) {
+        const int32_t end = min(n_pair, (int32_t)bp + pp);
+        for (int32_t base = (int32_t)bp + threadIdx.x; base < end; base += NT * PP) {
+            int2 r[PP];
+#pragma unroll
+            for (int q = 0; q < PP; ++q) {
+                const int32_t t = base + q * NT;
+                r[q] = t < end ? pair[t] : make_int2(0, -2);
+            }
+            T v0[PP][NF], v1[PP][NF];
+#pragma unroll
+            for (int q = 0; q < PP; ++q)
+#pragma unroll
+                for (int f = 0; f < NF; ++f) {
+                    v0[q][f] = r[q].y >= 0 ? w[f * stride + (r[q].x & IDX)] : T(0);
+                    v1[q][f] = r[q].y >= 0 ? w[f * stride + r[q].y] : T(0);
+                }
+#pragma unroll
+            for (int q = 0; q < PP; ++q)
+#pragma unroll
+                for (int f = 0; f < NF; ++f) {
+                    if (r[q].y >= 0) {
+                        T s = v0[q][f] + v1[q][f];
+                        if (MASK && r[q].x < 0) s = T(0);
+                        w[f * stride + (r[q].x & IDX)] = s;
+                        w[f * stride + r[q].y] = s;
+                    } else if (MASK && r[q].y == -1) {
+                        w[f * stride + (r[q].x & IDX)] = T(0);
+                    }
+                }
+        }
+    }
+    if (bq < n_quad) {
+        const int32_t end = min(n_quad, (int32_t)bq + pq);
+        for (int32_t t = (int32_t)bq + threadIdx.x; t < end; t += NT) {
+            const int4 r = quad[t];
+            const int32_t l0 = r.x & IDX;
+            T a[NF][4];
+#pragma unroll
+            for (int f = 0; f < NF; ++f) {
+                T* wf = w + f * stride;
+                a[f][0] = wf[l0]; a[f][1] = wf[r.y]; a[f][2] = wf[r.z];
+                a[f][3] = r.w >= 0 ? wf[r.w] : T(0);
+            }
+#pragma unroll
+            for (int f = 0; f < NF; ++f) {
+                T* wf = w + f * stride;
+                T s = (a[f][0] + a[f][1]) + a[f][2];
+                if (r.w >= 0) s += a[f][3];
+                if (MASK && r.x < 0) s = T(0);
+                wf[l0] = s; wf[r.y] = s; wf[r.z] = s;
+                if (r.w >= 0) wf[r.w] = s;
+            }
+        }
+    }
+    if (bg < n_big)                                           // rare (> 4 copies): field by field
+        for (int f = 0; f < NF; ++f)
+            gs_bigs<T, MASK, false, NT>(big, sh_idx, (int32_t)bg + threadIdx.x, min(n_big, (int32_t)bg + pg),
+                                        w + f * stride);
+}
+
 }  // namespace
 
 int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask) {
@@ -58,6 +136,33 @@ int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask) {
     if (prec == SEM_F64) { if (m) SEM_GS_LAUNCH(double, true); else SEM_GS_LAUNCH(double, false); }
     else { if (m) SEM_GS_LAUNCH(float, true); else SEM_GS_LAUNCH(float, false); }
 #undef SEM_GS_LAUNCH
+    SEM_CUDA_OK(c, cudaGetLastError());
+    return SEM_OK;
+}
+
+// nf = 2, 3 or 4 fields at w + f * stride (values of T) in one launch
+int sem_launch_gs_many(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec prec, bool apply_mask) {
+    const bool m = apply_mask && c->has_mask;
+    const int32_t np = (int32_t)c->n_pair, nq = (int32_t)c->n_quad, nb = (int32_t)c->n_big;
+    if (np + nq + nb == 0) return SEM_OK;
+    const double ops = (4.0 * np + 8.0 * nq + 16.0 * nb) * nf;
+    int64_t blocks = (int64_t)(ops / (4.0 * NT * PPT)) + 1;
+    const int64_t cap = (int64_t)c->num_sms * 4;
+    if (blocks > cap) blocks = cap;
+    blocks = (blocks + c->num_sms - 1) / c->num_sms * c->num_sms;
+#define SEM_GSM_LAUNCH(T, M, NF)                                                                                  \
+    k_gs_records_many<T, M, NF><<<(unsigned)blocks, NT, 0, c->stream>>>(np, c->d_own_pair, nq, c->d_own_quad, nb,  \
+                                                                         c->d_own_big, c->d_sh_idx, (T*)w, stride)
+#define SEM_GSM_NF(T, M)                                                                                          \
+    do {                                                                                                          \
+        if (nf == 2) SEM_GSM_LAUNCH(T, M, 2);                                                                     \
+        else if (nf == 3) SEM_GSM_LAUNCH(T, M, 3);                                                                \
+        else SEM_GSM_LAUNCH(T, M, 4);                                                                             \
+    } while (0)
+    if (prec == SEM_F64) { if (m) SEM_GSM_NF(double, true); else SEM_GSM_NF(double, false); }
+    else { if (m) SEM_GSM_NF(float, true); else SEM_GSM_NF(float, false); }
+#undef SEM_GSM_NF
+#undef SEM_GSM_LAUNCH
     SEM_CUDA_OK(c, cudaGetLastError());
     return SEM_OK;
 }

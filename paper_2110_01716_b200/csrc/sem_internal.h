@@ -127,6 +127,7 @@ int sem_launch_ax_gs(sem_ctx* c, const void* u, void* w, sem_prec prec, double l
                      const int* skip_flag);      // a3-a7: operator kernel + gather-scatter kernel
 // sem_gs.cu
 int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask);
+int sem_launch_gs_many(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec prec, bool apply_mask);
 // sem_transfer.cu
 int sem_launch_transfer(sem_ctx* coarse, sem_ctx* fine, const void* in, void* out, sem_prec prec, sem_transfer_dir dir,
                         const void* in_minus, const double* wt);

@@ -167,6 +167,24 @@ def run_projection(peak: float):
                   f"31 vectors read by the multi-dot, 61 read + 2 written by the update pass)")
 
 
+def run_gs_many(peak: float):
+    """NEXT-4, first piece: sem_gs_many (gatherScatterMany) on config 2 against nf separate sem_gs calls."""
+    mesh = inputs.config2()
+    print("| fields | precision | sem_gs x fields us | sem_gs_many us | speed-up |")
+    print("|---|---|---|---|---|")
+    with binding.Sem(mesh.E, mesh.N, mesh.vert, mesh.gid) as sem:
+        for dt, name in ((torch.float64, "FP64"), (torch.float32, "FP32")):
+            for nf in (2, 3, 4, 6):
+                w = torch.randn(nf, sem.nL, device="cuda", dtype=dt)
+
+                def separate():
+                    for f in range(nf):
+                        sem.gs(w[f])
+                t1 = _time(separate, 300)
+                t2 = _time(lambda: sem.gs_many(w), 300)
+                print(f"| {nf} | {name} | {t1:.1f} | {t2:.1f} | {t1 / t2:.2f} |", flush=True)
+
+
 def run_fdm(peak: float):
     """NEXT-2a: sem_fdm_apply (Eq. (3)) at the paper's per-GPU element count, m = N + 3 for N = 7, 5, 3, 1 and
     the paper's 8-5-1 / 8-6-4-1 schedules.  Bytes = b, Lambda^-1, u (m^3 each) + S (3 m^2) per element; flops = 12 m^4."""
@@ -190,6 +208,7 @@ def run_fdm(peak: float):
 
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--gs-many", action="store_true", help="NEXT-4: gather-scatter of several fields in one pass")
     ap.add_argument("--fdm", action="store_true", help="NEXT-2a: fast-diagonalisation local solve (Eq. (3)) at E = 7200")
     ap.add_argument("--proj", action="store_true", help="NEXT-3: projection onto previous solutions at config 2")
     ap.add_argument("--config5", type=int, default=0, help="run config 5 with this many elements per direction")
@@ -206,6 +225,8 @@ def main():
         return run_projection(peak)
     if args.fdm:
         return run_fdm(peak)
+    if args.gs_many:
+        return run_gs_many(peak)
     print(f"peak = {peak:.0f} GB/s (MEASURED_PEAKS.json hbm_gbs, else the profiling guide's fallback)")
     print("| case | E | N | nL | Ax us | Ax GB/s | frac of peak | gs us | Ax+gs us | Ax+gs GB/s | GDOF/s (E N^3) | "
           "Ax recomputed-G us | recomputed TFLOP/s |")

@@ -959,3 +959,52 @@ def test_fdm_setup_and_apply_pipeline(torch_cuda, binding, oracle_mod, m, E):
             du = torch_cuda.empty_like(db)
             sem.fdm_apply(m, dS, dL, db, du)
             assert relerr(du.cpu().numpy(), ou.ravel()) <= tol, (m, E, dt)
+
+
+# ------------------------------------------------- NEXT-4, first piece: gatherScatterMany (Table 3)
+@pytest.mark.parametrize("N,nf,pad", [(7, 3, 0), (7, 3, 40), (3, 4, 8), (5, 2, 0), (1, 7, 16), (2, 5, 0), (7, 1, 0)])
+def test_gs_many_bit_identical(torch_cuda, binding, oracle_mod, N, nf, pad):
+    """sem_gs_many on nf fields (stride nL + pad) against the oracle's gather-scatter of each field: same ascending-index
+    sums, so FP64 agrees to the last bit; the padding between fields is left untouched; FP32 at 1e-6.  Scrambled element
+    order; the 4x4x3 mesh has pair, quad and 8-copy records."""
+    m = inputs.box_mesh(4, 4, 3, N, permute_seed=6)
+    om = oracle_mod.Maps(m.gid)
+    rng = np.random.default_rng(100 + N)
+    w = rng.standard_normal((nf, m.nL + pad))                 # NOT continuous: a genuine gather-scatter input
+    ow = w.copy()
+    for f in range(nf):
+        ow[f, :m.nL] = oracle_mod.gs(w[f, :m.nL].copy(), om)
+    with binding.Sem(m.E, m.N, m.vert, m.gid) as sem:
+        dw = to_dev(torch_cuda, w)
+        sem.gs_many(dw)
+        assert np.array_equal(dw.cpu().numpy(), ow)
+        dw32 = to_dev(torch_cuda, w.astype(np.float32))
+        sem.gs_many(dw32)
+        assert relerr(dw32.cpu().numpy()[:, :m.nL], ow[:, :m.nL]) <= 1e-6
+        with pytest.raises(binding.SemError):
+            sem._check(sem._L.sem_gs_many(sem._h, dw.data_ptr(), 3, m.nL - 1, binding.SEM_F64, binding.SEM_OP_ADD))
+
+
+def test_gs_many_config2_three_fields(torch_cuda, binding, oracle_mod):
+    """Full size (config 2, three velocity-like fields): sem_gs_many equals sem_gs field by field, bit for bit, and the
+    oracle on sampled shared nodes."""
+    m = inputs.config2()
+    om = oracle_mod.Maps(m.gid)
+    rng = np.random.default_rng(8)
+    w = rng.standard_normal((3, m.nL))
+    with binding.Sem(m.E, m.N, m.vert, m.gid) as sem:
+        dw = to_dev(torch_cuda, w)
+        sem.gs_many(dw)
+        for f in range(3):
+            d1 = to_dev(torch_cuda, w[f])
+            sem.gs(d1)
+            assert torch_cuda.equal(d1, dw[f])
+        got = dw.cpu().numpy()
+    sample = rng.integers(0, om.U, 2000)
+    for g in sample:
+        idx = om.seg_idx[om.seg_off[g]:om.seg_off[g + 1]]
+        for f in range(3):
+            s = 0.0
+            for l in idx:                                     # ascending local index, like O5
+                s += w[f, l]
+            assert np.all(got[f, idx] == s)
