@@ -222,7 +222,17 @@ SEM_API int sem_fdm_apply(sem_ctx* ctx, int m, const void* S, const void* inv_la
  * m outside 2..16 or a B_d that is not positive definite. */
 SEM_API int sem_fdm_setup(int64_t E, int m, const double* A, const double* B, double* S, double* inv_lambda);
 
-/* Tuning knob for experiments: selects the Ax kernel variant (0 = default streaming kernel, 1 = simple kernel). */
+/* Measurement helper ("FP64 peak ... measure it"): a register-resident arithmetic microbenchmark on
+ * the current device, best of 5 launches after one warm-up, CUDA-event timed on `cuda_stream`; synchronises.  Not part
+ * of the method: bench.py quotes the FP64-ALU-bound kernels (a9 recomputed G, the fast-diagonalisation solve) against it.
+ *   kind        SEM_PEAK_FMA_F64 / SEM_PEAK_FMA_F32: independent FMA chains;  SEM_PEAK_DMMA_F64: mma.sync m8n8k4 f64
+ *   tflops_out  HOST  2 flops per FMA
+ * SEM_EINVAL for a bad kind or NULL; SEM_ECUDA without a device. */
+enum { SEM_PEAK_FMA_F64 = 0, SEM_PEAK_FMA_F32 = 1, SEM_PEAK_DMMA_F64 = 2 };
+SEM_API int sem_measure_peak(int kind, void* cuda_stream, double* tflops_out);
+
+/* Tuning knob for experiments: selects the Ax kernel variant (0 = default streaming kernel, 1 = simple kernel,
+ * 2 / 3 = FP64 p = 8 only: the tensor-core (DMMA m8n8k4) kernel with one warp per element, 8 / 14 warps per SM). */
 SEM_API int sem_set_variant(sem_ctx* ctx, int ax_variant);
 
 /* Last error text of this context ("" if none); valid until the next call on the context.  NULL ctx -> static text. */

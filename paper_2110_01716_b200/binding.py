@@ -55,6 +55,7 @@ SYMBOLS = {
     "sem_pmg_get_history": (_i32, [_vp, _vp, _i32]),
     "sem_fdm_apply": (_i32, [_vp, _i32, _vp, _vp, _vp, _vp, _i32]),
     "sem_fdm_setup": (_i32, [_i64, _i32, _vp, _vp, _vp, _vp]),
+    "sem_measure_peak": (_i32, [_i32, _vp, C.POINTER(_dbl)]),
     "sem_last_error": (C.c_char_p, [_vp]),
     "sem_ctx_destroy": (None, [_vp]),
 }
@@ -74,6 +75,16 @@ def fdm_setup(A: np.ndarray, B: np.ndarray):
     if rc != SEM_OK:
         raise SemError(rc, "sem_fdm_setup: bad arguments or a mass matrix that is not positive definite")
     return S, inv_lambda
+
+
+def measure_peak(kind: int) -> float:
+    """sem_measure_peak on torch's current stream: TFLOP/s of kind 0 = FP64 FMA, 1 = FP32 FMA, 2 = FP64 DMMA m8n8k4."""
+    import torch
+    out = _dbl(0.0)
+    rc = lib().sem_measure_peak(kind, C.c_void_p(torch.cuda.current_stream().cuda_stream), C.byref(out))
+    if rc != SEM_OK:
+        raise SemError(rc, "sem_measure_peak")
+    return float(out.value)
 
 
 class SemError(RuntimeError):

@@ -414,6 +414,181 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// ax_dmma: FP64, p = 8, ONE WARP per element; the r and s contractions of every k-plane run on the tensor cores as
+// mma.sync.m8n8k4.f64 (DMMA).  north_star / SURVEY H3: "DMMA (m8n8k4 fits p = 8) only if measured faster" -- this is the
+// kernel that measurement is made with (variant 2; profiles/r2_dmma.md).  The DMMA rate of the part equals its DFMA
+// rate, so the point is not flops: it is shared-memory wavefronts and issue slots.  Lane (g = lane / 4, t = lane % 4)
+// owns the two columns (j = g, i = 2t, 2t + 1) of the element, which is exactly the C-fragment layout of m8n8k4, and
+//   u_r = U_k D^T : A = the lane's own two u values (contraction index l = 2t + c for the two k-chunks c: a permutation
+//                   of l shared by A and B, so no shuffle), B = constant fragment of D;
+//   u_s = D U_k   : A = constant fragment of D, B = 2 values of the u plane read from shared memory;
+//   w  += g_r D   : A = the lane's own two g_r values, B = constant;      w += D^T g_s : A = constant, B = 2 values of
+//                   the g_s plane after one STS.128 + __syncwarp (the only exchange per plane);
+//   the t direction stays in the lane's registers as in ax_stream.
+// Per k-plane and element: 36 shared-memory wavefronts instead of 148, 8 DMMA + ~64 DFMA per lane instead of 2 x 126,
+// no CTA barrier at all.  Streaming of G and u is the same mbarrier ring as ax_stream.
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+template <int NS>
+struct DmmaSmem {
+    alignas(128) double g[NS][6 * 64];
+    alignas(128) double u[2][512];
+    alignas(16) double sgs[2][64];
+    alignas(8) uint64_t gfull[NS];
+    alignas(8) uint64_t ufull[2];
+    alignas(16) double D[64];
+};
+
+template <int NS, int MINB>
+__global__ void __launch_bounds__(32, MINB) ax_dmma(int64_t E, DParam<double, 8> dp, const double* __restrict__ Gs,
+                                                    const double* __restrict__ Bm, double lambda,
+                                                    const double* __restrict__ u, double* __restrict__ w,
+                                                    const int* __restrict__ skip_flag, double* __restrict__ dot_out) {
+    using SM = DmmaSmem<NS>;
+    constexpr int P = 8, P2 = 64, P3 = 512, SLAB = 6 * 64;
+    constexpr uint32_t GBYTES = SLAB * sizeof(double), UBYTES = P3 * sizeof(double);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    SM& sm = *reinterpret_cast<SM*>(smem_raw);
+    if (skip_flag && *skip_flag) return;
+    const int lane = threadIdx.x, g = lane >> 2, t = lane & 3;
+    const int64_t nmine = blockIdx.x < E ? (E - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+
+    const double* gsrc = Gs + (int64_t)blockIdx.x * (P * SLAB);
+    const int64_t gjump = (int64_t)(gridDim.x - 1) * (P * SLAB);
+    int64_t gleft = nmine * P;
+    uint64_t pol_g = 0, pol_u = 0;
+    auto issue_u = [&](int64_t n) {
+        const int64_t e = blockIdx.x + n * gridDim.x;
+        const int b = (int)(n & 1);
+        mbar_expect_tx(&sm.ufull[b], UBYTES);
+        bulk_g2s(&sm.u[b][0], u + e * P3, UBYTES, &sm.ufull[b], pol_u);
+    };
+    if (lane == 0) {
+#pragma unroll
+        for (int q = 0; q < NS; ++q) mbar_init(&sm.gfull[q], 1);
+        mbar_init(&sm.ufull[0], 1);
+        mbar_init(&sm.ufull[1], 1);
+        mbar_fence_init();
+    }
+    sm.D[lane] = dp.D[lane];
+    sm.D[lane + 32] = dp.D[lane + 32];
+    __syncwarp();
+    if (lane == 0 && nmine > 0) {
+        pol_g = policy_evict_first();
+        pol_u = policy_evict_last();
+        issue_u(0);
+        int gk = 0;
+        for (int q = 0; q < NS && gleft > 0; ++q) {
+            mbar_expect_tx(&sm.gfull[q], GBYTES);
+            bulk_g2s(&sm.g[q][0], gsrc, GBYTES, &sm.gfull[q], pol_g);
+            gsrc += SLAB;
+            if (++gk == P) { gk = 0; gsrc += gjump; }
+            --gleft;
+        }
+        if (nmine > 1) issue_u(1);
+    }
+    // constant fragments of D (volatile loads: pinned in registers, see DRows::init_shared)
+    double Br[2], As[2], BrT[2], AsT[2];
+    {
+        const uint32_t base = smem_u32(sm.D);
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            Br[c] = DRows<double, 8>::lds_volatile(base + (uint32_t)((g * 8 + 2 * t + c) * 8));      // D[i=g][l=2t+c]
+            As[c] = DRows<double, 8>::lds_volatile(base + (uint32_t)((g * 8 + 4 * c + t) * 8));      // D[j=g][l=4c+t]
+            BrT[c] = DRows<double, 8>::lds_volatile(base + (uint32_t)(((2 * t + c) * 8 + g) * 8));   // D[l=2t+c][i=g]
+            AsT[c] = DRows<double, 8>::lds_volatile(base + (uint32_t)(((4 * c + t) * 8 + g) * 8));   // D[l=4c+t][j=g]
+        }
+    }
+    double partial = 0.0;
+    int q = 0;
+    uint32_t gphase = 0;
+    const int own = g * 8 + 2 * t;                     // the lane's two nodes (j = g, i = 2t, 2t+1) inside a plane
+    double* wdst = w + (int64_t)blockIdx.x * P3 + own;
+    const int64_t wstep = (int64_t)gridDim.x * P3;
+    for (int64_t n = 0; n < nmine; ++n, wdst += wstep) {
+        const int ub = (int)(n & 1);
+        mbar_wait(&sm.ufull[ub], (uint32_t)((n >> 1) & 1));
+        const double* sue = &sm.u[ub][0];
+        double uk[P][2], wk[P][2];
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+            const double2 v = *reinterpret_cast<const double2*>(sue + k * P2 + own);
+            uk[k][0] = v.x; uk[k][1] = v.y; wk[k][0] = 0.0; wk[k][1] = 0.0;
+        }
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+            mbar_wait(&sm.gfull[q], gphase);
+            double G6[6][2];
+#pragma unroll
+            for (int c = 0; c < 6; ++c) {
+                const double2 v = *reinterpret_cast<const double2*>(&sm.g[q][c * P2 + own]);
+                G6[c][0] = v.x; G6[c][1] = v.y;
+            }
+            // u_r = U_k D^T  and  u_s = D U_k  on the tensor cores
+            double ur[2] = {0.0, 0.0}, us[2] = {0.0, 0.0};
+            dmma884(ur[0], ur[1], uk[k][0], Br[0]);
+            dmma884(us[0], us[1], As[0], sue[k * P2 + t * P + g]);
+            dmma884(ur[0], ur[1], uk[k][1], Br[1]);
+            dmma884(us[0], us[1], As[1], sue[k * P2 + (4 + t) * P + g]);
+            double ut[2] = {0.0, 0.0};
+#pragma unroll
+            for (int l = 0; l < P; ++l) { ut[0] += dp.D[k * P + l] * uk[l][0]; ut[1] += dp.D[k * P + l] * uk[l][1]; }
+            double gr[2], gs[2], gt[2];
+#pragma unroll
+            for (int b = 0; b < 2; ++b) {
+                gr[b] = G6[0][b] * ur[b] + G6[1][b] * us[b] + G6[2][b] * ut[b];
+                gs[b] = G6[1][b] * ur[b] + G6[3][b] * us[b] + G6[4][b] * ut[b];
+                gt[b] = G6[2][b] * ur[b] + G6[4][b] * us[b] + G6[5][b] * ut[b];
+            }
+            const int buf = k & 1;
+            *reinterpret_cast<double2*>(&sm.sgs[buf][own]) = make_double2(gs[0], gs[1]);
+#pragma unroll
+            for (int l = 0; l < P; ++l) { wk[l][0] += dp.D[k * P + l] * gt[0]; wk[l][1] += dp.D[k * P + l] * gt[1]; }
+            __syncwarp();
+            // every lane has consumed stage q (and, on the last plane, this element's u buffer): refill
+            if (lane == 0) {
+                if (gleft > 0) {
+                    mbar_expect_tx(&sm.gfull[q], GBYTES);
+                    bulk_g2s(&sm.g[q][0], gsrc, GBYTES, &sm.gfull[q], pol_g);
+                    gsrc += SLAB;
+                    if ((k + NS) % P == P - 1) gsrc += gjump;
+                    --gleft;
+                }
+                if (k == P - 1 && n + 2 < nmine) issue_u(n + 2);
+            }
+            // w_k += g_r D + D^T g_s
+            double a0[2] = {0.0, 0.0}, a1[2] = {0.0, 0.0};
+            dmma884(a0[0], a0[1], gr[0], BrT[0]);
+            dmma884(a1[0], a1[1], AsT[0], sm.sgs[buf][t * P + g]);
+            dmma884(a0[0], a0[1], gr[1], BrT[1]);
+            dmma884(a1[0], a1[1], AsT[1], sm.sgs[buf][(4 + t) * P + g]);
+            wk[k][0] += a0[0] + a1[0];
+            wk[k][1] += a0[1] + a1[1];
+            if (++q == NS) { q = 0; gphase ^= 1u; }
+        }
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+            double v0 = wk[k][0], v1 = wk[k][1];
+            if (Bm) {
+                const double2 bm = *reinterpret_cast<const double2*>(Bm + (wdst - w) + k * P2);
+                v0 += lambda * bm.x * uk[k][0];
+                v1 += lambda * bm.y * uk[k][1];
+            }
+            *reinterpret_cast<double2*>(wdst + k * P2) = make_double2(v0, v1);
+            partial += uk[k][0] * v0 + uk[k][1] * v1;
+        }
+    }
+    if (dot_out) {
+        for (int o = 16; o; o >>= 1) partial += __shfl_xor_sync(0xffffffffu, partial, o);
+        if (lane == 0) atomicAdd(dot_out, partial);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------------------------
 template <typename T, int P>
@@ -472,6 +647,24 @@ int launch_stream(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, doubl
     return SEM_OK;
 }
 
+template <int NS, int MINB>
+int launch_dmma(sem_ctx* c, const double* u, double* w, double lambda, const int* skip, double* dot) {
+    using SM = DmmaSmem<NS>;
+    const DParam<double, 8> dp = make_dparam<double, 8>(c);
+    const size_t smem = sizeof(SM) + 128;
+    auto kern = ax_dmma<NS, MINB>;
+    int blocks_per_sm = 0;
+    SEM_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    SEM_CUDA_OK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, 32, smem));
+    if (blocks_per_sm < 1) return sem_fail(c, SEM_ECUDA, "ax_dmma does not fit on an SM");
+    const int64_t cap = (int64_t)c->num_sms * blocks_per_sm;
+    const unsigned grid = (unsigned)(c->E < cap ? c->E : cap);
+    kern<<<grid, 32, smem, c->stream>>>(c->E, dp, c->d_G, lambda != 0.0 ? c->d_B : (const double*)nullptr, lambda, u, w,
+                                        skip, dot);
+    SEM_CUDA_OK(c, cudaGetLastError());
+    return SEM_OK;
+}
+
 // stage depth / residency per (T, P): sized so that ~7-8 CTAs fit in 227 KB and > 64 KB are in flight per SM
 template <typename T, int P> struct StreamCfg { static constexpr int NS = 4, MINB = 1; };
 template <> struct StreamCfg<double, 8> { static constexpr int NS = 5, MINB = 8; };
@@ -493,6 +686,10 @@ int dispatch_p(sem_ctx* c, const void* u, void* w, double lambda, const int* ski
     T* ww = (T*)w;
     const bool aligned = ((uintptr_t)u % 16) == 0;
     if (c->gmode == SEM_G_RECOMPUTE) return launch_simple<T, P, true>(c, uu, ww, (T)lambda, skip, dot);
+    if constexpr (P == 8 && sizeof(T) == 8) {          // variants 2, 3: the DMMA kernel (one warp per element)
+        if (aligned && c->ax_variant == 2) return launch_dmma<5, 8>(c, (const double*)u, (double*)w, lambda, skip, dot);
+        if (aligned && c->ax_variant == 3) return launch_dmma<3, 12>(c, (const double*)u, (double*)w, lambda, skip, dot);
+    }
     if constexpr (stream_ok<P>()) {
         if (c->ax_variant != 1 && aligned)
             return launch_stream<T, P, StreamCfg<T, P>::NS, StreamCfg<T, P>::MINB>(c, uu, ww, (T)lambda, skip, dot);
