@@ -12,6 +12,7 @@
 //   * persistent CTAs (one element group at a time, grid = SMs x resident CTAs) write w straight from registers.
 // ax_simple is the plain-load version of the same arithmetic: odd p, unaligned pointers, and the recomputed-G
 // variant (a9: G from the 8 trilinear vertices inside the kernel) use it.
+#include <mutex>
 #include <type_traits>
 
 #include "sem_geom_dev.cuh"
@@ -416,7 +417,7 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
 // ---------------------------------------------------------------------------------------------------------------
 // ax_dmma: FP64, p = 8, ONE WARP per element; the r and s contractions of every k-plane run on the tensor cores as
 // mma.sync.m8n8k4.f64 (DMMA).  north_star / SURVEY H3: "DMMA (m8n8k4 fits p = 8) only if measured faster" -- this is the
-// kernel that measurement is made with (variant 2; profiles/r2_dmma.md).  The DMMA rate of the part equals its DFMA
+// kernel that measurement was made with, and it won (profiles/r2_dmma.md): it is the default for FP64 p = 8.  The DMMA rate of the part equals its DFMA
 // rate, so the point is not flops: it is shared-memory wavefronts and issue slots.  Lane (g = lane / 4, t = lane % 4)
 // owns the two columns (j = g, i = 2t, 2t + 1) of the element, which is exactly the C-fragment layout of m8n8k4, and
 //   u_r = U_k D^T : A = the lane's own two u values (contraction index l = 2t + c for the two k-chunks c: a permutation
@@ -605,6 +606,26 @@ Gll1D make_gll(const sem_ctx* c) {
     return g;
 }
 
+// Resident CTAs per SM of one kernel instantiation with its dynamic shared memory, cached per device (the opt-in
+// attribute is per device as well).  One table per instantiation (the template parameter K is the kernel's type).
+template <typename K>
+int resident_blocks(sem_ctx* c, K kern, int threads, size_t smem, int* out) {
+    static std::mutex mu;
+    static int table[SEM_MAX_DEVICES] = {};
+    std::lock_guard<std::mutex> lk(mu);
+    const bool cacheable = c->device >= 0 && c->device < SEM_MAX_DEVICES;
+    if (!cacheable || !table[c->device]) {
+        int nb = 0;
+        SEM_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        SEM_CUDA_OK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, threads, smem));
+        if (nb < 1) return sem_fail(c, SEM_ECUDA, "Ax kernel does not fit on an SM");
+        if (!cacheable) { *out = nb; return SEM_OK; }
+        table[c->device] = nb;
+    }
+    *out = table[c->device];
+    return SEM_OK;
+}
+
 template <typename T, int P, bool RECOMP>
 int launch_simple(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, double* dot) {
     constexpr int EPB = epb_of<P>();
@@ -631,14 +652,8 @@ int launch_stream(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, doubl
     const DParam<T, P> dp = make_dparam<T, P>(c);
     const size_t smem = sizeof(SM) + 128;
     auto kern = ax_stream<T, P, NS, MINB>;
-    static thread_local int cached_dev = -1;
-    static thread_local int blocks_per_sm = 0;
-    if (cached_dev != c->device) {
-        SEM_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        SEM_CUDA_OK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, threads_of<P>(), smem));
-        if (blocks_per_sm < 1) return sem_fail(c, SEM_ECUDA, "ax_stream does not fit on an SM");
-        cached_dev = c->device;
-    }
+    int blocks_per_sm = 0;
+    if (int rc = resident_blocks(c, kern, threads_of<P>(), smem, &blocks_per_sm)) return rc;
     const int64_t cap = (int64_t)c->num_sms * blocks_per_sm;
     const unsigned grid = (unsigned)(ngroups < cap ? ngroups : cap);
     kern<<<grid, threads_of<P>(), smem, c->stream>>>(c->E, dp, Gs, lambda != T(0) ? Bm : (const T*)nullptr, lambda, u, w,
@@ -654,9 +669,7 @@ int launch_dmma(sem_ctx* c, const double* u, double* w, double lambda, const int
     const size_t smem = sizeof(SM) + 128;
     auto kern = ax_dmma<NS, MINB>;
     int blocks_per_sm = 0;
-    SEM_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    SEM_CUDA_OK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, 32, smem));
-    if (blocks_per_sm < 1) return sem_fail(c, SEM_ECUDA, "ax_dmma does not fit on an SM");
+    if (int rc = resident_blocks(c, kern, 32, smem, &blocks_per_sm)) return rc;
     const int64_t cap = (int64_t)c->num_sms * blocks_per_sm;
     const unsigned grid = (unsigned)(c->E < cap ? c->E : cap);
     kern<<<grid, 32, smem, c->stream>>>(c->E, dp, c->d_G, lambda != 0.0 ? c->d_B : (const double*)nullptr, lambda, u, w,
@@ -686,9 +699,11 @@ int dispatch_p(sem_ctx* c, const void* u, void* w, double lambda, const int* ski
     T* ww = (T*)w;
     const bool aligned = ((uintptr_t)u % 16) == 0;
     if (c->gmode == SEM_G_RECOMPUTE) return launch_simple<T, P, true>(c, uu, ww, (T)lambda, skip, dot);
-    if constexpr (P == 8 && sizeof(T) == 8) {          // variants 2, 3: the DMMA kernel (one warp per element)
-        if (aligned && c->ax_variant == 2) return launch_dmma<5, 8>(c, (const double*)u, (double*)w, lambda, skip, dot);
-        if (aligned && c->ax_variant == 3) return launch_dmma<3, 12>(c, (const double*)u, (double*)w, lambda, skip, dot);
+    // variant 0: the default kernel per (T, p); 1: ax_simple; 2: ax_stream where it exists (scalar contractions);
+    // 3: the DMMA kernel with 5 stages / 8 warps per SM (the configuration that mirrors ax_stream's residency)
+    if constexpr (P == 8 && sizeof(T) == 8) {
+        if (aligned && c->ax_variant == 0) return launch_dmma<3, 12>(c, (const double*)u, (double*)w, lambda, skip, dot);
+        if (aligned && c->ax_variant == 3) return launch_dmma<5, 8>(c, (const double*)u, (double*)w, lambda, skip, dot);
     }
     if constexpr (stream_ok<P>()) {
         if (c->ax_variant != 1 && aligned)
@@ -725,5 +740,5 @@ int sem_launch_ax_gs(sem_ctx* c, const void* u, void* w, sem_prec prec, double l
                      const int* skip_flag) {
     int rc;
     if ((rc = sem_launch_ax(c, u, w, prec, lambda, dot_out, skip_flag))) return rc;
-    return sem_launch_gs(c, w, prec, true);
+    return sem_launch_gs(c, w, prec, true, skip_flag);
 }

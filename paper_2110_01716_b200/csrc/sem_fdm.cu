@@ -16,6 +16,8 @@
 // S, Lambda^-1 and b reach shared memory by cp.async (coalesced, no registers); u is written straight from registers.
 // This is not the paper's kernel (OCCA, one thread block per element, operands in shared memory).  It is still bound
 // by the shared-memory pipe (a warp-uniform 128-bit load costs two wavefronts), see DESIGN.md section 6.
+#include <mutex>
+
 #include "sem_internal.h"
 #include "sem_fdm_dev.cuh"
 
@@ -27,14 +29,22 @@ template <typename T, int M, int LPT, int EPC, int NST, bool SREG>
 int launch_cfg(sem_ctx* c, const void* S, const void* invL, const void* b, void* u) {
     using C = fdm_cfg<T, M, LPT, EPC>;
     constexpr size_t SMEM = C::SMEM1 * NST;
-    static int resident = 0;                             // CTAs per SM of this instantiation
     auto kern = SREG ? k_fdm_sreg<T, M, LPT, EPC, 1, NST> : k_fdm<T, M, LPT, EPC, 1, NST>;
-    if (!resident) {
-        if (SMEM > 48 * 1024)
-            SEM_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
-        int nb = 0;
-        SEM_CUDA_OK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, C::NT, SMEM));
-        resident = nb > 0 ? nb : 1;
+    // CTAs per SM of this instantiation, per device (the attribute is per device too); guarded for concurrent callers
+    static std::mutex mu;
+    static int resident_of[SEM_MAX_DEVICES] = {};
+    int resident = 0;
+    {
+        std::lock_guard<std::mutex> lk(mu);
+        const int dev = c->device >= 0 && c->device < SEM_MAX_DEVICES ? c->device : 0;
+        if (!resident_of[dev] || dev != c->device) {
+            if (SMEM > 48 * 1024)
+                SEM_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
+            int nb = 0;
+            SEM_CUDA_OK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, C::NT, SMEM));
+            resident_of[dev] = nb > 0 ? nb : 1;
+        }
+        resident = resident_of[dev];
     }
     const int64_t ngrp = (c->E + C::EPC - 1) / C::EPC;
     int64_t grid = (int64_t)c->num_sms * resident;       // single wave of persistent CTAs (a grid cut down to equal

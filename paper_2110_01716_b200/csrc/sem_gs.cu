@@ -29,15 +29,16 @@ template <typename T, bool MASK>
 __global__ void __launch_bounds__(NT, GS_CTAS) k_gs_records(int32_t n_pair, const int2* __restrict__ pair, int32_t n_quad,
                                                    const int4* __restrict__ quad, int32_t n_big,
                                                    const int2* __restrict__ big, const int32_t* __restrict__ sh_idx,
-                                                   T* __restrict__ w) {
+                                                   T* __restrict__ w, const int* __restrict__ skip_flag) {
+    if (skip_flag && *skip_flag) return;                 // the PCG loop has converged: every later launch is a no-op
     // every CTA takes the same share of every record class (contiguous, whole 32-record rows): balanced by construction
     const int32_t b = blockIdx.x, nb = gridDim.x;
     const int32_t pp = ((n_pair + nb - 1) / nb + 31) & ~31, pq = ((n_quad + nb - 1) / nb + 31) & ~31,
                   pg = (n_big + nb - 1) / nb;
     const int64_t bp = (int64_t)b * pp, bq = (int64_t)b * pq, bg = (int64_t)b * pg;
-    if (bp < n_pair) gs_pairs<T, MASK, false, NT>(pair, (int32_t)bp + threadIdx.x, min(n_pair, (int32_t)bp + pp), w);
-    if (bq < n_quad) gs_quads<T, MASK, false, NT>(quad, (int32_t)bq + threadIdx.x, min(n_quad, (int32_t)bq + pq), w);
-    if (bg < n_big) gs_bigs<T, MASK, false, NT>(big, sh_idx, (int32_t)bg + threadIdx.x, min(n_big, (int32_t)bg + pg), w);
+    if (bp < n_pair) gs_pairs<T, MASK, NT>(pair, (int32_t)bp + threadIdx.x, min(n_pair, (int32_t)bp + pp), w);
+    if (bq < n_quad) gs_quads<T, MASK, NT>(quad, (int32_t)bq + threadIdx.x, min(n_quad, (int32_t)bq + pq), w);
+    if (bg < n_big) gs_bigs<T, MASK, NT>(big, sh_idx, (int32_t)bg + threadIdx.x, min(n_big, (int32_t)bg + pg), w);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -114,13 +115,13 @@ __global__ void __launch_bounds__(NT, 4) k_gs_records_many(int32_t n_pair, const
     }
     if (bg < n_big)                                           // rare (> 4 copies): field by field
         for (int f = 0; f < NF; ++f)
-            gs_bigs<T, MASK, false, NT>(big, sh_idx, (int32_t)bg + threadIdx.x, min(n_big, (int32_t)bg + pg),
+            gs_bigs<T, MASK, NT>(big, sh_idx, (int32_t)bg + threadIdx.x, min(n_big, (int32_t)bg + pg),
                                         w + f * stride);
 }
 
 }  // namespace
 
-int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask) {
+int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask, const int* skip_flag) {
     const bool m = apply_mask && c->has_mask;
     const int32_t np = (int32_t)c->n_pair, nq = (int32_t)c->n_quad, nb = (int32_t)c->n_big;
     if (np + nq + nb == 0) return SEM_OK;
@@ -132,7 +133,7 @@ int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask) {
     blocks = (blocks + c->num_sms - 1) / c->num_sms * c->num_sms;      // same number of CTAs on every SM
 #define SEM_GS_LAUNCH(T, M)                                                                                      \
     k_gs_records<T, M><<<(unsigned)blocks, NT, 0, c->stream>>>(np, c->d_own_pair, nq, c->d_own_quad, nb,          \
-                                                                c->d_own_big, c->d_sh_idx, (T*)w)
+                                                                c->d_own_big, c->d_sh_idx, (T*)w, skip_flag)
     if (prec == SEM_F64) { if (m) SEM_GS_LAUNCH(double, true); else SEM_GS_LAUNCH(double, false); }
     else { if (m) SEM_GS_LAUNCH(float, true); else SEM_GS_LAUNCH(float, false); }
 #undef SEM_GS_LAUNCH

@@ -1,6 +1,6 @@
-// sem_gs_dev.cuh — device-side record processing of the gather-scatter (a6 + a7), shared by the stand-alone kernel
-// (sem_gs.cu) and the gather-scatter tail phase of the operator kernel (sem_ax.cu).  See sem_gs.cu for the record
-// formats; sums run in ascending local index (O5), so every caller produces bit-identical results.
+// sem_gs_dev.cuh — device-side record processing of the gather-scatter (a6 + a7) used by the kernels of sem_gs.cu.
+// See sem_gs.cu for the record formats; sums run in ascending local index (O5), so results are bit-identical to the
+// oracle's.
 #pragma once
 #include <stdint.h>
 
@@ -9,23 +9,8 @@ namespace semgs {
 constexpr int32_t IDX = 0x7fffffff;
 constexpr int PPT = 4;           // pairs per thread in flight
 
-// COHERENT: read values with ld.relaxed.gpu (from L2): they were written by another, still running, kernel
-template <typename T, bool COHERENT>
-__device__ __forceinline__ T ld_val(const T* p) {
-    if constexpr (!COHERENT) return *p;
-    else if constexpr (sizeof(T) == 8) {
-        double v;
-        asm volatile("ld.relaxed.gpu.global.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
-        return v;
-    } else {
-        float v;
-        asm volatile("ld.relaxed.gpu.global.f32 %0, [%1];" : "=f"(v) : "l"(p) : "memory");
-        return v;
-    }
-}
-
 // records [first, end) with stride NTH between the records of one thread
-template <typename T, bool MASK, bool COHERENT, int NTH, int PP = PPT>
+template <typename T, bool MASK, int NTH, int PP = PPT>
 __device__ __forceinline__ void gs_pairs(const int2* __restrict__ pair, int32_t first, int32_t end, T* __restrict__ w) {
     for (int32_t base = first; base < end; base += NTH * PP) {
         int2 r[PP];
@@ -37,8 +22,8 @@ __device__ __forceinline__ void gs_pairs(const int2* __restrict__ pair, int32_t 
         T v0[PP], v1[PP];
 #pragma unroll
         for (int q = 0; q < PP; ++q) {
-            v0[q] = r[q].y >= 0 ? ld_val<T, COHERENT>(w + (r[q].x & IDX)) : T(0);
-            v1[q] = r[q].y >= 0 ? ld_val<T, COHERENT>(w + r[q].y) : T(0);
+            v0[q] = r[q].y >= 0 ? w[(r[q].x & IDX)] : T(0);
+            v1[q] = r[q].y >= 0 ? w[r[q].y] : T(0);
         }
 #pragma unroll
         for (int q = 0; q < PP; ++q) {
@@ -54,13 +39,13 @@ __device__ __forceinline__ void gs_pairs(const int2* __restrict__ pair, int32_t 
     }
 }
 
-template <typename T, bool MASK, bool COHERENT, int NTH>
+template <typename T, bool MASK, int NTH>
 __device__ __forceinline__ void gs_quads(const int4* __restrict__ quad, int32_t first, int32_t end, T* __restrict__ w) {
     for (int32_t t = first; t < end; t += NTH) {
         const int4 r = quad[t];
         const int32_t l0 = r.x & IDX;
-        const T a0 = ld_val<T, COHERENT>(w + l0), a1 = ld_val<T, COHERENT>(w + r.y), a2 = ld_val<T, COHERENT>(w + r.z);
-        const T a3 = r.w >= 0 ? ld_val<T, COHERENT>(w + r.w) : T(0);
+        const T a0 = w[l0], a1 = w[r.y], a2 = w[r.z];
+        const T a3 = r.w >= 0 ? w[r.w] : T(0);
         T s = (a0 + a1) + a2;
         if (r.w >= 0) s += a3;
         if (MASK && r.x < 0) s = T(0);
@@ -69,7 +54,7 @@ __device__ __forceinline__ void gs_quads(const int4* __restrict__ quad, int32_t 
     }
 }
 
-template <typename T, bool MASK, bool COHERENT, int NTH>
+template <typename T, bool MASK, int NTH>
 __device__ __forceinline__ void gs_bigs(const int2* __restrict__ big, const int32_t* __restrict__ sh_idx, int32_t first,
                                         int32_t end, T* __restrict__ w) {
     for (int32_t t = first; t < end; t += NTH) {
@@ -81,11 +66,11 @@ __device__ __forceinline__ void gs_bigs(const int2* __restrict__ big, const int3
 #pragma unroll
         for (int q = 0; q < 8; ++q) id[q] = q < cnt ? __ldg(&sh_idx[r.x + q]) : -1;
 #pragma unroll
-        for (int q = 0; q < 8; ++q) v[q] = id[q] >= 0 ? ld_val<T, COHERENT>(w + id[q]) : T(0);
+        for (int q = 0; q < 8; ++q) v[q] = id[q] >= 0 ? w[id[q]] : T(0);
         T s = v[0];
 #pragma unroll
         for (int q = 1; q < 8; ++q) if (id[q] >= 0) s += v[q];
-        for (int32_t q = 8; q < cnt; ++q) s += ld_val<T, COHERENT>(w + sh_idx[r.x + q]);
+        for (int32_t q = 8; q < cnt; ++q) s += w[sh_idx[r.x + q]];
         if (MASK && r.y < 0) s = T(0);
 #pragma unroll
         for (int q = 0; q < 8; ++q) if (id[q] >= 0) w[id[q]] = s;

@@ -8,6 +8,7 @@
 #include "../../include/sem.h"
 
 #define SEM_MAXP 16
+#define SEM_MAX_DEVICES 64      // per-device caches of launch configurations (occupancy, shared-memory opt-in)
 
 // Elements per CTA ("group") of the Ax kernels: enough elements to fill 64 threads with one (i,j) column each.
 // G is stored group-blocked so that one k-slab of one group is one contiguous chunk (one bulk copy):
@@ -81,8 +82,8 @@ struct sem_ctx {
     double* h_hist = nullptr;
     int hist_n = 0;
     // ---- p-multigrid transfer (NEXT-1, sem_transfer.cu) ----
-    void* d_J = nullptr;           // [SEM_MAXP^2] interpolation matrix of the last transfer, in its precision
-    int J_key = -1;                // (coarse p) * 2 + (FP32 ? 1 : 0) of what d_J holds
+    void* d_J = nullptr;           // interpolation matrices, one slot of SEM_MAXP^2 doubles per key = (coarse p) * 2 +
+    uint64_t J_have = 0;           // (FP32 ? 1 : 0), each written once (bit `key` of J_have): graphs never see a rewrite
     float* d_Minv32 = nullptr;     // Minv rounded to FP32 for the FP32 smoother (sem_cheby.cu)
     double lambda_of_minv32 = -1.0;
     void* d_cheb[3] = {nullptr, nullptr, nullptr};   // r, d, w of the Chebyshev smoother (sem_cheby.cu), nL doubles each
@@ -126,7 +127,7 @@ int sem_launch_ax(sem_ctx* c, const void* u, void* w, sem_prec prec, double lamb
 int sem_launch_ax_gs(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda, double* dot_out,
                      const int* skip_flag);      // a3-a7: operator kernel + gather-scatter kernel
 // sem_gs.cu
-int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask);
+int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask, const int* skip_flag = nullptr);
 int sem_launch_gs_many(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec prec, bool apply_mask);
 // sem_transfer.cu
 int sem_launch_transfer(sem_ctx* coarse, sem_ctx* fine, const void* in, void* out, sem_prec prec, sem_transfer_dir dir,

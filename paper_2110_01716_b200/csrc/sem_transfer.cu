@@ -102,17 +102,21 @@ void interp_matrix(const sem_ctx* cc, const sem_ctx* cf, double* J) {
     }
 }
 
+constexpr size_t J_SLOT_BYTES = sizeof(double) * SEM_MAXP * SEM_MAXP;
+
 template <typename T>
 int launch(sem_ctx* cf, int pc, const double* Jh, const void* in, void* out, bool restrict_, const void* in_minus,
            const double* wt) {
     const int pf = cf->p;
+    // One device copy of J per (coarse p, precision), each in its own slot of d_J and written once: a CUDA graph that
+    // recorded a transfer keeps pointing at a matrix that no later call with another level pair or precision rewrites.
     const int key = pc * 2 + (sizeof(T) == 8 ? 0 : 1);
-    if (cf->J_key != key) {                       // the matrix on the device is for another level pair / precision
+    const T* dJ = reinterpret_cast<const T*>(static_cast<const char*>(cf->d_J) + (size_t)key * J_SLOT_BYTES);
+    if (!((cf->J_have >> key) & 1ull)) {
         T hJ[SEM_MAXP * SEM_MAXP];
         for (int q = 0; q < pf * pc; ++q) hJ[q] = (T)Jh[q];          // S16: computed in double, rounded once
-        SEM_CUDA_OK(cf, cudaStreamSynchronize(cf->stream));          // earlier transfers may still read the old one
-        SEM_CUDA_OK(cf, cudaMemcpy(cf->d_J, hJ, sizeof(T) * pf * pc, cudaMemcpyHostToDevice));
-        cf->J_key = key;
+        SEM_CUDA_OK(cf, cudaMemcpy(const_cast<T*>(dJ), hJ, sizeof(T) * pf * pc, cudaMemcpyHostToDevice));
+        cf->J_have |= 1ull << key;
     }
     int epc = TNT / (pf * pf);
     if (epc < 1) epc = 1;
@@ -129,7 +133,7 @@ int launch(sem_ctx* cf, int pc, const double* Jh, const void* in, void* out, boo
     const int64_t ngrp = (cf->E + epc - 1) / epc;
     int64_t grid = (int64_t)cf->num_sms * 8;
     if (grid > ngrp) grid = ngrp;
-    kern<<<(unsigned)grid, TNT, smem, cf->stream>>>(cf->E, pc, pf, epc, (const T*)cf->d_J, (const T*)in, (T*)out,
+    kern<<<(unsigned)grid, TNT, smem, cf->stream>>>(cf->E, pc, pf, epc, dJ, (const T*)in, (T*)out,
                                                     (const T*)in_minus, wt);
     SEM_CUDA_OK(cf, cudaGetLastError());
     return SEM_OK;
@@ -161,7 +165,7 @@ int sem_launch_transfer(sem_ctx* coarse, sem_ctx* fine, const void* in, void* ou
     if (!in || !out || in == out) return sem_fail(fine, SEM_EINVAL, "sem_transfer: NULL or aliased vectors");
     if (prec != SEM_F64 && prec != SEM_F32) return sem_fail(fine, SEM_EINVAL, "sem_transfer: bad sem_prec");
     if (dir != SEM_PROLONG && dir != SEM_RESTRICT) return sem_fail(fine, SEM_EINVAL, "sem_transfer: bad direction");
-    if (!fine->d_J) SEM_CUDA_OK(fine, cudaMalloc((void**)&fine->d_J, sizeof(double) * SEM_MAXP * SEM_MAXP));
+    if (!fine->d_J) SEM_CUDA_OK(fine, cudaMalloc((void**)&fine->d_J, J_SLOT_BYTES * (2 * SEM_MAXP + 2)));
     double Jh[SEM_MAXP * SEM_MAXP];
     interp_matrix(coarse, fine, Jh);
     if (prec == SEM_F64) return launch<double>(fine, coarse->p, Jh, in, out, dir == SEM_RESTRICT, in_minus, wt);

@@ -92,6 +92,50 @@ def test_fdm_setup_host_matches_the_oracle_eigen_decomposition(built_lib):
         assert np.max(np.abs(u_lib - u_orc)) <= 1e-11 * np.max(np.abs(u_orc))
 
 
+def test_fdm_setup_dense_spd_pairs(built_lib):
+    """The seeded pairs above have a DIAGONAL mass matrix and a tridiagonal stiffness matrix; here both are dense SPD
+    (random orthogonal basis, seeded spectrum), m = 2 ... 16, so the Cholesky factor's off-diagonal code and the
+    congruence transform are exercised: S^T B S = I, S^T A S = diag(lambda) ascending, lambda equal to scipy's generalised
+    eigenvalues, and Eq. (3) with the library's (S, Lambda^-1) inverts the dense Kronecker-sum operator."""
+    import numpy as np
+    import scipy.linalg
+    import oracle
+    from paper_2110_01716_b200 import binding, inputs
+
+    def spd(m, seed, lo, hi):
+        Q, _ = np.linalg.qr(2.0 * inputs.hash_uniform01(seed, 3, np.arange(m * m)).reshape(m, m) - 1.0)
+        ev = lo + (hi - lo) * inputs.hash_uniform01(seed, 4, np.arange(m))
+        return (Q * ev) @ Q.T
+
+    for m in range(2, 17):
+        E = 3
+        A = np.empty((E, 3, m, m))
+        B = np.empty((E, 3, m, m))
+        for e in range(E):
+            for d in range(3):
+                A[e, d] = spd(m, 1000 * m + 10 * e + d, 0.5, 40.0)
+                B[e, d] = spd(m, 7000 * m + 10 * e + d, 0.2, 3.0)
+        S, invL = binding.fdm_setup(A, B)
+        for e in range(E):
+            lam = []
+            for d in range(3):
+                ref = scipy.linalg.eigh(A[e, d], B[e, d], eigvals_only=True)
+                D = S[e, d].T @ A[e, d] @ S[e, d]
+                assert np.max(np.abs(S[e, d].T @ B[e, d] @ S[e, d] - np.eye(m))) <= 1e-12, (m, e, d)
+                assert np.max(np.abs(D - np.diag(np.diag(D)))) <= 1e-11 * ref[-1], (m, e, d)
+                assert np.max(np.abs(np.diag(D) - ref)) <= 1e-11 * ref[-1], (m, e, d)
+                lam.append(np.diag(D))
+            assert np.max(np.abs(invL[e] * oracle.fdm_inv_lambda(*[np.asarray(l) for l in lam])[...] ** -1 - 1.0)) <= 1e-11
+        if m <= 6:                                           # Eq. (3) inverts the dense separable operator (kron order z,y,x)
+            e = 0
+            Ax, Ay, Az = A[e]
+            Bx, By, Bz = B[e]
+            K = np.kron(Bz, np.kron(By, Ax)) + np.kron(Bz, np.kron(Ay, Bx)) + np.kron(Az, np.kron(By, Bx))
+            b = 2.0 * inputs.hash_uniform01(3, 5, np.arange(m ** 3)) - 1.0
+            u = oracle.fdm_apply(S[e:e + 1], invL[e:e + 1], b.reshape(1, m, m, m)).ravel()
+            assert np.max(np.abs(K @ u - b)) <= 1e-9 * np.max(np.abs(b)), m
+
+
 def test_fdm_setup_bad_args(built_lib):
     import numpy as np
     from paper_2110_01716_b200 import binding

@@ -175,7 +175,7 @@ def _ax_case(torch, binding, oracle_mod, mesh, variant=0, mode=0, lam=0.0, dtype
 
 
 @pytest.mark.parametrize("N", [1, 2, 3, 4, 5, 6, 7, 8, 9, 11, 13, 15])
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3])
 def test_ax_f64_all_orders(torch_cuda, binding, oracle_mod, N, variant):
     # 5*3*3 = 45 elements: not a multiple of the elements-per-block of any p (ragged tail), several blocks
     m = inputs.box_mesh(5, 3, 3, N, "random", seed=N)
@@ -202,7 +202,7 @@ def test_ax_recomputed_G(torch_cuda, binding, oracle_mod, N):
     assert _ax_case(torch_cuda, binding, oracle_mod, m, mode=1) <= TOL64
 
 
-@pytest.mark.parametrize("N,variant", [(7, 0), (7, 1), (4, 0), (3, 0)])
+@pytest.mark.parametrize("N,variant", [(7, 0), (7, 1), (7, 2), (7, 3), (4, 0), (3, 0)])
 def test_ax_helmholtz(torch_cuda, binding, oracle_mod, N, variant):
     m = inputs.box_mesh(3, 3, 3, N, "smooth")
     assert _ax_case(torch_cuda, binding, oracle_mod, m, variant=variant, lam=37.5) <= TOL64
