@@ -208,6 +208,28 @@ def cheby(G, N, maps: Maps, mask_u, b_u, x0_u, order: int, lmin: float, lmax: fl
     return x
 
 
+def cheby_pc(A, P, b_u, x0_u, order: int, lmin: float, lmax: float) -> np.ndarray:
+    """The Chebyshev semi-iteration of S23 (Saad, Alg. 12.1) with a general preconditioner application P in place of
+    diag^-1 (NEXT-2b: P = the Schwarz operator), written out in numpy:
+        theta = (lmax+lmin)/2, delta = (lmax-lmin)/2, sigma = theta/delta, rho_0 = 1/sigma
+        r = P(b - A x);  d = r/theta
+        k = 1 .. order-1:  x += d;  r -= P(A d);  rho_k = 1/(2 sigma - rho_{k-1});  d = rho_k rho_{k-1} d + (2 rho_k/delta) r
+        x += d"""
+    theta, delta = 0.5 * (lmax + lmin), 0.5 * (lmax - lmin)
+    sigma = theta / delta
+    rho = 1.0 / sigma
+    x = np.zeros_like(np.asarray(b_u, dtype=np.float64)) if x0_u is None else np.array(x0_u, dtype=np.float64)
+    r = P(b_u - A(x)) if x0_u is not None else P(np.asarray(b_u, dtype=np.float64))
+    d = r / theta
+    for _ in range(1, order):
+        x = x + d
+        r = r - P(A(d))
+        rho1 = 1.0 / (2.0 * sigma - rho)
+        d = rho1 * rho * d + (2.0 * rho1 / delta) * r
+        rho = rho1
+    return x + d
+
+
 # ---- NEXT-1c: p-multigrid V-cycle preconditioner (P:103, P:109, P:146) -------------------------------------------
 class Level:
     """One p-multigrid level: its own discretisation of order N on the same elements (S17)."""
@@ -237,7 +259,24 @@ class Level:
         return apply_Ag(self.G, self.N, self.maps, self.mask_u, x_u, self.lam)
 
     def smooth(self, b_u, x0_u, order):
+        if getattr(self, "schwarz", None) is not None:
+            return cheby_pc(self.A, self.schwarz.apply, b_u, x0_u, order, self.slmin, self.slmax)
         return cheby(self.G, self.N, self.maps, self.mask_u, b_u, x0_u, order, self.lmin, self.lmax, self.lam)
+
+    def use_schwarz(self, mesh, restricted: bool = False, lmin_frac: float = 0.1, lmax_safety: float = 1.1,
+                    power_its: int = 60):
+        """Switch this level's smoother to Chebyshev-accelerated Schwarz (NEXT-2b): bounds of S A by
+        power iteration x safety, lmin a fraction of lmax, as for Chebyshev-Jacobi (S23)."""
+        self.schwarz = Schwarz(mesh, self.maps, self.mask_u, restricted)
+        v = np.where(self.mask_u != 0, 0.0, np.cos(np.arange(self.maps.U) ** 2 * 1.7))
+        lam = 1.0
+        for _ in range(power_its):
+            w = self.schwarz.apply(self.A(v))
+            lam = float(np.linalg.norm(w) / np.linalg.norm(v))
+            v = w / np.linalg.norm(w)
+        self.slmax = lmax_safety * lam
+        self.slmin = lmin_frac * self.slmax
+        return self
 
 
 def vcycle(levels, r_u, smooth_order: int, coarse_order: int, lvl: int = 0):
@@ -377,3 +416,149 @@ def fdm_apply(S: np.ndarray, inv_lambda: np.ndarray, b: np.ndarray) -> np.ndarra
         t = np.einsum("jb,kba->kja", Sy, t)              # S_y
         u[e] = np.einsum("ia,kja->kji", Sx, t)           # S_x
     return u
+
+
+# ---- NEXT-2b: overlapping additive Schwarz smoother around Eq. (3) (reading S29 in DESIGN.md) ---------------
+# P:103 "The Schwarz smoothers are implemented by solving local Poisson problems on domains extended into adjacent elements
+# by one layer.  Thus, for an 8 x 8 x 8 brick (N = 7), one solves a 10 x 10 x 10 local problem"; "We exchange
+# face data only to get the domain extensions -- meaning 6 exchanges per element instead of 26 ... a restricted additive
+# Schwarz (RAS) variant, that does not require communication after the local solve".  The paper cites Lottes & Fischer
+# (2005) for the construction and prints none of it; what is written out below is reading S29:
+#   * extended block of element e: m = N + 3 points per direction; index 1..N+1 = the element's own nodes, index 0 and
+#     m-1 = the face neighbour's node ONE LAYER IN from the shared face; only the 6 face layers are filled ("face data
+#     only"), the edge and corner positions of the block hold no node (right-hand side 0, nothing scattered back);
+#   * local operator  A~ = Bz x By x Ax + Bz x Ay x Bx + Az x By x Bx  from 1-D stiffness/mass pairs on the extended
+#     line [left neighbour | element | right neighbour]: the 1-D spectral-element matrices (2/L) D^T diag(rho) D and
+#     (L/2) diag(rho) of the three segments assembled, and the rows/columns of the m retained nodes kept (all other
+#     nodes of the neighbours held at zero).  L = mean length of the element's 4 edges in that local direction;
+#   * where there is no neighbour the ghost point is decoupled (unit row, zero right-hand side); on a Dirichlet face the
+#     face node is decoupled as well;
+#   * z = W^1/2 sum_e R_e^T A~_e^-1 R_e (W^1/2 r) with W = 1 / (number of block positions that map to the node), then the
+#     Dirichlet mask: the weighting is split over both sides so that S stays symmetric positive definite (S A then has a
+#     real positive spectrum, which the Chebyshev acceleration and the CG outer iteration assume); RAS: only the
+#     element's own nodes are scattered back, z = W sum_e R^_e^T A~_e^-1 R_e r with W = 1 / multiplicity (not symmetric).
+def schwarz_lengths(vert: np.ndarray) -> np.ndarray:
+    """L[e][d], d = r, s, t: mean length of the 4 edges of the trilinear element that run in local direction d
+    (vertex v = a + 2b + 4c: the edges of direction d join v and v + 2^d for the 4 vertices v whose bit d is 0)."""
+    v = _f64(vert).reshape(-1, 8, 3)
+    L = np.empty((v.shape[0], 3))
+    for d in range(3):
+        starts = [q for q in range(8) if not (q >> d) & 1]
+        L[:, d] = np.mean([np.linalg.norm(v[:, q + (1 << d)] - v[:, q], axis=1) for q in starts], axis=0)
+    return L
+
+
+def schwarz_ops_1d(N: int, Lm: float, Ll, Lr, dirichlet_l: bool, dirichlet_r: bool):
+    """(A, B), each m x m with m = N + 3, of one element's extended line (reading S29).  Lm = the element's length,
+    Ll / Lr = the left / right neighbour's length in the direction normal to the shared face (None: no neighbour, then
+    dirichlet_l / dirichlet_r says whether that end face is a Dirichlet face)."""
+    _, rho, D = gll(N)
+    Kh = D.T @ np.diag(rho) @ D                           # reference 1-D stiffness on [-1, 1]
+    m = N + 3
+    A = np.zeros((m, m))
+    B = np.zeros(m)
+    A[1:N + 2, 1:N + 2] += (2.0 / Lm) * Kh                # the element itself: block positions 1 .. N+1
+    B[1:N + 2] += (Lm / 2.0) * rho
+    if Ll is not None:                                    # left neighbour: its last two nodes (one-in, shared face)
+        A[0:2, 0:2] += (2.0 / Ll) * Kh[N - 1:N + 1, N - 1:N + 1]
+        B[0:2] += (Ll / 2.0) * rho[N - 1:N + 1]
+    else:
+        A[0, 0], B[0] = 1.0, 1.0                          # no ghost point: decoupled unit row
+        if dirichlet_l:
+            A[1, :] = 0.0
+            A[:, 1] = 0.0
+            A[1, 1], B[1] = 1.0, 1.0
+    if Lr is not None:                                    # right neighbour: its first two nodes (shared face, one-in)
+        A[m - 2:m, m - 2:m] += (2.0 / Lr) * Kh[0:2, 0:2]
+        B[m - 2:m] += (Lr / 2.0) * rho[0:2]
+    else:
+        A[m - 1, m - 1], B[m - 1] = 1.0, 1.0
+        if dirichlet_r:
+            A[m - 2, :] = 0.0
+            A[:, m - 2] = 0.0
+            A[m - 2, m - 2], B[m - 2] = 1.0, 1.0
+    return A, np.diag(B)
+
+
+class Schwarz:
+    """The additive Schwarz smoother z = S r of one level (unique-node storage), reading S29.
+    R[e][c][b][a] = unique node behind position (a, b, c) of element e's extended block, -1 where there is none."""
+
+    def __init__(self, mesh, maps: Maps, mask_u: np.ndarray, restricted: bool = False):
+        N, p, E = mesh.N, mesh.N + 1, mesh.vert.shape[0]
+        assert N >= 2, "a face needs an interior node to identify the face neighbour"
+        m, p3 = N + 3, p ** 3
+        self.N, self.m, self.maps, self.mask_u, self.restricted = N, m, maps, np.asarray(mask_u), restricted
+        gid = np.ascontiguousarray(mesh.gid, dtype=np.int64).reshape(E, p, p, p)            # [e][k][j][i]
+        l2u = maps.l2u.reshape(E, p, p, p)
+        L = schwarz_lengths(mesh.vert)
+        order = np.argsort(gid.reshape(E, p3), axis=1, kind="stable")                       # per element: gid -> local index
+        sorted_gid = np.take_along_axis(gid.reshape(E, p3), order, axis=1)
+        R = -np.ones((E, m, m, m), dtype=np.int64)
+        R[:, 1:p + 1, 1:p + 1, 1:p + 1] = l2u
+        self.nbr = -np.ones((E, 6), dtype=np.int64)
+        Lnb = [[None] * 6 for _ in range(E)]
+        dirf = np.zeros((E, 6), dtype=bool)
+        c0 = p // 2                                                                           # a face-interior node
+        for e in range(E):
+            for f in range(6):
+                axis, side = f // 2, f % 2                                                    # axis 0/1/2 = i/j/k; side 0: index 0, 1: index N
+                sl = [slice(None)] * 3                                                        # [k][j][i] slices of my face
+                sl[2 - axis] = 0 if side == 0 else N
+                fg = gid[e][tuple(sl)]                                                        # [p][p] gids of my face nodes
+                ctr = l2u[e][tuple(sl)][c0, c0]
+                copies = maps.seg_idx[maps.seg_off[ctr]:maps.seg_off[ctr + 1]] // p3
+                others = [int(x) for x in copies if x != e]
+                if len(others) != 1:                                                          # domain boundary
+                    dirf[e, f] = self.mask_u[ctr] != 0
+                    continue
+                n = others[0]
+                self.nbr[e, f] = n
+                pos = np.searchsorted(sorted_gid[n], fg.ravel())
+                assert np.array_equal(sorted_gid[n][pos], fg.ravel()), "face nodes not found in the neighbour"
+                ln = order[n][pos]                                                            # neighbour's local indices of my face nodes
+                ci, cj, ck = ln % p, (ln // p) % p, ln // (p * p)
+                coords = [ci, cj, ck]
+                naxis = [a for a in range(3) if np.all(coords[a] == coords[a][0]) and coords[a][0] in (0, N)]
+                assert len(naxis) == 1
+                na = naxis[0]
+                coords[na] = np.where(coords[na] == 0, 1, N - 1)                              # one layer in
+                one_in = l2u[n].ravel()[coords[0] + p * (coords[1] + p * coords[2])].reshape(fg.shape)
+                Lnb[e][f] = L[n, na]
+                gl = [slice(1, p + 1)] * 3                                                    # my ghost layer in the block
+                gl[2 - axis] = 0 if side == 0 else m - 1
+                R[e][tuple(gl)] = one_in
+        self.R = R
+        # 1-D operator pairs, their eigen-decompositions (Eq. (3)) per element and direction
+        self.A1 = np.empty((E, 3, m, m))
+        self.B1 = np.empty((E, 3, m, m))
+        self.S = np.empty((E, 3, m, m))
+        self.invL = np.empty((E, m, m, m))
+        for e in range(E):
+            lam = []
+            for d in range(3):
+                self.A1[e, d], self.B1[e, d] = schwarz_ops_1d(N, L[e, d], Lnb[e][2 * d], Lnb[e][2 * d + 1],
+                                                              bool(dirf[e, 2 * d]), bool(dirf[e, 2 * d + 1]))
+                self.S[e, d], l = fdm_eig(self.A1[e, d], self.B1[e, d])
+                lam.append(l)
+            tot = lam[2][:, None, None] + lam[1][None, :, None] + lam[0][None, None, :]
+            self.invL[e] = np.where(tot > 1e-12 * tot.max(), 1.0 / np.where(tot > 0, tot, 1.0), 0.0)   # all-Neumann block
+        own = np.zeros((m, m, m), dtype=bool)
+        own[1:p + 1, 1:p + 1, 1:p + 1] = True
+        self.back = (R >= 0) & (own[None] if restricted else True)                            # positions scattered back
+        cnt = np.zeros(maps.U)
+        np.add.at(cnt, R[self.back], 1.0)
+        self.W = 1.0 / cnt
+
+    def extended_rhs(self, r_u):
+        return np.where(self.R >= 0, np.asarray(r_u)[np.maximum(self.R, 0)], 0.0)
+
+    def apply(self, r_u):
+        pre = np.ones(self.maps.U) if self.restricted else np.sqrt(self.W)
+        post = self.W if self.restricted else np.sqrt(self.W)
+        u = fdm_apply(self.S, self.invL, self.extended_rhs(pre * np.asarray(r_u)))
+        z = np.zeros(self.maps.U)
+        np.add.at(z, self.R[self.back], u[self.back])
+        z *= post
+        z[self.mask_u != 0] = 0.0
+        return z

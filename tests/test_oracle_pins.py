@@ -765,3 +765,146 @@ def test_F3_fdm_is_symmetric_positive_definite_on_the_synthetic_pairs(oracle_mod
         K = (np.kron(B[e, 2], np.kron(B[e, 1], A[e, 0])) + np.kron(B[e, 2], np.kron(A[e, 1], B[e, 0]))
              + np.kron(A[e, 2], np.kron(B[e, 1], B[e, 0])))
         assert np.max(np.abs(K @ Fb[e].ravel() - b[e].ravel())) <= 1e-10 * np.max(np.abs(b[e]))
+
+
+# ---------------------------------------- NEXT-2b: overlapping additive Schwarz smoother (reading S29)
+def _rectilinear(nx, ny, nz, N, stretch):
+    """An affine box mesh whose grid lines are moved by x -> x^stretch per coordinate: elements stay rectangular
+    boxes but neighbouring elements have different lengths."""
+    m = inputs.box_mesh(nx, ny, nz, N, "affine")
+    m.vert = m.vert ** np.asarray(stretch)[None, None, :]
+    return m
+
+
+def _window_ids(mesh, ex, ey, ez):
+    """Unique-grid (positional gid) ids of the (N+3)^3 tensor window around element (ex, ey, ez): -1 outside the mesh."""
+    N = mesh.N
+    NX, NY, NZ = mesh.nx * N + 1, mesh.ny * N + 1, mesh.nz * N + 1
+    ids = -np.ones((N + 3, N + 3, N + 3), dtype=np.int64)
+    for c in range(N + 3):
+        for b in range(N + 3):
+            for a in range(N + 3):
+                x, y, z = ex * N - 1 + a, ey * N - 1 + b, ez * N - 1 + c
+                if 0 <= x < NX and 0 <= y < NY and 0 <= z < NZ:
+                    ids[c, b, a] = x + NX * (y + NY * z)
+    return ids
+
+
+@pytest.mark.parametrize("stretch", [(1.0, 1.0, 1.0), (1.6, 0.7, 1.3)])
+def test_W1_local_operator_is_the_assembled_operator_on_the_window(oracle_mod, stretch):
+    """On a rectilinear mesh the assembled operator is a sum of Kronecker products of the 1-D assembled matrices, so its
+    restriction to the tensor window of (N+3)^3 nodes around an element IS Bz x By x Ax + ... with the 1-D matrices
+    restricted to the window: the separable local operator of the Schwarz block (reading S29: three assembled 1-D segments,
+    retained rows and columns) must equal rows/columns of the dense assembled operator, which is pinned by P9 and shares
+    no code with it.  A wrong neighbour length, a wrong corner block of the neighbour's 1-D matrix, a swapped Kronecker
+    order or a transposed direction fails.  Interior element (all 6 neighbours) and, with the Dirichlet mask, a corner
+    element (3 boundary faces: decoupled ghost and face rows)."""
+    N = 3
+    m = _rectilinear(3, 3, 3, N, stretch)
+    for masked, (ex, ey, ez) in ((False, (1, 1, 1)), (True, (0, 2, 0)), (False, (2, 0, 1))):
+        maps = oracle_mod.Maps(m.gid)
+        mask_u = oracle_mod.mask_unique(m.dirichlet, maps) if masked else np.zeros(maps.U, np.uint8)
+        sw = oracle_mod.Schwarz(m, maps, mask_u)
+        G, _, rc = oracle_mod.geom_trilinear(m.vert, N)
+        assert rc == 0
+        Ad = np.stack([oracle_mod.apply_Ag(G, N, maps, mask_u, e) for e in np.eye(maps.U)], axis=1)
+        e = ex + 3 * (ey + 3 * ez)
+        (Ax, Ay, Az), (Bx, By, Bz) = sw.A1[e], sw.B1[e]
+        K = np.kron(Bz, np.kron(By, Ax)) + np.kron(Bz, np.kron(Ay, Bx)) + np.kron(Az, np.kron(By, Bx))
+        ids = _window_ids(m, ex, ey, ez).ravel()
+        live = ids >= 0
+        u_of = np.searchsorted(maps.uniq_gid, np.maximum(ids, 0))
+        live &= mask_u[u_of] == 0                               # Dirichlet nodes are decoupled unit rows in the block
+        Aw = Ad[np.ix_(u_of[live], u_of[live])]
+        assert np.max(np.abs(K[np.ix_(live, live)] - Aw)) <= 1e-13 * np.max(np.abs(Aw)), (stretch, masked)
+        dead = ~live                                            # positions without a node: decoupled from the live ones
+        assert not dead.any() or np.max(np.abs(K[np.ix_(live, dead)])) == 0.0
+        # the block's node map: every filled position points at the window's node; face layers only
+        R = sw.R[e].ravel()
+        assert np.array_equal(R[R >= 0], u_of[R >= 0])
+        nfaces = int((sw.nbr[e] >= 0).sum())
+        assert int((R >= 0).sum()) == (N + 1) ** 3 + nfaces * (N + 1) ** 2
+
+
+def test_W2_schwarz_is_symmetric_positive_and_better_conditioned_than_jacobi(oracle_mod):
+    """sum_e R_e^T A~_e^-1 R_e is symmetric positive definite on the free nodes (every A~_e^-1 is, and the blocks cover
+    every node) and so is S = W^1/2 M W^1/2; S A has a real positive spectrum, and on a deformed mesh its condition number is far below that
+    of diag^-1 A (why the paper uses it as the pMG smoother).  The weights are 1 / (positions per node):
+    their reciprocals add up to the number of filled block positions, p^3 + (#face neighbours) p^2 per element."""
+    m = inputs.box_mesh(3, 3, 2, 4, "smooth", amp=0.03)
+    L = oracle_mod.Level(m)
+    sw = oracle_mod.Schwarz(m, L.maps, L.mask_u)
+    free = L.mask_u == 0
+    n = L.maps.U
+    p = m.N + 1
+
+    def unweighted(r):
+        u = oracle_mod.fdm_apply(sw.S, sw.invL, sw.extended_rhs(r))
+        z = np.zeros(n)
+        np.add.at(z, sw.R[sw.back], u[sw.back])
+        return z
+    M = _dense_of(unweighted, n)[np.ix_(free, free)]
+    assert np.max(np.abs(M - M.T)) <= 1e-12 * np.max(np.abs(M))
+    assert np.linalg.eigvalsh(0.5 * (M + M.T)).min() > 0.0
+    A = _dense_of(L.A, n)[np.ix_(free, free)]
+    S = _dense_of(lambda r: sw.apply(np.where(free, r, 0.0)), n)[np.ix_(free, free)]
+    assert np.max(np.abs(S - S.T)) <= 1e-12 * np.max(np.abs(S))
+    Wh = np.sqrt(sw.W[free])
+    assert np.max(np.abs(S - Wh[:, None] * M * Wh[None, :])) <= 1e-12 * np.max(np.abs(S))
+    Lc = np.linalg.cholesky(A)
+    ev = np.linalg.eigvalsh(Lc.T @ S @ Lc)                    # = spectrum of S A (similar), real because S, A are SPD
+    assert ev.min() > 0.0
+    evj = np.linalg.eigvals(np.diag(L.Minv[free]) @ A).real
+    assert ev.max() / ev.min() < 0.5 * evj.max() / evj.min()
+    assert round(float(np.sum(1.0 / sw.W))) == sum(p ** 3 + int((sw.nbr[e] >= 0).sum()) * p * p for e in range(m.E))
+    # masked nodes come out zero; RAS: own nodes only, weights 1 / multiplicity
+    z = sw.apply(np.where(free, np.cos(np.arange(n)), 0.0))
+    assert np.all(z[~free] == 0.0)
+    ras = oracle_mod.Schwarz(m, L.maps, L.mask_u, restricted=True)
+    assert np.max(np.abs(ras.W * L.maps.mult - 1.0)) == 0.0
+
+
+def test_W3_one_affine_element_is_solved_exactly(oracle_mod):
+    """One affine element with homogeneous Dirichlet faces: no neighbour, the block is the element, the separable operator
+    is the element's own (P7), so S is the exact inverse on the interior nodes: S A x = x.  (A wrong boundary row, weight
+    or eigen-index order fails.)  Also with a different length per direction."""
+    for scale in ((1.0, 1.0, 1.0), (0.5, 2.0, 1.25)):
+        m = inputs.box_mesh(1, 1, 1, 5, "affine")
+        m.vert = m.vert * np.asarray(scale)[None, None, :]
+        L = oracle_mod.Level(m, power_its=2)
+        sw = oracle_mod.Schwarz(m, L.maps, L.mask_u)
+        free = L.mask_u == 0
+        x = np.where(free, np.sin(1.0 + np.arange(L.maps.U) ** 2), 0.0)
+        assert np.max(np.abs(sw.apply(L.A(x)) - x)) <= 1e-11 * np.max(np.abs(x)), scale
+
+
+def test_W4_chebyshev_with_a_general_preconditioner_reduces_to_chebyshev_jacobi(oracle_mod, pmg_levels):
+    """cheby_pc (numpy, any preconditioner) with P = diag^-1 reproduces the C++ oracle's Chebyshev-Jacobi smoother, which
+    C1 pins against the exact error polynomial."""
+    L0 = pmg_levels[0]
+    b = L0.A(np.where(L0.mask_u != 0, 0.0, np.cos(np.arange(L0.maps.U) * 0.37)))
+    x0 = np.where(L0.mask_u != 0, 0.0, np.sin(np.arange(L0.maps.U) * 0.11))
+    for order, guess in ((1, None), (3, None), (4, x0)):
+        ref = L0.smooth(b, guess, order)
+        got = oracle_mod.cheby_pc(L0.A, lambda r: L0.Minv * r, b, guess, order, L0.lmin, L0.lmax)
+        assert np.max(np.abs(got - ref)) <= 1e-12 * np.max(np.abs(ref)), order
+
+
+def test_W5_schwarz_smoothing_beats_jacobi_smoothing_in_the_vcycle(oracle_mod):
+    """The same V-cycle and flexible PCG with Chebyshev-Schwarz smoothing on the levels that can carry it needs fewer
+    iterations than with Chebyshev-Jacobi smoothing ("we switched from Chebyshev-Jacobi to Chebyshev-Schwarz") and
+    reaches the same (dense direct) solution."""
+    meshes = [inputs.box_mesh(3, 3, 2, N, "smooth") for N in (5, 3, 1)]
+    lj = [oracle_mod.Level(m) for m in meshes]
+    ls = [oracle_mod.Level(m) for m in meshes]
+    for L, m in zip(ls[:-1], meshes[:-1]):
+        L.use_schwarz(m)
+    L0 = lj[0]
+    free = L0.mask_u == 0
+    rng = np.random.default_rng(4)
+    xs = np.where(free, rng.standard_normal(L0.maps.U), 0.0)
+    b = L0.A(xs)
+    rj = oracle_mod.fpcg(lj[0], lambda r: oracle_mod.vcycle(lj, r, 2, 8), b, tol=1e-10, maxit=60)
+    rs = oracle_mod.fpcg(ls[0], lambda r: oracle_mod.vcycle(ls, r, 2, 8), b, tol=1e-10, maxit=60)
+    assert rs["hist"][-1] <= 1e-10 and rs["iters"] < rj["iters"]
+    assert np.max(np.abs(rs["x"] - xs)) <= 1e-8 * np.max(np.abs(xs))
