@@ -651,10 +651,33 @@ def main():
             with binding.Pmg(lv, [0.1 * l for l in lam], lam, 2, 8, binding.SEM_F32) as mg:
                 mg.fpcg(rhs, x, 1e-8, 3)                 # warm-up: allocations, graph capture
                 (it_m, rel_m), ms_m = wall(lambda: mg.fpcg(rhs, x, 1e-8, 200))
+                # NEXT-2b: the same cycle with Chebyshev-accelerated overlapping Schwarz smoothing on N = 7 and N = 3
+                t0 = time.perf_counter()
+                for s_ in lv[:2]:
+                    s_.schwarz_setup()
+                ms_setup = (time.perf_counter() - t0) * 1e3
+                lams = [1.1 * lv[0].lambda_max_schwarz(0, 30), 1.1 * lv[1].lambda_max_schwarz(0, 30), lam[2]]
+                mg.set_smoother(binding.SEM_SMOOTH_CHEBY_SCHWARZ, [0.1 * l for l in lams], lams)
+                mg.fpcg(rhs, x, 1e-8, 3)
+                (it_s, rel_s), ms_s = wall(lambda: mg.fpcg(rhs, x, 1e-8, 200))
+            r32 = rhs.float()
+            z32 = torch.empty_like(r32)
+            us_sw = event_time_us(torch, lambda: lv[0].schwarz(r32, z32), 300)
+            us_ras = event_time_us(torch, lambda: lv[0].schwarz(r32, z32, binding.SEM_SCHWARZ_RAS), 300)
             lv[0].pcg(rhs, x.zero_(), 1e-8, 20)
             (it_j, rel_j), ms_j = wall(lambda: lv[0].pcg(rhs, x.zero_(), 1e-8, 5000))
-            solve = {"tol": 1e-8, "levels": "N = 7-3-1, Chebyshev-Jacobi order 2, FP32 V-cycle, FP64 flexible PCG",
-                     "pmg_fcg": {"iters": it_m, "relres": rel_m, "ms": ms_m},
+            m10 = mesh.N + 3
+            # algorithmic bytes of one Schwarz application, FP32: read r (4), write + read the block b~ around Eq. (3)
+            # (2 x 4 m^3/p^3), Lambda^-1 and S, write + read-modify-write z (gs counted as 8 S/nL)
+            sw_bytes = 4.0 * (nL + mesh.E * (5 * m10 ** 3 + 3 * m10 * m10) + nL) + 8.0 * S
+            solve = {"tol": 1e-8, "levels": "N = 7-3-1, smoother order 2, FP32 V-cycle, FP64 flexible PCG",
+                     "pmg_fcg": {"smoother": "Chebyshev-Jacobi", "iters": it_m, "relres": rel_m, "ms": ms_m},
+                     "pmg_fcg_schwarz": {"smoother": "Chebyshev-accelerated additive Schwarz (NEXT-2b) on N = 7, 3",
+                                         "iters": it_s, "relres": rel_s, "ms": ms_s, "setup_ms": ms_setup},
+                     "schwarz_apply_f32": {"us_asm": us_sw, "us_ras": us_ras, "algorithmic_GBs": sw_bytes / us_sw / 1e3,
+                                           "frac_of_measured_hbm_peak": sw_bytes / us_sw / 1e3 / peak,
+                                           "what": "sem_schwarz at E = 7200, N = 7 (10^3 blocks): extension gather, "
+                                                   "Eq. (3), weighted combination, gather-scatter"},
                      "jacobi_pcg": {"iters": it_j, "relres": rel_j, "ms": ms_j}}
             for s_ in lv:
                 s_.close()

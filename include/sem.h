@@ -222,6 +222,48 @@ SEM_API int sem_fdm_apply(sem_ctx* ctx, int m, const void* S, const void* inv_la
  * m outside 2..16 or a B_d that is not positive definite. */
 SEM_API int sem_fdm_setup(int64_t E, int m, const double* A, const double* B, double* S, double* inv_lambda);
 
+/* NEXT-2b.  The overlapping additive Schwarz smoother around sem_fdm_apply ("The Schwarz smoothers
+ * are implemented by solving local Poisson problems on domains extended into adjacent elements by one layer"
+ * "We exchange face data only to get the domain extensions -- meaning 6 exchanges per element instead of 26", the
+ * restricted variant "that does not require communication after the local solve"; Table 2 `gs_ext`, `fdm`, `fdm_apply`).
+ * The paper cites Lottes & Fischer (2005) and prints no formula; the construction is reading S29 of DESIGN.md:
+ *   block of element e: m = N + 3 points per direction: index 1..N+1 its own nodes, index 0 / m-1 the face neighbour's
+ *     node one layer in from the shared face; only the 6 face layers are filled, block edges and corners hold no node;
+ *   A~_e = Bz x By x Ax + Bz x Ay x Bx + Az x By x Bx from the 1-D pairs of the line [left | element | right]: the 1-D
+ *     spectral-element matrices (2/L) D^T diag(rho) D, (L/2) diag(rho) of the three segments assembled and the m retained
+ *     rows/columns kept; L = mean length of the element's 4 edges in that local direction; without a neighbour the ghost
+ *     point is a decoupled unit row, on a Dirichlet face the face node too;
+ *   z = M W^1/2 QQ^T sum_e R_e^T A~_e^-1 R_e (W^1/2 r),  W = 1 / (block positions mapping to the node), split over both
+ *     sides so that S is symmetric positive definite; SEM_SCHWARZ_RAS scatters back the element's own nodes only and
+ *     weights the result by W = 1 / multiplicity (not symmetric).
+ * sem_schwarz_setup (after sem_geom; N >= 2, else SEM_EINVAL; synchronises; host work O(E)): finds the face neighbours
+ * from the gather-scatter maps, builds the 1-D pairs, their eigen-decompositions (as sem_fdm_setup) in FP64 and FP32, and
+ * both weight vectors.  sem_geom discards it.  SEM_EMESH if a shared face cannot be matched node for node.
+ * sem_schwarz: r, z DEVICE, local layout, continuous, `prec` values, r assembled; z may alias r.  Three element-local
+ * kernels (extension gather, Eq. (3) in place, weighted combination) and the gather-scatter with the Dirichlet mask;
+ * asynchronous on the context's stream.  SEM_ESTATE before sem_schwarz_setup.
+ * sem_get_schwarz (parity accessor, HOST buffers, any may be NULL): nbr [E][6] (face f = 2 axis + side; -1 = boundary),
+ * A, B [E][3][m][m] the 1-D pairs, W [E][p^3] the weight vector of `kind` as applied (ASM: W^1/2; RAS: W). */
+typedef enum { SEM_SCHWARZ_ASM = 0, SEM_SCHWARZ_RAS = 1 } sem_schwarz_kind;
+SEM_API int sem_schwarz_setup(sem_ctx* ctx);
+SEM_API int sem_schwarz(sem_ctx* ctx, const void* r, void* z, sem_prec prec, sem_schwarz_kind kind);
+SEM_API int sem_get_schwarz(sem_ctx* ctx, int32_t* nbr, double* A, double* B, double* W, sem_schwarz_kind kind);
+
+/* Chebyshev-accelerated Schwarz ("Chebyshev-accelerated overlapping Schwarz"; "we switched from
+ * Chebyshev-Jacobi to Chebyshev-Schwarz"): the recurrence of sem_cheby with the Schwarz operator S in place of diag^-1,
+ * for bounds [lmin, lmax] of S A given by the caller (sem_lambda_max_schwarz).  Arguments as sem_cheby. */
+SEM_API int sem_cheby_schwarz(sem_ctx* ctx, const void* b, void* x, int order, double lmin, double lmax, int zero_guess,
+                              sem_prec prec, sem_schwarz_kind kind);
+/* `iters` power iterations on S A (FP64, synchronises): the last estimate ||S A v|| / ||v||, as sem_lambda_max. */
+SEM_API int sem_lambda_max_schwarz(sem_ctx* ctx, sem_schwarz_kind kind, int iters, double* lam_out);
+
+/* Smoother of a sem_pmg (default SEM_SMOOTH_CHEBY_JACOBI).  With SEM_SMOOTH_CHEBY_SCHWARZ / _RAS every level with N >= 2
+ * is smoothed by sem_cheby_schwarz of `smooth_order` steps (sem_schwarz_setup is run on it if needed) with the bounds
+ * given here; levels with N = 1 and the coarsest level keep Chebyshev-Jacobi with the bounds of sem_pmg_create.
+ *   lmin, lmax  HOST [nlevels], bounds of S A per level (ignored where Jacobi stays).  Drops recorded graphs. */
+typedef enum { SEM_SMOOTH_CHEBY_JACOBI = 0, SEM_SMOOTH_CHEBY_SCHWARZ = 1, SEM_SMOOTH_CHEBY_RAS = 2 } sem_smoother;
+SEM_API int sem_pmg_set_smoother(sem_pmg* mg, sem_smoother smoother, const double* lmin, const double* lmax);
+
 /* Measurement helper ("FP64 peak ... measure it"): a register-resident arithmetic microbenchmark on
  * the current device, best of 5 launches after one warm-up, CUDA-event timed on `cuda_stream`; synchronises.  Not part
  * of the method: bench.py quotes the FP64-ALU-bound kernels (a9 recomputed G, the fast-diagonalisation solve) against it.

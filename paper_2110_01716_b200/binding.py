@@ -18,6 +18,8 @@ SEM_F64, SEM_F32 = 0, 1
 SEM_OP_ADD = 0
 SEM_G_STORED, SEM_G_RECOMPUTE = 0, 1
 SEM_PROLONG, SEM_RESTRICT = 0, 1
+SEM_SCHWARZ_ASM, SEM_SCHWARZ_RAS = 0, 1
+SEM_SMOOTH_CHEBY_JACOBI, SEM_SMOOTH_CHEBY_SCHWARZ, SEM_SMOOTH_CHEBY_RAS = 0, 1, 2
 SEM_OK, SEM_EINVAL, SEM_EMESH, SEM_ECUDA, SEM_ENOMEM, SEM_ESTATE = 0, -1, -2, -3, -4, -5
 _ERRNAME = {-1: "SEM_EINVAL", -2: "SEM_EMESH", -3: "SEM_ECUDA", -4: "SEM_ENOMEM", -5: "SEM_ESTATE"}
 
@@ -56,6 +58,12 @@ SYMBOLS = {
     "sem_fdm_apply": (_i32, [_vp, _i32, _vp, _vp, _vp, _vp, _i32]),
     "sem_fdm_setup": (_i32, [_i64, _i32, _vp, _vp, _vp, _vp]),
     "sem_measure_peak": (_i32, [_i32, _vp, C.POINTER(_dbl)]),
+    "sem_schwarz_setup": (_i32, [_vp]),
+    "sem_schwarz": (_i32, [_vp, _vp, _vp, _i32, _i32]),
+    "sem_get_schwarz": (_i32, [_vp, _vp, _vp, _vp, _vp, _i32]),
+    "sem_cheby_schwarz": (_i32, [_vp, _vp, _vp, _i32, _dbl, _dbl, _i32, _i32, _i32]),
+    "sem_lambda_max_schwarz": (_i32, [_vp, _i32, _i32, C.POINTER(_dbl)]),
+    "sem_pmg_set_smoother": (_i32, [_vp, _i32, C.POINTER(_dbl), C.POINTER(_dbl)]),
     "sem_last_error": (C.c_char_p, [_vp]),
     "sem_ctx_destroy": (None, [_vp]),
 }
@@ -261,6 +269,35 @@ class Sem:
     def set_variant(self, v: int):
         self._check(self._L.sem_set_variant(self._h, v))
 
+    # ---- NEXT-2b: overlapping Schwarz smoother ----
+    def schwarz_setup(self):
+        self._check(self._L.sem_schwarz_setup(self._h))
+        return self
+
+    def schwarz(self, r, z, kind: int = SEM_SCHWARZ_ASM):
+        self._check(self._L.sem_schwarz(self._h, self._vec(r), self._vec(z), self._prec(r), kind))
+        return z
+
+    def get_schwarz(self, kind: int = SEM_SCHWARZ_ASM):
+        """(nbr[E][6], A[E][3][m][m], B[E][3][m][m], W[E][p^3]) of the Schwarz smoother (parity accessor)."""
+        m = self.p + 2
+        nbr = np.empty((self.E, 6), np.int32)
+        A, B = np.empty((self.E, 3, m, m)), np.empty((self.E, 3, m, m))
+        W = np.empty((self.E, self.p ** 3))
+        self._check(self._L.sem_get_schwarz(self._h, _np_ptr(nbr), _np_ptr(A), _np_ptr(B), _np_ptr(W), kind))
+        return nbr, A, B, W
+
+    def cheby_schwarz(self, b, x, order: int, lmin: float, lmax: float, zero_guess: bool = False,
+                      kind: int = SEM_SCHWARZ_ASM):
+        self._check(self._L.sem_cheby_schwarz(self._h, self._vec(b), self._vec(x), order, lmin, lmax, int(zero_guess),
+                                              self._prec(x), kind))
+        return x
+
+    def lambda_max_schwarz(self, kind: int = SEM_SCHWARZ_ASM, iters: int = 30) -> float:
+        lam = C.c_double(0.0)
+        self._check(self._L.sem_lambda_max_schwarz(self._h, kind, iters, C.byref(lam)))
+        return lam.value
+
     def pcg_history(self, n: int) -> np.ndarray:
         h = np.full(n, np.nan)
         self._check(self._L.sem_get_pcg_history(self._h, _np_ptr(h), n))
@@ -313,6 +350,15 @@ class Pmg:
         if rc != SEM_OK:
             raise SemError(rc, "; ".join(self._L.sem_last_error(lv._h).decode() for lv in self.levels))
         self._h = h
+
+    def set_smoother(self, smoother: int, lmin=None, lmax=None):
+        n = len(self.levels)
+        lo = (C.c_double * n)(*lmin) if lmin is not None else None
+        hi = (C.c_double * n)(*lmax) if lmax is not None else None
+        rc = self._L.sem_pmg_set_smoother(self._h, smoother, lo, hi)
+        if rc != SEM_OK:
+            raise SemError(rc, "; ".join(self._L.sem_last_error(lv._h).decode() for lv in self.levels))
+        return self
 
     def vcycle(self, r, z):
         rc = self._L.sem_pmg_vcycle(self._h, C.c_void_p(r.data_ptr()), C.c_void_p(z.data_ptr()))

@@ -105,13 +105,83 @@ int run(sem_ctx* c, const T* b, T* x, int order, double lmin, double lmax, bool 
     return SEM_OK;
 }
 
+// ---- the same recurrence with the Schwarz operator S (sem_schwarz.cu) in place of diag^-1: r and w hold S-applied
+// vectors, so the vector kernels carry no Minv ----
+// r = b - q (q == nullptr: r = b)
+template <typename T>
+__global__ void __launch_bounds__(256) k_pc_resid(int64_t n, const T* __restrict__ b, const T* __restrict__ q,
+                                                  T* __restrict__ r) {
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x)
+        r[l] = q ? b[l] - q[l] : b[l];
+}
+// d = r / theta;  ONLY (order == 1): x <- x0 + d (x0 = 0 with a zero guess)
+template <typename T, bool ONLY>
+__global__ void __launch_bounds__(256) k_pc_first(int64_t n, const T* __restrict__ r, T inv_theta, bool xzero,
+                                                  T* __restrict__ x, T* __restrict__ d) {
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
+        const T dl = r[l] * inv_theta;
+        if constexpr (ONLY) x[l] = xzero ? dl : x[l] + dl;
+        else d[l] = dl;
+    }
+}
+// x += d; r -= w (w = S A d); d = c1 d + c2 r; LAST folds the final x += d in
+template <typename T, bool XZERO, bool LAST>
+__global__ void __launch_bounds__(256) k_pc_step(int64_t n, const T* __restrict__ w, T c1, T c2, T* __restrict__ x,
+                                                 T* __restrict__ r, T* __restrict__ d) {
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
+        const T dl = d[l];
+        const T rl = r[l] - w[l];
+        const T dn = c1 * dl + c2 * rl;
+        const T x0 = XZERO ? T(0) : x[l];
+        if constexpr (LAST) x[l] = x0 + dl + dn;
+        else { x[l] = x0 + dl; r[l] = rl; d[l] = dn; }
+    }
+}
+
+template <typename T>
+int run_schwarz(sem_ctx* c, const T* b, T* x, int order, double lmin, double lmax, bool zero_guess, int kind) {
+    cudaStream_t st = c->stream;
+    const int64_t n = c->nL;
+    const sem_prec prec = sizeof(T) == 8 ? SEM_F64 : SEM_F32;
+    T* r = (T*)c->d_cheb[0];
+    T* d = (T*)c->d_cheb[1];
+    T* w = (T*)c->d_cheb[2];
+    const unsigned grid = (unsigned)c->num_sms * 8;
+    const double theta = 0.5 * (lmax + lmin), delta = 0.5 * (lmax - lmin), sigma = theta / delta;
+    double rho = 1.0 / sigma;
+    int rc;
+    const T* q = nullptr;
+    if (!zero_guess) {
+        if ((rc = sem_launch_ax_gs(c, x, w, prec, c->lambda, nullptr, nullptr))) return rc;      // x is masked on entry
+        q = w;
+    }
+    k_pc_resid<T><<<grid, 256, 0, st>>>(n, b, q, r);
+    if ((rc = sem_launch_schwarz(c, r, r, prec, kind))) return rc;                               // r = S (b - A x)
+    if (order == 1) k_pc_first<T, true><<<grid, 256, 0, st>>>(n, r, (T)(1.0 / theta), zero_guess, x, d);
+    else k_pc_first<T, false><<<grid, 256, 0, st>>>(n, r, (T)(1.0 / theta), zero_guess, x, d);
+    for (int k = 1; k < order; ++k) {
+        if ((rc = sem_launch_ax_gs(c, d, w, prec, c->lambda, nullptr, nullptr))) return rc;
+        if ((rc = sem_launch_schwarz(c, w, w, prec, kind))) return rc;                           // w = S A d
+        const double rho1 = 1.0 / (2.0 * sigma - rho);
+        const T c1 = (T)(rho1 * rho), c2 = (T)(2.0 * rho1 / delta);
+        const bool xzero = zero_guess && k == 1, last = k == order - 1;
+        if (xzero && last) k_pc_step<T, true, true><<<grid, 256, 0, st>>>(n, w, c1, c2, x, r, d);
+        else if (xzero) k_pc_step<T, true, false><<<grid, 256, 0, st>>>(n, w, c1, c2, x, r, d);
+        else if (last) k_pc_step<T, false, true><<<grid, 256, 0, st>>>(n, w, c1, c2, x, r, d);
+        else k_pc_step<T, false, false><<<grid, 256, 0, st>>>(n, w, c1, c2, x, r, d);
+        rho = rho1;
+    }
+    SEM_CUDA_OK(c, cudaGetLastError());
+    return SEM_OK;
+}
+
 // power iteration helpers: v = Minv * w, s[0] += wt v v   /   v *= scale
 __global__ void __launch_bounds__(256) k_pow_apply(int64_t n, const double* __restrict__ w, const double* __restrict__ Minv,
                                                    const double* __restrict__ wt, double* __restrict__ v,
                                                    double* __restrict__ s) {
     double acc = 0.0;
     for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
-        const double vl = Minv[l] * w[l];
+        const double vl = Minv ? Minv[l] * w[l] : w[l];      // Minv == nullptr: w already holds S A v
         v[l] = vl;
         acc += wt[l] * vl * vl;
     }
@@ -203,4 +273,63 @@ extern "C" int sem_cheby(sem_ctx* c, const void* b, void* x, int order, double l
     }
     if (prec == SEM_F64) return run<double>(c, (const double*)b, (double*)x, order, lmin, lmax, zero_guess != 0);
     return run<float>(c, (const float*)b, (float*)x, order, lmin, lmax, zero_guess != 0);
+}
+
+
+// Chebyshev-accelerated Schwarz: see include/sem.h.
+extern "C" int sem_cheby_schwarz(sem_ctx* c, const void* b, void* x, int order, double lmin, double lmax, int zero_guess,
+                                 sem_prec prec, sem_schwarz_kind kind) {
+    if (!c) return SEM_EINVAL;
+    c->err.clear();
+    if (!b || !x || b == x) return sem_fail(c, SEM_EINVAL, "sem_cheby_schwarz: NULL or aliased vectors");
+    if (prec != SEM_F64 && prec != SEM_F32) return sem_fail(c, SEM_EINVAL, "sem_cheby_schwarz: bad sem_prec");
+    if (kind != SEM_SCHWARZ_ASM && kind != SEM_SCHWARZ_RAS) return sem_fail(c, SEM_EINVAL, "sem_cheby_schwarz: bad kind");
+    if (order < 1 || !(lmin > 0.0) || !(lmax > lmin))
+        return sem_fail(c, SEM_EINVAL, "sem_cheby_schwarz: need order >= 1 and 0 < lmin < lmax");
+    if (((uintptr_t)x % 16) || ((uintptr_t)b % (prec == SEM_F64 ? 8 : 4)))
+        return sem_fail(c, SEM_EINVAL, "sem_cheby_schwarz: x must be 16-byte aligned");
+    if (!c->sw) return sem_fail(c, SEM_ESTATE, "sem_cheby_schwarz before sem_schwarz_setup");
+    if (c->lambda != 0.0 && !c->with_mass) return sem_fail(c, SEM_ESTATE, "lambda != 0 needs with_mass");
+    int rc;
+    if (prec == SEM_F32 && c->gmode == SEM_G_STORED && (rc = sem_build_g32(c))) return rc;
+    for (int q = 0; q < 3; ++q)
+        if (!c->d_cheb[q]) SEM_CUDA_OK(c, cudaMalloc(&c->d_cheb[q], c->nL * sizeof(double)));
+    if (prec == SEM_F64)
+        return run_schwarz<double>(c, (const double*)b, (double*)x, order, lmin, lmax, zero_guess != 0, (int)kind);
+    return run_schwarz<float>(c, (const float*)b, (float*)x, order, lmin, lmax, zero_guess != 0, (int)kind);
+}
+
+extern "C" int sem_lambda_max_schwarz(sem_ctx* c, sem_schwarz_kind kind, int iters, double* lam_out) {
+    if (!c || !lam_out) return SEM_EINVAL;
+    c->err.clear();
+    if (iters < 1) return sem_fail(c, SEM_EINVAL, "sem_lambda_max_schwarz: iters < 1");
+    if (kind != SEM_SCHWARZ_ASM && kind != SEM_SCHWARZ_RAS) return sem_fail(c, SEM_EINVAL, "bad sem_schwarz_kind");
+    if (!c->sw) return sem_fail(c, SEM_ESTATE, "sem_lambda_max_schwarz before sem_schwarz_setup");
+    int rc;
+    if (!c->d_Minv || c->lambda_of_diag != c->lambda) {
+        if ((rc = sem_build_diag(c))) return rc;              // the dot weights wt
+    }
+    for (int q = 0; q < 3; ++q)
+        if (!c->d_cheb[q]) SEM_CUDA_OK(c, cudaMalloc(&c->d_cheb[q], c->nL * sizeof(double)));
+    double *v = (double*)c->d_cheb[0], *w = (double*)c->d_cheb[1], *s = (double*)c->d_cheb[2];
+    cudaStream_t st = c->stream;
+    const unsigned grid = (unsigned)c->num_sms * 8;
+    k_pow_start<<<grid, 256, 0, st>>>(c->nL, c->d_l2u, c->d_wt, v);
+    double lam = 0.0;
+    for (int it = 0; it <= iters; ++it) {
+        SEM_CUDA_OK(c, cudaMemsetAsync(s, 0, sizeof(double), st));
+        if ((rc = sem_launch_ax_gs(c, v, w, SEM_F64, c->lambda, nullptr, nullptr))) return rc;
+        if ((rc = sem_launch_schwarz(c, w, w, SEM_F64, (int)kind))) return rc;
+        k_pow_apply<<<grid, 256, 0, st>>>(c->nL, w, nullptr, c->d_wt, v, s);
+        double h = 0.0;
+        SEM_CUDA_OK(c, cudaMemcpyAsync(&h, s, sizeof(double), cudaMemcpyDeviceToHost, st));
+        SEM_CUDA_OK(c, cudaStreamSynchronize(st));
+        const double wnorm = sqrt(h);
+        if (!(wnorm > 0.0)) return sem_fail(c, SEM_EINVAL, "sem_lambda_max_schwarz: operator annihilates the start vector");
+        if (it > 0) lam = wnorm;
+        k_pow_scale<<<grid, 256, 0, st>>>(c->nL, 1.0 / wnorm, v);
+    }
+    SEM_CUDA_OK(c, cudaGetLastError());
+    *lam_out = lam;
+    return SEM_OK;
 }

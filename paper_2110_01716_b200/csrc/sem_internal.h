@@ -19,6 +19,8 @@ __host__ __device__ inline int64_t sem_g_off(int64_t e, int k, int p, int epb, i
     return ((grp * p + k) * epb + (e - grp * epb)) * slab;
 }
 
+struct sem_schwarz_data;            // sem_schwarz.cu
+
 struct sem_ctx {
     // ---- discretisation (a0) ----
     int64_t E = 0;
@@ -87,6 +89,7 @@ struct sem_ctx {
     float* d_Minv32 = nullptr;     // Minv rounded to FP32 for the FP32 smoother (sem_cheby.cu)
     double lambda_of_minv32 = -1.0;
     void* d_cheb[3] = {nullptr, nullptr, nullptr};   // r, d, w of the Chebyshev smoother (sem_cheby.cu), nL doubles each
+    sem_schwarz_data* sw = nullptr; // NEXT-2b: face links, 1-D operator factorisations, weights (sem_schwarz_setup)
     uint64_t generation = 0;       // bumped whenever device pointers or parameters that launches capture may change
                                    // (sem_geom, sem_set_lambda): invalidates CUDA graphs recorded over this context
     // ---- CUDA graph of one sem_ax_gs application (sem_api.cu), valid for the argument set it was recorded with ----
@@ -129,6 +132,9 @@ int sem_launch_ax_gs(sem_ctx* c, const void* u, void* w, sem_prec prec, double l
 // sem_gs.cu
 int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask, const int* skip_flag = nullptr);
 int sem_launch_gs_many(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec prec, bool apply_mask);
+// sem_schwarz.cu
+void sem_schwarz_free(sem_ctx* c);
+int sem_launch_schwarz(sem_ctx* c, const void* r, void* z, sem_prec prec, int kind);   // z may alias r
 // sem_transfer.cu
 int sem_launch_transfer(sem_ctx* coarse, sem_ctx* fine, const void* in, void* out, sem_prec prec, sem_transfer_dir dir,
                         const void* in_minus, const double* wt);

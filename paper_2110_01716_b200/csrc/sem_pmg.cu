@@ -23,6 +23,8 @@ struct sem_pmg {
     std::vector<double> lmin, lmax;
     int smooth_order = 2, coarse_order = 8;
     sem_prec prec = SEM_F32;
+    sem_smoother smoother = SEM_SMOOTH_CHEBY_JACOBI;
+    std::vector<double> slmin, slmax;   // bounds of S A per level for the Schwarz smoothers
     std::vector<void*> r, z, w;         // per level work vectors (r, z below the finest; w above the coarsest)
     // flexible PCG (sem_fpcg): FP64 outer vectors on the finest level, FP32 copies for an FP32 cycle, 4 device scalars
     double* f[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};      // r, p, q, z, zold
@@ -45,13 +47,23 @@ struct sem_pmg {
 
 namespace {
 
+// pre-/post-smoothing of level l: Chebyshev-Jacobi, or Chebyshev-Schwarz on the levels that can carry it (N >= 2)
+template <typename T>
+int smooth(sem_pmg* mg, int l, const T* r, T* z, int zero_guess) {
+    sem_ctx* c = mg->lv[l];
+    if (mg->smoother != SEM_SMOOTH_CHEBY_JACOBI && c->N >= 2)
+        return sem_cheby_schwarz(c, r, z, mg->smooth_order, mg->slmin[l], mg->slmax[l], zero_guess, mg->prec,
+                                 mg->smoother == SEM_SMOOTH_CHEBY_RAS ? SEM_SCHWARZ_RAS : SEM_SCHWARZ_ASM);
+    return sem_cheby(c, r, z, mg->smooth_order, mg->lmin[l], mg->lmax[l], zero_guess, mg->prec);
+}
+
 template <typename T>
 int cycle(sem_pmg* mg, int l, const T* r, T* z) {
     sem_ctx* c = mg->lv[l];
     const int last = (int)mg->lv.size() - 1;
     int rc;
     if (l == last) return sem_cheby(c, r, z, mg->coarse_order, mg->lmin[l], mg->lmax[l], 1, mg->prec);
-    if ((rc = sem_cheby(c, r, z, mg->smooth_order, mg->lmin[l], mg->lmax[l], 1, mg->prec))) return rc;
+    if ((rc = smooth<T>(mg, l, r, z, 1))) return rc;
     T* w = (T*)mg->w[l];
     if ((rc = sem_launch_ax_gs(c, z, w, mg->prec, c->lambda, nullptr, nullptr))) return rc;
     sem_ctx* cc = mg->lv[l + 1];
@@ -63,7 +75,7 @@ int cycle(sem_pmg* mg, int l, const T* r, T* z) {
     if ((rc = sem_launch_gs(cc, rc_, mg->prec, /*apply_mask=*/true))) return rc;
     if ((rc = cycle<T>(mg, l + 1, rc_, zc))) return rc;
     if ((rc = sem_launch_transfer(cc, c, zc, z, mg->prec, SEM_PROLONG, nullptr, c->d_wt))) return rc;
-    return sem_cheby(c, r, z, mg->smooth_order, mg->lmin[l], mg->lmax[l], 0, mg->prec);
+    return smooth<T>(mg, l, r, z, 0);
 }
 
 __device__ __forceinline__ void block_add(double v, double* __restrict__ out) {
@@ -309,6 +321,32 @@ extern "C" int sem_pmg_create(sem_pmg** out, int nlevels, sem_ctx* const* levels
         if (rc) { sem_pmg_destroy(mg); return rc; }
     }
     *out = mg;
+    return SEM_OK;
+}
+
+extern "C" int sem_pmg_set_smoother(sem_pmg* mg, sem_smoother smoother, const double* lmin, const double* lmax) {
+    if (!mg) return SEM_EINVAL;
+    sem_ctx* c0 = mg->lv[0];
+    c0->err.clear();
+    if (smoother != SEM_SMOOTH_CHEBY_JACOBI && smoother != SEM_SMOOTH_CHEBY_SCHWARZ && smoother != SEM_SMOOTH_CHEBY_RAS)
+        return sem_fail(c0, SEM_EINVAL, "sem_pmg_set_smoother: bad sem_smoother");
+    const int nl = (int)mg->lv.size();
+    if (smoother != SEM_SMOOTH_CHEBY_JACOBI) {
+        if (!lmin || !lmax) return sem_fail(c0, SEM_EINVAL, "sem_pmg_set_smoother: NULL bounds");
+        mg->slmin.assign(lmin, lmin + nl);
+        mg->slmax.assign(lmax, lmax + nl);
+        for (int l = 0; l < nl - 1; ++l) {
+            sem_ctx* c = mg->lv[l];
+            if (c->N < 2) continue;
+            if (!(lmin[l] > 0.0) || !(lmax[l] > lmin[l])) return sem_fail(c0, SEM_EINVAL, "sem_pmg_set_smoother: bad bounds");
+            int rc = sem_schwarz_setup(c);
+            if (rc) return rc;
+        }
+    }
+    mg->smoother = smoother;
+    if (mg->g_exec) { cudaGraphExecDestroy(mg->g_exec); mg->g_exec = nullptr; }
+    if (mg->it_exec) { cudaGraphExecDestroy(mg->it_exec); mg->it_exec = nullptr; }
+    mg->g_r = nullptr; mg->g_z = nullptr; mg->g_calls = 0;
     return SEM_OK;
 }
 

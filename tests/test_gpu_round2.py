@@ -233,3 +233,159 @@ def test_measure_peak(torch_cuda, binding):
     assert 0.8 < dm / f64 < 1.25
     with pytest.raises(binding.SemError):
         binding.measure_peak(7)
+
+
+# --------------------------------------------------------------------------- NEXT-2b: overlapping Schwarz smoother
+def _schwarz_case(N, masked, permute):
+    return inputs.box_mesh(4, 3, 3, N, "random", seed=11 + N, permute_seed=5 if permute else None)
+
+
+@pytest.mark.parametrize("N,masked,permute", [(7, True, True), (7, False, False), (3, True, False), (2, True, True),
+                                              (5, False, True), (4, True, False)])
+def test_schwarz_setup_and_apply_parity(torch_cuda, binding, oracle_mod, N, masked, permute):
+    """sem_schwarz_setup / sem_schwarz against the oracle's Schwarz (reading S29): face neighbours bit-exact, 1-D operator
+    pairs 1e-13, weights 1e-14, and z = S r for the additive and the restricted variant in FP64 (1e-10: the library's
+    Jacobi eigen-solver and scipy's differ in the last digits of S) and FP32 (1e-5), on a deformed mesh, with and without
+    the Dirichlet mask, in lexicographic and in scrambled element order."""
+    m = _schwarz_case(N, masked, permute)
+    maps = oracle_mod.Maps(m.gid)
+    mask_u = oracle_mod.mask_unique(m.dirichlet, maps) if masked else np.zeros(maps.U, np.uint8)
+    r_u = np.where(mask_u != 0, 0.0, inputs.field_normal(maps.uniq_gid, 21))
+    with binding.Sem(m.E, m.N, m.vert, m.gid, m.dirichlet if masked else None) as sem:
+        sem.geom()
+        with pytest.raises(binding.SemError) as err:
+            sem.schwarz(to_dev(torch_cuda, r_u[maps.l2u]), torch_cuda.empty(sem.nL, device="cuda", dtype=torch_cuda.float64))
+        assert err.value.code == binding.SEM_ESTATE
+        sem.schwarz_setup()
+        for kind, restricted in ((binding.SEM_SCHWARZ_ASM, False), (binding.SEM_SCHWARZ_RAS, True)):
+            sw = oracle_mod.Schwarz(m, maps, mask_u, restricted)
+            nbr, A, B, W = sem.get_schwarz(kind)
+            assert np.array_equal(nbr, sw.nbr)
+            assert np.max(np.abs(A - sw.A1)) <= 1e-13 * np.max(np.abs(sw.A1))
+            assert np.max(np.abs(B - sw.B1)) <= 1e-13 * np.max(np.abs(sw.B1))
+            Wo = (sw.W if restricted else np.sqrt(sw.W))[maps.l2u]
+            assert np.max(np.abs(W.ravel() - Wo)) <= 1e-14
+            oz = sw.apply(r_u)[maps.l2u]
+            for dt, tol in ((torch_cuda.float64, 1e-10), (torch_cuda.float32, TOL32)):
+                dr = to_dev(torch_cuda, r_u[maps.l2u], dt)
+                dz = torch_cuda.full_like(dr, float("nan"))
+                sem.schwarz(dr, dz, kind)
+                torch_cuda.cuda.synchronize()
+                assert relerr(dz.cpu().numpy(), oz) <= tol, (N, kind, dt)
+                sem.schwarz(dr, dr, kind)                      # in place
+                assert torch_cuda.equal(dr, dz)
+
+
+def test_schwarz_needs_an_interior_face_node(torch_cuda, binding):
+    m = inputs.box_mesh(3, 3, 3, 1, "affine")
+    with binding.Sem(m.E, m.N, m.vert, m.gid) as sem:
+        sem.geom()
+        with pytest.raises(binding.SemError) as err:
+            sem.schwarz_setup()
+        assert err.value.code == binding.SEM_EINVAL
+
+
+@pytest.mark.parametrize("N,order,zero_guess,kind", [(7, 2, True, 0), (5, 3, False, 0), (3, 1, True, 0), (4, 2, False, 1)])
+def test_cheby_schwarz_parity(torch_cuda, binding, oracle_mod, N, order, zero_guess, kind):
+    """sem_cheby_schwarz against the oracle's cheby_pc with the Schwarz operator, and sem_lambda_max_schwarz against the
+    dense-free power iteration of the oracle (same start-independent limit: compared loosely)."""
+    m = _schwarz_case(N, True, False)
+    L = oracle_mod.Level(m, power_its=5)
+    L.use_schwarz(m, restricted=bool(kind), power_its=40)
+    b_u = L.A(np.where(L.mask_u != 0, 0.0, inputs.field_normal(L.maps.uniq_gid, 3)))
+    x0_u = None if zero_guess else np.where(L.mask_u != 0, 0.0, inputs.field_normal(L.maps.uniq_gid, 4))
+    ox = oracle_mod.cheby_pc(L.A, L.schwarz.apply, b_u, x0_u, order, L.slmin, L.slmax)[L.maps.l2u]
+    with binding.Sem(m.E, m.N, m.vert, m.gid, m.dirichlet) as sem:
+        sem.geom()
+        sem.schwarz_setup()
+        lam = sem.lambda_max_schwarz(kind, 40)
+        assert abs(1.1 * lam - L.slmax) <= 0.05 * L.slmax
+        for dt, tol in ((torch_cuda.float64, 1e-9), (torch_cuda.float32, 5e-5)):
+            db = to_dev(torch_cuda, b_u[L.maps.l2u], dt)
+            dx = torch_cuda.full_like(db, float("nan")) if zero_guess else to_dev(torch_cuda, x0_u[L.maps.l2u], dt)
+            sem.cheby_schwarz(db, dx, order, L.slmin, L.slmax, zero_guess, kind)
+            torch_cuda.cuda.synchronize()
+            assert relerr(dx.cpu().numpy(), ox) <= tol, (N, order, dt)
+
+
+def test_vcycle_and_fpcg_with_schwarz_smoothing(torch_cuda, binding, oracle_mod):
+    """The V-cycle with Chebyshev-Schwarz smoothing on the levels with N >= 2 (sem_pmg_set_smoother) against the oracle's
+    cycle with the same smoother, FP64 1e-9 / FP32 1e-4, and flexible PCG around it: the oracle's iteration count,
+    which is below the Chebyshev-Jacobi cycle's on the same problem."""
+    orders = (7, 3, 1)
+    meshes = [inputs.box_mesh(4, 3, 3, N, "random", seed=3) for N in orders]
+    olv = [oracle_mod.Level(m) for m in meshes]
+    ojac = [oracle_mod.Level(m) for m in meshes]
+    for L, m in zip(olv[:-1], meshes[:-1]):
+        L.use_schwarz(m)
+    L0 = olv[0]
+    xs = np.where(L0.mask_u != 0, 0.0, inputs.field_normal(L0.maps.uniq_gid, 17))
+    b_u = L0.A(xs)
+    oz = oracle_mod.vcycle(olv, b_u, 2, 8)
+    ores = oracle_mod.fpcg(L0, lambda r: oracle_mod.vcycle(olv, r, 2, 8), b_u, tol=1e-8, maxit=60)
+    ojres = oracle_mod.fpcg(ojac[0], lambda r: oracle_mod.vcycle(ojac, r, 2, 8), b_u, tol=1e-8, maxit=60)
+    assert ores["iters"] < ojres["iters"]
+    side = torch_cuda.cuda.Stream()
+    with torch_cuda.cuda.stream(side):
+        sems = [binding.Sem(m.E, m.N, m.vert, m.gid, m.dirichlet).geom() for m in meshes]
+        try:
+            slmin = [getattr(l, "slmin", l.lmin) for l in olv]
+            slmax = [getattr(l, "slmax", l.lmax) for l in olv]
+            for prec, dt, tol in ((binding.SEM_F64, torch_cuda.float64, 1e-9), (binding.SEM_F32, torch_cuda.float32, 1e-4)):
+                with binding.Pmg(sems, [l.lmin for l in olv], [l.lmax for l in olv], 2, 8, prec) as mg:
+                    mg.set_smoother(binding.SEM_SMOOTH_CHEBY_SCHWARZ, slmin, slmax)
+                    dr = to_dev(torch_cuda, b_u[L0.maps.l2u], dt)
+                    dz = torch_cuda.full_like(dr, float("nan"))
+                    for _ in range(3):                           # eager, captured, replayed
+                        mg.vcycle(dr, dz)
+                    side.synchronize()
+                    assert relerr(dz.cpu().numpy(), oz[L0.maps.l2u]) <= tol, prec
+                    b = to_dev(torch_cuda, b_u[L0.maps.l2u])
+                    x = torch_cuda.full_like(b, float("nan"))
+                    it, rel = mg.fpcg(b, x, 1e-8, 60)
+                    assert rel <= 1e-8 and abs(it - ores["iters"]) <= (0 if prec == binding.SEM_F64 else 1)
+                    assert relerr(x.cpu().numpy(), ores["x"][L0.maps.l2u]) <= 1e-6
+        finally:
+            for s_ in sems:
+                s_.close()
+
+
+@pytest.mark.slow
+def test_schwarz_config2_full_size_f32(torch_cuda, binding, oracle_mod):
+    """VERDICT r1 item 5's bar: the Schwarz smoother at E = 7200, N = 7 in FP32 (the paper's preconditioner precision,
+    P:109) against the FP64 oracle at 1e-5, and the flexible-PCG iteration count of the 7-3-1 cycle with Chebyshev-Schwarz
+    smoothing at config 2 below the Chebyshev-Jacobi cycle's."""
+    m = inputs.config2()
+    maps = oracle_mod.Maps(m.gid)
+    mask_u = oracle_mod.mask_unique(m.dirichlet, maps)
+    sw = oracle_mod.Schwarz(m, maps, mask_u)
+    r_u = np.where(mask_u != 0, 0.0, inputs.field_normal(maps.uniq_gid, 2))
+    oz = sw.apply(r_u)[maps.l2u]
+    side = torch_cuda.cuda.Stream()
+    with torch_cuda.cuda.stream(side):
+        lv = []
+        for N in (7, 3, 1):
+            mN = inputs.config4(N)
+            lv.append(binding.Sem(mN.E, N, mN.vert, mN.gid, mN.dirichlet).geom())
+        try:
+            lv[0].schwarz_setup()
+            dr = to_dev(torch_cuda, r_u[maps.l2u], torch_cuda.float32)
+            dz = torch_cuda.full_like(dr, float("nan"))
+            lv[0].schwarz(dr, dz)
+            side.synchronize()
+            assert relerr(dz.cpu().numpy(), oz) <= TOL32
+            lv[1].schwarz_setup()
+            lamj = [1.1 * s_.lambda_max(30) for s_ in lv]
+            lams = [1.1 * lv[0].lambda_max_schwarz(0, 30), 1.1 * lv[1].lambda_max_schwarz(0, 30), lamj[2]]
+            u = to_dev(torch_cuda, inputs.field_uniform(m.gid, 0).ravel())
+            rhs = torch_cuda.empty_like(u)
+            lv[0].ax_gs(u, rhs)
+            x = torch_cuda.zeros_like(u)
+            with binding.Pmg(lv, [0.1 * l for l in lamj], lamj, 2, 8, binding.SEM_F32) as mg:
+                it_j, rel_j = mg.fpcg(rhs, x, 1e-8, 100)
+                mg.set_smoother(binding.SEM_SMOOTH_CHEBY_SCHWARZ, [0.1 * l for l in lams], lams)
+                it_s, rel_s = mg.fpcg(rhs, x, 1e-8, 100)
+            assert rel_j <= 1e-8 and rel_s <= 1e-8 and it_s < it_j, (it_s, it_j)
+        finally:
+            for s_ in lv:
+                s_.close()
