@@ -58,71 +58,124 @@ __host__ __device__ inline int face_node(int p, int axis, int side, int fa, int 
     return (k * p + j) * p + i;
 }
 
-// b~: one thread per block position
-template <typename T>
-__global__ void __launch_bounds__(256) k_schwarz_ext(int64_t E, int p, const int4* __restrict__ link,
-                                                     const int32_t* __restrict__ nrm, const T* __restrict__ r,
+// one-layer-in node of the face neighbour behind my face node (fa, fb), and the block position of the neighbour's ghost
+// node that lies on my one-layer-in node (fa, fb) of that face
+__device__ __forceinline__ int nbr_one_in(int p, const int4 lk, int nf, int fa, int fb) {
+    const int na = nf & 3, ns = nf >> 2;
+    const int stride = na == 0 ? 1 : (na == 1 ? p : p * p);
+    return lk.y + fa * lk.z + fb * lk.w + (ns ? -stride : stride);
+}
+__device__ __forceinline__ int nbr_ghost_pos(int p, const int4 lk, int nf, int fa, int fb) {
+    const int m = p + 2, na = nf & 3, ns = nf >> 2;
+    const int ln = lk.y + fa * lk.z + fb * lk.w;                               // neighbour's face node behind mine
+    int ci = ln % p + 1, cj = (ln / p) % p + 1, ck = ln / (p * p) + 1;          // block coordinates
+    if (na == 0) ci += ns ? 1 : -1;                                             // one step OUT of the neighbour
+    else if (na == 1) cj += ns ? 1 : -1;
+    else ck += ns ? 1 : -1;
+    return (ck * m + cj) * m + ci;
+}
+
+// b~ (`gs_ext`): one CTA per element.  Three index ranges instead of a test per block position: the p^3 own nodes, the
+// 6 p^2 face-layer entries (gathered from the neighbours), the 12 p + 8 edge and corner positions (zero).
+// PC: p at compile time for the orders of the paper's level schedules (0: run-time p).
+template <typename T, int PC>
+__global__ void __launch_bounds__(256) k_schwarz_ext(int64_t E, int p_rt, const int4* __restrict__ link_g,
+                                                     const int32_t* __restrict__ nrm_g, const T* __restrict__ r,
                                                      const T* __restrict__ pre, T* __restrict__ ext) {
-    const int m = p + 2, m3 = m * m * m, p3 = p * p * p;
+    const int p = PC ? PC : p_rt;
+    const int m = p + 2, m2 = m * m, m3 = m2 * m, p2 = p * p, p3 = p2 * p;
+    __shared__ int4 link[6];
+    __shared__ int32_t nrm[6];
     for (int64_t e = blockIdx.x; e < E; e += gridDim.x) {
-        for (int q = threadIdx.x; q < m3; q += blockDim.x) {
-            const int a = q % m, b = (q / m) % m, c = q / (m * m);
-            const int ga = (a == 0 || a == m - 1), gb = (b == 0 || b == m - 1), gc = (c == 0 || c == m - 1);
+        __syncthreads();
+        if (threadIdx.x < 6) { link[threadIdx.x] = link_g[e * 6 + threadIdx.x]; nrm[threadIdx.x] = nrm_g[e * 6 + threadIdx.x]; }
+        __syncthreads();
+        T* xe = ext + e * m3;
+        for (int l = threadIdx.x; l < p3; l += blockDim.x) {                    // own nodes
+            const int i = l % p, j = (l / p) % p, k = l / p2;
+            const T v = pre ? pre[e * p3 + l] * r[e * p3 + l] : r[e * p3 + l];
+            xe[(k + 1) * m2 + (j + 1) * m + (i + 1)] = v;
+        }
+        for (int t = threadIdx.x; t < 6 * p2; t += blockDim.x) {                // face layers
+            const int f = t / p2, fa = (t % p2) % p, fb = (t % p2) / p;
+            const int axis = f >> 1, g = (f & 1) ? m - 1 : 0;
+            const int a = axis == 0 ? g : fa + 1, b = axis == 0 ? fa + 1 : (axis == 1 ? g : fb + 1),
+                      c = axis == 2 ? g : fb + 1;
+            const int4 lk = link[f];
             T v = T(0);
-            if (ga + gb + gc == 0) {
-                const int64_t l = e * p3 + ((c - 1) * p + (b - 1)) * p + (a - 1);
-                v = pre ? pre[l] * r[l] : r[l];
-            } else if (ga + gb + gc == 1) {
-                const int axis = ga ? 0 : (gb ? 1 : 2);
-                const int side = (ga ? a : (gb ? b : c)) != 0;
-                const int fa = axis == 0 ? b - 1 : a - 1, fb = axis == 2 ? b - 1 : c - 1;
-                const int4 lk = link[e * 6 + 2 * axis + side];
-                if (lk.x >= 0) {
-                    const int32_t nf = nrm[e * 6 + 2 * axis + side];
-                    const int na = nf & 3, ns = nf >> 2;
-                    int stride = 1;
-                    for (int t = 0; t < na; ++t) stride *= p;
-                    const int l = lk.y + fa * lk.z + fb * lk.w + (ns ? -stride : stride);      // one layer in
-                    v = pre ? pre[(int64_t)lk.x * p3 + l] * r[(int64_t)lk.x * p3 + l] : r[(int64_t)lk.x * p3 + l];
-                }
+            if (lk.x >= 0) {
+                const int64_t src = (int64_t)lk.x * p3 + nbr_one_in(p, lk, nrm[f], fa, fb);
+                v = pre ? pre[src] * r[src] : r[src];
             }
-            ext[e * m3 + q] = v;
+            xe[c * m2 + b * m + a] = v;
+        }
+        for (int t = threadIdx.x; t < 12 * p + 8; t += blockDim.x) {            // edges and corners of the block: no node
+            int a, b, c;
+            if (t < 12 * p) {
+                const int ed = t / p, q = t % p + 1, ax = ed >> 2, s0 = (ed & 1) ? m - 1 : 0, s1 = (ed & 2) ? m - 1 : 0;
+                a = ax == 0 ? q : s0;
+                b = ax == 1 ? q : (ax == 0 ? s0 : s1);
+                c = ax == 2 ? q : s1;
+            } else {
+                const int cn = t - 12 * p;
+                a = (cn & 1) ? m - 1 : 0; b = (cn & 2) ? m - 1 : 0; c = (cn & 4) ? m - 1 : 0;
+            }
+            xe[c * m2 + b * m + a] = T(0);
         }
     }
 }
 
-// z_L = W (own part of u~ + ghost layers of the face neighbours), one thread per local node
-template <typename T, bool RESTRICTED>
-__global__ void __launch_bounds__(256) k_schwarz_combine(int64_t E, int p, const int4* __restrict__ link,
-                                                         const int32_t* __restrict__ nrm, const T* __restrict__ ext,
+// z_L = W (own part of u~ + ghost layers of the face neighbours): the own part goes to shared memory, the 6 p^2 ghost
+// values are loaded together, and are added face by face (a node of two one-layer-in planes receives its contributions
+// in a fixed order: results are bit-repeatable)
+template <typename T, bool RESTRICTED, int PC>
+__global__ void __launch_bounds__(256) k_schwarz_combine(int64_t E, int p_rt, const int4* __restrict__ link_g,
+                                                         const int32_t* __restrict__ nrm_g, const T* __restrict__ ext,
                                                          const T* __restrict__ W, T* __restrict__ z) {
-    const int m = p + 2, m3 = m * m * m, p3 = p * p * p, N = p - 1;
+    const int p = PC ? PC : p_rt;
+    const int m = p + 2, m2 = m * m, m3 = m2 * m, p2 = p * p, p3 = p2 * p, N = p - 1;
+    __shared__ int4 link[6];
+    __shared__ int32_t nrm[6];
+    extern __shared__ __align__(16) unsigned char zs_raw[];
+    T* zs = reinterpret_cast<T*>(zs_raw);                                        // [p^3]
     for (int64_t e = blockIdx.x; e < E; e += gridDim.x) {
-        for (int l = threadIdx.x; l < p3; l += blockDim.x) {
-            const int i = l % p, j = (l / p) % p, k = l / (p * p);
-            T v = ext[e * m3 + ((k + 1) * m + (j + 1)) * m + (i + 1)];
-            if (!RESTRICTED) {
-                const int co[3] = {i, j, k};
-#pragma unroll
-                for (int axis = 0; axis < 3; ++axis)
-#pragma unroll
-                    for (int side = 0; side < 2; ++side) {
-                        if (co[axis] != (side ? N - 1 : 1)) continue;          // not in the one-layer-in plane of this face
-                        const int4 lk = link[e * 6 + 2 * axis + side];
-                        if (lk.x < 0) continue;
-                        const int fa = axis == 0 ? j : i, fb = axis == 2 ? j : k;
-                        const int ln = lk.y + fa * lk.z + fb * lk.w;            // neighbour's face node behind mine
-                        const int32_t nf = nrm[e * 6 + 2 * axis + side];
-                        const int na = nf & 3, ns = nf >> 2;
-                        int ci = ln % p + 1, cj = (ln / p) % p + 1, ck = ln / (p * p) + 1;   // block coordinates
-                        if (na == 0) ci += ns ? 1 : -1;                          // one step OUT of the neighbour: its ghost
-                        else if (na == 1) cj += ns ? 1 : -1;
-                        else ck += ns ? 1 : -1;
-                        v += ext[(int64_t)lk.x * m3 + (ck * m + cj) * m + ci];
-                    }
+        __syncthreads();
+        if (threadIdx.x < 6) { link[threadIdx.x] = link_g[e * 6 + threadIdx.x]; nrm[threadIdx.x] = nrm_g[e * 6 + threadIdx.x]; }
+        __syncthreads();
+        const T* xe = ext + e * m3;
+        if (RESTRICTED) {
+            for (int l = threadIdx.x; l < p3; l += blockDim.x) {
+                const int i = l % p, j = (l / p) % p, k = l / p2;
+                const T v = xe[(k + 1) * m2 + (j + 1) * m + (i + 1)];
+                z[e * p3 + l] = W ? W[e * p3 + l] * v : v;
             }
-            z[e * p3 + l] = W ? W[e * p3 + l] * v : v;
+            continue;
         }
+        // ghost values of the neighbours, two entries per thread at most (6 p^2 <= 2 x 256 up to p = 9; more: loop)
+        constexpr int MAXV = 6;
+        T gv[MAXV];
+        int nv = 0;
+        for (int t = threadIdx.x; t < 6 * p2 && nv < MAXV; t += blockDim.x, ++nv) {
+            const int f = t / p2, fa = (t % p2) % p, fb = (t % p2) / p;
+            const int4 lk = link[f];
+            gv[nv] = lk.x >= 0 ? ext[(int64_t)lk.x * m3 + nbr_ghost_pos(p, lk, nrm[f], fa, fb)] : T(0);
+        }
+        for (int l = threadIdx.x; l < p3; l += blockDim.x) {
+            const int i = l % p, j = (l / p) % p, k = l / p2;
+            zs[l] = xe[(k + 1) * m2 + (j + 1) * m + (i + 1)];
+        }
+        __syncthreads();
+        for (int f = 0; f < 6; ++f) {
+            nv = 0;
+            for (int t = threadIdx.x; t < 6 * p2 && nv < MAXV; t += blockDim.x, ++nv) {
+                if (t / p2 != f) continue;
+                const int fa = (t % p2) % p, fb = (t % p2) / p, axis = f >> 1, q = (f & 1) ? N - 1 : 1;
+                const int i = axis == 0 ? q : fa, j = axis == 0 ? fa : (axis == 1 ? q : fb), k = axis == 2 ? q : fb;
+                zs[(k * p + j) * p + i] += gv[nv];
+            }
+            __syncthreads();
+        }
+        for (int l = threadIdx.x; l < p3; l += blockDim.x) z[e * p3 + l] = W ? W[e * p3 + l] * zs[l] : zs[l];
     }
 }
 
@@ -140,6 +193,36 @@ __global__ void __launch_bounds__(256) k_inv_w(int64_t n, const double* __restri
     }
 }
 
+// p = 8, 6, 4 (N = 7, 5, 3: the upper levels of the 7-3-1 and 8-5-1 / 8-6-4-1 schedules run one order apart) and 9, 7, 5
+// are compiled with p fixed; any other order runs the generic instantiation
+template <typename T>
+void launch_ext(sem_ctx* c, unsigned grid, const T* r, const T* pre, T* ext) {
+    sem_schwarz_data* s = c->sw;
+#define SEM_SW_EXT(PP) k_schwarz_ext<T, PP><<<grid, 256, 0, c->stream>>>(c->E, c->p, s->d_link, s->d_nrm, r, pre, ext)
+    switch (c->p) {
+        case 4: SEM_SW_EXT(4); break;  case 5: SEM_SW_EXT(5); break;  case 6: SEM_SW_EXT(6); break;
+        case 7: SEM_SW_EXT(7); break;  case 8: SEM_SW_EXT(8); break;  case 9: SEM_SW_EXT(9); break;
+        default: SEM_SW_EXT(0);
+    }
+#undef SEM_SW_EXT
+}
+template <typename T>
+void launch_combine(sem_ctx* c, unsigned grid, bool restricted, const T* ext, const T* W, T* z) {
+    sem_schwarz_data* s = c->sw;
+#define SEM_SW_CMB(PP)                                                                                            \
+    do {                                                                                                          \
+        const size_t sm = sizeof(T) * c->p3;                                                                      \
+        if (restricted) k_schwarz_combine<T, true, PP><<<grid, 256, sm, c->stream>>>(c->E, c->p, s->d_link, s->d_nrm, ext, W, z); \
+        else k_schwarz_combine<T, false, PP><<<grid, 256, sm, c->stream>>>(c->E, c->p, s->d_link, s->d_nrm, ext, W, z);          \
+    } while (0)
+    switch (c->p) {
+        case 4: SEM_SW_CMB(4); break;  case 5: SEM_SW_CMB(5); break;  case 6: SEM_SW_CMB(6); break;
+        case 7: SEM_SW_CMB(7); break;  case 8: SEM_SW_CMB(8); break;  case 9: SEM_SW_CMB(9); break;
+        default: SEM_SW_CMB(0);
+    }
+#undef SEM_SW_CMB
+}
+
 template <typename T>
 int apply(sem_ctx* c, const T* r, T* z, int kind) {
     sem_schwarz_data* s = c->sw;
@@ -148,15 +231,11 @@ int apply(sem_ctx* c, const T* r, T* z, int kind) {
     const T* iL = sizeof(T) == 8 ? (const T*)s->d_iL64 : (const T*)s->d_iL32;
     const T* W = sizeof(T) == 8 ? (const T*)s->d_W64[kind] : (const T*)s->d_W32[kind];
     T* ext = (T*)s->d_ext;
-    const unsigned grid = (unsigned)(c->E < (int64_t)c->num_sms * 8 ? c->E : (int64_t)c->num_sms * 8);
-    k_schwarz_ext<T><<<grid, 256, 0, c->stream>>>(c->E, c->p, s->d_link, s->d_nrm, r,
-                                                  kind == SEM_SCHWARZ_ASM ? W : (const T*)nullptr, ext);
+    const unsigned grid = (unsigned)c->E;
+    launch_ext<T>(c, grid, r, kind == SEM_SCHWARZ_ASM ? W : (const T*)nullptr, ext);
     int rc = sem_fdm_apply(c, s->m, S, iL, ext, ext, prec);
     if (rc) return rc;
-    if (kind == SEM_SCHWARZ_RAS)
-        k_schwarz_combine<T, true><<<grid, 256, 0, c->stream>>>(c->E, c->p, s->d_link, s->d_nrm, ext, W, z);
-    else
-        k_schwarz_combine<T, false><<<grid, 256, 0, c->stream>>>(c->E, c->p, s->d_link, s->d_nrm, ext, W, z);
+    launch_combine<T>(c, grid, kind == SEM_SCHWARZ_RAS, ext, W, z);
     SEM_CUDA_OK(c, cudaGetLastError());
     return sem_launch_gs(c, z, prec, /*apply_mask=*/true);
 }
@@ -320,14 +399,11 @@ extern "C" int sem_schwarz_setup(sem_ctx* c) {
     double* ones = nullptr;
     SEM_CUDA_OK(c, cudaMalloc((void**)&ones, c->nL * sizeof(double)));
     const unsigned vgrid = (unsigned)c->num_sms * 8;
-    const unsigned egrid = (unsigned)(E < (int64_t)c->num_sms * 8 ? E : (int64_t)c->num_sms * 8);
+    const unsigned egrid = (unsigned)E;
     for (int k = 0; k < 2; ++k) {
         k_fill<double><<<vgrid, 256, 0, st>>>(c->nL, 1.0, ones);
-        k_schwarz_ext<double><<<egrid, 256, 0, st>>>(E, p, s->d_link, s->d_nrm, ones, nullptr, (double*)s->d_ext);
-        if (k == SEM_SCHWARZ_RAS)
-            k_schwarz_combine<double, true><<<egrid, 256, 0, st>>>(E, p, s->d_link, s->d_nrm, (const double*)s->d_ext, nullptr, ones);
-        else
-            k_schwarz_combine<double, false><<<egrid, 256, 0, st>>>(E, p, s->d_link, s->d_nrm, (const double*)s->d_ext, nullptr, ones);
+        launch_ext<double>(c, egrid, ones, nullptr, (double*)s->d_ext);
+        launch_combine<double>(c, egrid, k == SEM_SCHWARZ_RAS, (const double*)s->d_ext, nullptr, ones);
         if ((rc = sem_launch_gs(c, ones, SEM_F64, /*apply_mask=*/false))) { cudaFree(ones); return rc; }
         k_inv_w<<<vgrid, 256, 0, st>>>(c->nL, ones, k == SEM_SCHWARZ_ASM, s->d_W64[k], s->d_W32[k]);
     }
