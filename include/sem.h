@@ -92,6 +92,23 @@ SEM_API int sem_gs(sem_ctx* ctx, void* w, sem_prec prec, sem_op op);
  * SEM_EINVAL for nfields < 1 or field_stride < nL. */
 SEM_API int sem_gs_many(sem_ctx* ctx, void* w, int nfields, int64_t field_stride, sem_prec prec, sem_op op);
 
+/* NEXT-4: the operator and the Jacobi-PCG solve on several fields that share the geometry ("Each
+ * Stokes substep requires the solution of 3 Helmholtz problems -- one for each velocity component -- ... efficiently
+ * treated by using Jacobi-preconditioned conjugate gradient iteration").  Field f is the local-layout vector at
+ * u + f * field_stride / w + f * field_stride (values of `prec`; field_stride >= nL, even for the FP64 fused path).
+ * sem_ax_gs_many: w_f = M QQ^T (D^T G D + lambda B) u_f for every field; each result is what sem_ax_gs gives for that
+ *   field (same arithmetic; FP64 p = 8 with stored G: groups of 3 or 2 fields share ONE pass over G, 48 + 16 nf bytes per
+ *   node instead of 64 nf; other orders and FP32 run field by field), followed by sem_gs_many's kernels with the mask.
+ *   Asynchronous.
+ * sem_pcg_many: nfields <= 8 independent Jacobi-PCG solves in lockstep, each with its own alpha, beta, stopping test
+ *   (||r_f|| <= tol ||r_f,0||) and breakdown handling, i.e. each field's iterates are those of sem_pcg on it alone; the
+ *   operator pass is shared as above.  b, x DEVICE FP64 as in sem_pcg, at field_stride; iters_out, relres_out HOST
+ *   [nfields].  Synchronises. */
+SEM_API int sem_ax_gs_many(sem_ctx* ctx, const void* u, void* w, int nfields, int64_t field_stride, sem_prec prec,
+                           double lambda);
+SEM_API int sem_pcg_many(sem_ctx* ctx, const double* b, double* x, int nfields, int64_t field_stride, double tol, int maxit,
+                         int* iters_out, double* relres_out);
+
 /* a3-a7.  w = M QQ^T (D^T G D + lambda B) u, with M zeroing Dirichlet nodes (if the context has any).  u must be
  * continuous (equal on all copies of a shared node).  Called repeatedly with the same (u, w, prec, lambda) on a
  * non-default stream, the second call records the two kernels into a CUDA graph and later calls replay it (still

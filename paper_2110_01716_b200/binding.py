@@ -33,6 +33,8 @@ SYMBOLS = {
     "sem_ax_gs": (_i32, [_vp, _vp, _vp, _i32, _dbl]),
     "sem_gs_many": (_i32, [_vp, _vp, _i32, _i64, _i32, _i32]),
     "sem_pcg": (_i32, [_vp, _vp, _vp, _dbl, _i32, C.POINTER(_i32), C.POINTER(_dbl)]),
+    "sem_ax_gs_many": (_i32, [_vp, _vp, _vp, _i32, _i64, _i32, _dbl]),
+    "sem_pcg_many": (_i32, [_vp, _vp, _vp, _i32, _i64, _dbl, _i32, C.POINTER(_i32), C.POINTER(_dbl)]),
     "sem_set_lambda": (_i32, [_vp, _dbl]),
     "sem_get_pcg_history": (_i32, [_vp, _vp, _i32]),
     "sem_get_counts": (_i32, [_vp, C.POINTER(_i64), C.POINTER(_i64), C.POINTER(_i64), C.POINTER(_i64)]),
@@ -209,6 +211,29 @@ class Sem:
         self._check(self._L.sem_gs_many(self._h, C.c_void_p(w.data_ptr()), w.shape[0], w.shape[1], self._prec(w),
                                         SEM_OP_ADD))
         return w
+
+    def _fields(self, t):
+        assert t.is_cuda and t.is_contiguous() and t.dim() == 2 and t.shape[1] >= self.nL, \
+            "need a contiguous [nfields][stride >= nL] CUDA tensor"
+        return C.c_void_p(t.data_ptr()), int(t.shape[0]), int(t.shape[1])
+
+    def ax_gs_many(self, u, w, lam: float = 0.0):
+        """sem_ax_gs_many on contiguous [nfields][stride] CUDA tensors."""
+        pu, nf, st = self._fields(u)
+        pw, nfw, stw = self._fields(w)
+        assert (nf, st) == (nfw, stw) and u.dtype == w.dtype
+        self._check(self._L.sem_ax_gs_many(self._h, pu, pw, nf, st, self._prec(u), lam))
+        return w
+
+    def pcg_many(self, b, x, tol: float, maxit: int):
+        """sem_pcg_many on contiguous [nfields][stride] FP64 CUDA tensors: (iters[nf], relres[nf])."""
+        pb, nf, st = self._fields(b)
+        px, nfx, stx = self._fields(x)
+        assert (nf, st) == (nfx, stx)
+        it = (C.c_int * nf)()
+        rel = (C.c_double * nf)()
+        self._check(self._L.sem_pcg_many(self._h, pb, px, nf, st, tol, maxit, it, rel))
+        return list(it), list(rel)
 
     def ax_gs(self, u, w, lam: float = 0.0):
         assert u.dtype == w.dtype

@@ -24,6 +24,19 @@ static int require_geom(sem_ctx* c, const char* who) {
     return SEM_OK;
 }
 
+// gather-scatter (with the Dirichlet mask) of nf fields in launches of 4, 3 or 2; a single one by sem_gs's kernel
+int sem_launch_gs_fields(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec prec, bool mask, const int* skip) {
+    const size_t vs = prec == SEM_F64 ? 8 : 4;
+    for (int f = 0; f < nf;) {
+        const int left = nf - f, take = left >= 4 && left != 5 ? 4 : left >= 3 ? 3 : left;
+        void* wf = (char*)w + (size_t)f * (size_t)stride * vs;
+        const int rc = take == 1 ? sem_launch_gs(c, wf, prec, mask, skip) : sem_launch_gs_many(c, wf, take, stride, prec, mask, skip);
+        if (rc) return rc;
+        f += take;
+    }
+    return SEM_OK;
+}
+
 extern "C" {
 
 int sem_mesh_setup(sem_ctx** out, int64_t E, int N, const double* vertex_xyz, const int64_t* gid,
@@ -118,6 +131,17 @@ int sem_gs_many(sem_ctx* c, void* w, int nfields, int64_t field_stride, sem_prec
         f += take;
     }
     return SEM_OK;
+}
+
+int sem_ax_gs_many(sem_ctx* c, const void* u, void* w, int nfields, int64_t field_stride, sem_prec prec, double lambda) {
+    int rc = check_vec(c, u, w, prec, lambda, "sem_ax_gs_many");
+    if (rc) return rc;
+    if ((rc = require_geom(c, "sem_ax_gs_many"))) return rc;
+    if (nfields < 1 || field_stride < c->nL)
+        return sem_fail(c, SEM_EINVAL, "sem_ax_gs_many: nfields < 1 or field_stride < nL");
+    if (prec == SEM_F32 && c->gmode == SEM_G_STORED && (rc = sem_build_g32(c))) return rc;
+    if ((rc = sem_launch_ax_many(c, u, w, nfields, field_stride, prec, lambda, nullptr, 0, nullptr))) return rc;
+    return sem_launch_gs_fields(c, w, nfields, field_stride, prec, true, nullptr);
 }
 
 int sem_ax_gs(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda) {

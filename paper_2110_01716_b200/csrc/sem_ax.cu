@@ -590,6 +590,180 @@ __global__ void __launch_bounds__(32, MINB) ax_dmma(int64_t E, DParam<double, 8>
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// ax_dmma_many: the same operator applied to NF fields that share the geometric factors (NEXT-4: "3 Helmholtz problems --
+// one for each velocity component"): G is streamed ONCE per element and k-plane and used for all NF fields, so the
+// compulsory traffic is 48 + 16 NF bytes per node instead of 64 NF (NF = 3: 96 instead of 192).  One warp per element
+// as in ax_dmma; the w accumulators of all fields stay in registers (NF x 16 doubles), the u columns are re-read from
+// shared memory plane by plane (they cannot stay in registers as well).  Field f lives at u + f * stride, w + f * stride.
+// ---------------------------------------------------------------------------------------------------------------
+template <int NF, int NS>
+struct DmmaManySmem {
+    alignas(128) double g[NS][6 * 64];
+    alignas(128) double u[NF][512];
+    alignas(16) double sgs[2][64];
+    alignas(8) uint64_t gfull[NS];
+    alignas(8) uint64_t ufull;
+    alignas(16) double D[64];
+};
+
+template <int NF, int NS, int MINB>
+__global__ void __launch_bounds__(32, MINB) ax_dmma_many(int64_t E, DParam<double, 8> dp, const double* __restrict__ Gs,
+                                                         const double* __restrict__ Bm, double lambda,
+                                                         const double* __restrict__ u, double* __restrict__ w,
+                                                         int64_t stride, const int* __restrict__ skip_flag,
+                                                         double* __restrict__ dot_out, int64_t dot_stride) {
+    using SM = DmmaManySmem<NF, NS>;
+    constexpr int P = 8, P2 = 64, P3 = 512, SLAB = 6 * 64;
+    constexpr uint32_t GBYTES = SLAB * sizeof(double), UBYTES = P3 * sizeof(double);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    SM& sm = *reinterpret_cast<SM*>(smem_raw);
+    if (skip_flag && *skip_flag) return;
+    const int lane = threadIdx.x, g = lane >> 2, t = lane & 3;
+    const int64_t nmine = blockIdx.x < E ? (E - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+
+    const double* gsrc = Gs + (int64_t)blockIdx.x * (P * SLAB);
+    const int64_t gjump = (int64_t)(gridDim.x - 1) * (P * SLAB);
+    int64_t gleft = nmine * P;
+    uint64_t pol_g = 0, pol_u = 0;
+    auto issue_u = [&](int64_t n) {                      // the NF element blocks of u: one barrier phase per element
+        const int64_t e = blockIdx.x + n * gridDim.x;
+        mbar_expect_tx(&sm.ufull, NF * UBYTES);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) bulk_g2s(&sm.u[f][0], u + f * stride + e * P3, UBYTES, &sm.ufull, pol_u);
+    };
+    if (lane == 0) {
+#pragma unroll
+        for (int q = 0; q < NS; ++q) mbar_init(&sm.gfull[q], 1);
+        mbar_init(&sm.ufull, 1);
+        mbar_fence_init();
+    }
+    sm.D[lane] = dp.D[lane];
+    sm.D[lane + 32] = dp.D[lane + 32];
+    __syncwarp();
+    if (lane == 0 && nmine > 0) {
+        pol_g = policy_evict_first();
+        pol_u = policy_evict_last();
+        issue_u(0);
+        int gk = 0;
+        for (int q = 0; q < NS && gleft > 0; ++q) {
+            mbar_expect_tx(&sm.gfull[q], GBYTES);
+            bulk_g2s(&sm.g[q][0], gsrc, GBYTES, &sm.gfull[q], pol_g);
+            gsrc += SLAB;
+            if (++gk == P) { gk = 0; gsrc += gjump; }
+            --gleft;
+        }
+    }
+    double Br[2], As[2], BrT[2], AsT[2];
+    {
+        const uint32_t base = smem_u32(sm.D);
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            Br[c] = DRows<double, 8>::lds_volatile(base + (uint32_t)((g * 8 + 2 * t + c) * 8));
+            As[c] = DRows<double, 8>::lds_volatile(base + (uint32_t)((g * 8 + 4 * c + t) * 8));
+            BrT[c] = DRows<double, 8>::lds_volatile(base + (uint32_t)(((2 * t + c) * 8 + g) * 8));
+            AsT[c] = DRows<double, 8>::lds_volatile(base + (uint32_t)(((4 * c + t) * 8 + g) * 8));
+        }
+    }
+    double partial[NF];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) partial[f] = 0.0;
+    int q = 0;
+    uint32_t gphase = 0;
+    const int own = g * 8 + 2 * t;
+    for (int64_t n = 0; n < nmine; ++n) {
+        const int64_t e = blockIdx.x + n * gridDim.x;
+        mbar_wait(&sm.ufull, (uint32_t)(n & 1));
+        double wk[NF][P][2];
+#pragma unroll
+        for (int f = 0; f < NF; ++f)
+#pragma unroll
+            for (int k = 0; k < P; ++k) { wk[f][k][0] = 0.0; wk[f][k][1] = 0.0; }
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+            mbar_wait(&sm.gfull[q], gphase);
+            double G6[6][2];
+#pragma unroll
+            for (int c = 0; c < 6; ++c) {
+                const double2 v = *reinterpret_cast<const double2*>(&sm.g[q][c * P2 + own]);
+                G6[c][0] = v.x; G6[c][1] = v.y;
+            }
+#pragma unroll
+            for (int f = 0; f < NF; ++f) {
+                const double* sue = &sm.u[f][0];
+                double uk[P][2];
+#pragma unroll
+                for (int l = 0; l < P; ++l) {
+                    const double2 v = *reinterpret_cast<const double2*>(sue + l * P2 + own);
+                    uk[l][0] = v.x; uk[l][1] = v.y;
+                }
+                double ur[2] = {0.0, 0.0}, us[2] = {0.0, 0.0};
+                dmma884(ur[0], ur[1], uk[k][0], Br[0]);
+                dmma884(us[0], us[1], As[0], sue[k * P2 + t * P + g]);
+                dmma884(ur[0], ur[1], uk[k][1], Br[1]);
+                dmma884(us[0], us[1], As[1], sue[k * P2 + (4 + t) * P + g]);
+                double ut[2] = {0.0, 0.0};
+#pragma unroll
+                for (int l = 0; l < P; ++l) { ut[0] += dp.D[k * P + l] * uk[l][0]; ut[1] += dp.D[k * P + l] * uk[l][1]; }
+                double gr[2], gs[2], gt[2];
+#pragma unroll
+                for (int b = 0; b < 2; ++b) {
+                    gr[b] = G6[0][b] * ur[b] + G6[1][b] * us[b] + G6[2][b] * ut[b];
+                    gs[b] = G6[1][b] * ur[b] + G6[3][b] * us[b] + G6[4][b] * ut[b];
+                    gt[b] = G6[2][b] * ur[b] + G6[4][b] * us[b] + G6[5][b] * ut[b];
+                }
+                const int buf = (k * NF + f) & 1;
+                *reinterpret_cast<double2*>(&sm.sgs[buf][own]) = make_double2(gs[0], gs[1]);
+#pragma unroll
+                for (int l = 0; l < P; ++l) { wk[f][l][0] += dp.D[k * P + l] * gt[0]; wk[f][l][1] += dp.D[k * P + l] * gt[1]; }
+                __syncwarp();
+                if (f == NF - 1 && lane == 0 && gleft > 0) {      // every lane has consumed stage q for all fields: refill
+                    mbar_expect_tx(&sm.gfull[q], GBYTES);
+                    bulk_g2s(&sm.g[q][0], gsrc, GBYTES, &sm.gfull[q], pol_g);
+                    gsrc += SLAB;
+                    if ((k + NS) % P == P - 1) gsrc += gjump;
+                    --gleft;
+                }
+                double a0[2] = {0.0, 0.0}, a1[2] = {0.0, 0.0};
+                dmma884(a0[0], a0[1], gr[0], BrT[0]);
+                dmma884(a1[0], a1[1], AsT[0], sm.sgs[buf][t * P + g]);
+                dmma884(a0[0], a0[1], gr[1], BrT[1]);
+                dmma884(a1[0], a1[1], AsT[1], sm.sgs[buf][(4 + t) * P + g]);
+                wk[f][k][0] += a0[0] + a1[0];
+                wk[f][k][1] += a0[1] + a1[1];
+            }
+            if (++q == NS) { q = 0; gphase ^= 1u; }
+        }
+        // results: w = wk (+ lambda B u), the fused dots sum_l u_l w_l per field; then the u buffers are free again
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+            double* wdst = w + f * stride + e * P3 + own;
+#pragma unroll
+            for (int k = 0; k < P; ++k) {
+                const double2 uv = *reinterpret_cast<const double2*>(&sm.u[f][k * P2 + own]);
+                double v0 = wk[f][k][0], v1 = wk[f][k][1];
+                if (Bm) {
+                    const double2 bm = *reinterpret_cast<const double2*>(Bm + e * P3 + own + k * P2);
+                    v0 += lambda * bm.x * uv.x;
+                    v1 += lambda * bm.y * uv.y;
+                }
+                *reinterpret_cast<double2*>(wdst + k * P2) = make_double2(v0, v1);
+                partial[f] += uv.x * v0 + uv.y * v1;
+            }
+        }
+        __syncwarp();
+        if (lane == 0 && n + 1 < nmine) issue_u(n + 1);
+    }
+    if (dot_out) {
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+            double v = partial[f];
+            for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            if (lane == 0) atomicAdd(dot_out + f * dot_stride, v);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------------------------
 template <typename T, int P>
@@ -678,6 +852,24 @@ int launch_dmma(sem_ctx* c, const double* u, double* w, double lambda, const int
     return SEM_OK;
 }
 
+template <int NF>
+int launch_dmma_many(sem_ctx* c, const double* u, double* w, int64_t stride, double lambda, const int* skip, double* dot,
+                     int64_t dot_stride) {
+    constexpr int NS = 3, MINB = 8;
+    using SM = DmmaManySmem<NF, NS>;
+    const DParam<double, 8> dp = make_dparam<double, 8>(c);
+    const size_t smem = sizeof(SM) + 128;
+    auto kern = ax_dmma_many<NF, NS, MINB>;
+    int blocks_per_sm = 0;
+    if (int rc = resident_blocks(c, kern, 32, smem, &blocks_per_sm)) return rc;
+    const int64_t cap = (int64_t)c->num_sms * blocks_per_sm;
+    const unsigned grid = (unsigned)(c->E < cap ? c->E : cap);
+    kern<<<grid, 32, smem, c->stream>>>(c->E, dp, c->d_G, lambda != 0.0 ? c->d_B : (const double*)nullptr, lambda, u, w,
+                                        stride, skip, dot, dot_stride);
+    SEM_CUDA_OK(c, cudaGetLastError());
+    return SEM_OK;
+}
+
 // stage depth / residency per (T, P): sized so that ~7-8 CTAs fit in 227 KB and > 64 KB are in flight per SM
 template <typename T, int P> struct StreamCfg { static constexpr int NS = 4, MINB = 1; };
 template <> struct StreamCfg<double, 8> { static constexpr int NS = 5, MINB = 8; };
@@ -741,4 +933,28 @@ int sem_launch_ax_gs(sem_ctx* c, const void* u, void* w, sem_prec prec, double l
     int rc;
     if ((rc = sem_launch_ax(c, u, w, prec, lambda, dot_out, skip_flag))) return rc;
     return sem_launch_gs(c, w, prec, true, skip_flag);
+}
+
+// NEXT-4: the operator on nf fields (u + f * stride -> w + f * stride).  FP64 p = 8 with stored G and 16-byte aligned
+// fields: groups of 3 (or 2) fields share one pass over G (ax_dmma_many); everything else: field by field.
+// dot_out + f * dot_stride receives sum_l u_l w_l of field f (nullptr: none).
+int sem_launch_ax_many(sem_ctx* c, const void* u, void* w, int nf, int64_t stride, sem_prec prec, double lambda,
+                       double* dot_out, int64_t dot_stride, const int* skip_flag) {
+    const size_t vs = prec == SEM_F64 ? 8 : 4;
+    const bool fused = prec == SEM_F64 && c->p == 8 && c->gmode == SEM_G_STORED && c->ax_variant == 0 &&
+                       ((uintptr_t)u % 16) == 0 && ((uintptr_t)w % 16) == 0 && (stride % 2) == 0;
+    int f = 0, rc;
+    while (f < nf) {
+        const int left = nf - f;
+        const int take = !fused ? 1 : (left >= 3 && left != 4 ? 3 : (left >= 2 ? 2 : 1));
+        const char* uf = (const char*)u + (size_t)f * (size_t)stride * vs;
+        char* wf = (char*)w + (size_t)f * (size_t)stride * vs;
+        double* df = dot_out ? dot_out + f * dot_stride : nullptr;
+        if (take == 3) rc = launch_dmma_many<3>(c, (const double*)uf, (double*)wf, stride, lambda, skip_flag, df, dot_stride);
+        else if (take == 2) rc = launch_dmma_many<2>(c, (const double*)uf, (double*)wf, stride, lambda, skip_flag, df, dot_stride);
+        else rc = sem_launch_ax(c, uf, wf, prec, lambda, df, skip_flag);
+        if (rc) return rc;
+        f += take;
+    }
+    return SEM_OK;
 }

@@ -52,7 +52,8 @@ __global__ void __launch_bounds__(NT, 4) k_gs_records_many(int32_t n_pair, const
                                                            const int4* __restrict__ quad, int32_t n_big,
                                                            const int2* __restrict__ big,
                                                            const int32_t* __restrict__ sh_idx, T* __restrict__ w,
-                                                           int64_t stride) {
+                                                           int64_t stride, const int* __restrict__ skip_flag) {
+    if (skip_flag && *skip_flag) return;
     const int32_t b = blockIdx.x, nb = gridDim.x;
     const int32_t pp = ((n_pair + nb - 1) / nb + 31) & ~31, pq = ((n_quad + nb - 1) / nb + 31) & ~31,
                   pg = (n_big + nb - 1) / nb;
@@ -142,7 +143,8 @@ int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask, const int
 }
 
 // nf = 2, 3 or 4 fields at w + f * stride (values of T) in one launch
-int sem_launch_gs_many(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec prec, bool apply_mask) {
+int sem_launch_gs_many(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec prec, bool apply_mask,
+                       const int* skip_flag) {
     const bool m = apply_mask && c->has_mask;
     const int32_t np = (int32_t)c->n_pair, nq = (int32_t)c->n_quad, nb = (int32_t)c->n_big;
     if (np + nq + nb == 0) return SEM_OK;
@@ -153,7 +155,7 @@ int sem_launch_gs_many(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec pre
     blocks = (blocks + c->num_sms - 1) / c->num_sms * c->num_sms;
 #define SEM_GSM_LAUNCH(T, M, NF)                                                                                  \
     k_gs_records_many<T, M, NF><<<(unsigned)blocks, NT, 0, c->stream>>>(np, c->d_own_pair, nq, c->d_own_quad, nb,  \
-                                                                         c->d_own_big, c->d_sh_idx, (T*)w, stride)
+                                                                         c->d_own_big, c->d_sh_idx, (T*)w, stride, skip_flag)
 #define SEM_GSM_NF(T, M)                                                                                          \
     do {                                                                                                          \
         if (nf == 2) SEM_GSM_LAUNCH(T, M, 2);                                                                     \

@@ -129,9 +129,16 @@ int sem_launch_ax(sem_ctx* c, const void* u, void* w, sem_prec prec, double lamb
                   const int* skip_flag);
 int sem_launch_ax_gs(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda, double* dot_out,
                      const int* skip_flag);      // a3-a7: operator kernel + gather-scatter kernel
+int sem_launch_ax_many(sem_ctx* c, const void* u, void* w, int nf, int64_t stride, sem_prec prec, double lambda,
+                       double* dot_out, int64_t dot_stride, const int* skip_flag);
 // sem_gs.cu
 int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask, const int* skip_flag = nullptr);
-int sem_launch_gs_many(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec prec, bool apply_mask);
+int sem_launch_gs_many(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec prec, bool apply_mask,
+                       const int* skip_flag = nullptr);
+// sem_api.cu
+int sem_launch_gs_fields(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec prec, bool mask, const int* skip);
+// sem_api.cu
+int sem_launch_gs_fields(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec prec, bool mask, const int* skip);
 // sem_schwarz.cu
 void sem_schwarz_free(sem_ctx* c);
 int sem_launch_schwarz(sem_ctx* c, const void* r, void* z, sem_prec prec, int kind);   // z may alias r

@@ -226,3 +226,125 @@ extern "C" int sem_pcg(sem_ctx* c, const double* b, double* x, double tol, int m
     if (relres_out) *relres_out = c->h_hist[iters];
     return SEM_OK;
 }
+
+
+// ---------------------------------------------------------------------------------------------------------------
+// NEXT-4: Jacobi-PCG on nf right-hand sides at once ("3 Helmholtz problems -- one for each velocity component ...
+// Jacobi-preconditioned conjugate gradient iteration").  Every field runs exactly the recurrence of sem_pcg with its own
+// alpha, beta, stopping test and breakdown flag (own scalar slots), so each field's iterates are those sem_pcg would
+// produce for it alone; what is shared is the operator pass: one sem_launch_ax_many reads G once for all fields, and
+// one gather-scatter launch handles up to 4 of them.  The loop ends when every field has stopped.
+// ---------------------------------------------------------------------------------------------------------------
+namespace {
+__global__ void k_all_done(int nf, const PcgFlags* const* flags, int* __restrict__ all_done) {
+    int d = 1;
+    for (int f = 0; f < nf; ++f) d &= flags[f]->done != 0;
+    *all_done = d;
+}
+}  // namespace
+
+extern "C" int sem_pcg_many(sem_ctx* c, const double* b, double* x, int nfields, int64_t field_stride, double tol,
+                            int maxit, int* iters_out, double* relres_out) {
+    if (!c) return SEM_EINVAL;
+    c->err.clear();
+    if (!b || !x) return sem_fail(c, SEM_EINVAL, "sem_pcg_many: NULL vector");
+    if (nfields < 1 || nfields > 8 || field_stride < c->nL || (field_stride & 1))
+        return sem_fail(c, SEM_EINVAL, "sem_pcg_many: need 1 <= nfields <= 8 and an even field_stride >= nL");
+    if (((uintptr_t)x % 16) || ((uintptr_t)b % 8)) return sem_fail(c, SEM_EINVAL, "sem_pcg_many: x must be 16-byte aligned");
+    if (!(tol > 0.0) && maxit <= 0) return sem_fail(c, SEM_EINVAL, "sem_pcg_many: tol <= 0 with maxit <= 0");
+    if (!c->geom_done) return sem_fail(c, SEM_ESTATE, "sem_pcg_many before sem_geom");
+    if (c->lambda != 0.0 && !c->with_mass) return sem_fail(c, SEM_ESTATE, "lambda != 0 needs with_mass");
+    if (maxit < 0) maxit = 0;
+    cudaStream_t st = c->stream;
+    const int64_t n = c->nL, fs = field_stride;
+    const int nf = nfields;
+    int rc;
+    if (!c->pcg_ready || c->lambda_of_diag != c->lambda) {
+        if ((rc = sem_build_diag(c))) return rc;
+        if (!c->d_r) {
+            SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_r, n * sizeof(double)));
+            SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_p, n * sizeof(double)));
+            SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_w, n * sizeof(double)));
+        }
+        c->pcg_ready = true;
+    }
+    // work vectors r, p, w of all fields at the caller's stride; per-field scalar slots and flags
+    const int64_t slot = 4 * ((int64_t)maxit + 2) + 8;           // doubles per field (as in sem_pcg)
+    double *R = nullptr, *P = nullptr, *W = nullptr, *scal = nullptr;
+    const PcgFlags** d_fl = nullptr;
+    int* d_all = nullptr;
+    auto cleanup = [&]() { cudaFree(R); cudaFree(P); cudaFree(W); cudaFree(scal); cudaFree((void*)d_fl); cudaFree(d_all); };
+    cudaError_t e = cudaMalloc((void**)&R, nf * fs * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&P, nf * fs * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&W, nf * fs * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&scal, nf * slot * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&d_fl, nf * sizeof(PcgFlags*));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&d_all, sizeof(int));
+    if (e != cudaSuccess) { cleanup(); return sem_fail(c, SEM_ENOMEM, "sem_pcg_many: %s", cudaGetErrorString(e)); }
+    auto fail = [&](int code) { cudaStreamSynchronize(st); cleanup(); return code; };
+    PcgFlags* fl[8];
+    for (int f = 0; f < nf; ++f) fl[f] = reinterpret_cast<PcgFlags*>(scal + f * slot + 4 * ((int64_t)maxit + 2));
+    cudaMemsetAsync(scal, 0, nf * slot * sizeof(double), st);
+    cudaMemsetAsync(d_all, 0, sizeof(int), st);
+    cudaMemcpyAsync((void*)d_fl, fl, nf * sizeof(PcgFlags*), cudaMemcpyHostToDevice, st);
+    const unsigned vgrid = (unsigned)c->num_sms * 8;
+    for (int f = 0; f < nf; ++f) k_mask_vec<<<vgrid, 256, 0, st>>>(n, c->d_wt, x + f * fs);
+    if ((rc = sem_launch_ax_many(c, x, W, nf, fs, SEM_F64, c->lambda, nullptr, 0, nullptr))) return fail(rc);
+    if ((rc = sem_launch_gs_fields(c, W, nf, fs, SEM_F64, true, nullptr))) return fail(rc);
+    for (int f = 0; f < nf; ++f)
+        k_pcg_init<<<vgrid, 256, 0, st>>>(n, b + f * fs, W + f * fs, c->d_Minv, c->d_wt, x + f * fs, R + f * fs, P + f * fs,
+                                          scal + f * slot);
+    double rr0[8];
+    for (int f = 0; f < nf; ++f) {
+        double h0[4];
+        cudaMemcpyAsync(h0, scal + f * slot, 4 * sizeof(double), cudaMemcpyDeviceToHost, st);
+        if (cudaStreamSynchronize(st) != cudaSuccess) return fail(sem_fail(c, SEM_ECUDA, "sem_pcg_many: init failed"));
+        rr0[f] = h0[1];
+    }
+    const double tol2 = tol > 0.0 ? tol * tol : 0.0;
+    // a field with a zero initial residual has nothing to do: raise its flag now
+    for (int f = 0; f < nf; ++f)
+        if (!(rr0[f] > 0.0) || maxit == 0) {
+            const PcgFlags done = {1, 0, 0, 0};
+            cudaMemcpyAsync(fl[f], &done, sizeof(done), cudaMemcpyHostToDevice, st);
+        }
+    PcgFlags hf[8] = {};
+    const int batch = 16;
+    for (int it = 1; it <= maxit; ++it) {
+        k_all_done<<<1, 1, 0, st>>>(nf, d_fl, d_all);
+        if ((rc = sem_launch_ax_many(c, P, W, nf, fs, SEM_F64, c->lambda, scal + 4 * it, slot, d_all))) return fail(rc);
+        if ((rc = sem_launch_gs_fields(c, W, nf, fs, SEM_F64, true, d_all))) return fail(rc);
+        for (int f = 0; f < nf; ++f) {
+            double* sc = scal + f * slot;
+            if (c->d_wt8)
+                k_pcg_update<true><<<vgrid, 256, 0, st>>>(n, it, P + f * fs, W + f * fs, c->d_Minv, c->d_wt, c->d_wt8, x + f * fs, R + f * fs, sc, fl[f]);
+            else
+                k_pcg_update<false><<<vgrid, 256, 0, st>>>(n, it, P + f * fs, W + f * fs, c->d_Minv, c->d_wt, nullptr, x + f * fs, R + f * fs, sc, fl[f]);
+            k_pcg_direction<<<vgrid, 256, 0, st>>>(n, it, maxit, tol2, R + f * fs, c->d_Minv, P + f * fs, sc, fl[f]);
+        }
+        if (it % batch == 0 || it == maxit) {
+            bool all = true;
+            for (int f = 0; f < nf; ++f) cudaMemcpyAsync(&hf[f], fl[f], sizeof(PcgFlags), cudaMemcpyDeviceToHost, st);
+            if (cudaStreamSynchronize(st) != cudaSuccess) return fail(sem_fail(c, SEM_ECUDA, "sem_pcg_many: loop failed"));
+            for (int f = 0; f < nf; ++f) all = all && hf[f].done;
+            if (all) break;
+        }
+    }
+    if (cudaGetLastError() != cudaSuccess) return fail(sem_fail(c, SEM_ECUDA, "sem_pcg_many: launch failed"));
+    for (int f = 0; f < nf; ++f) {
+        const int iters = hf[f].iters;
+        double rel = rr0[f] > 0.0 ? 1.0 : 0.0;
+        if (iters > 0) {
+            double s1[4], s0[4];
+            cudaMemcpyAsync(s1, scal + f * slot + 4 * (int64_t)iters, sizeof(s1), cudaMemcpyDeviceToHost, st);
+            cudaMemcpyAsync(s0, scal + f * slot + 4 * (int64_t)(iters - 1), sizeof(s0), cudaMemcpyDeviceToHost, st);
+            cudaStreamSynchronize(st);
+            rel = hf[f].breakdown ? (iters > 1 ? sqrt(s0[1] / rr0[f]) : 1.0) : sqrt(s1[1] / rr0[f]);
+        }
+        if (iters_out) iters_out[f] = iters;
+        if (relres_out) relres_out[f] = rel;
+    }
+    cudaStreamSynchronize(st);
+    cleanup();
+    return SEM_OK;
+}

@@ -389,3 +389,82 @@ def test_schwarz_config2_full_size_f32(torch_cuda, binding, oracle_mod):
         finally:
             for s_ in lv:
                 s_.close()
+
+
+# --------------------------------------------------------------------------- NEXT-4: several fields sharing the geometry
+@pytest.mark.parametrize("N,nf,pad,dtype,lam", [(7, 3, 0, "f64", 0.0), (7, 3, 64, "f64", 7.5), (7, 2, 0, "f64", 0.0),
+                                                (7, 5, 16, "f64", 0.0), (7, 4, 0, "f64", 3.0), (7, 1, 0, "f64", 0.0),
+                                                (5, 3, 8, "f64", 0.0), (7, 3, 0, "f32", 0.0), (3, 3, 4, "f32", 2.0)])
+def test_ax_gs_many_parity(torch_cuda, binding, oracle_mod, N, nf, pad, dtype, lam):
+    """sem_ax_gs_many (the three velocity components share the geometry): every field against the oracle's
+    independent M QQ^T (A_L + lambda B) u_f at 1e-12 / 1e-5.  FP64 N = 7 takes the fused kernel (groups of 3 and 2 fields
+    read G once); other orders and FP32 run field by field.  More elements than resident warps; padded field stride."""
+    m = inputs.box_mesh(13, 12, 11, N, "random", seed=2) if N == 7 else inputs.box_mesh(6, 5, 4, N, "random", seed=2)
+    oG, _, rc = oracle_mod.geom_trilinear(m.vert, m.N)
+    assert rc == 0
+    om = oracle_mod.Maps(m.gid)
+    msk = oracle_mod.mask_unique(m.dirichlet, om)[om.l2u] != 0
+    tdt = torch_cuda.float64 if dtype == "f64" else torch_cuda.float32
+    tol = TOL64 if dtype == "f64" else TOL32
+    us = [inputs.field_uniform(m.gid, 30 + f) for f in range(nf)]
+    ows = [np.where(msk, 0.0, oracle_mod.gs(oracle_mod.ax(oG, u, m.N, lam).ravel(), om)) for u in us]
+    with binding.Sem(m.E, m.N, m.vert, m.gid, m.dirichlet) as sem:
+        sem.geom(with_mass=lam != 0.0)
+        stride = sem.nL + pad
+        du = torch_cuda.zeros(nf, stride, device="cuda", dtype=tdt)
+        for f in range(nf):
+            du[f, :sem.nL] = to_dev(torch_cuda, us[f].ravel(), tdt)
+        dw = torch_cuda.full_like(du, float("nan"))
+        sem.ax_gs_many(du, dw, lam)
+        torch_cuda.cuda.synchronize()
+        for f in range(nf):
+            assert relerr(dw[f, :sem.nL].cpu().numpy(), ows[f]) <= tol, (N, nf, f)
+        if pad:
+            assert bool(torch_cuda.isnan(dw[:, sem.nL:]).all())          # the padding is not touched
+        # each field equals what sem_ax_gs gives for it alone (same arithmetic, same summation order in the gs)
+        if dtype == "f64":
+            w1 = torch_cuda.empty(sem.nL, device="cuda", dtype=tdt)
+            sem.ax_gs(du[0, :sem.nL].contiguous(), w1, lam)
+            assert relerr(w1.cpu().numpy(), ows[0]) <= tol
+
+
+def test_pcg_many_matches_independent_solves(torch_cuda, binding, oracle_mod):
+    """sem_pcg_many: three right-hand sides in lockstep, each with its own alpha / beta / stopping test -- every field
+    reproduces the oracle's Jacobi-PCG on it alone (iteration count, relres, solution at 1e-9), although the fields
+    converge at different iterations and one right-hand side is zero (0 iterations); Helmholtz shift lambda > 0 as in
+    the velocity solves."""
+    m = inputs.box_mesh(5, 4, 4, 7, "smooth")
+    lam = 40.0
+    oG, _, rc = oracle_mod.geom_trilinear(m.vert, m.N)
+    om = oracle_mod.Maps(m.gid)
+    mask_u = oracle_mod.mask_unique(m.dirichlet, om)
+    xs = [np.where(mask_u != 0, 0.0, inputs.field_normal(om.uniq_gid, 50 + f)) for f in range(3)]
+    xs[1] = xs[1] * 0.0
+    xyz = oracle_mod.node_xyz(m.vert, m.N).reshape(-1, 3)
+    smooth = np.zeros(om.U)
+    smooth[om.l2u] = np.sin(np.pi * xyz[:, 0]) * np.sin(np.pi * xyz[:, 1]) * np.sin(np.pi * xyz[:, 2])
+    xs[2] = np.where(mask_u != 0, 0.0, smooth)                       # a smooth solution: stops at another iteration
+    bs = [oracle_mod.apply_Ag(oG, m.N, om, mask_u, x, lam) for x in xs]
+    ores = [oracle_mod.pcg(oG, m.N, om, mask_u, b, tol=1e-9, maxit=400, lam=lam) for b in bs]
+    assert ores[1]["iters"] == 0 and ores[2]["iters"] != ores[0]["iters"]
+    with binding.Sem(m.E, m.N, m.vert, m.gid, m.dirichlet) as sem:
+        sem.geom(with_mass=True)
+        sem.set_lambda(lam)
+        stride = sem.nL + 32
+        b = torch_cuda.zeros(3, stride, device="cuda", dtype=torch_cuda.float64)
+        for f in range(3):
+            b[f, :sem.nL] = to_dev(torch_cuda, bs[f][om.l2u])
+        x = torch_cuda.zeros_like(b)
+        its, rels = sem.pcg_many(b, x, 1e-9, 400)
+        for f in range(3):
+            assert its[f] == ores[f]["iters"], (f, its, [o["iters"] for o in ores])
+            assert abs(rels[f] - ores[f]["relres"]) <= 1e-4 * ores[f]["relres"] + 1e-30      # recurrence residual after ~140 iterations
+            if ores[f]["iters"]:
+                xo = ores[f]["x"][om.l2u]
+                assert relerr(x[f, :sem.nL].cpu().numpy(), xo) <= TOLPCG, f
+            else:
+                assert float(x[f].abs().max()) == 0.0
+        # maxit reached: every field reports maxit iterations
+        x.zero_()
+        its, _ = sem.pcg_many(b, x, 1e-30, 7)
+        assert its[0] == 7 and its[1] == 0 and its[2] == 7
