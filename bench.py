@@ -474,6 +474,63 @@ def run_leg(args):
     raise SystemExit(f"unknown --leg {leg}")
 
 
+def run_sharded(args):
+    """--sharded-n n: NEXT-4, the operator with the ELEMENTS partitioned over the ranks (contiguous blocks of a config-5
+    style mesh of n^3 elements, scrambled order), one interface exchange per application over NCCL
+    (paper_2110_01716_b200/sharded.py).  Strong scaling: the total work is fixed.  Not the default multi-GPU mode
+    (north_star scopes the headline to replicas); this build could only run it on one GPU and as a one-GPU emulation."""
+    import torch
+    import torch.distributed as dist
+
+    from paper_2110_01716_b200 import build, inputs, sharded
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if not dist.is_initialized():
+        if world == 1:
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            os.environ.setdefault("MASTER_PORT", "29531")
+        dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", local))
+    if rank == 0:
+        build.build()
+    dist.barrier()
+    mesh = inputs.config5(args.sharded_n)
+    b = sharded.partition_bounds(mesh.E, world)
+    sl = slice(b[rank], b[rank + 1])
+    sh = sharded.ShardedSem(sharded.DistComm(), b[rank + 1] - b[rank], mesh.N, mesh.vert[sl], mesh.gid[sl],
+                            mesh.dirichlet[sl]).geom()
+    u = torch.from_numpy(inputs.field_uniform(mesh.gid[sl], 0).ravel()).cuda()
+    w = torch.empty_like(u)
+    K, W = max(args.steps, 20), max(args.warmup, 3)
+    for _ in range(W):
+        sh.ax_gs(u, w)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    dist.barrier()
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(K):
+        sh.ax_gs(u, w)
+    e1.record()
+    torch.cuda.synchronize()
+    dist.barrier()
+    ms = max_over_ranks(e0.elapsed_time(e1), world, "cuda")
+    ib = torch.tensor([sh.interface_bytes()], device="cuda", dtype=torch.float64)
+    dist.all_reduce(ib)
+    if rank == 0:
+        print(json.dumps({
+            "metric": "Ax+gs GDOF/s (FP64, N=7), elements partitioned over the ranks", "value": mesh.dofs * K / (ms * 1e-3) / 1e9,
+            "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"config5-style {args.sharded_n}^3 hex, N=7, scrambled order, Dirichlet; contiguous "
+                                   f"element blocks per rank, one interface exchange per application",
+                       "E": mesh.E, "interface_bytes_sent_per_step_all_ranks": float(ib.item())},
+            "gpu_launches": K * (2 + 2 * len(sh.uniq))}))
+    sh.close()
+    dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -487,11 +544,15 @@ def main():
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--pcg-iters", type=int, default=300)
     ap.add_argument("--config5-n", type=int, default=100, help="elements per direction of the config-5 leg (0 = skip)")
+    ap.add_argument("--sharded-n", type=int, default=0,
+                    help="NEXT-4: > 0 runs the element-partitioned operator on a config-5 style mesh of n^3 elements")
     ap.add_argument("--max-n", type=int, default=64)
     ap.add_argument("--orders", default="3,5,7,9")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.sharded_n > 0:
+        return run_sharded(args)
     if args.leg != "headline":
         return run_leg(args)
     args.warmup = max(args.warmup, 3)

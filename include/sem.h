@@ -109,6 +109,18 @@ SEM_API int sem_ax_gs_many(sem_ctx* ctx, const void* u, void* w, int nfields, in
 SEM_API int sem_pcg_many(sem_ctx* ctx, const double* b, double* x, int nfields, int64_t field_stride, double tol, int maxit,
                          int* iters_out, double* relres_out);
 
+/* NEXT-4: the device side of the gather-scatter across ranks when the elements are partitioned over
+ * several GPUs, one context per rank over its own elements with the GLOBAL node ids ("exchange-and-sum of shared
+ * interface values").  After the rank-local sem_ax_gs, for every rank r that shares nodes with this one:
+ *   sem_iface_pack  buf[q] = w[first local copy of unique node uniq[q]]   (the rank-local sum), q < n
+ *   (exchange of the buffers: NCCL send/recv or peer copies, done by the caller -- paper_2110_01716_b200/sharded.py)
+ *   sem_iface_add   w[every local copy of unique node uniq[q]] += buf[q];  Dirichlet nodes stay zero
+ * with the received buffers added in ascending rank order on every rank.  uniq DEVICE int32 [n]: rank-local unique-node
+ * indices (positions in sem_get_maps' uniq_gid) of the shared nodes, in ascending global id -- the same order on both
+ * sides; each node at most once per list.  buf, w DEVICE, `prec` values.  Asynchronous on the context's stream. */
+SEM_API int sem_iface_pack(sem_ctx* ctx, const int32_t* uniq, int64_t n, const void* w, void* buf, sem_prec prec);
+SEM_API int sem_iface_add(sem_ctx* ctx, const int32_t* uniq, int64_t n, const void* buf, void* w, sem_prec prec);
+
 /* a3-a7.  w = M QQ^T (D^T G D + lambda B) u, with M zeroing Dirichlet nodes (if the context has any).  u must be
  * continuous (equal on all copies of a shared node).  Called repeatedly with the same (u, w, prec, lambda) on a
  * non-default stream, the second call records the two kernels into a CUDA graph and later calls replay it (still

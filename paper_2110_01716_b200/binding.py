@@ -33,6 +33,8 @@ SYMBOLS = {
     "sem_ax_gs": (_i32, [_vp, _vp, _vp, _i32, _dbl]),
     "sem_gs_many": (_i32, [_vp, _vp, _i32, _i64, _i32, _i32]),
     "sem_pcg": (_i32, [_vp, _vp, _vp, _dbl, _i32, C.POINTER(_i32), C.POINTER(_dbl)]),
+    "sem_iface_pack": (_i32, [_vp, _vp, _i64, _vp, _vp, _i32]),
+    "sem_iface_add": (_i32, [_vp, _vp, _i64, _vp, _vp, _i32]),
     "sem_ax_gs_many": (_i32, [_vp, _vp, _vp, _i32, _i64, _i32, _dbl]),
     "sem_pcg_many": (_i32, [_vp, _vp, _vp, _i32, _i64, _dbl, _i32, C.POINTER(_i32), C.POINTER(_dbl)]),
     "sem_set_lambda": (_i32, [_vp, _dbl]),
@@ -234,6 +236,18 @@ class Sem:
         rel = (C.c_double * nf)()
         self._check(self._L.sem_pcg_many(self._h, pb, px, nf, st, tol, maxit, it, rel))
         return list(it), list(rel)
+
+    def iface_pack(self, uniq, w, buf):
+        """sem_iface_pack: buf[q] = w[first copy of unique node uniq[q]] (uniq: int32 CUDA tensor)."""
+        self._check(self._L.sem_iface_pack(self._h, C.c_void_p(uniq.data_ptr()), int(uniq.numel()), self._vec(w),
+                                           C.c_void_p(buf.data_ptr()), self._prec(w)))
+        return buf
+
+    def iface_add(self, uniq, buf, w):
+        """sem_iface_add: every copy of unique node uniq[q] += buf[q] (Dirichlet nodes stay zero)."""
+        self._check(self._L.sem_iface_add(self._h, C.c_void_p(uniq.data_ptr()), int(uniq.numel()),
+                                          C.c_void_p(buf.data_ptr()), self._vec(w), self._prec(w)))
+        return w
 
     def ax_gs(self, u, w, lam: float = 0.0):
         assert u.dtype == w.dtype

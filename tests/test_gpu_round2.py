@@ -468,3 +468,56 @@ def test_pcg_many_matches_independent_solves(torch_cuda, binding, oracle_mod):
         x.zero_()
         its, _ = sem.pcg_many(b, x, 1e-30, 7)
         assert its[0] == 7 and its[1] == 0 and its[2] == 7
+
+
+# --------------------------------------------------------------------------- NEXT-4: elements partitioned over ranks
+@pytest.mark.parametrize("world,masked,dtype", [(2, True, "f64"), (3, False, "f64"), (4, True, "f32")])
+def test_sharded_apply_emulated_on_one_gpu(torch_cuda, binding, oracle_mod, world, masked, dtype):
+    """The sharded operator of paper_2110_01716_b200/sharded.py with all ranks' contexts on ONE GPU, phase by phase (local
+    sem_ax_gs + sem_iface_pack on every rank, buffer hand-over, sem_iface_add on every rank; no kernel waits on another):
+    every rank's result equals the single-context sem_ax_gs -- bit for bit on the nodes that live on one rank only, to
+    round-off on interface nodes -- and the oracle.  Scrambled element order, so the interfaces are ragged and nodes are
+    shared by up to `world` ranks."""
+    from paper_2110_01716_b200 import sharded
+    m = inputs.box_mesh(6, 5, 4, 7, "random", seed=8, permute_seed=2)
+    tdt = torch_cuda.float64 if dtype == "f64" else torch_cuda.float32
+    tol = TOL64 if dtype == "f64" else TOL32
+    u = inputs.field_uniform(m.gid, 12)
+    ow = _ax_gs_oracle(oracle_mod, m, u, masked).reshape(m.E, -1)
+    with binding.Sem(m.E, m.N, m.vert, m.gid, m.dirichlet if masked else None) as one:
+        one.geom()
+        du = to_dev(torch_cuda, u.ravel(), tdt)
+        w1 = torch_cuda.empty_like(du)
+        one.ax_gs(du, w1)
+        w1 = w1.cpu().numpy().reshape(m.E, -1)
+    b = sharded.partition_bounds(m.E, world)
+    cands = [sharded.surface_gids(m.gid[b[r]:b[r + 1]], m.N) for r in range(world)]
+    shards = []
+    try:
+        for r in range(world):
+            sl = slice(b[r], b[r + 1])
+            s = sharded.ShardedSem(sharded.LocalComm(r, world, cands), b[r + 1] - b[r], m.N, m.vert[sl], m.gid[sl],
+                                   m.dirichlet[sl] if masked else None, dtype=tdt)
+            shards.append(s.geom())
+        us = [to_dev(torch_cuda, u[b[r]:b[r + 1]].ravel(), tdt) for r in range(world)]
+        ws = [torch_cuda.full_like(x, float("nan")) for x in us]
+        sharded.emulated_ax_gs(shards, us, ws)
+        torch_cuda.cuda.synchronize()
+        n_shared = 0
+        for r, s in enumerate(shards):
+            got = ws[r].cpu().numpy().reshape(b[r + 1] - b[r], -1)
+            assert relerr(got, ow[b[r]:b[r + 1]]) <= tol * max(1.0, np.max(np.abs(ow)) / np.max(np.abs(ow[b[r]:b[r + 1]])))
+            maps = s.sem.maps()
+            shared_u = np.zeros(maps["uniq_gid"].size, bool)
+            for q in s.uniq.values():
+                shared_u[q.cpu().numpy()] = True
+            shared = shared_u[maps["l2u"]].reshape(got.shape)
+            n_shared += int(shared.sum())
+            assert np.array_equal(got[~shared], w1[b[r]:b[r + 1]][~shared])          # one rank only: bit-identical
+            assert np.max(np.abs(got - w1[b[r]:b[r + 1]])) <= tol * np.max(np.abs(w1))
+            for q, lst in s.plan.items():                                             # symmetric plan, same order
+                assert np.array_equal(lst, shards[q].plan[r])
+        assert n_shared > 0
+    finally:
+        for s in shards:
+            s.close()
