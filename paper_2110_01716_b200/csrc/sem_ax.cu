@@ -306,7 +306,7 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
                                                                    const T* __restrict__ Gs, const T* __restrict__ Bm,
                                                                    T lambda, const T* __restrict__ u,
                                                                    T* __restrict__ w, const int* __restrict__ skip_flag,
-                                                                   double* __restrict__ dot_out) {
+                                                                   double* __restrict__ dot_out, int u_keep) {
     using SM = StreamSmem<T, P, NS>;
     constexpr int EPB = SM::EPB, P2 = SM::P2, P3 = SM::P3, SLAB = SM::SLAB, NT = threads_of<P>();
     constexpr bool FULL = EPB * P2 == NT;           // every thread owns a column
@@ -347,7 +347,7 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
     __syncthreads();
     if (tid == 0 && nmine > 0) {
         pol_g = policy_evict_first();
-        pol_u = policy_evict_last();
+        pol_u = u_keep ? policy_evict_last() : policy_evict_first();
         issue_u(0);
         int gk = 0;
         for (int q = 0; q < NS && gleft > 0; ++q) {
@@ -448,7 +448,8 @@ template <int NS, int MINB>
 __global__ void __launch_bounds__(32, MINB) ax_dmma(int64_t E, DParam<double, 8> dp, const double* __restrict__ Gs,
                                                     const double* __restrict__ Bm, double lambda,
                                                     const double* __restrict__ u, double* __restrict__ w,
-                                                    const int* __restrict__ skip_flag, double* __restrict__ dot_out) {
+                                                    const int* __restrict__ skip_flag, double* __restrict__ dot_out,
+                                                    int u_keep) {
     using SM = DmmaSmem<NS>;
     constexpr int P = 8, P2 = 64, P3 = 512, SLAB = 6 * 64;
     constexpr uint32_t GBYTES = SLAB * sizeof(double), UBYTES = P3 * sizeof(double);
@@ -480,7 +481,7 @@ __global__ void __launch_bounds__(32, MINB) ax_dmma(int64_t E, DParam<double, 8>
     __syncwarp();
     if (lane == 0 && nmine > 0) {
         pol_g = policy_evict_first();
-        pol_u = policy_evict_last();
+        pol_u = u_keep ? policy_evict_last() : policy_evict_first();
         issue_u(0);
         int gk = 0;
         for (int q = 0; q < NS && gleft > 0; ++q) {
@@ -611,7 +612,7 @@ __global__ void __launch_bounds__(32, MINB) ax_dmma_many(int64_t E, DParam<doubl
                                                          const double* __restrict__ Bm, double lambda,
                                                          const double* __restrict__ u, double* __restrict__ w,
                                                          int64_t stride, const int* __restrict__ skip_flag,
-                                                         double* __restrict__ dot_out, int64_t dot_stride) {
+                                                         double* __restrict__ dot_out, int64_t dot_stride, int u_keep) {
     using SM = DmmaManySmem<NF, NS>;
     constexpr int P = 8, P2 = 64, P3 = 512, SLAB = 6 * 64;
     constexpr uint32_t GBYTES = SLAB * sizeof(double), UBYTES = P3 * sizeof(double);
@@ -642,7 +643,7 @@ __global__ void __launch_bounds__(32, MINB) ax_dmma_many(int64_t E, DParam<doubl
     __syncwarp();
     if (lane == 0 && nmine > 0) {
         pol_g = policy_evict_first();
-        pol_u = policy_evict_last();
+        pol_u = u_keep ? policy_evict_last() : policy_evict_first();
         issue_u(0);
         int gk = 0;
         for (int q = 0; q < NS && gleft > 0; ++q) {
@@ -800,18 +801,29 @@ int resident_blocks(sem_ctx* c, K kern, int threads, size_t smem, int* out) {
     return SEM_OK;
 }
 
+// u is loaded with the L2 evict-last policy only when a field is small enough to survive in L2 until its next use (config
+// 2: the next application, or the next kernel of a PCG iteration, finds it there); a field that streams anyway must not
+// crowd out the w values the gather-scatter is about to re-read
+inline int u_keep(const sem_ctx* c, size_t bytes_per_node) { return (size_t)c->nL * bytes_per_node <= ((size_t)40 << 20); }
+
+// element range of this launch: everything, or the chunk sem_launch_ax_gs is working on (whole element groups)
+struct ElemRange { int64_t e0, ne; };
+inline ElemRange elem_range(const sem_ctx* c) { return c->rng_ne > 0 ? ElemRange{c->rng_e0, c->rng_ne} : ElemRange{0, c->E}; }
+
 template <typename T, int P, bool RECOMP>
 int launch_simple(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, double* dot) {
-    constexpr int EPB = epb_of<P>();
-    const int64_t ngroups = (c->E + EPB - 1) / EPB;
-    const T* Gs = sizeof(T) == 8 ? (const T*)c->d_G : (const T*)c->d_G32;
-    const T* Bm = sizeof(T) == 8 ? (const T*)c->d_B : (const T*)c->d_B32;
+    constexpr int EPB = epb_of<P>(), P3 = P * P * P;
+    const ElemRange r = elem_range(c);                   // a sub-range of whole element groups, or everything
+    const int64_t ngroups = (r.ne + EPB - 1) / EPB;
     const int64_t slab = sizeof(T) == 8 ? c->slab_f64 : c->slab_f32;
+    const T* Gs = (sizeof(T) == 8 ? (const T*)c->d_G : (const T*)c->d_G32) + (r.e0 / EPB) * P * EPB * slab;
+    const T* Bm = sizeof(T) == 8 ? (const T*)c->d_B : (const T*)c->d_B32;
     const unsigned grid = (unsigned)(ngroups < (int64_t)c->num_sms * 32 ? ngroups : (int64_t)c->num_sms * 32);
     const DParam<T, P> dp = make_dparam<T, P>(c);
     const Gll1D gll = make_gll(c);
-    ax_simple<T, P, RECOMP><<<grid, threads_of<P>(), 0, c->stream>>>(c->E, dp, gll, slab, Gs, c->d_vert,
-                                                                    lambda != T(0) ? Bm : nullptr, lambda, u, w, skip, dot);
+    ax_simple<T, P, RECOMP><<<grid, threads_of<P>(), 0, c->stream>>>(
+        r.ne, dp, gll, slab, Gs, c->d_vert + r.e0 * 24, lambda != T(0) ? Bm + r.e0 * P3 : nullptr, lambda, u + r.e0 * P3,
+        w + r.e0 * P3, skip, dot);
     SEM_CUDA_OK(c, cudaGetLastError());
     return SEM_OK;
 }
@@ -819,9 +831,10 @@ int launch_simple(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, doubl
 template <typename T, int P, int NS, int MINB>
 int launch_stream(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, double* dot) {
     using SM = StreamSmem<T, P, NS>;
-    constexpr int EPB = epb_of<P>();
-    const int64_t ngroups = (c->E + EPB - 1) / EPB;
-    const T* Gs = sizeof(T) == 8 ? (const T*)c->d_G : (const T*)c->d_G32;
+    constexpr int EPB = epb_of<P>(), P3 = P * P * P;
+    const ElemRange r = elem_range(c);
+    const int64_t ngroups = (r.ne + EPB - 1) / EPB;
+    const T* Gs = (sizeof(T) == 8 ? (const T*)c->d_G : (const T*)c->d_G32) + (r.e0 / EPB) * P * EPB * SM::SLAB;
     const T* Bm = sizeof(T) == 8 ? (const T*)c->d_B : (const T*)c->d_B32;
     const DParam<T, P> dp = make_dparam<T, P>(c);
     const size_t smem = sizeof(SM) + 128;
@@ -830,8 +843,8 @@ int launch_stream(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, doubl
     if (int rc = resident_blocks(c, kern, threads_of<P>(), smem, &blocks_per_sm)) return rc;
     const int64_t cap = (int64_t)c->num_sms * blocks_per_sm;
     const unsigned grid = (unsigned)(ngroups < cap ? ngroups : cap);
-    kern<<<grid, threads_of<P>(), smem, c->stream>>>(c->E, dp, Gs, lambda != T(0) ? Bm : (const T*)nullptr, lambda, u, w,
-                                                     skip, dot);
+    kern<<<grid, threads_of<P>(), smem, c->stream>>>(r.ne, dp, Gs, lambda != T(0) ? Bm + r.e0 * P3 : (const T*)nullptr,
+                                                     lambda, u + r.e0 * P3, w + r.e0 * P3, skip, dot, u_keep(c, sizeof(T)));
     SEM_CUDA_OK(c, cudaGetLastError());
     return SEM_OK;
 }
@@ -844,10 +857,12 @@ int launch_dmma(sem_ctx* c, const double* u, double* w, double lambda, const int
     auto kern = ax_dmma<NS, MINB>;
     int blocks_per_sm = 0;
     if (int rc = resident_blocks(c, kern, 32, smem, &blocks_per_sm)) return rc;
+    const ElemRange r = elem_range(c);
     const int64_t cap = (int64_t)c->num_sms * blocks_per_sm;
-    const unsigned grid = (unsigned)(c->E < cap ? c->E : cap);
-    kern<<<grid, 32, smem, c->stream>>>(c->E, dp, c->d_G, lambda != 0.0 ? c->d_B : (const double*)nullptr, lambda, u, w,
-                                        skip, dot);
+    const unsigned grid = (unsigned)(r.ne < cap ? r.ne : cap);
+    kern<<<grid, 32, smem, c->stream>>>(r.ne, dp, c->d_G + r.e0 * (8 * 6 * 64),
+                                        lambda != 0.0 ? c->d_B + r.e0 * 512 : (const double*)nullptr, lambda,
+                                        u + r.e0 * 512, w + r.e0 * 512, skip, dot, u_keep(c, 8));
     SEM_CUDA_OK(c, cudaGetLastError());
     return SEM_OK;
 }
@@ -865,7 +880,7 @@ int launch_dmma_many(sem_ctx* c, const double* u, double* w, int64_t stride, dou
     const int64_t cap = (int64_t)c->num_sms * blocks_per_sm;
     const unsigned grid = (unsigned)(c->E < cap ? c->E : cap);
     kern<<<grid, 32, smem, c->stream>>>(c->E, dp, c->d_G, lambda != 0.0 ? c->d_B : (const double*)nullptr, lambda, u, w,
-                                        stride, skip, dot, dot_stride);
+                                        stride, skip, dot, dot_stride, u_keep(c, 8 * NF));
     SEM_CUDA_OK(c, cudaGetLastError());
     return SEM_OK;
 }
@@ -931,8 +946,24 @@ int sem_launch_ax(sem_ctx* c, const void* u, void* w, sem_prec prec, double lamb
 int sem_launch_ax_gs(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda, double* dot_out,
                      const int* skip_flag) {
     int rc;
-    if ((rc = sem_launch_ax(c, u, w, prec, lambda, dot_out, skip_flag))) return rc;
-    return sem_launch_gs(c, w, prec, true, skip_flag);
+    const int nch = (int)c->chunk_e0.size() - 1;
+    if (nch < 2) {
+        if ((rc = sem_launch_ax(c, u, w, prec, lambda, dot_out, skip_flag))) return rc;
+        return sem_launch_gs(c, w, prec, true, skip_flag);
+    }
+    // The field does not fit in L2 (the gather-scatter then runs at 2x its bytes in DRAM sectors):
+    // operator and gather-scatter alternate chunk by chunk.  The records are sorted by the element group of a node's LAST
+    // copy, so the records of chunk q only touch values written by chunks <= q, a few tens of MB ago: still in L2 for any
+    // element order with locality (every box mesh in lexicographic order; not config 5's scrambled order).
+    for (int q = 0; q < nch; ++q) {
+        c->rng_e0 = c->chunk_e0[q];
+        c->rng_ne = c->chunk_e0[q + 1] - c->chunk_e0[q];
+        rc = sem_launch_ax(c, u, w, prec, lambda, dot_out, skip_flag);
+        c->rng_ne = 0;
+        if (rc) return rc;
+        if ((rc = sem_launch_gs_range(c, w, prec, true, skip_flag, q))) return rc;
+    }
+    return SEM_OK;
 }
 
 // NEXT-4: the operator on nf fields (u + f * stride -> w + f * stride).  FP64 p = 8 with stored G and 16-byte aligned

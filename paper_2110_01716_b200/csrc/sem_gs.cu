@@ -122,9 +122,8 @@ __global__ void __launch_bounds__(NT, 4) k_gs_records_many(int32_t n_pair, const
 
 }  // namespace
 
-int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask, const int* skip_flag) {
-    const bool m = apply_mask && c->has_mask;
-    const int32_t np = (int32_t)c->n_pair, nq = (int32_t)c->n_quad, nb = (int32_t)c->n_big;
+static int launch_records(sem_ctx* c, void* w, sem_prec prec, bool m, const int* skip_flag, int32_t p0, int32_t np,
+                          int32_t q0, int32_t nq, int32_t b0, int32_t nb) {
     if (np + nq + nb == 0) return SEM_OK;
     // one wave of CTAs (8 x 256 threads per SM), fewer when there is less than one row of PPT pairs per thread
     const double ops = 4.0 * np + 8.0 * nq + 16.0 * nb;
@@ -133,13 +132,25 @@ int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask, const int
     if (blocks > cap) blocks = cap;
     blocks = (blocks + c->num_sms - 1) / c->num_sms * c->num_sms;      // same number of CTAs on every SM
 #define SEM_GS_LAUNCH(T, M)                                                                                      \
-    k_gs_records<T, M><<<(unsigned)blocks, NT, 0, c->stream>>>(np, c->d_own_pair, nq, c->d_own_quad, nb,          \
-                                                                c->d_own_big, c->d_sh_idx, (T*)w, skip_flag)
+    k_gs_records<T, M><<<(unsigned)blocks, NT, 0, c->stream>>>(np, c->d_own_pair + p0, nq, c->d_own_quad + q0, nb, \
+                                                                c->d_own_big + b0, c->d_sh_idx, (T*)w, skip_flag)
     if (prec == SEM_F64) { if (m) SEM_GS_LAUNCH(double, true); else SEM_GS_LAUNCH(double, false); }
     else { if (m) SEM_GS_LAUNCH(float, true); else SEM_GS_LAUNCH(float, false); }
 #undef SEM_GS_LAUNCH
     SEM_CUDA_OK(c, cudaGetLastError());
     return SEM_OK;
+}
+
+int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask, const int* skip_flag) {
+    return launch_records(c, w, prec, apply_mask && c->has_mask, skip_flag, 0, (int32_t)c->n_pair, 0, (int32_t)c->n_quad, 0,
+                          (int32_t)c->n_big);
+}
+
+// the records owned by the element groups of chunk `chunk` (sem_ctx::chunk_e0 / chunk_rec)
+int sem_launch_gs_range(sem_ctx* c, void* w, sem_prec prec, bool apply_mask, const int* skip_flag, int chunk) {
+    const int32_t *P = c->chunk_rec[0].data(), *Q = c->chunk_rec[1].data(), *B = c->chunk_rec[2].data();
+    return launch_records(c, w, prec, apply_mask && c->has_mask, skip_flag, P[chunk], P[chunk + 1] - P[chunk], Q[chunk],
+                          Q[chunk + 1] - Q[chunk], B[chunk], B[chunk + 1] - B[chunk]);
 }
 
 // nf = 2, 3 or 4 fields at w + f * stride (values of T) in one launch

@@ -4,6 +4,7 @@
 #include <stdint.h>
 
 #include <string>
+#include <vector>
 
 #include "../../include/sem.h"
 
@@ -53,6 +54,11 @@ struct sem_ctx {
     int4* d_own_quad = nullptr;
     int2* d_own_big = nullptr;
     int64_t n_pair = 0, n_quad = 0, n_big = 0;
+    // chunks of whole element groups for fields that do not fit in L2 (empty: no chunking): element bounds and, per
+    // record class, the first record owned by each chunk (records are sorted by owner group)
+    std::vector<int64_t> chunk_e0;
+    std::vector<int32_t> chunk_rec[3];
+    int64_t rng_e0 = 0, rng_ne = 0;          // element range of the Ax launch in flight (sem_launch_ax_gs), 0 = all
     // Dirichlet (S14)
     bool has_mask = false;
     uint8_t* d_mask_u = nullptr;   // [U] 1 = masked unique node
@@ -133,6 +139,7 @@ int sem_launch_ax_many(sem_ctx* c, const void* u, void* w, int nf, int64_t strid
                        double* dot_out, int64_t dot_stride, const int* skip_flag);
 // sem_gs.cu
 int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask, const int* skip_flag = nullptr);
+int sem_launch_gs_range(sem_ctx* c, void* w, sem_prec prec, bool apply_mask, const int* skip_flag, int chunk);
 int sem_launch_gs_many(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec prec, bool apply_mask,
                        const int* skip_flag = nullptr);
 // sem_api.cu

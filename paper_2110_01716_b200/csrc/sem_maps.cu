@@ -4,6 +4,8 @@
 //   seg_idx = local indices ordered by (gid, l) ascending, i.e. a STABLE sort of l by gid.
 // All integer work, bit-exact.  The sort and the scans are CUB device primitives (setup, untimed); everything on
 // the timed path (sem_gs.cu) is hand-written.
+#include <stdlib.h>
+
 #include <cub/cub.cuh>
 
 #include "sem_internal.h"
@@ -359,6 +361,27 @@ int sem_build_gs_records(sem_ctx* c) {
                                        cudaMemcpyDeviceToHost, st));
     SEM_CUDA_OK(c, cudaStreamSynchronize(st));
     c->n_pair = h_tot[0]; c->n_quad = h_tot[1]; c->n_big = h_tot[2];
+    // chunks for fields larger than L2: 64 MB of FP64 field per chunk (measured best at 64^3 elements, N = 7: 48-64 MB;
+    // smaller chunks pay the operator's ramp and tail per launch), only when there are at least 2 of them
+    c->chunk_e0.clear();
+    for (int cls = 0; cls < 3; ++cls) c->chunk_rec[cls].clear();
+    {
+        int64_t cg = (int64_t)((64.0 * 1024 * 1024) / (8.0 * group_nodes));
+        if (cg < 1) cg = 1;
+        if (const char* env = getenv("SEM_CHUNK_GROUPS")) cg = atoll(env) > 0 ? atoll(env) : (int64_t)ng + 1;   // tests
+        const int64_t nch = (ng + cg - 1) / cg;
+        if (nch >= 2) {
+            for (int64_t q = 0; q <= nch; ++q) {
+                const int64_t g0 = q * cg < ng ? q * cg : ng;
+                c->chunk_e0.push_back(g0 * c->epb < c->E ? g0 * c->epb : c->E);
+                for (int cls = 0; cls < 3; ++cls) {
+                    int32_t off = 0;
+                    SEM_CUDA_OK(c, cudaMemcpy(&off, d_offc + cls * ((int64_t)ng + 1) + g0, sizeof(int32_t), cudaMemcpyDeviceToHost));
+                    c->chunk_rec[cls].push_back(off);
+                }
+            }
+        }
+    }
     SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_own_pair, (size_t)(c->n_pair ? c->n_pair : 1) * sizeof(int2)));
     SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_own_quad, (size_t)(c->n_quad ? c->n_quad : 1) * sizeof(int4)));
     SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_own_big, (size_t)(c->n_big ? c->n_big : 1) * sizeof(int2)));

@@ -521,3 +521,38 @@ def test_sharded_apply_emulated_on_one_gpu(torch_cuda, binding, oracle_mod, worl
     finally:
         for s in shards:
             s.close()
+
+
+# --------------------------------------------------------------------------- fields larger than L2: chunked Ax / gs
+@pytest.mark.parametrize("N,dtype", [(7, "f64"), (3, "f32"), (4, "f64"), (2, "f64")])
+def test_chunked_ax_gs_is_bit_identical(torch_cuda, binding, oracle_mod, monkeypatch, N, dtype):
+    """When the field does not fit in L2, sem_ax_gs alternates operator and gather-scatter chunk by chunk (records are
+    sorted by the owner group of a node's last copy).  Forced here on a small scrambled mesh through SEM_CHUNK_GROUPS:
+    the result is bit-identical to the un-chunked path, equals the oracle, and the PCG loop (fused dot, skip flag) runs
+    through it unchanged."""
+    import os
+    m = inputs.box_mesh(6, 5, 4, N, "random", seed=4, permute_seed=9)
+    u = inputs.field_uniform(m.gid, 5)
+    ow = _ax_gs_oracle(oracle_mod, m, u, True)
+    tdt = torch_cuda.float64 if dtype == "f64" else torch_cuda.float32
+    outs, its, xs = [], [], []
+    for chunk in (None, "3", "7"):
+        if chunk is None:
+            monkeypatch.delenv("SEM_CHUNK_GROUPS", raising=False)
+        else:
+            monkeypatch.setenv("SEM_CHUNK_GROUPS", chunk)
+        with binding.Sem(m.E, m.N, m.vert, m.gid, m.dirichlet) as sem:
+            sem.geom()
+            du = to_dev(torch_cuda, u.ravel(), tdt)
+            dw = torch_cuda.full_like(du, float("nan"))
+            sem.ax_gs(du, dw)
+            torch_cuda.cuda.synchronize()
+            outs.append(dw.clone())
+            if dtype == "f64":
+                b = dw.clone()
+                x = torch_cuda.zeros_like(b)
+                its.append(sem.pcg(b, x, 1e-10, 300)[0])
+                xs.append(x.cpu().numpy())
+    assert relerr(outs[0].cpu().numpy(), ow) <= (TOL64 if dtype == "f64" else TOL32)
+    assert torch_cuda.equal(outs[1], outs[0]) and torch_cuda.equal(outs[2], outs[0])
+    assert len(set(its)) <= 1 and all(relerr(x, xs[0]) <= 1e-9 for x in xs[1:])
