@@ -10,7 +10,7 @@
 //     (cp.async.bulk + mbarrier transaction counts, evict-first in L2) issued NS slabs ahead, so the bytes in flight per
 //     SM do not depend on registers or occupancy;  u arrives the same way, double-buffered per element;
 //   * persistent CTAs (one element group at a time, grid = SMs x resident CTAs) write w straight from registers.
-// ax_simple is the plain-load version of the same arithmetic: odd p, unaligned pointers, and the recomputed-G
+// ax_simple is the plain-load version of the same arithmetic: p > 12, unaligned pointers, and the recomputed-G
 // variant (a9: G from the 8 trilinear vertices inside the kernel) use it.
 #include <mutex>
 #include <type_traits>
@@ -286,12 +286,15 @@ __global__ void __launch_bounds__(threads_of<P>()) ax_simple(int64_t E, DParam<T
 
 // ---------------------------------------------------------------------------------------------------------------
 // ax_stream: persistent CTAs, G slabs and u elements arrive by bulk async copies into shared-memory rings.
-// Requires even P (so every chunk is a multiple of 16 bytes) and 16-byte aligned u.
+// Any P <= 12 and 16-byte aligned u.  The G slabs are padded to 16 bytes (sem_geom.cu) and always arrive by bulk copies;
+// u arrives by bulk copies when an element block is a multiple of 16 bytes (even p), by plain loads otherwise (odd p).
 //
 template <typename T, int P, int NS>
 struct StreamSmem {
     static constexpr int EPB = epb_of<P>(), P2 = P * P, P3 = P2 * P;
-    static constexpr int SLAB = 6 * P2;                      // values per element slab
+    // values per element slab, padded to 16 bytes (sem_geom.cu: slab_f64 / slab_f32): only FP32 with odd p needs the pad
+    static constexpr int SLAB = 6 * P2 + ((6 * P2 * (int)sizeof(T)) % 16 ? 2 : 0);
+    static constexpr bool UBULK = (P3 * (int)sizeof(T)) % 16 == 0;   // element blocks of u are 16-byte multiples: bulk copies
     alignas(128) T g[NS][EPB * SLAB];
     alignas(128) T u[2][EPB * P3];
     alignas(16) T sgr[2][EPB * P2];
@@ -320,6 +323,7 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
     const int ij = lane_ok ? tid % P2 : 0;
     const int j = ij / P, i = ij % P;
 
+    constexpr bool UBULK = SM::UBULK;               // odd p: u arrives by plain loads (its blocks are not 16-byte multiples)
     const int64_t ngroups = (E + EPB - 1) / EPB;
     const int64_t nmine = blockIdx.x < ngroups ? (ngroups - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
     const int tail_n = (int)(E - (ngroups - 1) * EPB);          // elements of the globally last group
@@ -348,7 +352,7 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
     if (tid == 0 && nmine > 0) {
         pol_g = policy_evict_first();
         pol_u = u_keep ? policy_evict_last() : policy_evict_first();
-        issue_u(0);
+        if (UBULK) issue_u(0);
         int gk = 0;
         for (int q = 0; q < NS && gleft > 0; ++q) {
             mbar_expect_tx(&sm.gfull[q], GBYTES);
@@ -357,7 +361,7 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
             if (++gk == P) { gk = 0; gsrc += gjump; }
             --gleft;
         }
-        if (nmine > 1) issue_u(1);
+        if (UBULK && nmine > 1) issue_u(1);
     }
     DRows<T, P> dr;
     dr.init_shared(sm.D, i, j);
@@ -370,12 +374,24 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
     int64_t grp = blockIdx.x;
     for (int64_t n = 0; n < nmine; ++n, grp += gridDim.x, wdst += wstep) {
         const bool ok = (FULL && EPB == 1) ? true : (lane_ok && grp * EPB + slot < E);
-        const int ub = (int)(n & 1);
-        mbar_wait(&sm.ufull[ub], (uint32_t)((n >> 1) & 1));
+        const int ub = UBULK ? (int)(n & 1) : 0;
         const T* sue = &sm.u[ub][slot * P3];
         T uk[P], wk[P];
+        if constexpr (UBULK) {
+            mbar_wait(&sm.ufull[ub], (uint32_t)((n >> 1) & 1));
 #pragma unroll
-        for (int k = 0; k < P; ++k) { uk[k] = sue[k * P2 + ij]; wk[k] = T(0); }
+            for (int k = 0; k < P; ++k) { uk[k] = sue[k * P2 + ij]; wk[k] = T(0); }
+        } else {
+            // (every thread passed the barrier after part 1 of the previous group's last slab: its u is no longer read)
+            const T* usrc = u + (grp * EPB + slot) * P3 + ij;
+#pragma unroll
+            for (int k = 0; k < P; ++k) {
+                uk[k] = ok ? usrc[k * P2] : T(0);
+                wk[k] = T(0);
+                if (FULL || lane_ok) sm.u[0][slot * P3 + k * P2 + ij] = uk[k];
+            }
+            __syncthreads();
+        }
 #pragma unroll
         for (int k = 0; k < P; ++k) {
             mbar_wait(&sm.gfull[q], gphase);
@@ -396,7 +412,7 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
                     if ((k + NS) % P == P - 1) gsrc += gjump;     // that was the last slab of its group
                     --gleft;
                 }
-                if (k == P - 1 && n + 2 < nmine) issue_u(n + 2);
+                if (UBULK && k == P - 1 && n + 2 < nmine) issue_u(n + 2);
             }
             wk[k] += slab_part2<T, P>(dr, i, j, &sm.sgr[buf][slot * P2], &sm.sgs[buf][slot * P2]);
             if (++q == NS) { q = 0; gphase ^= 1u; }
@@ -898,7 +914,15 @@ template <> struct StreamCfg<float, 6> { static constexpr int NS = 6, MINB = 6; 
 template <> struct StreamCfg<double, 10> { static constexpr int NS = 4, MINB = 3; };
 template <> struct StreamCfg<float, 10> { static constexpr int NS = 6, MINB = 4; };
 
-template <int P> constexpr bool stream_ok() { return P % 2 == 0 && P <= 12; }
+template <int P> constexpr bool stream_ok() { return P <= 12; }
+template <> struct StreamCfg<double, 9> { static constexpr int NS = 4, MINB = 4; };
+template <> struct StreamCfg<float, 9> { static constexpr int NS = 6, MINB = 5; };
+template <> struct StreamCfg<double, 7> { static constexpr int NS = 4, MINB = 4; };
+template <> struct StreamCfg<float, 7> { static constexpr int NS = 5, MINB = 6; };
+template <> struct StreamCfg<double, 5> { static constexpr int NS = 4, MINB = 6; };
+template <> struct StreamCfg<float, 5> { static constexpr int NS = 4, MINB = 8; };
+template <> struct StreamCfg<double, 3> { static constexpr int NS = 3, MINB = 8; };
+template <> struct StreamCfg<float, 3> { static constexpr int NS = 3, MINB = 8; };
 
 template <typename T, int P>
 int dispatch_p(sem_ctx* c, const void* u, void* w, double lambda, const int* skip, double* dot) {
