@@ -547,7 +547,7 @@ def main():
     ap.add_argument("--sharded-n", type=int, default=0,
                     help="NEXT-4: > 0 runs the element-partitioned operator on a config-5 style mesh of n^3 elements")
     ap.add_argument("--max-n", type=int, default=64)
-    ap.add_argument("--orders", default="3,5,7,9")
+    ap.add_argument("--orders", default="3,5,7,8,9")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
