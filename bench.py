@@ -721,6 +721,16 @@ def main():
                 mg.set_smoother(binding.SEM_SMOOTH_CHEBY_SCHWARZ, [0.1 * l for l in lams], lams)
                 mg.fpcg(rhs, x, 1e-8, 3)
                 (it_s, rel_s), ms_s = wall(lambda: mg.fpcg(rhs, x, 1e-8, 200))
+                # the restricted variant: one fused kernel per application, no exchange after the local solve
+                lamr = [1.1 * lv[0].lambda_max_schwarz(1, 30), 1.1 * lv[1].lambda_max_schwarz(1, 30), lam[2]]
+                mg.set_smoother(binding.SEM_SMOOTH_CHEBY_RAS, [0.1 * l for l in lamr], lamr)
+                mg.fpcg(rhs, x, 1e-8, 3)
+                (it_r, rel_r), ms_r = wall(lambda: mg.fpcg(rhs, x, 1e-8, 200))
+            # Schwarz is the stronger smoother: one Chebyshev step per smoothing (order 1) is its best cycle here
+            with binding.Pmg(lv, [0.1 * l for l in lam], lam, 1, 8, binding.SEM_F32) as mg1:
+                mg1.set_smoother(binding.SEM_SMOOTH_CHEBY_RAS, [0.1 * l for l in lamr], lamr)
+                mg1.fpcg(rhs, x, 1e-8, 3)
+                (it_r1, rel_r1), ms_r1 = wall(lambda: mg1.fpcg(rhs, x, 1e-8, 200))
             r32 = rhs.float()
             z32 = torch.empty_like(r32)
             us_sw = event_time_us(torch, lambda: lv[0].schwarz(r32, z32), 300)
@@ -735,6 +745,12 @@ def main():
                      "pmg_fcg": {"smoother": "Chebyshev-Jacobi", "iters": it_m, "relres": rel_m, "ms": ms_m},
                      "pmg_fcg_schwarz": {"smoother": "Chebyshev-accelerated additive Schwarz (NEXT-2b) on N = 7, 3",
                                          "iters": it_s, "relres": rel_s, "ms": ms_s, "setup_ms": ms_setup},
+                     "pmg_fcg_ras": {"smoother": "Chebyshev-accelerated restricted additive Schwarz on N = 7, 3 (fused: "
+                                                 "gather, Eq. (3), weighted own part in one kernel)",
+                                     "iters": it_r, "relres": rel_r, "ms": ms_r},
+                     "pmg_fcg_ras_order1": {"smoother": "the same with smoother order 1 (one RAS application before and "
+                                                        "after the coarse correction)",
+                                            "iters": it_r1, "relres": rel_r1, "ms": ms_r1},
                      "schwarz_apply_f32": {"us_asm": us_sw, "us_ras": us_ras, "algorithmic_GBs": sw_bytes / us_sw / 1e3,
                                            "frac_of_measured_hbm_peak": sw_bytes / us_sw / 1e3 / peak,
                                            "what": "sem_schwarz at E = 7200, N = 7 (10^3 blocks): extension gather, "

@@ -150,25 +150,27 @@ int run_schwarz(sem_ctx* c, const T* b, T* x, int order, double lmin, double lma
     const double theta = 0.5 * (lmax + lmin), delta = 0.5 * (lmax - lmin), sigma = theta / delta;
     double rho = 1.0 / sigma;
     int rc;
-    const T* q = nullptr;
+    // S is applied out of place (its restricted variant is then one fused kernel): t receives S(.)
+    T* t = (T*)c->d_cheb4;
     if (!zero_guess) {
         if ((rc = sem_launch_ax_gs(c, x, w, prec, c->lambda, nullptr, nullptr))) return rc;      // x is masked on entry
-        q = w;
+        k_pc_resid<T><<<grid, 256, 0, st>>>(n, b, w, w);                                           // w = b - A x
+        if ((rc = sem_launch_schwarz(c, w, r, prec, kind))) return rc;                             // r = S (b - A x)
+    } else {
+        if ((rc = sem_launch_schwarz(c, b, r, prec, kind))) return rc;                             // r = S b
     }
-    k_pc_resid<T><<<grid, 256, 0, st>>>(n, b, q, r);
-    if ((rc = sem_launch_schwarz(c, r, r, prec, kind))) return rc;                               // r = S (b - A x)
     if (order == 1) k_pc_first<T, true><<<grid, 256, 0, st>>>(n, r, (T)(1.0 / theta), zero_guess, x, d);
     else k_pc_first<T, false><<<grid, 256, 0, st>>>(n, r, (T)(1.0 / theta), zero_guess, x, d);
     for (int k = 1; k < order; ++k) {
         if ((rc = sem_launch_ax_gs(c, d, w, prec, c->lambda, nullptr, nullptr))) return rc;
-        if ((rc = sem_launch_schwarz(c, w, w, prec, kind))) return rc;                           // w = S A d
+        if ((rc = sem_launch_schwarz(c, w, t, prec, kind))) return rc;                           // t = S A d
         const double rho1 = 1.0 / (2.0 * sigma - rho);
         const T c1 = (T)(rho1 * rho), c2 = (T)(2.0 * rho1 / delta);
         const bool xzero = zero_guess && k == 1, last = k == order - 1;
-        if (xzero && last) k_pc_step<T, true, true><<<grid, 256, 0, st>>>(n, w, c1, c2, x, r, d);
-        else if (xzero) k_pc_step<T, true, false><<<grid, 256, 0, st>>>(n, w, c1, c2, x, r, d);
-        else if (last) k_pc_step<T, false, true><<<grid, 256, 0, st>>>(n, w, c1, c2, x, r, d);
-        else k_pc_step<T, false, false><<<grid, 256, 0, st>>>(n, w, c1, c2, x, r, d);
+        if (xzero && last) k_pc_step<T, true, true><<<grid, 256, 0, st>>>(n, t, c1, c2, x, r, d);
+        else if (xzero) k_pc_step<T, true, false><<<grid, 256, 0, st>>>(n, t, c1, c2, x, r, d);
+        else if (last) k_pc_step<T, false, true><<<grid, 256, 0, st>>>(n, t, c1, c2, x, r, d);
+        else k_pc_step<T, false, false><<<grid, 256, 0, st>>>(n, t, c1, c2, x, r, d);
         rho = rho1;
     }
     SEM_CUDA_OK(c, cudaGetLastError());
@@ -294,6 +296,7 @@ extern "C" int sem_cheby_schwarz(sem_ctx* c, const void* b, void* x, int order, 
     if (prec == SEM_F32 && c->gmode == SEM_G_STORED && (rc = sem_build_g32(c))) return rc;
     for (int q = 0; q < 3; ++q)
         if (!c->d_cheb[q]) SEM_CUDA_OK(c, cudaMalloc(&c->d_cheb[q], c->nL * sizeof(double)));
+    if (!c->d_cheb4) SEM_CUDA_OK(c, cudaMalloc(&c->d_cheb4, c->nL * sizeof(double)));
     if (prec == SEM_F64)
         return run_schwarz<double>(c, (const double*)b, (double*)x, order, lmin, lmax, zero_guess != 0, (int)kind);
     return run_schwarz<float>(c, (const float*)b, (float*)x, order, lmin, lmax, zero_guess != 0, (int)kind);

@@ -25,11 +25,11 @@ namespace {
 
 using namespace sem_fdm_dev;
 
-template <typename T, int M, int LPT, int EPC, int NST, bool SREG>
-int launch_cfg(sem_ctx* c, const void* S, const void* invL, const void* b, void* u) {
+template <typename T, int M, int LPT, int EPC, int NST, bool SREG, class IO>
+int launch_cfg(sem_ctx* c, const void* S, const void* invL, const IO io) {
     using C = fdm_cfg<T, M, LPT, EPC>;
-    constexpr size_t SMEM = C::SMEM1 * NST;
-    auto kern = SREG ? k_fdm_sreg<T, M, LPT, EPC, 1, NST> : k_fdm<T, M, LPT, EPC, 1, NST>;
+    constexpr size_t SMEM = C::SMEM1 * NST + IO::extra_bytes(EPC);
+    auto kern = SREG ? k_fdm_sreg<T, M, LPT, EPC, 1, NST, IO> : k_fdm<T, M, LPT, EPC, 1, NST, IO>;
     // CTAs per SM of this instantiation, per device (the attribute is per device too); guarded for concurrent callers
     static std::mutex mu;
     static int resident_of[SEM_MAX_DEVICES] = {};
@@ -49,7 +49,7 @@ int launch_cfg(sem_ctx* c, const void* S, const void* invL, const void* b, void*
     const int64_t ngrp = (c->E + C::EPC - 1) / C::EPC;
     int64_t grid = (int64_t)c->num_sms * resident;       // single wave of persistent CTAs (a grid cut down to equal
     if (grid > ngrp) grid = ngrp;                        // shares per CTA measured 8-10 % slower)
-    kern<<<(unsigned)grid, C::NT, SMEM, c->stream>>>(c->E, (const T*)S, (const T*)invL, (const T*)b, (T*)u);
+    kern<<<(unsigned)grid, C::NT, SMEM, c->stream>>>(c->E, (const T*)S, (const T*)invL, io);
     SEM_CUDA_OK(c, cudaGetLastError());
     return SEM_OK;
 }
@@ -59,31 +59,45 @@ int launch_cfg(sem_ctx* c, const void* S, const void* invL, const void* b, void*
 //               about 128 threads' worth of elements below; one shared-memory stage (the resident CTAs hide the
 //               copies) up to m = 11, two from m = 12 on (few CTAs fit).
 //   k_fdm_sreg: S_d resident in registers, where it measured faster: FP32 m = 8, 10, 12 and FP64 m = 8, 10.
-template <typename T, int M>
-int launch_m(sem_ctx* c, const void* S, const void* invL, const void* b, void* u) {
+template <typename T, int M, class IO>
+int launch_m(sem_ctx* c, const void* S, const void* invL, const IO io) {
     constexpr bool F32 = sizeof(T) == 4;
-    if constexpr (M == 8) return launch_cfg<T, M, 4, 2, 1, true>(c, S, invL, b, u);
-    else if constexpr (M == 10) return launch_cfg<T, M, 4, 1, 1, true>(c, S, invL, b, u);
-    else if constexpr (M == 12 && F32) return launch_cfg<T, M, 5, 1, 1, true>(c, S, invL, b, u);
+    if constexpr (M == 8) return launch_cfg<T, M, 4, 2, 1, true, IO>(c, S, invL, io);
+    else if constexpr (M == 10) return launch_cfg<T, M, 4, 1, 1, true, IO>(c, S, invL, io);
+    else if constexpr (M == 12 && F32) return launch_cfg<T, M, 5, 1, 1, true, IO>(c, S, invL, io);
     else {
         constexpr int LPT = (M >= 6 && !(!F32 && M >= 12)) ? 2 : 1;
         constexpr int TPE = (M * M + LPT - 1) / LPT;
         constexpr int EPC = (M >= 8 || 128 / TPE < 1) ? 1 : 128 / TPE;
-        constexpr int NST = M >= 12 ? 2 : 1;
-        return launch_cfg<T, M, LPT, EPC, NST, false>(c, S, invL, b, u);
+        constexpr int NST = (M >= 12 && IO::extra_bytes(1) == 0) ? 2 : 1;     // the I/O policy's area is single-staged
+        return launch_cfg<T, M, LPT, EPC, NST, false, IO>(c, S, invL, io);
     }
 }
 
 template <typename T>
 int launch(sem_ctx* c, int m, const void* S, const void* invL, const void* b, void* u) {
     switch (m) {
-#define SEM_FDM_CASE(MM) case MM: return launch_m<T, MM>(c, S, invL, b, u);
+#define SEM_FDM_CASE(MM) case MM: return launch_m<T, MM>(c, S, invL, PlainIO<T, MM>{(const T*)b, (T*)u});
         SEM_FDM_CASE(2) SEM_FDM_CASE(3) SEM_FDM_CASE(4) SEM_FDM_CASE(5) SEM_FDM_CASE(6) SEM_FDM_CASE(7) SEM_FDM_CASE(8)
         SEM_FDM_CASE(9) SEM_FDM_CASE(10) SEM_FDM_CASE(11) SEM_FDM_CASE(12) SEM_FDM_CASE(13) SEM_FDM_CASE(14)
         SEM_FDM_CASE(15) SEM_FDM_CASE(16)
 #undef SEM_FDM_CASE
     }
     return sem_fail(c, SEM_EINVAL, "sem_fdm_apply: m = %d outside 2..16", m);
+}
+
+// the restricted additive Schwarz smoother in one kernel: gather -> Eq. (3) -> weighted own part (SchwarzIO)
+template <typename T>
+int launch_schwarz(sem_ctx* c, int m, const void* S, const void* invL, const void* r, const int4* link,
+                   const int32_t* nrm, const void* W, void* z) {
+    switch (m) {
+#define SEM_FDM_CASE(MM) \
+    case MM: return launch_m<T, MM>(c, S, invL, SchwarzIO<T, MM>{(const T*)r, link, nrm, (const T*)W, (T*)z});
+        SEM_FDM_CASE(4) SEM_FDM_CASE(5) SEM_FDM_CASE(6) SEM_FDM_CASE(7) SEM_FDM_CASE(8) SEM_FDM_CASE(9) SEM_FDM_CASE(10)
+        SEM_FDM_CASE(11) SEM_FDM_CASE(12) SEM_FDM_CASE(13) SEM_FDM_CASE(14) SEM_FDM_CASE(15) SEM_FDM_CASE(16)
+#undef SEM_FDM_CASE
+    }
+    return sem_fail(c, SEM_EINVAL, "Schwarz local solve: m = %d outside 4..16", m);
 }
 
 }  // namespace
@@ -99,4 +113,11 @@ extern "C" int sem_fdm_apply(sem_ctx* ctx, int m, const void* S, const void* inv
         return sem_fail(ctx, SEM_EINVAL, "sem_fdm_apply: S, inv_lambda, b, u must be 16-byte aligned");
     if (prec == SEM_F64) return launch<double>(ctx, m, S, inv_lambda, b, u);
     return launch<float>(ctx, m, S, inv_lambda, b, u);
+}
+
+// NEXT-2b, restricted variant fused (sem_schwarz.cu): z_L = W (A~^-1 R r)|own nodes, straight from r, no block in HBM
+int sem_launch_fdm_schwarz(sem_ctx* c, int m, const void* S, const void* invL, const void* r, const int4* link,
+                           const int32_t* nrm, const void* W, void* z, sem_prec prec) {
+    if (prec == SEM_F64) return launch_schwarz<double>(c, m, S, invL, r, link, nrm, W, z);
+    return launch_schwarz<float>(c, m, S, invL, r, link, nrm, W, z);
 }

@@ -122,17 +122,112 @@ __device__ __forceinline__ void copy_rows_async(T* __restrict__ sdst, const T* _
     }
 }
 
+// Where the m^3 blocks come from and where the result goes.
+//   PlainIO    b[E][m^3] -> u[E][m^3] (sem_fdm_apply).
+//   SchwarzIO  the restricted additive Schwarz smoother in ONE kernel (NEXT-2b, sem_schwarz.cu): the block is GATHERED
+//              from the residual r -- the element's own nodes into the interior, the face neighbours' one-layer-in
+//              values into the 6 face layers through the links resolved at setup, zeros on the block's edges and corners
+//              -- by 4/8-byte cp.async straight into shared memory, and only the element's own part of the solution
+//              is written, weighted (W = 1 / multiplicity): the blocks never touch HBM.
+template <typename T, int M>
+struct PlainIO {
+    const T* b;
+    T* u;
+    static constexpr size_t extra_bytes(int) { return 0; }
+    template <int NT, int PS>
+    __device__ __forceinline__ void load(T* __restrict__ sB, unsigned char*, int64_t e0, int ne) const {
+        copy_rows_async<T, M, NT, PS>(sB, b + e0 * (M * M * M), ne * M * M);
+    }
+    __device__ __forceinline__ void store(const unsigned char*, int, int64_t e, int o, int q, T v) const {
+        u[e * (M * M * M) + o * (M * M) + q] = v;
+    }
+};
+
+template <typename T, int M>
+struct SchwarzIO {
+    const T* r;            // residual, local layout [E][p^3], p = M - 2
+    const int4* link;      // [E][6] (neighbour, base, stride a, stride b), neighbour < 0: none
+    const int32_t* nrm;    // [E][6] neighbour's face axis | side << 2
+    const T* W;            // [E][p^3] weight of the result
+    T* z;                  // [E][p^3]
+    // per element of the CTA, after the stage(s): the 6 links (int4 + int) and the element's weights (cp.async too)
+    static constexpr int P = M - 2, P3 = P * P * P;
+    static constexpr size_t EL_BYTES = 128 + ((P3 * sizeof(T) + 15) / 16) * 16;
+    static constexpr size_t extra_bytes(int epc) { return (size_t)epc * EL_BYTES; }
+    template <int NT, int PS>
+    __device__ __forceinline__ void load(T* __restrict__ sB0, unsigned char* extra, int64_t e0, int ne) const {
+        constexpr int P2 = P * P, MP = fdm_cfg<T, M, 1, 1>::MP, B_EL = M * PS;
+        for (int t = threadIdx.x; t < ne * 6; t += NT) {                               // links of the group, once
+            const int el = t / 6, f = t - el * 6;
+            int4* lk = reinterpret_cast<int4*>(extra + el * EL_BYTES);
+            int32_t* nf = reinterpret_cast<int32_t*>(extra + el * EL_BYTES + 96);
+            lk[f] = link[(e0 + el) * 6 + f];
+            nf[f] = nrm[(e0 + el) * 6 + f];
+        }
+        __syncthreads();
+        for (int el = 0; el < ne; ++el) {
+            const int64_t e = e0 + el;
+            T* sB = sB0 + el * B_EL;
+            const int4* lk6 = reinterpret_cast<const int4*>(extra + el * EL_BYTES);
+            const int32_t* nf6 = reinterpret_cast<const int32_t*>(extra + el * EL_BYTES + 96);
+            T* sW = reinterpret_cast<T*>(extra + el * EL_BYTES + 128);
+            for (int t = threadIdx.x; t < P3; t += NT) {                               // own nodes, and their weights
+                const int i = t % P, j = (t / P) % P, k = t / P2;
+                cp_async<(int)sizeof(T)>(sB + (k + 1) * PS + (j + 1) * MP + (i + 1), r + e * P3 + t);
+                cp_async<(int)sizeof(T)>(sW + t, W + e * P3 + t);
+            }
+            for (int t = threadIdx.x; t < 6 * P2; t += NT) {                           // face layers
+                const int f = t / P2, fa = (t % P2) % P, fb = (t % P2) / P, axis = f >> 1, g = (f & 1) ? M - 1 : 0;
+                const int a = axis == 0 ? g : fa + 1, b = axis == 0 ? fa + 1 : (axis == 1 ? g : fb + 1),
+                          c = axis == 2 ? g : fb + 1;
+                const int4 lk = lk6[f];
+                T* dst = sB + c * PS + b * MP + a;
+                if (lk.x >= 0) {
+                    const int nf = nf6[f], na = nf & 3, ns = nf >> 2;
+                    const int stride = na == 0 ? 1 : (na == 1 ? P : P2);
+                    const int l = lk.y + fa * lk.z + fb * lk.w + (ns ? -stride : stride);
+                    cp_async<(int)sizeof(T)>(dst, r + (int64_t)lk.x * P3 + l);
+                } else {
+                    *dst = T(0);
+                }
+            }
+            for (int t = threadIdx.x; t < 12 * P + 8; t += NT) {                       // edges and corners: no node
+                int a, b, c;
+                if (t < 12 * P) {
+                    const int ed = t / P, q = t % P + 1, ax = ed >> 2, s0 = (ed & 1) ? M - 1 : 0, s1 = (ed & 2) ? M - 1 : 0;
+                    a = ax == 0 ? q : s0;
+                    b = ax == 1 ? q : (ax == 0 ? s0 : s1);
+                    c = ax == 2 ? q : s1;
+                } else {
+                    const int cn = t - 12 * P;
+                    a = (cn & 1) ? M - 1 : 0; b = (cn & 2) ? M - 1 : 0; c = (cn & 4) ? M - 1 : 0;
+                }
+                sB[c * PS + b * MP + a] = T(0);
+            }
+        }
+    }
+    __device__ __forceinline__ void store(const unsigned char* extra, int el, int64_t e, int o, int q, T v) const {
+        const int j = q / M, i = q - j * M;
+        if (o >= 1 && o <= P && j >= 1 && j <= P && i >= 1 && i <= P) {
+            const int l = ((o - 1) * P + (j - 1)) * P + (i - 1);
+            const T* sW = reinterpret_cast<const T*>(extra + el * EL_BYTES + 128);
+            z[e * P3 + l] = sW[l] * v;
+        }
+    }
+};
+
 // MINB = resident CTAs per SM the register allocation is held to.  NSTAGE = 2: two shared-memory stages of
 // {S, Lambda^-1, block}: while a group of EPC elements is worked on in one stage, the next group's operands land in the
 // other (cp.async).  NSTAGE = 1: one stage (half the shared memory, twice the resident CTAs hide the copy instead).
-template <typename T, int M, int LPT_, int EPC_, int MINB, int NSTAGE>
+template <typename T, int M, int LPT_, int EPC_, int MINB, int NSTAGE, class IO = PlainIO<T, M>>
 __global__ void __launch_bounds__((fdm_cfg<T, M, LPT_, EPC_>::NT), MINB)
-k_fdm(int64_t E, const T* __restrict__ S, const T* __restrict__ invL, const T* b, T* u) {
+k_fdm(int64_t E, const T* __restrict__ S, const T* __restrict__ invL, const IO io) {
     using C = fdm_cfg<T, M, LPT_, EPC_>;
     constexpr int MP = C::MP, LPT = C::LPT, TPE = C::TPE, EPC = C::EPC, M2 = M * M, M3 = M * M * M, NT = C::NT;
     constexpr int STG = C::STAGE, PS = C::PS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T* smem = reinterpret_cast<T*>(smem_raw);
+    unsigned char* xtra = smem_raw + sizeof(T) * (size_t)(NSTAGE * STG);     // the I/O policy's own area (one stage only)
     const int el = threadIdx.x / TPE, tl = threadIdx.x - el * TPE;
     const int64_t ngrp = (E + EPC - 1) / EPC;
 
@@ -142,7 +237,7 @@ k_fdm(int64_t E, const T* __restrict__ S, const T* __restrict__ invL, const T* b
         T* st = smem + stage * STG;
         copy_rows_async<T, M, NT, M * MP>(st, S + e0 * 3 * M2, ne * 3 * M);
         copy_rows_async<T, M, NT, PS>(st + EPC * C::S_EL, invL + e0 * M3, ne * M2);
-        copy_rows_async<T, M, NT, PS>(st + EPC * (C::S_EL + C::B_EL), b + e0 * M3, ne * M2);
+        io.template load<NT, PS>(st + EPC * (C::S_EL + C::B_EL), xtra, e0, ne);
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
 
@@ -208,7 +303,7 @@ k_fdm(int64_t E, const T* __restrict__ S, const T* __restrict__ invL, const T* b
         __syncthreads();
         // ---- phase 5: S_z on k-lines, u to global (coalesced) ----
         contract_lines<T, M, LPT, false>(sS + 2 * M * MP, ld_outer, [&](int r, int o, T x) {
-            if (live && ok[r]) u[e * M3 + o * M2 + q[r]] = x;
+            if (live && ok[r]) io.store(xtra, el, e, o, q[r], x);
         });
     }
 }
@@ -238,14 +333,15 @@ __device__ __forceinline__ void apply_matrix(const T (&Sr)[M][fdm_cfg<T, M, 1, 1
     }
 }
 
-template <typename T, int M, int LPS, int EPC_, int MINB, int NSTAGE>
+template <typename T, int M, int LPS, int EPC_, int MINB, int NSTAGE, class IO = PlainIO<T, M>>
 __global__ void __launch_bounds__((fdm_cfg<T, M, LPS, EPC_>::NT), MINB)
-k_fdm_sreg(int64_t E, const T* __restrict__ S, const T* __restrict__ invL, const T* b, T* u) {
+k_fdm_sreg(int64_t E, const T* __restrict__ S, const T* __restrict__ invL, const IO io) {
     using C = fdm_cfg<T, M, LPS, EPC_>;
     constexpr int MP = C::MP, TPE = C::TPE, EPC = C::EPC, M2 = M * M, M3 = M * M * M, NT = C::NT;
     constexpr int STG = C::STAGE, PS = C::PS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T* smem = reinterpret_cast<T*>(smem_raw);
+    unsigned char* xtra = smem_raw + sizeof(T) * (size_t)(NSTAGE * STG);     // the I/O policy's own area (one stage only)
     const int el = threadIdx.x / TPE, tl = threadIdx.x - el * TPE;
     const int64_t ngrp = (E + EPC - 1) / EPC;
 
@@ -255,7 +351,7 @@ k_fdm_sreg(int64_t E, const T* __restrict__ S, const T* __restrict__ invL, const
         T* st = smem + stage * STG;
         copy_rows_async<T, M, NT, M * MP>(st, S + e0 * 3 * M2, ne * 3 * M);
         copy_rows_async<T, M, NT, PS>(st + EPC * C::S_EL, invL + e0 * M3, ne * M2);
-        copy_rows_async<T, M, NT, PS>(st + EPC * (C::S_EL + C::B_EL), b + e0 * M3, ne * M2);
+        io.template load<NT, PS>(st + EPC * (C::S_EL + C::B_EL), xtra, e0, ne);
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
 
@@ -328,7 +424,7 @@ k_fdm_sreg(int64_t E, const T* __restrict__ S, const T* __restrict__ invL, const
 #pragma unroll
             for (int l = 0; l < M; ++l) in[l] = line[l * PS];
             apply_matrix<T, M, false>(Sr, in, [&](int o, T v) {
-                if (live) u[e * M3 + o * M2 + q] = v;
+                if (live) io.store(xtra, el, e, o, q, v);
             });
         }
     }

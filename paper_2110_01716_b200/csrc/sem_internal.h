@@ -94,6 +94,7 @@ struct sem_ctx {
     uint64_t J_have = 0;           // (FP32 ? 1 : 0), each written once (bit `key` of J_have): graphs never see a rewrite
     float* d_Minv32 = nullptr;     // Minv rounded to FP32 for the FP32 smoother (sem_cheby.cu)
     double lambda_of_minv32 = -1.0;
+    void* d_cheb4 = nullptr;       // fourth work vector of the Chebyshev-Schwarz smoother (S applied out of place)
     void* d_cheb[3] = {nullptr, nullptr, nullptr};   // r, d, w of the Chebyshev smoother (sem_cheby.cu), nL doubles each
     sem_schwarz_data* sw = nullptr; // NEXT-2b: face links, 1-D operator factorisations, weights (sem_schwarz_setup)
     uint64_t generation = 0;       // bumped whenever device pointers or parameters that launches capture may change
@@ -146,6 +147,9 @@ int sem_launch_gs_many(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec pre
 int sem_launch_gs_fields(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec prec, bool mask, const int* skip);
 // sem_api.cu
 int sem_launch_gs_fields(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec prec, bool mask, const int* skip);
+// sem_fdm.cu
+int sem_launch_fdm_schwarz(sem_ctx* c, int m, const void* S, const void* invL, const void* r, const int4* link,
+                           const int32_t* nrm, const void* W, void* z, sem_prec prec);
 // sem_schwarz.cu
 void sem_schwarz_free(sem_ctx* c);
 int sem_launch_schwarz(sem_ctx* c, const void* r, void* z, sem_prec prec, int kind);   // z may alias r

@@ -232,6 +232,13 @@ int apply(sem_ctx* c, const T* r, T* z, int kind) {
     const T* W = sizeof(T) == 8 ? (const T*)s->d_W64[kind] : (const T*)s->d_W32[kind];
     T* ext = (T*)s->d_ext;
     const unsigned grid = (unsigned)c->E;
+    if (kind == SEM_SCHWARZ_RAS && r != z) {
+        // restricted variant: one kernel (gather from r into the shared-memory block, Eq. (3), weighted own part to z)
+        // and the gather-scatter; in place (r == z) an element would read neighbour values already overwritten
+        int rc1 = sem_launch_fdm_schwarz(c, s->m, S, iL, r, s->d_link, s->d_nrm, W, z, prec);
+        if (rc1) return rc1;
+        return sem_launch_gs(c, z, prec, /*apply_mask=*/true);
+    }
     launch_ext<T>(c, grid, r, kind == SEM_SCHWARZ_ASM ? W : (const T*)nullptr, ext);
     int rc = sem_fdm_apply(c, s->m, S, iL, ext, ext, prec);
     if (rc) return rc;
