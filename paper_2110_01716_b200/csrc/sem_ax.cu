@@ -450,23 +450,23 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
                  : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
-template <int NS>
+template <int NS, int NU>
 struct DmmaSmem {
     alignas(128) double g[NS][6 * 64];
-    alignas(128) double u[2][512];
+    alignas(128) double u[NU][512];          // NU = 2: the next element's u lands while this one is worked on
     alignas(16) double sgs[2][64];
     alignas(8) uint64_t gfull[NS];
-    alignas(8) uint64_t ufull[2];
+    alignas(8) uint64_t ufull[NU];
     alignas(16) double D[64];
 };
 
-template <int NS, int MINB>
+template <int NS, int MINB, int NU>
 __global__ void __launch_bounds__(32, MINB) ax_dmma(int64_t E, DParam<double, 8> dp, const double* __restrict__ Gs,
                                                     const double* __restrict__ Bm, double lambda,
                                                     const double* __restrict__ u, double* __restrict__ w,
                                                     const int* __restrict__ skip_flag, double* __restrict__ dot_out,
                                                     int u_keep) {
-    using SM = DmmaSmem<NS>;
+    using SM = DmmaSmem<NS, NU>;
     constexpr int P = 8, P2 = 64, P3 = 512, SLAB = 6 * 64;
     constexpr uint32_t GBYTES = SLAB * sizeof(double), UBYTES = P3 * sizeof(double);
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -481,15 +481,15 @@ __global__ void __launch_bounds__(32, MINB) ax_dmma(int64_t E, DParam<double, 8>
     uint64_t pol_g = 0, pol_u = 0;
     auto issue_u = [&](int64_t n) {
         const int64_t e = blockIdx.x + n * gridDim.x;
-        const int b = (int)(n & 1);
+        const int b = (int)(n % NU);
         mbar_expect_tx(&sm.ufull[b], UBYTES);
         bulk_g2s(&sm.u[b][0], u + e * P3, UBYTES, &sm.ufull[b], pol_u);
     };
     if (lane == 0) {
 #pragma unroll
         for (int q = 0; q < NS; ++q) mbar_init(&sm.gfull[q], 1);
-        mbar_init(&sm.ufull[0], 1);
-        mbar_init(&sm.ufull[1], 1);
+#pragma unroll
+        for (int q = 0; q < NU; ++q) mbar_init(&sm.ufull[q], 1);
         mbar_fence_init();
     }
     sm.D[lane] = dp.D[lane];
@@ -507,7 +507,7 @@ __global__ void __launch_bounds__(32, MINB) ax_dmma(int64_t E, DParam<double, 8>
             if (++gk == P) { gk = 0; gsrc += gjump; }
             --gleft;
         }
-        if (nmine > 1) issue_u(1);
+        if (NU == 2 && nmine > 1) issue_u(1);
     }
     // constant fragments of D (volatile loads: pinned in registers, see DRows::init_shared)
     double Br[2], As[2], BrT[2], AsT[2];
@@ -528,8 +528,8 @@ __global__ void __launch_bounds__(32, MINB) ax_dmma(int64_t E, DParam<double, 8>
     double* wdst = w + (int64_t)blockIdx.x * P3 + own;
     const int64_t wstep = (int64_t)gridDim.x * P3;
     for (int64_t n = 0; n < nmine; ++n, wdst += wstep) {
-        const int ub = (int)(n & 1);
-        mbar_wait(&sm.ufull[ub], (uint32_t)((n >> 1) & 1));
+        const int ub = (int)(n % NU);
+        mbar_wait(&sm.ufull[ub], (uint32_t)((n / NU) & 1));
         const double* sue = &sm.u[ub][0];
         double uk[P][2], wk[P][2];
 #pragma unroll
@@ -576,7 +576,7 @@ __global__ void __launch_bounds__(32, MINB) ax_dmma(int64_t E, DParam<double, 8>
                     if ((k + NS) % P == P - 1) gsrc += gjump;
                     --gleft;
                 }
-                if (k == P - 1 && n + 2 < nmine) issue_u(n + 2);
+                if (k == P - 1 && n + NU < nmine) issue_u(n + NU);
             }
             // w_k += g_r D + D^T g_s
             double a0[2] = {0.0, 0.0}, a1[2] = {0.0, 0.0};
@@ -865,12 +865,12 @@ int launch_stream(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, doubl
     return SEM_OK;
 }
 
-template <int NS, int MINB>
+template <int NS, int MINB, int NU = 2>
 int launch_dmma(sem_ctx* c, const double* u, double* w, double lambda, const int* skip, double* dot) {
-    using SM = DmmaSmem<NS>;
+    using SM = DmmaSmem<NS, NU>;
     const DParam<double, 8> dp = make_dparam<double, 8>(c);
     const size_t smem = sizeof(SM) + 128;
-    auto kern = ax_dmma<NS, MINB>;
+    auto kern = ax_dmma<NS, MINB, NU>;
     int blocks_per_sm = 0;
     if (int rc = resident_blocks(c, kern, 32, smem, &blocks_per_sm)) return rc;
     const ElemRange r = elem_range(c);
