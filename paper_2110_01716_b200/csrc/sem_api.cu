@@ -37,10 +37,8 @@ int sem_launch_gs_fields(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec p
     return SEM_OK;
 }
 
-extern "C" {
-
-int sem_mesh_setup(sem_ctx** out, int64_t E, int N, const double* vertex_xyz, const int64_t* gid,
-                   const uint8_t* dirichlet, void* cuda_stream) {
+int sem_mesh_setup_impl(sem_ctx** out, int64_t E, int N, const double* vertex_xyz, const int64_t* gid,
+                        const uint8_t* dirichlet, void* cuda_stream, bool is_inner) {
     if (!out) return SEM_EINVAL;
     *out = nullptr;
     if (E <= 0 || N < 1 || N > SEM_MAXP - 1 || !vertex_xyz || !gid) return SEM_EINVAL;
@@ -50,6 +48,7 @@ int sem_mesh_setup(sem_ctx** out, int64_t E, int N, const double* vertex_xyz, co
     sem_ctx* c = new (std::nothrow) sem_ctx();
     if (!c) return SEM_ENOMEM;
     *out = c;
+    c->is_inner = is_inner;
     c->E = E; c->N = N; c->p = (int)p; c->p3 = p * p * p; c->nL = nL;
     c->epb = sem_epb((int)p);
     c->ngroups = (E + c->epb - 1) / c->epb;
@@ -65,6 +64,13 @@ int sem_mesh_setup(sem_ctx** out, int64_t E, int N, const double* vertex_xyz, co
     int rc = sem_build_maps(c, gid, dirichlet);
     if (rc) return rc;
     return sem_build_gs_records(c);
+}
+
+extern "C" {
+
+int sem_mesh_setup(sem_ctx** out, int64_t E, int N, const double* vertex_xyz, const int64_t* gid,
+                   const uint8_t* dirichlet, void* cuda_stream) {
+    return sem_mesh_setup_impl(out, E, N, vertex_xyz, gid, dirichlet, cuda_stream, false);
 }
 
 int sem_geom(sem_ctx* c, const double* node_xyz, sem_gmode mode, int with_mass) {
@@ -84,7 +90,7 @@ int sem_geom(sem_ctx* c, const double* node_xyz, sem_gmode mode, int with_mass) 
     int rc = sem_build_geom(c, node_xyz);
     if (rc) return rc;
     c->geom_done = true;
-    return SEM_OK;
+    return sem_inner_build(c, node_xyz);          // large mesh in an order without locality: inner context for sem_pcg
 }
 
 static int check_vec(sem_ctx* c, const void* u, const void* w, sem_prec prec, double lambda, const char* who) {
@@ -270,6 +276,7 @@ void sem_ctx_destroy(sem_ctx* c) {
     if (!c) return;
     cudaStreamSynchronize(c->stream);
     if (c->ag_exec) cudaGraphExecDestroy(c->ag_exec);
+    sem_inner_free(c);
     sem_schwarz_free(c);
     void* ptrs[] = {c->d_vert, c->d_l2u, c->d_mult, c->d_seg_off, c->d_seg_idx, c->d_uniq_gid, c->d_sh_off, c->d_sh_idx,
                     c->d_sh_masked, c->d_mask_u, c->d_mask1_idx, c->d_G, c->d_G32, c->d_B, c->d_B32, c->d_detJ,

@@ -96,6 +96,12 @@ struct sem_ctx {
     double lambda_of_minv32 = -1.0;
     void* d_cheb4 = nullptr;       // fourth work vector of the Chebyshev-Schwarz smoother (S applied out of place)
     void* d_cheb[3] = {nullptr, nullptr, nullptr};   // r, d, w of the Chebyshev smoother (sem_cheby.cu), nL doubles each
+    // element renumbering for the solver's own vectors (sem_inner.cu): a second context over the same elements sorted by
+    // smallest global id, used by sem_pcg on large meshes whose element order has no locality
+    sem_ctx* inner = nullptr;
+    bool is_inner = false;
+    int32_t* d_perm = nullptr;      // [E] inner position q holds caller element d_perm[q]
+    double *d_bi = nullptr, *d_xi = nullptr;
     sem_schwarz_data* sw = nullptr; // NEXT-2b: face links, 1-D operator factorisations, weights (sem_schwarz_setup)
     uint64_t generation = 0;       // bumped whenever device pointers or parameters that launches capture may change
                                    // (sem_geom, sem_set_lambda): invalidates CUDA graphs recorded over this context
@@ -147,6 +153,12 @@ int sem_launch_gs_many(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec pre
 int sem_launch_gs_fields(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec prec, bool mask, const int* skip);
 // sem_api.cu
 int sem_launch_gs_fields(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec prec, bool mask, const int* skip);
+// sem_api.cu / sem_inner.cu
+int sem_mesh_setup_impl(sem_ctx** out, int64_t E, int N, const double* vertex_xyz, const int64_t* gid,
+                        const uint8_t* dirichlet, void* cuda_stream, bool is_inner);
+int sem_inner_build(sem_ctx* c, const double* node_xyz_host);
+void sem_inner_free(sem_ctx* c);
+int sem_inner_pcg(sem_ctx* c, const double* b, double* x, double tol, int maxit, int* iters_out, double* relres_out);
 // sem_fdm.cu
 int sem_launch_fdm_schwarz(sem_ctx* c, int m, const void* S, const void* invL, const void* r, const int4* link,
                            const int32_t* nrm, const void* W, void* z, sem_prec prec);

@@ -152,6 +152,7 @@ extern "C" int sem_pcg(sem_ctx* c, const double* b, double* x, double tol, int m
     if (!c->geom_done) return sem_fail(c, SEM_ESTATE, "sem_pcg before sem_geom");
     if (c->lambda != 0.0 && !c->with_mass) return sem_fail(c, SEM_ESTATE, "lambda != 0 needs with_mass");
     if (maxit < 0) maxit = 0;
+    if (c->inner) return sem_inner_pcg(c, b, x, tol, maxit, iters_out, relres_out);     // sem_inner.cu
     cudaStream_t st = c->stream;
     const int64_t n = c->nL;
     if (!c->pcg_ready || c->lambda_of_diag != c->lambda) {

@@ -556,3 +556,51 @@ def test_chunked_ax_gs_is_bit_identical(torch_cuda, binding, oracle_mod, monkeyp
     assert relerr(outs[0].cpu().numpy(), ow) <= (TOL64 if dtype == "f64" else TOL32)
     assert torch_cuda.equal(outs[1], outs[0]) and torch_cuda.equal(outs[2], outs[0])
     assert len(set(its)) <= 1 and all(relerr(x, xs[0]) <= 1e-9 for x in xs[1:])
+
+
+# --------------------------------------------------------------------------- element renumbering inside sem_pcg
+@pytest.mark.parametrize("iso", [False, True])
+def test_pcg_through_the_inner_renumbered_context(torch_cuda, binding, oracle_mod, monkeypatch, iso):
+    """Large meshes in an element order without locality get a second context over the same elements sorted by their
+    smallest global id, and sem_pcg runs there (b, x gathered / scattered in 4 KB blocks).  Forced here with SEM_INNER=1 on
+    a small scrambled mesh: iteration count, residual history and solution equal the oracle's, with trilinear and with
+    isoparametric (node_xyz) geometry, a non-zero initial guess and the Helmholtz shift; a lexicographic mesh of the same
+    size gets no inner context even when large (checked through the unchanged result with SEM_INNER unset)."""
+    m = inputs.box_mesh(5, 4, 4, 5, "random", seed=7, permute_seed=11)
+    lam = 3.0
+    om = oracle_mod.Maps(m.gid)
+    xyz = oracle_mod.node_xyz(m.vert, m.N)
+    if iso:
+        oG, _, rc = oracle_mod.geom_iso(xyz, m.N)
+    else:
+        oG, _, rc = oracle_mod.geom_trilinear(m.vert, m.N)
+    assert rc == 0
+    mask_u = oracle_mod.mask_unique(m.dirichlet, om)
+    xs = np.where(mask_u != 0, 0.0, inputs.field_normal(om.uniq_gid, 9))
+    x0 = np.where(mask_u != 0, 0.0, 0.3 * inputs.field_normal(om.uniq_gid, 10))
+    b_u = oracle_mod.apply_Ag(oG, m.N, om, mask_u, xs, lam)
+    ores = oracle_mod.pcg(oG, m.N, om, mask_u, b_u, x0_u=x0, tol=1e-10, maxit=300, lam=lam)
+    results = []
+    for inner in ("1", None):
+        if inner is None:
+            monkeypatch.delenv("SEM_INNER", raising=False)
+        else:
+            monkeypatch.setenv("SEM_INNER", inner)
+        with binding.Sem(m.E, m.N, m.vert, m.gid, m.dirichlet) as sem:
+            sem.geom(node_xyz=xyz if iso else None, with_mass=True)
+            sem.set_lambda(lam)
+            b = to_dev(torch_cuda, b_u[om.l2u])
+            x = to_dev(torch_cuda, x0[om.l2u])
+            it, rel = sem.pcg(b, x, 1e-10, 300)
+            assert it == ores["iters"], (inner, it, ores["iters"])
+            assert relerr(x.cpu().numpy(), ores["x"][om.l2u]) <= TOLPCG
+            h = sem.pcg_history(it + 1)
+            assert np.max(np.abs(h - ores["hist"]) / ores["hist"]) <= 1e-5
+            results.append(x.cpu().numpy())
+            # the operator on the caller's vectors is untouched by the inner context
+            du = to_dev(torch_cuda, inputs.field_uniform(m.gid, 3).ravel())
+            dw = torch_cuda.empty_like(du)
+            sem.ax_gs(du, dw, lam)
+            ow = oracle_mod.gs(oracle_mod.ax(oG, inputs.field_uniform(m.gid, 3), m.N, lam).ravel(), om)
+            assert relerr(dw.cpu().numpy(), np.where(mask_u[om.l2u] != 0, 0.0, ow)) <= TOL64
+    assert relerr(results[0], results[1]) <= 1e-9
