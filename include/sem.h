@@ -302,10 +302,10 @@ SEM_API int sem_pmg_set_smoother(sem_pmg* mg, sem_smoother smoother, const doubl
 enum { SEM_PEAK_FMA_F64 = 0, SEM_PEAK_FMA_F32 = 1, SEM_PEAK_DMMA_F64 = 2 };
 SEM_API int sem_measure_peak(int kind, void* cuda_stream, double* tflops_out);
 
-/* Tuning knob for experiments: selects the Ax kernel variant.  0 = the default per (precision, p): for FP64 p = 8 the
- * tensor-core kernel (one warp per element, r/s contractions as DMMA m8n8k4), else the streaming kernel; 1 = the simple
- * plain-load kernel; 2 = the scalar streaming kernel where it exists (even p <= 12); 3 = FP64 p = 8 only: the
- * tensor-core kernel with 5 ring stages and 8 warps per SM. */
+/* Tuning knob for experiments: selects the Ax kernel variant.  0 = the default per (precision, p): p = 8 runs on the
+ * tensor cores, one warp per element (FP64: r/s contractions as DMMA m8n8k4; FP32: as TF32 m16n8k8 in three passes,
+ * FP32-level accuracy), every other p <= 12 the streaming kernel; 1 = the simple plain-load kernel; 2 = the scalar
+ * streaming kernel (p <= 12); 3 = FP64 p = 8 only: the DMMA kernel with 5 ring stages and 8 warps per SM. */
 SEM_API int sem_set_variant(sem_ctx* ctx, int ax_variant);
 
 /* Last error text of this context ("" if none); valid until the next call on the context.  NULL ctx -> static text. */

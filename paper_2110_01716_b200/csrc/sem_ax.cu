@@ -607,6 +607,214 @@ __global__ void __launch_bounds__(32, MINB) ax_dmma(int64_t E, DParam<double, 8>
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// ax_tf32: FP32, p = 8, one warp per element like ax_dmma, the r and s contractions on the tensor cores as
+// mma.sync.m16n8k8 TF32 in THREE passes (x = hi + lo with hi = tf32(x), lo = tf32(x - hi); hi*hi + lo*hi + hi*lo, the
+// dropped lo*lo term is 2^-22 relative: FP32-level accuracy, inside the 1e-5 bar of S16; accumulation in FP32).  There
+// is no exact single-pass FP32 tensor-core path (TF32 carries 10 mantissa bits).  The scalar FP32 kernel issues the same
+// shared-memory traffic as the FP64 one for half the bytes and sits at 0.71 of the HBM roofline; here two k-planes share
+// one MMA in the r direction (M = 16 = two planes of 8 rows; the lane's own four values are its A fragment through the
+// same permuted contraction index as in ax_dmma), the s direction takes one MMA per plane with D in the upper half of A.
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void split_tf32(float x, uint32_t& hi, uint32_t& lo) {
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(hi) : "f"(x));
+    const float rest = x - __uint_as_float(hi);
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(lo) : "f"(rest));
+}
+__device__ __forceinline__ void mma1688(float (&d)[4], const uint32_t (&a)[4], const uint32_t (&b)[2]) {
+    asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
+}
+// d += a * b in three TF32 passes; the operands arrive already split
+__device__ __forceinline__ void mma3(float (&d)[4], const uint32_t (&ah)[4], const uint32_t (&al)[4],
+                                     const uint32_t (&bh)[2], const uint32_t (&bl)[2]) {
+    mma1688(d, al, bh);
+    mma1688(d, ah, bl);
+    mma1688(d, ah, bh);
+}
+
+template <int NS>
+struct Tf32Smem {
+    alignas(128) float g[NS][2][6 * 64];        // a stage = the slabs of two consecutive planes: one bulk copy of 3 KB
+    alignas(128) float u[2][512];
+    alignas(16) float sgs[2][2][64];            // [buffer][plane of the pair][j * 8 + i]
+    alignas(8) uint64_t gfull[NS];
+    alignas(8) uint64_t ufull[2];
+    alignas(16) float D[64];
+};
+
+template <int NS, int MINB>
+__global__ void __launch_bounds__(32, MINB) ax_tf32(int64_t E, DParam<float, 8> dp, const float* __restrict__ Gs,
+                                                    const float* __restrict__ Bm, float lambda,
+                                                    const float* __restrict__ u, float* __restrict__ w,
+                                                    const int* __restrict__ skip_flag, double* __restrict__ dot_out,
+                                                    int u_keep) {
+    using SM = Tf32Smem<NS>;
+    constexpr int P = 8, P2 = 64, P3 = 512, SLAB = 6 * 64;
+    constexpr uint32_t GBYTES = 2 * SLAB * sizeof(float), UBYTES = P3 * sizeof(float);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    SM& sm = *reinterpret_cast<SM*>(smem_raw);
+    if (skip_flag && *skip_flag) return;
+    const int lane = threadIdx.x, g = lane >> 2, t = lane & 3;
+    const int64_t nmine = blockIdx.x < E ? (E - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+
+    const float* gsrc = Gs + (int64_t)blockIdx.x * (P * SLAB);
+    const int64_t gjump = (int64_t)(gridDim.x - 1) * (P * SLAB);
+    int64_t gleft = nmine * (P / 2);                  // plane pairs still to issue
+    int gk = 0;                                       // pair index (within its element) of the next one
+    uint64_t pol_g = 0, pol_u = 0;
+    auto issue_u = [&](int64_t n) {
+        const int64_t e = blockIdx.x + n * gridDim.x;
+        const int b = (int)(n & 1);
+        mbar_expect_tx(&sm.ufull[b], UBYTES);
+        bulk_g2s(&sm.u[b][0], u + e * P3, UBYTES, &sm.ufull[b], pol_u);
+    };
+    auto issue_g = [&](int stage) {
+        mbar_expect_tx(&sm.gfull[stage], GBYTES);
+        bulk_g2s(&sm.g[stage][0][0], gsrc, GBYTES, &sm.gfull[stage], pol_g);
+        gsrc += 2 * SLAB;
+        if (++gk == P / 2) { gk = 0; gsrc += gjump; }
+        --gleft;
+    };
+    if (lane == 0) {
+#pragma unroll
+        for (int q = 0; q < NS; ++q) mbar_init(&sm.gfull[q], 1);
+        mbar_init(&sm.ufull[0], 1);
+        mbar_init(&sm.ufull[1], 1);
+        mbar_fence_init();
+    }
+    sm.D[lane] = dp.D[lane];
+    sm.D[lane + 32] = dp.D[lane + 32];
+    __syncwarp();
+    if (lane == 0 && nmine > 0) {
+        pol_g = policy_evict_first();
+        pol_u = u_keep ? policy_evict_last() : policy_evict_first();
+        issue_u(0);
+        for (int q = 0; q < NS && gleft > 0; ++q) issue_g(q);
+        if (nmine > 1) issue_u(1);
+    }
+    // constant fragments of D, split once: B of the r contractions, A (rows 0-7; rows 8-15 zero) of the s contractions
+    uint32_t Brh[2], Brl[2], BrTh[2], BrTl[2], Ash[4], Asl[4], AsTh[4], AsTl[4];
+    {
+        const uint32_t base = smem_u32(sm.D);
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            split_tf32(DRows<float, 8>::lds_volatile(base + (uint32_t)((g * 8 + 2 * t + c) * 4)), Brh[c], Brl[c]);     // D[i=g][l=2t+c]
+            split_tf32(DRows<float, 8>::lds_volatile(base + (uint32_t)(((2 * t + c) * 8 + g) * 4)), BrTh[c], BrTl[c]); // D[l=2t+c][i=g]
+            split_tf32(DRows<float, 8>::lds_volatile(base + (uint32_t)((g * 8 + 4 * c + t) * 4)), Ash[2 * c], Asl[2 * c]);     // D[j=g][l=4c+t]
+            split_tf32(DRows<float, 8>::lds_volatile(base + (uint32_t)(((4 * c + t) * 8 + g) * 4)), AsTh[2 * c], AsTl[2 * c]); // D[l=4c+t][j=g]
+            Ash[2 * c + 1] = Asl[2 * c + 1] = AsTh[2 * c + 1] = AsTl[2 * c + 1] = 0u;
+        }
+    }
+    float partial = 0.f;
+    int q = 0;
+    uint32_t gphase = 0;
+    const int own = g * 8 + 2 * t;
+    float* wdst = w + (int64_t)blockIdx.x * P3 + own;
+    const int64_t wstep = (int64_t)gridDim.x * P3;
+    for (int64_t n = 0; n < nmine; ++n, wdst += wstep) {
+        const int ub = (int)(n & 1);
+        mbar_wait(&sm.ufull[ub], (uint32_t)((n >> 1) & 1));
+        const float* sue = &sm.u[ub][0];
+        float uk[P][2], wk[P][2];
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+            const float2 v = *reinterpret_cast<const float2*>(sue + k * P2 + own);
+            uk[k][0] = v.x; uk[k][1] = v.y; wk[k][0] = 0.f; wk[k][1] = 0.f;
+        }
+#pragma unroll
+        for (int k = 0; k < P; k += 2) {
+            mbar_wait(&sm.gfull[q], gphase);
+            // u_r of both planes in one MMA: A = the lane's own four values
+            float ur[4] = {0.f, 0.f, 0.f, 0.f};
+            {
+                uint32_t ah[4], al[4];
+                split_tf32(uk[k][0], ah[0], al[0]);
+                split_tf32(uk[k + 1][0], ah[1], al[1]);
+                split_tf32(uk[k][1], ah[2], al[2]);
+                split_tf32(uk[k + 1][1], ah[3], al[3]);
+                mma3(ur, ah, al, Brh, Brl);
+            }
+            float gr[2][2], gt[2][2];
+            const int buf = (k >> 1) & 1;
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {                       // the two planes of the pair
+                const int kk = k + h;
+                float us4[4] = {0.f, 0.f, 0.f, 0.f};
+                {
+                    uint32_t bh[2], bl[2];
+                    split_tf32(sue[kk * P2 + t * P + g], bh[0], bl[0]);
+                    split_tf32(sue[kk * P2 + (4 + t) * P + g], bh[1], bl[1]);
+                    mma3(us4, Ash, Asl, bh, bl);
+                }
+                float ut[2] = {0.f, 0.f};
+#pragma unroll
+                for (int l = 0; l < P; ++l) { ut[0] += dp.D[kk * P + l] * uk[l][0]; ut[1] += dp.D[kk * P + l] * uk[l][1]; }
+                float G6[6][2];
+#pragma unroll
+                for (int c = 0; c < 6; ++c) {
+                    const float2 v = *reinterpret_cast<const float2*>(&sm.g[q][h][c * P2 + own]);
+                    G6[c][0] = v.x; G6[c][1] = v.y;
+                }
+                float gs[2];
+#pragma unroll
+                for (int b = 0; b < 2; ++b) {
+                    const float r_ = ur[2 * h + b], s_ = us4[b], t_ = ut[b];
+                    gr[h][b] = G6[0][b] * r_ + G6[1][b] * s_ + G6[2][b] * t_;
+                    gs[b] = G6[1][b] * r_ + G6[3][b] * s_ + G6[4][b] * t_;
+                    gt[h][b] = G6[2][b] * r_ + G6[4][b] * s_ + G6[5][b] * t_;
+                }
+                *reinterpret_cast<float2*>(&sm.sgs[buf][h][own]) = make_float2(gs[0], gs[1]);
+#pragma unroll
+                for (int l = 0; l < P; ++l) { wk[l][0] += dp.D[kk * P + l] * gt[h][0]; wk[l][1] += dp.D[kk * P + l] * gt[h][1]; }
+            }
+            __syncwarp();
+            if (lane == 0) {                                    // the stage is consumed by every lane: refill
+                if (gleft > 0) issue_g(q);
+                if (k == P - 2 && n + 2 < nmine) issue_u(n + 2);
+            }
+            // w += g_r D (both planes, one MMA) + D^T g_s (one MMA per plane)
+            float ar[4] = {0.f, 0.f, 0.f, 0.f};
+            {
+                uint32_t ah[4], al[4];
+                split_tf32(gr[0][0], ah[0], al[0]);
+                split_tf32(gr[1][0], ah[1], al[1]);
+                split_tf32(gr[0][1], ah[2], al[2]);
+                split_tf32(gr[1][1], ah[3], al[3]);
+                mma3(ar, ah, al, BrTh, BrTl);
+            }
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                float as4[4] = {0.f, 0.f, 0.f, 0.f};
+                uint32_t bh[2], bl[2];
+                split_tf32(sm.sgs[buf][h][t * P + g], bh[0], bl[0]);
+                split_tf32(sm.sgs[buf][h][(4 + t) * P + g], bh[1], bl[1]);
+                mma3(as4, AsTh, AsTl, bh, bl);
+                wk[k + h][0] += ar[2 * h] + as4[0];
+                wk[k + h][1] += ar[2 * h + 1] + as4[1];
+            }
+            if (++q == NS) { q = 0; gphase ^= 1u; }
+        }
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+            float v0 = wk[k][0], v1 = wk[k][1];
+            if (Bm) {
+                const float2 bm = *reinterpret_cast<const float2*>(Bm + (wdst - w) + k * P2);
+                v0 += lambda * bm.x * uk[k][0];
+                v1 += lambda * bm.y * uk[k][1];
+            }
+            *reinterpret_cast<float2*>(wdst + k * P2) = make_float2(v0, v1);
+            partial += uk[k][0] * v0 + uk[k][1] * v1;
+        }
+    }
+    if (dot_out) {
+        double v = (double)partial;
+        for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) atomicAdd(dot_out, v);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // ax_dmma_many: the same operator applied to NF fields that share the geometric factors (NEXT-4: "3 Helmholtz problems --
 // one for each velocity component"): G is streamed ONCE per element and k-plane and used for all NF fields, so the
 // compulsory traffic is 48 + 16 NF bytes per node instead of 64 NF (NF = 3: 96 instead of 192).  One warp per element
@@ -883,6 +1091,24 @@ int launch_dmma(sem_ctx* c, const double* u, double* w, double lambda, const int
     return SEM_OK;
 }
 
+template <int NS, int MINB>
+int launch_tf32(sem_ctx* c, const float* u, float* w, float lambda, const int* skip, double* dot) {
+    using SM = Tf32Smem<NS>;
+    const DParam<float, 8> dp = make_dparam<float, 8>(c);
+    const size_t smem = sizeof(SM) + 128;
+    auto kern = ax_tf32<NS, MINB>;
+    int blocks_per_sm = 0;
+    if (int rc = resident_blocks(c, kern, 32, smem, &blocks_per_sm)) return rc;
+    const ElemRange r = elem_range(c);
+    const int64_t cap = (int64_t)c->num_sms * blocks_per_sm;
+    const unsigned grid = (unsigned)(r.ne < cap ? r.ne : cap);
+    kern<<<grid, 32, smem, c->stream>>>(r.ne, dp, c->d_G32 + r.e0 * (8 * 6 * 64),
+                                        lambda != 0.f ? c->d_B32 + r.e0 * 512 : (const float*)nullptr, lambda,
+                                        u + r.e0 * 512, w + r.e0 * 512, skip, dot, u_keep(c, 4));
+    SEM_CUDA_OK(c, cudaGetLastError());
+    return SEM_OK;
+}
+
 template <int NF>
 int launch_dmma_many(sem_ctx* c, const double* u, double* w, int64_t stride, double lambda, const int* skip, double* dot,
                      int64_t dot_stride) {
@@ -930,11 +1156,14 @@ int dispatch_p(sem_ctx* c, const void* u, void* w, double lambda, const int* ski
     T* ww = (T*)w;
     const bool aligned = ((uintptr_t)u % 16) == 0;
     if (c->gmode == SEM_G_RECOMPUTE) return launch_simple<T, P, true>(c, uu, ww, (T)lambda, skip, dot);
-    // variant 0: the default kernel per (T, p); 1: ax_simple; 2: ax_stream where it exists (scalar contractions);
-    // 3: the DMMA kernel with 5 stages / 8 warps per SM (the configuration that mirrors ax_stream's residency)
+    // variant 0: the default kernel per (T, p): p = 8 runs on the tensor cores (FP64: DMMA, FP32: TF32 x 3);
+    // 1: ax_simple; 2: ax_stream (scalar contractions); 3: FP64 p = 8: the DMMA kernel with 5 stages / 8 warps per SM
     if constexpr (P == 8 && sizeof(T) == 8) {
         if (aligned && c->ax_variant == 0) return launch_dmma<3, 12>(c, (const double*)u, (double*)w, lambda, skip, dot);
         if (aligned && c->ax_variant == 3) return launch_dmma<5, 8>(c, (const double*)u, (double*)w, lambda, skip, dot);
+    }
+    if constexpr (P == 8 && sizeof(T) == 4) {          // FP32 p = 8: the TF32 x 3 tensor-core kernel
+        if (aligned && c->ax_variant == 0) return launch_tf32<3, 12>(c, (const float*)u, (float*)w, (float)lambda, skip, dot);
     }
     if constexpr (stream_ok<P>()) {
         if (c->ax_variant != 1 && aligned)

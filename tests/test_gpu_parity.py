@@ -209,7 +209,7 @@ def test_ax_helmholtz(torch_cuda, binding, oracle_mod, N, variant):
 
 
 @pytest.mark.parametrize("N", [1, 2, 3, 5, 7, 9])
-@pytest.mark.parametrize("variant,mode", [(0, 0), (1, 0), (0, 1)])
+@pytest.mark.parametrize("variant,mode", [(0, 0), (1, 0), (2, 0), (0, 1)])
 def test_ax_f32(torch_cuda, binding, oracle_mod, N, variant, mode):
     m = inputs.box_mesh(5, 4, 3, N, "smooth")
     assert _ax_case(torch_cuda, binding, oracle_mod, m, variant=variant, mode=mode, dtype="f32") <= TOL32

@@ -93,6 +93,27 @@ def test_ax_dmma_vs_scalar_kernels(torch_cuda, binding, oracle_mod, variant):
             assert relerr(dw.cpu().numpy().reshape(ow.shape), ow) <= TOL64, (variant, lam)
 
 
+@pytest.mark.parametrize("variant", [0, 2])
+def test_ax_tf32_vs_scalar_kernel(torch_cuda, binding, oracle_mod, variant):
+    """FP32 p = 8: the TF32 x 3 tensor-core kernel (variant 0: hi*hi + lo*hi + hi*lo, FP32 accumulation) and the scalar
+    streaming kernel (variant 2) against the FP64 oracle at 1e-5 (S16), more elements than resident warps, with and
+    without the Helmholtz term, inputs spanning six orders of magnitude (the split must not lose the small ones)."""
+    m = inputs.box_mesh(22, 22, 23, 7, "random", seed=1)
+    oG, _, rc = oracle_mod.geom_trilinear(m.vert, m.N)
+    assert rc == 0
+    u = inputs.field_normal(m.gid, 4) * (10.0 ** (6.0 * inputs.hash_uniform01(3, 7, m.gid) - 3.0))
+    for lam in (0.0, 12.5):
+        ow = oracle_mod.ax(oG, u, m.N, lam)
+        with binding.Sem(m.E, m.N, m.vert, m.gid) as sem:
+            sem.geom(with_mass=lam != 0.0)
+            sem.set_variant(variant)
+            du = to_dev(torch_cuda, u.ravel(), torch_cuda.float32)
+            dw = torch_cuda.full_like(du, float("nan"))
+            sem.ax(du, dw, lam)
+            torch_cuda.cuda.synchronize()
+            assert relerr(dw.cpu().numpy().reshape(ow.shape), ow) <= TOL32, (variant, lam)
+
+
 def test_ax_dmma_bit_repeatable(torch_cuda, binding):
     """The default FP64 p = 8 path (DMMA operator + record gather-scatter) has no atomics on data: repeated applications
     give bit-identical results, eager or replayed from the CUDA graph."""
