@@ -109,7 +109,7 @@ int sem_ax(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda) {
     int rc = check_vec(c, u, w, prec, lambda, "sem_ax");
     if (rc) return rc;
     if ((rc = require_geom(c, "sem_ax"))) return rc;
-    if (prec == SEM_F32 && c->gmode == SEM_G_STORED && (rc = sem_build_g32(c))) return rc;
+    if (prec == SEM_F32 && (rc = sem_build_g32(c))) return rc;
     return sem_launch_ax(c, u, w, prec, lambda, nullptr, nullptr);
 }
 
@@ -145,7 +145,7 @@ int sem_ax_gs_many(sem_ctx* c, const void* u, void* w, int nfields, int64_t fiel
     if ((rc = require_geom(c, "sem_ax_gs_many"))) return rc;
     if (nfields < 1 || field_stride < c->nL)
         return sem_fail(c, SEM_EINVAL, "sem_ax_gs_many: nfields < 1 or field_stride < nL");
-    if (prec == SEM_F32 && c->gmode == SEM_G_STORED && (rc = sem_build_g32(c))) return rc;
+    if (prec == SEM_F32 && (rc = sem_build_g32(c))) return rc;
     if ((rc = sem_launch_ax_many(c, u, w, nfields, field_stride, prec, lambda, nullptr, 0, nullptr))) return rc;
     return sem_launch_gs_fields(c, w, nfields, field_stride, prec, true, nullptr);
 }
@@ -154,7 +154,7 @@ int sem_ax_gs(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda) 
     int rc = check_vec(c, u, w, prec, lambda, "sem_ax_gs");
     if (rc) return rc;
     if ((rc = require_geom(c, "sem_ax_gs"))) return rc;
-    if (prec == SEM_F32 && c->gmode == SEM_G_STORED && (rc = sem_build_g32(c))) return rc;
+    if (prec == SEM_F32 && (rc = sem_build_g32(c))) return rc;
     // Repeated applications with the same arguments (a time loop, a benchmark) replay a two-node CUDA graph: the
     // operator kernel and the gather-scatter kernel then start back to back instead of paying a stream launch each
     // (an empty 2000-CTA kernel costs 4 us per launch on this machine).  The first call with a new argument set runs

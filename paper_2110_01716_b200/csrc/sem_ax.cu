@@ -1046,7 +1046,7 @@ int launch_simple(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, doubl
     const DParam<T, P> dp = make_dparam<T, P>(c);
     const Gll1D gll = make_gll(c);
     ax_simple<T, P, RECOMP><<<grid, threads_of<P>(), 0, c->stream>>>(
-        r.ne, dp, gll, slab, Gs, c->d_vert + r.e0 * 24, lambda != T(0) ? Bm + r.e0 * P3 : nullptr, lambda, u + r.e0 * P3,
+        r.ne, dp, gll, slab, Gs, c->d_vert + r.e0 * 24, (lambda != T(0) && Bm) ? Bm + r.e0 * P3 : nullptr, lambda, u + r.e0 * P3,
         w + r.e0 * P3, skip, dot);
     SEM_CUDA_OK(c, cudaGetLastError());
     return SEM_OK;

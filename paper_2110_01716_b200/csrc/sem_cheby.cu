@@ -265,7 +265,7 @@ extern "C" int sem_cheby(sem_ctx* c, const void* b, void* x, int order, double l
     if (!c->d_Minv || c->lambda_of_diag != c->lambda) {
         if ((rc = sem_build_diag(c))) return rc;
     }
-    if (prec == SEM_F32 && c->gmode == SEM_G_STORED && (rc = sem_build_g32(c))) return rc;
+    if (prec == SEM_F32 && (rc = sem_build_g32(c))) return rc;
     for (int q = 0; q < 3; ++q)
         if (!c->d_cheb[q]) SEM_CUDA_OK(c, cudaMalloc(&c->d_cheb[q], c->nL * sizeof(double)));
     if (prec == SEM_F32 && (!c->d_Minv32 || c->lambda_of_minv32 != c->lambda)) {       // S16: rounded once from double
@@ -293,7 +293,7 @@ extern "C" int sem_cheby_schwarz(sem_ctx* c, const void* b, void* x, int order, 
     if (!c->sw) return sem_fail(c, SEM_ESTATE, "sem_cheby_schwarz before sem_schwarz_setup");
     if (c->lambda != 0.0 && !c->with_mass) return sem_fail(c, SEM_ESTATE, "lambda != 0 needs with_mass");
     int rc;
-    if (prec == SEM_F32 && c->gmode == SEM_G_STORED && (rc = sem_build_g32(c))) return rc;
+    if (prec == SEM_F32 && (rc = sem_build_g32(c))) return rc;
     for (int q = 0; q < 3; ++q)
         if (!c->d_cheb[q]) SEM_CUDA_OK(c, cudaMalloc(&c->d_cheb[q], c->nL * sizeof(double)));
     if (!c->d_cheb4) SEM_CUDA_OK(c, cudaMalloc(&c->d_cheb4, c->nL * sizeof(double)));

@@ -166,17 +166,46 @@ int sem_build_geom(sem_ctx* c, const double* node_xyz_host) {
     if (e != cudaSuccess) return sem_fail(c, SEM_ECUDA, "geometry kernel: %s", cudaGetErrorString(e));
     SEM_CUDA_OK(c, cudaGetLastError());
     if (h_bad) return sem_fail(c, SEM_EMESH, "non-positive Jacobian determinant in at least one node");
+    sem_release_G(c);                    // recompute mode keeps no stored G (48 B per node): rebuilt on demand
     return SEM_OK;
 }
 
-int sem_build_g32(sem_ctx* c) {
-    if (c->d_G32) return SEM_OK;
+// Recompute mode (a9): the operator never reads the stored G, so it is not kept; the Jacobi diagonal and sem_get_geom
+// rebuild it from the vertices for the duration of the call (trilinear geometry only: sem_geom enforces it).
+int sem_ensure_G(sem_ctx* c) {
+    if (c->d_G) return SEM_OK;
     cudaStream_t st = c->stream;
-    const int64_t nslabs = c->ngroups * c->epb * c->p;
-    SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_G32, nslabs * c->slab_f32 * sizeof(float)));
-    if (c->slab_f32 != c->slab_f64) SEM_CUDA_OK(c, cudaMemsetAsync(c->d_G32, 0, nslabs * c->slab_f32 * sizeof(float), st));
-    k_g32<<<c->num_sms * 8, 256, 0, st>>>(nslabs, 6 * c->p * c->p, c->slab_f64, c->slab_f32, c->d_G, c->d_G32);
-    if (c->with_mass) {
+    const int64_t gcount = c->ngroups * c->epb * c->p * c->slab_f64;
+    SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_G, gcount * sizeof(double)));
+    if (c->ngroups * c->epb != c->E) SEM_CUDA_OK(c, cudaMemsetAsync(c->d_G, 0, gcount * sizeof(double), st));
+    int* d_bad = nullptr;
+    SEM_CUDA_OK(c, cudaMalloc((void**)&d_bad, sizeof(int)));
+    cudaMemsetAsync(d_bad, 0, sizeof(int), st);
+    k_geom<<<nblk(c->nL), 256, 0, st>>>(c->E, c->p, c->epb, make_gll(c), c->d_vert, nullptr, c->slab_f64, c->d_G, c->d_B,
+                                         c->d_detJ, d_bad);
+    const cudaError_t e = cudaStreamSynchronize(st);
+    cudaFree(d_bad);
+    if (e != cudaSuccess) return sem_fail(c, SEM_ECUDA, "geometry kernel: %s", cudaGetErrorString(e));
+    return SEM_OK;
+}
+
+void sem_release_G(sem_ctx* c) {
+    if (c->gmode != SEM_G_RECOMPUTE || !c->d_G) return;
+    cudaStreamSynchronize(c->stream);
+    cudaFree(c->d_G);
+    c->d_G = nullptr;
+}
+
+// FP32 copies (S16: rounded once from double): G32 in stored mode, B32 whenever the mass factor exists
+int sem_build_g32(sem_ctx* c) {
+    cudaStream_t st = c->stream;
+    if (!c->d_G32 && c->gmode == SEM_G_STORED) {
+        const int64_t nslabs = c->ngroups * c->epb * c->p;
+        SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_G32, nslabs * c->slab_f32 * sizeof(float)));
+        if (c->slab_f32 != c->slab_f64) SEM_CUDA_OK(c, cudaMemsetAsync(c->d_G32, 0, nslabs * c->slab_f32 * sizeof(float), st));
+        k_g32<<<c->num_sms * 8, 256, 0, st>>>(nslabs, 6 * c->p * c->p, c->slab_f64, c->slab_f32, c->d_G, c->d_G32);
+    }
+    if (!c->d_B32 && c->with_mass) {
         SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_B32, c->nL * sizeof(float)));
         k_convert<double, float><<<c->num_sms * 8, 256, 0, st>>>(c->nL, c->d_B, c->d_B32);
     }
@@ -191,9 +220,11 @@ int sem_build_diag(sem_ctx* c) {
         SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_Minv, c->nL * sizeof(double)));
         SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_wt, c->nL * sizeof(double)));
     }
-    k_diag_local<<<nblk(c->nL), 256, 0, st>>>(c->E, c->p, c->epb, make_gll(c), c->slab_f64, c->d_G, c->d_B, c->lambda, c->d_diag);
-    int rc = sem_launch_gs(c, c->d_diag, SEM_F64, /*apply_mask=*/false);
+    int rc = sem_ensure_G(c);
     if (rc) return rc;
+    k_diag_local<<<nblk(c->nL), 256, 0, st>>>(c->E, c->p, c->epb, make_gll(c), c->slab_f64, c->d_G, c->d_B, c->lambda, c->d_diag);
+    sem_release_G(c);
+    if ((rc = sem_launch_gs(c, c->d_diag, SEM_F64, /*apply_mask=*/false))) return rc;
     if (!c->d_wt8) SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_wt8, c->nL));
     int* d_big = nullptr;
     SEM_CUDA_OK(c, cudaMalloc((void**)&d_big, sizeof(int)));
@@ -215,6 +246,7 @@ int sem_build_diag(sem_ctx* c) {
 int sem_geom_export(sem_ctx* c, double* G_host, double* detJ_host) {
     cudaStream_t st = c->stream;
     if (G_host) {
+        if (int rg = sem_ensure_G(c)) return rg;
         const int ncomp = c->with_mass ? 7 : 6;
         const int64_t cnt = c->E * ncomp * c->p3;
         double* d_out = nullptr;
@@ -223,6 +255,7 @@ int sem_geom_export(sem_ctx* c, double* G_host, double* detJ_host) {
         cudaError_t e = cudaMemcpyAsync(G_host, d_out, cnt * sizeof(double), cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
         cudaFree(d_out);
+        sem_release_G(c);
         if (e != cudaSuccess) return sem_fail(c, SEM_ECUDA, "export G: %s", cudaGetErrorString(e));
     }
     if (detJ_host) {

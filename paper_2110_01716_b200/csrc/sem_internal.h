@@ -135,6 +135,8 @@ int sem_build_gs_records(sem_ctx* c);
 // sem_geom.cu
 int sem_build_geom(sem_ctx* c, const double* node_xyz_host);
 int sem_build_g32(sem_ctx* c);
+int sem_ensure_G(sem_ctx* c);       // recompute mode keeps no stored G: rebuilt for the diagonal / the accessor
+void sem_release_G(sem_ctx* c);
 int sem_build_diag(sem_ctx* c);
 int sem_geom_export(sem_ctx* c, double* G_host, double* detJ_host);
 // sem_ax.cu

@@ -625,3 +625,32 @@ def test_pcg_through_the_inner_renumbered_context(torch_cuda, binding, oracle_mo
             ow = oracle_mod.gs(oracle_mod.ax(oG, inputs.field_uniform(m.gid, 3), m.N, lam).ravel(), om)
             assert relerr(dw.cpu().numpy(), np.where(mask_u[om.l2u] != 0, 0.0, ow)) <= TOL64
     assert relerr(results[0], results[1]) <= 1e-9
+
+
+def test_recompute_mode_keeps_no_stored_G_and_handles_helmholtz_in_fp32(torch_cuda, binding, oracle_mod):
+    """SEM_G_RECOMPUTE (a9): no stored G is kept, yet the Jacobi diagonal, sem_get_geom and the PCG loop work
+    (G is rebuilt for the duration of those calls), and the FP32 operator with lambda > 0 finds its mass factor."""
+    m = inputs.box_mesh(5, 4, 3, 7, "random", seed=6)
+    lam = 4.0
+    oG, odJ, rc = oracle_mod.geom_trilinear(m.vert, m.N)
+    om = oracle_mod.Maps(m.gid)
+    mask_u = oracle_mod.mask_unique(m.dirichlet, om)
+    u = inputs.field_uniform(m.gid, 2)
+    ow = oracle_mod.ax(oG, u, m.N, lam)
+    with binding.Sem(m.E, m.N, m.vert, m.gid, m.dirichlet) as sem:
+        sem.geom(mode=binding.SEM_G_RECOMPUTE, with_mass=True)
+        sem.set_lambda(lam)
+        for dt, tol in ((torch_cuda.float64, TOL64), (torch_cuda.float32, TOL32)):
+            du = to_dev(torch_cuda, u.ravel(), dt)
+            dw = torch_cuda.full_like(du, float("nan"))
+            sem.ax(du, dw, lam)
+            assert relerr(dw.cpu().numpy().reshape(ow.shape), ow) <= tol, dt
+        G, dJ = sem.get_geom()
+        assert np.max(np.abs(G - oG)) <= 1e-12 * np.max(np.abs(oG)) and np.max(np.abs(dJ - odJ)) <= 1e-12 * np.max(np.abs(odJ))
+        xs = np.where(mask_u != 0, 0.0, inputs.field_normal(om.uniq_gid, 5))
+        b_u = oracle_mod.apply_Ag(oG, m.N, om, mask_u, xs, lam)
+        ores = oracle_mod.pcg(oG, m.N, om, mask_u, b_u, tol=1e-9, maxit=200, lam=lam)
+        b = to_dev(torch_cuda, b_u[om.l2u])
+        x = torch_cuda.zeros_like(b)
+        it, _ = sem.pcg(b, x, 1e-9, 200)
+        assert it == ores["iters"] and relerr(x.cpu().numpy(), ores["x"][om.l2u]) <= TOLPCG
