@@ -459,6 +459,7 @@ def run_leg(args):
                      (3573, 9), (3573, 7)):
             mesh = inputs.box_mesh(E, 1, 1, 1)
             with binding.Sem(mesh.E, 1, mesh.vert, mesh.gid) as sem:
+                sem.set_variant(args.variant if args.variant >= 100 else 100)      # 101: the FP32 tensor-core kernel
                 A, B = inputs.fdm_pairs(E, m, 7)
                 S, invL = binding.fdm_setup(A, B)
                 for dt, name in ((torch.float32, "FP32"), (torch.float64, "FP64")):

@@ -306,7 +306,13 @@ SEM_API int sem_measure_peak(int kind, void* cuda_stream, double* tflops_out);
 /* Tuning knob for experiments: selects the Ax kernel variant.  0 = the default per (precision, p): p = 8 runs on the
  * tensor cores, one warp per element (FP64: r/s contractions as DMMA m8n8k4; FP32: as TF32 m16n8k8 in three passes,
  * FP32-level accuracy), every other p <= 12 the streaming kernel; 1 = the simple plain-load kernel; 2 = the scalar
- * streaming kernel (p <= 12); 3 = FP64 p = 8 only: the DMMA kernel with 5 ring stages and 8 warps per SM. */
+ * streaming kernel (p <= 12); 3 = FP64 p = 8 only: the DMMA kernel with 5 ring stages and 8 warps per SM.
+ * 100 + v selects the kernel of sem_fdm_apply / the fused restricted Schwarz instead: 100 = the scalar line kernels
+ * (default), 101 = FP32, 6 <= m <= 12: the tensor-core kernel (every 1-D contraction as TF32 m16n8k8 in three passes;
+ * measured slower than the scalar kernels at every m, kept as the measurement north_star asks for).
+ * Environment knobs read at setup (tests, experiments): SEM_CHUNK_GROUPS = element groups per chunk of the chunked
+ * operator / gather-scatter (fields larger than L2; a huge value disables it); SEM_INNER = 0 / 1 never / always build the
+ * renumbered inner context that sem_pcg uses on large meshes without locality. */
 SEM_API int sem_set_variant(sem_ctx* ctx, int ax_variant);
 
 /* Last error text of this context ("" if none); valid until the next call on the context.  NULL ctx -> static text. */

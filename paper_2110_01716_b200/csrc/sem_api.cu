@@ -205,7 +205,8 @@ int sem_set_lambda(sem_ctx* c, double lambda) {
 
 int sem_set_variant(sem_ctx* c, int ax_variant) {
     if (!c) return SEM_EINVAL;
-    c->ax_variant = ax_variant;
+    if (ax_variant >= 100) c->fdm_variant = ax_variant - 100;      // 100 + v: the local-solve kernel (sem_fdm.cu)
+    else c->ax_variant = ax_variant;
     return SEM_OK;
 }
 

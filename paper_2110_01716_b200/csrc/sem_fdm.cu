@@ -59,9 +59,40 @@ int launch_cfg(sem_ctx* c, const void* S, const void* invL, const IO io) {
 //               about 128 threads' worth of elements below; one shared-memory stage (the resident CTAs hide the
 //               copies) up to m = 11, two from m = 12 on (few CTAs fit).
 //   k_fdm_sreg: S_d resident in registers, where it measured faster: FP32 m = 8, 10, 12 and FP64 m = 8, 10.
+// FP32 tensor-core variant (k_fdm_mma): one warp per element
+template <int M, class IO>
+int launch_mma(sem_ctx* c, const void* S, const void* invL, const IO io) {
+    using C = fdm_cfg<float, M, 1, 1>;
+    const size_t smem = C::SMEM1 + IO::extra_bytes(1);
+    auto kern = k_fdm_mma<M, 1, IO>;
+    static std::mutex mu;
+    static int resident_of[SEM_MAX_DEVICES] = {};
+    int resident = 0;
+    {
+        std::lock_guard<std::mutex> lk(mu);
+        const int dev = c->device >= 0 && c->device < SEM_MAX_DEVICES ? c->device : 0;
+        if (!resident_of[dev] || dev != c->device) {
+            if (smem > 48 * 1024)
+                SEM_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            int nb = 0;
+            SEM_CUDA_OK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, 32, smem));
+            resident_of[dev] = nb > 0 ? nb : 1;
+        }
+        resident = resident_of[dev];
+    }
+    int64_t grid = (int64_t)c->num_sms * resident;
+    if (grid > c->E) grid = c->E;
+    kern<<<(unsigned)grid, 32, smem, c->stream>>>(c->E, (const float*)S, (const float*)invL, io);
+    SEM_CUDA_OK(c, cudaGetLastError());
+    return SEM_OK;
+}
+
 template <typename T, int M, class IO>
 int launch_m(sem_ctx* c, const void* S, const void* invL, const IO io) {
     constexpr bool F32 = sizeof(T) == 4;
+    if constexpr (F32 && M >= 6 && M <= 12) {
+        if (c->fdm_variant == 1) return launch_mma<M, IO>(c, S, invL, io);
+    }
     if constexpr (M == 8) return launch_cfg<T, M, 4, 2, 1, true, IO>(c, S, invL, io);
     else if constexpr (M == 10) return launch_cfg<T, M, 4, 1, 1, true, IO>(c, S, invL, io);
     else if constexpr (M == 12 && F32) return launch_cfg<T, M, 5, 1, 1, true, IO>(c, S, invL, io);

@@ -430,4 +430,120 @@ k_fdm_sreg(int64_t E, const T* __restrict__ S, const T* __restrict__ invL, const
     }
 }
 
+// ---- tensor-core variant (FP32): every 1-D contraction as mma.sync.m16n8k8 TF32 in three passes -----------------------
+// P:107 "the application of S and S^T (implemented as dgemm)": a contraction of the m^2 lines of a block with an m x m
+// matrix IS a small GEMM, [m^2 x m] x [m x m].  One warp per element; 16 lines form the M dimension of an MMA tile, the
+// contraction index and the output index are padded to multiples of 8 (zeros), the matrix of the phase is the B operand
+// (split once per phase into hi + lo TF32 parts, as in ax_tf32: hi*hi + lo*hi + hi*lo, FP32 accumulation, FP32-level
+// accuracy).  A tile's lines are read by that tile only, so the block is updated in place with one __syncwarp per tile.
+__device__ __forceinline__ void fdm_split_tf32(float x, uint32_t& hi, uint32_t& lo) {
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(hi) : "f"(x));
+    const float rest = x - __uint_as_float(hi);
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(lo) : "f"(rest));
+}
+__device__ __forceinline__ void fdm_mma1688(float (&d)[4], const uint32_t (&a)[4], const uint32_t (&b)[2]) {
+    asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
+}
+
+// One phase: out[line][o] = sum_l Mat[o][l] in[line][l] for all M^2 lines of direction DIR (0: i-lines, 1: j-lines,
+// 2: k-lines), Mat = S (TRANSPOSED: S^T), in place in the block sB.  SCALE: the result is multiplied by Lambda^-1 (sL, same
+// layout as the block).  LAST: the result goes to the I/O policy instead of the block.
+template <int M, int DIR, bool TRANSPOSED, bool SCALE, bool LAST, class IO>
+__device__ __forceinline__ void fdm_mma_phase(float* __restrict__ sB, const float* __restrict__ sS,
+                                              const float* __restrict__ sL, const IO& io, const unsigned char* xtra,
+                                              int64_t e) {
+    using C = fdm_cfg<float, M, 1, 1>;
+    constexpr int MP = C::MP, PS = C::PS, M2 = M * M;
+    constexpr int KS = (M + 7) / 8, NTI = (M + 7) / 8, TILES = (M2 + 15) / 16;
+    constexpr int LSTR = DIR == 0 ? 1 : (DIR == 1 ? MP : PS);         // stride of the line's own index
+    const int lane = threadIdx.x, g = lane >> 2, t = lane & 3;
+    // B fragments of the phase: B[l][o] = Mat[o][l];  Mat = S^T: S[l][o], Mat = S: S[o][l];  S row-major [M][MP]
+    uint32_t bh[KS][NTI][2], bl[KS][NTI][2];
+#pragma unroll
+    for (int ks = 0; ks < KS; ++ks)
+#pragma unroll
+        for (int nt = 0; nt < NTI; ++nt)
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int l = ks * 8 + t + 4 * h, o = nt * 8 + g;
+                const float v = (l < M && o < M) ? (TRANSPOSED ? sS[l * MP + o] : sS[o * MP + l]) : 0.f;
+                fdm_split_tf32(v, bh[ks][nt][h], bl[ks][nt][h]);
+            }
+#pragma unroll 1
+    for (int T = 0; T < TILES; ++T) {
+        int base[2];
+        bool ok[2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int q = T * 16 + g + 8 * h;
+            ok[h] = q < M2;
+            const int a = ok[h] ? q / M : 0, c = ok[h] ? q - a * M : 0;
+            base[h] = DIR == 0 ? a * PS + c * MP : (DIR == 1 ? a * PS + c : a * MP + c);
+        }
+        uint32_t ah[KS][4], al[KS][4];
+#pragma unroll
+        for (int ks = 0; ks < KS; ++ks)
+#pragma unroll
+            for (int f = 0; f < 4; ++f) {                               // a0 (g, t), a1 (g+8, t), a2 (g, t+4), a3 (g+8, t+4)
+                const int h = f & 1, l = ks * 8 + t + 4 * (f >> 1);
+                const float v = (ok[h] && l < M) ? sB[base[h] + l * LSTR] : 0.f;
+                fdm_split_tf32(v, ah[ks][f], al[ks][f]);
+            }
+        float acc[NTI][4];
+#pragma unroll
+        for (int nt = 0; nt < NTI; ++nt) {
+            acc[nt][0] = acc[nt][1] = acc[nt][2] = acc[nt][3] = 0.f;
+#pragma unroll
+            for (int ks = 0; ks < KS; ++ks) {
+                fdm_mma1688(acc[nt], al[ks], bh[ks][nt]);
+                fdm_mma1688(acc[nt], ah[ks], bl[ks][nt]);
+                fdm_mma1688(acc[nt], ah[ks], bh[ks][nt]);
+            }
+        }
+        __syncwarp();                                                   // every lane holds its inputs: the lines may be overwritten
+#pragma unroll
+        for (int nt = 0; nt < NTI; ++nt)
+#pragma unroll
+            for (int f = 0; f < 4; ++f) {                               // c0 (g, 2t), c1 (g, 2t+1), c2 (g+8, 2t), c3 (g+8, 2t+1)
+                const int h = f >> 1, o = nt * 8 + 2 * t + (f & 1);
+                if (!ok[h] || o >= M) continue;
+                float v = acc[nt][f];
+                if constexpr (SCALE) v *= sL[base[h] + o * LSTR];
+                if constexpr (LAST) io.store(xtra, 0, e, o, T * 16 + g + 8 * h, v);      // DIR == 2: o = k, line = j * M + i
+                else sB[base[h] + o * LSTR] = v;
+            }
+    }
+    __syncwarp();
+}
+
+template <int M, int MINB, class IO>
+__global__ void __launch_bounds__(32, MINB) k_fdm_mma(int64_t E, const float* __restrict__ S, const float* __restrict__ invL,
+                                                      const IO io) {
+    using C = fdm_cfg<float, M, 1, 1>;
+    constexpr int MP = C::MP, PS = C::PS, M2 = M * M, M3 = M2 * M, NT = 32;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float* smem = reinterpret_cast<float*>(smem_raw);
+    unsigned char* xtra = smem_raw + sizeof(float) * (size_t)C::STAGE;
+    float* sS = smem;                                   // [3][M][MP]: x, y, z
+    float* sL = smem + C::S_EL;                         // [c][b][MP]
+    float* sB = smem + C::S_EL + C::B_EL;               // [k][j][MP]
+    for (int64_t e = blockIdx.x; e < E; e += gridDim.x) {
+        __syncthreads();                                // the previous element is no longer read
+        copy_rows_async<float, M, NT, M * MP>(sS, S + e * 3 * M2, 3 * M);
+        copy_rows_async<float, M, NT, PS>(sL, invL + e * M3, M2);
+        io.template load<NT, PS>(sB, xtra, e, 1);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncthreads();
+        fdm_mma_phase<M, 2, true, false, false>(sB, sS + 2 * M * MP, sL, io, xtra, e);     // S_z^T
+        fdm_mma_phase<M, 1, true, false, false>(sB, sS + M * MP, sL, io, xtra, e);         // S_y^T
+        fdm_mma_phase<M, 0, true, true, false>(sB, sS, sL, io, xtra, e);                   // S_x^T, then Lambda^-1
+        fdm_mma_phase<M, 0, false, false, false>(sB, sS, sL, io, xtra, e);                 // S_x
+        fdm_mma_phase<M, 1, false, false, false>(sB, sS + M * MP, sL, io, xtra, e);        // S_y
+        fdm_mma_phase<M, 2, false, false, true>(sB, sS + 2 * M * MP, sL, io, xtra, e);     // S_z, result to the policy
+    }
+}
+
 }  // namespace sem_fdm_dev

@@ -115,6 +115,7 @@ struct sem_ctx {
     uint64_t ag_gen = 0;
     // ---- misc ----
     int ax_variant = 0;
+    int fdm_variant = 0;           // sem_set_variant(100 + v): 0 = scalar local-solve kernels, 1 = FP32 tensor-core kernel
     std::string err;
 };
 

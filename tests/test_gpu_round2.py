@@ -654,3 +654,31 @@ def test_recompute_mode_keeps_no_stored_G_and_handles_helmholtz_in_fp32(torch_cu
         x = torch_cuda.zeros_like(b)
         it, _ = sem.pcg(b, x, 1e-9, 200)
         assert it == ores["iters"] and relerr(x.cpu().numpy(), ores["x"][om.l2u]) <= TOLPCG
+
+
+@pytest.mark.parametrize("m,E", [(10, 900), (8, 700), (6, 500), (12, 300), (7, 450)])
+def test_fdm_apply_tensor_core_variant(torch_cuda, binding, oracle_mod, m, E):
+    """The FP32 tensor-core variant of the local solve (sem_set_variant(101): TF32 m16n8k8 in three passes, lines padded
+    to MMA tiles) against the oracle's Eq. (3) at 1e-5, in place and out of place."""
+    mesh = inputs.box_mesh(E, 1, 1, 1)
+    A, B = inputs.fdm_pairs(E, m, seed=70 + m)
+    S = np.empty_like(A)
+    lam = []
+    for e in range(E):
+        le = []
+        for d in range(3):
+            S[e, d], l = oracle_mod.fdm_eig(A[e, d], B[e, d])
+            le.append(l)
+        lam.append(oracle_mod.fdm_inv_lambda(*le))
+    iL = np.stack(lam)
+    b = 2.0 * inputs.hash_uniform01(9, 12, np.arange(E * m ** 3)).reshape(E, m, m, m) - 1.0
+    ou = oracle_mod.fdm_apply(S, iL, b)
+    with binding.Sem(mesh.E, 1, mesh.vert, mesh.gid) as sem:
+        sem.set_variant(101)
+        dS, dL, db = (to_dev(torch_cuda, a.ravel(), torch_cuda.float32) for a in (S, iL, b))
+        du = torch_cuda.full_like(db, float("nan"))
+        sem.fdm_apply(m, dS, dL, db, du)
+        torch_cuda.cuda.synchronize()
+        assert relerr(du.cpu().numpy(), ou.ravel()) <= TOL32
+        sem.fdm_apply(m, dS, dL, db, db)
+        assert torch_cuda.equal(db, du)
