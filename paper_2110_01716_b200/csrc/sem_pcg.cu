@@ -16,7 +16,10 @@
 namespace {
 
 // device scalars: slot(it) = 4*it + {0: p.q, 1: r.r, 2: r.z};  it = 0 holds the initial r.r and r.z
-struct PcgFlags { int done; int iters; int breakdown; int pad; };
+// `it` / `ticket` / `pq`: the graph-replayed loop keeps the iteration number on the device (k_pcg_direction's last block
+// advances it) and the operator adds p.q into the fixed slot `pq` (k_pcg_update moves it into the iteration's slot,
+// k_pcg_direction clears it): then every launch of an iteration has the same arguments and a batch is one CUDA graph
+struct PcgFlags { int done; int iters; int breakdown; int it; unsigned int ticket; int pad; double pq; };
 
 __device__ __forceinline__ void block_sum2_atomic(double a, double b, double* __restrict__ outa,
                                                   double* __restrict__ outb) {
@@ -69,7 +72,10 @@ __global__ void __launch_bounds__(256) k_pcg_update(int64_t n, int it, const dou
                                                     double* __restrict__ x, double* __restrict__ r,
                                                     double* __restrict__ scal, PcgFlags* __restrict__ flags) {
     if (flags->done) return;
-    const double pq = scal[4 * it + 0];
+    const bool dev_it = it < 0;                         // graph replay: iteration number and p.q live in `flags`
+    if (dev_it) it = flags->it;
+    const double pq = dev_it ? flags->pq : scal[4 * it + 0];
+    if (dev_it && blockIdx.x == 0 && threadIdx.x == 0) scal[4 * it + 0] = pq;
     if (!(pq > 0.0)) {                                  // breakdown (S13): stop, keep x
         if (blockIdx.x == 0 && threadIdx.x == 0) { flags->breakdown = 1; flags->iters = it; }
         // `done` is raised by k_pcg_direction so that no block of this kernel can observe it half-way
@@ -121,6 +127,8 @@ __global__ void __launch_bounds__(256) k_pcg_direction(int64_t n, int it, int ma
     if (flags->done) return;
     const bool first = blockIdx.x == 0 && threadIdx.x == 0;
     if (flags->breakdown) { if (first) flags->done = 1; return; }
+    const bool dev_it = it < 0;
+    if (dev_it) it = flags->it;
     const double rr = scal[4 * it + 1];
     const bool stop = rr <= tol2 * scal[1] || it >= maxit;
     if (first) { flags->iters = it; if (stop) flags->done = 1; }
@@ -138,6 +146,13 @@ __global__ void __launch_bounds__(256) k_pcg_direction(int64_t n, int it, int ma
         p2[v] = pv;
     }
     if ((n & 1) && first) p[n - 1] = Minv[n - 1] * r[n - 1] + beta * p[n - 1];
+    if (dev_it) {                                       // the last block to finish advances the iteration, clears p.q
+        __shared__ unsigned int last;
+        __syncthreads();
+        if (threadIdx.x == 0) last = atomicAdd(&flags->ticket, 1u) == gridDim.x - 1;
+        __syncthreads();
+        if (last && threadIdx.x == 0) { flags->ticket = 0; flags->pq = 0.0; flags->it = it + 1; }
+    }
 }
 
 }  // namespace
@@ -165,7 +180,7 @@ extern "C" int sem_pcg(sem_ctx* c, const double* b, double* x, double tol, int m
         }
         c->pcg_ready = true;
     }
-    const int64_t need = 4 * ((int64_t)maxit + 2) + 8;      // doubles; the flags live after the slots
+    const int64_t need = 4 * ((int64_t)maxit + 2) + 8;      // doubles; the flags (40 bytes) live after the slots
     if (need > c->scal_cap) {
         cudaFree(c->d_scal);
         c->d_scal = nullptr;
@@ -188,22 +203,55 @@ extern "C" int sem_pcg(sem_ctx* c, const double* b, double* x, double tol, int m
     SEM_CUDA_OK(c, cudaGetLastError());
     const double rr0 = h0[1];
     int iters = 0;
-    PcgFlags hf = {0, 0, 0, 0};
+    PcgFlags hf = {};
     if (rr0 > 0.0 && maxit > 0) {
         const double tol2 = tol > 0.0 ? tol * tol : 0.0;
         const int batch = 16;
-        for (int it = 1; it <= maxit; ++it) {
-            rc = sem_launch_ax_gs(c, c->d_p, c->d_w, SEM_F64, c->lambda, scal + 4 * it, &flags->done);
-            if (rc) return rc;
+        auto iteration = [&](int it) -> int {            // it < 0: iteration number and p.q on the device (graph replay)
+            double* dot = it < 0 ? &flags->pq : scal + 4 * it;
+            int r1 = sem_launch_ax_gs(c, c->d_p, c->d_w, SEM_F64, c->lambda, dot, &flags->done);
+            if (r1) return r1;
             if (c->d_wt8)
                 k_pcg_update<true><<<vgrid, 256, 0, st>>>(n, it, c->d_p, c->d_w, c->d_Minv, c->d_wt, c->d_wt8, x, c->d_r, scal, flags);
             else
                 k_pcg_update<false><<<vgrid, 256, 0, st>>>(n, it, c->d_p, c->d_w, c->d_Minv, c->d_wt, nullptr, x, c->d_r, scal, flags);
             k_pcg_direction<<<vgrid, 256, 0, st>>>(n, it, maxit, tol2, c->d_r, c->d_Minv, c->d_p, scal, flags);
-            if (it % batch == 0 || it == maxit) {
+            return SEM_OK;
+        };
+        // One CUDA graph of `batch` iterations, replayed until the device raises `done` (non-default streams; meshes
+        // whose operator is a single launch pair).  The kernels' sum is what an iteration costs; the ~2 us of stream-launch
+        // gap per kernel is what the graph removes.
+        cudaGraphExec_t gexec = nullptr;
+        const bool graphable = st != nullptr && st != cudaStreamLegacy && c->chunk_e0.size() < 3 && maxit >= batch;
+        if (graphable && cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+            for (int q = 0; q < batch && rc == SEM_OK; ++q) rc = iteration(-1);
+            cudaGraph_t graph = nullptr;
+            const cudaError_t e = cudaStreamEndCapture(st, &graph);
+            if (rc != SEM_OK || e != cudaSuccess || !graph || cudaGraphInstantiate(&gexec, graph, 0) != cudaSuccess) gexec = nullptr;
+            if (graph) cudaGraphDestroy(graph);
+            cudaGetLastError();
+            if (rc != SEM_OK) return rc;
+        } else {
+            cudaGetLastError();
+        }
+        if (gexec) {
+            const int one = 1;
+            SEM_CUDA_OK(c, cudaMemcpyAsync(&flags->it, &one, sizeof(int), cudaMemcpyHostToDevice, st));
+            for (int it0 = 1; it0 <= maxit; it0 += batch) {
+                SEM_CUDA_OK(c, cudaGraphLaunch(gexec, st));
                 SEM_CUDA_OK(c, cudaMemcpyAsync(&hf, flags, sizeof(hf), cudaMemcpyDeviceToHost, st));
                 SEM_CUDA_OK(c, cudaStreamSynchronize(st));
                 if (hf.done) break;
+            }
+            cudaGraphExecDestroy(gexec);
+        } else {
+            for (int it = 1; it <= maxit; ++it) {
+                if ((rc = iteration(it))) return rc;
+                if (it % batch == 0 || it == maxit) {
+                    SEM_CUDA_OK(c, cudaMemcpyAsync(&hf, flags, sizeof(hf), cudaMemcpyDeviceToHost, st));
+                    SEM_CUDA_OK(c, cudaStreamSynchronize(st));
+                    if (hf.done) break;
+                }
             }
         }
         SEM_CUDA_OK(c, cudaGetLastError());
@@ -306,7 +354,8 @@ extern "C" int sem_pcg_many(sem_ctx* c, const double* b, double* x, int nfields,
     // a field with a zero initial residual has nothing to do: raise its flag now
     for (int f = 0; f < nf; ++f)
         if (!(rr0[f] > 0.0) || maxit == 0) {
-            const PcgFlags done = {1, 0, 0, 0};
+            PcgFlags done = {};
+            done.done = 1;
             cudaMemcpyAsync(fl[f], &done, sizeof(done), cudaMemcpyHostToDevice, st);
         }
     PcgFlags hf[8] = {};

@@ -682,3 +682,40 @@ def test_fdm_apply_tensor_core_variant(torch_cuda, binding, oracle_mod, m, E):
         assert relerr(du.cpu().numpy(), ou.ravel()) <= TOL32
         sem.fdm_apply(m, dS, dL, db, db)
         assert torch_cuda.equal(db, du)
+
+
+def test_pcg_graph_replay_on_side_stream(torch_cuda, binding, oracle_mod):
+    """On a non-default stream sem_pcg replays one CUDA graph of 16 iterations (iteration number and p.q kept on the
+    device): the config-1 trajectory after 20 iterations (maxit ends inside the second batch), a converged solve
+    (iteration count, history, solution) and a zero right-hand side equal the oracle's, as on the default stream."""
+    m = inputs.config1()
+    om = oracle_mod.Maps(m.gid)
+    oG, _, rc = oracle_mod.geom_trilinear(m.vert, m.N)
+    mask_u = oracle_mod.mask_unique(m.dirichlet, om)
+    xyz = oracle_mod.node_xyz(m.vert, m.N).reshape(-1, 3)
+    us = np.zeros(om.U)
+    us[om.l2u] = np.sin(np.pi * xyz[:, 0]) * np.sin(np.pi * xyz[:, 1]) * np.sin(np.pi * xyz[:, 2])
+    us[mask_u != 0] = 0.0
+    b_u = oracle_mod.apply_Ag(oG, m.N, om, mask_u, us)
+    o20 = oracle_mod.pcg(oG, m.N, om, mask_u, b_u, tol=1e-30, maxit=20)
+    ofull = oracle_mod.pcg(oG, m.N, om, mask_u, b_u, tol=1e-10, maxit=400)
+    side = torch_cuda.cuda.Stream()
+    with torch_cuda.cuda.stream(side):
+        with binding.Sem(m.E, m.N, m.vert, m.gid, m.dirichlet) as sem:
+            sem.geom()
+            b = to_dev(torch_cuda, b_u[om.l2u])
+            for _ in range(2):                                   # the second call builds its graph anew
+                x = torch_cuda.zeros_like(b)
+                it, rel = sem.pcg(b, x, 1e-30, 20)
+                assert it == 20 and abs(rel - o20["relres"]) <= 1e-9 * o20["relres"]
+                assert relerr(x.cpu().numpy(), o20["x"][om.l2u]) <= TOLPCG
+            x = torch_cuda.zeros_like(b)
+            it, rel = sem.pcg(b, x, 1e-10, 400)
+            assert it == ofull["iters"] and rel <= 1e-10
+            assert relerr(x.cpu().numpy(), ofull["x"][om.l2u]) <= TOLPCG
+            h = sem.pcg_history(it + 1)
+            big = ofull["hist"] >= 1e-4                          # below that the recurrence residual drifts by round-off
+            assert np.max(np.abs(h - ofull["hist"])[big] / ofull["hist"][big]) <= 1e-5
+            xz = torch_cuda.ones_like(b)
+            itz, relz = sem.pcg(torch_cuda.zeros_like(b), xz.zero_(), 1e-8, 50)
+            assert itz == 0
