@@ -199,3 +199,52 @@ def fdm_pairs(E: int, m: int, seed: int):
             A[e, d, q[:-1], q[1:]] = A[e, d, q[1:], q[:-1]] = -1.0 / s[1:-1]
             B[e, d, q, q] = 0.5 * (s[:-1] + s[1:])
     return A, B
+
+
+# ---- re-oriented elements: the same mesh with every element's local frame rotated (unstructured-mesh orientations) -------
+def _proper_rotations():
+    """The 24 signed permutations (pi, s) of the reference cube with determinant +1: old coordinate a = s[a] * new
+    coordinate pi[a]."""
+    import itertools
+    out = []
+    for pi in itertools.permutations(range(3)):
+        par = 1
+        for a in range(3):
+            for b in range(a + 1, 3):
+                if pi[a] > pi[b]:
+                    par = -par
+        for s in itertools.product((1, -1), repeat=3):
+            if par * s[0] * s[1] * s[2] == 1:
+                out.append((pi, s))
+    return out
+
+
+def reorient(mesh: BoxMesh, seed: int) -> BoxMesh:
+    """The same elements, nodes and global ids, but every element's local (r, s, t) frame replaced by one of the 24
+    proper rotations of the reference cube, chosen by a hash of (seed, element): local node (i0', i1', i2') of the new
+    element is old local node i_a = i'_{pi[a]} (s[a] = +1) or N - i'_{pi[a]} (s[a] = -1), vertices alike.  Neighbouring
+    elements then meet with arbitrary relative orientation, as in an unstructured hexahedral mesh; the Jacobian
+    determinant stays positive.  Mesh layout only: no method arithmetic."""
+    N, p, E = mesh.N, mesh.N + 1, mesh.E
+    rots = _proper_rotations()
+    pick = (hash_uniform01(seed, 30, np.arange(E)) * len(rots)).astype(np.int64) % len(rots)
+    gid = mesh.gid.reshape(E, p, p, p).copy()
+    dirf = mesh.dirichlet.reshape(E, p, p, p).copy()
+    vert = mesh.vert.copy()
+    idx = np.arange(p)
+    for e in range(E):
+        pi, s = rots[int(pick[e])]
+        # new index tuple n = (n0, n1, n2) = (i', j', k'); old index o_a = n[pi[a]] or N - n[pi[a]]
+        n = np.meshgrid(idx, idx, idx, indexing="ij")            # n[0] = i', n[1] = j', n[2] = k'  (arrays [i'][j'][k'])
+        o = [n[pi[a]] if s[a] > 0 else N - n[pi[a]] for a in range(3)]
+        g_old, d_old = mesh.gid.reshape(E, p, p, p)[e], mesh.dirichlet.reshape(E, p, p, p)[e]
+        g_new = g_old[o[2], o[1], o[0]]                          # arrays are stored [k][j][i]; result indexed [i'][j'][k']
+        d_new = d_old[o[2], o[1], o[0]]
+        gid[e] = np.transpose(g_new, (2, 1, 0))
+        dirf[e] = np.transpose(d_new, (2, 1, 0))
+        for v in range(8):
+            nb = [(v >> a) & 1 for a in range(3)]
+            ob = [nb[pi[a]] if s[a] > 0 else 1 - nb[pi[a]] for a in range(3)]
+            vert[e, v] = mesh.vert[e, ob[0] + 2 * ob[1] + 4 * ob[2]]
+    return BoxMesh(mesh.nx, mesh.ny, mesh.nz, N, vert, np.ascontiguousarray(gid.reshape(E, p ** 3)),
+                   np.ascontiguousarray(dirf.reshape(E, p ** 3)), mesh.perm, mesh.name + "_reoriented")

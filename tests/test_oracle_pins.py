@@ -908,3 +908,35 @@ def test_W5_schwarz_smoothing_beats_jacobi_smoothing_in_the_vcycle(oracle_mod):
     rs = oracle_mod.fpcg(ls[0], lambda r: oracle_mod.vcycle(ls, r, 2, 8), b, tol=1e-10, maxit=60)
     assert rs["hist"][-1] <= 1e-10 and rs["iters"] < rj["iters"]
     assert np.max(np.abs(rs["x"] - xs)) <= 1e-8 * np.max(np.abs(xs))
+
+
+def test_W6_results_do_not_depend_on_the_elements_local_orientation(oracle_mod):
+    """Rotating every element's local (r, s, t) frame by a seeded proper rotation of the cube (inputs.reorient: the same
+    nodes and global ids, neighbours now meet with arbitrary relative orientation, as in an unstructured mesh) changes
+    every local array but no unique-node result: the assembled operator, the Jacobi diagonal, the PCG iterates and both
+    Schwarz variants.  A face link that assumes aligned neighbours, a wrong factor order or a transposed D fails."""
+    m0 = inputs.box_mesh(3, 3, 2, 4, "random", seed=5)
+    m1 = inputs.reorient(m0, 7)
+    assert not np.array_equal(m0.gid, m1.gid)
+    o0, o1 = oracle_mod.Maps(m0.gid), oracle_mod.Maps(m1.gid)
+    assert np.array_equal(o0.uniq_gid, o1.uniq_gid) and np.array_equal(o0.mult, o1.mult)
+    G0, dJ0, rc0 = oracle_mod.geom_trilinear(m0.vert, m0.N)
+    G1, dJ1, rc1 = oracle_mod.geom_trilinear(m1.vert, m1.N)
+    assert rc0 == 0 and rc1 == 0 and dJ1.min() > 0.0
+    k0, k1 = oracle_mod.mask_unique(m0.dirichlet, o0), oracle_mod.mask_unique(m1.dirichlet, o1)
+    assert np.array_equal(k0, k1)
+    x = np.where(k0 != 0, 0.0, inputs.field_normal(o0.uniq_gid, 3))
+    y0, y1 = oracle_mod.apply_Ag(G0, m0.N, o0, k0, x, 2.0), oracle_mod.apply_Ag(G1, m1.N, o1, k1, x, 2.0)
+    assert np.max(np.abs(y0 - y1)) <= 1e-13 * np.max(np.abs(y0))
+    d0, d1 = np.zeros(o0.U), np.zeros(o1.U)
+    np.add.at(d0, o0.l2u, oracle_mod.diag_local(G0, m0.N).ravel())
+    np.add.at(d1, o1.l2u, oracle_mod.diag_local(G1, m1.N).ravel())
+    assert np.max(np.abs(d0 - d1)) <= 1e-13 * np.max(np.abs(d0))
+    r0 = oracle_mod.pcg(G0, m0.N, o0, k0, y0, tol=1e-10, maxit=300, lam=2.0)
+    r1 = oracle_mod.pcg(G1, m1.N, o1, k1, y1, tol=1e-10, maxit=300, lam=2.0)
+    assert r0["iters"] == r1["iters"] and np.max(np.abs(r0["x"] - r1["x"])) <= 1e-9 * np.max(np.abs(r0["x"]))
+    for restricted in (False, True):
+        s0 = oracle_mod.Schwarz(m0, o0, k0, restricted)
+        s1 = oracle_mod.Schwarz(m1, o1, k1, restricted)
+        z0, z1 = s0.apply(x), s1.apply(x)
+        assert np.max(np.abs(z0 - z1)) <= 1e-12 * np.max(np.abs(z0)), restricted
