@@ -785,3 +785,40 @@ def test_reoriented_elements(torch_cuda, binding, oracle_mod, N):
     finally:
         for s in shards:
             s.close()
+
+
+def test_vcycle_ras_on_reoriented_levels(torch_cuda, binding, oracle_mod):
+    """The 7-3-1 V-cycle with Chebyshev-RAS smoothing (order 1) on levels whose elements are all rotated the same seeded
+    way (the transfers are element-local tensor products, so every level must use the same frames): the cycle equals the
+    oracle's (FP64 1e-9) and flexible PCG takes the oracle's iteration count."""
+    orders = (7, 3, 1)
+    meshes = [inputs.reorient(inputs.box_mesh(4, 3, 3, N, "random", seed=3), 5) for N in orders]
+    olv = [oracle_mod.Level(m) for m in meshes]
+    for L, m in zip(olv[:-1], meshes[:-1]):
+        L.use_schwarz(m, restricted=True)
+    L0 = olv[0]
+    xs = np.where(L0.mask_u != 0, 0.0, inputs.field_normal(L0.maps.uniq_gid, 17))
+    b_u = L0.A(xs)
+    oz = oracle_mod.vcycle(olv, b_u, 1, 8)
+    ores = oracle_mod.fpcg(L0, lambda r: oracle_mod.vcycle(olv, r, 1, 8), b_u, tol=1e-8, maxit=60)
+    side = torch_cuda.cuda.Stream()
+    with torch_cuda.cuda.stream(side):
+        sems = [binding.Sem(m.E, m.N, m.vert, m.gid, m.dirichlet).geom() for m in meshes]
+        try:
+            slmin = [getattr(l, "slmin", l.lmin) for l in olv]
+            slmax = [getattr(l, "slmax", l.lmax) for l in olv]
+            with binding.Pmg(sems, [l.lmin for l in olv], [l.lmax for l in olv], 1, 8, binding.SEM_F64) as mg:
+                mg.set_smoother(binding.SEM_SMOOTH_CHEBY_RAS, slmin, slmax)
+                dr = to_dev(torch_cuda, b_u[L0.maps.l2u])
+                dz = torch_cuda.full_like(dr, float("nan"))
+                for _ in range(3):
+                    mg.vcycle(dr, dz)
+                side.synchronize()
+                assert relerr(dz.cpu().numpy(), oz[L0.maps.l2u]) <= 1e-9
+                x = torch_cuda.full_like(dr, float("nan"))
+                it, rel = mg.fpcg(dr, x, 1e-8, 60)
+                assert rel <= 1e-8 and it == ores["iters"]
+                assert relerr(x.cpu().numpy(), ores["x"][L0.maps.l2u]) <= 1e-7
+        finally:
+            for s_ in sems:
+                s_.close()
