@@ -137,7 +137,12 @@ SEM_API int sem_ax_gs(sem_ctx* ctx, const void* u, void* w, sem_prec prec, doubl
  *   iters_out   HOST  number of operator applications in the loop
  *   relres_out  HOST  ||r|| / r0 from the recurrence
  * Reaching maxit is not an error; r0 == 0 (e.g. b == 0 with x0 == 0) returns x = M x0 after 0 iterations;
- * p.q <= 0 stops (breakdown) with SEM_OK. */
+ * p.q <= 0 stops (breakdown) with SEM_OK.
+ * Execution: all scalars stay on the device (no host round trip per iteration; the host polls a flag every 16
+ * iterations); on a non-default stream 16 iterations are one CUDA graph, replayed.  The dot products are reduced with
+ * FP64 atomics, so iterates are repeatable to round-off, not bit for bit.  On a large mesh (fields > 256 MB) whose
+ * element order has no locality the loop runs on an inner copy of the context with the elements sorted by smallest
+ * global id (b and x are gathered / scattered in element blocks); results are unchanged to round-off. */
 SEM_API int sem_pcg(sem_ctx* ctx, const double* b, double* x, double tol, int maxit, int* iters_out, double* relres_out);
 
 /* Helmholtz shift used by sem_pcg and by the Jacobi diagonal (default 0).  Requires with_mass if != 0. */

@@ -10,6 +10,11 @@
 //     (cp.async.bulk + mbarrier transaction counts, evict-first in L2) issued NS slabs ahead, so the bytes in flight per
 //     SM do not depend on registers or occupancy;  u arrives the same way, double-buffered per element;
 //   * persistent CTAs (one element group at a time, grid = SMs x resident CTAs) write w straight from registers.
+// That is ax_stream (every p <= 12; odd p takes u by plain loads).  At p = 8 -- the paper's N = 7 -- the r and s
+// contractions run on the tensor cores instead, one WARP per element with the same streaming ring: ax_dmma (FP64,
+// mma.sync m8n8k4; the measured DMMA path north_star asks for: it won), ax_tf32 (FP32, m16n8k8 TF32 in three passes),
+// ax_dmma_many (2 or 3 fields sharing one pass over G).  Kernels in this file, in order: ax_simple, ax_stream, ax_dmma,
+// ax_tf32, ax_dmma_many; then the launchers and the chunked operator / gather-scatter driver (sem_launch_ax_gs).
 // ax_simple is the plain-load version of the same arithmetic: p > 12, unaligned pointers, and the recomputed-G
 // variant (a9: G from the 8 trilinear vertices inside the kernel) use it.
 #include <mutex>
