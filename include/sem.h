@@ -317,7 +317,8 @@ SEM_API int sem_measure_peak(int kind, void* cuda_stream, double* tflops_out);
  * measured slower than the scalar kernels at every m, kept as the measurement north_star asks for).
  * Environment knobs read at setup (tests, experiments): SEM_CHUNK_GROUPS = element groups per chunk of the chunked
  * operator / gather-scatter (fields larger than L2; a huge value disables it); SEM_INNER = 0 / 1 never / always build the
- * renumbered inner context that sem_pcg uses on large meshes without locality. */
+ * renumbered inner context that sem_pcg uses on large meshes without locality; SEM_COARSE = 0 keeps sem_cheby at N = 1
+ * on the matrix-free operator (default: the assembled N = 1 operator, one kernel per Chebyshev step). */
 SEM_API int sem_set_variant(sem_ctx* ctx, int ax_variant);
 
 /* Last error text of this context ("" if none); valid until the next call on the context.  NULL ctx -> static text. */

@@ -82,6 +82,7 @@ int sem_geom(sem_ctx* c, const double* node_xyz, sem_gmode mode, int with_mass) 
         return sem_fail(c, SEM_ESTATE, "SEM_G_RECOMPUTE needs trilinear geometry (node_xyz == NULL)");
     c->geom_done = false;
     sem_schwarz_free(c);        // the Schwarz smoother's factorisations belong to the geometry (and are baked into graphs)
+    sem_coarse_free(c);         // so does the assembled coarse operator
     ++c->generation;
     c->pcg_ready = false;
     c->lambda_of_diag = -1.0;   // invalidates the Jacobi diagonal (lambda >= 0 always)
@@ -279,6 +280,7 @@ void sem_ctx_destroy(sem_ctx* c) {
     if (c->ag_exec) cudaGraphExecDestroy(c->ag_exec);
     sem_inner_free(c);
     sem_schwarz_free(c);
+    sem_coarse_free(c);
     void* ptrs[] = {c->d_vert, c->d_l2u, c->d_mult, c->d_seg_off, c->d_seg_idx, c->d_uniq_gid, c->d_sh_off, c->d_sh_idx,
                     c->d_sh_masked, c->d_mask_u, c->d_mask1_idx, c->d_G, c->d_G32, c->d_B, c->d_B32, c->d_detJ,
                     c->d_diag, c->d_Minv, c->d_wt, c->d_wt8, c->d_r, c->d_p, c->d_w, c->d_scal, 

@@ -12,6 +12,7 @@
 // one operator application and ONE fused vector kernel (x += d; r -= Minv w; d = c1 d + c2 r); the final x += d is
 // folded into the last step, which then writes only x, and a zero initial guess is never read or pre-zeroed.
 #include <math.h>
+#include <stdlib.h>
 
 #include "sem_internal.h"
 
@@ -272,6 +273,20 @@ extern "C" int sem_cheby(sem_ctx* c, const void* b, void* x, int order, double l
         if (!c->d_Minv32) SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_Minv32, c->nL * sizeof(float)));
         k_minv32<<<(unsigned)c->num_sms * 8, 256, 0, c->stream>>>(c->nL, c->d_Minv, c->d_Minv32);
         c->lambda_of_minv32 = c->lambda;
+    }
+    // N = 1 (the coarsest multigrid level): the operator is assembled once and a whole step is one kernel (sem_coarse.cu).
+    // The assembly runs operator applications and synchronises, so it happens on an eager call, never inside a capture.
+    if (c->p == 2 && c->gmode == SEM_G_STORED) {
+        const char* env = getenv("SEM_COARSE");
+        if (!(env && env[0] == '0')) {
+            cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+            if (c->stream != cudaStreamLegacy && c->stream != nullptr) cudaStreamIsCapturing(c->stream, &cs);
+            const bool have = c->coarse != nullptr && sem_coarse_is_current(c);
+            if (have || cs == cudaStreamCaptureStatusNone) {
+                if (!have && (rc = sem_coarse_build(c))) return rc;
+                return sem_coarse_cheby(c, b, x, order, lmin, lmax, zero_guess != 0, prec);
+            }
+        }
     }
     if (prec == SEM_F64) return run<double>(c, (const double*)b, (double*)x, order, lmin, lmax, zero_guess != 0);
     return run<float>(c, (const float*)b, (float*)x, order, lmin, lmax, zero_guess != 0);

@@ -21,6 +21,7 @@ __host__ __device__ inline int64_t sem_g_off(int64_t e, int k, int p, int epb, i
 }
 
 struct sem_schwarz_data;            // sem_schwarz.cu
+struct sem_coarse_data;             // sem_coarse.cu
 
 struct sem_ctx {
     // ---- discretisation (a0) ----
@@ -102,6 +103,7 @@ struct sem_ctx {
     bool is_inner = false;
     int32_t* d_perm = nullptr;      // [E] inner position q holds caller element d_perm[q]
     double *d_bi = nullptr, *d_xi = nullptr;
+    sem_coarse_data* coarse = nullptr;   // N = 1: assembled operator of the coarsest multigrid level (sem_coarse.cu)
     sem_schwarz_data* sw = nullptr; // NEXT-2b: face links, 1-D operator factorisations, weights (sem_schwarz_setup)
     uint64_t generation = 0;       // bumped whenever device pointers or parameters that launches capture may change
                                    // (sem_geom, sem_set_lambda): invalidates CUDA graphs recorded over this context
@@ -165,6 +167,12 @@ int sem_inner_pcg(sem_ctx* c, const double* b, double* x, double tol, int maxit,
 // sem_fdm.cu
 int sem_launch_fdm_schwarz(sem_ctx* c, int m, const void* S, const void* invL, const void* r, const int4* link,
                            const int32_t* nrm, const void* W, void* z, sem_prec prec);
+// sem_coarse.cu
+int sem_coarse_build(sem_ctx* c);
+void sem_coarse_free(sem_ctx* c);
+bool sem_coarse_is_current(const sem_ctx* c);     // built for the context's current lambda
+int sem_coarse_cheby(sem_ctx* c, const void* b, void* x, int order, double lmin, double lmax, bool zero_guess,
+                     sem_prec prec);
 // sem_schwarz.cu
 void sem_schwarz_free(sem_ctx* c);
 int sem_launch_schwarz(sem_ctx* c, const void* r, void* z, sem_prec prec, int kind);   // z may alias r

@@ -822,3 +822,37 @@ def test_vcycle_ras_on_reoriented_levels(torch_cuda, binding, oracle_mod):
         finally:
             for s_ in sems:
                 s_.close()
+
+
+@pytest.mark.parametrize("masked,lam,order,zero_guess", [(True, 0.0, 8, True), (False, 2.5, 5, False), (True, 1.0, 1, True),
+                                                         (True, 0.0, 2, False)])
+def test_assembled_coarse_operator(torch_cuda, binding, oracle_mod, monkeypatch, masked, lam, order, zero_guess):
+    """N = 1: sem_cheby runs on the assembled operator (one kernel per Chebyshev step, no gather-scatter).  Against the
+    oracle's Chebyshev-Jacobi and against the matrix-free path (SEM_COARSE=0), FP64 1e-11 and FP32 1e-5, masked and not,
+    Helmholtz, zero and non-zero guess, re-oriented scrambled elements; the result stays continuous bit for bit."""
+    m = inputs.reorient(inputs.box_mesh(6, 5, 4, 1, "random", seed=12, permute_seed=3), 2)
+    if not masked:
+        m.dirichlet[:] = 0
+    L = oracle_mod.Level(m, power_its=30, lam=lam)
+    b_u = L.A(np.where(L.mask_u != 0, 0.0, inputs.field_normal(L.maps.uniq_gid, 3))) + 0.1
+    b_u[L.mask_u != 0] = 0.0
+    x0_u = None if zero_guess else np.where(L.mask_u != 0, 0.0, inputs.field_normal(L.maps.uniq_gid, 4))
+    ox = L.smooth(b_u, x0_u, order)[L.maps.l2u]
+    outs = {}
+    for env in ("1", "0"):
+        monkeypatch.setenv("SEM_COARSE", env)
+        with binding.Sem(m.E, m.N, m.vert, m.gid, m.dirichlet if masked else None) as sem:
+            sem.geom(with_mass=lam != 0.0)
+            sem.set_lambda(lam)
+            for dt, tol in ((torch_cuda.float64, 1e-11), (torch_cuda.float32, TOL32)):
+                db = to_dev(torch_cuda, b_u[L.maps.l2u], dt)
+                dx = torch_cuda.full_like(db, float("nan")) if zero_guess else to_dev(torch_cuda, x0_u[L.maps.l2u], dt)
+                sem.cheby(db, dx, order, L.lmin, L.lmax, zero_guess)
+                torch_cuda.cuda.synchronize()
+                got = dx.cpu().numpy()
+                assert relerr(got, ox) <= tol, (env, dt)
+                outs[(env, dt)] = got
+                if env == "1":                                  # every copy of a unique node holds the same bits
+                    first = L.maps.seg_idx[L.maps.seg_off[:-1]]
+                    assert np.array_equal(got, got[first][L.maps.l2u])
+    assert relerr(outs[("1", torch_cuda.float64)], outs[("0", torch_cuda.float64)]) <= 1e-12
