@@ -476,60 +476,124 @@ def run_leg(args):
 
 
 def run_sharded(args):
-    """--sharded-n n: NEXT-4, the operator with the ELEMENTS partitioned over the ranks (contiguous blocks of a config-5
-    style mesh of n^3 elements, scrambled order), one interface exchange per application over NCCL
-    (paper_2110_01716_b200/sharded.py).  Strong scaling: the total work is fixed.  Not the default multi-GPU mode
-    (north_star scopes the headline to replicas); this build could only run it on one GPU and as a one-GPU emulation."""
+    """--sharded-n n: NEXT-4, operator and Jacobi-PCG with the ELEMENTS partitioned over the ranks (contiguous blocks of
+    a config-5 style mesh of n^3 elements, scrambled order unless --sharded-lex), interface exchange and all-reduces
+    through the hooks of paper_2110_01716_b200/sharded.py.  Strong scaling: the total work is fixed.  Not the default
+    multi-GPU mode (north_star scopes the headline to replicas).  Under torchrun: one rank per GPU over NCCL.  With
+    --emulate-ranks R (one process, one GPU): R ranks on R host threads sharing the GPU, which serialises them -- the
+    time is the SUM over ranks and shows what the partition costs (split launches, pack / add kernels, hook calls)
+    against the single-context call on the same mesh, not a speed-up."""
     import torch
     import torch.distributed as dist
 
-    from paper_2110_01716_b200 import build, inputs, sharded
-    world = int(os.environ.get("WORLD_SIZE", "1"))
+    from paper_2110_01716_b200 import binding, build, inputs, sharded
+    emu = args.emulate_ranks
+    world = emu if emu > 0 else int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
-    if not dist.is_initialized():
-        if world == 1:
-            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-            os.environ.setdefault("MASTER_PORT", "29531")
-        dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", local))
-    if rank == 0:
+    if emu == 0:
+        if not dist.is_initialized():
+            if world == 1:
+                os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+                os.environ.setdefault("MASTER_PORT", "29531")
+            dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", local))
+        if rank == 0:
+            build.build()
+        dist.barrier()
+    else:
         build.build()
-    dist.barrier()
-    mesh = inputs.config5(args.sharded_n)
-    b = sharded.partition_bounds(mesh.E, world)
-    sl = slice(b[rank], b[rank + 1])
-    sh = sharded.ShardedSem(sharded.DistComm(), b[rank + 1] - b[rank], mesh.N, mesh.vert[sl], mesh.gid[sl],
-                            mesh.dirichlet[sl]).geom()
-    u = torch.from_numpy(inputs.field_uniform(mesh.gid[sl], 0).ravel()).cuda()
-    w = torch.empty_like(u)
+    n = args.sharded_n
+    mesh = inputs.box_mesh(n, n, n, 7, "random", seed=3, name=f"lex{n}") if args.sharded_lex else inputs.config5(n)
+    # the scrambled order has no locality: contiguous blocks would put every element on the interface -> bisection
+    part = ([np.arange(lo, hi) for lo, hi in zip(sharded.partition_bounds(mesh.E, world)[:-1],
+                                                 sharded.partition_bounds(mesh.E, world)[1:])]
+            if args.sharded_lex else sharded.partition_rcb(mesh.vert, world))
     K, W = max(args.steps, 20), max(args.warmup, 3)
-    for _ in range(W):
-        sh.ax_gs(u, w)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize()
-    dist.barrier()
-    torch.cuda.synchronize()
-    e0.record()
-    for _ in range(K):
-        sh.ax_gs(u, w)
-    e1.record()
-    torch.cuda.synchronize()
-    dist.barrier()
-    ms = max_over_ranks(e0.elapsed_time(e1), world, "cuda")
-    ib = torch.tensor([sh.interface_bytes()], device="cuda", dtype=torch.float64)
-    dist.all_reduce(ib)
+    pcg_its = 50
+    side = torch.cuda.Stream()
+    torch.cuda.set_stream(side)
+
+    def make(r, comm):
+        sl = part[r]
+        sh = sharded.ShardedSem(comm, len(sl), mesh.N, mesh.vert[sl], mesh.gid[sl], mesh.dirichlet[sl],
+                                stream=side).geom()
+        u = torch.from_numpy(sh.to_local(inputs.field_uniform(mesh.gid[sl], 0)).ravel()).cuda()
+        return sh, u, torch.empty_like(u), torch.zeros_like(u)
+
+    def timed(fn):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        if emu == 0:
+            dist.barrier()
+            torch.cuda.synchronize()
+        e0.record(side)
+        fn()
+        e1.record(side)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1)
+
+    if emu > 0:
+        gath = sharded.local_gathers(mesh.N, [mesh.gid[part[r]] for r in range(world)],
+                                     [mesh.dirichlet[part[r]] for r in range(world)])
+        tw = sharded.ThreadWorld(world, timeout=600.0)
+        parts = [make(r, sharded.ThreadComm(tw, r, *gath)) for r in range(world)]
+
+        def apply_all(k):
+            sharded.run_ranks(world, lambda r: [parts[r][0].ax_gs(parts[r][1], parts[r][2]) for _ in range(k)], tw)
+
+        def pcg_all():
+            return sharded.run_ranks(world, lambda r: parts[r][0].pcg(parts[r][1], parts[r][3].zero_(), 1e-30, pcg_its), tw)
+
+        apply_all(W)
+        ms = timed(lambda: apply_all(K))
+        pcg_all()
+        ms_pcg = timed(pcg_all)
+        with binding.Sem(mesh.E, mesh.N, mesh.vert, mesh.gid, mesh.dirichlet, stream=side) as one:
+            one.geom()
+            u1 = torch.from_numpy(inputs.field_uniform(mesh.gid, 0).ravel()).cuda()
+            w1, x1 = torch.empty_like(u1), torch.zeros_like(u1)
+            for _ in range(W):
+                one.ax_gs(u1, w1)
+            ms_one = timed(lambda: [one.ax_gs(u1, w1) for _ in range(K)])
+            one.pcg(u1, x1, 1e-30, pcg_its)
+            ms_pcg_one = timed(lambda: one.pcg(u1, x1.zero_(), 1e-30, pcg_its))
+        shs = [p[0] for p in parts]
+        ib = float(sum(s.interface_bytes() for s in shs))
+        extra = {"emulated_ranks_on_one_gpu": world, "time_is": "sum over ranks (they share the GPU)",
+                 "single_context_ms_per_step": ms_one / K, "single_context_pcg_ms_per_iter": ms_pcg_one / pcg_its,
+                 "interface_elements_per_rank": [s.n_iface for s in shs], "elements_per_rank": [s.E for s in shs],
+                 "chunks_per_rank": [len(s.sem.chunks()[0]) - 1 for s in shs]}
+        launches = K * sum(2 * (len(s.sem.chunks()[0]) - 1) + 2 * len(s.uniq) for s in shs)
+    else:
+        sh, u, w, x = make(rank, sharded.DistComm())
+        for _ in range(W):
+            sh.ax_gs(u, w)
+        ms = max_over_ranks(timed(lambda: [sh.ax_gs(u, w) for _ in range(K)]), world, "cuda")
+        sh.pcg(u, x, 1e-30, pcg_its)
+        ms_pcg = max_over_ranks(timed(lambda: sh.pcg(u, x.zero_(), 1e-30, pcg_its)), world, "cuda")
+        t = torch.tensor([sh.interface_bytes()], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t)
+        ib = float(t.item())
+        shs = [sh]
+        extra = {"interface_elements_this_rank": sh.n_iface, "elements_this_rank": sh.E}
+        launches = K * (2 * (len(sh.sem.chunks()[0]) - 1) + 2 * len(sh.uniq))
     if rank == 0:
         print(json.dumps({
             "metric": "Ax+gs GDOF/s (FP64, N=7), elements partitioned over the ranks", "value": mesh.dofs * K / (ms * 1e-3) / 1e9,
-            "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K, "higher_is_better": True,
+            "unit": UNIT, "n_gpus": 1 if emu else world, "steps": K, "warmup": W, "ms_per_step": ms / K, "higher_is_better": True,
             "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"config5-style {args.sharded_n}^3 hex, N=7, scrambled order, Dirichlet; contiguous "
-                                   f"element blocks per rank, one interface exchange per application",
-                       "E": mesh.E, "interface_bytes_sent_per_step_all_ranks": float(ib.item())},
-            "gpu_launches": K * (2 + 2 * len(sh.uniq))}))
-    sh.close()
-    dist.destroy_process_group()
+            "config": {"workload": f"{'lexicographic' if args.sharded_lex else 'config5-style scrambled'} {n}^3 hex, N=7, "
+                                   "random +-10 % vertices, Dirichlet; "
+                                   f"{'contiguous element blocks' if args.sharded_lex else 'coordinate bisection'} per rank, interface "
+                                   "elements first, exchange started after the interface chunk",
+                       "E": mesh.E, "interface_bytes_sent_per_step_all_ranks": ib, **extra},
+            "pcg_sharded": {"iters": pcg_its, "ms_per_iter": ms_pcg / pcg_its, "allreduces_per_iter": 2},
+            "gpu_launches": launches}))
+    for s in shs:
+        s.close()
+    if emu == 0:
+        dist.destroy_process_group()
 
 
 def main():
@@ -545,6 +609,9 @@ def main():
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--pcg-iters", type=int, default=300)
     ap.add_argument("--config5-n", type=int, default=100, help="elements per direction of the config-5 leg (0 = skip)")
+    ap.add_argument("--emulate-ranks", type=int, default=0,
+                    help="with --sharded-n, one process: this many ranks on host threads sharing one GPU")
+    ap.add_argument("--sharded-lex", action="store_true", help="with --sharded-n: lexicographic element order (slabs)")
     ap.add_argument("--sharded-n", type=int, default=0,
                     help="NEXT-4: > 0 runs the element-partitioned operator on a config-5 style mesh of n^3 elements")
     ap.add_argument("--max-n", type=int, default=64)

@@ -122,6 +122,50 @@ SEM_API int sem_pcg_many(sem_ctx* ctx, const double* b, double* x, int nfields, 
 SEM_API int sem_iface_pack(sem_ctx* ctx, const int32_t* uniq, int64_t n, const void* w, void* buf, sem_prec prec);
 SEM_API int sem_iface_add(sem_ctx* ctx, const int32_t* uniq, int64_t n, const void* buf, void* w, sem_prec prec);
 
+/* NEXT-4, the sharded operator and solver (P:89 overlap of the non-local gather-scatter with interior work; P:101;
+ * P:119-121).  The library runs every kernel; the transport between ranks is the caller's and reaches the library
+ * through three hooks, each called on the host from inside the library call and expected to ORDER its work on the
+ * context's stream (enqueue and return; no host synchronisation needed) and to return 0 on success:
+ *   gs_begin(user, w, prec)    the rank-local sums of all nodes shared with other ranks are final in w (DEVICE, [nL]
+ *                              values of sem_prec `prec`): pack them (sem_iface_pack) and start sending/receiving;
+ *   gs_end(user, w, prec)      wait for the peers' buffers and add them (sem_iface_add, ascending rank order);
+ *                              between the two calls the library launches work that touches no shared node;
+ *   allreduce(user, s, n)      s DEVICE double[n]: replace by the sum over all ranks, the same bits on every rank.
+ * The hooks struct is read during the call only.  Dirichlet flags must agree between the ranks on shared nodes. */
+typedef struct sem_shard_hooks {
+    int (*gs_begin)(void* user, void* w, int prec);
+    int (*gs_end)(void* user, void* w, int prec);
+    int (*allreduce)(void* user, double* scalars, int n);
+    void* user;
+} sem_shard_hooks;
+
+/* Declares that elements [0, n_iface_elems) of this context are the only ones that touch nodes shared with other ranks
+ * (the caller orders its elements that way; 0 = unknown, no overlap).  The sharded calls then run operator and
+ * gather-scatter of those elements first, call gs_begin, run the remaining elements, and call gs_end: the exchange
+ * overlaps the interior work (A18).  Rounded up to whole element groups.  Drops cached graphs.  Host call. */
+SEM_API int sem_shard_set_interface(sem_ctx* ctx, int64_t n_iface_elems);
+
+/* The chunks sem_ax_gs / sem_pcg work in (fields larger than L2, or the interface split): *n_chunks (1 = one launch
+ * pair), their element bounds (HOST, n_chunks + 1 values, cap = room in elem_bounds; NULL to skip) and how many leading
+ * chunks precede gs_begin in the sharded calls (0 = none).  Any pointer may be NULL.  Host call. */
+SEM_API int sem_get_chunks(sem_ctx* ctx, int64_t* elem_bounds, int cap, int* n_chunks, int* iface_chunks);
+
+/* w = M QQ^T (D^T G D + lambda B) u with QQ^T summing over ALL ranks' copies: sem_ax_gs on this rank's elements with the
+ * exchange through the hooks.  Same arguments as sem_ax_gs.  Nodes that live on one rank only are bit-identical to
+ * the single-context result when their copies are summed in the same order (always for 1 or 2 copies; for more when
+ * the rank keeps the caller's element order); everything else agrees to round-off. */
+SEM_API int sem_ax_gs_sharded(sem_ctx* ctx, const void* u, void* w, sem_prec prec, double lambda,
+                              const sem_shard_hooks* hooks);
+
+/* a8 on the partitioned mesh: every rank calls this with its part of b and x (DEVICE, [nL] of its context, x 16-byte
+ * aligned) and the same tol / maxit.  The recurrence, stopping test and breakdown rule are sem_pcg's (S12-S14); the
+ * dots are summed over ranks by TWO all-reduces per iteration (p.q; r.r and r.z together), in place on device scalars,
+ * so every rank takes the same decisions; the Jacobi diagonal and the dot weights (1 / multiplicity) are assembled over
+ * all ranks through the hooks at the first call and when lambda changes.  iters_out / relres_out / the history
+ * (sem_get_pcg_history) are the same on every rank.  Synchronises the stream every 8 iterations. */
+SEM_API int sem_pcg_sharded(sem_ctx* ctx, const double* b, double* x, double tol, int maxit,
+                            const sem_shard_hooks* hooks, int* iters_out, double* relres_out);
+
 /* a3-a7.  w = M QQ^T (D^T G D + lambda B) u, with M zeroing Dirichlet nodes (if the context has any).  u must be
  * continuous (equal on all copies of a shared node).  Called repeatedly with the same (u, w, prec, lambda) on a
  * non-default stream, the second call records the two kernels into a CUDA graph and later calls replay it (still

@@ -68,11 +68,48 @@ SYMBOLS = {
     "sem_cheby_schwarz": (_i32, [_vp, _vp, _vp, _i32, _dbl, _dbl, _i32, _i32, _i32]),
     "sem_lambda_max_schwarz": (_i32, [_vp, _i32, _i32, C.POINTER(_dbl)]),
     "sem_pmg_set_smoother": (_i32, [_vp, _i32, C.POINTER(_dbl), C.POINTER(_dbl)]),
+    "sem_shard_set_interface": (_i32, [_vp, _i64]),
+    "sem_get_chunks": (_i32, [_vp, _vp, _i32, C.POINTER(_i32), C.POINTER(_i32)]),
+    "sem_ax_gs_sharded": (_i32, [_vp, _vp, _vp, _i32, _dbl, _vp]),
+    "sem_pcg_sharded": (_i32, [_vp, _vp, _vp, _dbl, _i32, _vp, C.POINTER(_i32), C.POINTER(_dbl)]),
     "sem_last_error": (C.c_char_p, [_vp]),
     "sem_ctx_destroy": (None, [_vp]),
 }
 
 _lib = None
+
+# sem_shard_hooks (include/sem.h): the transport of a sharded solve, called back from inside the library
+_GS_HOOK = C.CFUNCTYPE(_i32, _vp, _vp, _i32)
+_AR_HOOK = C.CFUNCTYPE(_i32, _vp, _vp, _i32)
+
+
+class _ShardHooksStruct(C.Structure):
+    _fields_ = [("gs_begin", _GS_HOOK), ("gs_end", _GS_HOOK), ("allreduce", _AR_HOOK), ("user", _vp)]
+
+
+class ShardHooks:
+    """Wraps three Python callables as a sem_shard_hooks struct.  gs_begin(w_ptr, prec), gs_end(w_ptr, prec) and
+    allreduce(scalars_ptr, n) get raw DEVICE addresses (int).  An exception inside a hook makes the library call fail;
+    it is kept in `.error` and re-raised by the binding."""
+
+    def __init__(self, gs_begin, gs_end, allreduce):
+        self.error = None
+
+        def guard(fn):
+            def call(_user, ptr, k):
+                try:
+                    fn(int(ptr or 0), int(k))
+                    return 0
+                except BaseException as exc:          # must not propagate into the C caller
+                    self.error = exc
+                    return 1
+            return call
+
+        self._keep = (_GS_HOOK(guard(gs_begin)), _GS_HOOK(guard(gs_end)), _AR_HOOK(guard(allreduce)))
+        self.struct = _ShardHooksStruct(self._keep[0], self._keep[1], self._keep[2], None)
+
+    def ref(self):
+        return C.cast(C.byref(self.struct), _vp)
 
 
 def fdm_setup(A: np.ndarray, B: np.ndarray):
@@ -237,17 +274,61 @@ class Sem:
         self._check(self._L.sem_pcg_many(self._h, pb, px, nf, st, tol, maxit, it, rel))
         return list(it), list(rel)
 
-    def iface_pack(self, uniq, w, buf):
+    def _vec_or_ptr(self, w, prec):
+        """A field as a CUDA tensor, or as a raw device address (int) with its precision given (hook callbacks)."""
+        if isinstance(w, int):
+            assert prec in (SEM_F64, SEM_F32)
+            return C.c_void_p(w), prec
+        return self._vec(w), self._prec(w)
+
+    def iface_pack(self, uniq, w, buf, prec=None):
         """sem_iface_pack: buf[q] = w[first copy of unique node uniq[q]] (uniq: int32 CUDA tensor)."""
-        self._check(self._L.sem_iface_pack(self._h, C.c_void_p(uniq.data_ptr()), int(uniq.numel()), self._vec(w),
-                                           C.c_void_p(buf.data_ptr()), self._prec(w)))
+        pw, pr = self._vec_or_ptr(w, prec)
+        self._check(self._L.sem_iface_pack(self._h, C.c_void_p(uniq.data_ptr()), int(uniq.numel()), pw,
+                                           C.c_void_p(buf.data_ptr()), pr))
         return buf
 
-    def iface_add(self, uniq, buf, w):
+    def iface_add(self, uniq, buf, w, prec=None):
         """sem_iface_add: every copy of unique node uniq[q] += buf[q] (Dirichlet nodes stay zero)."""
+        pw, pr = self._vec_or_ptr(w, prec)
         self._check(self._L.sem_iface_add(self._h, C.c_void_p(uniq.data_ptr()), int(uniq.numel()),
-                                          C.c_void_p(buf.data_ptr()), self._vec(w), self._prec(w)))
+                                          C.c_void_p(buf.data_ptr()), pw, pr))
         return w
+
+    def shard_set_interface(self, n_iface_elems: int):
+        """sem_shard_set_interface: elements [0, n) are the only ones touching nodes shared with other ranks."""
+        self._check(self._L.sem_shard_set_interface(self._h, int(n_iface_elems)))
+        return self
+
+    def chunks(self):
+        """sem_get_chunks: (element bounds of the chunks, number of leading chunks that precede gs_begin)."""
+        n, ic = C.c_int(0), C.c_int(0)
+        self._check(self._L.sem_get_chunks(self._h, None, 0, C.byref(n), C.byref(ic)))
+        e0 = np.zeros(n.value + 1, dtype=np.int64)
+        self._check(self._L.sem_get_chunks(self._h, _np_ptr(e0), e0.size, None, None))
+        return e0, ic.value
+
+    def _check_hooks(self, rc: int, hooks: "ShardHooks"):
+        if hooks.error is not None:
+            exc, hooks.error = hooks.error, None
+            raise exc
+        self._check(rc)
+
+    def ax_gs_sharded(self, u, w, hooks: "ShardHooks", lam: float = 0.0):
+        assert u.dtype == w.dtype
+        self._check_hooks(self._L.sem_ax_gs_sharded(self._h, self._vec(u), self._vec(w), self._prec(u), lam, hooks.ref()),
+                          hooks)
+        return w
+
+    def pcg_sharded(self, b, x, tol: float, maxit: int, hooks: "ShardHooks"):
+        """sem_pcg_sharded on this rank's part; returns (iters, relres), the same on every rank."""
+        import torch
+
+        assert b.dtype == torch.float64 and x.dtype == torch.float64
+        it, rel = C.c_int(0), C.c_double(0.0)
+        self._check_hooks(self._L.sem_pcg_sharded(self._h, self._vec(b), self._vec(x), tol, maxit, hooks.ref(),
+                                                  C.byref(it), C.byref(rel)), hooks)
+        return it.value, rel.value
 
     def ax_gs(self, u, w, lam: float = 0.0):
         assert u.dtype == w.dtype

@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libsem.so")
-SOURCES = ["sem_api.cu", "sem_gll.cpp", "sem_maps.cu", "sem_geom.cu", "sem_gs.cu", "sem_ax.cu", "sem_pcg.cu", "sem_transfer.cu", "sem_cheby.cu", "sem_pmg.cu", "sem_proj.cu", "sem_fdm.cu", "sem_fdm_setup.cpp", "sem_peaks.cu", "sem_schwarz.cu", "sem_iface.cu", "sem_inner.cu", "sem_coarse.cu"]
+SOURCES = ["sem_api.cu", "sem_gll.cpp", "sem_maps.cu", "sem_geom.cu", "sem_gs.cu", "sem_ax.cu", "sem_pcg.cu", "sem_transfer.cu", "sem_cheby.cu", "sem_pmg.cu", "sem_proj.cu", "sem_fdm.cu", "sem_fdm_setup.cpp", "sem_peaks.cu", "sem_schwarz.cu", "sem_iface.cu", "sem_inner.cu", "sem_coarse.cu", "sem_shard.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC",
          "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr"]

@@ -284,7 +284,7 @@ void sem_ctx_destroy(sem_ctx* c) {
     void* ptrs[] = {c->d_vert, c->d_l2u, c->d_mult, c->d_seg_off, c->d_seg_idx, c->d_uniq_gid, c->d_sh_off, c->d_sh_idx,
                     c->d_sh_masked, c->d_mask_u, c->d_mask1_idx, c->d_G, c->d_G32, c->d_B, c->d_B32, c->d_detJ,
                     c->d_diag, c->d_Minv, c->d_wt, c->d_wt8, c->d_r, c->d_p, c->d_w, c->d_scal, 
-                    c->d_own_pair, c->d_own_quad, c->d_own_big, c->d_J, c->d_cheb[0], c->d_cheb[1], c->d_cheb[2], c->d_cheb4, c->d_Minv32};
+                    c->d_own_pair, c->d_own_quad, c->d_own_big, c->d_J, c->d_cheb[0], c->d_cheb[1], c->d_cheb[2], c->d_cheb4, c->d_Minv32, c->d_Minv_g, c->d_wt_g};
     for (void* p : ptrs) cudaFree(p);
     cudaGetLastError();
     delete[] c->h_hist;

@@ -1213,10 +1213,17 @@ int sem_launch_ax_gs(sem_ctx* c, const void* u, void* w, sem_prec prec, double l
     // operator and gather-scatter alternate chunk by chunk.  The records are sorted by the element group of a node's LAST
     // copy, so the records of chunk q only touch values written by chunks <= q, a few tens of MB ago: still in L2 for any
     // element order with locality (every box mesh in lexicographic order; not config 5's scrambled order).
-    for (int q = 0; q < nch; ++q) {
+    return sem_launch_ax_gs_chunks(c, u, w, prec, lambda, dot_out, skip_flag, 0, nch);
+}
+
+// chunks [q0, q1) of the chunked operator + gather-scatter (the sharded apply starts its exchange between two ranges)
+int sem_launch_ax_gs_chunks(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda, double* dot_out,
+                            const int* skip_flag, int q0, int q1) {
+    int rc;
+    for (int q = q0; q < q1; ++q) {
         c->rng_e0 = c->chunk_e0[q];
         c->rng_ne = c->chunk_e0[q + 1] - c->chunk_e0[q];
-        rc = sem_launch_ax(c, u, w, prec, lambda, dot_out, skip_flag);
+        rc = c->rng_ne > 0 ? sem_launch_ax(c, u, w, prec, lambda, dot_out, skip_flag) : SEM_OK;
         c->rng_ne = 0;
         if (rc) return rc;
         if ((rc = sem_launch_gs_range(c, w, prec, true, skip_flag, q))) return rc;

@@ -59,6 +59,13 @@ struct sem_ctx {
     // record class, the first record owned by each chunk (records are sorted by owner group)
     std::vector<int64_t> chunk_e0;
     std::vector<int32_t> chunk_rec[3];
+    std::vector<int32_t> grp_rec[3];         // host copy of the per-group record offsets, [ngroups + 1] per class
+    // sharded solves (sem_shard.cu): the first iface_chunks chunks hold every element that touches a node shared with
+    // another rank (0: the exchange starts after the whole apply); Minv / dot weights assembled over all ranks
+    int iface_chunks = 0;
+    double* d_Minv_g = nullptr;
+    double* d_wt_g = nullptr;
+    double lambda_of_shard = -1.0;
     int64_t rng_e0 = 0, rng_ne = 0;          // element range of the Ax launch in flight (sem_launch_ax_gs), 0 = all
     // Dirichlet (S14)
     bool has_mask = false;
@@ -146,12 +153,21 @@ int sem_geom_export(sem_ctx* c, double* G_host, double* detJ_host);
 int sem_launch_ax(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda, double* dot_out,
                   const int* skip_flag);
 int sem_launch_ax_gs(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda, double* dot_out,
-                     const int* skip_flag);      // a3-a7: operator kernel + gather-scatter kernel
+                     const int* skip_flag);
+int sem_launch_ax_gs_chunks(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda, double* dot_out,
+                            const int* skip_flag, int q0, int q1);      // a3-a7: operator kernel + gather-scatter kernel
 int sem_launch_ax_many(sem_ctx* c, const void* u, void* w, int nf, int64_t stride, sem_prec prec, double lambda,
                        double* dot_out, int64_t dot_stride, const int* skip_flag);
 // sem_gs.cu
 int sem_launch_gs(sem_ctx* c, void* w, sem_prec prec, bool apply_mask, const int* skip_flag = nullptr);
 int sem_launch_gs_range(sem_ctx* c, void* w, sem_prec prec, bool apply_mask, const int* skip_flag, int chunk);
+// sem_shard.cu
+int sem_hooks_ok(sem_ctx* c, const sem_shard_hooks* h, const char* who);
+int sem_launch_ax_gs_sharded(sem_ctx* c, const void* u, void* w, sem_prec prec, double lambda, double* dot_out,
+                             const int* skip_flag, const sem_shard_hooks* h);
+int sem_shard_build_diag(sem_ctx* c, const sem_shard_hooks* h);
+void sem_set_chunk_groups(sem_ctx* c, const std::vector<int64_t>& group_bounds);
+void sem_default_chunks(sem_ctx* c, int64_t first_groups);
 int sem_launch_gs_many(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec prec, bool apply_mask,
                        const int* skip_flag = nullptr);
 // sem_api.cu

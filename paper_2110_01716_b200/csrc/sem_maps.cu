@@ -316,6 +316,36 @@ int ex_scan(sem_ctx* c, Tmp& tmp, const T* in, T* out, int64_t n) {
 
 }  // namespace
 
+// chunk table from ascending group bounds (first = 0, last = ngroups); fewer than 2 chunks: no chunking
+void sem_set_chunk_groups(sem_ctx* c, const std::vector<int64_t>& gb) {
+    c->chunk_e0.clear();
+    for (int cls = 0; cls < 3; ++cls) c->chunk_rec[cls].clear();
+    if (gb.size() < 3) return;
+    for (int64_t g0 : gb) {
+        c->chunk_e0.push_back(g0 * c->epb < c->E ? g0 * c->epb : c->E);
+        for (int cls = 0; cls < 3; ++cls) c->chunk_rec[cls].push_back(c->grp_rec[cls][(size_t)g0]);
+    }
+}
+
+// chunks for fields larger than L2: 64 MB of FP64 field per chunk (measured best at 64^3 elements, N = 7: 48-64 MB;
+// smaller chunks pay the operator's ramp and tail per launch), only when there are at least 2 of them.  first_groups
+// > 0 (sem_shard_set_interface): the first chunk is exactly those groups, the rest is cut the same way.
+void sem_default_chunks(sem_ctx* c, int64_t first_groups) {
+    const int64_t ng = c->ngroups;
+    int64_t cg = (int64_t)((64.0 * 1024 * 1024) / (8.0 * (double)(c->epb * c->p3)));
+    if (cg < 1) cg = 1;
+    if (const char* env = getenv("SEM_CHUNK_GROUPS")) cg = atoll(env) > 0 ? atoll(env) : ng + 1;   // tests
+    std::vector<int64_t> gb;
+    gb.push_back(0);
+    if (first_groups > 0 && first_groups < ng) gb.push_back(first_groups);
+    const int64_t g_from = gb.back(), rest = ng - g_from;
+    const int64_t nch = (rest + cg - 1) / cg;
+    if (nch >= 2)
+        for (int64_t q = 1; q < nch; ++q) gb.push_back(g_from + q * cg);
+    gb.push_back(ng);
+    sem_set_chunk_groups(c, gb);
+}
+
 int sem_build_gs_records(sem_ctx* c) {
     cudaStream_t st = c->stream;
     const int32_t ng = (int32_t)c->ngroups;
@@ -361,27 +391,13 @@ int sem_build_gs_records(sem_ctx* c) {
                                        cudaMemcpyDeviceToHost, st));
     SEM_CUDA_OK(c, cudaStreamSynchronize(st));
     c->n_pair = h_tot[0]; c->n_quad = h_tot[1]; c->n_big = h_tot[2];
-    // chunks for fields larger than L2: 64 MB of FP64 field per chunk (measured best at 64^3 elements, N = 7: 48-64 MB;
-    // smaller chunks pay the operator's ramp and tail per launch), only when there are at least 2 of them
-    c->chunk_e0.clear();
-    for (int cls = 0; cls < 3; ++cls) c->chunk_rec[cls].clear();
-    {
-        int64_t cg = (int64_t)((64.0 * 1024 * 1024) / (8.0 * group_nodes));
-        if (cg < 1) cg = 1;
-        if (const char* env = getenv("SEM_CHUNK_GROUPS")) cg = atoll(env) > 0 ? atoll(env) : (int64_t)ng + 1;   // tests
-        const int64_t nch = (ng + cg - 1) / cg;
-        if (nch >= 2) {
-            for (int64_t q = 0; q <= nch; ++q) {
-                const int64_t g0 = q * cg < ng ? q * cg : ng;
-                c->chunk_e0.push_back(g0 * c->epb < c->E ? g0 * c->epb : c->E);
-                for (int cls = 0; cls < 3; ++cls) {
-                    int32_t off = 0;
-                    SEM_CUDA_OK(c, cudaMemcpy(&off, d_offc + cls * ((int64_t)ng + 1) + g0, sizeof(int32_t), cudaMemcpyDeviceToHost));
-                    c->chunk_rec[cls].push_back(off);
-                }
-            }
-        }
+    // host copy of the per-group record offsets (3 classes x (ng + 1)): chunk tables are cut from it
+    for (int cls = 0; cls < 3; ++cls) {
+        c->grp_rec[cls].assign((size_t)ng + 1, 0);
+        SEM_CUDA_OK(c, cudaMemcpy(c->grp_rec[cls].data(), d_offc + cls * ((int64_t)ng + 1), ((size_t)ng + 1) * sizeof(int32_t),
+                                  cudaMemcpyDeviceToHost));
     }
+    sem_default_chunks(c, 0);
     SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_own_pair, (size_t)(c->n_pair ? c->n_pair : 1) * sizeof(int2)));
     SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_own_quad, (size_t)(c->n_quad ? c->n_quad : 1) * sizeof(int4)));
     SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_own_big, (size_t)(c->n_big ? c->n_big : 1) * sizeof(int2)));

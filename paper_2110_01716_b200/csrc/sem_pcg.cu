@@ -278,6 +278,99 @@ extern "C" int sem_pcg(sem_ctx* c, const double* b, double* x, double tol, int m
 
 
 // ---------------------------------------------------------------------------------------------------------------
+// NEXT-4: the same recurrence with the elements partitioned over ranks.  Each rank runs this call on
+// its own context with its part of b and x.  Per iteration: the sharded operator (sem_shard.cu: rank-local operator and
+// gather-scatter, interface exchange through the hooks, started after the interface chunk when sem_shard_set_interface
+// was called), ONE all-reduce of p.q, the update kernel, ONE all-reduce of (r.r, r.z), the direction kernel.  The
+// scalars stay on the device as in sem_pcg: the all-reduce works in place on the iteration's slot, every rank then
+// holds the same bits, takes the same stopping decision, and the host polls the flag every 8 iterations.  Dot weights
+// are 1 / (multiplicity over ALL ranks), the preconditioner is the diagonal assembled over all ranks.
+// ---------------------------------------------------------------------------------------------------------------
+extern "C" int sem_pcg_sharded(sem_ctx* c, const double* b, double* x, double tol, int maxit,
+                               const sem_shard_hooks* hooks, int* iters_out, double* relres_out) {
+    if (!c) return SEM_EINVAL;
+    c->err.clear();
+    if (!b || !x) return sem_fail(c, SEM_EINVAL, "sem_pcg_sharded: NULL vector");
+    if (((uintptr_t)x % 16) || ((uintptr_t)b % 8)) return sem_fail(c, SEM_EINVAL, "sem_pcg_sharded: x must be 16-byte aligned");
+    if (!(tol > 0.0) && maxit <= 0) return sem_fail(c, SEM_EINVAL, "sem_pcg_sharded: tol <= 0 with maxit <= 0");
+    if (!c->geom_done) return sem_fail(c, SEM_ESTATE, "sem_pcg_sharded before sem_geom");
+    if (c->lambda != 0.0 && !c->with_mass) return sem_fail(c, SEM_ESTATE, "lambda != 0 needs with_mass");
+    int rc = sem_hooks_ok(c, hooks, "sem_pcg_sharded");
+    if (rc) return rc;
+    if (maxit < 0) maxit = 0;
+    cudaStream_t st = c->stream;
+    const int64_t n = c->nL;
+    if (!c->d_Minv_g || c->lambda_of_shard != c->lambda)
+        if ((rc = sem_shard_build_diag(c, hooks))) return rc;
+    if (!c->d_r) {
+        SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_r, n * sizeof(double)));
+        SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_p, n * sizeof(double)));
+        SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_w, n * sizeof(double)));
+    }
+    const int64_t need = 4 * ((int64_t)maxit + 2) + 8;
+    if (need > c->scal_cap) {
+        cudaFree(c->d_scal);
+        c->d_scal = nullptr;
+        SEM_CUDA_OK(c, cudaMalloc((void**)&c->d_scal, need * sizeof(double)));
+        c->scal_cap = need;
+    }
+    double* scal = c->d_scal;
+    PcgFlags* flags = reinterpret_cast<PcgFlags*>(scal + 4 * ((int64_t)maxit + 2));
+    SEM_CUDA_OK(c, cudaMemsetAsync(scal, 0, need * sizeof(double), st));
+    const unsigned vgrid = (unsigned)c->num_sms * 8;
+    auto reduce = [&](double* p, int cnt) -> int {
+        return hooks->allreduce(hooks->user, p, cnt) ? sem_fail(c, SEM_ECUDA, "sem_pcg_sharded: allreduce hook failed") : SEM_OK;
+    };
+
+    k_mask_vec<<<vgrid, 256, 0, st>>>(n, c->d_wt_g, x);
+    if ((rc = sem_launch_ax_gs_sharded(c, x, c->d_w, SEM_F64, c->lambda, nullptr, nullptr, hooks))) return rc;
+    k_pcg_init<<<vgrid, 256, 0, st>>>(n, b, c->d_w, c->d_Minv_g, c->d_wt_g, x, c->d_r, c->d_p, scal);
+    if ((rc = reduce(scal + 1, 2))) return rc;
+    double h0[4];
+    SEM_CUDA_OK(c, cudaMemcpyAsync(h0, scal, 4 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    SEM_CUDA_OK(c, cudaStreamSynchronize(st));
+    SEM_CUDA_OK(c, cudaGetLastError());
+    const double rr0 = h0[1];
+    int iters = 0;
+    PcgFlags hf = {};
+    if (rr0 > 0.0 && maxit > 0) {
+        const double tol2 = tol > 0.0 ? tol * tol : 0.0;
+        const int batch = 8;
+        for (int it = 1; it <= maxit; ++it) {
+            if ((rc = sem_launch_ax_gs_sharded(c, c->d_p, c->d_w, SEM_F64, c->lambda, scal + 4 * it, &flags->done, hooks))) return rc;
+            if ((rc = reduce(scal + 4 * it, 1))) return rc;
+            k_pcg_update<false><<<vgrid, 256, 0, st>>>(n, it, c->d_p, c->d_w, c->d_Minv_g, c->d_wt_g, nullptr, x, c->d_r, scal, flags);
+            if ((rc = reduce(scal + 4 * it + 1, 2))) return rc;
+            k_pcg_direction<<<vgrid, 256, 0, st>>>(n, it, maxit, tol2, c->d_r, c->d_Minv_g, c->d_p, scal, flags);
+            if (it % batch == 0 || it == maxit) {
+                SEM_CUDA_OK(c, cudaMemcpyAsync(&hf, flags, sizeof(hf), cudaMemcpyDeviceToHost, st));
+                SEM_CUDA_OK(c, cudaStreamSynchronize(st));
+                if (hf.done) break;
+            }
+        }
+        SEM_CUDA_OK(c, cudaGetLastError());
+        iters = hf.iters;
+    }
+    delete[] c->h_hist;
+    c->h_hist = new double[iters + 1];
+    c->hist_n = iters + 1;
+    c->h_hist[0] = rr0 > 0.0 ? 1.0 : 0.0;
+    if (iters > 0) {
+        double* slots = new double[4 * ((size_t)iters + 1)];
+        cudaError_t e = cudaMemcpyAsync(slots, scal, 4 * ((size_t)iters + 1) * sizeof(double), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) { delete[] slots; return sem_fail(c, SEM_ECUDA, "pcg history: %s", cudaGetErrorString(e)); }
+        for (int i = 1; i <= iters; ++i) c->h_hist[i] = sqrt(slots[4 * i + 1] / rr0);
+        if (hf.breakdown) c->h_hist[iters] = c->h_hist[iters - 1];
+        delete[] slots;
+    }
+    if (iters_out) *iters_out = iters;
+    if (relres_out) *relres_out = c->h_hist[iters];
+    return SEM_OK;
+}
+
+
+// ---------------------------------------------------------------------------------------------------------------
 // NEXT-4: Jacobi-PCG on nf right-hand sides at once ("3 Helmholtz problems -- one for each velocity component ...
 // Jacobi-preconditioned conjugate gradient iteration").  Every field runs exactly the recurrence of sem_pcg with its own
 // alpha, beta, stopping test and breakdown flag (own scalar slots), so each field's iterates are those sem_pcg would
