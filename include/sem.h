@@ -90,7 +90,11 @@ SEM_API int sem_gs(sem_ctx* ctx, void* w, sem_prec prec, sem_op op);
  * vector at w + f * field_stride (in values of `prec`, field_stride >= nL); every field receives exactly what sem_gs
  * would give it (bit-identical), but the gather-scatter records are read once for up to 4 fields and the value loads of
  * all of them are in flight together.  No mask is applied.  w DEVICE.  Asynchronous on the context's stream.
- * SEM_EINVAL for nfields < 1 or field_stride < nL. */
+ * SEM_EINVAL for nfields < 1 or field_stride < nL.
+ * field_stride = SEM_INTERLEAVED selects the NODE-INTERLEAVED layout instead: value of field f at local node l is
+ * w[l * nfields + f] (2 <= nfields <= 4): the copies of a node then share their 32-byte sectors between the fields,
+ * which is what the scattered accesses of the gather-scatter pay for. */
+#define SEM_INTERLEAVED 1
 SEM_API int sem_gs_many(sem_ctx* ctx, void* w, int nfields, int64_t field_stride, sem_prec prec, sem_op op);
 
 /* NEXT-4: the operator and the Jacobi-PCG solve on several fields that share the geometry ("Each

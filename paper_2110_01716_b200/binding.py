@@ -18,6 +18,7 @@ SEM_F64, SEM_F32 = 0, 1
 SEM_OP_ADD = 0
 SEM_G_STORED, SEM_G_RECOMPUTE = 0, 1
 SEM_PROLONG, SEM_RESTRICT = 0, 1
+SEM_INTERLEAVED = 1
 SEM_SCHWARZ_ASM, SEM_SCHWARZ_RAS = 0, 1
 SEM_SMOOTH_CHEBY_JACOBI, SEM_SMOOTH_CHEBY_SCHWARZ, SEM_SMOOTH_CHEBY_RAS = 0, 1, 2
 SEM_OK, SEM_EINVAL, SEM_EMESH, SEM_ECUDA, SEM_ENOMEM, SEM_ESTATE = 0, -1, -2, -3, -4, -5
@@ -244,11 +245,17 @@ class Sem:
         self._check(self._L.sem_gs(self._h, self._vec(w), self._prec(w), SEM_OP_ADD))
         return w
 
-    def gs_many(self, w):
-        """sem_gs_many on a contiguous [nfields][stride >= nL] CUDA tensor, in place."""
-        assert w.is_cuda and w.is_contiguous() and w.dim() == 2 and w.shape[1] >= self.nL
-        self._check(self._L.sem_gs_many(self._h, C.c_void_p(w.data_ptr()), w.shape[0], w.shape[1], self._prec(w),
-                                        SEM_OP_ADD))
+    def gs_many(self, w, interleaved: bool = False):
+        """sem_gs_many in place on a contiguous CUDA tensor: [nfields][stride >= nL], or -- interleaved=True -- the
+        node-interleaved layout [nL][nfields] (field_stride = SEM_INTERLEAVED, 2 to 4 fields)."""
+        assert w.is_cuda and w.is_contiguous() and w.dim() == 2
+        if interleaved:
+            assert w.shape[0] == self.nL
+            nf, stride = w.shape[1], SEM_INTERLEAVED
+        else:
+            assert w.shape[1] >= self.nL
+            nf, stride = w.shape[0], w.shape[1]
+        self._check(self._L.sem_gs_many(self._h, C.c_void_p(w.data_ptr()), nf, stride, self._prec(w), SEM_OP_ADD))
         return w
 
     def _fields(self, t):

@@ -126,9 +126,11 @@ int sem_gs_many(sem_ctx* c, void* w, int nfields, int64_t field_stride, sem_prec
     int rc = check_vec(c, nullptr, w, prec, 0.0, "sem_gs_many");
     if (rc) return rc;
     if (op != SEM_OP_ADD) return sem_fail(c, SEM_EINVAL, "sem_gs_many: only SEM_OP_ADD is defined (P:119)");
-    if (nfields < 1 || field_stride < c->nL)
-        return sem_fail(c, SEM_EINVAL, "sem_gs_many: nfields < 1 or field_stride < nL");
+    const bool inter = field_stride == SEM_INTERLEAVED;
+    if (inter ? (nfields < 2 || nfields > 4) : (nfields < 1 || field_stride < c->nL))
+        return sem_fail(c, SEM_EINVAL, "sem_gs_many: nfields < 1 or field_stride < nL (interleaved: 2 <= nfields <= 4)");
     if (!c->d_sh_off) return sem_fail(c, SEM_ESTATE, "sem_gs_many on a context whose setup failed");
+    if (inter) return sem_launch_gs_many(c, w, nfields, 1, prec, false);
     const size_t vs = prec == SEM_F64 ? 8 : 4;
     for (int f = 0; f < nfields;) {                          // launches of 4, 3 or 2 fields; a single one by sem_gs's kernel
         const int left = nfields - f, take = left >= 4 && left != 5 ? 4 : left >= 3 ? 3 : left;

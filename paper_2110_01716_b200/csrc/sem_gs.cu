@@ -47,13 +47,38 @@ __global__ void __launch_bounds__(NT, GS_CTAS) k_gs_records(int32_t n_pair, cons
 // value loads of all NF fields in flight together.  Same ascending-index sums per field, so each field is bit-identical
 // to sem_gs applied to it alone.
 // ---------------------------------------------------------------------------------------------------------------
-template <typename T, bool MASK, int NF>
+template <typename T, bool MASK, int NF, bool INTER>
 __global__ void __launch_bounds__(NT, 4) k_gs_records_many(int32_t n_pair, const int2* __restrict__ pair, int32_t n_quad,
                                                            const int4* __restrict__ quad, int32_t n_big,
                                                            const int2* __restrict__ big,
                                                            const int32_t* __restrict__ sh_idx, T* __restrict__ w,
                                                            int64_t stride, const int* __restrict__ skip_flag) {
     if (skip_flag && *skip_flag) return;
+    // value of field f at local node l: planar fields w + f * stride, or node-interleaved [nL][NF]
+    auto at = [&](int f, int32_t l) -> T& { return INTER ? w[(int64_t)l * NF + f] : w[f * stride + l]; };
+    // all NF values of a node: interleaved fields whose NF values fill whole 16-byte words move as vectors
+    constexpr bool VEC = INTER && (NF * sizeof(T)) % 16 == 0;
+    constexpr int NV = VEC ? (int)(NF * sizeof(T) / 16) : 1;
+    auto ldn = [&](int32_t l, T (&v)[NF]) {
+        if constexpr (VEC) {
+            const int4* src = reinterpret_cast<const int4*>(w + (int64_t)l * NF);
+#pragma unroll
+            for (int q = 0; q < NV; ++q) reinterpret_cast<int4*>(v)[q] = src[q];
+        } else {
+#pragma unroll
+            for (int f = 0; f < NF; ++f) v[f] = at(f, l);
+        }
+    };
+    auto stn = [&](int32_t l, const T (&v)[NF]) {
+        if constexpr (VEC) {
+            int4* dst = reinterpret_cast<int4*>(w + (int64_t)l * NF);
+#pragma unroll
+            for (int q = 0; q < NV; ++q) dst[q] = reinterpret_cast<const int4*>(v)[q];
+        } else {
+#pragma unroll
+            for (int f = 0; f < NF; ++f) at(f, l) = v[f];
+        }
+    };
     const int32_t b = blockIdx.x, nb = gridDim.x;
     const int32_t pp = ((n_pair + nb - 1) / nb + 31) & ~31, pq = ((n_quad + nb - 1) / nb + 31) & ~31,
                   pg = (n_big + nb - 1) / nb;
@@ -68,27 +93,28 @@ __global__ void __launch_bounds__(NT, 4) k_gs_records_many(int32_t n_pair, const
                 const int32_t t = base + q * NT;
                 r[q] = t < end ? pair[t] : make_int2(0, -2);
             }
-            T v0[PP][NF], v1[PP][NF];
+            alignas(16) T v0[PP][NF], v1[PP][NF];
 #pragma unroll
-            for (int q = 0; q < PP; ++q)
+            for (int q = 0; q < PP; ++q) {
+                if (r[q].y >= 0) { ldn(r[q].x & IDX, v0[q]); ldn(r[q].y, v1[q]); }
+            }
 #pragma unroll
-                for (int f = 0; f < NF; ++f) {
-                    v0[q][f] = r[q].y >= 0 ? w[f * stride + (r[q].x & IDX)] : T(0);
-                    v1[q][f] = r[q].y >= 0 ? w[f * stride + r[q].y] : T(0);
-                }
+            for (int q = 0; q < PP; ++q) {
+                if (r[q].y >= 0) {
 #pragma unroll
-            for (int q = 0; q < PP; ++q)
-#pragma unroll
-                for (int f = 0; f < NF; ++f) {
-                    if (r[q].y >= 0) {
+                    for (int f = 0; f < NF; ++f) {
                         T s = v0[q][f] + v1[q][f];
                         if (MASK && r[q].x < 0) s = T(0);
-                        w[f * stride + (r[q].x & IDX)] = s;
-                        w[f * stride + r[q].y] = s;
-                    } else if (MASK && r[q].y == -1) {
-                        w[f * stride + (r[q].x & IDX)] = T(0);
+                        v0[q][f] = s;
                     }
+                    stn(r[q].x & IDX, v0[q]);
+                    stn(r[q].y, v0[q]);
+                } else if (MASK && r[q].y == -1) {
+#pragma unroll
+                    for (int f = 0; f < NF; ++f) v0[q][f] = T(0);
+                    stn(r[q].x & IDX, v0[q]);
                 }
+            }
         }
     }
     if (bq < n_quad) {
@@ -96,28 +122,25 @@ __global__ void __launch_bounds__(NT, 4) k_gs_records_many(int32_t n_pair, const
         for (int32_t t = (int32_t)bq + threadIdx.x; t < end; t += NT) {
             const int4 r = quad[t];
             const int32_t l0 = r.x & IDX;
-            T a[NF][4];
+            alignas(16) T a[4][NF];
+            ldn(l0, a[0]); ldn(r.y, a[1]); ldn(r.z, a[2]);
+            if (r.w >= 0) ldn(r.w, a[3]);
 #pragma unroll
             for (int f = 0; f < NF; ++f) {
-                T* wf = w + f * stride;
-                a[f][0] = wf[l0]; a[f][1] = wf[r.y]; a[f][2] = wf[r.z];
-                a[f][3] = r.w >= 0 ? wf[r.w] : T(0);
-            }
-#pragma unroll
-            for (int f = 0; f < NF; ++f) {
-                T* wf = w + f * stride;
-                T s = (a[f][0] + a[f][1]) + a[f][2];
-                if (r.w >= 0) s += a[f][3];
+                T s = (a[0][f] + a[1][f]) + a[2][f];
+                if (r.w >= 0) s += a[3][f];
                 if (MASK && r.x < 0) s = T(0);
-                wf[l0] = s; wf[r.y] = s; wf[r.z] = s;
-                if (r.w >= 0) wf[r.w] = s;
+                a[0][f] = s;
             }
+            stn(l0, a[0]); stn(r.y, a[0]); stn(r.z, a[0]);
+            if (r.w >= 0) stn(r.w, a[0]);
         }
     }
     if (bg < n_big)                                           // rare (> 4 copies): field by field
-        for (int f = 0; f < NF; ++f)
-            gs_bigs<T, MASK, NT>(big, sh_idx, (int32_t)bg + threadIdx.x, min(n_big, (int32_t)bg + pg),
-                                        w + f * stride);
+        for (int f = 0; f < NF; ++f) {
+            if (INTER) gs_bigs<T, MASK, NT, NF>(big, sh_idx, (int32_t)bg + threadIdx.x, min(n_big, (int32_t)bg + pg), w + f);
+            else gs_bigs<T, MASK, NT>(big, sh_idx, (int32_t)bg + threadIdx.x, min(n_big, (int32_t)bg + pg), w + f * stride);
+        }
 }
 
 }  // namespace
@@ -164,18 +187,22 @@ int sem_launch_gs_many(sem_ctx* c, void* w, int nf, int64_t stride, sem_prec pre
     const int64_t cap = (int64_t)c->num_sms * 4;
     if (blocks > cap) blocks = cap;
     blocks = (blocks + c->num_sms - 1) / c->num_sms * c->num_sms;
-#define SEM_GSM_LAUNCH(T, M, NF)                                                                                  \
-    k_gs_records_many<T, M, NF><<<(unsigned)blocks, NT, 0, c->stream>>>(np, c->d_own_pair, nq, c->d_own_quad, nb,  \
-                                                                         c->d_own_big, c->d_sh_idx, (T*)w, stride, skip_flag)
+    const bool inter = stride == 1;                              // node-interleaved fields [nL][nf]
+#define SEM_GSM_LAUNCH(T, M, NF, I)                                                                               \
+    k_gs_records_many<T, M, NF, I><<<(unsigned)blocks, NT, 0, c->stream>>>(np, c->d_own_pair, nq, c->d_own_quad, nb, \
+                                                                            c->d_own_big, c->d_sh_idx, (T*)w, stride, skip_flag)
+#define SEM_GSM_I(T, M, NF)                                                                                       \
+    do { if (inter) SEM_GSM_LAUNCH(T, M, NF, true); else SEM_GSM_LAUNCH(T, M, NF, false); } while (0)
 #define SEM_GSM_NF(T, M)                                                                                          \
     do {                                                                                                          \
-        if (nf == 2) SEM_GSM_LAUNCH(T, M, 2);                                                                     \
-        else if (nf == 3) SEM_GSM_LAUNCH(T, M, 3);                                                                \
-        else SEM_GSM_LAUNCH(T, M, 4);                                                                             \
+        if (nf == 2) SEM_GSM_I(T, M, 2);                                                                          \
+        else if (nf == 3) SEM_GSM_I(T, M, 3);                                                                     \
+        else SEM_GSM_I(T, M, 4);                                                                                  \
     } while (0)
     if (prec == SEM_F64) { if (m) SEM_GSM_NF(double, true); else SEM_GSM_NF(double, false); }
     else { if (m) SEM_GSM_NF(float, true); else SEM_GSM_NF(float, false); }
 #undef SEM_GSM_NF
+#undef SEM_GSM_I
 #undef SEM_GSM_LAUNCH
     SEM_CUDA_OK(c, cudaGetLastError());
     return SEM_OK;

@@ -54,7 +54,8 @@ __device__ __forceinline__ void gs_quads(const int4* __restrict__ quad, int32_t 
     }
 }
 
-template <typename T, bool MASK, int NTH>
+// NSTR: distance between consecutive nodes in values of T (1; NF for node-interleaved fields, w pointing at field f)
+template <typename T, bool MASK, int NTH, int NSTR = 1>
 __device__ __forceinline__ void gs_bigs(const int2* __restrict__ big, const int32_t* __restrict__ sh_idx, int32_t first,
                                         int32_t end, T* __restrict__ w) {
     for (int32_t t = first; t < end; t += NTH) {
@@ -66,15 +67,15 @@ __device__ __forceinline__ void gs_bigs(const int2* __restrict__ big, const int3
 #pragma unroll
         for (int q = 0; q < 8; ++q) id[q] = q < cnt ? __ldg(&sh_idx[r.x + q]) : -1;
 #pragma unroll
-        for (int q = 0; q < 8; ++q) v[q] = id[q] >= 0 ? w[id[q]] : T(0);
+        for (int q = 0; q < 8; ++q) v[q] = id[q] >= 0 ? w[(int64_t)id[q] * NSTR] : T(0);
         T s = v[0];
 #pragma unroll
         for (int q = 1; q < 8; ++q) if (id[q] >= 0) s += v[q];
-        for (int32_t q = 8; q < cnt; ++q) s += w[sh_idx[r.x + q]];
+        for (int32_t q = 8; q < cnt; ++q) s += w[(int64_t)sh_idx[r.x + q] * NSTR];
         if (MASK && r.y < 0) s = T(0);
 #pragma unroll
-        for (int q = 0; q < 8; ++q) if (id[q] >= 0) w[id[q]] = s;
-        for (int32_t q = 8; q < cnt; ++q) w[sh_idx[r.x + q]] = s;
+        for (int q = 0; q < 8; ++q) if (id[q] >= 0) w[(int64_t)id[q] * NSTR] = s;
+        for (int32_t q = 8; q < cnt; ++q) w[(int64_t)sh_idx[r.x + q] * NSTR] = s;
     }
 }
 

@@ -1002,3 +1002,26 @@ def test_sharded_hooks_nccl_world1(torch_cuda, binding, oracle_mod):
     finally:
         if own:
             dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("N,nf", [(3, 2), (7, 3), (4, 4), (1, 2), (7, 4)])
+def test_gs_many_node_interleaved(torch_cuda, binding, oracle_mod, N, nf):
+    """sem_gs_many with field_stride = SEM_INTERLEAVED (fields stored [nL][nf]; 16-byte vector accesses when nf values fill
+    whole 16-byte words): every field bit-identical to the oracle's gather-scatter (same ascending-index sums), FP32
+    1e-6; 1 or 5 fields are refused."""
+    m = inputs.box_mesh(4, 4, 3, N, permute_seed=6)
+    om = oracle_mod.Maps(m.gid)
+    rng = np.random.default_rng(300 + N)
+    w = rng.standard_normal((nf, m.nL))
+    ow = np.stack([oracle_mod.gs(w[f].copy(), om) for f in range(nf)])
+    with binding.Sem(m.E, m.N, m.vert, m.gid) as sem:
+        dw = to_dev(torch_cuda, np.ascontiguousarray(w.T))
+        sem.gs_many(dw, interleaved=True)
+        assert np.array_equal(dw.cpu().numpy().T, ow)
+        d32 = to_dev(torch_cuda, np.ascontiguousarray(w.T.astype(np.float32)))
+        sem.gs_many(d32, interleaved=True)
+        assert relerr(d32.cpu().numpy().T, ow) <= 1e-6
+        for bad in (1, 5):
+            with pytest.raises(binding.SemError):
+                sem._check(sem._L.sem_gs_many(sem._h, dw.data_ptr(), bad, binding.SEM_INTERLEAVED, binding.SEM_F64,
+                                              binding.SEM_OP_ADD))
