@@ -359,7 +359,9 @@ SEM_API int sem_measure_peak(int kind, void* cuda_stream, double* tflops_out);
 /* Tuning knob for experiments: selects the Ax kernel variant.  0 = the default per (precision, p): p = 8 runs on the
  * tensor cores, one warp per element (FP64: r/s contractions as DMMA m8n8k4; FP32: as TF32 m16n8k8 in three passes,
  * FP32-level accuracy), every other p <= 12 the streaming kernel; 1 = the simple plain-load kernel; 2 = the scalar
- * streaming kernel (p <= 12); 3 = FP64 p = 8 only: the DMMA kernel with 5 ring stages and 8 warps per SM.
+ * streaming kernel (p <= 12); 3 = FP64 p = 8 only: the DMMA kernel with 5 ring stages and 8 warps per SM; 4 = the
+ * pencil kernel (8 <= p <= 12: every 1-D contraction by a thread that owns a whole line of p values; the default for
+ * FP32 p = 9 and FP64 p = 12, where it measured faster than the streaming kernel).
  * 100 + v selects the kernel of sem_fdm_apply / the fused restricted Schwarz instead: 100 = the scalar line kernels
  * (default), 101 = FP32, 6 <= m <= 12: the tensor-core kernel (every 1-D contraction as TF32 m16n8k8 in three passes;
  * measured slower than the scalar kernels at every m, kept as the measurement north_star asks for).

@@ -13,10 +13,13 @@
 // That is ax_stream (every p <= 12; odd p takes u by plain loads).  At p = 8 -- the paper's N = 7 -- the r and s
 // contractions run on the tensor cores instead, one WARP per element with the same streaming ring: ax_dmma (FP64,
 // mma.sync m8n8k4; the measured DMMA path north_star asks for: it won), ax_tf32 (FP32, m16n8k8 TF32 in three passes),
-// ax_dmma_many (2 or 3 fields sharing one pass over G).  Kernels in this file, in order: ax_simple, ax_stream, ax_dmma,
-// ax_tf32, ax_dmma_many; then the launchers and the chunked operator / gather-scatter driver (sem_launch_ax_gs).
+// ax_dmma_many (2 or 3 fields sharing one pass over G).  Kernels in this file, in order: ax_simple, ax_stream, ax_pencil
+// (a measured alternative for p >= 8, one pencil of p values per thread and contraction), ax_dmma, ax_tf32,
+// ax_dmma_many; then the launchers and the chunked operator / gather-scatter driver (sem_launch_ax_gs).
 // ax_simple is the plain-load version of the same arithmetic: p > 12, unaligned pointers, and the recomputed-G
 // variant (a9: G from the 8 trilinear vertices inside the kernel) use it.
+#include <array>
+#include <map>
 #include <mutex>
 #include <type_traits>
 
@@ -431,6 +434,216 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
                 partial += uk[k] * v;
             }
         }
+    }
+    if (dot_out) block_dot_flush(partial, dot_out);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// ax_pencil: p >= 8, one element per CTA -- a measured ALTERNATIVE to ax_stream (sem_set_variant 4; the default only
+// where it won: FP32 p = 9, FP64 p = 12).  ax_stream gives thread (i, j) a k-column and keeps FOUR rows / columns of D
+// in its registers (80 registers at p = 10 in FP64), reads 4p shared-memory values per node and plane, and synchronises
+// the CTA once per plane: at p = 10 that is 166 registers, 12 warps per SM, 333 shared-memory wavefronts per plane
+// (0.79 per cycle and SM: the shared-memory pipe) and 0.69 of the HBM roofline.
+// Here every 1-D contraction is done by a thread that owns a whole PENCIL of p values along the contracted direction:
+// p inputs, p outputs, p^2 FMAs whose D operands have compile-time indices (uniform registers fed from the constant
+// bank; no per-thread rows of D).  Per element:
+//   A   thread (k, j): u_r along i for its row -> R;  thread (k, i): u_s along j for its column -> S          | barrier
+//   B   thread (j, i): u_t along k in registers; per plane k: G from the slab ring, (g_r, g_s, g_t) = G (u_r, u_s, u_t),
+//       g_r, g_s overwrite R, S in place, g_t stays in registers; then w_t = D^T g_t in registers         | barrier
+//   C1  thread (k, j): D^T g_r along its row, in place in R                                                  | barrier
+//   C2  thread (k, i): D^T g_s along its column, added into R                                                | barrier
+//   C3  thread (j, i): w = w_t + R (+ lambda B u) -> global, fused dot                                       | barrier
+// 20 shared-memory accesses per node instead of 48 (ncu at p = 10: 29.7 M wavefronts against 46.0 M), 5 CTA barriers
+// per element instead of p, 128 registers.  The G slabs are released by a second ("empty") mbarrier per ring stage on
+// which every thread arrives after its loads, so phase B has no CTA barrier; thread 0 refills the previous stage.
+// Measured (profiles/r2_sweep.md): no faster than ax_stream at p = 10, 11 in FP64 -- the uniform-register traffic for D
+// (LDCU / R2UR / moves) adds 0.9 instructions per FMA, and phase B consumes the element's G in one burst, so the CTA
+// waits for the ring (long-scoreboard and branch stalls on the full barriers) with only 16 warps per SM to hide it.
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+template <typename T, int P>
+__device__ __forceinline__ void store_row(T* __restrict__ ptr, const T (&v)[P]) {
+    if constexpr ((P * sizeof(T)) % 16 == 0) {
+        constexpr int V = 16 / sizeof(T);
+        using VT = typename std::conditional<sizeof(T) == 8, double2, float4>::type;
+#pragma unroll
+        for (int q = 0; q < P / V; ++q) {
+            VT o;
+            if constexpr (sizeof(T) == 8) { o.x = v[2 * q]; o.y = v[2 * q + 1]; }
+            else { o.x = v[4 * q]; o.y = v[4 * q + 1]; o.z = v[4 * q + 2]; o.w = v[4 * q + 3]; }
+            reinterpret_cast<VT*>(ptr)[q] = o;
+        }
+    } else if constexpr (sizeof(T) == 4 && (P * sizeof(T)) % 8 == 0) {
+#pragma unroll
+        for (int q = 0; q < P / 2; ++q) reinterpret_cast<float2*>(ptr)[q] = make_float2(v[2 * q], v[2 * q + 1]);
+    } else {
+#pragma unroll
+        for (int l = 0; l < P; ++l) ptr[l] = v[l];
+    }
+}
+
+// out[a] = sum_l D[a][l] in[l]  (TR = false)   or   sum_l D[l][a] in[l]  (TR = true); all D indices compile-time
+template <typename T, int P, bool TR>
+__device__ __forceinline__ void pencil_apply(const DParam<T, P>& dp, const T (&in)[P], T (&out)[P]) {
+#pragma unroll
+    for (int a = 0; a < P; ++a) {
+        T acc = T(0);
+#pragma unroll
+        for (int l = 0; l < P; ++l) acc += (TR ? dp.D[l * P + a] : dp.D[a * P + l]) * in[l];
+        out[a] = acc;
+    }
+}
+
+template <typename T, int P, int NS>
+struct PencilSmem {
+    static constexpr int P2 = P * P, P3 = P2 * P;
+    static constexpr int SLAB = 6 * P2 + ((6 * P2 * (int)sizeof(T)) % 16 ? 2 : 0);
+    static constexpr bool UBULK = (P3 * (int)sizeof(T)) % 16 == 0;
+    alignas(128) T g[NS][SLAB];
+    alignas(128) T u[2][P3];
+    alignas(16) T R[P3];
+    alignas(16) T S[P3];
+    alignas(8) uint64_t gfull[NS];
+    alignas(8) uint64_t gempty[NS];
+    alignas(8) uint64_t ufull[2];
+};
+
+template <typename T, int P, int NS, int MINB>
+__global__ void __launch_bounds__(threads_of<P>(), MINB) ax_pencil(int64_t E, DParam<T, P> dp, const T* __restrict__ Gs,
+                                                                   const T* __restrict__ Bm, T lambda,
+                                                                   const T* __restrict__ u, T* __restrict__ w,
+                                                                   const int* __restrict__ skip_flag,
+                                                                   double* __restrict__ dot_out, int u_keep) {
+    static_assert(epb_of<P>() == 1, "ax_pencil: one element per CTA");
+    using SM = PencilSmem<T, P, NS>;
+    constexpr int P2 = SM::P2, P3 = SM::P3, SLAB = SM::SLAB, NT = threads_of<P>();
+    constexpr bool UBULK = SM::UBULK;
+    constexpr uint32_t GBYTES = SLAB * sizeof(T), UBYTES = P3 * sizeof(T);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    SM& sm = *reinterpret_cast<SM*>(smem_raw);
+    if (skip_flag && *skip_flag) return;
+    const int tid = threadIdx.x;
+    const bool act = tid < P2;
+    const int64_t nmine = blockIdx.x < E ? (E - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+
+    // producer state (thread 0): slabs in consumption order
+    const T* gsrc = Gs + (int64_t)blockIdx.x * (P * SLAB);
+    const int64_t gjump = (int64_t)(gridDim.x - 1) * (P * SLAB);
+    int64_t gleft = nmine * P;
+    int gk = 0;
+    uint64_t pol_g = 0, pol_u = 0;
+    auto issue_g = [&](int q) {
+        mbar_expect_tx(&sm.gfull[q], GBYTES);
+        bulk_g2s(&sm.g[q][0], gsrc, GBYTES, &sm.gfull[q], pol_g);
+        gsrc += SLAB;
+        if (++gk == P) { gk = 0; gsrc += gjump; }
+        --gleft;
+    };
+    auto issue_u = [&](int64_t n) {
+        const int b = (int)(n & 1);
+        mbar_expect_tx(&sm.ufull[b], UBYTES);
+        bulk_g2s(&sm.u[b][0], u + (blockIdx.x + n * gridDim.x) * P3, UBYTES, &sm.ufull[b], pol_u);
+    };
+    if (tid == 0) {
+#pragma unroll
+        for (int q = 0; q < NS; ++q) { mbar_init(&sm.gfull[q], 1); mbar_init(&sm.gempty[q], P2); }
+        mbar_init(&sm.ufull[0], 1);
+        mbar_init(&sm.ufull[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (tid == 0 && nmine > 0) {
+        pol_g = policy_evict_first();
+        pol_u = u_keep ? policy_evict_last() : policy_evict_first();
+        if (UBULK) issue_u(0);
+        for (int q = 0; q < NS && gleft > 0; ++q) issue_g(q);
+        if (UBULK && nmine > 1) issue_u(1);
+    }
+    int q = 0, pq = 0;                 // ring stage of the slab being consumed / of the previous one (thread 0)
+    uint32_t gphase = 0, pphase = 0;
+    bool have_prev = false;
+    T partial = T(0);
+    const int cb = (tid / P) * P2 + tid % P;       // column pencil (k, i) of this thread: base index, stride P
+    for (int64_t n = 0; n < nmine; ++n) {
+        const int64_t e = blockIdx.x + n * gridDim.x;
+        const int ub = UBULK ? (int)(n & 1) : 0;
+        T* su = &sm.u[ub][0];
+        if constexpr (UBULK) {
+            mbar_wait(&sm.ufull[ub], (uint32_t)((n >> 1) & 1));
+        } else {
+            for (int idx = tid; idx < P3; idx += NT) su[idx] = u[e * P3 + idx];
+            __syncthreads();
+        }
+        T wt[P];
+        if (act) {
+            T in[P], out[P];
+            load_row<T, P>(su + tid * P, in);                     // A: u_r for row (k, j) = tid
+            pencil_apply<T, P, false>(dp, in, out);
+            store_row<T, P>(&sm.R[tid * P], out);
+#pragma unroll
+            for (int l = 0; l < P; ++l) in[l] = su[cb + l * P];   // A: u_s for column (k, i)
+            pencil_apply<T, P, false>(dp, in, out);
+#pragma unroll
+            for (int j = 0; j < P; ++j) sm.S[cb + j * P] = out[j];
+        }
+        __syncthreads();
+        if (act) {
+            T uk[P], gt[P];
+#pragma unroll
+            for (int k = 0; k < P; ++k) uk[k] = su[k * P2 + tid];
+            pencil_apply<T, P, false>(dp, uk, gt);                // u_t along k
+#pragma unroll
+            for (int k = 0; k < P; ++k) {
+                mbar_wait(&sm.gfull[q], gphase);
+                T g[6];
+#pragma unroll
+                for (int c = 0; c < 6; ++c) g[c] = sm.g[q][c * P2 + tid];
+                mbar_arrive(&sm.gempty[q]);
+                if (tid == 0) {                                   // refill the stage of the previous slab
+                    if (have_prev && gleft > 0) { mbar_wait(&sm.gempty[pq], pphase); issue_g(pq); }
+                    pq = q; pphase = gphase; have_prev = true;
+                }
+                const T ur = sm.R[k * P2 + tid], us = sm.S[k * P2 + tid], ut = gt[k];
+                sm.R[k * P2 + tid] = g[0] * ur + g[1] * us + g[2] * ut;
+                sm.S[k * P2 + tid] = g[1] * ur + g[3] * us + g[4] * ut;
+                gt[k] = g[2] * ur + g[4] * us + g[5] * ut;
+                if (++q == NS) { q = 0; gphase ^= 1u; }
+            }
+            pencil_apply<T, P, true>(dp, gt, wt);                 // w_t = D^T g_t along k
+        }
+        __syncthreads();
+        if (act) {                                                // C1: D^T g_r along the row, in place
+            T in[P], out[P];
+            load_row<T, P>(&sm.R[tid * P], in);
+            pencil_apply<T, P, true>(dp, in, out);
+            store_row<T, P>(&sm.R[tid * P], out);
+        }
+        __syncthreads();
+        if (act) {                                                // C2: D^T g_s along the column, added into R
+            T in[P], out[P];
+#pragma unroll
+            for (int l = 0; l < P; ++l) in[l] = sm.S[cb + l * P];
+            pencil_apply<T, P, true>(dp, in, out);
+#pragma unroll
+            for (int j = 0; j < P; ++j) sm.R[cb + j * P] += out[j];
+        }
+        __syncthreads();
+        if (act) {                                                // C3: results
+            T* wdst = w + e * P3 + tid;
+#pragma unroll
+            for (int k = 0; k < P; ++k) {
+                const T uu = su[k * P2 + tid];
+                T v = wt[k] + sm.R[k * P2 + tid];
+                if (Bm) v += lambda * Bm[e * P3 + k * P2 + tid] * uu;
+                wdst[k * P2] = v;
+                partial += uu * v;
+            }
+        }
+        __syncthreads();                                          // R, S and this u buffer are free again
+        if (UBULK && tid == 0 && n + 2 < nmine) issue_u(n + 2);
     }
     if (dot_out) block_dot_flush(partial, dot_out);
 }
@@ -1011,22 +1224,30 @@ Gll1D make_gll(const sem_ctx* c) {
 }
 
 // Resident CTAs per SM of one kernel instantiation with its dynamic shared memory, cached per device (the opt-in
-// attribute is per device as well).  One table per instantiation (the template parameter K is the kernel's type).
+// attribute is per device as well).  Keyed by the kernel's ADDRESS: two instantiations can share one function-pointer
+// type (ax_stream<double,10,..> and ax_pencil<double,10,..>; ax_dmma<3,12> and ax_dmma<5,8>), so a table per type would
+// hand the second one the first one's occupancy and never raise its shared-memory limit.
 template <typename K>
 int resident_blocks(sem_ctx* c, K kern, int threads, size_t smem, int* out) {
     static std::mutex mu;
-    static int table[SEM_MAX_DEVICES] = {};
+    static std::map<const void*, std::array<int, SEM_MAX_DEVICES>> tables;
     std::lock_guard<std::mutex> lk(mu);
     const bool cacheable = c->device >= 0 && c->device < SEM_MAX_DEVICES;
-    if (!cacheable || !table[c->device]) {
+    std::array<int, SEM_MAX_DEVICES>* table = nullptr;
+    if (cacheable) {
+        auto it = tables.find((const void*)kern);
+        if (it == tables.end()) it = tables.emplace((const void*)kern, std::array<int, SEM_MAX_DEVICES>{}).first;
+        table = &it->second;
+    }
+    if (!cacheable || !(*table)[c->device]) {
         int nb = 0;
         SEM_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         SEM_CUDA_OK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, threads, smem));
         if (nb < 1) return sem_fail(c, SEM_ECUDA, "Ax kernel does not fit on an SM");
         if (!cacheable) { *out = nb; return SEM_OK; }
-        table[c->device] = nb;
+        (*table)[c->device] = nb;
     }
-    *out = table[c->device];
+    *out = (*table)[c->device];
     return SEM_OK;
 }
 
@@ -1072,6 +1293,26 @@ int launch_stream(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, doubl
     if (int rc = resident_blocks(c, kern, threads_of<P>(), smem, &blocks_per_sm)) return rc;
     const int64_t cap = (int64_t)c->num_sms * blocks_per_sm;
     const unsigned grid = (unsigned)(ngroups < cap ? ngroups : cap);
+    kern<<<grid, threads_of<P>(), smem, c->stream>>>(r.ne, dp, Gs, lambda != T(0) ? Bm + r.e0 * P3 : (const T*)nullptr,
+                                                     lambda, u + r.e0 * P3, w + r.e0 * P3, skip, dot, u_keep(c, sizeof(T)));
+    SEM_CUDA_OK(c, cudaGetLastError());
+    return SEM_OK;
+}
+
+template <typename T, int P, int NS, int MINB>
+int launch_pencil(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, double* dot) {
+    using SM = PencilSmem<T, P, NS>;
+    constexpr int P3 = P * P * P;
+    const ElemRange r = elem_range(c);
+    const T* Gs = (sizeof(T) == 8 ? (const T*)c->d_G : (const T*)c->d_G32) + r.e0 * P * SM::SLAB;
+    const T* Bm = sizeof(T) == 8 ? (const T*)c->d_B : (const T*)c->d_B32;
+    const DParam<T, P> dp = make_dparam<T, P>(c);
+    const size_t smem = sizeof(SM) + 128;
+    auto kern = ax_pencil<T, P, NS, MINB>;
+    int blocks_per_sm = 0;
+    if (int rc = resident_blocks(c, kern, threads_of<P>(), smem, &blocks_per_sm)) return rc;
+    const int64_t cap = (int64_t)c->num_sms * blocks_per_sm;
+    const unsigned grid = (unsigned)(r.ne < cap ? r.ne : cap);
     kern<<<grid, threads_of<P>(), smem, c->stream>>>(r.ne, dp, Gs, lambda != T(0) ? Bm + r.e0 * P3 : (const T*)nullptr,
                                                      lambda, u + r.e0 * P3, w + r.e0 * P3, skip, dot, u_keep(c, sizeof(T)));
     SEM_CUDA_OK(c, cudaGetLastError());
@@ -1169,6 +1410,12 @@ int dispatch_p(sem_ctx* c, const void* u, void* w, double lambda, const int* ski
     }
     if constexpr (P == 8 && sizeof(T) == 4) {          // FP32 p = 8: the TF32 x 3 tensor-core kernel
         if (aligned && c->ax_variant == 0) return launch_tf32<3, 12>(c, (const float*)u, (float*)w, (float)lambda, skip, dot);
+    }
+    // the pencil kernel (variant 4, p = 8 ... 12): the default only where it measured faster than ax_stream
+    if constexpr (P >= 8 && P <= 12) {
+        constexpr bool WINS = (sizeof(T) == 4 && P == 9) || (sizeof(T) == 8 && P == 12);
+        if (aligned && (c->ax_variant == 4 || (WINS && c->ax_variant == 0)))
+            return launch_pencil<T, P, 4, (P == 8 ? 8 : sizeof(T) == 8 ? 4 : 5)>(c, uu, ww, (T)lambda, skip, dot);
     }
     if constexpr (stream_ok<P>()) {
         if (c->ax_variant != 1 && aligned)

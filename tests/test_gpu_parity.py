@@ -174,8 +174,8 @@ def _ax_case(torch, binding, oracle_mod, mesh, variant=0, mode=0, lam=0.0, dtype
     return relerr(w, ow)
 
 
-@pytest.mark.parametrize("N", [1, 2, 3, 4, 5, 6, 7, 8, 9, 11, 13, 15])
-@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+@pytest.mark.parametrize("N", [1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 13, 15])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4])
 def test_ax_f64_all_orders(torch_cuda, binding, oracle_mod, N, variant):
     # 5*3*3 = 45 elements: not a multiple of the elements-per-block of any p (ragged tail), several blocks
     m = inputs.box_mesh(5, 3, 3, N, "random", seed=N)
@@ -196,20 +196,29 @@ def test_ax_many_elements_per_cta(torch_cuda, binding, oracle_mod, N):
     assert _ax_case(torch_cuda, binding, oracle_mod, m) <= TOL64
 
 
+@pytest.mark.parametrize("N,dtype", [(7, "f64"), (8, "f64"), (8, "f32"), (9, "f64"), (11, "f64"), (11, "f32")])
+def test_ax_pencil_many_elements_per_cta(torch_cuda, binding, oracle_mod, N, dtype):
+    """The pencil kernel (variant 4) with several elements per persistent CTA: the G ring and its empty-barriers wrap
+    many times, u alternates between its two buffers (even p) or is re-staged (odd p)."""
+    n = {7: 16, 8: 14, 9: 13, 11: 11}[N]
+    m = inputs.box_mesh(n, n, n + 1, N, "random", seed=2)
+    assert _ax_case(torch_cuda, binding, oracle_mod, m, variant=4, dtype=dtype) <= (TOL64 if dtype == "f64" else TOL32)
+
+
 @pytest.mark.parametrize("N", [1, 2, 3, 5, 7, 9])
 def test_ax_recomputed_G(torch_cuda, binding, oracle_mod, N):
     m = inputs.box_mesh(4, 3, 3, N, "random", seed=3)
     assert _ax_case(torch_cuda, binding, oracle_mod, m, mode=1) <= TOL64
 
 
-@pytest.mark.parametrize("N,variant", [(7, 0), (7, 1), (7, 2), (7, 3), (4, 0), (3, 0)])
+@pytest.mark.parametrize("N,variant", [(7, 0), (7, 1), (7, 2), (7, 3), (4, 0), (3, 0), (8, 4), (9, 4), (11, 0), (7, 4)])
 def test_ax_helmholtz(torch_cuda, binding, oracle_mod, N, variant):
     m = inputs.box_mesh(3, 3, 3, N, "smooth")
     assert _ax_case(torch_cuda, binding, oracle_mod, m, variant=variant, lam=37.5) <= TOL64
 
 
 @pytest.mark.parametrize("N", [1, 2, 3, 5, 7, 9])
-@pytest.mark.parametrize("variant,mode", [(0, 0), (1, 0), (2, 0), (0, 1)])
+@pytest.mark.parametrize("variant,mode", [(0, 0), (1, 0), (2, 0), (0, 1), (4, 0)])
 def test_ax_f32(torch_cuda, binding, oracle_mod, N, variant, mode):
     m = inputs.box_mesh(5, 4, 3, N, "smooth")
     assert _ax_case(torch_cuda, binding, oracle_mod, m, variant=variant, mode=mode, dtype="f32") <= TOL32
