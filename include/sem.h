@@ -237,6 +237,22 @@ SEM_API int sem_cheby(sem_ctx* ctx, const void* b, void* x, int order, double lm
  * estimate ||diag^-1 A v|| / ||v||, which approaches lambda_max from below: multiply by a safety factor (1.1). */
 SEM_API int sem_lambda_max(sem_ctx* ctx, int iters, double* lam_out);
 
+/* The Chebyshev-Jacobi smoother of sem_cheby, FP64, for callers that cannot allocate device memory (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc).  It calls no cudaMalloc / cudaFree and no allocating
+ * library routine: its three work vectors live in a static device array inside the library, 3 x SEM_NOALLOC_MAX_NODES
+ * doubles (12 MB, held by every GPU that loads the library until the process exits).  b, x, order, lmin, lmax,
+ * zero_guess as in sem_cheby; the result equals sem_cheby's matrix-free FP64 path.
+ * Requirements: nL <= SEM_NOALLOC_MAX_NODES (else SEM_EINVAL with a message naming the limit); stored geometric
+ * factors; the Jacobi diagonal already built for the current lambda by an earlier sem_get_diag / sem_cheby / sem_pcg
+ * call (else SEM_ESTATE: building it would allocate); the context's device current.  The first call on a device
+ * resolves the array's address (cudaGetSymbolAddress; no allocation) -- make it outside stream capture.
+ * Every call on a device, from any context, shares the array, which keeps the previous call's contents (a call only
+ * reads what it wrote itself, nothing needs clearing): calls that overlap on the GPU (different streams) race.
+ * Asynchronous on the context's stream. */
+#define SEM_NOALLOC_MAX_NODES (1 << 19)
+SEM_API int sem_cheby_noalloc(sem_ctx* ctx, const double* b, double* x, int order, double lmin, double lmax,
+                              int zero_guess);
+
 /* NEXT-1c.  p-multigrid V-cycle preconditioner z = M^-1 r over `nlevels` contexts, finest first
  * (the cycle is reading S25 in DESIGN.md and is written out in csrc/sem_pmg.cu): Chebyshev-Jacobi
  * pre- and post-smoothing of `smooth_order` steps on every level but the coarsest, multiplicity-weighted restriction

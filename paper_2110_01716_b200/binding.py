@@ -19,6 +19,7 @@ SEM_OP_ADD = 0
 SEM_G_STORED, SEM_G_RECOMPUTE = 0, 1
 SEM_PROLONG, SEM_RESTRICT = 0, 1
 SEM_INTERLEAVED = 1
+SEM_NOALLOC_MAX_NODES = 1 << 19
 SEM_SCHWARZ_ASM, SEM_SCHWARZ_RAS = 0, 1
 SEM_SMOOTH_CHEBY_JACOBI, SEM_SMOOTH_CHEBY_SCHWARZ, SEM_SMOOTH_CHEBY_RAS = 0, 1, 2
 SEM_OK, SEM_EINVAL, SEM_EMESH, SEM_ECUDA, SEM_ENOMEM, SEM_ESTATE = 0, -1, -2, -3, -4, -5
@@ -50,6 +51,7 @@ SYMBOLS = {
     "sem_get_interp": (_i32, [_vp, _vp, _vp]),
     "sem_cheby": (_i32, [_vp, _vp, _vp, _i32, _dbl, _dbl, _i32, _i32]),
     "sem_lambda_max": (_i32, [_vp, _i32, C.POINTER(_dbl)]),
+    "sem_cheby_noalloc": (_i32, [_vp, _vp, _vp, _i32, _dbl, _dbl, _i32]),
     "sem_pmg_create": (_i32, [C.POINTER(_vp), _i32, C.POINTER(_vp), C.POINTER(_dbl), C.POINTER(_dbl), _i32, _i32, _i32]),
     "sem_pmg_vcycle": (_i32, [_vp, _vp, _vp]),
     "sem_pmg_destroy": (None, [_vp]),
@@ -386,6 +388,14 @@ class Sem:
     def cheby(self, b, x, order: int, lmin: float, lmax: float, zero_guess: bool = False):
         self._check(self._L.sem_cheby(self._h, self._vec(b), self._vec(x), order, lmin, lmax, int(zero_guess),
                                       self._prec(x)))
+        return x
+
+    def cheby_noalloc(self, b, x, order: int, lmin: float, lmax: float, zero_guess: bool = False):
+        """sem_cheby_noalloc: FP64, nL <= SEM_NOALLOC_MAX_NODES, work vectors in the library's static device array."""
+        import torch
+
+        assert b.dtype == torch.float64 and x.dtype == torch.float64
+        self._check(self._L.sem_cheby_noalloc(self._h, self._vec(b), self._vec(x), order, lmin, lmax, int(zero_guess)))
         return x
 
     def lambda_max(self, iters: int = 30) -> float:

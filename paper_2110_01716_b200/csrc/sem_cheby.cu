@@ -14,6 +14,8 @@
 #include <math.h>
 #include <stdlib.h>
 
+#include <mutex>
+
 #include "sem_internal.h"
 
 namespace {
@@ -349,5 +351,94 @@ extern "C" int sem_lambda_max_schwarz(sem_ctx* c, sem_schwarz_kind kind, int ite
     }
     SEM_CUDA_OK(c, cudaGetLastError());
     *lam_out = lam;
+    return SEM_OK;
+}
+
+
+// ---------------------------------------------------------------------------------------------------------------
+// sem_cheby_noalloc: the Chebyshev-Jacobi smoother (FP64) for callers that cannot allocate device memory -- code under
+// CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  sem_cheby allocates its three work
+// vectors (and, if needed, the Jacobi diagonal) on first use; this entry point allocates NOTHING: r, d, w live in the
+// file-scope array below (3 x SEM_NOALLOC_MAX_NODES doubles = 12 MB, part of the library image: every GPU that loads
+// the library holds it until the process exits), and the Jacobi diagonal must already be current.
+// The array's name is a device symbol: in host code it is only a stand-in, so its device address is resolved once per
+// device with cudaGetSymbolAddress (that device current) and that pointer is what the kernels get.
+// All calls (all contexts on a device) share the array; it keeps the last call's contents, and every value a call reads
+// from it was written earlier by the same call (k_cheb_first writes all of r and d, the operator all of w), so nothing
+// has to be cleared.  Two calls that overlap on the GPU (different streams) race on it.
+// ---------------------------------------------------------------------------------------------------------------
+static __device__ __align__(256) double sem_noalloc_scratch[3 * (size_t)SEM_NOALLOC_MAX_NODES];
+
+namespace {
+
+std::mutex noalloc_mu;
+double* noalloc_ptr[SEM_MAX_DEVICES] = {};      // device address of sem_noalloc_scratch, per device
+
+// set-up, once per device: the context's device must be the current one
+int noalloc_resolve(sem_ctx* c, double** out) {
+    if (c->device < 0 || c->device >= SEM_MAX_DEVICES) return sem_fail(c, SEM_EINVAL, "sem_cheby_noalloc: device index out of range");
+    int cur = -1;
+    SEM_CUDA_OK(c, cudaGetDevice(&cur));
+    if (cur != c->device) return sem_fail(c, SEM_ESTATE, "sem_cheby_noalloc: the context's device %d is not current (%d)", c->device, cur);
+    std::lock_guard<std::mutex> lk(noalloc_mu);
+    if (!noalloc_ptr[cur]) {
+        double* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress((void**)&p, sem_noalloc_scratch);
+        if (e != cudaSuccess || !p) return sem_fail(c, SEM_ECUDA, "sem_cheby_noalloc: cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+        noalloc_ptr[cur] = p;
+    }
+    *out = noalloc_ptr[cur];
+    return SEM_OK;
+}
+
+}  // namespace
+
+extern "C" int sem_cheby_noalloc(sem_ctx* c, const double* b, double* x, int order, double lmin, double lmax,
+                                 int zero_guess) {
+    if (!c) return SEM_EINVAL;
+    c->err.clear();
+    if (!b || !x || b == x) return sem_fail(c, SEM_EINVAL, "sem_cheby_noalloc: NULL or aliased vectors");
+    if (order < 1 || !(lmin > 0.0) || !(lmax > lmin))
+        return sem_fail(c, SEM_EINVAL, "sem_cheby_noalloc: need order >= 1 and 0 < lmin < lmax");
+    if (((uintptr_t)x % 16) || ((uintptr_t)b % 8)) return sem_fail(c, SEM_EINVAL, "sem_cheby_noalloc: x must be 16-byte aligned");
+    if (c->nL > (int64_t)SEM_NOALLOC_MAX_NODES)
+        return sem_fail(c, SEM_EINVAL, "sem_cheby_noalloc: %lld local nodes exceed SEM_NOALLOC_MAX_NODES = %d (use sem_cheby)",
+                        (long long)c->nL, (int)SEM_NOALLOC_MAX_NODES);
+    if (!c->geom_done) return sem_fail(c, SEM_ESTATE, "sem_cheby_noalloc before sem_geom");
+    if (c->gmode != SEM_G_STORED) return sem_fail(c, SEM_ESTATE, "sem_cheby_noalloc needs stored geometric factors");
+    if (c->lambda != 0.0 && !c->with_mass) return sem_fail(c, SEM_ESTATE, "lambda != 0 needs with_mass");
+    if (!c->d_Minv || c->lambda_of_diag != c->lambda)
+        return sem_fail(c, SEM_ESTATE, "sem_cheby_noalloc: the Jacobi diagonal is not built for this lambda "
+                                       "(call sem_get_diag, sem_cheby or sem_pcg once before)");
+    double* s = nullptr;
+    int rc = noalloc_resolve(c, &s);
+    if (rc) return rc;
+    cudaStream_t st = c->stream;
+    const int64_t n = c->nL;
+    double *r = s, *d = s + SEM_NOALLOC_MAX_NODES, *w = s + 2 * (size_t)SEM_NOALLOC_MAX_NODES;
+    const double* Minv = c->d_Minv;
+    const unsigned grid = (unsigned)c->num_sms * 8;
+    const double theta = 0.5 * (lmax + lmin), delta = 0.5 * (lmax - lmin), sigma = theta / delta;
+    double rho = 1.0 / sigma;
+    const double* q = nullptr;
+    if (!zero_guess) {
+        k_mask_x<double><<<grid, 256, 0, st>>>(n, Minv, x);
+        if ((rc = sem_launch_ax_gs(c, x, w, SEM_F64, c->lambda, nullptr, nullptr))) return rc;
+        q = w;
+    }
+    if (order == 1) k_cheb_first<double, true><<<grid, 256, 0, st>>>(n, b, q, Minv, 1.0 / theta, x, r, d);
+    else k_cheb_first<double, false><<<grid, 256, 0, st>>>(n, b, q, Minv, 1.0 / theta, x, r, d);
+    for (int k = 1; k < order; ++k) {
+        if ((rc = sem_launch_ax_gs(c, d, w, SEM_F64, c->lambda, nullptr, nullptr))) return rc;
+        const double rho1 = 1.0 / (2.0 * sigma - rho);
+        const double c1 = rho1 * rho, c2 = 2.0 * rho1 / delta;
+        const bool xzero = zero_guess && k == 1, last = k == order - 1;
+        if (xzero && last) k_cheb_step<double, true, true><<<grid, 256, 0, st>>>(n, w, Minv, c1, c2, x, r, d);
+        else if (xzero) k_cheb_step<double, true, false><<<grid, 256, 0, st>>>(n, w, Minv, c1, c2, x, r, d);
+        else if (last) k_cheb_step<double, false, true><<<grid, 256, 0, st>>>(n, w, Minv, c1, c2, x, r, d);
+        else k_cheb_step<double, false, false><<<grid, 256, 0, st>>>(n, w, Minv, c1, c2, x, r, d);
+        rho = rho1;
+    }
+    SEM_CUDA_OK(c, cudaGetLastError());
     return SEM_OK;
 }
