@@ -825,6 +825,184 @@ __global__ void __launch_bounds__(32, MINB) ax_dmma(int64_t E, DParam<double, 8>
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// ax_dmma_rg: a9 (north_star: "recomputed geometric factors to cut bytes per node"), FP64, p = 8, trilinear elements.
+// The tensor-core kernel above without the G ring: the six factors of a node are recomputed in registers from the
+// element's 8 vertices (192 bytes, bulk-copied beside u) -- 16 bytes per node of HBM traffic instead of 64, about
+// twice the FP64 arithmetic (the 3 x 3 Jacobian of the trilinear map is linear in t for fixed (r, s), so a lane keeps
+// 24 coefficients for its two columns and a plane costs 6 FMAs for J, then the adjugate, one division and
+// G = (W / det) adj adj^T: ~65 FMA-pipe instructions per node against ~57 for the whole rest of the operator).
+// The kernel is bound by the FP64 pipe, not by memory; it replaces ax_simple<RECOMP> for p = 8.
+// lambda B u is accumulated plane by plane (B = W det comes out of the same computation).
+// ---------------------------------------------------------------------------------------------------------------
+struct GllP8 { double xi[8], rho[8]; };
+
+template <int NU>
+struct DmmaRgSmem {
+    alignas(128) double u[NU][512];
+    alignas(16) double vert[NU][24];
+    alignas(16) double sgs[2][64];
+    alignas(8) uint64_t ufull[NU];
+    alignas(16) double D[64];
+    alignas(16) double xr[16];               // xi, rho for lane-dependent indices (a by-value parameter indexed
+};                                           // dynamically would be copied to local memory)
+
+template <int MINB, int NU, bool HELM>
+__global__ void __launch_bounds__(32, MINB) ax_dmma_rg(int64_t E, DParam<double, 8> dp, GllP8 gll,
+                                                       const double* __restrict__ vert, double lambda,
+                                                       const double* __restrict__ u, double* __restrict__ w,
+                                                       const int* __restrict__ skip_flag, double* __restrict__ dot_out,
+                                                       int u_keep) {
+    using SM = DmmaRgSmem<NU>;
+    constexpr int P = 8, P2 = 64, P3 = 512;
+    constexpr uint32_t UBYTES = P3 * sizeof(double), VBYTES = 24 * sizeof(double);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    SM& sm = *reinterpret_cast<SM*>(smem_raw);
+    if (skip_flag && *skip_flag) return;
+    const int lane = threadIdx.x, g = lane >> 2, t = lane & 3;
+    const int64_t nmine = blockIdx.x < E ? (E - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    uint64_t pol_u = 0, pol_v = 0;
+    auto issue_u = [&](int64_t n) {
+        const int64_t e = blockIdx.x + n * gridDim.x;
+        const int b = (int)(n % NU);
+        mbar_expect_tx(&sm.ufull[b], UBYTES + VBYTES);
+        bulk_g2s(&sm.u[b][0], u + e * P3, UBYTES, &sm.ufull[b], pol_u);
+        bulk_g2s(&sm.vert[b][0], vert + e * 24, VBYTES, &sm.ufull[b], pol_v);
+    };
+    if (lane == 0) {
+#pragma unroll
+        for (int q = 0; q < NU; ++q) mbar_init(&sm.ufull[q], 1);
+        mbar_fence_init();
+    }
+    sm.D[lane] = dp.D[lane];
+    sm.D[lane + 32] = dp.D[lane + 32];
+#pragma unroll
+    for (int q = 0; q < 8; ++q)
+        if (lane == q) { sm.xr[q] = gll.xi[q]; sm.xr[8 + q] = gll.rho[q]; }
+    __syncwarp();
+    if (lane == 0 && nmine > 0) {
+        pol_v = policy_evict_first();
+        pol_u = u_keep ? policy_evict_last() : policy_evict_first();
+        issue_u(0);
+        if (NU == 2 && nmine > 1) issue_u(1);
+    }
+    double Br[2], As[2], BrT[2], AsT[2];
+    {
+        const uint32_t base = smem_u32(sm.D);
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            Br[c] = DRows<double, 8>::lds_volatile(base + (uint32_t)((g * 8 + 2 * t + c) * 8));
+            As[c] = DRows<double, 8>::lds_volatile(base + (uint32_t)((g * 8 + 4 * c + t) * 8));
+            BrT[c] = DRows<double, 8>::lds_volatile(base + (uint32_t)(((2 * t + c) * 8 + g) * 8));
+            AsT[c] = DRows<double, 8>::lds_volatile(base + (uint32_t)(((4 * c + t) * 8 + g) * 8));
+        }
+    }
+    // the lane's two columns: (r, s) = (xi_i, xi_j), i = 2t, 2t + 1, j = g; W_ij = rho_i rho_j
+    const double sj = sm.xr[g], rj = sm.xr[8 + g];
+    const double ri[2] = {sm.xr[2 * t], sm.xr[2 * t + 1]};
+    const double Wij[2] = {sm.xr[8 + 2 * t] * rj, sm.xr[8 + 2 * t + 1] * rj};
+    double partial = 0.0;
+    const int own = g * 8 + 2 * t;
+    double* wdst = w + (int64_t)blockIdx.x * P3 + own;
+    const int64_t wstep = (int64_t)gridDim.x * P3;
+    for (int64_t n = 0; n < nmine; ++n, wdst += wstep) {
+        const int ub = (int)(n % NU);
+        mbar_wait(&sm.ufull[ub], (uint32_t)((n / NU) & 1));
+        const double* sue = &sm.u[ub][0];
+        // Jacobian coefficients of the lane's two columns: dx/dr = Ja + Jb t, dx/ds = Jc + Jd t, dx/dt = Je (S5)
+        double Ja[3], Jb[3], Jc[2][3], Jd[2][3], Je[2][3];
+        {
+            double X[8][3], cf[8][3];
+#pragma unroll
+            for (int v = 0; v < 8; ++v)
+#pragma unroll
+                for (int d = 0; d < 3; ++d) X[v][d] = sm.vert[ub][v * 3 + d];
+            sem_trilinear_coef(X, cf);
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                Ja[d] = cf[1][d] + cf[4][d] * sj;
+                Jb[d] = cf[5][d] + cf[7][d] * sj;
+#pragma unroll
+                for (int b = 0; b < 2; ++b) {
+                    Jc[b][d] = cf[2][d] + cf[4][d] * ri[b];
+                    Jd[b][d] = cf[6][d] + cf[7][d] * ri[b];
+                    Je[b][d] = cf[3][d] + cf[5][d] * ri[b] + (cf[6][d] + cf[7][d] * ri[b]) * sj;
+                }
+            }
+        }
+        double uk[P][2], wk[P][2];
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+            const double2 v = *reinterpret_cast<const double2*>(sue + k * P2 + own);
+            uk[k][0] = v.x; uk[k][1] = v.y; wk[k][0] = 0.0; wk[k][1] = 0.0;
+        }
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+            const double tk = gll.xi[k], rk = gll.rho[k];
+            double ur[2] = {0.0, 0.0}, us[2] = {0.0, 0.0};
+            dmma884(ur[0], ur[1], uk[k][0], Br[0]);
+            dmma884(us[0], us[1], As[0], sue[k * P2 + t * P + g]);
+            dmma884(ur[0], ur[1], uk[k][1], Br[1]);
+            dmma884(us[0], us[1], As[1], sue[k * P2 + (4 + t) * P + g]);
+            double ut[2] = {0.0, 0.0};
+#pragma unroll
+            for (int l = 0; l < P; ++l) { ut[0] += dp.D[k * P + l] * uk[l][0]; ut[1] += dp.D[k * P + l] * uk[l][1]; }
+            // G (u_r, u_s, u_t) without forming G:  G = (W / det) A A^T with the adjugate rows a_0 = x_s x x_t,
+            // a_1 = x_t x x_r, a_2 = x_r x x_s of the Jacobian columns, so  G v = (W / det) A (A^T v): 21 FMAs
+            // instead of 24 for G plus 9 for the product; det = x_r . a_0; one reciprocal
+            double gr[2], gs[2], gt[2], Bk[2];
+#pragma unroll
+            for (int b = 0; b < 2; ++b) {
+                double xr[3], xs[3];
+#pragma unroll
+                for (int d = 0; d < 3; ++d) { xr[d] = Ja[d] + Jb[d] * tk; xs[d] = Jc[b][d] + Jd[b][d] * tk; }
+                const double* xt = Je[b];
+                const double a0x = xs[1] * xt[2] - xs[2] * xt[1], a0y = xs[2] * xt[0] - xs[0] * xt[2],
+                             a0z = xs[0] * xt[1] - xs[1] * xt[0];
+                const double a1x = xt[1] * xr[2] - xt[2] * xr[1], a1y = xt[2] * xr[0] - xt[0] * xr[2],
+                             a1z = xt[0] * xr[1] - xt[1] * xr[0];
+                const double a2x = xr[1] * xs[2] - xr[2] * xs[1], a2y = xr[2] * xs[0] - xr[0] * xs[2],
+                             a2z = xr[0] * xs[1] - xr[1] * xs[0];
+                const double det = xr[0] * a0x + xr[1] * a0y + xr[2] * a0z;
+                const double Wk = Wij[b] * rk;
+                const double sc = Wk * __drcp_rn(det);
+                const double zx = a0x * ur[b] + a1x * us[b] + a2x * ut[b];
+                const double zy = a0y * ur[b] + a1y * us[b] + a2y * ut[b];
+                const double zz = a0z * ur[b] + a1z * us[b] + a2z * ut[b];
+                gr[b] = sc * (a0x * zx + a0y * zy + a0z * zz);
+                gs[b] = sc * (a1x * zx + a1y * zy + a1z * zz);
+                gt[b] = sc * (a2x * zx + a2y * zy + a2z * zz);
+                Bk[b] = HELM ? lambda * Wk * det : 0.0;
+            }
+            const int buf = k & 1;
+            *reinterpret_cast<double2*>(&sm.sgs[buf][own]) = make_double2(gs[0], gs[1]);
+#pragma unroll
+            for (int l = 0; l < P; ++l) { wk[l][0] += dp.D[k * P + l] * gt[0]; wk[l][1] += dp.D[k * P + l] * gt[1]; }
+            __syncwarp();
+            double a0[2] = {0.0, 0.0}, a1[2] = {0.0, 0.0};
+            dmma884(a0[0], a0[1], gr[0], BrT[0]);
+            dmma884(a1[0], a1[1], AsT[0], sm.sgs[buf][t * P + g]);
+            dmma884(a0[0], a0[1], gr[1], BrT[1]);
+            dmma884(a1[0], a1[1], AsT[1], sm.sgs[buf][(4 + t) * P + g]);
+            wk[k][0] += a0[0] + a1[0];
+            wk[k][1] += a0[1] + a1[1];
+            if constexpr (HELM) { wk[k][0] += Bk[0] * uk[k][0]; wk[k][1] += Bk[1] * uk[k][1]; }
+        }
+        // every lane has read this element's u (the last plane's B operands before the __syncwarp above): refill
+        __syncwarp();
+        if (lane == 0 && n + NU < nmine) issue_u(n + NU);
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+            *reinterpret_cast<double2*>(wdst + k * P2) = make_double2(wk[k][0], wk[k][1]);
+            partial += uk[k][0] * wk[k][0] + uk[k][1] * wk[k][1];
+        }
+    }
+    if (dot_out) {
+        for (int o = 16; o; o >>= 1) partial += __shfl_xor_sync(0xffffffffu, partial, o);
+        if (lane == 0) atomicAdd(dot_out, partial);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // ax_tf32: FP32, p = 8, one warp per element like ax_dmma, the r and s contractions on the tensor cores as
 // mma.sync.m16n8k8 TF32 in THREE passes (x = hi + lo with hi = tf32(x), lo = tf32(x - hi); hi*hi + lo*hi + hi*lo, the
 // dropped lo*lo term is 2^-22 relative: FP32-level accuracy, inside the 1e-5 bar of S16; accumulation in FP32).  There
@@ -1337,6 +1515,25 @@ int launch_dmma(sem_ctx* c, const double* u, double* w, double lambda, const int
     return SEM_OK;
 }
 
+template <int MINB, int NU = 2>
+int launch_dmma_rg(sem_ctx* c, const double* u, double* w, double lambda, const int* skip, double* dot) {
+    using SM = DmmaRgSmem<NU>;
+    const DParam<double, 8> dp = make_dparam<double, 8>(c);
+    GllP8 gll;
+    for (int i = 0; i < 8; ++i) { gll.xi[i] = c->xi[i]; gll.rho[i] = c->rho[i]; }
+    const size_t smem = sizeof(SM) + 128;
+    auto kern = lambda != 0.0 ? ax_dmma_rg<MINB, NU, true> : ax_dmma_rg<MINB, NU, false>;
+    int blocks_per_sm = 0;
+    if (int rc = resident_blocks(c, kern, 32, smem, &blocks_per_sm)) return rc;
+    const ElemRange r = elem_range(c);
+    const int64_t cap = (int64_t)c->num_sms * blocks_per_sm;
+    const unsigned grid = (unsigned)(r.ne < cap ? r.ne : cap);
+    kern<<<grid, 32, smem, c->stream>>>(r.ne, dp, gll, c->d_vert + r.e0 * 24, lambda, u + r.e0 * 512, w + r.e0 * 512, skip, dot,
+                                        u_keep(c, 8));
+    SEM_CUDA_OK(c, cudaGetLastError());
+    return SEM_OK;
+}
+
 template <int NS, int MINB>
 int launch_tf32(sem_ctx* c, const float* u, float* w, float lambda, const int* skip, double* dot) {
     using SM = Tf32Smem<NS>;
@@ -1401,7 +1598,12 @@ int dispatch_p(sem_ctx* c, const void* u, void* w, double lambda, const int* ski
     const T* uu = (const T*)u;
     T* ww = (T*)w;
     const bool aligned = ((uintptr_t)u % 16) == 0;
-    if (c->gmode == SEM_G_RECOMPUTE) return launch_simple<T, P, true>(c, uu, ww, (T)lambda, skip, dot);
+    if (c->gmode == SEM_G_RECOMPUTE) {
+        if constexpr (P == 8 && sizeof(T) == 8) {      // a9 on the tensor cores, no G traffic; variant 1 keeps ax_simple
+            if (aligned && c->ax_variant != 1) return launch_dmma_rg<8>(c, (const double*)u, (double*)w, lambda, skip, dot);
+        }
+        return launch_simple<T, P, true>(c, uu, ww, (T)lambda, skip, dot);
+    }
     // variant 0: the default kernel per (T, p): p = 8 runs on the tensor cores (FP64: DMMA, FP32: TF32 x 3);
     // 1: ax_simple; 2: ax_stream (scalar contractions); 3: FP64 p = 8: the DMMA kernel with 5 stages / 8 warps per SM
     if constexpr (P == 8 && sizeof(T) == 8) {

@@ -1025,3 +1025,30 @@ def test_gs_many_node_interleaved(torch_cuda, binding, oracle_mod, N, nf):
             with pytest.raises(binding.SemError):
                 sem._check(sem._L.sem_gs_many(sem._h, dw.data_ptr(), bad, binding.SEM_INTERLEAVED, binding.SEM_F64,
                                               binding.SEM_OP_ADD))
+
+
+@pytest.mark.parametrize("lam", [0.0, 2.5])
+def test_ax_recomputed_G_tensor_core_kernel(torch_cuda, binding, oracle_mod, lam):
+    """a9 at p = 8, FP64: ax_dmma_rg (the factors recomputed in registers from the 8 vertices, contractions on the tensor
+    cores) with several elements per persistent warp (both u / vertex buffers and their barrier phases wrap) and a ragged
+    last round; against the oracle (1e-12), the stored-G operator and ax_simple's recomputation; Helmholtz term included."""
+    m = inputs.box_mesh(14, 13, 13, 7, "random", seed=9, permute_seed=1)          # 2366 elements on <= 1184 warps
+    oG, _, rc = oracle_mod.geom_trilinear(m.vert, m.N)
+    assert rc == 0
+    u = inputs.field_uniform(m.gid, 4)
+    ow = oracle_mod.ax(oG, u, m.N, lam)
+    du = to_dev(torch_cuda, u.ravel())
+    got = {}
+    for mode, variant in ((binding.SEM_G_RECOMPUTE, 0), (binding.SEM_G_RECOMPUTE, 1), (binding.SEM_G_STORED, 0)):
+        with binding.Sem(m.E, m.N, m.vert, m.gid) as sem:
+            sem.geom(mode=mode, with_mass=lam != 0.0)
+            sem.set_variant(variant)
+            dw = torch_cuda.full_like(du, float("nan"))
+            sem.ax(du, dw, lam)
+            got[(mode, variant)] = dw.cpu().numpy().reshape(ow.shape)
+            if mode == binding.SEM_G_RECOMPUTE and variant == 0:                  # run to run: bit-identical
+                dw2 = torch_cuda.full_like(du, float("nan"))
+                sem.ax(du, dw2, lam)
+                assert torch_cuda.equal(dw, dw2)
+    for k, w in got.items():
+        assert relerr(w, ow) <= TOL64, k
