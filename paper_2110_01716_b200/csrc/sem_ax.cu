@@ -16,8 +16,8 @@
 // ax_dmma_many (2 or 3 fields sharing one pass over G).  Kernels in this file, in order: ax_simple, ax_stream, ax_pencil
 // (a measured alternative for p >= 8, one pencil of p values per thread and contraction), ax_dmma, ax_tf32,
 // ax_dmma_many; then the launchers and the chunked operator / gather-scatter driver (sem_launch_ax_gs).
-// ax_simple is the plain-load version of the same arithmetic: p > 12, unaligned pointers, and the recomputed-G
-// variant (a9: G from the 8 trilinear vertices inside the kernel) use it.
+// ax_simple is the plain-load version of the same arithmetic: p > 12 and unaligned pointers use it.  a9 (G recomputed
+// from the 8 trilinear vertices inside the kernel): ax_dmma_rg for FP64 p = 8, ax_stream<..., RG> for p <= 12, ax_simple beyond.
 #include <array>
 #include <map>
 #include <mutex>
@@ -185,6 +185,78 @@ __device__ __forceinline__ T slab_part2(const DRows<T, P>& dr, int i, int j, con
     return ar + as;
 }
 
+// ---- a9 inside the streaming kernel: the geometric factors of a node recomputed from the element's 8 vertices ----
+template <typename T, int P>
+struct GllP { T xi[P], rho[P]; };            // by value: compile-time indices come from the constant bank
+
+// Column (i, j) of a trilinear element (S5): x_r = Ja + Jb t, x_s = Jc + Jd t, x_t = Je for all nodes of the column
+template <typename T>
+struct ColJac { T Ja[3], Jb[3], Jc[3], Jd[3], Je[3], Wij; };
+
+template <typename T>
+__device__ __forceinline__ void col_jac_init(const double* __restrict__ vert_e, bool active, T r, T s, T Wij,
+                                             ColJac<T>& cj) {
+    double X[8][3], cf[8][3];
+#pragma unroll
+    for (int v = 0; v < 8; ++v)
+#pragma unroll
+        for (int d = 0; d < 3; ++d) X[v][d] = active ? __ldg(vert_e + v * 3 + d) : (double)((v >> d) & 1);
+    sem_trilinear_coef(X, cf);               // vertex differences in FP64 even on the FP32 path (no cancellation)
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        cj.Ja[d] = (T)cf[1][d] + (T)cf[4][d] * s;
+        cj.Jb[d] = (T)cf[5][d] + (T)cf[7][d] * s;
+        cj.Jc[d] = (T)cf[2][d] + (T)cf[4][d] * r;
+        cj.Jd[d] = (T)cf[6][d] + (T)cf[7][d] * r;
+        cj.Je[d] = (T)cf[3][d] + (T)cf[5][d] * r + ((T)cf[6][d] + (T)cf[7][d] * r) * s;
+    }
+    cj.Wij = Wij;
+}
+
+// (g_r, g_s, g_t) = G (u_r, u_s, u_t) at t = tk, W = Wij rho_k, without forming G:  G = (W / det) A A^T with the adjugate
+// rows a_0 = x_s x x_t, a_1 = x_t x x_r, a_2 = x_r x x_s, so G v = (W / det) A (A^T v); det = x_r . a_0
+template <typename T>
+__device__ __forceinline__ void col_jac_apply(const ColJac<T>& cj, T tk, T rk, T ur, T us, T ut, T& gr, T& gs, T& gt) {
+    T xr[3], xs[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) { xr[d] = cj.Ja[d] + cj.Jb[d] * tk; xs[d] = cj.Jc[d] + cj.Jd[d] * tk; }
+    const T* xt = cj.Je;
+    const T a0x = xs[1] * xt[2] - xs[2] * xt[1], a0y = xs[2] * xt[0] - xs[0] * xt[2], a0z = xs[0] * xt[1] - xs[1] * xt[0];
+    const T a1x = xt[1] * xr[2] - xt[2] * xr[1], a1y = xt[2] * xr[0] - xt[0] * xr[2], a1z = xt[0] * xr[1] - xt[1] * xr[0];
+    const T a2x = xr[1] * xs[2] - xr[2] * xs[1], a2y = xr[2] * xs[0] - xr[0] * xs[2], a2z = xr[0] * xs[1] - xr[1] * xs[0];
+    const T det = xr[0] * a0x + xr[1] * a0y + xr[2] * a0z;
+    T rdet;
+    if constexpr (sizeof(T) == 8) rdet = __drcp_rn(det); else rdet = __frcp_rn(det);
+    const T sc = cj.Wij * rk * rdet;
+    const T zx = a0x * ur + a1x * us + a2x * ut;
+    const T zy = a0y * ur + a1y * us + a2y * ut;
+    const T zz = a0z * ur + a1z * us + a2z * ut;
+    gr = sc * (a0x * zx + a0y * zy + a0z * zz);
+    gs = sc * (a1x * zx + a1y * zy + a1z * zz);
+    gt = sc * (a2x * zx + a2y * zy + a2z * zz);
+}
+
+// slab_part1 with the factors recomputed (same contractions)
+template <typename T, int P>
+__device__ __forceinline__ void slab_part1_rg(const DParam<T, P>& dp, const DRows<T, P>& dr, const T* __restrict__ su,
+                                              const T (&uk)[P], T (&wk)[P], const ColJac<T>& cj, T tk, T rk, int k, int i,
+                                              int j, T& gr_out, T& gs_out) {
+    T row[P];
+    load_row<T, P>(su + (k * P + j) * P, row);
+    const T* col = su + k * P * P + i;
+    T ur = T(0), us = T(0), ut = T(0);
+#pragma unroll
+    for (int l = 0; l < P; ++l) {
+        ur += dr.Di[l] * row[l];
+        us += dr.Dj[l] * col[l * P];
+        ut += dp.D[k * P + l] * uk[l];
+    }
+    T gt;
+    col_jac_apply<T>(cj, tk, rk, ur, us, ut, gr_out, gs_out, gt);
+#pragma unroll
+    for (int l = 0; l < P; ++l) wk[l] += dp.D[k * P + l] * gt;
+}
+
 template <typename T>
 __device__ __forceinline__ void block_dot_flush(T partial, double* __restrict__ dot_out) {
     __shared__ double red[32];
@@ -297,28 +369,32 @@ __global__ void __launch_bounds__(threads_of<P>()) ax_simple(int64_t E, DParam<T
 // Any P <= 12 and 16-byte aligned u.  The G slabs are padded to 16 bytes (sem_geom.cu) and always arrive by bulk copies;
 // u arrives by bulk copies when an element block is a multiple of 16 bytes (even p), by plain loads otherwise (odd p).
 //
-template <typename T, int P, int NS>
+template <typename T, int P, int NS, bool RG = false>
 struct StreamSmem {
     static constexpr int EPB = epb_of<P>(), P2 = P * P, P3 = P2 * P;
     // values per element slab, padded to 16 bytes (sem_geom.cu: slab_f64 / slab_f32): only FP32 with odd p needs the pad
     static constexpr int SLAB = 6 * P2 + ((6 * P2 * (int)sizeof(T)) % 16 ? 2 : 0);
     static constexpr bool UBULK = (P3 * (int)sizeof(T)) % 16 == 0;   // element blocks of u are 16-byte multiples: bulk copies
-    alignas(128) T g[NS][EPB * SLAB];
+    alignas(128) T g[RG ? 1 : NS][RG ? 16 : EPB * SLAB];     // RG (recomputed factors, a9): no G ring
     alignas(128) T u[2][EPB * P3];
     alignas(16) T sgr[2][EPB * P2];
     alignas(16) T sgs[2][EPB * P2];
     alignas(8) uint64_t gfull[NS];
     alignas(8) uint64_t ufull[2];
     alignas(16) T D[P * P];                                  // copy of D for DRows::init_shared
+    alignas(16) T xr[2 * P];                                 // RG: xi, rho for the thread-dependent indices i, j
 };
 
-template <typename T, int P, int NS, int MINB>
+// RG = true (a9): the factors are recomputed per node from the element's vertices (col_jac_*), Gs is not read, `vert`
+// points at the first element's 8 vertices and gl holds the GLL points / weights.
+template <typename T, int P, int NS, int MINB, bool RG = false>
 __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DParam<T, P> dp,
                                                                    const T* __restrict__ Gs, const T* __restrict__ Bm,
                                                                    T lambda, const T* __restrict__ u,
                                                                    T* __restrict__ w, const int* __restrict__ skip_flag,
-                                                                   double* __restrict__ dot_out, int u_keep) {
-    using SM = StreamSmem<T, P, NS>;
+                                                                   double* __restrict__ dot_out, int u_keep,
+                                                                   const double* __restrict__ vert, GllP<T, P> gl) {
+    using SM = StreamSmem<T, P, NS, RG>;
     constexpr int EPB = SM::EPB, P2 = SM::P2, P3 = SM::P3, SLAB = SM::SLAB, NT = threads_of<P>();
     constexpr bool FULL = EPB * P2 == NT;           // every thread owns a column
     constexpr uint32_t GBYTES = EPB * SLAB * sizeof(T);
@@ -339,7 +415,7 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
     // ---- producer (thread 0): slabs are issued in consumption order, NS ahead; G is padded to whole groups ----
     const T* gsrc = Gs + (int64_t)blockIdx.x * (P * EPB * SLAB);
     const int64_t gjump = (int64_t)(gridDim.x - 1) * (P * EPB * SLAB);
-    int64_t gleft = nmine * P;
+    int64_t gleft = RG ? 0 : nmine * P;
     uint64_t pol_g = 0, pol_u = 0;
     auto issue_u = [&](int64_t n) {
         const int64_t grp = blockIdx.x + n * gridDim.x;
@@ -356,6 +432,11 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
         mbar_fence_init();
     }
     for (int t = tid; t < P * P; t += NT) sm.D[t] = dp.D[t];
+    if constexpr (RG) {
+#pragma unroll
+        for (int q = 0; q < P; ++q)
+            if (tid == q) { sm.xr[q] = gl.xi[q]; sm.xr[P + q] = gl.rho[q]; }
+    }
     __syncthreads();
     if (tid == 0 && nmine > 0) {
         pol_g = policy_evict_first();
@@ -374,6 +455,8 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
     DRows<T, P> dr;
     dr.init_shared(sm.D, i, j);
     T partial = T(0);
+    T rg_r = T(0), rg_s = T(0), rg_W = T(0);       // RG: this thread's (r, s) = (xi_i, xi_j) and rho_i rho_j
+    if constexpr (RG) { rg_r = sm.xr[i]; rg_s = sm.xr[j]; rg_W = sm.xr[P + i] * sm.xr[P + j]; }
 
     int q = 0;                 // ring stage of the slab being consumed
     uint32_t gphase = 0;       // its mbarrier parity
@@ -400,15 +483,21 @@ __global__ void __launch_bounds__(threads_of<P>(), MINB) ax_stream(int64_t E, DP
             }
             __syncthreads();
         }
+        ColJac<T> cj;
+        if constexpr (RG) col_jac_init<T>(vert + (grp * EPB + slot) * 24, ok, rg_r, rg_s, rg_W, cj);
 #pragma unroll
         for (int k = 0; k < P; ++k) {
-            mbar_wait(&sm.gfull[q], gphase);
-            T g[6];
-#pragma unroll
-            for (int c = 0; c < 6; ++c) g[c] = sm.g[q][slot * SLAB + c * P2 + ij];
             const int buf = k & 1;
             T gr, gs;
-            slab_part1<T, P>(dp, dr, sue, uk, wk, g, k, i, j, gr, gs);
+            if constexpr (RG) {
+                slab_part1_rg<T, P>(dp, dr, sue, uk, wk, cj, gl.xi[k], gl.rho[k], k, i, j, gr, gs);
+            } else {
+                mbar_wait(&sm.gfull[q], gphase);
+                T g[6];
+#pragma unroll
+                for (int c = 0; c < 6; ++c) g[c] = sm.g[q][slot * SLAB + c * P2 + ij];
+                slab_part1<T, P>(dp, dr, sue, uk, wk, g, k, i, j, gr, gs);
+            }
             if (FULL || lane_ok) { sm.sgr[buf][slot * P2 + ij] = gr; sm.sgs[buf][slot * P2 + ij] = gs; }
             __syncthreads();
             // every thread has consumed stage q (and, on the last slab, this group's u buffer): refill
@@ -1456,23 +1545,27 @@ int launch_simple(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, doubl
     return SEM_OK;
 }
 
-template <typename T, int P, int NS, int MINB>
+template <typename T, int P, int NS, int MINB, bool RG = false>
 int launch_stream(sem_ctx* c, const T* u, T* w, T lambda, const int* skip, double* dot) {
-    using SM = StreamSmem<T, P, NS>;
+    using SM = StreamSmem<T, P, NS, RG>;
     constexpr int EPB = epb_of<P>(), P3 = P * P * P;
     const ElemRange r = elem_range(c);
     const int64_t ngroups = (r.ne + EPB - 1) / EPB;
-    const T* Gs = (sizeof(T) == 8 ? (const T*)c->d_G : (const T*)c->d_G32) + (r.e0 / EPB) * P * EPB * SM::SLAB;
+    const T* Gs = RG ? nullptr
+                     : (sizeof(T) == 8 ? (const T*)c->d_G : (const T*)c->d_G32) + (r.e0 / EPB) * P * EPB * SM::SLAB;
     const T* Bm = sizeof(T) == 8 ? (const T*)c->d_B : (const T*)c->d_B32;
     const DParam<T, P> dp = make_dparam<T, P>(c);
+    GllP<T, P> gl;
+    for (int q = 0; q < P; ++q) { gl.xi[q] = (T)c->xi[q]; gl.rho[q] = (T)c->rho[q]; }
     const size_t smem = sizeof(SM) + 128;
-    auto kern = ax_stream<T, P, NS, MINB>;
+    auto kern = ax_stream<T, P, NS, MINB, RG>;
     int blocks_per_sm = 0;
     if (int rc = resident_blocks(c, kern, threads_of<P>(), smem, &blocks_per_sm)) return rc;
     const int64_t cap = (int64_t)c->num_sms * blocks_per_sm;
     const unsigned grid = (unsigned)(ngroups < cap ? ngroups : cap);
-    kern<<<grid, threads_of<P>(), smem, c->stream>>>(r.ne, dp, Gs, lambda != T(0) ? Bm + r.e0 * P3 : (const T*)nullptr,
-                                                     lambda, u + r.e0 * P3, w + r.e0 * P3, skip, dot, u_keep(c, sizeof(T)));
+    kern<<<grid, threads_of<P>(), smem, c->stream>>>(r.ne, dp, Gs, (lambda != T(0) && Bm) ? Bm + r.e0 * P3 : (const T*)nullptr,
+                                                     lambda, u + r.e0 * P3, w + r.e0 * P3, skip, dot, u_keep(c, sizeof(T)),
+                                                     RG ? c->d_vert + r.e0 * 24 : (const double*)nullptr, gl);
     SEM_CUDA_OK(c, cudaGetLastError());
     return SEM_OK;
 }
@@ -1584,6 +1677,13 @@ template <> struct StreamCfg<double, 10> { static constexpr int NS = 4, MINB = 3
 template <> struct StreamCfg<float, 10> { static constexpr int NS = 6, MINB = 4; };
 
 template <int P> constexpr bool stream_ok() { return P <= 12; }
+// resident CTAs the recomputed-G instantiation is compiled for (15 more live values per thread than the stored-G one)
+// (FP64-pipe bound, little shared memory: registers first, occupancy second)
+template <typename T, int P> struct StreamCfgRG {
+    static constexpr int WANT = sizeof(T) == 8 ? (P >= 9 ? 255 : P >= 7 ? 208 : 168) : (P >= 11 ? 192 : 128);   // registers per thread
+    static constexpr int FIT = 65536 / (threads_of<P>() * WANT);
+    static constexpr int MINB = FIT < 1 ? 1 : (FIT > 8 ? 8 : FIT);
+};
 template <> struct StreamCfg<double, 9> { static constexpr int NS = 4, MINB = 4; };
 template <> struct StreamCfg<float, 9> { static constexpr int NS = 6, MINB = 5; };
 template <> struct StreamCfg<double, 7> { static constexpr int NS = 4, MINB = 4; };
@@ -1600,7 +1700,12 @@ int dispatch_p(sem_ctx* c, const void* u, void* w, double lambda, const int* ski
     const bool aligned = ((uintptr_t)u % 16) == 0;
     if (c->gmode == SEM_G_RECOMPUTE) {
         if constexpr (P == 8 && sizeof(T) == 8) {      // a9 on the tensor cores, no G traffic; variant 1 keeps ax_simple
-            if (aligned && c->ax_variant != 1) return launch_dmma_rg<8>(c, (const double*)u, (double*)w, lambda, skip, dot);
+            if (aligned && c->ax_variant != 1 && c->ax_variant != 2)
+                return launch_dmma_rg<8>(c, (const double*)u, (double*)w, lambda, skip, dot);
+        }
+        if constexpr (stream_ok<P>()) {                // every other p <= 12 (and variant 2): the streaming kernel, no G ring
+            if (aligned && c->ax_variant != 1)
+                return launch_stream<T, P, 1, StreamCfgRG<T, P>::MINB, true>(c, uu, ww, (T)lambda, skip, dot);
         }
         return launch_simple<T, P, true>(c, uu, ww, (T)lambda, skip, dot);
     }

@@ -1052,3 +1052,33 @@ def test_ax_recomputed_G_tensor_core_kernel(torch_cuda, binding, oracle_mod, lam
                 assert torch_cuda.equal(dw, dw2)
     for k, w in got.items():
         assert relerr(w, ow) <= TOL64, k
+
+
+@pytest.mark.parametrize("N,dtype", [(1, "f64"), (2, "f32"), (3, "f64"), (4, "f64"), (4, "f32"), (5, "f64"), (6, "f64"),
+                                     (6, "f32"), (7, "f32"), (8, "f64"), (9, "f64"), (9, "f32"), (10, "f64"), (11, "f64"),
+                                     (11, "f32"), (7, "f64v2")])
+def test_ax_recomputed_G_streaming_kernel(torch_cuda, binding, oracle_mod, N, dtype):
+    """a9 at the other orders: ax_stream<..., RG> (no G ring; the factors recomputed per node from the vertices) with more
+    element groups than resident CTAs (the u buffers wrap, ragged last group), Helmholtz term included, against the
+    oracle -- FP64 1e-12, FP32 1e-5 -- and against ax_simple's recomputation."""
+    n = {1: 30, 2: 24, 3: 22, 4: 18, 5: 16, 6: 15, 7: 14, 8: 13, 9: 12, 10: 11, 11: 11}[N]
+    m = inputs.box_mesh(n, n, n + 1, N, "random", seed=20 + N, permute_seed=N)
+    variant = 2 if dtype == "f64v2" else 0                      # p = 8 FP64: variant 2 selects the streaming kernel
+    f64 = dtype != "f32"
+    tdt, tol = (torch_cuda.float64, TOL64) if f64 else (torch_cuda.float32, TOL32)
+    lam = 1.5
+    oG, _, rc = oracle_mod.geom_trilinear(m.vert, m.N)
+    assert rc == 0
+    u = inputs.field_uniform(m.gid, 6)
+    ow = oracle_mod.ax(oG, u, m.N, lam)
+    du = to_dev(torch_cuda, u.ravel(), tdt)
+    with binding.Sem(m.E, m.N, m.vert, m.gid) as sem:
+        sem.geom(mode=binding.SEM_G_RECOMPUTE, with_mass=True)
+        outs = []
+        for v in (variant, 1):
+            sem.set_variant(v)
+            dw = torch_cuda.full_like(du, float("nan"))
+            sem.ax(du, dw, lam)
+            outs.append(dw.cpu().numpy().reshape(ow.shape))
+            assert relerr(outs[-1], ow) <= tol, v
+        assert relerr(outs[0], outs[1].astype(np.float64)) <= 10 * tol
