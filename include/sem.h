@@ -70,7 +70,10 @@ SEM_API int sem_mesh_setup(sem_ctx** out, int64_t E, int N, const double* vertex
  *             Jm is the analytic derivative of the trilinear blend of the 8 vertices (S5).
  *   mode      SEM_G_STORED: G kept in HBM (48 B/node FP64).  SEM_G_RECOMPUTE: sem_ax recomputes G from the 8
  *             vertices inside the kernel (a9; needs node_xyz == NULL) and no stored G is kept (it is rebuilt for the
- *             duration of sem_get_geom and of the Jacobi-diagonal build).
+ *             duration of sem_get_geom and of the Jacobi-diagonal build).  The operator then moves 16 B per node
+ *             instead of 64 and is bound by the FP64 pipe; at N = 7 in FP64 (tensor-core kernel) it is faster than the
+ *             stored-G operator once u and w no longer fit in L2 (1.26x at 64^3 elements), slower below; at other
+ *             orders the stored-G operator is faster.
  *   with_mass keep B (needed for lambda != 0 and for sem_get_geom's 7th factor)
  * Returns SEM_EMESH if any detJ <= 0.  Also builds the exact assembled diagonal for Jacobi (O7). */
 SEM_API int sem_geom(sem_ctx* ctx, const double* node_xyz, sem_gmode mode, int with_mass);
