@@ -357,7 +357,7 @@ def run_leg(args):
         torch.cuda.set_stream(torch.cuda.default_stream())
         mesh = inputs.config2()
         with binding.Sem(mesh.E, mesh.N, mesh.vert, mesh.gid, mesh.dirichlet) as sem:
-            sem.geom()
+            sem.geom(mode=args.gmode)                # --gmode 1: the recomputed-G operator (a9)
             sem.set_variant(args.variant)
             u = torch.from_numpy(inputs.field_uniform(mesh.gid, 0).ravel()).cuda()
             w = torch.empty_like(u)
@@ -624,6 +624,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=50)
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--gmode", type=int, default=0, help="--leg ncu: 0 = stored G, 1 = SEM_G_RECOMPUTE")
     ap.add_argument("--pcg-iters", type=int, default=300)
     ap.add_argument("--config5-n", type=int, default=100, help="elements per direction of the config-5 leg (0 = skip)")
     ap.add_argument("--emulate-ranks", type=int, default=0,
