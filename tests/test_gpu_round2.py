@@ -1082,3 +1082,38 @@ def test_ax_recomputed_G_streaming_kernel(torch_cuda, binding, oracle_mod, N, dt
             outs.append(dw.cpu().numpy().reshape(ow.shape))
             assert relerr(outs[-1], ow) <= tol, v
         assert relerr(outs[0], outs[1].astype(np.float64)) <= 10 * tol
+
+
+@pytest.mark.parametrize("N,inner", [(7, "0"), (5, "0"), (7, "1")])
+def test_recomputed_G_through_chunks_and_inner_context(torch_cuda, binding, oracle_mod, monkeypatch, N, inner):
+    """SEM_G_RECOMPUTE on the paths large meshes take: the chunked operator / gather-scatter (element ranges offset into
+    the vertex array) and the renumbered inner context of sem_pcg, both forced on a small scrambled mesh.  Ax+gs equals the
+    oracle and is bit-identical to the un-chunked recomputed result; the PCG loop takes the oracle's iteration count."""
+    m = inputs.box_mesh(6, 5, 4, N, "random", seed=4, permute_seed=9)
+    om = oracle_mod.Maps(m.gid)
+    oG, _, _ = oracle_mod.geom_trilinear(m.vert, m.N)
+    mask_u = oracle_mod.mask_unique(m.dirichlet, om)
+    u = inputs.field_uniform(m.gid, 5)
+    ow = _ax_gs_oracle(oracle_mod, m, u, True)
+    xs = np.where(mask_u != 0, 0.0, inputs.field_normal(om.uniq_gid, 7))
+    b_u = oracle_mod.apply_Ag(oG, m.N, om, mask_u, xs)
+    ores = oracle_mod.pcg(oG, m.N, om, mask_u, b_u, tol=1e-9, maxit=300)
+    monkeypatch.setenv("SEM_INNER", inner)
+    outs = []
+    for chunk in (None, "3"):
+        if chunk is None:
+            monkeypatch.delenv("SEM_CHUNK_GROUPS", raising=False)
+        else:
+            monkeypatch.setenv("SEM_CHUNK_GROUPS", chunk)
+        with binding.Sem(m.E, m.N, m.vert, m.gid, m.dirichlet) as sem:
+            sem.geom(mode=binding.SEM_G_RECOMPUTE)
+            du = to_dev(torch_cuda, u.ravel())
+            dw = torch_cuda.full_like(du, float("nan"))
+            sem.ax_gs(du, dw)
+            outs.append(dw.clone())
+            assert relerr(dw.cpu().numpy(), ow) <= TOL64
+            b = to_dev(torch_cuda, b_u[om.l2u])
+            x = torch_cuda.zeros_like(b)
+            it, _ = sem.pcg(b, x, 1e-9, 300)
+            assert it == ores["iters"] and relerr(x.cpu().numpy(), ores["x"][om.l2u]) <= TOLPCG
+    assert torch_cuda.equal(outs[0], outs[1])
