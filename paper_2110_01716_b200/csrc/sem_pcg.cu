@@ -453,10 +453,12 @@ extern "C" int sem_pcg_many(sem_ctx* c, const double* b, double* x, int nfields,
         }
     PcgFlags hf[8] = {};
     const int batch = 16;
-    for (int it = 1; it <= maxit; ++it) {
+    auto iteration = [&](int it) -> int {                // it < 0: iteration numbers and p.q on the device (graph replay)
         k_all_done<<<1, 1, 0, st>>>(nf, d_fl, d_all);
-        if ((rc = sem_launch_ax_many(c, P, W, nf, fs, SEM_F64, c->lambda, scal + 4 * it, slot, d_all))) return fail(rc);
-        if ((rc = sem_launch_gs_fields(c, W, nf, fs, SEM_F64, true, d_all))) return fail(rc);
+        double* dot = it < 0 ? &fl[0]->pq : scal + 4 * it;      // field f: + f * slot doubles in both cases
+        int r1 = sem_launch_ax_many(c, P, W, nf, fs, SEM_F64, c->lambda, dot, slot, d_all);
+        if (r1) return r1;
+        if ((r1 = sem_launch_gs_fields(c, W, nf, fs, SEM_F64, true, d_all))) return r1;
         for (int f = 0; f < nf; ++f) {
             double* sc = scal + f * slot;
             if (c->d_wt8)
@@ -465,12 +467,50 @@ extern "C" int sem_pcg_many(sem_ctx* c, const double* b, double* x, int nfields,
                 k_pcg_update<false><<<vgrid, 256, 0, st>>>(n, it, P + f * fs, W + f * fs, c->d_Minv, c->d_wt, nullptr, x + f * fs, R + f * fs, sc, fl[f]);
             k_pcg_direction<<<vgrid, 256, 0, st>>>(n, it, maxit, tol2, R + f * fs, c->d_Minv, P + f * fs, sc, fl[f]);
         }
-        if (it % batch == 0 || it == maxit) {
-            bool all = true;
-            for (int f = 0; f < nf; ++f) cudaMemcpyAsync(&hf[f], fl[f], sizeof(PcgFlags), cudaMemcpyDeviceToHost, st);
-            if (cudaStreamSynchronize(st) != cudaSuccess) return fail(sem_fail(c, SEM_ECUDA, "sem_pcg_many: loop failed"));
-            for (int f = 0; f < nf; ++f) all = all && hf[f].done;
+        return SEM_OK;
+    };
+    auto poll = [&](bool& all) -> int {
+        all = true;
+        for (int f = 0; f < nf; ++f) cudaMemcpyAsync(&hf[f], fl[f], sizeof(PcgFlags), cudaMemcpyDeviceToHost, st);
+        if (cudaStreamSynchronize(st) != cudaSuccess) return sem_fail(c, SEM_ECUDA, "sem_pcg_many: loop failed");
+        for (int f = 0; f < nf; ++f) all = all && hf[f].done;
+        return SEM_OK;
+    };
+    // as in sem_pcg: one CUDA graph of `batch` lockstep iterations, replayed until every field has stopped
+    cudaGraphExec_t gexec = nullptr;
+    const bool graphable = st != nullptr && st != cudaStreamLegacy && maxit >= batch;
+    if (graphable && cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+        rc = SEM_OK;
+        for (int q = 0; q < batch && rc == SEM_OK; ++q) rc = iteration(-1);
+        cudaGraph_t graph = nullptr;
+        const cudaError_t ec = cudaStreamEndCapture(st, &graph);
+        if (rc != SEM_OK || ec != cudaSuccess || !graph || cudaGraphInstantiate(&gexec, graph, 0) != cudaSuccess) gexec = nullptr;
+        if (graph) cudaGraphDestroy(graph);
+        cudaGetLastError();
+        if (rc != SEM_OK) return fail(rc);
+    } else {
+        cudaGetLastError();
+    }
+    if (gexec) {
+        const int one = 1;
+        for (int f = 0; f < nf; ++f) cudaMemcpyAsync(&fl[f]->it, &one, sizeof(int), cudaMemcpyHostToDevice, st);
+        for (int it0 = 1; it0 <= maxit; it0 += batch) {
+            bool all = false;
+            if (cudaGraphLaunch(gexec, st) != cudaSuccess || (rc = poll(all))) {
+                cudaGraphExecDestroy(gexec);
+                return fail(rc ? rc : sem_fail(c, SEM_ECUDA, "sem_pcg_many: graph launch failed"));
+            }
             if (all) break;
+        }
+        cudaGraphExecDestroy(gexec);
+    } else {
+        for (int it = 1; it <= maxit; ++it) {
+            if ((rc = iteration(it))) return fail(rc);
+            if (it % batch == 0 || it == maxit) {
+                bool all = false;
+                if ((rc = poll(all))) return fail(rc);
+                if (all) break;
+            }
         }
     }
     if (cudaGetLastError() != cudaSuccess) return fail(sem_fail(c, SEM_ECUDA, "sem_pcg_many: launch failed"));
