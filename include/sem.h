@@ -112,7 +112,8 @@ SEM_API int sem_gs_many(sem_ctx* ctx, void* w, int nfields, int64_t field_stride
  *   (||r_f|| <= tol ||r_f,0||) and breakdown handling, i.e. each field's iterates are those of sem_pcg on it alone; the
  *   operator pass is shared as above.  b, x DEVICE FP64 as in sem_pcg, at field_stride; iters_out, relres_out HOST
  *   [nfields].  On a non-default stream 16 lockstep iterations are one CUDA graph, replayed (as in sem_pcg): three
- *   Helmholtz fields at config 2 take 287 us per iteration against 3 x 103 us for three sem_pcg solves.  Synchronises. */
+ *   Helmholtz fields at config 2 take 275 - 281 us per iteration against 3 x 103 us for three sem_pcg solves (the vector
+ *   kernels run on groups of 3 or 2 fields and read the Jacobi diagonal and the dot weights once per group).  Synchronises. */
 SEM_API int sem_ax_gs_many(sem_ctx* ctx, const void* u, void* w, int nfields, int64_t field_stride, sem_prec prec,
                            double lambda);
 SEM_API int sem_pcg_many(sem_ctx* ctx, const double* b, double* x, int nfields, int64_t field_stride, double tol, int maxit,

@@ -383,6 +383,151 @@ __global__ void k_all_done(int nf, const PcgFlags* const* flags, int* __restrict
     for (int f = 0; f < nf; ++f) d &= flags[f]->done != 0;
     *all_done = d;
 }
+
+// The two vector kernels of an iteration for NF fields at once (field f at + f * fs): exactly k_pcg_update /
+// k_pcg_direction per field (own alpha, beta, flags, slots), but Minv and the dot weights are read once for all fields
+// (57 -> 48 + 9 / NF and 32 -> 24 + 8 / NF bytes per node and field).
+template <int NF>
+struct ManyArgs {
+    double* scal[NF];
+    PcgFlags* flags[NF];
+};
+
+template <bool W8, int NF>
+__global__ void __launch_bounds__(256) k_pcg_update_many(int64_t n, int it_arg, const double* __restrict__ p,
+                                                         const double* __restrict__ w, const double* __restrict__ Minv,
+                                                         const double* __restrict__ wt, const uint8_t* __restrict__ wt8,
+                                                         double* __restrict__ x, double* __restrict__ r, int64_t fs,
+                                                         ManyArgs<NF> a) {
+    bool act[NF];
+    double alpha[NF];
+    int itf[NF];
+    bool any = false;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+        PcgFlags* fl = a.flags[f];
+        act[f] = false; alpha[f] = 0.0; itf[f] = 0;
+        if (fl->done) continue;
+        const bool dev_it = it_arg < 0;
+        const int it = dev_it ? fl->it : it_arg;
+        const double pq = dev_it ? fl->pq : a.scal[f][4 * it + 0];
+        if (dev_it && blockIdx.x == 0 && threadIdx.x == 0) a.scal[f][4 * it + 0] = pq;
+        if (!(pq > 0.0)) {                              // breakdown (S13): stop this field, keep its x
+            if (blockIdx.x == 0 && threadIdx.x == 0) { fl->breakdown = 1; fl->iters = it; }
+            continue;
+        }
+        act[f] = true; any = true; itf[f] = it;
+        alpha[f] = a.scal[f][4 * (it - 1) + 2] / pq;
+    }
+    if (!any) return;
+    double srr[NF], srz[NF];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) { srr[f] = 0.0; srz[f] = 0.0; }
+    const int64_t n2 = n >> 1;
+    const double2* m2 = reinterpret_cast<const double2*>(Minv);
+    const double2* t2 = reinterpret_cast<const double2*>(wt);
+    for (int64_t v = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; v < n2; v += (int64_t)gridDim.x * blockDim.x) {
+        const double2 mv = m2[v];
+        double2 tv;
+        if constexpr (W8) {
+            const uchar2 c8 = reinterpret_cast<const uchar2*>(wt8)[v];
+            tv = make_double2(wt_of(c8.x), wt_of(c8.y));
+        } else {
+            tv = t2[v];
+        }
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+            if (!act[f]) continue;
+            const double2 pv = reinterpret_cast<const double2*>(p + f * fs)[v], wv = reinterpret_cast<const double2*>(w + f * fs)[v];
+            double2 xv = reinterpret_cast<double2*>(x + f * fs)[v], rv = reinterpret_cast<double2*>(r + f * fs)[v];
+            xv.x += alpha[f] * pv.x; xv.y += alpha[f] * pv.y;
+            rv.x -= alpha[f] * wv.x; rv.y -= alpha[f] * wv.y;
+            reinterpret_cast<double2*>(x + f * fs)[v] = xv;
+            reinterpret_cast<double2*>(r + f * fs)[v] = rv;
+            const double ax = tv.x * rv.x * rv.x, ay = tv.y * rv.y * rv.y;
+            srr[f] += ax + ay;
+            srz[f] += ax * mv.x + ay * mv.y;
+        }
+    }
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+        const int64_t l = n - 1;
+        const double wl = W8 ? wt_of(wt8[l]) : wt[l];
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+            if (!act[f]) continue;
+            x[f * fs + l] += alpha[f] * p[f * fs + l];
+            const double rl = r[f * fs + l] - alpha[f] * w[f * fs + l];
+            r[f * fs + l] = rl;
+            srr[f] += wl * rl * rl;
+            srz[f] += wl * rl * rl * Minv[l];
+        }
+    }
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+        if (act[f]) block_sum2_atomic(srr[f], srz[f], a.scal[f] + 4 * itf[f] + 1, a.scal[f] + 4 * itf[f] + 2);
+        __syncthreads();                                // the reduction's shared buffer is reused by the next field
+    }
+}
+
+template <int NF>
+__global__ void __launch_bounds__(256) k_pcg_direction_many(int64_t n, int it_arg, int maxit, double tol2,
+                                                            const double* __restrict__ r, const double* __restrict__ Minv,
+                                                            double* __restrict__ p, int64_t fs, ManyArgs<NF> a) {
+    const bool first = blockIdx.x == 0 && threadIdx.x == 0;
+    const bool dev_it = it_arg < 0;
+    bool act[NF];
+    double beta[NF];
+    int itf[NF];
+    bool any = false;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+        PcgFlags* fl = a.flags[f];
+        act[f] = false; beta[f] = 0.0; itf[f] = 0;
+        if (fl->done) continue;
+        if (fl->breakdown) { if (first) fl->done = 1; continue; }
+        const int it = dev_it ? fl->it : it_arg;
+        const double rr = a.scal[f][4 * it + 1];
+        const bool stop = rr <= tol2 * a.scal[f][1] || it >= maxit;
+        if (first) { fl->iters = it; if (stop) fl->done = 1; }
+        if (stop) continue;
+        act[f] = true; any = true; itf[f] = it;
+        beta[f] = a.scal[f][4 * it + 2] / a.scal[f][4 * (it - 1) + 2];
+    }
+    if (!any) return;
+    const int64_t n2 = n >> 1;
+    const double2* m2 = reinterpret_cast<const double2*>(Minv);
+    for (int64_t v = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; v < n2; v += (int64_t)gridDim.x * blockDim.x) {
+        const double2 mv = m2[v];
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+            if (!act[f]) continue;
+            const double2 rv = reinterpret_cast<const double2*>(r + f * fs)[v];
+            double2 pv = reinterpret_cast<double2*>(p + f * fs)[v];
+            pv.x = mv.x * rv.x + beta[f] * pv.x;
+            pv.y = mv.y * rv.y + beta[f] * pv.y;
+            reinterpret_cast<double2*>(p + f * fs)[v] = pv;
+        }
+    }
+    if ((n & 1) && first) {
+#pragma unroll
+        for (int f = 0; f < NF; ++f)
+            if (act[f]) p[f * fs + n - 1] = Minv[n - 1] * r[f * fs + n - 1] + beta[f] * p[f * fs + n - 1];
+    }
+    if (dev_it) {                                       // per field: the last block advances the iteration, clears p.q
+        __shared__ unsigned int last[NF];
+        __syncthreads();
+        if (threadIdx.x == 0) {
+#pragma unroll
+            for (int f = 0; f < NF; ++f) last[f] = act[f] ? (atomicAdd(&a.flags[f]->ticket, 1u) == gridDim.x - 1) : 0u;
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+#pragma unroll
+            for (int f = 0; f < NF; ++f)
+                if (last[f]) { a.flags[f]->ticket = 0; a.flags[f]->pq = 0.0; a.flags[f]->it = itf[f] + 1; }
+        }
+    }
+}
 }  // namespace
 
 extern "C" int sem_pcg_many(sem_ctx* c, const double* b, double* x, int nfields, int64_t field_stride, double tol,
@@ -459,13 +604,27 @@ extern "C" int sem_pcg_many(sem_ctx* c, const double* b, double* x, int nfields,
         int r1 = sem_launch_ax_many(c, P, W, nf, fs, SEM_F64, c->lambda, dot, slot, d_all);
         if (r1) return r1;
         if ((r1 = sem_launch_gs_fields(c, W, nf, fs, SEM_F64, true, d_all))) return r1;
-        for (int f = 0; f < nf; ++f) {
+        for (int f = 0; f < nf;) {                           // groups of 3 or 2 fields share Minv and the dot weights
+            const int left = nf - f, take = left >= 3 && left != 4 ? 3 : (left >= 2 ? 2 : 1);
             double* sc = scal + f * slot;
-            if (c->d_wt8)
-                k_pcg_update<true><<<vgrid, 256, 0, st>>>(n, it, P + f * fs, W + f * fs, c->d_Minv, c->d_wt, c->d_wt8, x + f * fs, R + f * fs, sc, fl[f]);
-            else
-                k_pcg_update<false><<<vgrid, 256, 0, st>>>(n, it, P + f * fs, W + f * fs, c->d_Minv, c->d_wt, nullptr, x + f * fs, R + f * fs, sc, fl[f]);
-            k_pcg_direction<<<vgrid, 256, 0, st>>>(n, it, maxit, tol2, R + f * fs, c->d_Minv, P + f * fs, sc, fl[f]);
+            if (take == 3) {
+                ManyArgs<3> a = {{sc, sc + slot, sc + 2 * slot}, {fl[f], fl[f + 1], fl[f + 2]}};
+                if (c->d_wt8) k_pcg_update_many<true, 3><<<vgrid, 256, 0, st>>>(n, it, P + f * fs, W + f * fs, c->d_Minv, c->d_wt, c->d_wt8, x + f * fs, R + f * fs, fs, a);
+                else k_pcg_update_many<false, 3><<<vgrid, 256, 0, st>>>(n, it, P + f * fs, W + f * fs, c->d_Minv, c->d_wt, nullptr, x + f * fs, R + f * fs, fs, a);
+                k_pcg_direction_many<3><<<vgrid, 256, 0, st>>>(n, it, maxit, tol2, R + f * fs, c->d_Minv, P + f * fs, fs, a);
+            } else if (take == 2) {
+                ManyArgs<2> a = {{sc, sc + slot}, {fl[f], fl[f + 1]}};
+                if (c->d_wt8) k_pcg_update_many<true, 2><<<vgrid, 256, 0, st>>>(n, it, P + f * fs, W + f * fs, c->d_Minv, c->d_wt, c->d_wt8, x + f * fs, R + f * fs, fs, a);
+                else k_pcg_update_many<false, 2><<<vgrid, 256, 0, st>>>(n, it, P + f * fs, W + f * fs, c->d_Minv, c->d_wt, nullptr, x + f * fs, R + f * fs, fs, a);
+                k_pcg_direction_many<2><<<vgrid, 256, 0, st>>>(n, it, maxit, tol2, R + f * fs, c->d_Minv, P + f * fs, fs, a);
+            } else {
+                if (c->d_wt8)
+                    k_pcg_update<true><<<vgrid, 256, 0, st>>>(n, it, P + f * fs, W + f * fs, c->d_Minv, c->d_wt, c->d_wt8, x + f * fs, R + f * fs, sc, fl[f]);
+                else
+                    k_pcg_update<false><<<vgrid, 256, 0, st>>>(n, it, P + f * fs, W + f * fs, c->d_Minv, c->d_wt, nullptr, x + f * fs, R + f * fs, sc, fl[f]);
+                k_pcg_direction<<<vgrid, 256, 0, st>>>(n, it, maxit, tol2, R + f * fs, c->d_Minv, P + f * fs, sc, fl[f]);
+            }
+            f += take;
         }
         return SEM_OK;
     };

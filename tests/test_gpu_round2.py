@@ -1117,3 +1117,50 @@ def test_recomputed_G_through_chunks_and_inner_context(torch_cuda, binding, orac
             it, _ = sem.pcg(b, x, 1e-9, 300)
             assert it == ores["iters"] and relerr(x.cpu().numpy(), ores["x"][om.l2u]) <= TOLPCG
     assert torch_cuda.equal(outs[0], outs[1])
+
+
+@pytest.mark.parametrize("nf,side_stream", [(1, True), (2, True), (3, True), (4, True), (5, True), (8, True), (5, False)])
+def test_pcg_many_groups_and_graph_replay(torch_cuda, binding, oracle_mod, nf, side_stream):
+    """sem_pcg_many for 1 ... 8 fields (vector kernels in groups of 3 and 2 fields, single leftovers) on a non-default stream,
+    where 16 lockstep iterations are one replayed CUDA graph, and on the default stream (eager launches): every field takes
+    the iteration count of sem_pcg on it alone and reaches its solution at 1e-9; the fields stop at different iterations
+    (different tolerances are emulated by scaling: one field is zero, one is a smooth mode)."""
+    m = inputs.box_mesh(5, 4, 3, 7, "random", seed=12)
+    lam = 3.0
+    om = oracle_mod.Maps(m.gid)
+    mask_u = oracle_mod.mask_unique(m.dirichlet, om)
+    xyz = oracle_mod.node_xyz(m.vert, m.N).reshape(-1, 3)
+    smooth = np.sin(np.pi * xyz[:, 0]) * np.sin(np.pi * xyz[:, 1]) * np.sin(np.pi * xyz[:, 2])
+    stream = torch_cuda.cuda.Stream() if side_stream else torch_cuda.cuda.current_stream()
+    with torch_cuda.cuda.stream(stream):
+        with binding.Sem(m.E, m.N, m.vert, m.gid, m.dirichlet) as sem:
+            sem.geom(with_mass=True)
+            sem.set_lambda(lam)
+            live = to_dev(torch_cuda, (mask_u[om.l2u] == 0).astype(np.float64))
+            us = []
+            for f in range(nf):
+                if f == 1:
+                    us.append(torch_cuda.zeros(sem.nL, device="cuda", dtype=torch_cuda.float64))
+                elif f == 2:
+                    us.append(to_dev(torch_cuda, smooth) * live)
+                else:
+                    us.append(to_dev(torch_cuda, inputs.field_normal(om.uniq_gid, 80 + f)[om.l2u]) * live)
+            b = torch_cuda.zeros(nf, sem.nL, device="cuda", dtype=torch_cuda.float64)
+            for f in range(nf):
+                sem.ax_gs(us[f].contiguous(), b[f], lam)
+            ref = []
+            for f in range(nf):
+                x1 = torch_cuda.zeros(sem.nL, device="cuda", dtype=torch_cuda.float64)
+                it1, rel1 = sem.pcg(b[f].contiguous(), x1, 1e-9, 300)
+                ref.append((it1, x1))
+            x = torch_cuda.zeros_like(b)
+            its, rels = sem.pcg_many(b, x, 1e-9, 300)
+            stream.synchronize()
+            assert len(set(r[0] for r in ref)) >= (2 if nf > 1 else 1)          # the fields do stop at different iterations
+            for f in range(nf):
+                assert its[f] == ref[f][0], (f, its, [r[0] for r in ref])
+                if ref[f][0]:
+                    assert relerr(x[f].cpu().numpy(), ref[f][1].cpu().numpy()) <= TOLPCG, f
+            x.zero_()
+            its2, _ = sem.pcg_many(b, x, 1e-30, 21)                              # one full batch + 5 iterations of the next
+            assert all(i == (0 if f == 1 else 21) for f, i in enumerate(its2))
